@@ -1,0 +1,225 @@
+"""ctypes front end of the fp64 CPU oracle (oracle/p3t_oracle.c).
+
+TEST INFRASTRUCTURE ONLY: imported by tests/, __graft_entry__.smoke() and the
+cpu_baseline / --impl reference legs of bench.py.  The product path
+(paper_1506_04553_b200) never imports this module.
+
+All arrays are fp64; callers pass the fp32-rounded inputs widened to double so
+that only arithmetic rounding separates the oracle from the GPU.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "p3t_oracle.c")
+_LIB = os.path.join(_HERE, "libp3t_oracle.so")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with gcc (-O2, OpenMP, strict IEEE: no -ffast-math)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-O2", "-fopenmp", "-fPIC", "-shared", "-std=c99", "-Wall",
+               "-o", _LIB, _SRC, "-lm"]
+        subprocess.run(cmd, check=True)
+    return _LIB
+
+
+def _p(a, t):
+    return None if a is None else a.ctypes.data_as(C.POINTER(t))
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        build()
+        L = C.CDLL(_LIB)
+        d, i64, vp, i32 = C.c_double, C.c_int64, C.c_void_p, C.c_int
+        pd, pi64, pi32 = C.POINTER(d), C.POINTER(i64), C.POINTER(C.c_int32)
+        L.p3t_oracle_K.restype = d; L.p3t_oracle_K.argtypes = [d]
+        L.p3t_oracle_Cin.restype = d; L.p3t_oracle_Cin.argtypes = [d]
+        L.p3t_oracle_G.restype = d; L.p3t_oracle_G.argtypes = [d, d]
+        L.p3t_oracle_W.restype = d; L.p3t_oracle_W.argtypes = [d, d]
+        L.p3t_oracle_pair_weights.restype = None
+        L.p3t_oracle_pair_weights.argtypes = [d, d, d, pd, pd]
+        L.p3t_oracle_direct.restype = None
+        L.p3t_oracle_direct.argtypes = [i64, pd, pd, d, d, d, i64, pi64, pd, pd, pd, pd]
+        L.p3t_oracle_neighbours.restype = i64
+        L.p3t_oracle_neighbours.argtypes = [i64, pd, d, d, i32, i64, pi64, pi64, pi64, pi32, d, pi64, i64]
+        L.p3t_oracle_neighbours_sweep.restype = None
+        L.p3t_oracle_neighbours_sweep.argtypes = [i64, pd, d, d, i32, pi64, pi64, pi64, pi32]
+        L.p3t_oracle_tree_build.restype = vp
+        L.p3t_oracle_tree_build.argtypes = [i64, pd, pd, i32, i32]
+        L.p3t_oracle_tree_free.restype = None; L.p3t_oracle_tree_free.argtypes = [vp]
+        L.p3t_oracle_tree_nnodes.restype = i64; L.p3t_oracle_tree_nnodes.argtypes = [vp]
+        L.p3t_oracle_tree_node.restype = None; L.p3t_oracle_tree_node.argtypes = [vp, i64, pd]
+        L.p3t_oracle_tree_perm.restype = None; L.p3t_oracle_tree_perm.argtypes = [vp, pi32]
+        L.p3t_oracle_tree_walk.restype = None
+        L.p3t_oracle_tree_walk.argtypes = [vp, d, d, d, d, d, i32, i64, pi64, pd, pd, pd, pi64, pi32, i64, pi64]
+        L.p3t_oracle_num_threads.restype = i32
+        _lib = L
+    return _lib
+
+
+def num_threads() -> int:
+    return int(lib().p3t_oracle_num_threads())
+
+
+def _f64(a):
+    return np.ascontiguousarray(np.asarray(a), dtype=np.float64)
+
+
+def _subset(subset):
+    if subset is None:
+        return None
+    return np.ascontiguousarray(np.asarray(subset), dtype=np.int64)
+
+
+# ---------------------------------------------------------------- O1 -------
+def K(x):
+    """Eq. 12."""
+    f = lib().p3t_oracle_K
+    return np.vectorize(lambda v: f(float(v)), otypes=[np.float64])(x)
+
+
+def W(y, gamma):
+    """Eq. 16-17, reading A1."""
+    f = lib().p3t_oracle_W
+    return np.vectorize(lambda v: f(float(v), float(gamma)), otypes=[np.float64])(y)
+
+
+def G(y, gamma):
+    f = lib().p3t_oracle_G
+    return np.vectorize(lambda v: f(float(v), float(gamma)), otypes=[np.float64])(y)
+
+
+def Cin(gamma):
+    return float(lib().p3t_oracle_Cin(float(gamma)))
+
+
+def pair_weights(s, r_in, r_out):
+    """(K, W) for softened separation s (Eq. 12-17 with Eq. 13-15's x, y, gamma)."""
+    k, w = C.c_double(), C.c_double()
+    lib().p3t_oracle_pair_weights(float(s), float(r_in), float(r_out), C.byref(k), C.byref(w))
+    return k.value, w.value
+
+
+# ---------------------------------------------------------------- O2 -------
+def direct(mass, pos, eps, r_in, r_out, subset=None, hard=False):
+    """Direct-sum soft acceleration [ns,3] and potential [ns] (Eq. 6, 8).
+
+    hard=True also returns the complementary (1-K), (1-W) sums (Eq. 5, 7).
+    """
+    m, q = _f64(mass), _f64(pos).reshape(-1, 3)
+    n = m.shape[0]
+    sub = _subset(subset)
+    ns = n if sub is None else sub.shape[0]
+    a_s, p_s = np.empty((ns, 3)), np.empty(ns)
+    a_h = np.empty((ns, 3)) if hard else None
+    p_h = np.empty(ns) if hard else None
+    d = C.c_double
+    lib().p3t_oracle_direct(n, _p(m, d), _p(q, d), float(eps), float(r_in), float(r_out), ns,
+                            _p(sub, C.c_int64), _p(a_s, d), _p(p_s, d), _p(a_h, d), _p(p_h, d))
+    return (a_s, p_s, a_h, p_h) if hard else (a_s, p_s)
+
+
+# ---------------------------------------------------------------- O3 -------
+def neighbours(pos, eps, h, subset=None, plain=False, band=1e-6):
+    """Exact neighbour sets by brute force.
+
+    Returns (offset[ns+1], nbr[total] ascending per list, band_pairs[nb,2]) where
+    band_pairs holds (k, j) with |s_kj/h - 1| < band (k indexes the subset).
+    """
+    q = _f64(pos).reshape(-1, 3)
+    n = q.shape[0]
+    sub = _subset(subset)
+    ns = n if sub is None else sub.shape[0]
+    count = np.zeros(ns, dtype=np.int64)
+    d, i64 = C.c_double, C.c_int64
+    L = lib()
+    nb = L.p3t_oracle_neighbours(n, _p(q, d), float(eps), float(h), int(plain), ns, _p(sub, i64),
+                                 _p(count, i64), None, None, float(band), None, 0)
+    offset = np.zeros(ns + 1, dtype=np.int64)
+    np.cumsum(count, out=offset[1:])
+    lst = np.empty(max(int(offset[-1]), 1), dtype=np.int32)
+    bp = np.empty((max(int(nb), 1), 2), dtype=np.int64)
+    L.p3t_oracle_neighbours(n, _p(q, d), float(eps), float(h), int(plain), ns, _p(sub, i64),
+                            None, _p(offset, i64), _p(lst, C.c_int32), float(band), _p(bp, i64), int(nb))
+    return offset, lst[: int(offset[-1])], bp[: int(nb)]
+
+
+def neighbours_sweep(pos, eps, h, plain=False):
+    """Exact neighbour sets of all particles by sort-and-sweep along x."""
+    q = _f64(pos).reshape(-1, 3)
+    n = q.shape[0]
+    order = np.ascontiguousarray(np.argsort(q[:, 0], kind="stable"), dtype=np.int64)
+    count = np.zeros(n, dtype=np.int64)
+    d, i64 = C.c_double, C.c_int64
+    L = lib()
+    L.p3t_oracle_neighbours_sweep(n, _p(q, d), float(eps), float(h), int(plain), _p(order, i64),
+                                  _p(count, i64), None, None)
+    offset = np.zeros(n + 1, dtype=np.int64)
+    np.cumsum(count, out=offset[1:])
+    lst = np.empty(max(int(offset[-1]), 1), dtype=np.int32)
+    L.p3t_oracle_neighbours_sweep(n, _p(q, d), float(eps), float(h), int(plain), _p(order, i64),
+                                  None, _p(offset, i64), _p(lst, C.c_int32))
+    return offset, lst[: int(offset[-1])]
+
+
+# ---------------------------------------------------------------- O4 -------
+class Tree:
+    """Pointer-based Barnes-Hut octree with monopole + quadrupole moments (L138)."""
+
+    NODE_FIELDS = 32
+
+    def __init__(self, mass, pos, nleaf=16, max_depth=21):
+        self.m, self.q = _f64(mass), _f64(pos).reshape(-1, 3)
+        self.n = self.m.shape[0]
+        d = C.c_double
+        self._h = lib().p3t_oracle_tree_build(self.n, _p(self.m, d), _p(self.q, d), int(nleaf), int(max_depth))
+
+    def __del__(self):
+        if getattr(self, "_h", None):
+            lib().p3t_oracle_tree_free(self._h)
+            self._h = None
+
+    @property
+    def nnodes(self):
+        return int(lib().p3t_oracle_tree_nnodes(self._h))
+
+    def nodes(self):
+        """Structured view of every node (for the moment / topology pins)."""
+        out = np.empty((self.nnodes, self.NODE_FIELDS))
+        row = np.empty(self.NODE_FIELDS)
+        for k in range(self.nnodes):
+            lib().p3t_oracle_tree_node(self._h, k, _p(row, C.c_double))
+            out[k] = row
+        return dict(g=out[:, 0:3], side=out[:, 3], M=out[:, 4], c=out[:, 5:8], Q=out[:, 8:14],
+                    bmin=out[:, 14:17], bmax=out[:, 17:20], first=out[:, 20].astype(np.int64),
+                    count=out[:, 21].astype(np.int64), leaf=out[:, 22].astype(bool),
+                    level=out[:, 23].astype(np.int64), child=out[:, 24:32].astype(np.int64))
+
+    def perm(self):
+        p = np.empty(self.n, dtype=np.int32)
+        lib().p3t_oracle_tree_perm(self._h, _p(p, C.c_int32))
+        return p
+
+    def walk(self, eps, theta, r_in, r_out, h, subset=None, box=None, use_quad=True, nbr_stride=0):
+        """Returns dict(acc[ns,3], pot[ns], n_pp[ns], n_pc[ns], nbr_count[ns], nbr[ns,stride])."""
+        sub = _subset(subset)
+        ns = self.n if sub is None else sub.shape[0]
+        acc, pot = np.empty((ns, 3)), np.empty(ns)
+        counts = np.zeros((ns, 2), dtype=np.int64)
+        nbr_count = np.zeros(ns, dtype=np.int64)
+        nbr = np.full((ns, nbr_stride), -1, dtype=np.int32) if nbr_stride else None
+        bx = None if box is None else _f64(box).reshape(ns, 6)
+        d, i64 = C.c_double, C.c_int64
+        lib().p3t_oracle_tree_walk(self._h, float(eps), float(theta), float(r_in), float(r_out), float(h),
+                                   int(use_quad), ns, _p(sub, i64), _p(bx, d), _p(acc, d), _p(pot, d),
+                                   _p(counts, i64), _p(nbr, C.c_int32), int(nbr_stride), _p(nbr_count, i64))
+        return dict(acc=acc, pot=pot, n_pp=counts[:, 0], n_pc=counts[:, 1], nbr_count=nbr_count, nbr=nbr)
