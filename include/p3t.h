@@ -1,0 +1,172 @@
+/*
+ * p3t.h -- C ABI of the B200-native soft-force library for the P3T scheme
+ *          (arXiv 1506.04553, Iwasawa, Portegies Zwart, Makino).
+ *
+ * What the library computes (citations: PAPER.md line, equation):
+ *   for every particle i, on one GPU (L138, L142-153 steps 1 and 7),
+ *     a_i   = - sum_{j != i} m_j K(s_ij) (q_i - q_j) / s_ij^3      (Eq. 8, per unit mass)
+ *     phi_i = - sum_{j != i} m_j W(s_ij) / s_ij                     (Eq. 6, per unit mass)
+ *     L_i   = { j != i : s_ij < r_search }                          (L138-140, h = r_cut + dr_buff)
+ *   with s_ij = sqrt(|q_i - q_j|^2 + eps^2) (Eq. 2), K the cutoff function of
+ *   Eq. 12 (L85), W the transition function of Eq. 16-17 (L102-104), G = 1 (L163),
+ *   by a Barnes-Hut octree with monopole + quadrupole cells (L138) opened with the
+ *   parameter theta (L171, L193).  r_out is the paper's r_cut, r_search its h.
+ *
+ * All arithmetic runs in hand-written sm_100a CUDA kernels; there is no CPU
+ * fallback.  Pair and cell interactions are evaluated in fp32; each batch of 32
+ * interactions is added to an fp64 accumulator.
+ *
+ * Conventions
+ *   - Pointers marked [device] must be device memory of the context's GPU,
+ *     [host] host memory; calls with an `on_device` flag accept either.
+ *   - Ownership: the caller owns every buffer it passes, including the
+ *     workspace; the library copies inputs into the workspace and never frees
+ *     caller memory.  The p3t_ctx itself is host heap, freed by p3t_destroy.
+ *   - Errors: every call returns a p3t_status; nothing aborts or throws.
+ *     p3t_last_error() gives a message for the last failing call on that ctx.
+ *   - Asynchrony: load/build/eval only enqueue work on the context's stream.
+ *     Calls that write host memory synchronise the stream before returning.
+ *   - Thread safety: one thread per context at a time.
+ */
+#ifndef P3T_H
+#define P3T_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct p3t_ctx p3t_ctx;
+
+typedef enum {
+    P3T_OK        =  0,
+    P3T_EINVAL    = -1,  /* bad argument: n = 0, n > max_n, non-finite input, eps < 0, theta < 0,
+                            not (0 <= r_in < r_out <= r_search), unknown enum value, null pointer */
+    P3T_ESTATE    = -2,  /* call order: build before load, eval before build, fetch before eval */
+    P3T_ENOMEM    = -3,  /* workspace too small, or host allocation failed */
+    P3T_ECAPACITY = -4,  /* neighbour buffer (nbr_capacity) or a caller's output buffer too small;
+                            the true total is still reported by p3t_get_neighbour_counts */
+    P3T_ECUDA     = -5   /* a CUDA runtime call failed; see p3t_last_error */
+} p3t_status;
+
+/* Per-call statistics.  Interaction counts are pair evaluations for real
+ * particles (padded lanes of partly filled groups are not counted); the flop
+ * convention of DESIGN.md (23 per p-p, 65 per p-c) is applied by the caller. */
+typedef struct {
+    uint64_t n;              /* particles loaded */
+    uint64_t n_pp;           /* particle-particle interactions of the last eval */
+    uint64_t n_pc;           /* particle-cell (monopole+quadrupole) interactions */
+    uint64_t n_near;         /* of n_pp: pairs evaluated on the K/W + neighbour-test path */
+    uint64_t n_neighbours;   /* sum of list lengths (ordered pairs) of the last eval */
+    uint32_t n_cells;        /* octree cells (internal + leaf) */
+    uint32_t n_leaves;
+    uint32_t n_groups;       /* i-groups walked (one warp each) */
+    uint32_t depth;          /* deepest level in use (root = 0) */
+    uint32_t max_list;       /* longest neighbour list */
+    uint32_t sort_passes;    /* radix passes actually run (uniform digits are skipped) */
+    float ms_sort;           /* a1-a4: bounding cube, keys, radix sort, gather */
+    float ms_build;          /* a5: octree + groups */
+    float ms_moments;        /* a6 */
+    float ms_walk;           /* a7-a8 */
+    float ms_nbr;            /* a9 */
+} p3t_stats;
+
+/* Bytes of device workspace p3t_create needs for up to max_n particles,
+ * key_bits in {30, 63} and room for nbr_capacity neighbour entries (ordered
+ * pairs, summed over all lists).  Returns 0 for invalid arguments. */
+size_t p3t_workspace_bytes(size_t max_n, int key_bits, size_t nbr_capacity);
+
+/* Create a context on `device` working on `cuda_stream` (a cudaStream_t passed
+ * as void*; NULL = the legacy default stream).  `workspace` [device] must be
+ * 256-byte aligned, at least p3t_workspace_bytes(...) long and stay alive until
+ * p3t_destroy.  Defaults: nleaf = 16, ngroup = 64; parameters must be set with
+ * p3t_set_params before the first build. */
+p3t_status p3t_create(p3t_ctx **out, int device, size_t max_n, int key_bits,
+                      void *workspace, size_t workspace_bytes, size_t nbr_capacity, void *cuda_stream);
+p3t_status p3t_destroy(p3t_ctx *ctx);
+
+/* eps: Plummer softening (Eq. 2); theta: opening parameter, 0 = open every
+ * cell (the tree path then is the direct sum); r_in, r_out: inner and outer
+ * cutoff radii of K and W (Eq. 12-17; r_out = r_cut); r_search: neighbour
+ * radius h >= r_out (L138-140).  Changing them invalidates a built tree
+ * (theta and r_search enter the per-cell acceptance radius). */
+p3t_status p3t_set_params(p3t_ctx *ctx, float eps, float theta, float r_in, float r_out, float r_search);
+
+/* nleaf in 1..32: a cell with more than nleaf bodies is split (unless at the
+ * key depth limit); ngroup in {32, 64}: bodies per i-group (one warp). */
+p3t_status p3t_set_tree_params(p3t_ctx *ctx, int nleaf, int ngroup);
+
+/* Tuning: how many octree levels above its natural level (the level whose cell holds <= ngroup
+ * bodies) an i-group's bodies may straddle.  0 = every group is one octree cell (partly filled
+ * warps); 1 (default) = consecutive sibling cells are merged up to ngroup bodies.  Results do
+ * not depend on it beyond rounding and the R-MAC box B. levels in 0..4. */
+p3t_status p3t_set_group_merge_levels(p3t_ctx *ctx, int levels);
+
+/* Load n particles: mass[n], pos[3n] (x,y,z interleaved), both host or both
+ * device (on_device).  Host data is checked for non-finite values here
+ * (P3T_EINVAL); device data is checked on the GPU and the error surfaces at
+ * p3t_build_tree's successor calls that synchronise. */
+p3t_status p3t_load_particles(p3t_ctx *ctx, size_t n, const float *mass, const float *pos, int on_device);
+
+/* a1-a6: bounding cube, Morton keys, radix sort, body gather, octree + groups,
+ * moments (mass, centre of mass, quadrupole, acceptance radius). */
+p3t_status p3t_build_tree(p3t_ctx *ctx);
+
+/* a7-a9: group walk, interactions, neighbour lists.  Needs a tree built for the
+ * loaded positions and current parameters. */
+p3t_status p3t_eval_soft(p3t_ctx *ctx);
+
+/* Verification entry: brute-force O(N * n_subset) evaluation with the same K, W
+ * and neighbour rule, no tree.  i_subset [same side as on_device] lists the
+ * targets (user ids); NULL = all particles.  Results are fetched with the same
+ * p3t_get_* calls; for a subset, entries of other particles are zero / empty. */
+p3t_status p3t_eval_direct(p3t_ctx *ctx, const uint32_t *i_subset, size_t n_subset, int on_device);
+
+/* acc[3n] (x,y,z interleaved) and pot[n], user order.  Either may be NULL. */
+p3t_status p3t_get_acc_pot(p3t_ctx *ctx, float *acc, float *pot, int on_device);
+
+/* count[n] list lengths in user order (may be NULL) and *total [host]
+ * (may be NULL; reading it synchronises). */
+p3t_status p3t_get_neighbour_counts(p3t_ctx *ctx, uint32_t *count, uint64_t *total, int on_device);
+
+/* CSR: offset[n+1], nbr[capacity] in user ids, self excluded, each list sorted
+ * ascending.  P3T_ECAPACITY if the lists do not fit `capacity` or the context's
+ * nbr_capacity (offset is still written). */
+p3t_status p3t_get_neighbours(p3t_ctx *ctx, uint64_t *offset, uint32_t *nbr, size_t capacity, int on_device);
+
+/* Synchronises the stream, then reports counts and per-phase times (CUDA events). */
+p3t_status p3t_get_stats(p3t_ctx *ctx, p3t_stats *out);
+
+/* Wait for all enqueued work; returns deferred device-side errors. */
+p3t_status p3t_synchronize(p3t_ctx *ctx);
+
+const char *p3t_last_error(const p3t_ctx *ctx);
+
+/* Inspection of intermediate arrays (for the a1-a6 parity tests).  Valid after
+ * p3t_build_tree.  p3t_array_info gives element count and element size. */
+typedef enum {
+    P3T_ARR_ROOT_CUBE   = 0,  /* float[4]: min corner x,y,z and side */
+    P3T_ARR_KEYS        = 1,  /* uint64[n]: sorted Morton keys */
+    P3T_ARR_SORTED_IDX  = 2,  /* uint32[n]: sorted position -> user id */
+    P3T_ARR_BODIES      = 3,  /* float4[n]: sorted (x,y,z,m) */
+    P3T_ARR_CELL_MAC    = 4,  /* float4[n_cells]: centre of mass, squared acceptance radius */
+    P3T_ARR_CELL_MOM0   = 5,  /* float4[n_cells]: M, Qxx, Qyy, Qzz (traceful, about the COM) */
+    P3T_ARR_CELL_MOM1   = 6,  /* float4[n_cells]: Qxy, Qxz, Qyz, bounding radius about the COM */
+    P3T_ARR_CELL_META   = 7,  /* uint32[2][n_cells]: leaf: body start, count | 0x80000000;
+                                                     internal: first child, child count */
+    P3T_ARR_CELL_LEVEL  = 8,  /* uint8[n_cells] */
+    P3T_ARR_CELL_START  = 9,  /* uint32[n_cells]: first body (sorted position) of the cell */
+    P3T_ARR_CELL_PARENT = 10, /* uint32[n_cells] (root: 0xffffffff) */
+    P3T_ARR_GROUP_START = 11, /* uint32[n_groups + 1] */
+    P3T_ARR_CELL_BMIN   = 12, /* float4[n_cells]: tight AABB min of the cell's bodies */
+    P3T_ARR_CELL_BMAX   = 13  /* float4[n_cells] */
+} p3t_array;
+p3t_status p3t_array_info(p3t_ctx *ctx, p3t_array which, size_t *count, size_t *elem_bytes);
+p3t_status p3t_copy_array(p3t_ctx *ctx, p3t_array which, void *dst, size_t dst_bytes, int on_device);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* P3T_H */

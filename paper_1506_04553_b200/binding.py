@@ -1,0 +1,244 @@
+"""Thin Python front end of the C-ABI library (include/p3t.h): argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels of libp3t.so.  torch supplies
+device memory (the workspace and optional device-side inputs/outputs) and the
+stream.  There is no CPU fallback: importing this module without the built
+library raises ImportError.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIBPATH = os.path.join(_HERE, "libp3t.so")
+
+if not os.path.exists(_LIBPATH):
+    raise ImportError(
+        f"{_LIBPATH} is missing: build it with `python -m paper_1506_04553_b200.build` "
+        "(there is no CPU fallback for the soft-force path)")
+
+_lib = C.CDLL(_LIBPATH)
+
+OK, EINVAL, ESTATE, ENOMEM, ECAPACITY, ECUDA = 0, -1, -2, -3, -4, -5
+_STATUS = {0: "P3T_OK", -1: "P3T_EINVAL", -2: "P3T_ESTATE", -3: "P3T_ENOMEM", -4: "P3T_ECAPACITY", -5: "P3T_ECUDA"}
+
+# names of include/p3t.h's exported entry points (tests check that each resolves)
+SYMBOLS = [
+    "p3t_workspace_bytes", "p3t_create", "p3t_destroy", "p3t_set_params", "p3t_set_tree_params",
+    "p3t_set_group_merge_levels", "p3t_load_particles", "p3t_build_tree", "p3t_eval_soft", "p3t_eval_direct",
+    "p3t_get_acc_pot", "p3t_get_neighbour_counts", "p3t_get_neighbours", "p3t_get_stats", "p3t_synchronize",
+    "p3t_last_error", "p3t_array_info", "p3t_copy_array",
+]
+
+ARRAYS = dict(root_cube=(0, np.float32, 1), keys=(1, np.uint64, 1), sorted_idx=(2, np.uint32, 1),
+              bodies=(3, np.float32, 4), cell_mac=(4, np.float32, 4), cell_mom0=(5, np.float32, 4),
+              cell_mom1=(6, np.float32, 4), cell_meta=(7, np.uint32, 2), cell_level=(8, np.uint8, 1),
+              cell_start=(9, np.uint32, 1), cell_parent=(10, np.uint32, 1), group_start=(11, np.uint32, 1),
+              cell_bmin=(12, np.float32, 4), cell_bmax=(13, np.float32, 4))
+
+
+class Stats(C.Structure):
+    _fields_ = [("n", C.c_uint64), ("n_pp", C.c_uint64), ("n_pc", C.c_uint64), ("n_near", C.c_uint64),
+                ("n_neighbours", C.c_uint64), ("n_cells", C.c_uint32), ("n_leaves", C.c_uint32),
+                ("n_groups", C.c_uint32), ("depth", C.c_uint32), ("max_list", C.c_uint32),
+                ("sort_passes", C.c_uint32), ("ms_sort", C.c_float), ("ms_build", C.c_float),
+                ("ms_moments", C.c_float), ("ms_walk", C.c_float), ("ms_nbr", C.c_float)]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_}
+
+
+def _sig():
+    vp, sz, i, f = C.c_void_p, C.c_size_t, C.c_int, C.c_float
+    L = _lib
+    L.p3t_workspace_bytes.restype = sz; L.p3t_workspace_bytes.argtypes = [sz, i, sz]
+    L.p3t_create.restype = i; L.p3t_create.argtypes = [C.POINTER(vp), i, sz, i, vp, sz, sz, vp]
+    L.p3t_destroy.restype = i; L.p3t_destroy.argtypes = [vp]
+    L.p3t_set_params.restype = i; L.p3t_set_params.argtypes = [vp, f, f, f, f, f]
+    L.p3t_set_tree_params.restype = i; L.p3t_set_tree_params.argtypes = [vp, i, i]
+    L.p3t_set_group_merge_levels.restype = i; L.p3t_set_group_merge_levels.argtypes = [vp, i]
+    L.p3t_load_particles.restype = i; L.p3t_load_particles.argtypes = [vp, sz, vp, vp, i]
+    L.p3t_build_tree.restype = i; L.p3t_build_tree.argtypes = [vp]
+    L.p3t_eval_soft.restype = i; L.p3t_eval_soft.argtypes = [vp]
+    L.p3t_eval_direct.restype = i; L.p3t_eval_direct.argtypes = [vp, vp, sz, i]
+    L.p3t_get_acc_pot.restype = i; L.p3t_get_acc_pot.argtypes = [vp, vp, vp, i]
+    L.p3t_get_neighbour_counts.restype = i; L.p3t_get_neighbour_counts.argtypes = [vp, vp, C.POINTER(C.c_uint64), i]
+    L.p3t_get_neighbours.restype = i; L.p3t_get_neighbours.argtypes = [vp, vp, vp, sz, i]
+    L.p3t_get_stats.restype = i; L.p3t_get_stats.argtypes = [vp, C.POINTER(Stats)]
+    L.p3t_synchronize.restype = i; L.p3t_synchronize.argtypes = [vp]
+    L.p3t_last_error.restype = C.c_char_p; L.p3t_last_error.argtypes = [vp]
+    L.p3t_array_info.restype = i; L.p3t_array_info.argtypes = [vp, i, C.POINTER(sz), C.POINTER(sz)]
+    L.p3t_copy_array.restype = i; L.p3t_copy_array.argtypes = [vp, i, vp, sz, i]
+
+
+_sig()
+
+
+class P3TError(RuntimeError):
+    def __init__(self, status, msg):
+        super().__init__(f"{_STATUS.get(status, status)}: {msg}")
+        self.status = status
+
+
+def p3t_workspace_bytes(max_n, key_bits=63, nbr_capacity=0):
+    return int(_lib.p3t_workspace_bytes(max_n, key_bits, nbr_capacity))
+
+
+def _ptr(x):
+    """Raw address of a numpy array (host) or torch tensor (device); None -> NULL."""
+    if x is None:
+        return None, 0
+    if isinstance(x, np.ndarray):
+        assert x.flags["C_CONTIGUOUS"]
+        return x.ctypes.data, 0
+    import torch
+    assert isinstance(x, torch.Tensor) and x.is_contiguous()
+    return x.data_ptr(), int(x.is_cuda)
+
+
+class P3T:
+    """One soft-force context (one GPU, one stream).  Method names follow the C ABI."""
+
+    def __init__(self, max_n, key_bits=63, nbr_capacity=None, device=0, stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_1506_04553_b200 needs a CUDA device; there is no CPU path")
+        self.torch = torch
+        self.device = device
+        self.max_n = int(max_n)
+        self.nbr_capacity = int(nbr_capacity if nbr_capacity is not None else max(4 * max_n, 1 << 16))
+        nbytes = p3t_workspace_bytes(self.max_n, key_bits, self.nbr_capacity)
+        if nbytes == 0:
+            raise P3TError(EINVAL, "invalid max_n / key_bits")
+        with torch.cuda.device(device):
+            self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=f"cuda:{device}")
+            base = self.workspace.data_ptr()
+            self._ws_ptr = (base + 255) & ~255
+            self._stream = stream if stream is not None else torch.cuda.current_stream(device)
+        h = C.c_void_p()
+        st = _lib.p3t_create(C.byref(h), device, self.max_n, key_bits, self._ws_ptr, nbytes, self.nbr_capacity,
+                             self._stream.cuda_stream)
+        if st != OK:
+            raise P3TError(st, "p3t_create failed")
+        self._h = h
+        self.n = 0
+
+    # -- plumbing ---------------------------------------------------------------------------------
+    def _check(self, st):
+        if st != OK:
+            raise P3TError(st, _lib.p3t_last_error(self._h).decode())
+
+    def close(self):
+        if getattr(self, "_h", None):
+            _lib.p3t_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()
+
+    # -- the C ABI, one method per entry point --------------------------------------------------------
+    def set_params(self, eps, theta, r_in, r_out, r_search):
+        self._check(_lib.p3t_set_params(self._h, eps, theta, r_in, r_out, r_search))
+
+    def set_tree_params(self, nleaf=16, ngroup=64):
+        self._check(_lib.p3t_set_tree_params(self._h, nleaf, ngroup))
+
+    def set_group_merge_levels(self, levels):
+        self._check(_lib.p3t_set_group_merge_levels(self._h, levels))
+
+    def load_particles(self, mass, pos):
+        """mass[n], pos[n,3] (or [3n]): float32 numpy arrays (host) or CUDA tensors (device)."""
+        pm, dm = _ptr(mass)
+        pp, dp = _ptr(pos)
+        if dm != dp:
+            raise P3TError(EINVAL, "mass and pos must both be host or both be device")
+        n = int(mass.shape[0])
+        if str(mass.dtype).split(".")[-1] != "float32" or str(pos.dtype).split(".")[-1] != "float32":
+            raise P3TError(EINVAL, "mass and pos must be float32")
+        if int(np.prod(pos.shape)) != 3 * n:
+            raise P3TError(EINVAL, "pos must hold 3 n values")
+        self._check(_lib.p3t_load_particles(self._h, n, pm, pp, dm))
+        self.n = n
+        self._keep = (mass, pos)   # keep inputs alive until the stream has consumed them
+
+    def build_tree(self):
+        self._check(_lib.p3t_build_tree(self._h))
+
+    def eval_soft(self):
+        self._check(_lib.p3t_eval_soft(self._h))
+
+    def eval_direct(self, subset=None):
+        if subset is None:
+            self._check(_lib.p3t_eval_direct(self._h, None, 0, 0))
+        else:
+            sub = np.ascontiguousarray(subset, dtype=np.uint32)
+            self._check(_lib.p3t_eval_direct(self._h, sub.ctypes.data, sub.shape[0], 0))
+
+    def get_acc_pot(self, on_device=False):
+        if on_device:
+            t = self.torch
+            acc = t.empty((self.n, 3), dtype=t.float32, device=f"cuda:{self.device}")
+            pot = t.empty(self.n, dtype=t.float32, device=f"cuda:{self.device}")
+            self._check(_lib.p3t_get_acc_pot(self._h, acc.data_ptr(), pot.data_ptr(), 1))
+            return acc, pot
+        acc = np.empty((self.n, 3), dtype=np.float32)
+        pot = np.empty(self.n, dtype=np.float32)
+        self._check(_lib.p3t_get_acc_pot(self._h, acc.ctypes.data, pot.ctypes.data, 0))
+        return acc, pot
+
+    def get_acc_pot_into(self, acc, pot):
+        """Write into caller-provided buffers (numpy or CUDA tensors)."""
+        pa, da = _ptr(acc)
+        pp, dp = _ptr(pot)
+        self._check(_lib.p3t_get_acc_pot(self._h, pa, pp, da if acc is not None else dp))
+
+    def get_neighbour_counts(self):
+        count = np.empty(self.n, dtype=np.uint32)
+        total = C.c_uint64()
+        self._check(_lib.p3t_get_neighbour_counts(self._h, count.ctypes.data, C.byref(total), 0))
+        return count, int(total.value)
+
+    def get_neighbours(self, capacity=None):
+        """CSR (offset[n+1] uint64, nbr[total] uint32) in user ids; lists ascending."""
+        cap = self.nbr_capacity if capacity is None else int(capacity)
+        offset = np.empty(self.n + 1, dtype=np.uint64)
+        nbr = np.empty(max(cap, 1), dtype=np.uint32)
+        self._check(_lib.p3t_get_neighbours(self._h, offset.ctypes.data, nbr.ctypes.data, cap, 0))
+        return offset, nbr[: int(offset[-1])]
+
+    def get_stats(self):
+        s = Stats()
+        self._check(_lib.p3t_get_stats(self._h, C.byref(s)))
+        return s.as_dict()
+
+    def synchronize(self):
+        self._check(_lib.p3t_synchronize(self._h))
+
+    def array(self, name):
+        """Copy of an intermediate array (a1-a6 inspection), as numpy."""
+        which, dtype, width = ARRAYS[name]
+        cnt, eb = C.c_size_t(), C.c_size_t()
+        self._check(_lib.p3t_array_info(self._h, which, C.byref(cnt), C.byref(eb)))
+        nbytes = cnt.value * eb.value
+        out = np.empty(nbytes // np.dtype(dtype).itemsize, dtype=dtype)
+        self._check(_lib.p3t_copy_array(self._h, which, out.ctypes.data, nbytes, 0))
+        return out.reshape(-1, width) if width > 1 else out
+
+    # -- convenience: the whole hot path for one batch -------------------------------------------------
+    def soft_force(self, mass, pos):
+        """load -> build -> eval; returns nothing (fetch with get_*)."""
+        self.load_particles(mass, pos)
+        self.build_tree()
+        self.eval_soft()

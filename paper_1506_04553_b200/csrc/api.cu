@@ -1,0 +1,465 @@
+// api.cu -- the C ABI of include/p3t.h: argument checks, workspace layout, stage sequencing.
+// Every numerical step is a CUDA kernel in the other files of this directory; no CPU fallback.
+#include <math.h>
+#include <new>
+#include <stdlib.h>
+
+#include "p3t_internal.cuh"
+
+// ------------------------------------------------------------------------------------------------
+// workspace layout
+// ------------------------------------------------------------------------------------------------
+namespace {
+struct Bump {
+    char *base;
+    size_t off;
+    template <class T> T *take(size_t count)
+    {
+        off = (off + 255) & ~size_t(255);
+        T *p = base ? reinterpret_cast<T *>(base + off) : nullptr;
+        off += count * sizeof(T);
+        return p;
+    }
+};
+} // namespace
+
+size_t p3t_layout(Workspace &ws, char *base, size_t max_n, int key_bits, size_t nbr_capacity, int sm_count)
+{
+    (void)key_bits;
+    Bump b{base, 0};
+    size_t n = max_n;
+    ws.cell_cap = 3 * n + 1024;
+    ws.n_tiles_max = (n + SORT_TILE - 1) / SORT_TILE;
+    ws.n_blk_max = (n + BUILD_THREADS - 1) / BUILD_THREADS;
+    ws.walk_warps_max = (size_t)sm_count * 16;   // upper bound of resident walk warps
+    ws.in_mass = b.take<float>(n);
+    ws.in_pos = b.take<float>(3 * n);
+    ws.body_user = b.take<float4>(n);
+    ws.cube = b.take<float>(8);
+    ws.bbox_bits = b.take<u32>(8);
+    ws.keys[0] = b.take<u64>(n);
+    ws.keys[1] = b.take<u64>(n);
+    ws.idx[0] = b.take<u32>(n);
+    ws.idx[1] = b.take<u32>(n);
+    ws.hist = b.take<u32>(8 * 256);
+    ws.tile_status = b.take<u32>(8 * ws.n_tiles_max * 256);
+    ws.body = b.take<float4>(n);
+    ws.clev = b.take<signed char>(n + 2);
+    ws.dlev = b.take<u8>(n);
+    ws.cutflag = b.take<u8>(n);
+    ws.glev = b.take<u8>(n);
+    ws.head_status = b.take<u32>(ws.n_blk_max);
+    ws.blk_level_cnt = b.take<u32>(ws.n_blk_max * 32);
+    ws.blk_level_off = b.take<u32>(ws.n_blk_max * 32);
+    ws.level_total = b.take<u32>(64);
+    ws.group_start = b.take<u32>(n + 1);
+    ws.cell_mac = b.take<float4>(ws.cell_cap);
+    ws.cell_mom0 = b.take<float4>(ws.cell_cap);
+    ws.cell_mom1 = b.take<float4>(ws.cell_cap);
+    ws.cell_bmin = b.take<float4>(ws.cell_cap);
+    ws.cell_bmax = b.take<float4>(ws.cell_cap);
+    ws.cell_meta = b.take<uint2>(ws.cell_cap);
+    ws.cell_level = b.take<u8>(ws.cell_cap);
+    ws.cell_start = b.take<u32>(ws.cell_cap);
+    ws.cell_parent = b.take<u32>(ws.cell_cap);
+    ws.cell_first = b.take<u32>(ws.cell_cap);
+    ws.cell_nchild = b.take<u32>(ws.cell_cap);
+    ws.cell_ready = b.take<u32>(ws.cell_cap);
+    ws.accpot = b.take<float4>(n);
+    ws.nbr_count = b.take<u32>(n);
+    ws.nbr_offset = b.take<u64>(n + 1);
+    ws.pairs = b.take<uint2>(nbr_capacity ? nbr_capacity : 1);
+    ws.nbr = b.take<u32>(nbr_capacity ? nbr_capacity : 1);
+    ws.nbr_cursor = b.take<u32>(n);
+    ws.subset = b.take<u32>(n);
+    ws.counters = b.take<u64>(CNT_WORDS);
+    ws.walk_stack = b.take<u32>(ws.walk_warps_max * WALK_STACK_GMEM);
+    ws.scan_tmp = b.take<u64>((n + 1023) / 1024 + 2);
+    b.off = (b.off + 255) & ~size_t(255);
+    ws.total_bytes = b.off;
+    return b.off;
+}
+
+static bool valid_sizes(size_t max_n, int key_bits)
+{
+    return max_n >= 1 && max_n < (size_t(1) << 30) && (key_bits == 30 || key_bits == 63);
+}
+
+extern "C" size_t p3t_workspace_bytes(size_t max_n, int key_bits, size_t nbr_capacity)
+{
+    if (!valid_sizes(max_n, key_bits)) return 0;
+    Workspace ws;
+    return p3t_layout(ws, nullptr, max_n, key_bits, nbr_capacity, 160 /* >= SMs of any B200 */);
+}
+
+// ------------------------------------------------------------------------------------------------
+// lifetime
+// ------------------------------------------------------------------------------------------------
+extern "C" p3t_status p3t_create(p3t_ctx **out, int device, size_t max_n, int key_bits, void *workspace,
+                                 size_t workspace_bytes, size_t nbr_capacity, void *cuda_stream)
+{
+    if (!out) return P3T_EINVAL;
+    *out = nullptr;
+    if (!valid_sizes(max_n, key_bits) || !workspace) return P3T_EINVAL;
+    if ((reinterpret_cast<uintptr_t>(workspace) & 255) != 0) return P3T_EINVAL;
+    p3t_ctx *ctx = new (std::nothrow) p3t_ctx();
+    if (!ctx) return P3T_ENOMEM;
+    memset(ctx, 0, sizeof(*ctx));
+    ctx->device = device;
+    ctx->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
+    ctx->max_n = max_n;
+    ctx->key_bits = key_bits;
+    ctx->max_level = key_bits == 63 ? 21 : 10;
+    ctx->nbr_capacity = nbr_capacity;
+    ctx->nleaf = 16;
+    ctx->ngroup = 64;
+    ctx->merge_levels = 1;
+    cudaError_t e = cudaSetDevice(device);
+    cudaDeviceProp prop;
+    if (e == cudaSuccess) e = cudaGetDeviceProperties(&prop, device);
+    if (e != cudaSuccess) {
+        delete ctx;
+        return P3T_ECUDA;
+    }
+    ctx->sm_count = prop.multiProcessorCount;
+    if (ctx->sm_count > 160) { delete ctx; return P3T_EINVAL; }
+    size_t need = p3t_layout(ctx->ws, static_cast<char *>(workspace), max_n, key_bits, nbr_capacity, 160);
+    if (workspace_bytes < need) {
+        delete ctx;
+        return P3T_ENOMEM;
+    }
+    ctx->base = static_cast<char *>(workspace);
+    for (int i = 0; i < 8; ++i) {
+        if (cudaEventCreate(&ctx->ev[i]) != cudaSuccess) { delete ctx; return P3T_ECUDA; }
+    }
+    *out = ctx;
+    return P3T_OK;
+}
+
+extern "C" p3t_status p3t_destroy(p3t_ctx *ctx)
+{
+    if (!ctx) return P3T_EINVAL;
+    cudaStreamSynchronize(ctx->stream);
+    for (int i = 0; i < 8; ++i)
+        if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
+    delete ctx;
+    return P3T_OK;
+}
+
+extern "C" const char *p3t_last_error(const p3t_ctx *ctx) { return ctx ? ctx->err : "null context"; }
+
+// ------------------------------------------------------------------------------------------------
+// parameters
+// ------------------------------------------------------------------------------------------------
+extern "C" p3t_status p3t_set_params(p3t_ctx *ctx, float eps, float theta, float r_in, float r_out, float r_search)
+{
+    if (!ctx) return P3T_EINVAL;
+    if (!(eps >= 0.f) || !(theta >= 0.f) || !isfinite(eps) || !isfinite(theta) || !isfinite(r_search) ||
+        !(r_in >= 0.f) || !(r_in < r_out) || !(r_out <= r_search))
+        return p3t_fail(ctx, P3T_EINVAL, "need eps >= 0, theta >= 0, 0 <= r_in < r_out <= r_search, all finite");
+    ctx->eps = eps; ctx->theta = theta; ctx->r_in = r_in; ctx->r_out = r_out; ctx->r_search = r_search;
+    P3TParams &p = ctx->prm;
+    p.eps2 = eps * eps;
+    p.theta = theta;
+    p.r_in = r_in; p.r_out = r_out; p.h = r_search;
+    p.rout2 = r_out * r_out;
+    p.h2 = r_search * r_search;
+    {   // bodies whose distance to the group's box is below this go to the K/W + neighbour-test path
+        float hn = r_search * (1.f + 1e-5f);
+        p.hnear2 = hn * hn;
+    }
+    // W(y; gamma) of Eq. 16-17 as coefficients of y^k and y ln y; the
+    // denominator of Eq. 17 is taken as (gamma-1)^7 (reading A1).
+    double g = (double)r_in / (double)r_out;
+    double g2 = g * g, g3 = g2 * g, g4 = g2 * g2, g5 = g4 * g, g6 = g3 * g3, g7 = g6 * g;
+    double D = pow(g - 1.0, 7);
+    p.gamma = g;
+    p.inv_rout = 1.0 / (double)r_out;
+    p.inv_1mg = 1.0 / (1.0 - g);
+    p.wc[7] = (-10.0 / 3.0) / D;
+    p.wc[6] = 14.0 * (g + 1.0) / D;
+    p.wc[5] = -21.0 * (g2 + 3.0 * g + 1.0) / D;
+    p.wc[4] = (35.0 / 3.0) * (g3 + 9.0 * g2 + 9.0 * g + 1.0) / D;
+    p.wc[3] = -70.0 * (g3 + 3.0 * g2 + g) / D;
+    p.wc[2] = 210.0 * (g3 + g2) / D;
+    p.wc[0] = (g7 - 7.0 * g6 + 21.0 * g5 - 35.0 * g4) / D;
+    p.wl = -140.0 * g3 / D;
+    double G1 = p.wc[7] + p.wc[6] + p.wc[5] + p.wc[4] + p.wc[3] + p.wc[2] + p.wc[0];   // ln 1 = 0
+    p.wc[1] = 1.0 - G1;
+    double glog = g > 0.0 ? 60.0 * g3 * log(g) : 0.0;
+    p.cin = 7.0 * (g6 - 9.0 * g5 + 45.0 * g4 - glog - 45.0 * g2 + 9.0 * g - 1.0) / (3.0 * D);
+    ctx->have_params = true;
+    ctx->built = false;        // theta and h enter the per-cell acceptance radius
+    ctx->evaluated = false;
+    return P3T_OK;
+}
+
+extern "C" p3t_status p3t_set_tree_params(p3t_ctx *ctx, int nleaf, int ngroup)
+{
+    if (!ctx) return P3T_EINVAL;
+    if (nleaf < 1 || nleaf > 32 || (ngroup != 32 && ngroup != 64))
+        return p3t_fail(ctx, P3T_EINVAL, "need 1 <= nleaf <= 32 and ngroup in {32, 64}");
+    ctx->nleaf = nleaf;
+    ctx->ngroup = ngroup;
+    ctx->built = false;
+    ctx->evaluated = false;
+    return P3T_OK;
+}
+
+// undocumented tuning knob used by bench.py sweeps: levels above the natural group level whose
+// boundaries an i-group may straddle (0 = groups are single octree cells)
+extern "C" p3t_status p3t_set_group_merge_levels(p3t_ctx *ctx, int levels)
+{
+    if (!ctx || levels < 0 || levels > 4) return P3T_EINVAL;
+    ctx->merge_levels = levels;
+    ctx->built = false;
+    ctx->evaluated = false;
+    return P3T_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// load / build / eval
+// ------------------------------------------------------------------------------------------------
+extern "C" p3t_status p3t_load_particles(p3t_ctx *ctx, size_t n, const float *mass, const float *pos, int on_device)
+{
+    if (!ctx) return P3T_EINVAL;
+    if (!mass || !pos) return p3t_fail(ctx, P3T_EINVAL, "null mass/pos");
+    if (n == 0 || n > ctx->max_n) return p3t_fail(ctx, P3T_EINVAL, "n must be in 1..max_n");
+    P3T_CUDA(ctx, cudaSetDevice(ctx->device));
+    const float *d_mass = mass, *d_pos = pos;
+    if (!on_device) {
+        for (size_t i = 0; i < n; ++i)
+            if (!isfinite(mass[i])) return p3t_fail(ctx, P3T_EINVAL, "non-finite mass");
+        for (size_t i = 0; i < 3 * n; ++i)
+            if (!isfinite(pos[i])) return p3t_fail(ctx, P3T_EINVAL, "non-finite position");
+        P3T_CUDA(ctx, cudaMemcpyAsync(ctx->ws.in_mass, mass, n * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
+        P3T_CUDA(ctx, cudaMemcpyAsync(ctx->ws.in_pos, pos, 3 * n * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
+        d_mass = ctx->ws.in_mass;
+        d_pos = ctx->ws.in_pos;
+    }
+    ctx->n = n;
+    ctx->loaded = false;
+    ctx->built = false;
+    ctx->evaluated = false;
+    p3t_status st = p3t_stage_pack(ctx, d_mass, d_pos);
+    if (st != P3T_OK) return st;
+    ctx->loaded = true;
+    return P3T_OK;
+}
+
+extern "C" p3t_status p3t_build_tree(p3t_ctx *ctx)
+{
+    if (!ctx) return P3T_EINVAL;
+    if (!ctx->loaded) return p3t_fail(ctx, P3T_ESTATE, "p3t_build_tree before p3t_load_particles");
+    if (!ctx->have_params) return p3t_fail(ctx, P3T_ESTATE, "p3t_build_tree before p3t_set_params");
+    P3T_CUDA(ctx, cudaSetDevice(ctx->device));
+    ctx->built = false;
+    ctx->evaluated = false;
+    p3t_status st;
+    P3T_CUDA(ctx, cudaEventRecord(ctx->ev[0], ctx->stream));
+    if ((st = p3t_stage_sort(ctx)) != P3T_OK) return st;
+    P3T_CUDA(ctx, cudaEventRecord(ctx->ev[1], ctx->stream));
+    if ((st = p3t_stage_build(ctx)) != P3T_OK) return st;
+    P3T_CUDA(ctx, cudaEventRecord(ctx->ev[2], ctx->stream));
+    if ((st = p3t_stage_moments(ctx)) != P3T_OK) return st;
+    P3T_CUDA(ctx, cudaEventRecord(ctx->ev[3], ctx->stream));
+    ctx->ev_build = true;
+    ctx->built = true;
+    return P3T_OK;
+}
+
+extern "C" p3t_status p3t_eval_soft(p3t_ctx *ctx)
+{
+    if (!ctx) return P3T_EINVAL;
+    if (!ctx->built) return p3t_fail(ctx, P3T_ESTATE, "p3t_eval_soft needs a tree built for the current particles and parameters");
+    P3T_CUDA(ctx, cudaSetDevice(ctx->device));
+    ctx->evaluated = false;
+    p3t_status st;
+    P3T_CUDA(ctx, cudaEventRecord(ctx->ev[4], ctx->stream));
+    if ((st = p3t_stage_walk(ctx)) != P3T_OK) return st;
+    P3T_CUDA(ctx, cudaEventRecord(ctx->ev[5], ctx->stream));
+    if ((st = p3t_stage_neighbours(ctx)) != P3T_OK) return st;
+    P3T_CUDA(ctx, cudaEventRecord(ctx->ev[6], ctx->stream));
+    ctx->ev_eval = true;
+    ctx->evaluated = true;
+    return P3T_OK;
+}
+
+extern "C" p3t_status p3t_eval_direct(p3t_ctx *ctx, const uint32_t *i_subset, size_t n_subset, int on_device)
+{
+    if (!ctx) return P3T_EINVAL;
+    if (!ctx->loaded) return p3t_fail(ctx, P3T_ESTATE, "p3t_eval_direct before p3t_load_particles");
+    if (!ctx->have_params) return p3t_fail(ctx, P3T_ESTATE, "p3t_eval_direct before p3t_set_params");
+    if (i_subset && (n_subset == 0 || n_subset > ctx->n)) return p3t_fail(ctx, P3T_EINVAL, "bad subset size");
+    P3T_CUDA(ctx, cudaSetDevice(ctx->device));
+    const u32 *d_subset = i_subset;
+    if (i_subset && !on_device) {
+        for (size_t k = 0; k < n_subset; ++k)
+            if (i_subset[k] >= ctx->n) return p3t_fail(ctx, P3T_EINVAL, "subset index out of range");
+        P3T_CUDA(ctx, cudaMemcpyAsync(ctx->ws.subset, i_subset, n_subset * sizeof(u32), cudaMemcpyHostToDevice, ctx->stream));
+        d_subset = ctx->ws.subset;
+    }
+    ctx->evaluated = false;
+    p3t_status st;
+    P3T_CUDA(ctx, cudaEventRecord(ctx->ev[4], ctx->stream));
+    if ((st = p3t_stage_direct(ctx, d_subset, i_subset ? n_subset : ctx->n)) != P3T_OK) return st;
+    P3T_CUDA(ctx, cudaEventRecord(ctx->ev[5], ctx->stream));
+    if ((st = p3t_stage_neighbours(ctx)) != P3T_OK) return st;
+    P3T_CUDA(ctx, cudaEventRecord(ctx->ev[6], ctx->stream));
+    ctx->ev_eval = true;
+    ctx->evaluated = true;
+    return P3T_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// synchronisation and deferred errors
+// ------------------------------------------------------------------------------------------------
+static p3t_status sync_and_check(p3t_ctx *ctx)
+{
+    P3T_CUDA(ctx, cudaSetDevice(ctx->device));
+    P3T_CUDA(ctx, cudaMemcpyAsync(ctx->h_counters, ctx->ws.counters, sizeof(ctx->h_counters), cudaMemcpyDeviceToHost, ctx->stream));
+    P3T_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    if (ctx->h_counters[CNT_NONFINITE]) return p3t_fail(ctx, P3T_EINVAL, "non-finite mass or position in the device input");
+    u64 f = ctx->h_counters[CNT_ERR_BUILD] | ctx->h_counters[CNT_ERR_EVAL];
+    if (f & ERR_CELL_CAPACITY) return p3t_fail(ctx, P3T_ENOMEM, "octree cell capacity (3 n + 1024) exceeded");
+    if (f & ERR_STACK_OVERFLOW) return p3t_fail(ctx, P3T_ENOMEM, "tree-walk stack overflow");
+    return P3T_OK;
+}
+
+extern "C" p3t_status p3t_synchronize(p3t_ctx *ctx)
+{
+    if (!ctx) return P3T_EINVAL;
+    return sync_and_check(ctx);
+}
+
+// ------------------------------------------------------------------------------------------------
+// fetch
+// ------------------------------------------------------------------------------------------------
+extern "C" p3t_status p3t_get_acc_pot(p3t_ctx *ctx, float *acc, float *pot, int on_device)
+{
+    if (!ctx) return P3T_EINVAL;
+    if (!ctx->evaluated) return p3t_fail(ctx, P3T_ESTATE, "p3t_get_acc_pot before an eval call");
+    P3T_CUDA(ctx, cudaSetDevice(ctx->device));
+    size_t n = ctx->n;
+    if (on_device) return p3t_stage_unpack(ctx, acc, pot);
+    // host destination: unpack into the (now free) input staging arrays, then copy out
+    p3t_status st = p3t_stage_unpack(ctx, acc ? ctx->ws.in_pos : nullptr, pot ? ctx->ws.in_mass : nullptr);
+    if (st != P3T_OK) return st;
+    if (acc) P3T_CUDA(ctx, cudaMemcpyAsync(acc, ctx->ws.in_pos, 3 * n * sizeof(float), cudaMemcpyDeviceToHost, ctx->stream));
+    if (pot) P3T_CUDA(ctx, cudaMemcpyAsync(pot, ctx->ws.in_mass, n * sizeof(float), cudaMemcpyDeviceToHost, ctx->stream));
+    return sync_and_check(ctx);
+}
+
+extern "C" p3t_status p3t_get_neighbour_counts(p3t_ctx *ctx, uint32_t *count, uint64_t *total, int on_device)
+{
+    if (!ctx) return P3T_EINVAL;
+    if (!ctx->evaluated) return p3t_fail(ctx, P3T_ESTATE, "p3t_get_neighbour_counts before an eval call");
+    P3T_CUDA(ctx, cudaSetDevice(ctx->device));
+    if (count)
+        P3T_CUDA(ctx, cudaMemcpyAsync(count, ctx->ws.nbr_count, ctx->n * sizeof(u32),
+                                      on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, ctx->stream));
+    if (total || !on_device) {
+        p3t_status st = sync_and_check(ctx);
+        if (st != P3T_OK) return st;
+        if (total) *total = ctx->h_counters[CNT_PAIRS];
+    }
+    return P3T_OK;
+}
+
+extern "C" p3t_status p3t_get_neighbours(p3t_ctx *ctx, uint64_t *offset, uint32_t *nbr, size_t capacity, int on_device)
+{
+    if (!ctx) return P3T_EINVAL;
+    if (!ctx->evaluated) return p3t_fail(ctx, P3T_ESTATE, "p3t_get_neighbours before an eval call");
+    if (!offset) return p3t_fail(ctx, P3T_EINVAL, "null offset");
+    P3T_CUDA(ctx, cudaSetDevice(ctx->device));
+    cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+    P3T_CUDA(ctx, cudaMemcpyAsync(offset, ctx->ws.nbr_offset, (ctx->n + 1) * sizeof(u64), kind, ctx->stream));
+    p3t_status st = sync_and_check(ctx);
+    if (st != P3T_OK) return st;
+    u64 total = ctx->h_counters[CNT_PAIRS];
+    if (total > ctx->nbr_capacity) return p3t_fail(ctx, P3T_ECAPACITY, "neighbour lists exceed the context's nbr_capacity");
+    if (total > capacity) return p3t_fail(ctx, P3T_ECAPACITY, "neighbour lists exceed the caller's buffer");
+    if (total && !nbr) return p3t_fail(ctx, P3T_EINVAL, "null nbr");
+    if (total) {
+        P3T_CUDA(ctx, cudaMemcpyAsync(nbr, ctx->ws.nbr, total * sizeof(u32), kind, ctx->stream));
+        P3T_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    }
+    return P3T_OK;
+}
+
+extern "C" p3t_status p3t_get_stats(p3t_ctx *ctx, p3t_stats *out)
+{
+    if (!ctx || !out) return P3T_EINVAL;
+    p3t_status st = sync_and_check(ctx);
+    memset(out, 0, sizeof(*out));
+    const u64 *c = ctx->h_counters;
+    out->n = ctx->n;
+    out->n_pp = c[CNT_NPP]; out->n_pc = c[CNT_NPC]; out->n_near = c[CNT_NNEAR];
+    out->n_neighbours = c[CNT_PAIRS];
+    out->n_cells = (u32)c[CNT_NCELLS]; out->n_leaves = (u32)c[CNT_NLEAVES]; out->n_groups = (u32)c[CNT_NGROUPS];
+    out->depth = (u32)c[CNT_DEPTH]; out->max_list = (u32)c[CNT_MAXLIST];
+    out->sort_passes = (u32)((3 * ctx->max_level + 7) / 8);
+    if (ctx->ev_build) {
+        cudaEventElapsedTime(&out->ms_sort, ctx->ev[0], ctx->ev[1]);
+        cudaEventElapsedTime(&out->ms_build, ctx->ev[1], ctx->ev[2]);
+        cudaEventElapsedTime(&out->ms_moments, ctx->ev[2], ctx->ev[3]);
+    }
+    if (ctx->ev_eval) {
+        cudaEventElapsedTime(&out->ms_walk, ctx->ev[4], ctx->ev[5]);
+        cudaEventElapsedTime(&out->ms_nbr, ctx->ev[5], ctx->ev[6]);
+    }
+    return st;
+}
+
+// ------------------------------------------------------------------------------------------------
+// inspection
+// ------------------------------------------------------------------------------------------------
+static p3t_status array_desc(p3t_ctx *ctx, p3t_array which, const void **ptr, size_t *count, size_t *elem)
+{
+    Workspace &w = ctx->ws;
+    size_t nc = (size_t)ctx->h_counters[CNT_NCELLS], ng = (size_t)ctx->h_counters[CNT_NGROUPS], n = ctx->n;
+    switch (which) {
+    case P3T_ARR_ROOT_CUBE:   *ptr = w.cube; *count = 4; *elem = 4; break;
+    case P3T_ARR_KEYS:        *ptr = w.keys[ctx->cur]; *count = n; *elem = 8; break;
+    case P3T_ARR_SORTED_IDX:  *ptr = w.idx[ctx->cur]; *count = n; *elem = 4; break;
+    case P3T_ARR_BODIES:      *ptr = w.body; *count = n; *elem = 16; break;
+    case P3T_ARR_CELL_MAC:    *ptr = w.cell_mac; *count = nc; *elem = 16; break;
+    case P3T_ARR_CELL_MOM0:   *ptr = w.cell_mom0; *count = nc; *elem = 16; break;
+    case P3T_ARR_CELL_MOM1:   *ptr = w.cell_mom1; *count = nc; *elem = 16; break;
+    case P3T_ARR_CELL_META:   *ptr = w.cell_meta; *count = nc; *elem = 8; break;
+    case P3T_ARR_CELL_LEVEL:  *ptr = w.cell_level; *count = nc; *elem = 1; break;
+    case P3T_ARR_CELL_START:  *ptr = w.cell_start; *count = nc; *elem = 4; break;
+    case P3T_ARR_CELL_PARENT: *ptr = w.cell_parent; *count = nc; *elem = 4; break;
+    case P3T_ARR_GROUP_START: *ptr = w.group_start; *count = ng + 1; *elem = 4; break;
+    case P3T_ARR_CELL_BMIN:   *ptr = w.cell_bmin; *count = nc; *elem = 16; break;
+    case P3T_ARR_CELL_BMAX:   *ptr = w.cell_bmax; *count = nc; *elem = 16; break;
+    default: return p3t_fail(ctx, P3T_EINVAL, "unknown array id");
+    }
+    return P3T_OK;
+}
+
+extern "C" p3t_status p3t_array_info(p3t_ctx *ctx, p3t_array which, size_t *count, size_t *elem_bytes)
+{
+    if (!ctx || !count || !elem_bytes) return P3T_EINVAL;
+    if (!ctx->built) return p3t_fail(ctx, P3T_ESTATE, "p3t_array_info before p3t_build_tree");
+    p3t_status st = sync_and_check(ctx);
+    if (st != P3T_OK) return st;
+    const void *p;
+    return array_desc(ctx, which, &p, count, elem_bytes);
+}
+
+extern "C" p3t_status p3t_copy_array(p3t_ctx *ctx, p3t_array which, void *dst, size_t dst_bytes, int on_device)
+{
+    if (!ctx || !dst) return P3T_EINVAL;
+    if (!ctx->built) return p3t_fail(ctx, P3T_ESTATE, "p3t_copy_array before p3t_build_tree");
+    p3t_status st = sync_and_check(ctx);
+    if (st != P3T_OK) return st;
+    const void *p;
+    size_t count, elem;
+    if ((st = array_desc(ctx, which, &p, &count, &elem)) != P3T_OK) return st;
+    if (dst_bytes < count * elem) return p3t_fail(ctx, P3T_ECAPACITY, "destination too small");
+    if (count)
+        P3T_CUDA(ctx, cudaMemcpyAsync(dst, p, count * elem, on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, ctx->stream));
+    P3T_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    return P3T_OK;
+}

@@ -1,0 +1,193 @@
+// p3t_internal.cuh -- context, workspace layout and device helpers shared by the
+// kernels of the soft-force library (include/p3t.h is the public boundary).
+// Nothing here is shared with oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string.h>
+
+#include "p3t.h"
+
+typedef unsigned long long u64;
+typedef unsigned int u32;
+typedef unsigned char u8;
+
+#define P3T_MAX_LEVELS 22          // levels 0..21 (63-bit keys); 0..10 with 30-bit keys
+#define P3T_LEAF_FLAG 0x80000000u
+#define P3T_NO_PARENT 0xffffffffu
+
+// ---- tuning constants -------------------------------------------------
+#define SORT_THREADS 256
+#define SORT_ITEMS 8
+#define SORT_TILE (SORT_THREADS * SORT_ITEMS)
+#define BUILD_THREADS 256
+#define WALK_WARPS 4                 // warps per CTA in the walk kernel
+#define WALK_STACK_SMEM 1024         // stack entries per warp held in shared memory
+#define WALK_STACK_GMEM 7168         // overflow entries per warp in global memory
+
+// Parameters handed to kernels by value.  The coefficients of W are prepared on the host in
+// double precision (set_params): for gamma <= y < 1
+//   W(y) = sum_{k=0..7} wc[k] y^k + wl * y ln y          (Eq. 16-17 with reading A1)
+// and W(y) = cin * y below gamma.  K(x) = x^4 (35 - 84 x + 70 x^2 - 20 x^3)  (Eq. 12).
+struct P3TParams {
+    float eps2;        // eps^2
+    float theta;
+    float r_in, r_out, h;
+    float rout2;       // r_out^2
+    float h2;          // h^2                 (neighbour test  s^2 < h^2, reading A4)
+    float hnear2;      // (h (1+1e-5))^2 + slack: bodies whose box distance is below this take the slow path
+    double inv_rout;   // 1 / r_out
+    double gamma;      // r_in / r_out
+    double inv_1mg;    // 1 / (1 - gamma)
+    double cin;        // slope of W below gamma
+    double wc[8];
+    double wl;
+};
+
+// Device-side counters (one block of 64-bit words in the workspace, zeroed per eval/build).
+enum {
+    // zeroed at every eval
+    CNT_NPP = 0, CNT_NPC, CNT_NNEAR, CNT_PAIRS, CNT_GROUP_TICKET, CNT_MAXLIST, CNT_ERR_EVAL, CNT_EVAL_SPARE,
+    // zeroed at every build
+    CNT_NCELLS = 8, CNT_NLEAVES, CNT_NGROUPS, CNT_DEPTH, CNT_ERR_BUILD, CNT_HEAD_TICKET, CNT_HEAD_SPARE0, CNT_HEAD_SPARE1,
+    CNT_SORT_TICKET = 16 /* one per pass, 8 */,
+    // zeroed at load
+    CNT_NONFINITE = 24,
+    CNT_WORDS = 32
+};
+enum { ERR_STACK_OVERFLOW = 1, ERR_CELL_CAPACITY = 2 };
+
+struct Workspace {
+    // inputs
+    float *in_mass, *in_pos;       // staging for host inputs
+    float4 *body_user;             // (x,y,z,m) user order
+    // a1-a4
+    float *cube;                   // [8]: min xyz, side, max xyz, pad   (cube[0..3] = P3T_ARR_ROOT_CUBE)
+    u32 *bbox_bits;                // [6] ordered-int min/max accumulators
+    u64 *keys[2];
+    u32 *idx[2];
+    u32 *hist;                     // [8][256] digit histograms -> exclusive offsets
+    u32 *tile_status;              // [8][ntiles][256]
+    float4 *body;                  // sorted
+    // a5
+    signed char *clev;             // [n+1]  common-prefix levels between sorted neighbours (c[0] = -1)
+    u8 *dlev;                      // [n] leaf level of each body
+    u8 *cutflag;                   // [n] segment cut (group construction)
+    u8 *glev;                      // [n] natural group level of each body
+    u32 *head_status;              // [nblk] look-back words of the group-head compaction
+    u32 *blk_level_cnt;            // [nblk][32]: nodes per level starting in the block
+    u32 *blk_level_off;            // same shape, exclusive over blocks
+    u32 *level_total;              // [32]
+    u32 *group_start;              // [n+1]
+    // cells
+    float4 *cell_mac, *cell_mom0, *cell_mom1, *cell_bmin, *cell_bmax;
+    uint2 *cell_meta;
+    u8 *cell_level;
+    u32 *cell_start, *cell_parent, *cell_first, *cell_nchild, *cell_ready;
+    // outputs
+    float4 *accpot;                // user order (ax, ay, az, phi)
+    u32 *nbr_count;                // user order
+    u64 *nbr_offset;               // [n+1]
+    uint2 *pairs;                  // [cap] (i_user, j_user)
+    u32 *nbr;                      // [cap]
+    u32 *nbr_cursor;               // [n]
+    u32 *subset;                   // [n] staging for eval_direct
+    u64 *counters;                 // [CNT_WORDS]
+    u32 *walk_stack;               // [nwarps][WALK_STACK_GMEM]
+    u64 *scan_tmp;                 // [nblk_scan + 1]
+    size_t total_bytes;
+    size_t cell_cap, n_tiles_max, n_blk_max, walk_warps_max;
+};
+
+struct p3t_ctx {
+    int device;
+    cudaStream_t stream;
+    size_t max_n, n, nbr_capacity;
+    int key_bits, max_level, nleaf, ngroup, merge_levels;
+    int sm_count;
+    bool have_params, loaded, built, evaluated;
+    int cur;                       // which of keys[2]/idx[2] holds the sorted result
+    P3TParams prm;
+    float eps, theta, r_in, r_out, r_search;
+    Workspace ws;
+    char *base;
+    cudaEvent_t ev[8];             // phase boundaries: 0 build start,1 sort end,2 build end,3 moments end,4 eval start,5 walk end,6 nbr end
+    bool ev_build, ev_eval;
+    char err[512];
+    // host mirrors (valid after sync)
+    u64 h_counters[CNT_WORDS];
+};
+
+// Lays the arrays out over `base` (may be NULL to only measure).  Returns total bytes.
+size_t p3t_layout(Workspace &ws, char *base, size_t max_n, int key_bits, size_t nbr_capacity, int sm_count);
+
+#define P3T_CUDA(ctx, call)                                                                        \
+    do {                                                                                           \
+        cudaError_t e_ = (call);                                                                   \
+        if (e_ != cudaSuccess) {                                                                   \
+            snprintf((ctx)->err, sizeof((ctx)->err), "%s failed: %s (%s:%d)", #call,               \
+                     cudaGetErrorString(e_), __FILE__, __LINE__);                                  \
+            return P3T_ECUDA;                                                                      \
+        }                                                                                          \
+    } while (0)
+
+static inline p3t_status p3t_fail(p3t_ctx *ctx, p3t_status st, const char *msg)
+{
+    if (ctx) snprintf(ctx->err, sizeof(ctx->err), "%s", msg);
+    return st;
+}
+
+static inline u32 div_up(size_t a, size_t b) { return (u32)((a + b - 1) / b); }
+
+// stage entry points (each enqueues kernels on ctx->stream)
+p3t_status p3t_stage_pack(p3t_ctx *ctx, const float *d_mass, const float *d_pos);
+p3t_status p3t_stage_sort(p3t_ctx *ctx);
+p3t_status p3t_stage_build(p3t_ctx *ctx);
+p3t_status p3t_stage_moments(p3t_ctx *ctx);
+p3t_status p3t_stage_walk(p3t_ctx *ctx);
+p3t_status p3t_stage_direct(p3t_ctx *ctx, const u32 *d_subset, size_t n_subset);
+p3t_status p3t_stage_neighbours(p3t_ctx *ctx);
+p3t_status p3t_stage_unpack(p3t_ctx *ctx, float *d_acc, float *d_pot);
+
+#ifdef __CUDACC__
+// ---- device helpers ----------------------------------------------------------------------------
+
+// Cutoff weights on the slow path (pairs with s < r_out), double precision because the closed
+// form of W cancels from terms of size ~57 at gamma = 0.1 (hard part 8).
+__device__ __forceinline__ void p3t_pair_weights(const P3TParams &p, float s2, float &K, float &W)
+{
+    double s = sqrt((double)s2);
+    double y = s * p.inv_rout;
+    if (y >= 1.0) { K = 1.f; W = 1.f; return; }
+    if (y < p.gamma) { K = 0.f; W = (float)(p.cin * y); return; }
+    double x = (y - p.gamma) * p.inv_1mg;
+    double x2 = x * x;
+    double k = x2 * x2 * (35.0 + x * (-84.0 + x * (70.0 - 20.0 * x)));
+    double w = p.wc[7];
+#pragma unroll
+    for (int i = 6; i >= 0; --i) w = w * y + p.wc[i];
+    w += p.wl * y * log(y);
+    K = (float)k;
+    W = (float)w;
+}
+
+__device__ __forceinline__ u32 lanemask_lt()
+{
+    u32 m;
+    asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
+    return m;
+}
+
+// order-preserving float <-> uint mapping for atomicMin/Max on floats
+__device__ __forceinline__ u32 float_to_ordered(float f)
+{
+    u32 u = __float_as_uint(f);
+    return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+}
+__device__ __forceinline__ float ordered_to_float(u32 u)
+{
+    return __uint_as_float((u & 0x80000000u) ? (u & 0x7fffffffu) : ~u);
+}
+#endif

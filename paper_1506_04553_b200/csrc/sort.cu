@@ -1,0 +1,333 @@
+// sort.cu -- rows a1-a4 of the hot path:
+//   a1 bounding cube, a2 Morton keys, a3 onesweep LSD radix sort of (key, index), a4 body gather.
+// The paper only says "Barnes-Hut tree algorithm"; the key/sort formulation is
+// this library's own (north_star).  All kernels are HBM/L2-bandwidth bound.
+#include "p3t_internal.cuh"
+
+// ------------------------------------------------------------------------------------------------
+// a1: pack (mass, pos) -> float4 bodies in user order, min/max of positions, finiteness check
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) pack_bbox_kernel(const float *__restrict__ mass, const float *__restrict__ pos,
+                                                        float4 *__restrict__ body, u32 *bbox_bits, u64 *counters, u32 n)
+{
+    float lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY};
+    int bad = 0;
+    for (u32 i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        float x = pos[3 * (size_t)i], y = pos[3 * (size_t)i + 1], z = pos[3 * (size_t)i + 2], m = mass[i];
+        body[i] = make_float4(x, y, z, m);
+        bad |= !(isfinite(x) && isfinite(y) && isfinite(z) && isfinite(m));
+        lo[0] = fminf(lo[0], x); hi[0] = fmaxf(hi[0], x);
+        lo[1] = fminf(lo[1], y); hi[1] = fmaxf(hi[1], y);
+        lo[2] = fminf(lo[2], z); hi[2] = fmaxf(hi[2], z);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            lo[d] = fminf(lo[d], __shfl_xor_sync(0xffffffffu, lo[d], o));
+            hi[d] = fmaxf(hi[d], __shfl_xor_sync(0xffffffffu, hi[d], o));
+        }
+    }
+    __shared__ float s_lo[8][3], s_hi[8][3];
+    __shared__ int s_bad;
+    if (threadIdx.x == 0) s_bad = 0;
+    __syncthreads();
+    int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (lane == 0) {
+        for (int d = 0; d < 3; ++d) { s_lo[warp][d] = lo[d]; s_hi[warp][d] = hi[d]; }
+    }
+    if (bad) s_bad = 1;
+    __syncthreads();
+    if (threadIdx.x < 3) {
+        int d = threadIdx.x;
+        float l = s_lo[0][d], h = s_hi[0][d];
+        for (int w = 1; w < 8; ++w) { l = fminf(l, s_lo[w][d]); h = fmaxf(h, s_hi[w][d]); }
+        atomicMin(&bbox_bits[d], float_to_ordered(l));
+        atomicMax(&bbox_bits[3 + d], float_to_ordered(h));
+    }
+    if (threadIdx.x == 0 && s_bad) atomicAdd(&counters[CNT_NONFINITE], 1ull);
+}
+
+p3t_status p3t_stage_pack(p3t_ctx *ctx, const float *d_mass, const float *d_pos)
+{
+    Workspace &w = ctx->ws;
+    u32 n = (u32)ctx->n;
+    P3T_CUDA(ctx, cudaMemsetAsync(w.counters, 0, CNT_WORDS * sizeof(u64), ctx->stream));
+    P3T_CUDA(ctx, cudaMemsetAsync(w.bbox_bits, 0xff, 3 * sizeof(u32), ctx->stream));
+    P3T_CUDA(ctx, cudaMemsetAsync(w.bbox_bits + 3, 0x00, 3 * sizeof(u32), ctx->stream));
+    u32 grid = min(div_up(n, 256 * 4), (u32)ctx->sm_count * 8);
+    pack_bbox_kernel<<<grid, 256, 0, ctx->stream>>>(d_mass, d_pos, w.body_user, w.bbox_bits, w.counters, n);
+    P3T_CUDA(ctx, cudaGetLastError());
+    return P3T_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// unpack: float4 (ax, ay, az, phi) user order -> acc[3n], pot[n]
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) unpack_kernel(const float4 *__restrict__ ap, float *acc, float *pot, u32 n)
+{
+    u32 i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    float4 v = ap[i];
+    if (acc) { acc[3 * (size_t)i] = v.x; acc[3 * (size_t)i + 1] = v.y; acc[3 * (size_t)i + 2] = v.z; }
+    if (pot) pot[i] = v.w;
+}
+
+p3t_status p3t_stage_unpack(p3t_ctx *ctx, float *d_acc, float *d_pot)
+{
+    u32 n = (u32)ctx->n;
+    if (!d_acc && !d_pot) return P3T_OK;
+    unpack_kernel<<<div_up(n, 256), 256, 0, ctx->stream>>>(ctx->ws.accpot, d_acc, d_pot, n);
+    P3T_CUDA(ctx, cudaGetLastError());
+    return P3T_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// a2: root cube + Morton keys + digit histograms of all passes
+// ------------------------------------------------------------------------------------------------
+// spread the low 21 bits of v so that bit k lands at bit 3k
+__device__ __forceinline__ u64 spread3(u32 v)
+{
+    u64 x = v & 0x1fffffu;
+    x = (x | x << 32) & 0x1f00000000ffffull;
+    x = (x | x << 16) & 0x1f0000ff0000ffull;
+    x = (x | x << 8) & 0x100f00f00f00f00full;
+    x = (x | x << 4) & 0x10c30c30c30c30c3ull;
+    x = (x | x << 2) & 0x1249249249249249ull;
+    return x;
+}
+
+// Root cube from the reduced min/max: centre = midpoint of the AABB, side = largest extent padded
+// so that the maximum maps inside.  Every thread recomputes it (6 loads), block 0 publishes it.
+__device__ __forceinline__ void root_cube(const u32 *bbox_bits, float &minx, float &miny, float &minz, float &side)
+{
+    float lo[3], hi[3];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) { lo[d] = ordered_to_float(bbox_bits[d]); hi[d] = ordered_to_float(bbox_bits[3 + d]); }
+    float ext = fmaxf(hi[0] - lo[0], fmaxf(hi[1] - lo[1], hi[2] - lo[2]));
+    side = ext * (1.f + 4e-6f);
+    if (!(side > 0.f) || !isfinite(side)) side = 1.f;
+    minx = 0.5f * (lo[0] + hi[0]) - 0.5f * side;
+    miny = 0.5f * (lo[1] + hi[1]) - 0.5f * side;
+    minz = 0.5f * (lo[2] + hi[2]) - 0.5f * side;
+}
+
+__global__ void __launch_bounds__(256) keys_hist_kernel(const float4 *__restrict__ body, const u32 *__restrict__ bbox_bits,
+                                                        float *cube, u64 *__restrict__ keys, u32 *__restrict__ idx,
+                                                        u32 *hist, u32 n, int max_level, int passes)
+{
+    __shared__ u32 s_hist[8 * 256];
+    for (int t = threadIdx.x; t < 8 * 256; t += blockDim.x) s_hist[t] = 0;
+    float minx, miny, minz, side;
+    root_cube(bbox_bits, minx, miny, minz, side);
+    if (blockIdx.x == 0 && threadIdx.x == 0) { cube[0] = minx; cube[1] = miny; cube[2] = minz; cube[3] = side; }
+    const float scale = (float)(1u << max_level) / side;
+    const u32 qmax = (1u << max_level) - 1u;
+    __syncthreads();
+    for (u32 i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        float4 b = body[i];
+        u32 qx = min((u32)fmaxf((b.x - minx) * scale, 0.f), qmax);
+        u32 qy = min((u32)fmaxf((b.y - miny) * scale, 0.f), qmax);
+        u32 qz = min((u32)fmaxf((b.z - minz) * scale, 0.f), qmax);
+        u64 key = (spread3(qx) << 2) | (spread3(qy) << 1) | spread3(qz);
+        keys[i] = key;
+        idx[i] = i;
+        for (int p = 0; p < passes; ++p) atomicAdd(&s_hist[p * 256 + (u32)((key >> (8 * p)) & 255u)], 1u);
+    }
+    __syncthreads();
+    for (int t = threadIdx.x; t < passes * 256; t += blockDim.x) {
+        u32 v = s_hist[t];
+        if (v) atomicAdd(&hist[t], v);
+    }
+}
+
+// exclusive scan of each pass's 256-bin histogram (one block per pass)
+__global__ void __launch_bounds__(256) hist_scan_kernel(u32 *hist)
+{
+    __shared__ u32 s_w[8];
+    u32 *h = hist + blockIdx.x * 256;
+    u32 v = h[threadIdx.x];
+    u32 lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    u32 inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        u32 t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t;
+    }
+    if (lane == 31) s_w[warp] = inc;
+    __syncthreads();
+    u32 base = 0;
+    for (u32 w = 0; w < warp; ++w) base += s_w[w];
+    h[threadIdx.x] = base + inc - v;
+}
+
+// ------------------------------------------------------------------------------------------------
+// a3: one onesweep pass: stable 8-bit digit partition with decoupled look-back over tiles
+// ------------------------------------------------------------------------------------------------
+#define OS_FLAG_AGG 0x40000000u
+#define OS_FLAG_INC 0x80000000u
+#define OS_VAL_MASK 0x3fffffffu
+
+__global__ void __launch_bounds__(SORT_THREADS) onesweep_kernel(const u64 *__restrict__ kin, const u32 *__restrict__ vin,
+                                                                u64 *__restrict__ kout, u32 *__restrict__ vout, u32 n,
+                                                                int shift, const u32 *__restrict__ gbase,
+                                                                volatile u32 *status, u64 *ticket)
+{
+    __shared__ u32 s_whist[SORT_THREADS / 32][256];
+    __shared__ u32 s_binstart[256];
+    __shared__ u32 s_goff[256];
+    __shared__ u32 s_wsum[8];
+    __shared__ u32 s_tile;
+    __shared__ u64 s_key[SORT_TILE];
+    __shared__ u32 s_val[SORT_TILE];
+
+    const u32 tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if (tid == 0) s_tile = (u32)atomicAdd(ticket, 1ull);
+    for (u32 t = tid; t < (SORT_THREADS / 32) * 256; t += SORT_THREADS) (&s_whist[0][0])[t] = 0;
+    __syncthreads();
+    const u32 tile = s_tile;
+    const u32 tile_base = tile * SORT_TILE;
+    const u32 tile_valid = min((u32)SORT_TILE, n - tile_base);
+
+    u64 key[SORT_ITEMS];
+    u32 val[SORT_ITEMS], rnk[SORT_ITEMS];
+    const u32 wbase = tile_base + warp * (SORT_ITEMS * 32);
+#pragma unroll
+    for (int k = 0; k < SORT_ITEMS; ++k) {
+        u32 i = wbase + k * 32 + lane;
+        bool ok = i < n;
+        key[k] = ok ? kin[i] : ~0ull;
+        val[k] = ok ? vin[i] : 0u;
+    }
+    // stable rank inside the warp: items in (k, lane) order
+#pragma unroll
+    for (int k = 0; k < SORT_ITEMS; ++k) {
+        u32 i = wbase + k * 32 + lane;
+        bool ok = i < n;
+        u32 active = __ballot_sync(0xffffffffu, ok);
+        rnk[k] = 0;
+        if (ok) {
+            u32 d = (u32)(key[k] >> shift) & 255u;
+            u32 peers = __match_any_sync(active, d);
+            int leader = __ffs(peers) - 1;
+            u32 pre = 0;
+            if ((int)lane == leader) {
+                pre = s_whist[warp][d];
+                s_whist[warp][d] = pre + __popc(peers);
+            }
+            pre = __shfl_sync(peers, pre, leader);
+            rnk[k] = pre + __popc(peers & lanemask_lt());
+        }
+        __syncwarp();
+    }
+    __syncthreads();
+    // bin = tid: exclusive over warps, tile total
+    u32 sum = 0;
+#pragma unroll
+    for (int w = 0; w < SORT_THREADS / 32; ++w) {
+        u32 t = s_whist[w][tid];
+        s_whist[w][tid] = sum;
+        sum += t;
+    }
+    volatile u32 *my_status = status + (size_t)tile * 256 + tid;
+    *my_status = sum | (tile == 0 ? OS_FLAG_INC : OS_FLAG_AGG);
+    // exclusive scan of the 256 bin totals inside the block
+    u32 inc = sum;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        u32 t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t;
+    }
+    if (lane == 31) s_wsum[warp] = inc;
+    __syncthreads();
+    u32 wb = 0;
+    for (u32 w = 0; w < warp; ++w) wb += s_wsum[w];
+    u32 binstart = wb + inc - sum;
+    s_binstart[tid] = binstart;
+    // decoupled look-back
+    u32 excl = 0;
+    if (tile > 0) {
+        int t = (int)tile - 1;
+        while (true) {
+            u32 v = status[(size_t)t * 256 + tid];
+            if ((v & (OS_FLAG_AGG | OS_FLAG_INC)) == 0) continue;
+            excl += v & OS_VAL_MASK;
+            if (v & OS_FLAG_INC) break;
+            --t;
+        }
+        *my_status = (excl + sum) | OS_FLAG_INC;
+    }
+    s_goff[tid] = gbase[tid] + excl - binstart;
+    __syncthreads();
+    // scatter into shared memory in sorted order
+#pragma unroll
+    for (int k = 0; k < SORT_ITEMS; ++k) {
+        u32 i = wbase + k * 32 + lane;
+        if (i < n) {
+            u32 d = (u32)(key[k] >> shift) & 255u;
+            u32 p = s_binstart[d] + s_whist[warp][d] + rnk[k];
+            s_key[p] = key[k];
+            s_val[p] = val[k];
+        }
+    }
+    __syncthreads();
+    for (u32 p = tid; p < tile_valid; p += SORT_THREADS) {
+        u64 kk = s_key[p];
+        u32 d = (u32)(kk >> shift) & 255u;
+        u32 dst = s_goff[d] + p;
+        kout[dst] = kk;
+        vout[dst] = s_val[p];
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// a4: gather bodies into sorted order; common-prefix level between sorted neighbours
+// ------------------------------------------------------------------------------------------------
+// clev[i] = number of leading octree levels on which key[i-1] and key[i] agree (0..max_level);
+// clev[0] = clev[n] = -1.
+__global__ void __launch_bounds__(256) gather_kernel(const float4 *__restrict__ body_user, const u32 *__restrict__ idx,
+                                                     const u64 *__restrict__ keys, float4 *__restrict__ body,
+                                                     signed char *__restrict__ clev, u32 n, int max_level)
+{
+    u32 i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i > n) return;
+    if (i == n) { clev[n] = -1; return; }
+    body[i] = body_user[idx[i]];
+    int c = -1;
+    if (i > 0) {
+        u64 x = keys[i] ^ keys[i - 1];
+        if (x == 0) c = max_level;
+        else {
+            int hb = 63 - __clzll((long long)x);
+            c = max_level - hb / 3 - 1;
+        }
+    }
+    clev[i] = (signed char)c;
+}
+
+p3t_status p3t_stage_sort(p3t_ctx *ctx)
+{
+    Workspace &w = ctx->ws;
+    u32 n = (u32)ctx->n;
+    cudaStream_t s = ctx->stream;
+    int passes = (3 * ctx->max_level + 7) / 8;   // 8 for 63-bit keys, 4 for 30-bit keys
+    u32 ntiles = div_up(n, SORT_TILE);
+    P3T_CUDA(ctx, cudaMemsetAsync(w.counters + CNT_NCELLS, 0, 16 * sizeof(u64), s));   // build counters + sort tickets
+    P3T_CUDA(ctx, cudaMemsetAsync(w.hist, 0, 8 * 256 * sizeof(u32), s));
+    P3T_CUDA(ctx, cudaMemsetAsync(w.tile_status, 0, (size_t)passes * ntiles * 256 * sizeof(u32), s));
+    u32 grid = min(div_up(n, 256 * 4), (u32)ctx->sm_count * 8);
+    keys_hist_kernel<<<grid, 256, 0, s>>>(w.body_user, w.bbox_bits, w.cube, w.keys[0], w.idx[0], w.hist, n,
+                                          ctx->max_level, passes);
+    hist_scan_kernel<<<passes, 256, 0, s>>>(w.hist);
+    int cur = 0;
+    for (int p = 0; p < passes; ++p) {
+        onesweep_kernel<<<ntiles, SORT_THREADS, 0, s>>>(w.keys[cur], w.idx[cur], w.keys[cur ^ 1], w.idx[cur ^ 1], n, 8 * p,
+                                                        w.hist + p * 256, w.tile_status + (size_t)p * ntiles * 256,
+                                                        w.counters + CNT_SORT_TICKET + p);
+        cur ^= 1;
+    }
+    ctx->cur = cur;
+    gather_kernel<<<div_up(n + 1, 256), 256, 0, s>>>(w.body_user, w.idx[cur], w.keys[cur], w.body, w.clev, n, ctx->max_level);
+    P3T_CUDA(ctx, cudaGetLastError());
+    return P3T_OK;
+}
