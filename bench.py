@@ -1,0 +1,298 @@
+#!/usr/bin/env python
+"""bench.py -- soft-force throughput of the B200 path (and of the CPU oracle beside it).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--impl ours|reference]
+
+One "step" = one pass of the whole hot path (rows a1-a9 of DESIGN.md section 2) over one batch of
+synthetic input: load -> bounding cube, Morton keys, radix sort, gather -> octree + groups ->
+moments -> group walk + interactions -> neighbour CSR.  The default workload is BASELINE.json
+configs[2] (the N = 1,048,576 Salpeter-mass Plummer sphere the metric is quoted on).
+
+Timing: every step is bracketed by CUDA events on the stream the library launches on; between
+steps the L2 is flushed by writing a 512 MiB buffer (the 16 MB input is far smaller than the 126 MB
+L2); ms_per_step is the mean over the K timed steps; with N > 1 ranks each rank evaluates its own
+independent cluster (weak scaling, no data-path collective) and the slowest rank's time is used.
+Prints ONE JSON line on rank 0.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+FLOP_PP, FLOP_PC = 23, 65            # flops-per-interaction convention
+N_SM_NOMINAL, FP32_LANES = 148, 128
+METRIC = "soft-force particles/s (tree build + walk + neighbour lists, fp32)"
+CLOCK_QUERY = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+               "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+               "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return dict(hbm_gbs=d["hbm_gbs"], sm_max_mhz=d.get("sm_max_mhz", 1965.0), source="measured")
+    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
+
+
+def algorithmic_bytes_tree(n, key_bits, n_cells, n_groups):
+    """a1-a6 bytes the method must move (every array once per pass that reads or writes it)."""
+    passes = 8 if key_bits == 63 else 4
+    pack = 16 * n + 16 * n                        # a1: read mass+pos, write float4 bodies
+    keys = 16 * n + 12 * n                        # a2: read bodies, write u64 key + u32 idx
+    sort = passes * 2 * 12 * n                    # a3: each pass reads and writes (key, idx)
+    gather = 4 * n + 16 * n + 16 * n + 8 * n      # a4: idx, body in, body out, keys (common-prefix levels)
+    build = 4 * n + 32 * n_cells + 4 * n_groups   # a5: level/flag bytes per body, cell topology, group starts
+    moments = 16 * n + 88 * n_cells + 88 * n_cells  # a6: read bodies; write cells; parents re-read their children
+    return dict(sort=pack + keys + sort + gather, build=build, moments=moments)
+
+
+class ClockSampler:
+    def __init__(self, index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--query-gpu={CLOCK_QUERY}", "--format=csv,noheader,nounits",
+                                       "-lms", "100", "-i", str(index)], stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        out = dict(sm_mhz=None, sm_max_mhz=None, reasons=[], samples=0)
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        rows = [r.split(",") for r in open(self.f.name).read().strip().splitlines() if r.count(",") >= 8]
+        os.unlink(self.f.name)
+        if not rows:
+            return out
+        sm = sorted(float(r[1]) for r in rows)
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [nm for k, nm in enumerate(names) if any("Active" == r[5 + k].strip() for r in rows)]
+        power = max(float(r[3]) for r in rows)
+        return dict(sm_mhz=sm[len(sm) // 2], sm_max_mhz=float(rows[0][2]), reasons=reasons, samples=len(rows), power_w_max=power)
+
+
+def time_oracle(cfg, budget_particles):
+    """The CPU oracle as it stands (O4: fp64 Barnes-Hut, same theta and acceptance rule), on a bounded sample."""
+    from oracle import p3t_oracle as O
+
+    m, q = cfg["mass"].astype(np.float64), cfg["pos"].astype(np.float64)
+    n = cfg["n"]
+    t0 = time.perf_counter()
+    tree = O.Tree(m, q, nleaf=cfg["nleaf"], max_depth=21 if cfg["key_bits"] == 63 else 10)
+    t_build = time.perf_counter() - t0
+    ns = min(n, budget_particles)
+    sub = np.sort(np.random.default_rng(7).choice(n, ns, replace=False)).astype(np.int64)
+    t0 = time.perf_counter()
+    r = tree.walk(cfg["eps"], cfg["theta"], cfg["r_in"], cfg["r_out"], cfg["r_search"], subset=sub)
+    t_walk = time.perf_counter() - t0
+    t_full = t_build + t_walk * n / ns
+    return dict(value=n / t_full, unit="particles/s", cores=O.num_threads(), kind="oracle",
+                sample=f"O4 fp64 CPU Barnes-Hut (gcc -O2 -fopenmp): tree build over all {n} bodies ({t_build:.2f} s) + walk of "
+                       f"{ns} seeded random targets ({t_walk:.2f} s), walk time scaled by N/{ns}",
+                interactions_per_s=float((r["n_pp"].sum() + r["n_pc"].sum()) / t_walk)), t_build + t_walk
+
+
+def run_reference(args):
+    """--impl reference: the oracle timed on the host cores; rank 0 only."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    from paper_1506_04553_b200 import workloads
+
+    cfg = workloads.config(args.config)
+    times, last = [], None
+    for it in range(args.warmup + args.steps):
+        last, dt = time_oracle(cfg, args.ref_sample)
+        if it >= args.warmup:
+            times.append(cfg["n"] / last["value"])
+    t = float(np.mean(times))
+    value = cfg["n"] / t
+    cb = dict(last); cb["value"] = value
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": "particles/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": cfg["name"], "n": cfg["n"], "theta": cfg["theta"], "note": "each step = one bounded sample, extrapolated to N"},
+        "cpu_baseline": cb,
+        "e2e": {"value": value, "unit": "particles/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--ref-sample", type=int, default=131072, help="targets walked by the oracle per step")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--nleaf", type=int, default=None)
+    ap.add_argument("--ngroup", type=int, default=None)
+    ap.add_argument("--merge", type=int, default=None)
+    ap.add_argument("--n", type=int, default=None, help="override the particle count (not a bench value)")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    args.warmup = max(args.warmup, 3)
+
+    import torch
+
+    from paper_1506_04553_b200 import binding, workloads
+
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the soft-force path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+
+    cfg = workloads.config(args.config, n=args.n)
+    if world > 1 and rank > 0:      # independent cluster per rank: same recipe, another seed
+        from paper_1506_04553_b200.workloads import plummer, salpeter_masses
+        pos, _ = plummer(cfg["n"], workloads.SEED_BASE + args.config + 100 * rank)
+        cfg["pos"] = np.ascontiguousarray((pos - pos.mean(axis=0)).astype(np.float32))
+    n = cfg["n"]
+    nleaf, ngroup = args.nleaf or cfg["nleaf"], args.ngroup or cfg["ngroup"]
+    dev = f"cuda:{local}"
+    mass_d = torch.from_numpy(cfg["mass"]).to(dev)
+    pos_d = torch.from_numpy(cfg["pos"]).to(dev)
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)
+
+    ctx = binding.P3T(n, key_bits=cfg["key_bits"], nbr_capacity=max(n, 1 << 16), device=local)
+    ctx.set_params(cfg["eps"], cfg["theta"], cfg["r_in"], cfg["r_out"], cfg["r_search"])
+    ctx.set_tree_params(nleaf, ngroup)
+    if args.merge is not None:
+        ctx.set_group_merge_levels(args.merge)
+
+    def step():
+        ctx.load_particles(mass_d, pos_d)
+        ctx.build_tree()
+        ctx.eval_soft()
+
+    for _ in range(args.warmup):
+        flush.zero_()
+        step()
+    ctx.synchronize()
+    if dist:
+        dist.barrier()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local) if rank == 0 else None
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    phases = {k: [] for k in ("ms_sort", "ms_build", "ms_moments", "ms_walk", "ms_nbr")}
+    for a, b in ev:
+        flush.zero_()
+        a.record()
+        step()
+        b.record()
+        st = ctx.get_stats()           # synchronises; per-phase times come from the library's own CUDA events
+        for k in phases:
+            phases[k].append(st[k])
+    torch.cuda.synchronize()
+    if dist:
+        dist.barrier()
+    clocks = sampler.stop() if sampler else None
+    ms = float(np.mean([a.elapsed_time(b) for a, b in ev]))
+    if dist:
+        t = torch.tensor([ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    st = ctx.get_stats()
+    ph = {k: float(np.mean(v)) for k, v in phases.items()}
+
+    # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        mass_h = torch.from_numpy(cfg["mass"]).pin_memory().numpy()
+        pos_h = torch.from_numpy(cfg["pos"]).pin_memory().numpy()
+        acc_h = torch.empty((n, 3), dtype=torch.float32).pin_memory().numpy()
+        pot_h = torch.empty(n, dtype=torch.float32).pin_memory().numpy()
+        ts, d2h = [], 0
+        for it in range(2 + min(args.steps, 5)):
+            flush.zero_()
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            ctx.load_particles(mass_h, pos_h)
+            ctx.build_tree()
+            ctx.eval_soft()
+            ctx.get_acc_pot_into(acc_h, pot_h)
+            off, nbr = ctx.get_neighbours()
+            dt = time.perf_counter() - t0
+            d2h = acc_h.nbytes + pot_h.nbytes + off.nbytes + nbr.nbytes
+            if it >= 2:
+                ts.append(dt)
+        te = float(np.mean(ts))
+        if dist:
+            t = torch.tensor([te], device=dev, dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            te = float(t.item())
+        e2e = {"value": world * n / te, "unit": "particles/s", "h2d_bytes_per_step": int(mass_h.nbytes + pos_h.nbytes),
+               "d2h_bytes_per_step": int(d2h), "ms_per_step": 1e3 * te}
+
+    if rank != 0:
+        if dist:
+            dist.destroy_process_group()
+        return
+
+    peaks = measured_peaks()
+    n_sm = torch.cuda.get_device_properties(local).multi_processor_count
+    fp32_peak = 2 * FP32_LANES * n_sm * peaks["sm_max_mhz"] * 1e6 / 1e12          # TFLOP/s at the max SM clock
+    flops = FLOP_PP * st["n_pp"] + FLOP_PC * st["n_pc"]
+    walk_tflops = flops / (ph["ms_walk"] * 1e-3) / 1e12
+    ab = algorithmic_bytes_tree(n, cfg["key_bits"], st["n_cells"], st["n_groups"])
+    hbm = {k: ab[k] / (ph["ms_" + k] * 1e-3) / 1e9 for k in ab}
+    tree_ms = ph["ms_sort"] + ph["ms_build"] + ph["ms_moments"]
+    launches = 1 + (2 + st["sort_passes"] + 1) + 4 + 1 + 1 + 5
+
+    out = {
+        "metric": METRIC, "value": world * n / (ms * 1e-3), "unit": "particles/s", "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": cfg["name"], "n": n, "theta": cfg["theta"], "eps": cfg["eps"], "r_out": cfg["r_out"],
+                   "r_search": cfg["r_search"], "key_bits": cfg["key_bits"], "nleaf": nleaf, "ngroup": ngroup,
+                   "l2": "flushed between steps (512 MiB write)", "parallelism": f"{world} independent cluster(s), one per GPU"},
+        "interactions_per_s": (st["n_pp"] + st["n_pc"]) / (ph["ms_walk"] * 1e-3),
+        "walk_particles_per_s": n / (ph["ms_walk"] * 1e-3),
+        "interactions": {"n_pp": st["n_pp"], "n_pc": st["n_pc"], "n_near": st["n_near"], "n_neighbours": st["n_neighbours"],
+                         "pp_per_particle": st["n_pp"] / n, "pc_per_particle": st["n_pc"] / n},
+        "tree": {"n_cells": st["n_cells"], "n_leaves": st["n_leaves"], "n_groups": st["n_groups"], "depth": st["depth"]},
+        "phases_ms": ph,
+        "roofline": {"bound": "alu", "kernel": "walk_kernel (a7+a8)", "achieved": walk_tflops, "peak": fp32_peak, "unit": "TFLOP/s",
+                     "frac": walk_tflops / fp32_peak, "traffic": None,
+                     "peak_source": f"2 flop x {FP32_LANES} lanes x {n_sm} SMs x {peaks['sm_max_mhz']:.0f} MHz ({peaks['source']} sm_max_mhz; DESIGN.md section 8)",
+                     "convention": f"{FLOP_PP} flop per p-p, {FLOP_PC} flop per p-c"},
+        "roofline_hbm": {"bound": "hbm", "passes": "a1-a6 (sort, build, moments)", "achieved": sum(ab.values()) / (tree_ms * 1e-3) / 1e9,
+                         "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": sum(ab.values()) / (tree_ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                         "per_pass_gbs": hbm, "algorithmic_bytes": ab, "peak_source": peaks["source"]},
+        "clocks": clocks, "gpu_launches": launches * args.steps, "gpu_launches_per_step": launches,
+    }
+    if e2e:
+        out["e2e"] = e2e
+    if not args.no_cpu_baseline and world == 1:
+        out["cpu_baseline"], _ = time_oracle(cfg, args.ref_sample)
+    print(json.dumps(out))
+    if dist:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,173 @@
+"""Boundary behaviour of the C ABI on the GPU: error codes, call order, capacity, edge sizes, device I/O."""
+import numpy as np
+import pytest
+
+from paper_1506_04553_b200 import workloads
+from p3t_parity_helpers import assert_same_neighbour_sets, csr_sets, rel_err, widen
+
+pytestmark = pytest.mark.gpu
+
+
+def _binding():
+    from paper_1506_04553_b200 import binding
+
+    return binding
+
+
+def test_call_order_and_argument_errors():
+    b = _binding()
+    cfg = workloads.config(1, n=512)
+    with b.P3T(512, key_bits=30) as ctx:
+        for call in (ctx.build_tree, ctx.eval_soft, ctx.get_acc_pot, ctx.get_neighbours):
+            with pytest.raises(b.P3TError) as e:
+                call()
+            assert e.value.status == b.ESTATE
+        ctx.load_particles(cfg["mass"], cfg["pos"])
+        with pytest.raises(b.P3TError) as e:
+            ctx.build_tree()                                    # parameters not set
+        assert e.value.status == b.ESTATE
+        for bad in [(-1.0, 0.5, 0.001, 0.01, 0.012), (1e-3, -0.1, 0.001, 0.01, 0.012), (1e-3, 0.5, 0.01, 0.01, 0.012),
+                    (1e-3, 0.5, 0.001, 0.01, 0.009), (1e-3, 0.5, -0.001, 0.01, 0.012), (float("nan"), 0.5, 0.001, 0.01, 0.012)]:
+            with pytest.raises(b.P3TError) as e:
+                ctx.set_params(*bad)
+            assert e.value.status == b.EINVAL
+        with pytest.raises(b.P3TError):
+            ctx.set_tree_params(0, 64)
+        with pytest.raises(b.P3TError):
+            ctx.set_tree_params(16, 48)
+        ctx.set_params(cfg["eps"], 0.5, cfg["r_in"], cfg["r_out"], cfg["r_search"])
+        ctx.build_tree()
+        ctx.eval_soft()
+        ctx.get_acc_pot()
+        ctx.set_params(cfg["eps"], 0.6, cfg["r_in"], cfg["r_out"], cfg["r_search"])   # invalidates the tree
+        with pytest.raises(b.P3TError) as e:
+            ctx.eval_soft()
+        assert e.value.status == b.ESTATE
+        big = workloads.config(1, n=513)
+        with pytest.raises(b.P3TError) as e:
+            ctx.load_particles(big["mass"], big["pos"])         # n > max_n
+        assert e.value.status == b.EINVAL
+        bad = cfg["pos"].copy(); bad[7, 1] = np.inf
+        with pytest.raises(b.P3TError) as e:
+            ctx.load_particles(cfg["mass"], bad)
+        assert e.value.status == b.EINVAL
+    with pytest.raises(b.P3TError):
+        b.P3T(512, key_bits=31)
+
+
+def test_nonfinite_device_input_is_reported():
+    import torch
+
+    b = _binding()
+    cfg = workloads.config(1, n=512)
+    pos = torch.from_numpy(cfg["pos"]).cuda()
+    pos[3, 2] = float("nan")
+    with b.P3T(512, key_bits=63) as ctx:
+        ctx.set_params(cfg["eps"], 0.5, cfg["r_in"], cfg["r_out"], cfg["r_search"])
+        ctx.load_particles(torch.from_numpy(cfg["mass"]).cuda(), pos)
+        with pytest.raises(b.P3TError) as e:
+            ctx.synchronize()
+        assert e.value.status == b.EINVAL
+
+
+def test_neighbour_capacity_error_reports_total(oracle):
+    b = _binding()
+    cfg = workloads.config(1, n=2048)
+    r_in, r_out, h = 0.01, 0.1, 0.12
+    m, q = widen(cfg)
+    ooff, olst, band = oracle.neighbours(q, cfg["eps"], h)
+    want = int(ooff[-1])
+    assert want > 1000 and len(band) == 0
+    with b.P3T(2048, key_bits=63, nbr_capacity=100) as ctx:
+        ctx.set_params(cfg["eps"], 0.5, r_in, r_out, h)
+        ctx.soft_force(cfg["mass"], cfg["pos"])
+        with pytest.raises(b.P3TError) as e:
+            ctx.get_neighbours()
+        assert e.value.status == b.ECAPACITY
+        count, total = ctx.get_neighbour_counts()
+        assert total == want and np.array_equal(count.astype(np.int64), np.diff(ooff))
+        acc, pot = ctx.get_acc_pot()                            # forces are unaffected
+        a, p = oracle.direct(m, q, cfg["eps"], r_in, r_out)
+        assert np.median(rel_err(acc.astype(np.float64), a)) < 1e-3
+    with b.P3T(2048, key_bits=63, nbr_capacity=want) as ctx:    # retry with the reported total
+        ctx.set_params(cfg["eps"], 0.5, r_in, r_out, h)
+        ctx.soft_force(cfg["mass"], cfg["pos"])
+        off, nbr = ctx.get_neighbours()
+        assert_same_neighbour_sets(csr_sets(off, nbr), csr_sets(ooff, olst), band)
+        with pytest.raises(b.P3TError) as e:
+            ctx.get_neighbours(capacity=want - 1)               # caller's buffer too small
+        assert e.value.status == b.ECAPACITY
+
+
+@pytest.mark.parametrize("n", [1, 2, 3, 31, 32, 33, 63, 64, 65, 257, 2049])
+@pytest.mark.parametrize("theta", [0.0, 0.7])
+def test_small_and_ragged_sizes(oracle, n, theta):
+    b = _binding()
+    cfg = workloads.config(1, n=max(n, 8))
+    mass, pos = cfg["mass"][:n].copy(), np.ascontiguousarray(cfg["pos"][:n])
+    r_in, r_out, h = 0.02, 0.2, 0.25
+    with b.P3T(max(n, 1), key_bits=63) as ctx:
+        ctx.set_params(1e-3, theta, r_in, r_out, h)
+        ctx.soft_force(mass, pos)
+        acc, pot = ctx.get_acc_pot()
+        off, nbr = ctx.get_neighbours()
+    if n == 1:
+        assert not acc.any() and pot[0] == 0.0 and off.tolist() == [0, 0]
+        return
+    a, p = oracle.direct(mass.astype(np.float64), pos.astype(np.float64), np.float32(1e-3), np.float32(r_in), np.float32(r_out))
+    scale = np.abs(a).max()
+    tol = 1e-5 if theta == 0.0 else 2e-2
+    assert np.max(np.linalg.norm(acc - a, axis=1)) <= tol * scale
+    ooff, olst, band = oracle.neighbours(pos.astype(np.float64), np.float32(1e-3), np.float32(h))
+    assert_same_neighbour_sets(csr_sets(off, nbr), csr_sets(ooff, olst), band)
+
+
+def test_device_pointers_in_and_out(oracle):
+    import torch
+
+    b = _binding()
+    cfg = workloads.config(1, n=3000)
+    with b.P3T(3000, key_bits=63) as ctx:
+        ctx.set_params(cfg["eps"], cfg["theta"], cfg["r_in"], cfg["r_out"], cfg["r_search"])
+        ctx.soft_force(cfg["mass"], cfg["pos"])
+        acc_h, pot_h = ctx.get_acc_pot()
+        ctx.soft_force(torch.from_numpy(cfg["mass"]).cuda(), torch.from_numpy(cfg["pos"]).cuda())
+        acc_d, pot_d = ctx.get_acc_pot(on_device=True)
+        torch.cuda.synchronize()
+        assert np.array_equal(acc_d.cpu().numpy(), acc_h) and np.array_equal(pot_d.cpu().numpy(), pot_h)
+
+
+def test_results_are_deterministic_and_context_reusable():
+    b = _binding()
+    c1, c2 = workloads.config(1, n=4096), workloads.config(3, n=3000)
+    with b.P3T(4096, key_bits=63) as ctx:
+        outs = []
+        for cfg in (c1, c2, c1):
+            ctx.set_params(cfg["eps"], cfg["theta"], cfg["r_in"], 10 * cfg["r_out"], 12 * cfg["r_out"])
+            ctx.soft_force(cfg["mass"], cfg["pos"])
+            outs.append((ctx.get_acc_pot(), ctx.get_neighbours()))
+        (a0, p0), (o0, n0) = outs[0]
+        (a2, p2), (o2, n2) = outs[2]
+        assert np.array_equal(a0, a2) and np.array_equal(p0, p2) and np.array_equal(o0, o2) and np.array_equal(n0, n2)
+
+
+def test_all_bodies_at_one_point_and_massless_bodies(oracle):
+    b = _binding()
+    n = 100
+    mass = np.full(n, 1.0 / n, dtype=np.float32)
+    pos = np.zeros((n, 3), dtype=np.float32) + np.float32(0.25)
+    with b.P3T(n, key_bits=63) as ctx:
+        ctx.set_params(1e-2, 0.5, 0.001, 0.005, 0.005)          # r_out < eps: plain softened Newton
+        ctx.soft_force(mass, pos)
+        acc, pot = ctx.get_acc_pot()
+        assert not acc.any()
+        np.testing.assert_allclose(pot, -(n - 1) / n / np.float32(1e-2), rtol=1e-6)
+        assert ctx.get_neighbour_counts()[1] == 0
+    cfg = workloads.config(1, n=1000)
+    mass = cfg["mass"].copy(); mass[::3] = 0.0
+    with b.P3T(1000, key_bits=30) as ctx:
+        ctx.set_params(cfg["eps"], 0.5, cfg["r_in"], cfg["r_out"], cfg["r_search"])
+        ctx.soft_force(mass, cfg["pos"])
+        acc, pot = ctx.get_acc_pot()
+        a, p = oracle.direct(mass.astype(np.float64), cfg["pos"].astype(np.float64), cfg["eps"], cfg["r_in"], cfg["r_out"])
+        assert np.median(rel_err(acc.astype(np.float64), a)) < 1e-3

@@ -1,0 +1,127 @@
+"""GPU parity for rows a1-a6 (bounding cube, Morton keys, radix sort, gather, octree, moments).
+
+Integer / index work is compared bit-exactly with oracle/keytree.py; moments within fp32 tolerances
+of the fp64 recomputation from the body ranges.  Everything goes through the C ABI.
+"""
+import numpy as np
+import pytest
+
+from paper_1506_04553_b200 import workloads
+
+pytestmark = pytest.mark.gpu
+
+LEAF = 0x80000000
+
+
+def _build(cfg, key_bits=None, nleaf=16, ngroup=64, theta=None):
+    from paper_1506_04553_b200 import binding
+
+    kb = key_bits or cfg["key_bits"]
+    ctx = binding.P3T(cfg["n"], key_bits=kb)
+    ctx.set_params(cfg["eps"], cfg["theta"] if theta is None else theta, cfg["r_in"], cfg["r_out"], cfg["r_search"])
+    ctx.set_tree_params(nleaf, ngroup)
+    ctx.load_particles(cfg["mass"], cfg["pos"])
+    ctx.build_tree()
+    ctx.synchronize()
+    return ctx, (21 if kb == 63 else 10)
+
+
+CASES = [  # (config, n, key_bits, nleaf, ngroup)
+    (1, 4096, 30, 16, 64), (1, 4096, 63, 16, 32), (1, 5000, 63, 8, 64), (3, 20011, 63, 16, 64),
+    (4, 30000, 63, 16, 64), (1, 100, 30, 1, 32), (1, 7, 63, 16, 64),
+]
+
+
+@pytest.mark.parametrize("k,n,kb,nleaf,ngroup", CASES)
+def test_keys_sort_octree_match_keytree_oracle(k, n, kb, nleaf, ngroup):
+    from oracle import keytree
+
+    cfg = workloads.config(k, n=n)
+    ctx, max_level = _build(cfg, kb, nleaf, ngroup)
+    cube = ctx.array("root_cube")
+    # a1: the cube is the oracle's definition (centre = AABB midpoint, side = largest extent), padded
+    cmin, side = keytree.root_cube(cfg["pos"])
+    assert side <= cube[3] <= side * (1 + 1e-5)
+    np.testing.assert_allclose(cube[:3] + 0.5 * cube[3], cmin + 0.5 * side, atol=2e-6 * side)
+    assert np.all(cfg["pos"] >= cube[:3]) and np.all(cfg["pos"] < cube[:3] + cube[3])
+    # a2-a3: keys bit-exact, sorted; a4: permutation and gathered bodies
+    keys = ctx.array("keys")
+    idx = ctx.array("sorted_idx")
+    ref = keytree.morton_keys(cfg["pos"], cube[:3], cube[3], max_level)
+    assert np.array_equal(np.sort(idx), np.arange(n, dtype=np.uint32))
+    assert np.array_equal(keys, ref[idx])
+    assert np.all(keys[1:] >= keys[:-1])
+    order = np.argsort(ref, kind="stable")                     # LSD radix sort is stable
+    assert np.array_equal(idx, order.astype(np.uint32))
+    bodies = ctx.array("bodies")
+    assert np.array_equal(bodies[:, :3], cfg["pos"][idx]) and np.array_equal(bodies[:, 3], cfg["mass"][idx])
+    # a5: cells identical to the recursive construction, in the same numbering
+    cells = keytree.build_cells(keys, nleaf, max_level)
+    st = ctx.get_stats()
+    assert st["n_cells"] == len(cells)
+    assert st["n_leaves"] == sum(c["leaf"] for c in cells)
+    assert st["depth"] == max(c["level"] for c in cells)
+    level, start, parent, meta = ctx.array("cell_level"), ctx.array("cell_start"), ctx.array("cell_parent"), ctx.array("cell_meta")
+    assert np.array_equal(level, np.array([c["level"] for c in cells], dtype=np.uint8))
+    assert np.array_equal(start, np.array([c["start"] for c in cells], dtype=np.uint32))
+    assert np.array_equal(parent.astype(np.int64), np.array([c["parent"] if c["parent"] >= 0 else 0xffffffff for c in cells]))
+    for i, c in enumerate(cells):
+        if c["leaf"]:
+            assert meta[i, 0] == c["start"] and meta[i, 1] == (c["count"] | LEAF)
+        else:
+            assert meta[i, 0] == c["children"][0] and meta[i, 1] == len(c["children"])
+    # groups: a partition of the sorted bodies into runs of <= ngroup
+    gs = ctx.array("group_start").astype(np.int64)
+    assert st["n_groups"] == len(gs) - 1
+    assert gs[0] == 0 and gs[-1] == n and np.all(np.diff(gs) >= 1) and np.all(np.diff(gs) <= ngroup)
+    ctx.close()
+
+
+@pytest.mark.parametrize("k,n,kb", [(1, 4096, 30), (3, 20011, 63), (4, 30000, 63)])
+def test_moments_match_fp64_recomputation(k, n, kb):
+    from oracle import keytree
+
+    cfg = workloads.config(k, n=n)
+    ctx, max_level = _build(cfg, kb)
+    keys, bodies, cube = ctx.array("keys"), ctx.array("bodies"), ctx.array("root_cube")
+    cells = keytree.build_cells(keys, 16, max_level)
+    mac, m0, m1 = ctx.array("cell_mac"), ctx.array("cell_mom0"), ctx.array("cell_mom1")
+    bmin, bmax = ctx.array("cell_bmin"), ctx.array("cell_bmax")
+    theta, h = cfg["theta"], cfg["r_search"]
+    rng = np.random.default_rng(1)
+    pick = np.unique(np.concatenate([np.arange(min(64, len(cells))), rng.integers(0, len(cells), 1500)]))
+    for i in pick:
+        c = cells[i]
+        M, com, Q, lo, hi = keytree.moments(bodies, c["start"], c["count"])
+        ext = max(float((hi - lo).max()), 1e-30)
+        assert abs(m0[i, 0] - M) <= 2e-6 * M
+        np.testing.assert_allclose(mac[i, :3], com, atol=3e-6 * ext + 2e-7 * np.abs(com).max())
+        qscale = M * ext * ext
+        np.testing.assert_allclose(np.concatenate([m0[i, 1:], m1[i, :3]]), Q, atol=2e-5 * qscale + 1e-30)
+        assert np.array_equal(bmin[i, :3], lo.astype(np.float32)) and np.array_equal(bmax[i, :3], hi.astype(np.float32))
+        # acceptance radius: never below either clause of R-MAC (A9, A10)
+        g, l = keytree.cell_geometry(c, keys[c["start"]], cube[:3], cube[3], max_level)
+        delta = np.linalg.norm(com - g)
+        rmax = np.linalg.norm(bodies[c["start"]:c["start"] + c["count"], :3].astype(np.float64) - com, axis=1).max()
+        rc = np.sqrt(float(mac[i, 3]))
+        assert rc >= (l / theta + delta) * (1 - 1e-5)
+        assert rc >= h + rmax
+        assert rc <= max(l / theta + delta, h + 1.7321 * ext + 1e-30) * (1 + 1e-3) + 1e-4 * cube[3]
+    # root: total mass and centre of mass of everything
+    np.testing.assert_allclose(m0[0, 0], cfg["mass"].astype(np.float64).sum(), rtol=2e-6)
+    ctx.close()
+
+
+def test_coincident_points_make_a_deep_leaf():
+    from oracle import keytree
+
+    cfg = workloads.config(1, n=2000)
+    cfg["pos"][100:160] = cfg["pos"][100]                       # 60 bodies at one point
+    ctx, max_level = _build(cfg, 63)
+    keys = ctx.array("keys")
+    cells = keytree.build_cells(keys, 16, max_level)
+    meta, level = ctx.array("cell_meta"), ctx.array("cell_level")
+    assert ctx.get_stats()["n_cells"] == len(cells)
+    big = [(int(meta[i, 1]) & 0x7fffffff, int(level[i])) for i in range(len(cells)) if int(meta[i, 1]) & LEAF and (int(meta[i, 1]) & 0x7fffffff) > 16]
+    assert big == [(60, 21)]
+    ctx.close()
