@@ -15,29 +15,71 @@
 
 struct WarpShared {
     u32 stack[WALK_STACK_SMEM];
-    float4 far_buf[64];
+    // far ring: every entry is stored with its components duplicated, {x,x,y,y} and {z,z,m,m}, so
+    // that one LDS.128 yields two aligned register pairs for the packed fp32x2 pipe (no MOVs)
+    float4 far_xy[64], far_zm[64];
     float4 near_buf[64];
     u32 near_idx[64];
     u32 pc_idx[64];
-    float4 pc_a[32], pc_b[32], pc_c[32];
+    float4 pc[6][32];   // staged cells of one batch, duplicated pairs (see stage_pc)
 };
 
+// ---- arithmetic on V = float (one body per lane) or float2 (two bodies per lane, packed) -----------
+// Blackwell's FFMA2/FMUL2/FADD2 do two fp32 operations per issue slot at the full FP32 pipe rate
+// (measured 73.7 TFLOP/s against 72.2 for scalar FFMA, profiles/), which leaves issue slots for
+// the LDS, MUFU and integer instructions of the loop.
+__device__ __forceinline__ float vfma(float a, float b, float c) { return fmaf(a, b, c); }
+__device__ __forceinline__ float vmul(float a, float b) { return a * b; }
+__device__ __forceinline__ float vadd(float a, float b) { return a + b; }
+__device__ __forceinline__ float2 vfma(float2 a, float2 b, float2 c) { return __ffma2_rn(a, b, c); }
+__device__ __forceinline__ float2 vmul(float2 a, float2 b) { return __fmul2_rn(a, b); }
+__device__ __forceinline__ float2 vadd(float2 a, float2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ float rsq(float x)
+{
+    float r;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+__device__ __forceinline__ float vrsqrt(float a) { return rsq(a); }
+__device__ __forceinline__ float2 vrsqrt(float2 a) { return make_float2(rsq(a.x), rsq(a.y)); }
+template <class V> __device__ __forceinline__ V vdup(float a);
+template <> __device__ __forceinline__ float vdup<float>(float a) { return a; }
+template <> __device__ __forceinline__ float2 vdup<float2>(float a) { return make_float2(a, a); }
+template <class V> __device__ __forceinline__ V vpair(float a, float b);   // a duplicated pair read from shared memory
+template <> __device__ __forceinline__ float vpair<float>(float a, float) { return a; }
+template <> __device__ __forceinline__ float2 vpair<float2>(float a, float b) { return make_float2(a, b); }
+__device__ __forceinline__ float vget(float a, int) { return a; }
+__device__ __forceinline__ float vget(float2 a, int b) { return b ? a.y : a.x; }
+__device__ __forceinline__ float &vref(float &a, int) { return a; }
+__device__ __forceinline__ float &vref(float2 &a, int b) { return b ? a.y : a.x; }
+template <int NI> struct VecOf { typedef float type; };
+template <> struct VecOf<2> { typedef float2 type; };
+
 template <int NI> struct Acc {
-    float ax[NI], ay[NI], az[NI], ph[NI];      // current batch (fp32)
+    typedef typename VecOf<NI>::type V;
+    V ax, ay, az, ph;                          // current batch (fp32)
     double dax[NI], day[NI], daz[NI], dph[NI]; // running totals (fp64)
     __device__ __forceinline__ void zero()
     {
+        ax = ay = az = ph = vdup<V>(0.f);
 #pragma unroll
-        for (int b = 0; b < NI; ++b) { ax[b] = ay[b] = az[b] = ph[b] = 0.f; dax[b] = day[b] = daz[b] = dph[b] = 0.0; }
+        for (int b = 0; b < NI; ++b) dax[b] = day[b] = daz[b] = dph[b] = 0.0;
     }
     __device__ __forceinline__ void flush()
     {
 #pragma unroll
         for (int b = 0; b < NI; ++b) {
-            dax[b] += (double)ax[b]; day[b] += (double)ay[b]; daz[b] += (double)az[b]; dph[b] += (double)ph[b];
-            ax[b] = ay[b] = az[b] = ph[b] = 0.f;
+            dax[b] += (double)vget(ax, b); day[b] += (double)vget(ay, b);
+            daz[b] += (double)vget(az, b); dph[b] += (double)vget(ph, b);
         }
+        ax = ay = az = ph = vdup<V>(0.f);
     }
+};
+
+// the group's bodies as the loops consume them: negated coordinates (d = q_j + (-q_i) is one FADD2)
+template <int NI> struct Targets {
+    typedef typename VecOf<NI>::type V;
+    V nx, ny, nz;
 };
 
 __device__ __forceinline__ u32 stack_read(const WarpShared &ws, const u32 *gstack, u32 pos)
@@ -50,89 +92,101 @@ __device__ __forceinline__ void stack_write(WarpShared &ws, u32 *gstack, u32 pos
     else gstack[pos - WALK_STACK_SMEM] = v;
 }
 
-// ---- p-p, plain softened Newtonian (K = W = 1): 23 flop by the convention of DESIGN.md ---------
+// ---- p-p, plain softened Newtonian (K = W = 1): 13 FP32-pipe operations per interaction; counted as
+//      23 flop by the convention of DESIGN.md section 8 ---------------------------------------------
 template <int NI>
-__device__ __forceinline__ void eval_far(const float4 *buf, u32 head, u32 cnt, const float (&xi)[NI], const float (&yi)[NI],
-                                         const float (&zi)[NI], float eps2, Acc<NI> &acc)
+__device__ __forceinline__ void pp_body(const float4 &XY, const float4 &ZM, const Targets<NI> &t,
+                                        typename VecOf<NI>::type eps2, Acc<NI> &acc)
 {
+    typedef typename VecOf<NI>::type V;
+    V dx = vadd(vpair<V>(XY.x, XY.y), t.nx), dy = vadd(vpair<V>(XY.z, XY.w), t.ny), dz = vadd(vpair<V>(ZM.x, ZM.y), t.nz);
+    V r2 = vfma(dx, dx, vfma(dy, dy, vfma(dz, dz, eps2)));
+    V rinv = vrsqrt(r2);
+    V mrinv = vmul(vpair<V>(ZM.z, ZM.w), rinv);
+    V mr3 = vmul(mrinv, vmul(rinv, rinv));
+    acc.ax = vfma(mr3, dx, acc.ax);
+    acc.ay = vfma(mr3, dy, acc.ay);
+    acc.az = vfma(mr3, dz, acc.az);
+    acc.ph = vadd(acc.ph, mrinv);
+}
+
+template <int NI>
+__device__ __forceinline__ void eval_far(const WarpShared &ws, u32 head, u32 cnt, const Targets<NI> &t, float eps2s,
+                                         Acc<NI> &acc)
+{
+    typedef typename VecOf<NI>::type V;
+    const V eps2 = vdup<V>(eps2s);
     if (cnt == 32) {
 #pragma unroll 8
-        for (u32 j = 0; j < 32; ++j) {
-            float4 bj = buf[head + j];
-#pragma unroll
-            for (int b = 0; b < NI; ++b) {
-                float dx = bj.x - xi[b], dy = bj.y - yi[b], dz = bj.z - zi[b];
-                float r2 = fmaf(dx, dx, fmaf(dy, dy, fmaf(dz, dz, eps2)));
-                float rinv = rsqrtf(r2);
-                float mrinv = bj.w * rinv;
-                float mr3 = mrinv * (rinv * rinv);
-                acc.ax[b] = fmaf(mr3, dx, acc.ax[b]);
-                acc.ay[b] = fmaf(mr3, dy, acc.ay[b]);
-                acc.az[b] = fmaf(mr3, dz, acc.az[b]);
-                acc.ph[b] += mrinv;
-            }
-        }
+        for (u32 j = 0; j < 32; ++j) pp_body<NI>(ws.far_xy[head + j], ws.far_zm[head + j], t, eps2, acc);
     } else {
-        for (u32 j = 0; j < cnt; ++j) {
-            float4 bj = buf[head + j];
-#pragma unroll
-            for (int b = 0; b < NI; ++b) {
-                float dx = bj.x - xi[b], dy = bj.y - yi[b], dz = bj.z - zi[b];
-                float r2 = fmaf(dx, dx, fmaf(dy, dy, fmaf(dz, dz, eps2)));
-                float rinv = rsqrtf(r2);
-                float mrinv = bj.w * rinv;
-                float mr3 = mrinv * (rinv * rinv);
-                acc.ax[b] = fmaf(mr3, dx, acc.ax[b]);
-                acc.ay[b] = fmaf(mr3, dy, acc.ay[b]);
-                acc.az[b] = fmaf(mr3, dz, acc.az[b]);
-                acc.ph[b] += mrinv;
-            }
-        }
+        for (u32 j = 0; j < cnt; ++j) pp_body<NI>(ws.far_xy[head + j], ws.far_zm[head + j], t, eps2, acc);
     }
     acc.flush();
 }
 
-// ---- p-c, softened monopole + traceful quadrupole about the COM (R-QUAD), K = W = 1 -------------
-//   with d = c - q_i, s^2 = |d|^2 + eps^2:
-//   a   += d (M/s^3 + 7.5 dQd/s^7 - 1.5 trQ/s^5) - 3 Qd/s^5
-//   -phi += M/s + 1.5 dQd/s^5 - 0.5 trQ/s^3
+// ---- p-c, softened monopole + quadrupole about the centre of mass (rule R-QUAD), K = W = 1 ----------
+//   with d = c - q_i, s^2 = |d|^2 + eps^2 and the traceful Q of moments.cu, R-QUAD reads
+//     -phi = M/s + 1.5 dQd/s^5 - 0.5 trQ/s^3,   a = d (M/s^3 + 7.5 dQd/s^7 - 1.5 trQ/s^5) - 3 Qd/s^5.
+//   Staged per cell (stage_pc):  Q5 = 7.5 Q - 2.5 trQ I,  te5 = -2.5 trQ eps^2,  so that
+//     T = d.Q5 d + te5 = 7.5 dQd - 2.5 trQ s^2,   c1 = M + T/s^4,
+//     -phi = (0.8 M + 0.2 c1)/s,                   a = d c1/s^3 - 0.4 (Q5 d)/s^5
+//   which is the same expression (the eps^2 of the softened trace term is carried by te5), in
+//   33 FP32-pipe operations per interaction; counted as 65 flop by the convention of DESIGN.md.
 template <int NI>
-__device__ __forceinline__ void eval_pc(WarpShared &ws, u32 head, u32 cnt, const float4 *__restrict__ cell_mac,
-                                        const float4 *__restrict__ cell_mom0, const float4 *__restrict__ cell_mom1,
-                                        const float (&xi)[NI], const float (&yi)[NI], const float (&zi)[NI], float eps2,
-                                        Acc<NI> &acc, u32 lane)
+__device__ __forceinline__ void stage_pc(WarpShared &ws, u32 head, u32 cnt, const float4 *__restrict__ cell_mac,
+                                         const float4 *__restrict__ cell_mom0, const float4 *__restrict__ cell_mom1,
+                                         float eps2, u32 lane)
 {
     if (lane < cnt) {
         u32 c = ws.pc_idx[head + lane];   // head is 0 or 32 and cnt <= 32: no wrap
         float4 a = cell_mac[c], q0 = cell_mom0[c], q1 = cell_mom1[c];
-        ws.pc_a[lane] = make_float4(a.x, a.y, a.z, q0.x);                               // c, M
-        ws.pc_b[lane] = make_float4(q0.y, q0.z, q0.w, q0.y + q0.z + q0.w);              // Qxx Qyy Qzz trQ
-        ws.pc_c[lane] = make_float4(q1.x, q1.y, q1.z, 0.f);                             // Qxy Qxz Qyz
+        float tr25 = 2.5f * (q0.y + q0.z + q0.w);
+        float qxx = fmaf(7.5f, q0.y, -tr25), qyy = fmaf(7.5f, q0.z, -tr25), qzz = fmaf(7.5f, q0.w, -tr25);
+        float qxy = 7.5f * q1.x, qxz = 7.5f * q1.y, qyz = 7.5f * q1.z;
+        float te5 = -tr25 * eps2, m08 = 0.8f * q0.x;
+        ws.pc[0][lane] = make_float4(a.x, a.x, a.y, a.y);
+        ws.pc[1][lane] = make_float4(a.z, a.z, q0.x, q0.x);
+        ws.pc[2][lane] = make_float4(qxx, qxx, qyy, qyy);
+        ws.pc[3][lane] = make_float4(qzz, qzz, qxy, qxy);
+        ws.pc[4][lane] = make_float4(qxz, qxz, qyz, qyz);
+        ws.pc[5][lane] = make_float4(te5, te5, m08, m08);
     }
     __syncwarp();
+}
+
+template <int NI>
+__device__ __forceinline__ void eval_pc(WarpShared &ws, u32 head, u32 cnt, const float4 *__restrict__ cell_mac,
+                                        const float4 *__restrict__ cell_mom0, const float4 *__restrict__ cell_mom1,
+                                        const Targets<NI> &t, float eps2s, Acc<NI> &acc, u32 lane)
+{
+    typedef typename VecOf<NI>::type V;
+    stage_pc<NI>(ws, head, cnt, cell_mac, cell_mom0, cell_mom1, eps2s, lane);
+    const V eps2 = vdup<V>(eps2s), c02 = vdup<V>(0.2f), cm04 = vdup<V>(-0.4f);
 #pragma unroll 4
     for (u32 j = 0; j < cnt; ++j) {
-        float4 A = ws.pc_a[j], B = ws.pc_b[j], C = ws.pc_c[j];
-#pragma unroll
-        for (int b = 0; b < NI; ++b) {
-            float dx = A.x - xi[b], dy = A.y - yi[b], dz = A.z - zi[b];
-            float r2 = fmaf(dx, dx, fmaf(dy, dy, fmaf(dz, dz, eps2)));
-            float rinv = rsqrtf(r2);
-            float r2i = rinv * rinv;
-            float r3i = rinv * r2i;
-            float r5i = r3i * r2i;
-            float r7i = r5i * r2i;
-            float qdx = fmaf(B.x, dx, fmaf(C.x, dy, C.y * dz));
-            float qdy = fmaf(C.x, dx, fmaf(B.y, dy, C.z * dz));
-            float qdz = fmaf(C.y, dx, fmaf(C.z, dy, B.z * dz));
-            float dqd = fmaf(dx, qdx, fmaf(dy, qdy, dz * qdz));
-            float coef = fmaf(A.w, r3i, fmaf(7.5f * dqd, r7i, -1.5f * B.w * r5i));
-            float m3r5 = -3.f * r5i;
-            acc.ax[b] += fmaf(coef, dx, m3r5 * qdx);
-            acc.ay[b] += fmaf(coef, dy, m3r5 * qdy);
-            acc.az[b] += fmaf(coef, dz, m3r5 * qdz);
-            acc.ph[b] += fmaf(A.w, rinv, fmaf(1.5f * dqd, r5i, -0.5f * B.w * r3i));
-        }
+        const float4 P0 = ws.pc[0][j], P1 = ws.pc[1][j], P2 = ws.pc[2][j], P3 = ws.pc[3][j], P4 = ws.pc[4][j], P5 = ws.pc[5][j];
+        const V M = vpair<V>(P1.z, P1.w);
+        const V qxx = vpair<V>(P2.x, P2.y), qyy = vpair<V>(P2.z, P2.w), qzz = vpair<V>(P3.x, P3.y);
+        const V qxy = vpair<V>(P3.z, P3.w), qxz = vpair<V>(P4.x, P4.y), qyz = vpair<V>(P4.z, P4.w);
+        V dx = vadd(vpair<V>(P0.x, P0.y), t.nx), dy = vadd(vpair<V>(P0.z, P0.w), t.ny), dz = vadd(vpair<V>(P1.x, P1.y), t.nz);
+        V r2 = vfma(dx, dx, vfma(dy, dy, vfma(dz, dz, eps2)));
+        V rinv = vrsqrt(r2);
+        V r2i = vmul(rinv, rinv);
+        V r3i = vmul(r2i, rinv);
+        V r4i = vmul(r2i, r2i);
+        V n5 = vmul(r3i, vmul(cm04, r2i));                          // -0.4 / s^5
+        V qdx = vfma(qxx, dx, vfma(qxy, dy, vmul(qxz, dz)));
+        V qdy = vfma(qxy, dx, vfma(qyy, dy, vmul(qyz, dz)));
+        V qdz = vfma(qxz, dx, vfma(qyz, dy, vmul(qzz, dz)));
+        V T = vfma(dx, qdx, vfma(dy, qdy, vfma(dz, qdz, vpair<V>(P5.x, P5.y))));
+        V c1 = vfma(T, r4i, M);
+        V pphi = vfma(c02, c1, vpair<V>(P5.z, P5.w));
+        V coef = vmul(c1, r3i);
+        acc.ph = vfma(pphi, rinv, acc.ph);
+        acc.ax = vfma(coef, dx, vfma(n5, qdx, acc.ax));
+        acc.ay = vfma(coef, dy, vfma(n5, qdy, acc.ay));
+        acc.az = vfma(coef, dz, vfma(n5, qdz, acc.az));
     }
     __syncwarp();
     acc.flush();
@@ -156,16 +210,16 @@ __device__ __forceinline__ void eval_near(const WarpShared &ws, u32 head, u32 cn
             bool live = isorted[b] != 0xffffffffu && isorted[b] != js;
             bool hit = live && s2 < prm.h2;
             if (live) {
-                float rinv = rsqrtf(s2);
+                float rinv = rsq(s2);
                 float mrinv = bj.w * rinv;
                 float mr3 = mrinv * (rinv * rinv);
                 float K = 1.f, W = 1.f;
                 if (s2 < prm.rout2) p3t_pair_weights(prm, s2, K, W);
                 mr3 *= K;
-                acc.ax[b] = fmaf(mr3, dx, acc.ax[b]);
-                acc.ay[b] = fmaf(mr3, dy, acc.ay[b]);
-                acc.az[b] = fmaf(mr3, dz, acc.az[b]);
-                acc.ph[b] = fmaf(W, mrinv, acc.ph[b]);
+                vref(acc.ax, b) = fmaf(mr3, dx, vget(acc.ax, b));
+                vref(acc.ay, b) = fmaf(mr3, dy, vget(acc.ay, b));
+                vref(acc.az, b) = fmaf(mr3, dz, vget(acc.az, b));
+                vref(acc.ph, b) = fmaf(W, mrinv, vget(acc.ph, b));
             }
             u32 hb = __ballot_sync(0xffffffffu, hit);
             if (hb) {
@@ -232,6 +286,14 @@ walk_kernel(const float4 *__restrict__ body, const u32 *__restrict__ sorted_idx,
         }
         Acc<NI> acc;
         acc.zero();
+        Targets<NI> tg;
+        if (NI == 2) {
+            vref(tg.nx, 0) = -xi[0]; vref(tg.nx, 1) = -xi[NI - 1];
+            vref(tg.ny, 0) = -yi[0]; vref(tg.ny, 1) = -yi[NI - 1];
+            vref(tg.nz, 0) = -zi[0]; vref(tg.nz, 1) = -zi[NI - 1];
+        } else {
+            vref(tg.nx, 0) = -xi[0]; vref(tg.ny, 0) = -yi[0]; vref(tg.nz, 0) = -zi[0];
+        }
 
         u32 top = 1;
         if (lane == 0) ws.stack[0] = 0;   // root
@@ -282,7 +344,7 @@ walk_kernel(const float4 *__restrict__ body, const u32 *__restrict__ sorted_idx,
                 pc_cnt += __popc(ab);
                 __syncwarp();
                 if (pc_cnt >= 32) {
-                    eval_pc<NI>(ws, pc_head, 32, cell_mac, cell_mom0, cell_mom1, xi, yi, zi, prm.eps2, acc, lane);
+                    eval_pc<NI>(ws, pc_head, 32, cell_mac, cell_mom0, cell_mom1, tg, prm.eps2, acc, lane);
                     pc_head = (pc_head + 32) & 63u; pc_cnt -= 32; n_pc += 32;
                 }
             }
@@ -318,7 +380,11 @@ walk_kernel(const float4 *__restrict__ body, const u32 *__restrict__ sorted_idx,
                     bool isnear = hv && d2 < prm.hnear2;
                     bool isfar = hv && !isnear;
                     u32 fb = __ballot_sync(0xffffffffu, isfar), nb = __ballot_sync(0xffffffffu, isnear);
-                    if (isfar) ws.far_buf[(far_head + far_cnt + __popc(fb & lanemask_lt())) & 63u] = bj;
+                    if (isfar) {
+                        u32 slot = (far_head + far_cnt + __popc(fb & lanemask_lt())) & 63u;
+                        ws.far_xy[slot] = make_float4(bj.x, bj.x, bj.y, bj.y);
+                        ws.far_zm[slot] = make_float4(bj.z, bj.z, bj.w, bj.w);
+                    }
                     if (isnear) {
                         u32 slot = (near_head + near_cnt + __popc(nb & lanemask_lt())) & 63u;
                         ws.near_buf[slot] = bj;
@@ -328,7 +394,7 @@ walk_kernel(const float4 *__restrict__ body, const u32 *__restrict__ sorted_idx,
                     near_cnt += __popc(nb);
                     __syncwarp();
                     if (far_cnt >= 32) {
-                        eval_far<NI>(ws.far_buf, far_head, 32, xi, yi, zi, prm.eps2, acc);
+                        eval_far<NI>(ws, far_head, 32, tg, prm.eps2, acc);
                         far_head = (far_head + 32) & 63u; far_cnt -= 32; n_far += 32;
                     }
                     if (near_cnt >= 32) {
@@ -344,8 +410,8 @@ walk_kernel(const float4 *__restrict__ body, const u32 *__restrict__ sorted_idx,
             if (lane == 0) atomicOr(&counters[CNT_ERR_EVAL], (u64)ERR_STACK_OVERFLOW);
         }
         // ---- flush what is left in the rings
-        if (pc_cnt) { eval_pc<NI>(ws, pc_head, pc_cnt, cell_mac, cell_mom0, cell_mom1, xi, yi, zi, prm.eps2, acc, lane); n_pc += pc_cnt; }
-        if (far_cnt) { eval_far<NI>(ws.far_buf, far_head, far_cnt, xi, yi, zi, prm.eps2, acc); n_far += far_cnt; }
+        if (pc_cnt) { eval_pc<NI>(ws, pc_head, pc_cnt, cell_mac, cell_mom0, cell_mom1, tg, prm.eps2, acc, lane); n_pc += pc_cnt; }
+        if (far_cnt) { eval_far<NI>(ws, far_head, far_cnt, tg, prm.eps2, acc); n_far += far_cnt; }
         if (near_cnt) {
             eval_near<NI>(ws, near_head, near_cnt, xi, yi, zi, isorted, iuser, prm, sorted_idx, pairs, pair_cap, counters, nnb,
                           acc, lane);
