@@ -218,6 +218,9 @@ def main():
         ms = float(t.item())
     st = ctx.get_stats()
     ph = {k: float(np.mean(v)) for k, v in phases.items()}
+    ffma_scalar = ffma_packed = None
+    if rank == 0:      # pure-FFMA calibration kernel, outside the timed region
+        ffma_scalar, ffma_packed = ctx.measure_fp32_peak(False)[0], ctx.measure_fp32_peak(True)[0]
 
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
     e2e = None
@@ -279,7 +282,9 @@ def main():
         "roofline": {"bound": "alu", "kernel": "walk_kernel (a7+a8)", "achieved": walk_tflops, "peak": fp32_peak, "unit": "TFLOP/s",
                      "frac": walk_tflops / fp32_peak, "traffic": None,
                      "peak_source": f"2 flop x {FP32_LANES} lanes x {n_sm} SMs x {peaks['sm_max_mhz']:.0f} MHz ({peaks['source']} sm_max_mhz; DESIGN.md section 8)",
-                     "convention": f"{FLOP_PP} flop per p-p, {FLOP_PC} flop per p-c"},
+                     "convention": f"{FLOP_PP} flop per p-p, {FLOP_PC} flop per p-c",
+                     "ffma_microbench_tflops": {"scalar": ffma_scalar, "packed": ffma_packed},
+                     "frac_of_ffma_microbench": walk_tflops / max(ffma_scalar, ffma_packed)},
         "roofline_hbm": {"bound": "hbm", "passes": "a1-a6 (sort, build, moments)", "achieved": sum(ab.values()) / (tree_ms * 1e-3) / 1e9,
                          "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": sum(ab.values()) / (tree_ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
                          "per_pass_gbs": hbm, "algorithmic_bytes": ab, "peak_source": peaks["source"]},

@@ -144,6 +144,13 @@ p3t_status p3t_synchronize(p3t_ctx *ctx);
 
 const char *p3t_last_error(const p3t_ctx *ctx);
 
+/* Calibration of the ALU roofline denominator (not part of the hot path):
+ * runs a pure-FFMA kernel (packed = 0: scalar FFMA, 1: packed FFMA2) of `iters` outer
+ * iterations on the context's stream, synchronises, and returns the best of four timed
+ * launches as TFLOP/s (2 flop per fp32 FMA) in *tflops [host] and its duration in *ms
+ * [host, nullable].  P3T_EINVAL for null ctx/tflops or iters <= 0. */
+p3t_status p3t_measure_fp32_peak(p3t_ctx *ctx, int packed, int iters, double *tflops, float *ms);
+
 /* Inspection of intermediate arrays (for the a1-a6 parity tests).  Valid after
  * p3t_build_tree.  p3t_array_info gives element count and element size. */
 typedef enum {

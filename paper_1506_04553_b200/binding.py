@@ -30,7 +30,7 @@ SYMBOLS = [
     "p3t_workspace_bytes", "p3t_create", "p3t_destroy", "p3t_set_params", "p3t_set_tree_params",
     "p3t_set_group_merge_levels", "p3t_load_particles", "p3t_build_tree", "p3t_eval_soft", "p3t_eval_direct",
     "p3t_get_acc_pot", "p3t_get_neighbour_counts", "p3t_get_neighbours", "p3t_get_stats", "p3t_synchronize",
-    "p3t_last_error", "p3t_array_info", "p3t_copy_array",
+    "p3t_last_error", "p3t_array_info", "p3t_copy_array", "p3t_measure_fp32_peak",
 ]
 
 ARRAYS = dict(root_cube=(0, np.float32, 1), keys=(1, np.uint64, 1), sorted_idx=(2, np.uint32, 1),
@@ -72,6 +72,8 @@ def _sig():
     L.p3t_last_error.restype = C.c_char_p; L.p3t_last_error.argtypes = [vp]
     L.p3t_array_info.restype = i; L.p3t_array_info.argtypes = [vp, i, C.POINTER(sz), C.POINTER(sz)]
     L.p3t_copy_array.restype = i; L.p3t_copy_array.argtypes = [vp, i, vp, sz, i]
+    L.p3t_measure_fp32_peak.restype = i
+    L.p3t_measure_fp32_peak.argtypes = [vp, i, i, C.POINTER(C.c_double), C.POINTER(C.c_float)]
 
 
 _sig()
@@ -225,6 +227,12 @@ class P3T:
 
     def synchronize(self):
         self._check(_lib.p3t_synchronize(self._h))
+
+    def measure_fp32_peak(self, packed=True, iters=2048):
+        """Pure-FFMA calibration kernel: (TFLOP/s, ms) of the best of four launches."""
+        tf, ms = C.c_double(), C.c_float()
+        self._check(_lib.p3t_measure_fp32_peak(self._h, int(bool(packed)), int(iters), C.byref(tf), C.byref(ms)))
+        return tf.value, ms.value
 
     def array(self, name):
         """Copy of an intermediate array (a1-a6 inspection), as numpy."""
