@@ -24,7 +24,7 @@ typedef unsigned char u8;
 #define SORT_TILE (SORT_THREADS * SORT_ITEMS)
 #define BUILD_THREADS 256
 #define WALK_WARPS 4                 // warps per CTA in the walk kernel
-#define WALK_STACK_SMEM 1024         // stack entries per warp held in shared memory
+#define WALK_STACK_SMEM 512          // stack entries per warp held in shared memory
 #define WALK_STACK_GMEM 7168         // overflow entries per warp in global memory
 
 // Parameters handed to kernels by value.  The coefficients of W are prepared on the host in

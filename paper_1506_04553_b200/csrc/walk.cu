@@ -20,9 +20,23 @@ struct WarpShared {
     float4 far_xy[64], far_zm[64];
     float4 near_buf[64];
     u32 near_idx[64];
-    u32 pc_idx[64];
-    float4 pc[6][32];   // staged cells of one batch, duplicated pairs (see stage_pc)
+    float4 pc[6][64];   // p-c ring: staged cells, duplicated pairs (see stage_pc)
+    // landing area of the asynchronous copies (cp.async) of the 32 cells popped for the NEXT walk
+    // step: their latency is hidden behind the interaction batches of the current step
+    float4 l_mac[32], l_mom0[32], l_mom1[32];
+    uint2 l_meta[32];
 };
+
+__device__ __forceinline__ void cp_async16(void *smem, const void *gmem)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"((u32)__cvta_generic_to_shared(smem)), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async8(void *smem, const void *gmem)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((u32)__cvta_generic_to_shared(smem)), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
 // ---- arithmetic on V = float (one body per lane) or float2 (two bodies per lane, packed) -----------
 // Blackwell's FFMA2/FMUL2/FADD2 do two fp32 operations per issue slot at the full FP32 pipe rate
@@ -77,9 +91,16 @@ template <int NI> struct Acc {
 };
 
 // the group's bodies as the loops consume them: negated coordinates (d = q_j + (-q_i) is one FADD2)
+// seal(): passes each component through an identity shuffle, which makes the pairs opaque to ptxas:
+// it then keeps them in aligned register pairs for the whole walk instead of rebuilding them from
+// the registers of the body load with two MOVs at every use (once per group, 3*NI SHFLs).
+__device__ __forceinline__ float vseal1(float a) { return __shfl_sync(0xffffffffu, a, threadIdx.x & 31); }
+__device__ __forceinline__ void vseal(float &a) { a = vseal1(a); }
+__device__ __forceinline__ void vseal(float2 &a) { a = make_float2(vseal1(a.x), vseal1(a.y)); }
 template <int NI> struct Targets {
     typedef typename VecOf<NI>::type V;
     V nx, ny, nz;
+    __device__ __forceinline__ void seal() { vseal(nx); vseal(ny); vseal(nz); }
 };
 
 __device__ __forceinline__ u32 stack_read(const WarpShared &ws, const u32 *gstack, u32 pos)
@@ -133,39 +154,29 @@ __device__ __forceinline__ void eval_far(const WarpShared &ws, u32 head, u32 cnt
 //     -phi = (0.8 M + 0.2 c1)/s,                   a = d c1/s^3 - 0.4 (Q5 d)/s^5
 //   which is the same expression (the eps^2 of the softened trace term is carried by te5), in
 //   33 FP32-pipe operations per interaction; counted as 65 flop by the convention of DESIGN.md.
-template <int NI>
-__device__ __forceinline__ void stage_pc(WarpShared &ws, u32 head, u32 cnt, const float4 *__restrict__ cell_mac,
-                                         const float4 *__restrict__ cell_mom0, const float4 *__restrict__ cell_mom1,
-                                         float eps2, u32 lane)
+__device__ __forceinline__ void stage_pc(WarpShared &ws, u32 slot, const float4 &a, const float4 &q0, const float4 &q1, float eps2)
 {
-    if (lane < cnt) {
-        u32 c = ws.pc_idx[head + lane];   // head is 0 or 32 and cnt <= 32: no wrap
-        float4 a = cell_mac[c], q0 = cell_mom0[c], q1 = cell_mom1[c];
-        float tr25 = 2.5f * (q0.y + q0.z + q0.w);
-        float qxx = fmaf(7.5f, q0.y, -tr25), qyy = fmaf(7.5f, q0.z, -tr25), qzz = fmaf(7.5f, q0.w, -tr25);
-        float qxy = 7.5f * q1.x, qxz = 7.5f * q1.y, qyz = 7.5f * q1.z;
-        float te5 = -tr25 * eps2, m08 = 0.8f * q0.x;
-        ws.pc[0][lane] = make_float4(a.x, a.x, a.y, a.y);
-        ws.pc[1][lane] = make_float4(a.z, a.z, q0.x, q0.x);
-        ws.pc[2][lane] = make_float4(qxx, qxx, qyy, qyy);
-        ws.pc[3][lane] = make_float4(qzz, qzz, qxy, qxy);
-        ws.pc[4][lane] = make_float4(qxz, qxz, qyz, qyz);
-        ws.pc[5][lane] = make_float4(te5, te5, m08, m08);
-    }
-    __syncwarp();
+    float tr25 = 2.5f * (q0.y + q0.z + q0.w);
+    float qxx = fmaf(7.5f, q0.y, -tr25), qyy = fmaf(7.5f, q0.z, -tr25), qzz = fmaf(7.5f, q0.w, -tr25);
+    float qxy = 7.5f * q1.x, qxz = 7.5f * q1.y, qyz = 7.5f * q1.z;
+    float te5 = -tr25 * eps2, m08 = 0.8f * q0.x;
+    ws.pc[0][slot] = make_float4(a.x, a.x, a.y, a.y);
+    ws.pc[1][slot] = make_float4(a.z, a.z, q0.x, q0.x);
+    ws.pc[2][slot] = make_float4(qxx, qxx, qyy, qyy);
+    ws.pc[3][slot] = make_float4(qzz, qzz, qxy, qxy);
+    ws.pc[4][slot] = make_float4(qxz, qxz, qyz, qyz);
+    ws.pc[5][slot] = make_float4(te5, te5, m08, m08);
 }
 
 template <int NI>
-__device__ __forceinline__ void eval_pc(WarpShared &ws, u32 head, u32 cnt, const float4 *__restrict__ cell_mac,
-                                        const float4 *__restrict__ cell_mom0, const float4 *__restrict__ cell_mom1,
-                                        const Targets<NI> &t, float eps2s, Acc<NI> &acc, u32 lane)
+__device__ __forceinline__ void eval_pc(const WarpShared &ws, u32 head, u32 cnt, const Targets<NI> &t, float eps2s, Acc<NI> &acc)
 {
     typedef typename VecOf<NI>::type V;
-    stage_pc<NI>(ws, head, cnt, cell_mac, cell_mom0, cell_mom1, eps2s, lane);
     const V eps2 = vdup<V>(eps2s), c02 = vdup<V>(0.2f), cm04 = vdup<V>(-0.4f);
 #pragma unroll 4
     for (u32 j = 0; j < cnt; ++j) {
-        const float4 P0 = ws.pc[0][j], P1 = ws.pc[1][j], P2 = ws.pc[2][j], P3 = ws.pc[3][j], P4 = ws.pc[4][j], P5 = ws.pc[5][j];
+        const u32 e = head + j;
+        const float4 P0 = ws.pc[0][e], P1 = ws.pc[1][e], P2 = ws.pc[2][e], P3 = ws.pc[3][e], P4 = ws.pc[4][e], P5 = ws.pc[5][e];
         const V M = vpair<V>(P1.z, P1.w);
         const V qxx = vpair<V>(P2.x, P2.y), qyy = vpair<V>(P2.z, P2.w), qzz = vpair<V>(P3.x, P3.y);
         const V qxy = vpair<V>(P3.z, P3.w), qxz = vpair<V>(P4.x, P4.y), qyz = vpair<V>(P4.z, P4.w);
@@ -188,15 +199,14 @@ __device__ __forceinline__ void eval_pc(WarpShared &ws, u32 head, u32 cnt, const
         acc.ay = vfma(coef, dy, vfma(n5, qdy, acc.ay));
         acc.az = vfma(coef, dz, vfma(n5, qdz, acc.az));
     }
-    __syncwarp();
     acc.flush();
 }
 
 // ---- p-p slow path: K (Eq. 12) on the force, W (Eq. 16-17) on the potential, j != i by index,
 //      neighbour emission for s_ij < h (reading A4) -------------------------------------------------
 template <int NI>
-__device__ __forceinline__ void eval_near(const WarpShared &ws, u32 head, u32 cnt, const float (&xi)[NI], const float (&yi)[NI],
-                                          const float (&zi)[NI], const u32 (&isorted)[NI], const u32 (&iuser)[NI],
+__device__ __forceinline__ void eval_near(const WarpShared &ws, u32 head, u32 cnt, const Targets<NI> &t,
+                                          const u32 (&isorted)[NI], const u32 (&iuser)[NI],
                                           const P3TParams &prm, const u32 *__restrict__ sorted_idx, uint2 *pairs, u64 pair_cap,
                                           u64 *counters, u32 (&nnb)[NI], Acc<NI> &acc, u32 lane)
 {
@@ -205,7 +215,7 @@ __device__ __forceinline__ void eval_near(const WarpShared &ws, u32 head, u32 cn
         u32 js = ws.near_idx[head + j];
 #pragma unroll
         for (int b = 0; b < NI; ++b) {
-            float dx = bj.x - xi[b], dy = bj.y - yi[b], dz = bj.z - zi[b];
+            float dx = bj.x + vget(t.nx, b), dy = bj.y + vget(t.ny, b), dz = bj.z + vget(t.nz, b);
             float s2 = fmaf(dx, dx, fmaf(dy, dy, fmaf(dz, dz, prm.eps2)));
             bool live = isorted[b] != 0xffffffffu && isorted[b] != js;
             bool hit = live && s2 < prm.h2;
@@ -237,204 +247,252 @@ __device__ __forceinline__ void eval_near(const WarpShared &ws, u32 head, u32 cn
     acc.flush();
 }
 
-template <int NI>
-__global__ void __launch_bounds__(WALK_WARPS * 32, 16 / WALK_WARPS)
-walk_kernel(const float4 *__restrict__ body, const u32 *__restrict__ sorted_idx, const u32 *__restrict__ group_start,
-            const float4 *__restrict__ cell_mac, const float4 *__restrict__ cell_mom0, const float4 *__restrict__ cell_mom1,
-            const uint2 *__restrict__ cell_meta, P3TParams prm, float4 *__restrict__ accpot, u32 *__restrict__ nbr_count,
-            uint2 *pairs, u64 pair_cap, u32 *walk_stack, u64 *counters)
+// Arguments of the walk that do not change between groups.
+struct WalkArgs {
+    const float4 *__restrict__ body;
+    const u32 *__restrict__ sorted_idx;
+    const float4 *__restrict__ cell_mac, *__restrict__ cell_mom0, *__restrict__ cell_mom1;
+    const uint2 *__restrict__ cell_meta;
+    float4 *__restrict__ accpot;
+    u32 *__restrict__ nbr_count;
+    uint2 *pairs;
+    u64 pair_cap;
+    u64 *counters;
+};
+
+// pops up to 32 cells and starts the asynchronous copy of their records into the landing area
+__device__ __forceinline__ u32 pop_cells(WarpShared &ws, const u32 *gstack, const WalkArgs &A, u32 &top, u32 lane, u32 &cell)
 {
-    __shared__ WarpShared s_ws[WALK_WARPS];
+    const u32 take = min(32u, top);
+    top -= take;
+    cell = 0u;
+    if (lane < take) {
+        cell = stack_read(ws, gstack, top + lane);
+        cp_async16(&ws.l_mac[lane], &A.cell_mac[cell]);
+        cp_async8(&ws.l_meta[lane], &A.cell_meta[cell]);
+        cp_async16(&ws.l_mom0[lane], &A.cell_mom0[cell]);
+        cp_async16(&ws.l_mom1[lane], &A.cell_mom1[cell]);
+    }
+    cp_async_commit();
+    return take;
+}
+
+// One i-group: walk + interactions.  Walk step k consumes the 32 cell records that were requested
+// during step k-1, pushes children, requests the records of step k+1, and only then evaluates the
+// leaf bodies and the full interaction batches, so that the requests are in flight behind FP32 work.
+template <int NI>
+__device__ __forceinline__ void walk_group(WarpShared &ws, u32 *gstack, const WalkArgs &A, const P3TParams &prm, u32 gs, u32 ge,
+                                           u32 lane, u64 &tot_pp, u64 &tot_pc, u64 &tot_near)
+{
+    const u32 gcount = ge - gs;
+    // ---- my bodies; empty slots replicate the group's first body and are flagged dead
+    Targets<NI> tg;
+    u32 isorted[NI], iuser[NI], nnb[NI];
+    float lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY};
+#pragma unroll
+    for (int b = 0; b < NI; ++b) {
+        u32 k = gs + b * 32 + lane;
+        bool ok = k < ge;
+        float4 p = A.body[ok ? k : gs];
+        vref(tg.nx, b) = -p.x; vref(tg.ny, b) = -p.y; vref(tg.nz, b) = -p.z;
+        isorted[b] = ok ? k : 0xffffffffu;
+        iuser[b] = ok ? A.sorted_idx[k] : 0u;
+        nnb[b] = 0;
+        lo[0] = fminf(lo[0], p.x); hi[0] = fmaxf(hi[0], p.x);
+        lo[1] = fminf(lo[1], p.y); hi[1] = fmaxf(hi[1], p.y);
+        lo[2] = fminf(lo[2], p.z); hi[2] = fmaxf(hi[2], p.z);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            lo[d] = fminf(lo[d], __shfl_xor_sync(0xffffffffu, lo[d], o));
+            hi[d] = fmaxf(hi[d], __shfl_xor_sync(0xffffffffu, hi[d], o));
+        }
+    }
+    Acc<NI> acc;
+    acc.zero();
+    tg.seal();
+
+    u32 top = 1;
+    if (lane == 0) ws.stack[0] = 0;   // root
+    u32 far_head = 0, far_cnt = 0, near_head = 0, near_cnt = 0, pc_head = 0, pc_cnt = 0;
+    u32 n_far = 0, n_near = 0, n_pc = 0;
+    bool overflow = false;
+    __syncwarp();
+    u32 cell;
+    u32 take = pop_cells(ws, gstack, A, top, lane, cell);
+    while (take > 0) {
+        const bool have = lane < take;
+        cp_async_wait_all();
+        // ---- consume the landed records: acceptance test (R-MAC, folded radius of moments.cu)
+        bool accept = false;
+        u32 nch = 0, first = 0, lcount = 0, lstart = 0;
+        float4 a = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (have) {
+            a = ws.l_mac[lane];
+            float ex = fmaxf(0.f, fmaxf(lo[0] - a.x, a.x - hi[0]));
+            float ey = fmaxf(0.f, fmaxf(lo[1] - a.y, a.y - hi[1]));
+            float ez = fmaxf(0.f, fmaxf(lo[2] - a.z, a.z - hi[2]));
+            float d2 = fmaf(ex, ex, fmaf(ey, ey, ez * ez));
+            accept = d2 > a.w;
+            if (!accept) {
+                uint2 meta = ws.l_meta[lane];
+                if (meta.y & P3T_LEAF_FLAG) { lstart = meta.x; lcount = meta.y & ~P3T_LEAF_FLAG; }
+                else { first = meta.x; nch = meta.y; }
+            }
+        }
+        // ---- accepted cells -> p-c ring (at most 31 pending + 32 new entries, capacity 64)
+        {
+            u32 ab = __ballot_sync(0xffffffffu, accept);
+            if (accept)
+                stage_pc(ws, (pc_head + pc_cnt + __popc(ab & lanemask_lt())) & 63u, a, ws.l_mom0[lane], ws.l_mom1[lane], prm.eps2);
+            pc_cnt += __popc(ab);
+        }
+        // ---- children of opened internal cells -> stack
+        {
+            u32 inc = nch;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                u32 t = __shfl_up_sync(0xffffffffu, inc, o);
+                if (lane >= o) inc += t;
+            }
+            u32 total = __shfl_sync(0xffffffffu, inc, 31);
+            if (top + total > WALK_STACK_SMEM + WALK_STACK_GMEM) { overflow = true; break; }
+            u32 pos = top + inc - nch;
+            for (u32 c = 0; c < nch; ++c) stack_write(ws, gstack, pos + c, first + c);
+            top += total;
+        }
+        __syncwarp();
+        // ---- request the records of the next step before any interaction work
+        take = top > 0 ? pop_cells(ws, gstack, A, top, lane, cell) : 0u;
+        // ---- bodies of opened leaves -> near / far rings; the next chunk of 32 bodies is loaded
+        //      while the current one is tested and (when a ring fills) evaluated
+        {
+            u32 inc = lcount;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                u32 t = __shfl_up_sync(0xffffffffu, inc, o);
+                if (lane >= o) inc += t;
+            }
+            const u32 total = __shfl_sync(0xffffffffu, inc, 31);
+            const u32 excl = inc - lcount;
+            auto fetch = [&](u32 v0, float4 &bj, u32 &bidx, bool &hv) {
+                u32 v = v0 + lane;
+                u32 s = 0;   // owner lane: largest s with excl[s] <= v
+#pragma unroll
+                for (int step = 16; step > 0; step >>= 1) {
+                    u32 cand = s + step;
+                    u32 t = __shfl_sync(0xffffffffu, inc, cand - 1);   // = excl[cand]
+                    if (t <= v) s = cand;
+                }
+                u32 s_start = __shfl_sync(0xffffffffu, lstart, s);
+                u32 s_excl = __shfl_sync(0xffffffffu, excl, s);
+                hv = v < total;
+                bidx = s_start + (v - s_excl);
+                bj = A.body[hv ? bidx : gs];
+            };
+            float4 bj = make_float4(0.f, 0.f, 0.f, 0.f), bn = bj;
+            u32 bidx = 0, bidxn = 0;
+            bool hv = false, hvn = false;
+            if (total) fetch(0, bj, bidx, hv);
+            for (u32 v0 = 0; v0 < total; v0 += 32) {
+                hvn = false;
+                if (v0 + 32 < total) fetch(v0 + 32, bn, bidxn, hvn);
+                float ex = fmaxf(0.f, fmaxf(lo[0] - bj.x, bj.x - hi[0]));
+                float ey = fmaxf(0.f, fmaxf(lo[1] - bj.y, bj.y - hi[1]));
+                float ez = fmaxf(0.f, fmaxf(lo[2] - bj.z, bj.z - hi[2]));
+                float d2 = fmaf(ex, ex, fmaf(ey, ey, ez * ez));
+                bool isnear = hv && d2 < prm.hnear2;
+                bool isfar = hv && !isnear;
+                u32 fb = __ballot_sync(0xffffffffu, isfar), nb = __ballot_sync(0xffffffffu, isnear);
+                if (isfar) {
+                    u32 slot = (far_head + far_cnt + __popc(fb & lanemask_lt())) & 63u;
+                    ws.far_xy[slot] = make_float4(bj.x, bj.x, bj.y, bj.y);
+                    ws.far_zm[slot] = make_float4(bj.z, bj.z, bj.w, bj.w);
+                }
+                if (isnear) {
+                    u32 slot = (near_head + near_cnt + __popc(nb & lanemask_lt())) & 63u;
+                    ws.near_buf[slot] = bj;
+                    ws.near_idx[slot] = bidx;
+                }
+                far_cnt += __popc(fb);
+                near_cnt += __popc(nb);
+                __syncwarp();
+                if (far_cnt >= 32) {
+                    eval_far<NI>(ws, far_head, 32, tg, prm.eps2, acc);
+                    far_head = (far_head + 32) & 63u; far_cnt -= 32; n_far += 32;
+                }
+                if (near_cnt >= 32) {
+                    eval_near<NI>(ws, near_head, 32, tg, isorted, iuser, prm, A.sorted_idx, A.pairs, A.pair_cap, A.counters, nnb,
+                                  acc, lane);
+                    near_head = (near_head + 32) & 63u; near_cnt -= 32; n_near += 32;
+                }
+                __syncwarp();
+                bj = bn; bidx = bidxn; hv = hvn;
+            }
+        }
+        // ---- a full batch of accepted cells
+        if (pc_cnt >= 32) {
+            eval_pc<NI>(ws, pc_head, 32, tg, prm.eps2, acc);
+            pc_head = (pc_head + 32) & 63u; pc_cnt -= 32; n_pc += 32;
+            __syncwarp();
+        }
+    }
+    cp_async_wait_all();
+    if (overflow) {
+        if (lane == 0) atomicOr(&A.counters[CNT_ERR_EVAL], (u64)ERR_STACK_OVERFLOW);
+    }
+    // ---- flush what is left in the rings
+    __syncwarp();
+    if (pc_cnt) { eval_pc<NI>(ws, pc_head, pc_cnt, tg, prm.eps2, acc); n_pc += pc_cnt; }
+    if (far_cnt) { eval_far<NI>(ws, far_head, far_cnt, tg, prm.eps2, acc); n_far += far_cnt; }
+    if (near_cnt) {
+        eval_near<NI>(ws, near_head, near_cnt, tg, isorted, iuser, prm, A.sorted_idx, A.pairs, A.pair_cap, A.counters, nnb, acc, lane);
+        n_near += near_cnt;
+    }
+    __syncwarp();
+    // ---- results, user order
+#pragma unroll
+    for (int b = 0; b < NI; ++b) {
+        if (isorted[b] != 0xffffffffu) {
+            A.accpot[iuser[b]] = make_float4((float)acc.dax[b], (float)acc.day[b], (float)acc.daz[b], (float)(-acc.dph[b]));
+            A.nbr_count[iuser[b]] = nnb[b];
+        }
+    }
+    // each live body met itself once on the near path (distance 0 to its own group's box)
+    tot_pp += (u64)(n_far + n_near) * gcount - gcount;
+    tot_near += (u64)n_near * gcount - gcount;
+    tot_pc += (u64)n_pc * gcount;
+}
+
+// Persistent grid: 148 SMs x 4 CTAs x 4 warps; groups are handed out by an atomic ticket.  A group
+// of at most 32 bodies takes the one-body-per-lane path (half the FP32 work of the packed path).
+template <int NIMAX>
+__global__ void __launch_bounds__(WALK_WARPS * 32, 16 / WALK_WARPS)
+walk_kernel(WalkArgs A, const u32 *__restrict__ group_start, P3TParams prm, u32 *walk_stack)
+{
+    extern __shared__ __align__(16) unsigned char s_raw[];
     const u32 lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    WarpShared &ws = s_ws[warp];
+    WarpShared &ws = reinterpret_cast<WarpShared *>(s_raw)[warp];
     u32 *gstack = walk_stack + (size_t)(blockIdx.x * WALK_WARPS + warp) * WALK_STACK_GMEM;
-    const u32 ngroups = (u32)counters[CNT_NGROUPS];
+    const u32 ngroups = (u32)A.counters[CNT_NGROUPS];
     u64 tot_pp = 0, tot_pc = 0, tot_near = 0;
 
     while (true) {
         u32 g = 0;
-        if (lane == 0) g = (u32)atomicAdd(&counters[CNT_GROUP_TICKET], 1ull);
+        if (lane == 0) g = (u32)atomicAdd(&A.counters[CNT_GROUP_TICKET], 1ull);
         g = __shfl_sync(0xffffffffu, g, 0);
         if (g >= ngroups) break;
         const u32 gs = group_start[g], ge = group_start[g + 1];
-        const u32 gcount = ge - gs;
-
-        // ---- my bodies; empty slots replicate the group's first body and are flagged dead
-        float xi[NI], yi[NI], zi[NI];
-        u32 isorted[NI], iuser[NI], nnb[NI];
-        float lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY};
-#pragma unroll
-        for (int b = 0; b < NI; ++b) {
-            u32 k = gs + b * 32 + lane;
-            bool ok = k < ge;
-            float4 p = body[ok ? k : gs];
-            xi[b] = p.x; yi[b] = p.y; zi[b] = p.z;
-            isorted[b] = ok ? k : 0xffffffffu;
-            iuser[b] = ok ? sorted_idx[k] : 0u;
-            nnb[b] = 0;
-            lo[0] = fminf(lo[0], p.x); hi[0] = fmaxf(hi[0], p.x);
-            lo[1] = fminf(lo[1], p.y); hi[1] = fmaxf(hi[1], p.y);
-            lo[2] = fminf(lo[2], p.z); hi[2] = fmaxf(hi[2], p.z);
-        }
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-#pragma unroll
-            for (int d = 0; d < 3; ++d) {
-                lo[d] = fminf(lo[d], __shfl_xor_sync(0xffffffffu, lo[d], o));
-                hi[d] = fmaxf(hi[d], __shfl_xor_sync(0xffffffffu, hi[d], o));
-            }
-        }
-        Acc<NI> acc;
-        acc.zero();
-        Targets<NI> tg;
-        if (NI == 2) {
-            vref(tg.nx, 0) = -xi[0]; vref(tg.nx, 1) = -xi[NI - 1];
-            vref(tg.ny, 0) = -yi[0]; vref(tg.ny, 1) = -yi[NI - 1];
-            vref(tg.nz, 0) = -zi[0]; vref(tg.nz, 1) = -zi[NI - 1];
-        } else {
-            vref(tg.nx, 0) = -xi[0]; vref(tg.ny, 0) = -yi[0]; vref(tg.nz, 0) = -zi[0];
-        }
-
-        u32 top = 1;
-        if (lane == 0) ws.stack[0] = 0;   // root
-        u32 far_head = 0, far_cnt = 0, near_head = 0, near_cnt = 0, pc_head = 0, pc_cnt = 0;
-        u32 n_far = 0, n_near = 0, n_pc = 0;
-        bool overflow = false;
+        if (NIMAX == 2 && ge - gs > 32) walk_group<2>(ws, gstack, A, prm, gs, ge, lane, tot_pp, tot_pc, tot_near);
+        else walk_group<1>(ws, gstack, A, prm, gs, ge, lane, tot_pp, tot_pc, tot_near);
         __syncwarp();
-
-        while (top > 0) {
-            const u32 take = min(32u, top);
-            top -= take;
-            bool have = lane < take;
-            u32 cell = have ? stack_read(ws, gstack, top + lane) : 0u;
-            __syncwarp();
-            bool accept = false;
-            u32 nch = 0, first = 0, lcount = 0, lstart = 0;
-            if (have) {
-                float4 a = cell_mac[cell];
-                float ex = fmaxf(0.f, fmaxf(lo[0] - a.x, a.x - hi[0]));
-                float ey = fmaxf(0.f, fmaxf(lo[1] - a.y, a.y - hi[1]));
-                float ez = fmaxf(0.f, fmaxf(lo[2] - a.z, a.z - hi[2]));
-                float d2 = fmaf(ex, ex, fmaf(ey, ey, ez * ez));
-                accept = d2 > a.w;
-                if (!accept) {
-                    uint2 meta = cell_meta[cell];
-                    if (meta.y & P3T_LEAF_FLAG) { lstart = meta.x; lcount = meta.y & ~P3T_LEAF_FLAG; }
-                    else { first = meta.x; nch = meta.y; }
-                }
-            }
-            // ---- children of opened internal cells -> stack
-            {
-                u32 inc = nch;
-#pragma unroll
-                for (int o = 1; o < 32; o <<= 1) {
-                    u32 t = __shfl_up_sync(0xffffffffu, inc, o);
-                    if (lane >= o) inc += t;
-                }
-                u32 total = __shfl_sync(0xffffffffu, inc, 31);
-                if (top + total > WALK_STACK_SMEM + WALK_STACK_GMEM) { overflow = true; break; }
-                u32 pos = top + inc - nch;
-                for (u32 c = 0; c < nch; ++c) stack_write(ws, gstack, pos + c, first + c);
-                top += total;
-            }
-            // ---- accepted cells -> p-c ring
-            {
-                u32 ab = __ballot_sync(0xffffffffu, accept);
-                if (accept) ws.pc_idx[(pc_head + pc_cnt + __popc(ab & lanemask_lt())) & 63u] = cell;
-                pc_cnt += __popc(ab);
-                __syncwarp();
-                if (pc_cnt >= 32) {
-                    eval_pc<NI>(ws, pc_head, 32, cell_mac, cell_mom0, cell_mom1, tg, prm.eps2, acc, lane);
-                    pc_head = (pc_head + 32) & 63u; pc_cnt -= 32; n_pc += 32;
-                }
-            }
-            // ---- bodies of opened leaves -> near / far rings
-            {
-                u32 inc = lcount;
-#pragma unroll
-                for (int o = 1; o < 32; o <<= 1) {
-                    u32 t = __shfl_up_sync(0xffffffffu, inc, o);
-                    if (lane >= o) inc += t;
-                }
-                const u32 total = __shfl_sync(0xffffffffu, inc, 31);
-                const u32 excl = inc - lcount;
-                for (u32 v0 = 0; v0 < total; v0 += 32) {
-                    u32 v = v0 + lane;
-                    // owner lane: largest s with excl[s] <= v
-                    u32 s = 0;
-#pragma unroll
-                    for (int step = 16; step > 0; step >>= 1) {
-                        u32 cand = s + step;
-                        u32 t = __shfl_sync(0xffffffffu, inc, cand - 1);   // = excl[cand]
-                        if (t <= v) s = cand;
-                    }
-                    u32 s_start = __shfl_sync(0xffffffffu, lstart, s);
-                    u32 s_excl = __shfl_sync(0xffffffffu, excl, s);
-                    bool hv = v < total;
-                    u32 bidx = s_start + (v - s_excl);
-                    float4 bj = body[hv ? bidx : gs];
-                    float ex = fmaxf(0.f, fmaxf(lo[0] - bj.x, bj.x - hi[0]));
-                    float ey = fmaxf(0.f, fmaxf(lo[1] - bj.y, bj.y - hi[1]));
-                    float ez = fmaxf(0.f, fmaxf(lo[2] - bj.z, bj.z - hi[2]));
-                    float d2 = fmaf(ex, ex, fmaf(ey, ey, ez * ez));
-                    bool isnear = hv && d2 < prm.hnear2;
-                    bool isfar = hv && !isnear;
-                    u32 fb = __ballot_sync(0xffffffffu, isfar), nb = __ballot_sync(0xffffffffu, isnear);
-                    if (isfar) {
-                        u32 slot = (far_head + far_cnt + __popc(fb & lanemask_lt())) & 63u;
-                        ws.far_xy[slot] = make_float4(bj.x, bj.x, bj.y, bj.y);
-                        ws.far_zm[slot] = make_float4(bj.z, bj.z, bj.w, bj.w);
-                    }
-                    if (isnear) {
-                        u32 slot = (near_head + near_cnt + __popc(nb & lanemask_lt())) & 63u;
-                        ws.near_buf[slot] = bj;
-                        ws.near_idx[slot] = bidx;
-                    }
-                    far_cnt += __popc(fb);
-                    near_cnt += __popc(nb);
-                    __syncwarp();
-                    if (far_cnt >= 32) {
-                        eval_far<NI>(ws, far_head, 32, tg, prm.eps2, acc);
-                        far_head = (far_head + 32) & 63u; far_cnt -= 32; n_far += 32;
-                    }
-                    if (near_cnt >= 32) {
-                        eval_near<NI>(ws, near_head, 32, xi, yi, zi, isorted, iuser, prm, sorted_idx, pairs, pair_cap, counters,
-                                      nnb, acc, lane);
-                        near_head = (near_head + 32) & 63u; near_cnt -= 32; n_near += 32;
-                    }
-                    __syncwarp();
-                }
-            }
-        }
-        if (overflow) {
-            if (lane == 0) atomicOr(&counters[CNT_ERR_EVAL], (u64)ERR_STACK_OVERFLOW);
-        }
-        // ---- flush what is left in the rings
-        if (pc_cnt) { eval_pc<NI>(ws, pc_head, pc_cnt, cell_mac, cell_mom0, cell_mom1, tg, prm.eps2, acc, lane); n_pc += pc_cnt; }
-        if (far_cnt) { eval_far<NI>(ws, far_head, far_cnt, tg, prm.eps2, acc); n_far += far_cnt; }
-        if (near_cnt) {
-            eval_near<NI>(ws, near_head, near_cnt, xi, yi, zi, isorted, iuser, prm, sorted_idx, pairs, pair_cap, counters, nnb,
-                          acc, lane);
-            n_near += near_cnt;
-        }
-        __syncwarp();
-        // ---- results, user order
-#pragma unroll
-        for (int b = 0; b < NI; ++b) {
-            if (isorted[b] != 0xffffffffu) {
-                accpot[iuser[b]] = make_float4((float)acc.dax[b], (float)acc.day[b], (float)acc.daz[b], (float)(-acc.dph[b]));
-                nbr_count[iuser[b]] = nnb[b];
-            }
-        }
-        // each live body met itself once on the near path (distance 0 to its own group's box)
-        tot_pp += (u64)(n_far + n_near) * gcount - gcount;
-        tot_near += (u64)n_near * gcount - gcount;
-        tot_pc += (u64)n_pc * gcount;
     }
     if (lane == 0) {
-        atomicAdd(&counters[CNT_NPP], tot_pp);
-        atomicAdd(&counters[CNT_NPC], tot_pc);
-        atomicAdd(&counters[CNT_NNEAR], tot_near);
+        atomicAdd(&A.counters[CNT_NPP], tot_pp);
+        atomicAdd(&A.counters[CNT_NPC], tot_pc);
+        atomicAdd(&A.counters[CNT_NNEAR], tot_near);
     }
 }
 
@@ -445,14 +503,20 @@ p3t_status p3t_stage_walk(p3t_ctx *ctx)
     P3T_CUDA(ctx, cudaMemsetAsync(w.counters, 0, 8 * sizeof(u64), s));   // eval counters
     u32 grid = (u32)ctx->sm_count * (16 / WALK_WARPS);
     if ((size_t)grid * WALK_WARPS > w.walk_warps_max) grid = (u32)(w.walk_warps_max / WALK_WARPS);
-    if (ctx->ngroup == 64)
-        walk_kernel<2><<<grid, WALK_WARPS * 32, 0, s>>>(w.body, w.idx[ctx->cur], w.group_start, w.cell_mac, w.cell_mom0, w.cell_mom1,
-                                                        w.cell_meta, ctx->prm, w.accpot, w.nbr_count, w.pairs,
-                                                        (u64)ctx->nbr_capacity, w.walk_stack, w.counters);
-    else
-        walk_kernel<1><<<grid, WALK_WARPS * 32, 0, s>>>(w.body, w.idx[ctx->cur], w.group_start, w.cell_mac, w.cell_mom0, w.cell_mom1,
-                                                        w.cell_meta, ctx->prm, w.accpot, w.nbr_count, w.pairs,
-                                                        (u64)ctx->nbr_capacity, w.walk_stack, w.counters);
+    const size_t smem = sizeof(WarpShared) * WALK_WARPS;
+    static bool attr_set = false;
+    if (!attr_set) {
+        P3T_CUDA(ctx, cudaFuncSetAttribute(walk_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        P3T_CUDA(ctx, cudaFuncSetAttribute(walk_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_set = true;
+    }
+    WalkArgs A;
+    A.body = w.body; A.sorted_idx = w.idx[ctx->cur];
+    A.cell_mac = w.cell_mac; A.cell_mom0 = w.cell_mom0; A.cell_mom1 = w.cell_mom1; A.cell_meta = w.cell_meta;
+    A.accpot = w.accpot; A.nbr_count = w.nbr_count; A.pairs = w.pairs; A.pair_cap = (u64)ctx->nbr_capacity;
+    A.counters = w.counters;
+    if (ctx->ngroup == 64) walk_kernel<2><<<grid, WALK_WARPS * 32, smem, s>>>(A, w.group_start, ctx->prm, w.walk_stack);
+    else walk_kernel<1><<<grid, WALK_WARPS * 32, smem, s>>>(A, w.group_start, ctx->prm, w.walk_stack);
     P3T_CUDA(ctx, cudaGetLastError());
     return P3T_OK;
 }
