@@ -145,10 +145,12 @@ p3t_status p3t_synchronize(p3t_ctx *ctx);
 const char *p3t_last_error(const p3t_ctx *ctx);
 
 /* Calibration of the ALU roofline denominator (not part of the hot path):
- * runs a pure-FFMA kernel (packed = 0: scalar FFMA, 1: packed FFMA2) of `iters` outer
+ * runs a pure-FFMA kernel (packed = 0: scalar FFMA, 1: packed FFMA2; 2, 3, 4: FFMA2 whose sources
+ * are three distinct register pairs / pair x scalar-broadcast + pair / two distinct pairs -- the
+ * register-operand bandwidth test of profiles/ffma2_operand_bandwidth_r1.md) of `iters` outer
  * iterations on the context's stream, synchronises, and returns the best of four timed
  * launches as TFLOP/s (2 flop per fp32 FMA) in *tflops [host] and its duration in *ms
- * [host, nullable].  P3T_EINVAL for null ctx/tflops or iters <= 0. */
+ * [host, nullable].  P3T_EINVAL for null ctx/tflops, iters <= 0 or packed outside 0..4. */
 p3t_status p3t_measure_fp32_peak(p3t_ctx *ctx, int packed, int iters, double *tflops, float *ms);
 
 /* Inspection of intermediate arrays (for the a1-a6 parity tests).  Valid after
@@ -168,7 +170,10 @@ typedef enum {
     P3T_ARR_CELL_PARENT = 10, /* uint32[n_cells] (root: 0xffffffff) */
     P3T_ARR_GROUP_START = 11, /* uint32[n_groups + 1] */
     P3T_ARR_CELL_BMIN   = 12, /* float4[n_cells]: tight AABB min of the cell's bodies */
-    P3T_ARR_CELL_BMAX   = 13  /* float4[n_cells] */
+    P3T_ARR_CELL_BMAX   = 13, /* float4[n_cells] */
+    P3T_ARR_GROUP_STATS = 14  /* uint32[4][n_groups], valid after p3t_eval_soft: p-p list length,
+                                 p-c list length, start and end of the group's walk in ns
+                                 (low 32 bits of %globaltimer) -- load-balance diagnostics */
 } p3t_array;
 p3t_status p3t_array_info(p3t_ctx *ctx, p3t_array which, size_t *count, size_t *elem_bytes);
 p3t_status p3t_copy_array(p3t_ctx *ctx, p3t_array which, void *dst, size_t dst_bytes, int on_device);

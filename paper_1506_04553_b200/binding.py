@@ -36,7 +36,7 @@ SYMBOLS = [
 ARRAYS = dict(root_cube=(0, np.float32, 1), keys=(1, np.uint64, 1), sorted_idx=(2, np.uint32, 1),
               bodies=(3, np.float32, 4), cell_mac=(4, np.float32, 4), cell_mom0=(5, np.float32, 4),
               cell_mom1=(6, np.float32, 4), cell_meta=(7, np.uint32, 2), cell_level=(8, np.uint8, 1),
-              cell_start=(9, np.uint32, 1), cell_parent=(10, np.uint32, 1), group_start=(11, np.uint32, 1),
+              cell_start=(9, np.uint32, 1), cell_parent=(10, np.uint32, 1), group_start=(11, np.uint32, 1), group_stats=(14, np.uint32, 4),
               cell_bmin=(12, np.float32, 4), cell_bmax=(13, np.float32, 4))
 
 
@@ -229,9 +229,10 @@ class P3T:
         self._check(_lib.p3t_synchronize(self._h))
 
     def measure_fp32_peak(self, packed=True, iters=2048):
-        """Pure-FFMA calibration kernel: (TFLOP/s, ms) of the best of four launches."""
+        """Pure-FFMA calibration kernel: (TFLOP/s, ms) of the best of four launches.
+        packed: 0/False scalar FFMA, 1/True FFMA2, 2-4 the FFMA2 operand-pattern variants of include/p3t.h."""
         tf, ms = C.c_double(), C.c_float()
-        self._check(_lib.p3t_measure_fp32_peak(self._h, int(bool(packed)), int(iters), C.byref(tf), C.byref(ms)))
+        self._check(_lib.p3t_measure_fp32_peak(self._h, int(packed), int(iters), C.byref(tf), C.byref(ms)))
         return tf.value, ms.value
 
     def array(self, name):

@@ -31,7 +31,7 @@ size_t p3t_layout(Workspace &ws, char *base, size_t max_n, int key_bits, size_t 
     ws.cell_cap = 3 * n + 1024;
     ws.n_tiles_max = (n + SORT_TILE - 1) / SORT_TILE;
     ws.n_blk_max = (n + BUILD_THREADS - 1) / BUILD_THREADS;
-    ws.walk_warps_max = (size_t)sm_count * 16;   // upper bound of resident walk warps
+    ws.walk_warps_max = (size_t)sm_count * WALK_WARPS * WALK_CTAS;   // upper bound of resident walk warps
     ws.in_mass = b.take<float>(n);
     ws.in_pos = b.take<float>(3 * n);
     ws.body_user = b.take<float4>(n);
@@ -53,6 +53,7 @@ size_t p3t_layout(Workspace &ws, char *base, size_t max_n, int key_bits, size_t 
     ws.blk_level_off = b.take<u32>(ws.n_blk_max * 32);
     ws.level_total = b.take<u32>(64);
     ws.group_start = b.take<u32>(n + 1);
+    ws.group_stats = b.take<uint4>(n);
     ws.cell_mac = b.take<float4>(ws.cell_cap);
     ws.cell_mom0 = b.take<float4>(ws.cell_cap);
     ws.cell_mom1 = b.take<float4>(ws.cell_cap);
@@ -433,6 +434,7 @@ static p3t_status array_desc(p3t_ctx *ctx, p3t_array which, const void **ptr, si
     case P3T_ARR_GROUP_START: *ptr = w.group_start; *count = ng + 1; *elem = 4; break;
     case P3T_ARR_CELL_BMIN:   *ptr = w.cell_bmin; *count = nc; *elem = 16; break;
     case P3T_ARR_CELL_BMAX:   *ptr = w.cell_bmax; *count = nc; *elem = 16; break;
+    case P3T_ARR_GROUP_STATS: *ptr = w.group_stats; *count = ng; *elem = 16; break;
     default: return p3t_fail(ctx, P3T_EINVAL, "unknown array id");
     }
     return P3T_OK;

@@ -24,6 +24,9 @@ typedef unsigned char u8;
 #define SORT_TILE (SORT_THREADS * SORT_ITEMS)
 #define BUILD_THREADS 256
 #define WALK_WARPS 4                 // warps per CTA in the walk kernel
+#ifndef WALK_CTAS
+#define WALK_CTAS 4                  // resident CTAs per SM the walk kernel is compiled for (register budget)
+#endif
 #define WALK_STACK_SMEM 512          // stack entries per warp held in shared memory
 #define WALK_STACK_GMEM 7168         // overflow entries per warp in global memory
 
@@ -81,6 +84,7 @@ struct Workspace {
     u32 *blk_level_off;            // same shape, exclusive over blocks
     u32 *level_total;              // [32]
     u32 *group_start;              // [n+1]
+    uint4 *group_stats;            // [n] per-group diagnostics of the last walk (P3T_ARR_GROUP_STATS)
     // cells
     float4 *cell_mac, *cell_mom0, *cell_mom1, *cell_bmin, *cell_bmax;
     uint2 *cell_meta;

@@ -13,14 +13,29 @@
 // Pair terms:  Eq. 8 (L65) and Eq. 6 (L55) of PAPER.md; cell terms: rule R-QUAD of DESIGN.md.
 #include "p3t_internal.cuh"
 
+#ifdef P3T_WALK_PROFILE
+// sequential attribution of a warp's cycles to phases (diagnostic builds only)
+#define WP_SLOTS 12
+__device__ unsigned long long g_wprof[WP_SLOTS];
+#define WPROF_DECL u32 wp_acc[WP_SLOTS]; for (int k_ = 0; k_ < WP_SLOTS; ++k_) wp_acc[k_] = 0; u32 wp_last = (u32)clock64()
+#define WP(k) do { u32 t_ = (u32)clock64(); wp_acc[k] += t_ - wp_last; wp_last = t_; } while (0)
+#define WPC(k) (++wp_acc[k])
+#else
+#define WPROF_DECL
+#define WP(k)
+#define WPC(k)
+#endif
+
 struct WarpShared {
     u32 stack[WALK_STACK_SMEM];
-    // far ring: every entry is stored with its components duplicated, {x,x,y,y} and {z,z,m,m}, so
-    // that one LDS.128 yields two aligned register pairs for the packed fp32x2 pipe (no MOVs)
-    float4 far_xy[64], far_zm[64];
+    // far ring: (x, y, z, m) of each body, stored once.  The loops use a list entry as the scalar
+    // (broadcast) operand of the packed instructions (SASS: FFMA2 Rd, Rj.F32, Ra.F32x2, Rb.F32x2), so
+    // no duplicated pairs are needed: half the shared-memory traffic of a {x,x,y,y} layout, and a
+    // scalar operand costs one register-file read instead of two (profiles/ffma2_operand_bandwidth_r1.md)
+    float4 far[64];
     float4 near_buf[64];
     u32 near_idx[64];
-    float4 pc[6][64];   // p-c ring: staged cells, duplicated pairs (see stage_pc)
+    float4 pc[3][64];   // p-c ring: staged cells (see stage_pc)
     // landing area of the asynchronous copies (cp.async) of the 32 cells popped for the NEXT walk
     // step: their latency is hidden behind the interaction batches of the current step
     float4 l_mac[32], l_mom0[32], l_mom1[32];
@@ -59,9 +74,6 @@ __device__ __forceinline__ float2 vrsqrt(float2 a) { return make_float2(rsq(a.x)
 template <class V> __device__ __forceinline__ V vdup(float a);
 template <> __device__ __forceinline__ float vdup<float>(float a) { return a; }
 template <> __device__ __forceinline__ float2 vdup<float2>(float a) { return make_float2(a, a); }
-template <class V> __device__ __forceinline__ V vpair(float a, float b);   // a duplicated pair read from shared memory
-template <> __device__ __forceinline__ float vpair<float>(float a, float) { return a; }
-template <> __device__ __forceinline__ float2 vpair<float2>(float a, float b) { return make_float2(a, b); }
 __device__ __forceinline__ float vget(float a, int) { return a; }
 __device__ __forceinline__ float vget(float2 a, int b) { return b ? a.y : a.x; }
 __device__ __forceinline__ float &vref(float &a, int) { return a; }
@@ -116,14 +128,13 @@ __device__ __forceinline__ void stack_write(WarpShared &ws, u32 *gstack, u32 pos
 // ---- p-p, plain softened Newtonian (K = W = 1): 13 FP32-pipe operations per interaction; counted as
 //      23 flop by the convention of DESIGN.md section 8 ---------------------------------------------
 template <int NI>
-__device__ __forceinline__ void pp_body(const float4 &XY, const float4 &ZM, const Targets<NI> &t,
-                                        typename VecOf<NI>::type eps2, Acc<NI> &acc)
+__device__ __forceinline__ void pp_body(const float4 &B, const Targets<NI> &t, typename VecOf<NI>::type eps2, Acc<NI> &acc)
 {
     typedef typename VecOf<NI>::type V;
-    V dx = vadd(vpair<V>(XY.x, XY.y), t.nx), dy = vadd(vpair<V>(XY.z, XY.w), t.ny), dz = vadd(vpair<V>(ZM.x, ZM.y), t.nz);
+    V dx = vadd(vdup<V>(B.x), t.nx), dy = vadd(vdup<V>(B.y), t.ny), dz = vadd(vdup<V>(B.z), t.nz);
     V r2 = vfma(dx, dx, vfma(dy, dy, vfma(dz, dz, eps2)));
     V rinv = vrsqrt(r2);
-    V mrinv = vmul(vpair<V>(ZM.z, ZM.w), rinv);
+    V mrinv = vmul(vdup<V>(B.w), rinv);
     V mr3 = vmul(mrinv, vmul(rinv, rinv));
     acc.ax = vfma(mr3, dx, acc.ax);
     acc.ay = vfma(mr3, dy, acc.ay);
@@ -139,9 +150,9 @@ __device__ __forceinline__ void eval_far(const WarpShared &ws, u32 head, u32 cnt
     const V eps2 = vdup<V>(eps2s);
     if (cnt == 32) {
 #pragma unroll 8
-        for (u32 j = 0; j < 32; ++j) pp_body<NI>(ws.far_xy[head + j], ws.far_zm[head + j], t, eps2, acc);
+        for (u32 j = 0; j < 32; ++j) pp_body<NI>(ws.far[head + j], t, eps2, acc);
     } else {
-        for (u32 j = 0; j < cnt; ++j) pp_body<NI>(ws.far_xy[head + j], ws.far_zm[head + j], t, eps2, acc);
+        for (u32 j = 0; j < cnt; ++j) pp_body<NI>(ws.far[head + j], t, eps2, acc);
     }
     acc.flush();
 }
@@ -160,12 +171,9 @@ __device__ __forceinline__ void stage_pc(WarpShared &ws, u32 slot, const float4 
     float qxx = fmaf(7.5f, q0.y, -tr25), qyy = fmaf(7.5f, q0.z, -tr25), qzz = fmaf(7.5f, q0.w, -tr25);
     float qxy = 7.5f * q1.x, qxz = 7.5f * q1.y, qyz = 7.5f * q1.z;
     float te5 = -tr25 * eps2, m08 = 0.8f * q0.x;
-    ws.pc[0][slot] = make_float4(a.x, a.x, a.y, a.y);
-    ws.pc[1][slot] = make_float4(a.z, a.z, q0.x, q0.x);
-    ws.pc[2][slot] = make_float4(qxx, qxx, qyy, qyy);
-    ws.pc[3][slot] = make_float4(qzz, qzz, qxy, qxy);
-    ws.pc[4][slot] = make_float4(qxz, qxz, qyz, qyz);
-    ws.pc[5][slot] = make_float4(te5, te5, m08, m08);
+    ws.pc[0][slot] = make_float4(a.x, a.y, a.z, q0.x);
+    ws.pc[1][slot] = make_float4(qxx, qyy, qzz, qxy);
+    ws.pc[2][slot] = make_float4(qxz, qyz, te5, m08);
 }
 
 template <int NI>
@@ -176,11 +184,11 @@ __device__ __forceinline__ void eval_pc(const WarpShared &ws, u32 head, u32 cnt,
 #pragma unroll 4
     for (u32 j = 0; j < cnt; ++j) {
         const u32 e = head + j;
-        const float4 P0 = ws.pc[0][e], P1 = ws.pc[1][e], P2 = ws.pc[2][e], P3 = ws.pc[3][e], P4 = ws.pc[4][e], P5 = ws.pc[5][e];
-        const V M = vpair<V>(P1.z, P1.w);
-        const V qxx = vpair<V>(P2.x, P2.y), qyy = vpair<V>(P2.z, P2.w), qzz = vpair<V>(P3.x, P3.y);
-        const V qxy = vpair<V>(P3.z, P3.w), qxz = vpair<V>(P4.x, P4.y), qyz = vpair<V>(P4.z, P4.w);
-        V dx = vadd(vpair<V>(P0.x, P0.y), t.nx), dy = vadd(vpair<V>(P0.z, P0.w), t.ny), dz = vadd(vpair<V>(P1.x, P1.y), t.nz);
+        const float4 P0 = ws.pc[0][e], P1 = ws.pc[1][e], P2 = ws.pc[2][e];
+        const V M = vdup<V>(P0.w);
+        const V qxx = vdup<V>(P1.x), qyy = vdup<V>(P1.y), qzz = vdup<V>(P1.z);
+        const V qxy = vdup<V>(P1.w), qxz = vdup<V>(P2.x), qyz = vdup<V>(P2.y);
+        V dx = vadd(vdup<V>(P0.x), t.nx), dy = vadd(vdup<V>(P0.y), t.ny), dz = vadd(vdup<V>(P0.z), t.nz);
         V r2 = vfma(dx, dx, vfma(dy, dy, vfma(dz, dz, eps2)));
         V rinv = vrsqrt(r2);
         V r2i = vmul(rinv, rinv);
@@ -190,9 +198,9 @@ __device__ __forceinline__ void eval_pc(const WarpShared &ws, u32 head, u32 cnt,
         V qdx = vfma(qxx, dx, vfma(qxy, dy, vmul(qxz, dz)));
         V qdy = vfma(qxy, dx, vfma(qyy, dy, vmul(qyz, dz)));
         V qdz = vfma(qxz, dx, vfma(qyz, dy, vmul(qzz, dz)));
-        V T = vfma(dx, qdx, vfma(dy, qdy, vfma(dz, qdz, vpair<V>(P5.x, P5.y))));
+        V T = vfma(dx, qdx, vfma(dy, qdy, vfma(dz, qdz, vdup<V>(P2.z))));
         V c1 = vfma(T, r4i, M);
-        V pphi = vfma(c02, c1, vpair<V>(P5.z, P5.w));
+        V pphi = vfma(c02, c1, vdup<V>(P2.w));
         V coef = vmul(c1, r3i);
         acc.ph = vfma(pphi, rinv, acc.ph);
         acc.ax = vfma(coef, dx, vfma(n5, qdx, acc.ax));
@@ -247,6 +255,13 @@ __device__ __forceinline__ void eval_near(const WarpShared &ws, u32 head, u32 cn
     acc.flush();
 }
 
+__device__ __forceinline__ u64 globaltimer_ns()
+{
+    u64 t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+
 // Arguments of the walk that do not change between groups.
 struct WalkArgs {
     const float4 *__restrict__ body;
@@ -255,6 +270,7 @@ struct WalkArgs {
     const uint2 *__restrict__ cell_meta;
     float4 *__restrict__ accpot;
     u32 *__restrict__ nbr_count;
+    uint4 *__restrict__ group_stats;
     uint2 *pairs;
     u64 pair_cap;
     u64 *counters;
@@ -285,6 +301,7 @@ __device__ __forceinline__ void walk_group(WarpShared &ws, u32 *gstack, const Wa
                                            u32 lane, u64 &tot_pp, u64 &tot_pc, u64 &tot_near)
 {
     const u32 gcount = ge - gs;
+    WPROF_DECL;
     // ---- my bodies; empty slots replicate the group's first body and are flagged dead
     Targets<NI> tg;
     u32 isorted[NI], iuser[NI], nnb[NI];
@@ -313,6 +330,7 @@ __device__ __forceinline__ void walk_group(WarpShared &ws, u32 *gstack, const Wa
     Acc<NI> acc;
     acc.zero();
     tg.seal();
+    WP(9);
 
     u32 top = 1;
     if (lane == 0) ws.stack[0] = 0;   // root
@@ -324,7 +342,9 @@ __device__ __forceinline__ void walk_group(WarpShared &ws, u32 *gstack, const Wa
     u32 take = pop_cells(ws, gstack, A, top, lane, cell);
     while (take > 0) {
         const bool have = lane < take;
+        WP(8);
         cp_async_wait_all();
+        WP(2); WPC(10);
         // ---- consume the landed records: acceptance test (R-MAC, folded radius of moments.cu)
         bool accept = false;
         u32 nch = 0, first = 0, lcount = 0, lstart = 0;
@@ -349,6 +369,7 @@ __device__ __forceinline__ void walk_group(WarpShared &ws, u32 *gstack, const Wa
                 stage_pc(ws, (pc_head + pc_cnt + __popc(ab & lanemask_lt())) & 63u, a, ws.l_mom0[lane], ws.l_mom1[lane], prm.eps2);
             pc_cnt += __popc(ab);
         }
+        WP(3);
         // ---- children of opened internal cells -> stack
         {
             u32 inc = nch;
@@ -366,6 +387,7 @@ __device__ __forceinline__ void walk_group(WarpShared &ws, u32 *gstack, const Wa
         __syncwarp();
         // ---- request the records of the next step before any interaction work
         take = top > 0 ? pop_cells(ws, gstack, A, top, lane, cell) : 0u;
+        WP(4);
         // ---- bodies of opened leaves -> near / far rings; the next chunk of 32 bodies is loaded
         //      while the current one is tested and (when a ring fills) evaluated
         {
@@ -397,6 +419,7 @@ __device__ __forceinline__ void walk_group(WarpShared &ws, u32 *gstack, const Wa
             bool hv = false, hvn = false;
             if (total) fetch(0, bj, bidx, hv);
             for (u32 v0 = 0; v0 < total; v0 += 32) {
+                WPC(11);
                 hvn = false;
                 if (v0 + 32 < total) fetch(v0 + 32, bn, bidxn, hvn);
                 float ex = fmaxf(0.f, fmaxf(lo[0] - bj.x, bj.x - hi[0]));
@@ -408,8 +431,7 @@ __device__ __forceinline__ void walk_group(WarpShared &ws, u32 *gstack, const Wa
                 u32 fb = __ballot_sync(0xffffffffu, isfar), nb = __ballot_sync(0xffffffffu, isnear);
                 if (isfar) {
                     u32 slot = (far_head + far_cnt + __popc(fb & lanemask_lt())) & 63u;
-                    ws.far_xy[slot] = make_float4(bj.x, bj.x, bj.y, bj.y);
-                    ws.far_zm[slot] = make_float4(bj.z, bj.z, bj.w, bj.w);
+                    ws.far[slot] = bj;
                 }
                 if (isnear) {
                     u32 slot = (near_head + near_cnt + __popc(nb & lanemask_lt())) & 63u;
@@ -420,12 +442,16 @@ __device__ __forceinline__ void walk_group(WarpShared &ws, u32 *gstack, const Wa
                 near_cnt += __popc(nb);
                 __syncwarp();
                 if (far_cnt >= 32) {
+                    WP(5);
                     eval_far<NI>(ws, far_head, 32, tg, prm.eps2, acc);
+                    WP(0);
                     far_head = (far_head + 32) & 63u; far_cnt -= 32; n_far += 32;
                 }
                 if (near_cnt >= 32) {
+                    WP(5);
                     eval_near<NI>(ws, near_head, 32, tg, isorted, iuser, prm, A.sorted_idx, A.pairs, A.pair_cap, A.counters, nnb,
                                   acc, lane);
+                    WP(6);
                     near_head = (near_head + 32) & 63u; near_cnt -= 32; n_near += 32;
                 }
                 __syncwarp();
@@ -434,12 +460,15 @@ __device__ __forceinline__ void walk_group(WarpShared &ws, u32 *gstack, const Wa
         }
         // ---- a full batch of accepted cells
         if (pc_cnt >= 32) {
+            WP(5);
             eval_pc<NI>(ws, pc_head, 32, tg, prm.eps2, acc);
+            WP(1);
             pc_head = (pc_head + 32) & 63u; pc_cnt -= 32; n_pc += 32;
             __syncwarp();
         }
     }
     cp_async_wait_all();
+    WP(5);
     if (overflow) {
         if (lane == 0) atomicOr(&A.counters[CNT_ERR_EVAL], (u64)ERR_STACK_OVERFLOW);
     }
@@ -460,6 +489,10 @@ __device__ __forceinline__ void walk_group(WarpShared &ws, u32 *gstack, const Wa
             A.nbr_count[iuser[b]] = nnb[b];
         }
     }
+#ifdef P3T_WALK_PROFILE
+    WP(7);
+    if (lane == 0) for (int k_ = 0; k_ < WP_SLOTS; ++k_) atomicAdd(&g_wprof[k_], (unsigned long long)wp_acc[k_]);
+#endif
     // each live body met itself once on the near path (distance 0 to its own group's box)
     tot_pp += (u64)(n_far + n_near) * gcount - gcount;
     tot_near += (u64)n_near * gcount - gcount;
@@ -469,7 +502,7 @@ __device__ __forceinline__ void walk_group(WarpShared &ws, u32 *gstack, const Wa
 // Persistent grid: 148 SMs x 4 CTAs x 4 warps; groups are handed out by an atomic ticket.  A group
 // of at most 32 bodies takes the one-body-per-lane path (half the FP32 work of the packed path).
 template <int NIMAX>
-__global__ void __launch_bounds__(WALK_WARPS * 32, 16 / WALK_WARPS)
+__global__ void __launch_bounds__(WALK_WARPS * 32, WALK_CTAS)
 walk_kernel(WalkArgs A, const u32 *__restrict__ group_start, P3TParams prm, u32 *walk_stack)
 {
     extern __shared__ __align__(16) unsigned char s_raw[];
@@ -485,9 +518,14 @@ walk_kernel(WalkArgs A, const u32 *__restrict__ group_start, P3TParams prm, u32 
         g = __shfl_sync(0xffffffffu, g, 0);
         if (g >= ngroups) break;
         const u32 gs = group_start[g], ge = group_start[g + 1];
+        const u64 pp0 = tot_pp, pc0 = tot_pc;
+        const u32 t0 = (u32)globaltimer_ns();
         if (NIMAX == 2 && ge - gs > 32) walk_group<2>(ws, gstack, A, prm, gs, ge, lane, tot_pp, tot_pc, tot_near);
         else walk_group<1>(ws, gstack, A, prm, gs, ge, lane, tot_pp, tot_pc, tot_near);
         __syncwarp();
+        if (lane == 0)   // list lengths of this group (+1: the self term removed from tot_pp) and its time window
+            A.group_stats[g] = make_uint4((u32)((tot_pp - pp0) / (ge - gs)) + 1u, (u32)((tot_pc - pc0) / (ge - gs)), t0,
+                                          (u32)globaltimer_ns());
     }
     if (lane == 0) {
         atomicAdd(&A.counters[CNT_NPP], tot_pp);
@@ -496,12 +534,22 @@ walk_kernel(WalkArgs A, const u32 *__restrict__ group_start, P3TParams prm, u32 
     }
 }
 
+#ifdef P3T_WALK_PROFILE
+extern "C" void p3t_debug_wprof(unsigned long long *out)
+{
+    cudaDeviceSynchronize();
+    cudaMemcpyFromSymbol(out, g_wprof, sizeof(g_wprof));
+    unsigned long long z[WP_SLOTS] = {0};
+    cudaMemcpyToSymbol(g_wprof, z, sizeof(z));
+}
+#endif
+
 p3t_status p3t_stage_walk(p3t_ctx *ctx)
 {
     Workspace &w = ctx->ws;
     cudaStream_t s = ctx->stream;
     P3T_CUDA(ctx, cudaMemsetAsync(w.counters, 0, 8 * sizeof(u64), s));   // eval counters
-    u32 grid = (u32)ctx->sm_count * (16 / WALK_WARPS);
+    u32 grid = (u32)ctx->sm_count * WALK_CTAS;
     if ((size_t)grid * WALK_WARPS > w.walk_warps_max) grid = (u32)(w.walk_warps_max / WALK_WARPS);
     const size_t smem = sizeof(WarpShared) * WALK_WARPS;
     static bool attr_set = false;
@@ -513,7 +561,7 @@ p3t_status p3t_stage_walk(p3t_ctx *ctx)
     WalkArgs A;
     A.body = w.body; A.sorted_idx = w.idx[ctx->cur];
     A.cell_mac = w.cell_mac; A.cell_mom0 = w.cell_mom0; A.cell_mom1 = w.cell_mom1; A.cell_meta = w.cell_meta;
-    A.accpot = w.accpot; A.nbr_count = w.nbr_count; A.pairs = w.pairs; A.pair_cap = (u64)ctx->nbr_capacity;
+    A.accpot = w.accpot; A.nbr_count = w.nbr_count; A.group_stats = w.group_stats; A.pairs = w.pairs; A.pair_cap = (u64)ctx->nbr_capacity;
     A.counters = w.counters;
     if (ctx->ngroup == 64) walk_kernel<2><<<grid, WALK_WARPS * 32, smem, s>>>(A, w.group_start, ctx->prm, w.walk_stack);
     else walk_kernel<1><<<grid, WALK_WARPS * 32, smem, s>>>(A, w.group_start, ctx->prm, w.walk_stack);
