@@ -30,7 +30,7 @@ size_t p3t_layout(Workspace &ws, char *base, size_t max_n, int key_bits, size_t 
     size_t n = max_n;
     ws.cell_cap = 3 * n + 1024;
     ws.n_tiles_max = (n + SORT_TILE - 1) / SORT_TILE;
-    ws.n_blk_max = (n + BUILD_THREADS - 1) / BUILD_THREADS;
+    ws.n_blk_max = (n + BUILD_TILE - 1) / BUILD_TILE;
     ws.walk_warps_max = (size_t)sm_count * WALK_WARPS * WALK_CTAS;   // upper bound of resident walk warps
     ws.in_mass = b.take<float>(n);
     ws.in_pos = b.take<float>(3 * n);
@@ -42,15 +42,12 @@ size_t p3t_layout(Workspace &ws, char *base, size_t max_n, int key_bits, size_t 
     ws.idx[0] = b.take<u32>(n);
     ws.idx[1] = b.take<u32>(n);
     ws.hist = b.take<u32>(8 * 256);
-    ws.tile_status = b.take<u32>(8 * ws.n_tiles_max * 256);
+    ws.tile_status = b.take<u32>(2 * (ws.n_tiles_max + 64) * 256);   // + sentinel rows (sort.cu)
     ws.body = b.take<float4>(n);
     ws.clev = b.take<signed char>(n + 2);
-    ws.dlev = b.take<u8>(n);
-    ws.cutflag = b.take<u8>(n);
-    ws.glev = b.take<u8>(n);
-    ws.head_status = b.take<u32>(ws.n_blk_max);
-    ws.blk_level_cnt = b.take<u32>(ws.n_blk_max * 32);
-    ws.blk_level_off = b.take<u32>(ws.n_blk_max * 32);
+    ws.dlev = b.take<u8>(n + 4);
+    ws.cutflag = b.take<u8>(n + 4);
+    ws.build_tiles = b.take<uint4>(ws.n_blk_max * 8);
     ws.level_total = b.take<u32>(64);
     ws.group_start = b.take<u32>(n + 1);
     ws.group_stats = b.take<uint4>(n);

@@ -19,10 +19,11 @@ typedef unsigned char u8;
 #define P3T_NO_PARENT 0xffffffffu
 
 // ---- tuning constants -------------------------------------------------
-#define SORT_THREADS 256
+#define SORT_THREADS 512
 #define SORT_ITEMS 8
 #define SORT_TILE (SORT_THREADS * SORT_ITEMS)
 #define BUILD_THREADS 256
+#define BUILD_TILE 1024               // bodies per CTA of the build kernels (4 per thread)
 #define WALK_WARPS 4                 // warps per CTA in the walk kernel
 #ifndef WALK_CTAS
 #define WALK_CTAS 4                  // resident CTAs per SM the walk kernel is compiled for (register budget)
@@ -72,16 +73,13 @@ struct Workspace {
     u64 *keys[2];
     u32 *idx[2];
     u32 *hist;                     // [8][256] digit histograms -> exclusive offsets
-    u32 *tile_status;              // [8][ntiles][256]
+    u32 *tile_status;              // [2][ntiles][256] look-back words, ping-pong between passes
     float4 *body;                  // sorted
     // a5
     signed char *clev;             // [n+1]  common-prefix levels between sorted neighbours (c[0] = -1)
     u8 *dlev;                      // [n] leaf level of each body
     u8 *cutflag;                   // [n] segment cut (group construction)
-    u8 *glev;                      // [n] natural group level of each body
-    u32 *head_status;              // [nblk] look-back words of the group-head compaction
-    u32 *blk_level_cnt;            // [nblk][32]: nodes per level starting in the block
-    u32 *blk_level_off;            // same shape, exclusive over blocks
+    void *build_tiles;             // [nblk] 128-byte tile records of build.cu (node counts per level, cuts, heads)
     u32 *level_total;              // [32]
     u32 *group_start;              // [n+1]
     uint4 *group_stats;            // [n] per-group diagnostics of the last walk (P3T_ARR_GROUP_STATS)
@@ -112,6 +110,7 @@ struct p3t_ctx {
     int key_bits, max_level, nleaf, ngroup, merge_levels;
     int sm_count;
     bool have_params, loaded, built, evaluated;
+    bool status_clean;             // the look-back buffers have been zeroed once (they clean themselves afterwards)
     int cur;                       // which of keys[2]/idx[2] holds the sorted result
     P3TParams prm;
     float eps, theta, r_in, r_out, r_search;

@@ -113,8 +113,8 @@ __device__ __forceinline__ void root_cube(const u32 *bbox_bits, float &minx, flo
 }
 
 __global__ void __launch_bounds__(256) keys_hist_kernel(const float4 *__restrict__ body, const u32 *__restrict__ bbox_bits,
-                                                        float *cube, u64 *__restrict__ keys, u32 *__restrict__ idx,
-                                                        u32 *hist, u32 n, int max_level, int passes)
+                                                        float *cube, u64 *__restrict__ keys, u32 *hist, u32 n,
+                                                        int max_level, int passes)
 {
     __shared__ u32 s_hist[8 * 256];
     for (int t = threadIdx.x; t < 8 * 256; t += blockDim.x) s_hist[t] = 0;
@@ -131,7 +131,6 @@ __global__ void __launch_bounds__(256) keys_hist_kernel(const float4 *__restrict
         u32 qz = min((u32)fmaxf((b.z - minz) * scale, 0.f), qmax);
         u64 key = (spread3(qx) << 2) | (spread3(qy) << 1) | spread3(qz);
         keys[i] = key;
-        idx[i] = i;
         for (int p = 0; p < passes; ++p) atomicAdd(&s_hist[p * 256 + (u32)((key >> (8 * p)) & 255u)], 1u);
     }
     __syncthreads();
@@ -141,142 +140,185 @@ __global__ void __launch_bounds__(256) keys_hist_kernel(const float4 *__restrict
     }
 }
 
-// exclusive scan of each pass's 256-bin histogram (one block per pass)
-__global__ void __launch_bounds__(256) hist_scan_kernel(u32 *hist)
-{
-    __shared__ u32 s_w[8];
-    u32 *h = hist + blockIdx.x * 256;
-    u32 v = h[threadIdx.x];
-    u32 lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    u32 inc = v;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        u32 t = __shfl_up_sync(0xffffffffu, inc, o);
-        if (lane >= o) inc += t;
-    }
-    if (lane == 31) s_w[warp] = inc;
-    __syncthreads();
-    u32 base = 0;
-    for (u32 w = 0; w < warp; ++w) base += s_w[w];
-    h[threadIdx.x] = base + inc - v;
-}
-
 // ------------------------------------------------------------------------------------------------
-// a3: one onesweep pass: stable 8-bit digit partition with decoupled look-back over tiles
+// a3: one onesweep pass: stable 8-bit digit partition, chained over tiles by decoupled look-back
 // ------------------------------------------------------------------------------------------------
+// A tile is SORT_TILE consecutive keys, taken in ticket order (so every predecessor of a running tile
+// is running or done).  Per tile and bin one status word (flag | count) is published twice: the tile's
+// own count (AGG) as soon as it is known, the inclusive prefix (INC) once the look-back has reached
+// an INC word.  All tiles of a 1M-body pass are resident at once and publish their AGG words at about
+// the same time, so a look-back that reads one predecessor per L2 round trip needs ~sqrt(2 tiles)
+// dependent round trips (measured 35 us per pass); here every thread keeps SORT_LOOKBACK loads in
+// flight and consumes them in order, which divides the number of round trips by sqrt(SORT_LOOKBACK).
+// The status words of pass p live in buffer p & 1; every tile also zeroes its row of the other
+// buffer, which the next pass uses, so no memset runs between passes or between builds.
 #define OS_FLAG_AGG 0x40000000u
 #define OS_FLAG_INC 0x80000000u
 #define OS_VAL_MASK 0x3fffffffu
+#define SORT_LOOKBACK 8
 
-__global__ void __launch_bounds__(SORT_THREADS) onesweep_kernel(const u64 *__restrict__ kin, const u32 *__restrict__ vin,
-                                                                u64 *__restrict__ kout, u32 *__restrict__ vout, u32 n,
-                                                                int shift, const u32 *__restrict__ gbase,
-                                                                volatile u32 *status, u64 *ticket)
+__device__ __forceinline__ u32 ld_status(const u32 *p)
 {
-    __shared__ u32 s_whist[SORT_THREADS / 32][256];
-    __shared__ u32 s_binstart[256];
-    __shared__ u32 s_goff[256];
-    __shared__ u32 s_wsum[8];
-    __shared__ u32 s_tile;
-    __shared__ u64 s_key[SORT_TILE];
-    __shared__ u32 s_val[SORT_TILE];
+    u32 v;
+    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_status(u32 *p, u32 v)
+{
+    asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
 
+__global__ void fill_u32_kernel(u32 *p, u32 v) { p[blockIdx.x * blockDim.x + threadIdx.x] = v; }
+
+struct OnesweepSmem {
+    union {
+        u32 whist[SORT_THREADS / 32][256];                      // ranking: per-warp digit counts
+        struct { u64 key[SORT_TILE]; u32 val[SORT_TILE]; } x;   // exchange: the tile in digit order
+    };
+    u32 binstart[256];   // first local position of each bin
+    u32 goff[256];       // global position of local position 0 of each bin, minus binstart
+    u32 wsum[8];
+    u32 tile;
+};
+
+// status rows -SORT_LOOKBACK..-1 (in front of row 0) permanently hold INC | 0, so the look-back
+// window never needs a bounds check
+__global__ void __launch_bounds__(SORT_THREADS, 2) onesweep_kernel(const u64 *__restrict__ kin, const u32 *__restrict__ vin,
+                                                                   u64 *__restrict__ kout, u32 *__restrict__ vout, u32 n,
+                                                                   int shift, const u32 *__restrict__ ghist, u32 *status,
+                                                                   u32 *status_next, u64 *ticket)
+{
+    extern __shared__ __align__(16) unsigned char os_raw[];
+    OnesweepSmem &sm = *reinterpret_cast<OnesweepSmem *>(os_raw);
     const u32 tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    if (tid == 0) s_tile = (u32)atomicAdd(ticket, 1ull);
-    for (u32 t = tid; t < (SORT_THREADS / 32) * 256; t += SORT_THREADS) (&s_whist[0][0])[t] = 0;
+    if (tid == 0) sm.tile = (u32)atomicAdd(ticket, 1ull);
+#pragma unroll
+    for (u32 t = 0; t < 8; ++t) sm.whist[warp][t * 32 + lane] = 0;
     __syncthreads();
-    const u32 tile = s_tile;
+    const u32 tile = sm.tile;
     const u32 tile_base = tile * SORT_TILE;
     const u32 tile_valid = min((u32)SORT_TILE, n - tile_base);
+    if (tid < 256) status_next[(size_t)tile * 256 + tid] = 0;   // row of the buffer the next pass uses
 
     u64 key[SORT_ITEMS];
-    u32 val[SORT_ITEMS], rnk[SORT_ITEMS];
+    u32 val[SORT_ITEMS], pos[SORT_ITEMS];
     const u32 wbase = tile_base + warp * (SORT_ITEMS * 32);
 #pragma unroll
     for (int k = 0; k < SORT_ITEMS; ++k) {
         u32 i = wbase + k * 32 + lane;
         bool ok = i < n;
-        key[k] = ok ? kin[i] : ~0ull;
-        val[k] = ok ? vin[i] : 0u;
+        key[k] = ok ? kin[i] : ~0ull;       // padding keys have digit 255 and rank behind every real key
+        val[k] = ok ? (vin ? vin[i] : i) : 0u;
     }
-    // stable rank inside the warp: items in (k, lane) order
+    // global base of every bin: exclusive scan of this pass's histogram (256 counts)
+    u32 gcount = 0, ginc = 0;
+    if (tid < 256) {
+        gcount = ghist[tid];
+        ginc = gcount;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            u32 t = __shfl_up_sync(0xffffffffu, ginc, o);
+            if (lane >= o) ginc += t;
+        }
+        if (lane == 31) sm.wsum[warp] = ginc;
+    }
+    // stable rank inside the warp, items in (k, lane) order.  The peer masks of all items are found
+    // first; the per-warp counters are then advanced by the leaders in item order (shared-memory
+    // atomics of one warp execute in program order), so the eight rounds pipeline instead of
+    // forming a chain of match -> load -> store -> shuffle latencies.
+    u32 peers[SORT_ITEMS];
+#pragma unroll
+    for (int k = 0; k < SORT_ITEMS; ++k) peers[k] = __match_any_sync(0xffffffffu, (u32)(key[k] >> shift) & 255u);
 #pragma unroll
     for (int k = 0; k < SORT_ITEMS; ++k) {
-        u32 i = wbase + k * 32 + lane;
-        bool ok = i < n;
-        u32 active = __ballot_sync(0xffffffffu, ok);
-        rnk[k] = 0;
-        if (ok) {
-            u32 d = (u32)(key[k] >> shift) & 255u;
-            u32 peers = __match_any_sync(active, d);
-            int leader = __ffs(peers) - 1;
-            u32 pre = 0;
-            if ((int)lane == leader) {
-                pre = s_whist[warp][d];
-                s_whist[warp][d] = pre + __popc(peers);
-            }
-            pre = __shfl_sync(peers, pre, leader);
-            rnk[k] = pre + __popc(peers & lanemask_lt());
-        }
-        __syncwarp();
+        u32 d = (u32)(key[k] >> shift) & 255u;
+        pos[k] = 0;
+        if ((peers[k] & lanemask_lt()) == 0) pos[k] = atomicAdd(&sm.whist[warp][d], (u32)__popc(peers[k]));
+        __syncwarp();   // round k's updates are ordered before round k+1's (different lanes may lead the same digit)
     }
-    __syncthreads();
-    // bin = tid: exclusive over warps, tile total
-    u32 sum = 0;
 #pragma unroll
-    for (int w = 0; w < SORT_THREADS / 32; ++w) {
-        u32 t = s_whist[w][tid];
-        s_whist[w][tid] = sum;
-        sum += t;
+    for (int k = 0; k < SORT_ITEMS; ++k)
+        pos[k] = __shfl_sync(0xffffffffu, pos[k], __ffs(peers[k]) - 1) + __popc(peers[k] & lanemask_lt());
+    __syncthreads();
+    // threads 0..255 own one bin each: exclusive over warps, tile total, publish, look back
+    u32 sum = 0, gbase = 0;
+    if (tid < 256) {
+        for (u32 w = 0; w < warp; ++w) gbase += sm.wsum[w];
+        gbase += ginc - gcount;
+#pragma unroll
+        for (int w = 0; w < SORT_THREADS / 32; ++w) {
+            u32 t = sm.whist[w][tid];
+            sm.whist[w][tid] = sum;
+            sum += t;
+        }
+        if (tid == 255) sum -= SORT_TILE - tile_valid;   // padding keys are not part of the data
+        st_status(status + (size_t)tile * 256 + tid, sum | (tile == 0 ? OS_FLAG_INC : OS_FLAG_AGG));
     }
-    volatile u32 *my_status = status + (size_t)tile * 256 + tid;
-    *my_status = sum | (tile == 0 ? OS_FLAG_INC : OS_FLAG_AGG);
-    // exclusive scan of the 256 bin totals inside the block
+    __syncthreads();          // wsum is read above, rewritten below
     u32 inc = sum;
+    if (tid < 256) {
 #pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        u32 t = __shfl_up_sync(0xffffffffu, inc, o);
-        if (lane >= o) inc += t;
-    }
-    if (lane == 31) s_wsum[warp] = inc;
-    __syncthreads();
-    u32 wb = 0;
-    for (u32 w = 0; w < warp; ++w) wb += s_wsum[w];
-    u32 binstart = wb + inc - sum;
-    s_binstart[tid] = binstart;
-    // decoupled look-back
-    u32 excl = 0;
-    if (tile > 0) {
-        int t = (int)tile - 1;
-        while (true) {
-            u32 v = status[(size_t)t * 256 + tid];
-            if ((v & (OS_FLAG_AGG | OS_FLAG_INC)) == 0) continue;
-            excl += v & OS_VAL_MASK;
-            if (v & OS_FLAG_INC) break;
-            --t;
+        for (int o = 1; o < 32; o <<= 1) {
+            u32 t = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= o) inc += t;
         }
-        *my_status = (excl + sum) | OS_FLAG_INC;
+        if (lane == 31) sm.wsum[warp] = inc;
     }
-    s_goff[tid] = gbase[tid] + excl - binstart;
     __syncthreads();
-    // scatter into shared memory in sorted order
+    if (tid < 256) {
+        u32 wb = 0;
+        for (u32 w = 0; w < warp; ++w) wb += sm.wsum[w];
+        const u32 binstart = wb + inc - sum;
+        sm.binstart[tid] = binstart;
+        u32 excl = 0;
+        if (tile > 0) {
+            const u32 *p = status + (size_t)(tile - 1) * 256 + tid;
+            bool done = false;
+            while (!done) {
+                u32 v[SORT_LOOKBACK];
+#pragma unroll
+                for (int k = 0; k < SORT_LOOKBACK; ++k) v[k] = ld_status(p - k * 256);
+                bool go = true;
+                u32 used = 0;
+#pragma unroll
+                for (int k = 0; k < SORT_LOOKBACK; ++k) {
+                    const bool ready = v[k] >= OS_FLAG_AGG, isinc = v[k] >= OS_FLAG_INC;
+                    if (go && ready) { excl += v[k] & OS_VAL_MASK; ++used; }
+                    done = done || (go && isinc);
+                    go = go && ready && !isinc;
+                }
+                p -= used * 256;
+            }
+            st_status(status + (size_t)tile * 256 + tid, (excl + sum) | OS_FLAG_INC);
+        }
+        sm.goff[tid] = gbase + excl - binstart;
+    }
+    __syncthreads();
+    // final local position of every item (the per-warp counts are dead after this)
 #pragma unroll
     for (int k = 0; k < SORT_ITEMS; ++k) {
-        u32 i = wbase + k * 32 + lane;
-        if (i < n) {
-            u32 d = (u32)(key[k] >> shift) & 255u;
-            u32 p = s_binstart[d] + s_whist[warp][d] + rnk[k];
-            s_key[p] = key[k];
-            s_val[p] = val[k];
+        u32 d = (u32)(key[k] >> shift) & 255u;
+        pos[k] += sm.binstart[d] + sm.whist[warp][d];
+    }
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < SORT_ITEMS; ++k) {
+        if (pos[k] < tile_valid) {       // padding keys sit behind the valid ones
+            sm.x.key[pos[k]] = key[k];
+            sm.x.val[pos[k]] = val[k];
         }
     }
     __syncthreads();
-    for (u32 p = tid; p < tile_valid; p += SORT_THREADS) {
-        u64 kk = s_key[p];
-        u32 d = (u32)(kk >> shift) & 255u;
-        u32 dst = s_goff[d] + p;
-        kout[dst] = kk;
-        vout[dst] = s_val[p];
+#pragma unroll
+    for (int k = 0; k < SORT_ITEMS; ++k) {
+        u32 p = k * SORT_THREADS + tid;
+        if (p < tile_valid) {
+            u64 kk = sm.x.key[p];
+            u32 d = (u32)(kk >> shift) & 255u;
+            u32 dst = sm.goff[d] + p;
+            kout[dst] = kk;
+            vout[dst] = sm.x.val[p];
+        }
     }
 }
 
@@ -312,18 +354,29 @@ p3t_status p3t_stage_sort(p3t_ctx *ctx)
     cudaStream_t s = ctx->stream;
     int passes = (3 * ctx->max_level + 7) / 8;   // 8 for 63-bit keys, 4 for 30-bit keys
     u32 ntiles = div_up(n, SORT_TILE);
+    static bool attr_set = false;
+    if (!attr_set) {
+        P3T_CUDA(ctx, cudaFuncSetAttribute(onesweep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(OnesweepSmem)));
+        attr_set = true;
+    }
+    const size_t status_rows = w.n_tiles_max + SORT_LOOKBACK;   // SORT_LOOKBACK sentinel rows in front of row 0
+    if (!ctx->status_clean) {   // first build of this context: buffers zeroed, sentinel rows = INC | 0 
+        P3T_CUDA(ctx, cudaMemsetAsync(w.tile_status, 0, 2 * status_rows * 256 * sizeof(u32), s));
+        for (int b = 0; b < 2; ++b)
+            fill_u32_kernel<<<SORT_LOOKBACK, 256, 0, s>>>(w.tile_status + b * status_rows * 256, OS_FLAG_INC);
+        ctx->status_clean = true;
+    }
     P3T_CUDA(ctx, cudaMemsetAsync(w.counters + CNT_NCELLS, 0, 16 * sizeof(u64), s));   // build counters + sort tickets
     P3T_CUDA(ctx, cudaMemsetAsync(w.hist, 0, 8 * 256 * sizeof(u32), s));
-    P3T_CUDA(ctx, cudaMemsetAsync(w.tile_status, 0, (size_t)passes * ntiles * 256 * sizeof(u32), s));
     u32 grid = min(div_up(n, 256 * 4), (u32)ctx->sm_count * 8);
-    keys_hist_kernel<<<grid, 256, 0, s>>>(w.body_user, w.bbox_bits, w.cube, w.keys[0], w.idx[0], w.hist, n,
-                                          ctx->max_level, passes);
-    hist_scan_kernel<<<passes, 256, 0, s>>>(w.hist);
+    keys_hist_kernel<<<grid, 256, 0, s>>>(w.body_user, w.bbox_bits, w.cube, w.keys[0], w.hist, n, ctx->max_level, passes);
     int cur = 0;
     for (int p = 0; p < passes; ++p) {
-        onesweep_kernel<<<ntiles, SORT_THREADS, 0, s>>>(w.keys[cur], w.idx[cur], w.keys[cur ^ 1], w.idx[cur ^ 1], n, 8 * p,
-                                                        w.hist + p * 256, w.tile_status + (size_t)p * ntiles * 256,
-                                                        w.counters + CNT_SORT_TICKET + p);
+        u32 *st_cur = w.tile_status + ((size_t)(p & 1) * status_rows + SORT_LOOKBACK) * 256;
+        u32 *st_next = w.tile_status + ((size_t)((p + 1) & 1) * status_rows + SORT_LOOKBACK) * 256;
+        onesweep_kernel<<<ntiles, SORT_THREADS, sizeof(OnesweepSmem), s>>>(w.keys[cur], p == 0 ? nullptr : w.idx[cur], w.keys[cur ^ 1],
+                                                                           w.idx[cur ^ 1], n, 8 * p, w.hist + p * 256, st_cur, st_next,
+                                                                           w.counters + CNT_SORT_TICKET + p);
         cur ^= 1;
     }
     ctx->cur = cur;
