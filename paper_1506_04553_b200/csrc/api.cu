@@ -44,11 +44,12 @@ size_t p3t_layout(Workspace &ws, char *base, size_t max_n, int key_bits, size_t 
     ws.hist = b.take<u32>(8 * 256);
     ws.tile_status = b.take<u32>(2 * (ws.n_tiles_max + 64) * 256);   // + sentinel rows (sort.cu)
     ws.body = b.take<float4>(n);
-    ws.clev = b.take<signed char>(n + 2);
+    ws.clev = b.take<signed char>(n + 8);
     ws.dlev = b.take<u8>(n + 4);
     ws.cutflag = b.take<u8>(n + 4);
-    ws.build_tiles = b.take<uint4>(ws.n_blk_max * 8);
+    ws.build_tiles = b.take<uint4>((ws.n_blk_max + 8) * 16);
     ws.level_total = b.take<u32>(64);
+    ws.prev_ncells = b.take<u32>(4);
     ws.group_start = b.take<u32>(n + 1);
     ws.group_stats = b.take<uint4>(n);
     ws.cell_mac = b.take<float4>(ws.cell_cap);
@@ -112,6 +113,7 @@ extern "C" p3t_status p3t_create(p3t_ctx **out, int device, size_t max_n, int ke
     ctx->nleaf = 16;
     ctx->ngroup = 64;
     ctx->merge_levels = 1;
+    ctx->cells_dirty = true;
     cudaError_t e = cudaSetDevice(device);
     cudaDeviceProp prop;
     if (e == cudaSuccess) e = cudaGetDeviceProperties(&prop, device);
@@ -319,6 +321,7 @@ static p3t_status sync_and_check(p3t_ctx *ctx)
     P3T_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     if (ctx->h_counters[CNT_NONFINITE]) return p3t_fail(ctx, P3T_EINVAL, "non-finite mass or position in the device input");
     u64 f = ctx->h_counters[CNT_ERR_BUILD] | ctx->h_counters[CNT_ERR_EVAL];
+    if (ctx->h_counters[CNT_ERR_BUILD]) ctx->cells_dirty = true;
     if (f & ERR_CELL_CAPACITY) return p3t_fail(ctx, P3T_ENOMEM, "octree cell capacity (3 n + 1024) exceeded");
     if (f & ERR_STACK_OVERFLOW) return p3t_fail(ctx, P3T_ENOMEM, "tree-walk stack overflow");
     return P3T_OK;

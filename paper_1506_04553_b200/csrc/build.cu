@@ -23,15 +23,58 @@
 #define BUILD_WORDS (BUILD_WIN / 2)
 #define BUILD_PER_THREAD (BUILD_TILE / BUILD_THREADS)  // consecutive bodies per thread
 
-// per-tile record written by levels_kernel, completed by the scan of the last tile
+// Per-tile look-back words (flag | value, as in the radix sort) and the resulting exclusive prefixes.
+// status[0..23]: nodes per level starting in the tile (levels_kernel); status[24]: group heads in the
+// tile (emit_kernel).  BUILD_LOOKBACK sentinel records in front of record 0 hold INC | 0.
 struct TileRec {
-    u32 cnt[24];        // nodes per level starting in the tile  -> exclusive prefix over tiles
-    int lastcut;        // last cut position inside the tile (-1: none) -> last cut BEFORE the tile
-    int firstcut;       // first cut position inside the tile (tile end if none)
-    u32 heads_after;    // group heads at or after firstcut         -> exclusive prefix of all heads
-    u32 pad[5];
+    u32 status[32];
+    u32 excl[32];       // [0..23] exclusive prefix over tiles of the node counts per level
 };
-static_assert(sizeof(TileRec) == 128, "TileRec is one 128-byte line");
+static_assert(sizeof(TileRec) == 256, "TileRec is two 128-byte lines");
+#define BUILD_LOOKBACK 8
+#define TL_FLAG_AGG 0x40000000u
+#define TL_FLAG_INC 0x80000000u
+#define TL_VAL_MASK 0x3fffffffu
+
+__device__ __forceinline__ u32 ld_tile_status(const u32 *p)
+{
+    u32 v;
+    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_tile_status(u32 *p, u32 v)
+{
+    asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+// Decoupled look-back of one column: publishes `own` for `tile`, returns the sum over all tiles before it.
+// p0 points at status word `col` of record `tile`; records are sizeof(TileRec) apart.
+__device__ __forceinline__ u32 tile_lookback(u32 *p0, u32 tile, u32 own)
+{
+    const int stride = (int)(sizeof(TileRec) / sizeof(u32));
+    st_tile_status(p0, own | (tile == 0 ? TL_FLAG_INC : TL_FLAG_AGG));
+    u32 excl = 0;
+    if (tile > 0) {
+        const u32 *p = p0 - stride;
+        bool done = false;
+        while (!done) {
+            u32 v[BUILD_LOOKBACK];
+#pragma unroll
+            for (int k = 0; k < BUILD_LOOKBACK; ++k) v[k] = ld_tile_status(p - k * stride);
+            bool go = true;
+            u32 used = 0;
+#pragma unroll
+            for (int k = 0; k < BUILD_LOOKBACK; ++k) {
+                const bool ready = v[k] >= TL_FLAG_AGG, isinc = v[k] >= TL_FLAG_INC;
+                if (go && ready) { excl += v[k] & TL_VAL_MASK; ++used; }
+                done = done || (go && isinc);
+                go = go && ready && !isinc;
+            }
+            p -= used * stride;
+        }
+        st_tile_status(p0, (excl + own) | TL_FLAG_INC);
+    }
+    return excl;
+}
 
 #define BUILD_PAD 40   // zero words behind every window: shifted reads never leave the array
 struct Window { u32 w[BUILD_WORDS + BUILD_PAD]; };
@@ -107,27 +150,28 @@ __device__ __forceinline__ int win_get(const Window &win, int t) { return (int)(
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(BUILD_THREADS) levels_kernel(const signed char *__restrict__ clev, u8 *__restrict__ dlev,
                                                                u8 *__restrict__ cutflag, TileRec *tiles, u32 *level_total,
-                                                               u32 *group_start, u32 n, u32 ntiles, int max_level, int nleaf,
-                                                               int ngroup, int merge_levels, u64 *counters)
+                                                               u32 *prev_ncells, u32 n, u32 ntiles, int max_level, int nleaf, int ngroup,
+                                                               int merge_levels, u64 *counters)
 {
     // windows: c, leaf level, group level, minimum over NLEAF entries, two scratch
     __shared__ Window s_c, s_d, s_g, s_m, s_a, s_b;
     __shared__ int s_cnt[32];
-    __shared__ int s_wmax[BUILD_THREADS / 32], s_wfirst[BUILD_THREADS / 32];
-    __shared__ u32 s_wheads[BUILD_THREADS / 32];
-    __shared__ bool s_last;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const long long base = (long long)blockIdx.x * BUILD_TILE;
+    __shared__ u32 s_tile;
+    const int tid = threadIdx.x, lane = tid & 31;
+    if (tid == 0) s_tile = (u32)atomicAdd(&counters[CNT_HEAD_TICKET], 1ull);   // tiles in scheduling order (look-back)
+    __syncthreads();
+    const u32 tile = s_tile;
+    const long long base = (long long)tile * BUILD_TILE;
     // ---- window of biased c values (c + 1 in 0..22; 0 outside the array), two per word
-    for (int w = tid; w < BUILD_WORDS; w += BUILD_THREADS) {
-        u32 v = 0;
+    for (int q = tid; q < BUILD_WORDS / 2; q += BUILD_THREADS) {   // four c values (one 32-bit load) -> two words
+        const long long g = base - BUILD_HALO + 4 * q;
+        u32 raw = 0xffffffffu;   // c = -1 outside the array
+        if (g >= 0 && g <= (long long)n) raw = *reinterpret_cast<const u32 *>(clev + g);
+        u32 cb[4];
 #pragma unroll
-        for (int h = 0; h < 2; ++h) {
-            long long g = base - BUILD_HALO + 2 * w + h;
-            u32 cb = (g >= 0 && g <= (long long)n) ? (u32)((int)clev[g] + 1) : 0u;
-            v |= cb << (16 * h);
-        }
-        s_c.w[w] = v;
+        for (int h = 0; h < 4; ++h) cb[h] = (g + h <= (long long)n) ? (u32)((int)(signed char)(raw >> (8 * h)) + 1) : 0u;
+        s_c.w[2 * q] = cb[0] | (cb[1] << 16);
+        s_c.w[2 * q + 1] = cb[2] | (cb[3] << 16);
     }
     if (tid < BUILD_PAD) {
         s_c.w[BUILD_WORDS + tid] = 0; s_m.w[BUILD_WORDS + tid] = 0;
@@ -152,168 +196,50 @@ __global__ void __launch_bounds__(BUILD_THREADS) levels_kernel(const signed char
         sliding_max_to(&s_m, &s_a, &s_b, res1, w1);
     }
     // ---- my bodies: leaf level, cut flag, node counts per level (difference array)
-    int mycut_last = -1, mycut_first = 0x7fffffff;
-    int cuts[BUILD_PER_THREAD];
-#pragma unroll
-    for (int s = 0; s < BUILD_PER_THREAD; ++s) {
-        const int t = BUILD_HALO + tid * BUILD_PER_THREAD + s;
-        const long long i = base + tid * BUILD_PER_THREAD + s;
-        cuts[s] = -1;
-        if (i < (long long)n) {
-            const int c = win_get(s_c, t) - 1;
-            const int D = min(max_level, win_get(s_d, t));
-            const int g = min(max_level, win_get(s_g, t)), gp = i > 0 ? min(max_level, win_get(s_g, t - 1)) : 0;
-            dlev[i] = (u8)D;
-            const bool cut = (i == 0) || c < max(g, gp) - merge_levels;
-            cutflag[i] = cut ? 1 : 0;
-            if (cut) { cuts[s] = (int)i; mycut_last = (int)i; mycut_first = min(mycut_first, (int)i); }
-            if (D > c) { atomicAdd(&s_cnt[c + 1], 1); atomicAdd(&s_cnt[D + 1], -1); }
-        }
-    }
-    // ---- segment start of every body from the cuts inside the tile (inclusive max-scan)
-    int run = mycut_last;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        int t = __shfl_up_sync(0xffffffffu, run, o);
-        if (lane >= o) run = max(run, t);
-    }
-    int wfirst = mycut_first;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) wfirst = min(wfirst, __shfl_xor_sync(0xffffffffu, wfirst, o));
-    if (lane == 31) s_wmax[warp] = run;
-    if (lane == 0) s_wfirst[warp] = wfirst;
-    __syncthreads();
-    int seg = __shfl_up_sync(0xffffffffu, run, 1);   // last cut strictly before my first body (inside the tile)
-    if (lane == 0) seg = -1;
-    for (int w = 0; w < warp; ++w) seg = max(seg, s_wmax[w]);
-    u32 heads = 0;   // heads at or after the first cut of the tile
-#pragma unroll
-    for (int s = 0; s < BUILD_PER_THREAD; ++s) {
-        const long long i = base + tid * BUILD_PER_THREAD + s;
-        if (cuts[s] >= 0) seg = cuts[s];
-        if (i < (long long)n && seg >= 0 && ((u32)(i - seg) % (u32)ngroup) == 0) ++heads;
-    }
-    heads = __reduce_add_sync(0xffffffffu, heads);
-    if (lane == 0) s_wheads[warp] = heads;
-    __syncthreads();
-    if (tid == 0) {
-        TileRec &r = tiles[blockIdx.x];
-        int acc = 0;
-        for (int L = 0; L < 24; ++L) { acc += s_cnt[L]; r.cnt[L] = (u32)acc; }
-        int lastcut = -1, firstcut = 0x7fffffff;
-        u32 h = 0;
-        for (int w = 0; w < BUILD_THREADS / 32; ++w) { lastcut = max(lastcut, s_wmax[w]); firstcut = min(firstcut, s_wfirst[w]); h += s_wheads[w]; }
-        const long long tile_end = min((long long)n, base + BUILD_TILE);
-        r.lastcut = lastcut;
-        r.firstcut = firstcut == 0x7fffffff ? (int)tile_end : firstcut;
-        r.heads_after = h;
-        __threadfence();
-        s_last = atomicAdd(&counters[CNT_HEAD_TICKET], 1ull) + 1ull == (u64)ntiles;
-    }
-    __syncthreads();
-    if (!s_last) return;
-    // ---- last tile to finish: prefixes over all tiles.  Thread k owns a contiguous chunk of tiles.
-    __threadfence();
-    __shared__ u32 s_scan[BUILD_THREADS / 32][26];
-    __shared__ u32 s_tot[26];
-    const u32 per = (ntiles + BUILD_THREADS - 1) / BUILD_THREADS;
-    const u32 t0 = min(ntiles, (u32)tid * per), t1 = min(ntiles, t0 + per);
-    // (1) carried cut position: max-scan of lastcut
-    int mc = -1;
-    for (u32 t = t0; t < t1; ++t) mc = max(mc, __ldcg(&tiles[t].lastcut));
-    int mrun = mc;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        int t = __shfl_up_sync(0xffffffffu, mrun, o);
-        if (lane >= o) mrun = max(mrun, t);
-    }
-    if (lane == 31) s_wmax[warp] = mrun;
-    __syncthreads();
-    int carry = __shfl_up_sync(0xffffffffu, mrun, 1);
-    if (lane == 0) carry = -1;
-    for (int w = 0; w < warp; ++w) carry = max(carry, s_wmax[w]);
-    // (2) sums: 24 level counts + heads (heads of the leading partial segment depend on the carry)
-    u32 sums[25];
-#pragma unroll
-    for (int k = 0; k < 25; ++k) sums[k] = 0;
     {
-        int cpos = carry;
-        for (u32 t = t0; t < t1; ++t) {
-            const uint4 *src = reinterpret_cast<const uint4 *>(tiles[t].cnt);
+        const long long i0 = base + tid * BUILD_PER_THREAD;
+        u32 dl = 0, cf = 0;
 #pragma unroll
-            for (int q = 0; q < 6; ++q) {
-                uint4 v = __ldcg(src + q);
-                sums[4 * q] += v.x; sums[4 * q + 1] += v.y; sums[4 * q + 2] += v.z; sums[4 * q + 3] += v.w;
+        for (int s = 0; s < BUILD_PER_THREAD; ++s) {
+            const int t = BUILD_HALO + tid * BUILD_PER_THREAD + s;
+            const long long i = i0 + s;
+            if (i < (long long)n) {
+                const int c = win_get(s_c, t) - 1;
+                const int D = min(max_level, win_get(s_d, t));
+                const int g = min(max_level, win_get(s_g, t)), gp = i > 0 ? min(max_level, win_get(s_g, t - 1)) : 0;
+                const bool cut = (i == 0) || c < max(g, gp) - merge_levels;
+                dl |= (u32)D << (8 * s);
+                cf |= (cut ? 1u : 0u) << (8 * s);
+                if (D > c) { atomicAdd(&s_cnt[c + 1], 1); atomicAdd(&s_cnt[D + 1], -1); }
             }
-            const long long tb = (long long)t * BUILD_TILE;
-            const int fc = __ldcg(&tiles[t].firstcut), lc = __ldcg(&tiles[t].lastcut);
-            u32 lead = 0;   // heads in [tb, fc) of the segment that started at cpos
-            if (cpos >= 0 && fc > tb) {
-                const long long first = cpos + (((tb - cpos) + ngroup - 1) / ngroup) * (long long)ngroup;
-                if (first < fc) lead = (u32)((fc - 1 - first) / ngroup + 1);
-            }
-            sums[24] += lead + __ldcg(&tiles[t].heads_after);
-            if (lc >= 0) cpos = lc;
+        }
+        if (i0 < (long long)n) {   // dlev / cutflag are padded to a multiple of four bytes
+            *reinterpret_cast<u32 *>(dlev + i0) = dl;
+            *reinterpret_cast<u32 *>(cutflag + i0) = cf;
         }
     }
-    u32 incl[25];
-#pragma unroll
-    for (int k = 0; k < 25; ++k) {
-        u32 v = sums[k];
+    __syncthreads();
+    // ---- warp 0: nodes per level -> look-back over the tiles before -> exclusive prefixes
+    if (tid < 32) {
+        int v = lane < 24 ? s_cnt[lane] : 0;   // difference array -> counts per level
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
-            u32 t = __shfl_up_sync(0xffffffffu, v, o);
+            int t = __shfl_up_sync(0xffffffffu, v, o);
             if (lane >= o) v += t;
         }
-        incl[k] = v;
-        if (lane == 31) s_scan[warp][k] = v;
-    }
-    __syncthreads();
-    if (tid < 25) {
-        u32 acc = 0;
-        for (int w = 0; w < BUILD_THREADS / 32; ++w) { u32 t = s_scan[w][tid]; s_scan[w][tid] = acc; acc += t; }
-        s_tot[tid] = acc;
-    }
-    __syncthreads();
-    {   // (3) write the exclusive prefixes back into the tile records
-        u32 run25[25];
-#pragma unroll
-        for (int k = 0; k < 25; ++k) run25[k] = s_scan[warp][k] + incl[k] - sums[k];
-        int cpos = carry;
-        for (u32 t = t0; t < t1; ++t) {
-            TileRec &r = tiles[t];
-            uint4 *dst = reinterpret_cast<uint4 *>(r.cnt);
-            u32 own[24];
-#pragma unroll
-            for (int q = 0; q < 6; ++q) {
-                uint4 v = __ldcg(reinterpret_cast<const uint4 *>(r.cnt) + q);
-                own[4 * q] = v.x; own[4 * q + 1] = v.y; own[4 * q + 2] = v.z; own[4 * q + 3] = v.w;
-                dst[q] = make_uint4(run25[4 * q], run25[4 * q + 1], run25[4 * q + 2], run25[4 * q + 3]);
-            }
-#pragma unroll
-            for (int k = 0; k < 24; ++k) run25[k] += own[k];
-            const long long tb = (long long)t * BUILD_TILE;
-            const int fc = __ldcg(&r.firstcut), lc = __ldcg(&r.lastcut);
-            u32 lead = 0;
-            if (cpos >= 0 && fc > tb) {
-                const long long first = cpos + (((tb - cpos) + ngroup - 1) / ngroup) * (long long)ngroup;
-                if (first < fc) lead = (u32)((fc - 1 - first) / ngroup + 1);
-            }
-            const u32 h = lead + __ldcg(&r.heads_after);
-            r.heads_after = run25[24];
-            run25[24] += h;
-            r.lastcut = cpos;
-            if (lc >= 0) cpos = lc;
+        u32 tot = 0;
+        if (lane < 24) {
+            const u32 own = (u32)v;
+            const u32 excl = tile_lookback(&tiles[tile].status[lane], tile, own);
+            tiles[tile].excl[lane] = excl;
+            tot = excl + own;
         }
-    }
-    if (tid < 24) level_total[tid] = s_tot[tid];
-    if (tid == 0) {
-        u64 cells = 0, depth = 0;
-        for (int L = 0; L <= max_level; ++L) { cells += s_tot[L]; if (s_tot[L]) depth = (u64)L; }
-        counters[CNT_NCELLS] = cells;
-        counters[CNT_DEPTH] = depth;
-        counters[CNT_NGROUPS] = (u64)s_tot[24];
-        group_start[s_tot[24]] = n;
+        if (tile == ntiles - 1) {   // the last tile holds the totals: nodes per level, cells, deepest level in use
+            if (lane < 24) level_total[lane] = tot;
+            const u32 cells = __reduce_add_sync(0xffffffffu, tot);
+            const u32 dep = __reduce_max_sync(0xffffffffu, tot ? (u32)lane : 0u);
+            if (lane == 0) { counters[CNT_NCELLS] = (u64)cells; counters[CNT_DEPTH] = (u64)dep; *prev_ncells = cells; }
+        }
     }
 }
 
@@ -322,27 +248,47 @@ __global__ void __launch_bounds__(BUILD_THREADS) levels_kernel(const signed char
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(BUILD_THREADS) emit_kernel(
     const signed char *__restrict__ clev, const u8 *__restrict__ dlev, const u8 *__restrict__ cutflag,
-    const TileRec *__restrict__ tiles, const u32 *__restrict__ level_total, u32 n, int max_level, int ngroup, u32 cell_cap,
+    TileRec *tiles, const u32 *__restrict__ level_total, u32 n, u32 ntiles, int max_level, int ngroup, u32 cell_cap,
     u32 *__restrict__ cell_start, u8 *__restrict__ cell_level, u32 *__restrict__ cell_parent, u32 *__restrict__ cell_first,
     u32 *cell_nchild, uint2 *__restrict__ cell_meta, u32 *__restrict__ group_start, u64 *counters)
 {
-    __shared__ signed char s_c[BUILD_TILE + BUILD_HALO + 4];   // c[base .. base + TILE + HALO]
+    __shared__ __align__(16) signed char s_c[BUILD_TILE + BUILD_HALO + 4];   // c[base .. base + TILE + HALO]
     __shared__ u32 s_wcnt[BUILD_THREADS / 32][24];
     __shared__ u32 s_lvloff[24];
     __shared__ int s_lo, s_hi;
     __shared__ int s_wmax[BUILD_THREADS / 32];
     __shared__ u32 s_whead[BUILD_THREADS / 32];
+    __shared__ u32 s_tile, s_headbase;
+    __shared__ int s_carry;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const u32 base = blockIdx.x * BUILD_TILE;
-    for (int t = tid; t < BUILD_TILE + BUILD_HALO + 1; t += BUILD_THREADS) {
-        u32 g = base + t;
-        s_c[t] = g <= n ? clev[g] : (signed char)-1;
+    if (tid == 0) { s_tile = (u32)atomicAdd(&counters[CNT_HEAD_SPARE0], 1ull); s_lo = 99; s_hi = -1; }
+    __syncthreads();
+    const u32 tile = s_tile;
+    const u32 base = tile * BUILD_TILE;
+    for (int q = tid; q < (BUILD_TILE + BUILD_HALO + 4) / 4; q += BUILD_THREADS) {   // c[base ..] four at a time
+        const u32 g = base + 4 * q;
+        u32 raw = 0xffffffffu;
+        if (g <= n) raw = *reinterpret_cast<const u32 *>(clev + g);
+#pragma unroll
+        for (int h = 0; h < 4; ++h)
+            if (g + h > n) raw |= 0xffu << (8 * h);
+        *reinterpret_cast<u32 *>(&s_c[4 * q]) = raw;
     }
-    if (tid == 0) { s_lo = 99; s_hi = -1; }
     if (tid < 24) {
         u32 off = 0;
         for (int L = 0; L < tid; ++L) off += level_total[L];
-        s_lvloff[tid] = off + tiles[blockIdx.x].cnt[tid];
+        s_lvloff[tid] = off + tiles[tile].excl[tid];
+    }
+    // warp 7: the last cut before the tile, by a backward search over the cut flags (cutflag[0] = 1)
+    if (warp == BUILD_THREADS / 32 - 1) {
+        int found = -1;
+        for (long long top = (long long)base - 1; top >= 0 && found < 0; top -= 32) {
+            const long long pos = top - lane;
+            const bool hit = pos >= 0 && cutflag[pos];
+            const u32 b = __ballot_sync(0xffffffffu, hit);
+            if (b) found = (int)(top - (__ffs(b) - 1));   // lowest lane = nearest position
+        }
+        if (lane == 0) s_carry = found;
     }
     __syncthreads();
     int c[BUILD_PER_THREAD], D[BUILD_PER_THREAD];
@@ -414,7 +360,7 @@ __global__ void __launch_bounds__(BUILD_THREADS) emit_kernel(
                     u32 parent = P3T_NO_PARENT;
                     if (L > 0) {
                         parent = prev_flag[s] ? prev_rank[s] : prev_rank[s] - 1;
-                        atomicAdd(&cell_nchild[parent], 1u);
+                        atomicAdd(&cell_nchild[parent], L == D[s] ? 1u : 0x10001u);   // children | internal children << 16
                     }
                     cell_parent[rank] = parent;
                     if (prev_flag[s]) cell_first[prev_rank[s]] = rank;
@@ -426,6 +372,8 @@ __global__ void __launch_bounds__(BUILD_THREADS) emit_kernel(
                             while (i + cnt < n && clev[i + cnt] >= L) ++cnt;   // a deep leaf longer than the window
                         cell_meta[rank] = make_uint2(i, cnt | P3T_LEAF_FLAG);
                         ++nleaf_here;
+                    } else {
+                        cell_meta[rank] = make_uint2(0u, 0u);   // internal: completed by moments_kernel
                     }
                 } else {
                     atomicOr(&counters[CNT_ERR_BUILD], (u64)ERR_CELL_CAPACITY);
@@ -456,7 +404,7 @@ __global__ void __launch_bounds__(BUILD_THREADS) emit_kernel(
         __syncthreads();
         int seg = __shfl_up_sync(0xffffffffu, run, 1);
         if (lane == 0) seg = -1;
-        seg = max(seg, tiles[blockIdx.x].lastcut);   // cut carried in from the tiles before
+        seg = max(seg, s_carry);   // cut carried in from the tiles before
         for (int w = 0; w < warp; ++w) seg = max(seg, s_wmax[w]);
         bool head[BUILD_PER_THREAD];
         u32 mine = 0;
@@ -475,12 +423,28 @@ __global__ void __launch_bounds__(BUILD_THREADS) emit_kernel(
         }
         if (lane == 31) s_whead[warp] = inc;
         __syncthreads();
-        u32 pos = tiles[blockIdx.x].heads_after + inc - mine;
+        if (tid == 0) {   // heads of the tiles before: look-back (most predecessors are done by now)
+            u32 total = 0;
+            for (int w = 0; w < BUILD_THREADS / 32; ++w) total += s_whead[w];
+            const u32 excl = tile_lookback(&tiles[tile].status[24], tile, total);
+            s_headbase = excl;
+            if (tile == ntiles - 1) {
+                counters[CNT_NGROUPS] = (u64)(excl + total);
+                group_start[excl + total] = n;
+            }
+        }
+        __syncthreads();
+        u32 pos = s_headbase + inc - mine;
         for (int w = 0; w < warp; ++w) pos += s_whead[w];
 #pragma unroll
         for (int s = 0; s < BUILD_PER_THREAD; ++s)
             if (head[s]) group_start[pos++] = i0 + s;
     }
+}
+
+__global__ void tile_sentinel_kernel(TileRec *recs)
+{
+    recs[blockIdx.x].status[threadIdx.x] = TL_FLAG_INC;
 }
 
 p3t_status p3t_stage_build(p3t_ctx *ctx)
@@ -489,13 +453,18 @@ p3t_status p3t_stage_build(p3t_ctx *ctx)
     u32 n = (u32)ctx->n;
     cudaStream_t s = ctx->stream;
     u32 ntiles = div_up(n, BUILD_TILE);
-    // cell_nchild and cell_ready are adjacent in the workspace: one memset zeroes both
-    P3T_CUDA(ctx, cudaMemsetAsync(w.cell_nchild, 0, (size_t)((char *)(w.cell_ready + w.cell_cap) - (char *)w.cell_nchild), s));
-    levels_kernel<<<ntiles, BUILD_THREADS, 0, s>>>(w.clev, w.dlev, w.cutflag, (TileRec *)w.build_tiles, w.level_total, w.group_start,
-                                                  n, ntiles, ctx->max_level, ctx->nleaf, ctx->ngroup, ctx->merge_levels, w.counters);
-    emit_kernel<<<ntiles, BUILD_THREADS, 0, s>>>(w.clev, w.dlev, w.cutflag, (const TileRec *)w.build_tiles, w.level_total, n,
-                                                ctx->max_level, ctx->ngroup, (u32)w.cell_cap, w.cell_start, w.cell_level,
-                                                w.cell_parent, w.cell_first, w.cell_nchild, w.cell_meta, w.group_start, w.counters);
+    TileRec *recs = (TileRec *)w.build_tiles;       // BUILD_LOOKBACK sentinel records, then one per tile
+    if (!ctx->tiles_ready) {
+        tile_sentinel_kernel<<<BUILD_LOOKBACK, 32, 0, s>>>(recs);
+        ctx->tiles_ready = true;
+    }
+    TileRec *tiles = recs + BUILD_LOOKBACK;
+    P3T_CUDA(ctx, cudaMemsetAsync(tiles, 0, (size_t)ntiles * sizeof(TileRec), s));
+    levels_kernel<<<ntiles, BUILD_THREADS, 0, s>>>(w.clev, w.dlev, w.cutflag, tiles, w.level_total, w.prev_ncells, n, ntiles, ctx->max_level,
+                                                  ctx->nleaf, ctx->ngroup, ctx->merge_levels, w.counters);
+    emit_kernel<<<ntiles, BUILD_THREADS, 0, s>>>(w.clev, w.dlev, w.cutflag, tiles, w.level_total, n, ntiles, ctx->max_level,
+                                                ctx->ngroup, (u32)w.cell_cap, w.cell_start, w.cell_level, w.cell_parent,
+                                                w.cell_first, w.cell_nchild, w.cell_meta, w.group_start, w.counters);
     P3T_CUDA(ctx, cudaGetLastError());
     return P3T_OK;
 }

@@ -1,10 +1,7 @@
 // moments.cu -- row a6: bottom-up monopole + quadrupole moments ("up to the quadrupole moment",
-// PAPER.md L138), tight AABBs and the per-cell acceptance radius, in ONE launch.
+// PAPER.md L138), tight AABBs and the per-cell acceptance radius.
 //
-// One thread per cell.  Leaf threads reduce their bodies, then climb: a thread that finishes cell k
-// increments its parent's arrival counter; the thread that brings it to the parent's child count
-// merges the children (parallel-axis shift of the quadrupoles) and keeps climbing.  Children are
-// always merged in index order, so the result is deterministic.
+// Two launches (moments_kernel<0>: leaves, moments_kernel<1>: internal cells), one thread per cell.
 //
 // Acceptance radius (rule R-MAC of DESIGN.md, readings A9/A10): a cell C may be used as a multipole
 // by a group with box B iff  d(B, c_C)^2 > rcrit_C^2,
@@ -59,91 +56,132 @@ __device__ __forceinline__ void store_cell(u32 k, const Mom &m, int level, u64 k
     cell_bmax[k] = make_float4(m.hix, m.hiy, m.hiz, delta);
 }
 
-__global__ void __launch_bounds__(128) moments_kernel(
-    const float4 *__restrict__ body, const u64 *__restrict__ keys, const float *__restrict__ cube,
-    const u8 *__restrict__ cell_level, const u32 *__restrict__ cell_start, const u32 *__restrict__ cell_parent,
-    const u32 *__restrict__ cell_first, const u32 *__restrict__ cell_nchild, u32 *cell_ready, uint2 *cell_meta,
-    const u8 *__restrict__ dlev, float4 *cell_mac, float4 *cell_mom0, float4 *cell_mom1, float4 *cell_bmin,
-    float4 *cell_bmax, const u64 *__restrict__ counters, u32 cell_cap, int max_level, float theta, float h)
+// One cell from its children [first, first + nch), merged in index order: sums about the first child's
+// centre of mass (well conditioned), then the quadrupole is shifted to the centre of mass of the cell
+// (parallel-axis theorem).  All loads go to L2 (the records were written by other SMs in this launch).
+__device__ __forceinline__ void merge_children(u32 first, u32 nch, const float4 *cell_mac, const float4 *cell_mom0,
+                                               const float4 *cell_mom1, const float4 *cell_bmin, const float4 *cell_bmax, Mom &m)
 {
-    u32 ncell = (u32)min((u64)cell_cap, counters[CNT_NCELLS]);
-    u32 k = blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= ncell) return;
-    int level = cell_level[k];
-    u32 start = cell_start[k];
-    if (level != (int)dlev[start]) return;   // internal cell: computed by the last arriving child
-    // ---- leaf: two passes over its bodies (offsets from the first body keep the sums well conditioned)
-    Mom m;
-    {
-        uint2 meta = cell_meta[k];
-        u32 cnt = meta.y & ~P3T_LEAF_FLAG;
-        float4 b0 = body[start];
-        float sx = 0.f, sy = 0.f, sz = 0.f, M = 0.f;
-        m.lox = m.hix = b0.x; m.loy = m.hiy = b0.y; m.loz = m.hiz = b0.z;
-        for (u32 j = 0; j < cnt; ++j) {
-            float4 b = body[start + j];
-            M += b.w;
-            sx += b.w * (b.x - b0.x); sy += b.w * (b.y - b0.y); sz += b.w * (b.z - b0.z);
-            m.lox = fminf(m.lox, b.x); m.hix = fmaxf(m.hix, b.x);
-            m.loy = fminf(m.loy, b.y); m.hiy = fmaxf(m.hiy, b.y);
-            m.loz = fminf(m.loz, b.z); m.hiz = fmaxf(m.hiz, b.z);
-        }
-        float inv = M > 0.f ? 1.f / M : 0.f;
-        m.M = M;
-        m.cx = b0.x + sx * inv; m.cy = b0.y + sy * inv; m.cz = b0.z + sz * inv;
-        if (!(M > 0.f)) {   // massless leaf: centre of its box
-            m.cx = 0.5f * (m.lox + m.hix); m.cy = 0.5f * (m.loy + m.hiy); m.cz = 0.5f * (m.loz + m.hiz);
-        }
-        m.qxx = m.qyy = m.qzz = m.qxy = m.qxz = m.qyz = 0.f;
-        for (u32 j = 0; j < cnt; ++j) {
-            float4 b = body[start + j];
-            float rx = b.x - m.cx, ry = b.y - m.cy, rz = b.z - m.cz;
-            m.qxx += b.w * rx * rx; m.qyy += b.w * ry * ry; m.qzz += b.w * rz * rz;
-            m.qxy += b.w * rx * ry; m.qxz += b.w * rx * rz; m.qyz += b.w * ry * rz;
-        }
-    }
-    while (true) {
-        store_cell(k, m, level, keys[start], cube, max_level, theta, h, cell_mac, cell_mom0, cell_mom1, cell_bmin, cell_bmax);
-        u32 p = cell_parent[k];
-        if (p == P3T_NO_PARENT) break;
-        __threadfence();
-        u32 nch = cell_nchild[p];
-        u32 old = atomicAdd(&cell_ready[p], 1u);
-        if (old + 1 != nch) break;
-        __threadfence();
-        // ---- last arrival: merge the children of p in index order
-        u32 first = cell_first[p];
-        float M = 0.f, sx = 0.f, sy = 0.f, sz = 0.f;
-        float4 a0 = __ldcg(&cell_mac[first]);
-        m.lox = m.loy = m.loz = INFINITY; m.hix = m.hiy = m.hiz = -INFINITY;
-        for (u32 c = 0; c < nch; ++c) {
-            float4 a = __ldcg(&cell_mac[first + c]);
-            float4 q0 = __ldcg(&cell_mom0[first + c]);
-            float4 lo = __ldcg(&cell_bmin[first + c]), hi = __ldcg(&cell_bmax[first + c]);
-            M += q0.x;
-            sx += q0.x * (a.x - a0.x); sy += q0.x * (a.y - a0.y); sz += q0.x * (a.z - a0.z);
+    const float4 a0 = __ldcg(&cell_mac[first]);
+    float M = 0.f, sx = 0.f, sy = 0.f, sz = 0.f;
+    float qxx = 0.f, qyy = 0.f, qzz = 0.f, qxy = 0.f, qxz = 0.f, qyz = 0.f;
+    m.lox = m.loy = m.loz = INFINITY; m.hix = m.hiy = m.hiz = -INFINITY;
+#pragma unroll
+    for (int c = 0; c < 8; ++c) {
+        if ((u32)c < nch) {
+            const u32 ci = first + c;
+            const float4 a = __ldcg(&cell_mac[ci]), q0 = __ldcg(&cell_mom0[ci]), q1 = __ldcg(&cell_mom1[ci]);
+            const float4 lo = __ldcg(&cell_bmin[ci]), hi = __ldcg(&cell_bmax[ci]);
+            const float mc = q0.x, rx = a.x - a0.x, ry = a.y - a0.y, rz = a.z - a0.z;
+            M += mc;
+            sx += mc * rx; sy += mc * ry; sz += mc * rz;
+            qxx += q0.y + mc * rx * rx; qyy += q0.z + mc * ry * ry; qzz += q0.w + mc * rz * rz;
+            qxy += q1.x + mc * rx * ry; qxz += q1.y + mc * rx * rz; qyz += q1.z + mc * ry * rz;
             m.lox = fminf(m.lox, lo.x); m.loy = fminf(m.loy, lo.y); m.loz = fminf(m.loz, lo.z);
             m.hix = fmaxf(m.hix, hi.x); m.hiy = fmaxf(m.hiy, hi.y); m.hiz = fmaxf(m.hiz, hi.z);
         }
-        float inv = M > 0.f ? 1.f / M : 0.f;
-        m.M = M;
-        m.cx = a0.x + sx * inv; m.cy = a0.y + sy * inv; m.cz = a0.z + sz * inv;
-        if (!(M > 0.f)) {
-            m.cx = 0.5f * (m.lox + m.hix); m.cy = 0.5f * (m.loy + m.hiy); m.cz = 0.5f * (m.loz + m.hiz);
-        }
+    }
+    const float inv = M > 0.f ? 1.f / M : 0.f;
+    const float dx = sx * inv, dy = sy * inv, dz = sz * inv;
+    m.M = M;
+    m.cx = a0.x + dx; m.cy = a0.y + dy; m.cz = a0.z + dz;
+    m.qxx = fmaxf(qxx - M * dx * dx, 0.f); m.qyy = fmaxf(qyy - M * dy * dy, 0.f); m.qzz = fmaxf(qzz - M * dz * dz, 0.f);
+    m.qxy = qxy - M * dx * dy; m.qxz = qxz - M * dx * dz; m.qyz = qyz - M * dy * dz;
+    if (!(M > 0.f)) {
+        m.cx = 0.5f * (m.lox + m.hix); m.cy = 0.5f * (m.loy + m.hiy); m.cz = 0.5f * (m.loz + m.hiz);
         m.qxx = m.qyy = m.qzz = m.qxy = m.qxz = m.qyz = 0.f;
-        for (u32 c = 0; c < nch; ++c) {
-            float4 a = __ldcg(&cell_mac[first + c]);
-            float4 q0 = __ldcg(&cell_mom0[first + c]);
-            float4 q1 = __ldcg(&cell_mom1[first + c]);
-            float rx = a.x - m.cx, ry = a.y - m.cy, rz = a.z - m.cz;
-            m.qxx += q0.y + q0.x * rx * rx; m.qyy += q0.z + q0.x * ry * ry; m.qzz += q0.w + q0.x * rz * rz;
-            m.qxy += q1.x + q0.x * rx * ry; m.qxz += q1.y + q0.x * rx * rz; m.qyz += q1.z + q0.x * ry * rz;
+    }
+}
+
+// PHASE 0: every leaf from its bodies -- a streaming pass without atomics or fences.
+// PHASE 1: the internal cells.  cell_nchild[p] holds (children | internal children << 16), counted by
+//   emit_kernel.  A cell whose children are all leaves is computed at once; its thread then climbs:
+//   it arrives at the parent's counter and the last internal child to arrive merges the parent.
+//   Only internal cells (about one cell in eight) pay for a fence and an atomic, and the loads of a
+//   merge go to L2, so no acquire (L1 invalidation) is needed.  Children are merged in index order:
+//   the result is deterministic.  The counters are read-only here (a late thread must still see whether
+//   its cell waits for children); keys_hist_kernel of the next build zeroes them.
+template <int PHASE>
+__global__ void __launch_bounds__(128, 4) moments_kernel(
+    const float4 *__restrict__ body, const u64 *__restrict__ keys, const float *__restrict__ cube,
+    const u8 *__restrict__ cell_level, const u32 *__restrict__ cell_start, const u32 *__restrict__ cell_parent,
+    const u32 *__restrict__ cell_first, u32 *cell_nchild, u32 *cell_ready, uint2 *cell_meta,
+    float4 *cell_mac, float4 *cell_mom0, float4 *cell_mom1, float4 *cell_bmin,
+    float4 *cell_bmax, const u64 *__restrict__ counters, u32 cell_cap, int max_level, float theta, float h)
+{
+    const u32 ncell = (u32)min((u64)cell_cap, counters[CNT_NCELLS]);
+    for (u32 k0 = blockIdx.x * blockDim.x + threadIdx.x; k0 < ncell; k0 += gridDim.x * blockDim.x) {
+        u32 k = k0;
+        // emit_kernel writes cell_meta of internal cells as (0, 0): the leaf flag is valid for every cell
+        const uint2 meta = cell_meta[k];
+        const bool leaf = (meta.y & P3T_LEAF_FLAG) != 0;
+        if (leaf != (PHASE == 0)) continue;
+        int level = cell_level[k];
+        u32 start = cell_start[k];
+        Mom m;
+        if (PHASE == 0) {
+            // ---- leaf: one pass over its bodies, sums about the first body, then shifted to the centre of mass
+            const u32 cnt = meta.y & ~P3T_LEAF_FLAG;
+            const float4 b0 = body[start];
+            float sx = 0.f, sy = 0.f, sz = 0.f, M = 0.f;
+            float qxx = 0.f, qyy = 0.f, qzz = 0.f, qxy = 0.f, qxz = 0.f, qyz = 0.f;
+            m.lox = m.hix = b0.x; m.loy = m.hiy = b0.y; m.loz = m.hiz = b0.z;
+            for (u32 j0 = 0; j0 < cnt; j0 += 4) {
+                float4 bb[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) bb[u] = body[start + min(j0 + u, cnt - 1)];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    if (j0 + u < cnt) {
+                        const float4 b = bb[u];
+                        const float rx = b.x - b0.x, ry = b.y - b0.y, rz = b.z - b0.z;
+                        M += b.w;
+                        sx += b.w * rx; sy += b.w * ry; sz += b.w * rz;
+                        qxx += b.w * rx * rx; qyy += b.w * ry * ry; qzz += b.w * rz * rz;
+                        qxy += b.w * rx * ry; qxz += b.w * rx * rz; qyz += b.w * ry * rz;
+                        m.lox = fminf(m.lox, b.x); m.hix = fmaxf(m.hix, b.x);
+                        m.loy = fminf(m.loy, b.y); m.hiy = fmaxf(m.hiy, b.y);
+                        m.loz = fminf(m.loz, b.z); m.hiz = fmaxf(m.hiz, b.z);
+                    }
+                }
+            }
+            const float inv = M > 0.f ? 1.f / M : 0.f;
+            const float dx = sx * inv, dy = sy * inv, dz = sz * inv;   // centre of mass - first body
+            m.M = M;
+            m.cx = b0.x + dx; m.cy = b0.y + dy; m.cz = b0.z + dz;
+            m.qxx = fmaxf(qxx - M * dx * dx, 0.f); m.qyy = fmaxf(qyy - M * dy * dy, 0.f); m.qzz = fmaxf(qzz - M * dz * dz, 0.f);
+            m.qxy = qxy - M * dx * dy; m.qxz = qxz - M * dx * dz; m.qyz = qyz - M * dy * dz;
+            if (!(M > 0.f)) {   // massless leaf: centre of its box
+                m.cx = 0.5f * (m.lox + m.hix); m.cy = 0.5f * (m.loy + m.hiy); m.cz = 0.5f * (m.loz + m.hiz);
+                m.qxx = m.qyy = m.qzz = m.qxy = m.qxz = m.qyz = 0.f;
+            }
+            store_cell(k, m, level, keys[start], cube, max_level, theta, h, cell_mac, cell_mom0, cell_mom1, cell_bmin, cell_bmax);
+            continue;
         }
-        cell_meta[p] = make_uint2(first, nch);
-        k = p;
-        level = cell_level[k];
-        start = cell_start[k];
+        // ---- internal cell
+        u32 cw = cell_nchild[k];
+        if (cw >> 16) continue;          // has internal children: computed by the last of them to arrive
+        u32 first = cell_first[k], parent = cell_parent[k];
+        u64 key = keys[start];
+        while (true) {
+            const u32 nch = cw & 0xffffu;
+            // what the next step needs of the parent does not depend on this merge: requested now, so that
+            // one level of the climb costs the merge loads, a fence and an atomic, nothing more
+            u32 pcw = 0, pfirst = 0, pparent = P3T_NO_PARENT, pstart = 0;
+            int plevel = 0;
+            if (parent != P3T_NO_PARENT) {
+                pcw = cell_nchild[parent]; pfirst = cell_first[parent]; pparent = cell_parent[parent];
+                plevel = cell_level[parent]; pstart = cell_start[parent];
+            }
+            merge_children(first, nch, cell_mac, cell_mom0, cell_mom1, cell_bmin, cell_bmax, m);
+            const u64 pkey = parent != P3T_NO_PARENT ? keys[pstart] : 0ull;
+            store_cell(k, m, level, key, cube, max_level, theta, h, cell_mac, cell_mom0, cell_mom1, cell_bmin, cell_bmax);
+            cell_meta[k] = make_uint2(first, nch);
+            if (parent == P3T_NO_PARENT) break;
+            __threadfence();             // my record is visible before my arrival is
+            if (atomicAdd(&cell_ready[parent], 1u) + 1 != (pcw >> 16)) break;
+            k = parent; cw = pcw; first = pfirst; parent = pparent; level = plevel; start = pstart; key = pkey;
+        }
     }
 }
 
@@ -151,14 +189,18 @@ p3t_status p3t_stage_moments(p3t_ctx *ctx)
 {
     Workspace &w = ctx->ws;
     cudaStream_t s = ctx->stream;
-    // the number of cells lives on the device; launch for the upper bound the host knows and let
-    // surplus threads exit (cells <= min(cell_cap, n * (max_level + 1)))
+    // the number of cells lives on the device: grid-stride loops over it
     size_t bound = ctx->n * (size_t)(ctx->max_level + 1);
     if (bound > w.cell_cap) bound = w.cell_cap;
-    moments_kernel<<<div_up(bound, 128), 128, 0, s>>>(w.body, w.keys[ctx->cur], w.cube, w.cell_level, w.cell_start,
-                                                      w.cell_parent, w.cell_first, w.cell_nchild, w.cell_ready, w.cell_meta,
-                                                      w.dlev, w.cell_mac, w.cell_mom0, w.cell_mom1, w.cell_bmin, w.cell_bmax,
-                                                      w.counters, (u32)w.cell_cap, ctx->max_level, ctx->prm.theta, ctx->prm.h);
+    const u32 grid = (u32)min((size_t)div_up(bound, 128), (size_t)ctx->sm_count * 16);
+    moments_kernel<0><<<grid, 128, 0, s>>>(w.body, w.keys[ctx->cur], w.cube, w.cell_level, w.cell_start, w.cell_parent, w.cell_first,
+                                           w.cell_nchild, w.cell_ready, w.cell_meta, w.cell_mac, w.cell_mom0, w.cell_mom1,
+                                           w.cell_bmin, w.cell_bmax, w.counters, (u32)w.cell_cap, ctx->max_level, ctx->prm.theta,
+                                           ctx->prm.h);
+    moments_kernel<1><<<grid, 128, 0, s>>>(w.body, w.keys[ctx->cur], w.cube, w.cell_level, w.cell_start, w.cell_parent, w.cell_first,
+                                           w.cell_nchild, w.cell_ready, w.cell_meta, w.cell_mac, w.cell_mom0, w.cell_mom1,
+                                           w.cell_bmin, w.cell_bmax, w.counters, (u32)w.cell_cap, ctx->max_level, ctx->prm.theta,
+                                           ctx->prm.h);
     P3T_CUDA(ctx, cudaGetLastError());
     return P3T_OK;
 }

@@ -79,8 +79,9 @@ struct Workspace {
     signed char *clev;             // [n+1]  common-prefix levels between sorted neighbours (c[0] = -1)
     u8 *dlev;                      // [n] leaf level of each body
     u8 *cutflag;                   // [n] segment cut (group construction)
-    void *build_tiles;             // [nblk] 128-byte tile records of build.cu (node counts per level, cuts, heads)
+    void *build_tiles;             // [8 + nblk] 256-byte tile records of build.cu (look-back words, exclusive prefixes)
     u32 *level_total;              // [32]
+    u32 *prev_ncells;              // [1] cells of the previous build: their child counters are zeroed by the next one
     u32 *group_start;              // [n+1]
     uint4 *group_stats;            // [n] per-group diagnostics of the last walk (P3T_ARR_GROUP_STATS)
     // cells
@@ -110,6 +111,8 @@ struct p3t_ctx {
     int key_bits, max_level, nleaf, ngroup, merge_levels;
     int sm_count;
     bool have_params, loaded, built, evaluated;
+    bool cells_dirty;              // child counters need a memset before the next build
+    bool tiles_ready;              // sentinel records of the build look-back written
     bool status_clean;             // the look-back buffers have been zeroed once (they clean themselves afterwards)
     int cur;                       // which of keys[2]/idx[2] holds the sorted result
     P3TParams prm;

@@ -114,8 +114,14 @@ __device__ __forceinline__ void root_cube(const u32 *bbox_bits, float &minx, flo
 
 __global__ void __launch_bounds__(256) keys_hist_kernel(const float4 *__restrict__ body, const u32 *__restrict__ bbox_bits,
                                                         float *cube, u64 *__restrict__ keys, u32 *hist, u32 n,
-                                                        int max_level, int passes)
+                                                        int max_level, int passes, const u32 *__restrict__ prev_ncells,
+                                                        u32 cell_cap, u32 *cell_nchild, u32 *cell_ready)
 {
+    // child counters of the cells of the previous build -> 0 (emit_kernel accumulates into them)
+    for (u32 k = blockIdx.x * blockDim.x + threadIdx.x, nc = min(*prev_ncells, cell_cap); k < nc; k += gridDim.x * blockDim.x) {
+        cell_nchild[k] = 0;
+        cell_ready[k] = 0;
+    }
     __shared__ u32 s_hist[8 * 256];
     for (int t = threadIdx.x; t < 8 * 256; t += blockDim.x) s_hist[t] = 0;
     float minx, miny, minz, side;
@@ -369,7 +375,13 @@ p3t_status p3t_stage_sort(p3t_ctx *ctx)
     P3T_CUDA(ctx, cudaMemsetAsync(w.counters + CNT_NCELLS, 0, 16 * sizeof(u64), s));   // build counters + sort tickets
     P3T_CUDA(ctx, cudaMemsetAsync(w.hist, 0, 8 * 256 * sizeof(u32), s));
     u32 grid = min(div_up(n, 256 * 4), (u32)ctx->sm_count * 8);
-    keys_hist_kernel<<<grid, 256, 0, s>>>(w.body_user, w.bbox_bits, w.cube, w.keys[0], w.hist, n, ctx->max_level, passes);
+    if (ctx->cells_dirty) {   // first build, or the last one ended in an error: all child counters and prev_ncells -> 0
+        P3T_CUDA(ctx, cudaMemsetAsync(w.cell_nchild, 0, (size_t)((char *)(w.cell_ready + w.cell_cap) - (char *)w.cell_nchild), s));
+        P3T_CUDA(ctx, cudaMemsetAsync(w.prev_ncells, 0, sizeof(u32), s));
+        ctx->cells_dirty = false;
+    }
+    keys_hist_kernel<<<grid, 256, 0, s>>>(w.body_user, w.bbox_bits, w.cube, w.keys[0], w.hist, n, ctx->max_level, passes,
+                                          w.prev_ncells, (u32)w.cell_cap, w.cell_nchild, w.cell_ready);
     int cur = 0;
     for (int p = 0; p < passes; ++p) {
         u32 *st_cur = w.tile_status + ((size_t)(p & 1) * status_rows + SORT_LOOKBACK) * 256;
