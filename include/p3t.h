@@ -104,6 +104,14 @@ p3t_status p3t_set_tree_params(p3t_ctx *ctx, int nleaf, int ngroup);
  * not depend on it beyond rounding and the R-MAC box B. levels in 0..4. */
 p3t_status p3t_set_group_merge_levels(p3t_ctx *ctx, int levels);
 
+/* How i-groups are mapped to warps in the tree walk.  1: one warp per group -- results are bitwise
+ * reproducible.  2: the four warps of a CTA share one group through a common stack -- keeps the GPU busy
+ * when there are few groups (small n) and shortens the tail of the launch; which warp evaluates which
+ * cell depends on timing, so accelerations and potentials are reproducible to fp32 rounding of the
+ * batch sums (about 1e-7 relative) rather than bitwise; neighbour lists are identical.  0 (default):
+ * chosen from n.  P3T_EINVAL for another value. */
+p3t_status p3t_set_walk_mode(p3t_ctx *ctx, int mode);
+
 /* Load n particles: mass[n], pos[3n] (x,y,z interleaved), both host or both
  * device (on_device).  Host data is checked for non-finite values here
  * (P3T_EINVAL); device data is checked on the GPU and the error surfaces at

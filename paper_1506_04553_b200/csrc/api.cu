@@ -217,6 +217,14 @@ extern "C" p3t_status p3t_set_group_merge_levels(p3t_ctx *ctx, int levels)
     return P3T_OK;
 }
 
+extern "C" p3t_status p3t_set_walk_mode(p3t_ctx *ctx, int mode)
+{
+    if (!ctx || mode < 0 || mode > 2) return P3T_EINVAL;
+    ctx->walk_mode = mode;
+    ctx->evaluated = false;
+    return P3T_OK;
+}
+
 // ------------------------------------------------------------------------------------------------
 // load / build / eval
 // ------------------------------------------------------------------------------------------------

@@ -30,6 +30,9 @@ typedef unsigned char u8;
 #endif
 #define WALK_STACK_SMEM 512          // stack entries per warp held in shared memory
 #define WALK_STACK_GMEM 7168         // overflow entries per warp in global memory
+#ifndef WALK_COOP_BELOW_X2
+#define WALK_COOP_BELOW_X2 3           // auto mode: one CTA per group below WALK_COOP_BELOW_X2 / 2 groups per resident warp
+#endif
 
 // Parameters handed to kernels by value.  The coefficients of W are prepared on the host in
 // double precision (set_params): for gamma <= y < 1
@@ -109,6 +112,7 @@ struct p3t_ctx {
     cudaStream_t stream;
     size_t max_n, n, nbr_capacity;
     int key_bits, max_level, nleaf, ngroup, merge_levels;
+    int walk_mode;                 // 0 auto, 1 one warp per group, 2 one CTA per group (cooperative)
     int sm_count;
     bool have_params, loaded, built, evaluated;
     bool cells_dirty;              // child counters need a memset before the next build

@@ -27,7 +27,6 @@ __device__ unsigned long long g_wprof[WP_SLOTS];
 #endif
 
 struct WarpShared {
-    u32 stack[WALK_STACK_SMEM];
     // far ring: (x, y, z, m) of each body, stored once.  The loops use a list entry as the scalar
     // (broadcast) operand of the packed instructions (SASS: FFMA2 Rd, Rj.F32, Ra.F32x2, Rb.F32x2), so
     // no duplicated pairs are needed: half the shared-memory traffic of a {x,x,y,y} layout, and a
@@ -115,14 +114,44 @@ template <int NI> struct Targets {
     __device__ __forceinline__ void seal() { vseal(nx); vseal(ny); vseal(nz); }
 };
 
-__device__ __forceinline__ u32 stack_read(const WarpShared &ws, const u32 *gstack, u32 pos)
+// Walk stack: the first `cap` entries live in shared memory, the rest in a global overflow area.
+// One warp per group: each warp owns WALK_STACK_SMEM + WALK_STACK_GMEM entries.  Cooperative mode
+// (one CTA per group): the four regions form one stack shared by the CTA's warps.
+struct StackRef {
+    u32 *smem;
+    u32 *gmem;
+    u32 cap;       // shared-memory entries
+    u32 limit;     // total entries
+};
+__device__ __forceinline__ u32 stack_read(const StackRef &st, u32 pos) { return pos < st.cap ? st.smem[pos] : st.gmem[pos - st.cap]; }
+__device__ __forceinline__ void stack_write(const StackRef &st, u32 pos, u32 v)
 {
-    return pos < WALK_STACK_SMEM ? ws.stack[pos] : gstack[pos - WALK_STACK_SMEM];
+    if (pos < st.cap) st.smem[pos] = v;
+    else st.gmem[pos - st.cap] = v;
 }
-__device__ __forceinline__ void stack_write(WarpShared &ws, u32 *gstack, u32 pos, u32 v)
+
+// Control block of the cooperative mode (one per CTA, shared memory).  Invariant: top > 0 implies
+// busy > 0 (or nobody has started), so top == 0 && busy == 0 means the walk of the group is over.
+struct CtaCtl {
+    u32 top;       // entries on the shared stack
+    u32 busy;      // warps that hold popped cells whose children are not pushed yet
+    u32 lock;
+    u32 group;     // ticket of the group in flight
+    u32 err;
+    u32 stat[2];   // list lengths (p-p, p-c entries) summed over the warps, for P3T_ARR_GROUP_STATS
+    u32 pad;
+};
+__device__ __forceinline__ u32 vload(const u32 *p) { return *reinterpret_cast<const volatile u32 *>(p); }
+__device__ __forceinline__ void vstore(u32 *p, u32 v) { *reinterpret_cast<volatile u32 *>(p) = v; }
+__device__ __forceinline__ void ctl_lock(CtaCtl *c)
 {
-    if (pos < WALK_STACK_SMEM) ws.stack[pos] = v;
-    else gstack[pos - WALK_STACK_SMEM] = v;
+    while (atomicCAS(&c->lock, 0u, 1u) != 0u) { }
+    __threadfence_block();
+}
+__device__ __forceinline__ void ctl_unlock(CtaCtl *c)
+{
+    __threadfence_block();
+    atomicExch(&c->lock, 0u);
 }
 
 // ---- p-p, plain softened Newtonian (K = W = 1): 13 FP32-pipe operations per interaction; counted as
@@ -276,30 +305,70 @@ struct WalkArgs {
     u64 *counters;
 };
 
-// pops up to 32 cells and starts the asynchronous copy of their records into the landing area
-__device__ __forceinline__ u32 pop_cells(WarpShared &ws, const u32 *gstack, const WalkArgs &A, u32 &top, u32 lane, u32 &cell)
+// starts the asynchronous copy of the records of the popped cells into the landing area
+__device__ __forceinline__ void request_cells(WarpShared &ws, const WalkArgs &A, u32 take, u32 lane, u32 cell)
 {
-    const u32 take = min(32u, top);
-    top -= take;
-    cell = 0u;
     if (lane < take) {
-        cell = stack_read(ws, gstack, top + lane);
         cp_async16(&ws.l_mac[lane], &A.cell_mac[cell]);
         cp_async8(&ws.l_meta[lane], &A.cell_meta[cell]);
         cp_async16(&ws.l_mom0[lane], &A.cell_mom0[cell]);
         cp_async16(&ws.l_mom1[lane], &A.cell_mom1[cell]);
     }
     cp_async_commit();
+}
+// pops up to 32 cells of a warp-private stack
+__device__ __forceinline__ u32 pop_cells(WarpShared &ws, const StackRef &st, const WalkArgs &A, u32 &top, u32 lane)
+{
+    const u32 take = min(32u, top);
+    top -= take;
+    const u32 cell = lane < take ? stack_read(st, top + lane) : 0u;
+    request_cells(ws, A, take, lane, cell);
     return take;
+}
+// cooperative mode: a warp without cells takes up to 32 from the shared stack; waits while other warps may
+// still push; returns 0 when the walk of the group is over
+__device__ __forceinline__ u32 coop_acquire(WarpShared &ws, const StackRef &st, CtaCtl *c, const WalkArgs &A, u32 lane)
+{
+    for (;;) {
+        u32 state = 0;   // 0: wait, 1: try, 2: maybe over
+        if (lane == 0) {
+            const u32 t = vload(&c->top), b = vload(&c->busy);
+            state = t > 0 ? 1u : (b == 0 ? 2u : 0u);
+        }
+        state = __shfl_sync(0xffffffffu, state, 0);
+        if (state == 0) { __nanosleep(200); continue; }
+        u32 t = 0;
+        if (lane == 0) { ctl_lock(c); t = vload(&c->top); }
+        t = __shfl_sync(0xffffffffu, t, 0);
+        const u32 take = min(32u, t);
+        if (take == 0) {
+            u32 b = 0;
+            if (lane == 0) { b = vload(&c->busy); ctl_unlock(c); }
+            b = __shfl_sync(0xffffffffu, b, 0);
+            if (b == 0) return 0u;
+            continue;
+        }
+        const u32 cell = lane < take ? stack_read(st, t - take + lane) : 0u;
+        __syncwarp();
+        if (lane == 0) { vstore(&c->top, t - take); vstore(&c->busy, vload(&c->busy) + 1u); ctl_unlock(c); }
+        request_cells(ws, A, take, lane, cell);
+        return take;
+    }
 }
 
 // One i-group: walk + interactions.  Walk step k consumes the 32 cell records that were requested
 // during step k-1, pushes children, requests the records of step k+1, and only then evaluates the
 // leaf bodies and the full interaction batches, so that the requests are in flight behind FP32 work.
-template <int NI>
-__device__ __forceinline__ void walk_group(WarpShared &ws, u32 *gstack, const WalkArgs &A, const P3TParams &prm, u32 gs, u32 ge,
-                                           u32 lane, u64 &tot_pp, u64 &tot_pc, u64 &tot_near)
+// COOP: the four warps of the CTA work on the same group.  Each warp holds all the group's bodies, takes
+// cells from the shared stack (under a lock, lane 0), builds and evaluates its own lists; the partial
+// sums of warps 1-3 are added to warp 0's at the end.  Which warp meets which cell depends on timing,
+// so results are reproducible to fp32 rounding of the batch sums, not bitwise.
+template <int NI, bool COOP>
+__device__ __forceinline__ void walk_group(WarpShared *wsall, const StackRef &st, CtaCtl *ctl, const WalkArgs &A,
+                                           const P3TParams &prm, u32 gs, u32 ge, u32 lane, u32 warp, u64 &tot_pp, u64 &tot_pc,
+                                           u64 &tot_near)
 {
+    WarpShared &ws = wsall[warp];
     const u32 gcount = ge - gs;
     WPROF_DECL;
     // ---- my bodies; empty slots replicate the group's first body and are flagged dead
@@ -333,13 +402,12 @@ __device__ __forceinline__ void walk_group(WarpShared &ws, u32 *gstack, const Wa
     WP(9);
 
     u32 top = 1;
-    if (lane == 0) ws.stack[0] = 0;   // root
+    if (!COOP && lane == 0) st.smem[0] = 0;   // root (cooperative mode: placed by the kernel)
     u32 far_head = 0, far_cnt = 0, near_head = 0, near_cnt = 0, pc_head = 0, pc_cnt = 0;
     u32 n_far = 0, n_near = 0, n_pc = 0;
     bool overflow = false;
     __syncwarp();
-    u32 cell;
-    u32 take = pop_cells(ws, gstack, A, top, lane, cell);
+    u32 take = COOP ? coop_acquire(ws, st, ctl, A, lane) : pop_cells(ws, st, A, top, lane);
     while (take > 0) {
         const bool have = lane < take;
         WP(8);
@@ -379,14 +447,39 @@ __device__ __forceinline__ void walk_group(WarpShared &ws, u32 *gstack, const Wa
                 if (lane >= o) inc += t;
             }
             u32 total = __shfl_sync(0xffffffffu, inc, 31);
-            if (top + total > WALK_STACK_SMEM + WALK_STACK_GMEM) { overflow = true; break; }
-            u32 pos = top + inc - nch;
-            for (u32 c = 0; c < nch; ++c) stack_write(ws, gstack, pos + c, first + c);
-            top += total;
+            if (!COOP) {
+                if (top + total > st.limit) { overflow = true; break; }
+                u32 pos = top + inc - nch;
+                for (u32 c = 0; c < nch; ++c) stack_write(st, pos + c, first + c);
+                top += total;
+                __syncwarp();
+                // ---- request the records of the next step before any interaction work
+                take = top > 0 ? pop_cells(ws, st, A, top, lane) : 0u;
+            } else {
+                // one critical section: push the children, take the next 32 cells (mostly my own children)
+                u32 base = 0;
+                if (lane == 0) { ctl_lock(ctl); base = vload(&ctl->top); }
+                base = __shfl_sync(0xffffffffu, base, 0);
+                if (base + total > st.limit) {
+                    if (lane == 0) { vstore(&ctl->top, 0u); vstore(&ctl->busy, vload(&ctl->busy) - 1u); vstore(&ctl->err, 1u); ctl_unlock(ctl); }
+                    overflow = true;
+                    break;
+                }
+                u32 pos = base + inc - nch;
+                for (u32 c = 0; c < nch; ++c) stack_write(st, pos + c, first + c);
+                __syncwarp();
+                const u32 ntop = base + total;
+                take = min(32u, ntop);
+                const u32 cell = lane < take ? stack_read(st, ntop - take + lane) : 0u;
+                __syncwarp();
+                if (lane == 0) {
+                    vstore(&ctl->top, ntop - take);
+                    if (take == 0) vstore(&ctl->busy, vload(&ctl->busy) - 1u);
+                    ctl_unlock(ctl);
+                }
+                request_cells(ws, A, take, lane, cell);
+            }
         }
-        __syncwarp();
-        // ---- request the records of the next step before any interaction work
-        take = top > 0 ? pop_cells(ws, gstack, A, top, lane, cell) : 0u;
         WP(4);
         // ---- bodies of opened leaves -> near / far rings; the next chunk of 32 bodies is loaded
         //      while the current one is tested and (when a ring fills) evaluated
@@ -466,6 +559,7 @@ __device__ __forceinline__ void walk_group(WarpShared &ws, u32 *gstack, const Wa
             pc_head = (pc_head + 32) & 63u; pc_cnt -= 32; n_pc += 32;
             __syncwarp();
         }
+        if (COOP && take == 0) take = coop_acquire(ws, st, ctl, A, lane);
     }
     cp_async_wait_all();
     WP(5);
@@ -481,7 +575,36 @@ __device__ __forceinline__ void walk_group(WarpShared &ws, u32 *gstack, const Wa
         n_near += near_cnt;
     }
     __syncwarp();
+    if (COOP) {
+        // partial sums of warps 1-3 -> their own (now dead) p-c ring, neighbour counts -> far ring; warp 0 adds
+        // them in warp order and writes the results
+        double *red = reinterpret_cast<double *>(&ws.pc[0][0]);
+        u32 *rnb = reinterpret_cast<u32 *>(&ws.far[0]);
+        if (lane == 0) { atomicAdd(&ctl->stat[0], n_far + n_near); atomicAdd(&ctl->stat[1], n_pc); }
+        if (warp != 0) {
+#pragma unroll
+            for (int b = 0; b < NI; ++b) {
+                red[(4 * b + 0) * 32 + lane] = acc.dax[b]; red[(4 * b + 1) * 32 + lane] = acc.day[b];
+                red[(4 * b + 2) * 32 + lane] = acc.daz[b]; red[(4 * b + 3) * 32 + lane] = acc.dph[b];
+                rnb[b * 32 + lane] = nnb[b];
+            }
+        }
+        __syncthreads();
+        if (warp == 0) {
+            for (u32 w = 1; w < WALK_WARPS; ++w) {
+                const double *ro = reinterpret_cast<const double *>(&wsall[w].pc[0][0]);
+                const u32 *rn = reinterpret_cast<const u32 *>(&wsall[w].far[0]);
+#pragma unroll
+                for (int b = 0; b < NI; ++b) {
+                    acc.dax[b] += ro[(4 * b + 0) * 32 + lane]; acc.day[b] += ro[(4 * b + 1) * 32 + lane];
+                    acc.daz[b] += ro[(4 * b + 2) * 32 + lane]; acc.dph[b] += ro[(4 * b + 3) * 32 + lane];
+                    nnb[b] += rn[b * 32 + lane];
+                }
+            }
+        }
+    }
     // ---- results, user order
+    if (!COOP || warp == 0) {
 #pragma unroll
     for (int b = 0; b < NI; ++b) {
         if (isorted[b] != 0xffffffffu) {
@@ -489,43 +612,74 @@ __device__ __forceinline__ void walk_group(WarpShared &ws, u32 *gstack, const Wa
             A.nbr_count[iuser[b]] = nnb[b];
         }
     }
+    }
+    if (COOP) __syncthreads();   // the rings are reused by the next group
 #ifdef P3T_WALK_PROFILE
     WP(7);
     if (lane == 0) for (int k_ = 0; k_ < WP_SLOTS; ++k_) atomicAdd(&g_wprof[k_], (unsigned long long)wp_acc[k_]);
 #endif
     // each live body met itself once on the near path (distance 0 to its own group's box)
-    tot_pp += (u64)(n_far + n_near) * gcount - gcount;
-    tot_near += (u64)n_near * gcount - gcount;
+    const u64 self = (!COOP || warp == 0) ? gcount : 0;   // counted once per group (u64 arithmetic wraps harmlessly)
+    tot_pp += (u64)(n_far + n_near) * gcount - self;
+    tot_near += (u64)n_near * gcount - self;
     tot_pc += (u64)n_pc * gcount;
 }
 
-// Persistent grid: 148 SMs x 4 CTAs x 4 warps; groups are handed out by an atomic ticket.  A group
-// of at most 32 bodies takes the one-body-per-lane path (half the FP32 work of the packed path).
-template <int NIMAX>
+// Persistent grid: 148 SMs x 4 CTAs x 4 warps; groups are handed out by an atomic ticket, one per warp
+// (COOP = false) or one per CTA (COOP = true).  A group of at most 32 bodies takes the one-body-per-lane
+// path (half the FP32 work of the packed path).
+// Shared memory: WALK_WARPS x WarpShared | WALK_WARPS x WALK_STACK_SMEM stack words | CtaCtl
+template <int NIMAX, bool COOP>
 __global__ void __launch_bounds__(WALK_WARPS * 32, WALK_CTAS)
 walk_kernel(WalkArgs A, const u32 *__restrict__ group_start, P3TParams prm, u32 *walk_stack)
 {
     extern __shared__ __align__(16) unsigned char s_raw[];
     const u32 lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    WarpShared &ws = reinterpret_cast<WarpShared *>(s_raw)[warp];
-    u32 *gstack = walk_stack + (size_t)(blockIdx.x * WALK_WARPS + warp) * WALK_STACK_GMEM;
+    WarpShared *wsall = reinterpret_cast<WarpShared *>(s_raw);
+    u32 *sstack = reinterpret_cast<u32 *>(s_raw + sizeof(WarpShared) * WALK_WARPS);
+    CtaCtl *ctl = reinterpret_cast<CtaCtl *>(sstack + WALK_WARPS * WALK_STACK_SMEM);
+    StackRef st;
+    if (COOP) {
+        st.smem = sstack; st.cap = WALK_WARPS * WALK_STACK_SMEM;
+        st.gmem = walk_stack + (size_t)blockIdx.x * WALK_WARPS * WALK_STACK_GMEM;
+        st.limit = WALK_WARPS * (WALK_STACK_SMEM + WALK_STACK_GMEM);
+    } else {
+        st.smem = sstack + warp * WALK_STACK_SMEM; st.cap = WALK_STACK_SMEM;
+        st.gmem = walk_stack + (size_t)(blockIdx.x * WALK_WARPS + warp) * WALK_STACK_GMEM;
+        st.limit = WALK_STACK_SMEM + WALK_STACK_GMEM;
+    }
     const u32 ngroups = (u32)A.counters[CNT_NGROUPS];
     u64 tot_pp = 0, tot_pc = 0, tot_near = 0;
 
     while (true) {
         u32 g = 0;
-        if (lane == 0) g = (u32)atomicAdd(&A.counters[CNT_GROUP_TICKET], 1ull);
-        g = __shfl_sync(0xffffffffu, g, 0);
+        if (COOP) {
+            if (threadIdx.x == 0) {
+                ctl->group = (u32)atomicAdd(&A.counters[CNT_GROUP_TICKET], 1ull);
+                ctl->top = 1; ctl->busy = 0; ctl->lock = 0; ctl->err = 0; ctl->stat[0] = 0; ctl->stat[1] = 0;
+                sstack[0] = 0;   // root
+            }
+            __syncthreads();
+            g = ctl->group;
+        } else {
+            if (lane == 0) g = (u32)atomicAdd(&A.counters[CNT_GROUP_TICKET], 1ull);
+            g = __shfl_sync(0xffffffffu, g, 0);
+        }
         if (g >= ngroups) break;
         const u32 gs = group_start[g], ge = group_start[g + 1];
         const u64 pp0 = tot_pp, pc0 = tot_pc;
         const u32 t0 = (u32)globaltimer_ns();
-        if (NIMAX == 2 && ge - gs > 32) walk_group<2>(ws, gstack, A, prm, gs, ge, lane, tot_pp, tot_pc, tot_near);
-        else walk_group<1>(ws, gstack, A, prm, gs, ge, lane, tot_pp, tot_pc, tot_near);
+        if (NIMAX == 2 && ge - gs > 32) walk_group<2, COOP>(wsall, st, ctl, A, prm, gs, ge, lane, warp, tot_pp, tot_pc, tot_near);
+        else walk_group<1, COOP>(wsall, st, ctl, A, prm, gs, ge, lane, warp, tot_pp, tot_pc, tot_near);
         __syncwarp();
-        if (lane == 0)   // list lengths of this group (+1: the self term removed from tot_pp) and its time window
+        // diagnostics: list lengths of this group (+1: the self term removed from tot_pp) and its time window
+        if (COOP) {
+            if (threadIdx.x == 0) A.group_stats[g] = make_uint4(ctl->stat[0], ctl->stat[1], t0, (u32)globaltimer_ns());
+            __syncthreads();   // ctl is rewritten for the next group
+        } else if (lane == 0) {
             A.group_stats[g] = make_uint4((u32)((tot_pp - pp0) / (ge - gs)) + 1u, (u32)((tot_pc - pc0) / (ge - gs)), t0,
                                           (u32)globaltimer_ns());
+        }
     }
     if (lane == 0) {
         atomicAdd(&A.counters[CNT_NPP], tot_pp);
@@ -551,11 +705,13 @@ p3t_status p3t_stage_walk(p3t_ctx *ctx)
     P3T_CUDA(ctx, cudaMemsetAsync(w.counters, 0, 8 * sizeof(u64), s));   // eval counters
     u32 grid = (u32)ctx->sm_count * WALK_CTAS;
     if ((size_t)grid * WALK_WARPS > w.walk_warps_max) grid = (u32)(w.walk_warps_max / WALK_WARPS);
-    const size_t smem = sizeof(WarpShared) * WALK_WARPS;
+    const size_t smem = (sizeof(WarpShared) + WALK_STACK_SMEM * sizeof(u32)) * WALK_WARPS + sizeof(CtaCtl);
     static bool attr_set = false;
     if (!attr_set) {
-        P3T_CUDA(ctx, cudaFuncSetAttribute(walk_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        P3T_CUDA(ctx, cudaFuncSetAttribute(walk_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        P3T_CUDA(ctx, cudaFuncSetAttribute(walk_kernel<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        P3T_CUDA(ctx, cudaFuncSetAttribute(walk_kernel<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        P3T_CUDA(ctx, cudaFuncSetAttribute(walk_kernel<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        P3T_CUDA(ctx, cudaFuncSetAttribute(walk_kernel<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr_set = true;
     }
     WalkArgs A;
@@ -563,8 +719,17 @@ p3t_status p3t_stage_walk(p3t_ctx *ctx)
     A.cell_mac = w.cell_mac; A.cell_mom0 = w.cell_mom0; A.cell_mom1 = w.cell_mom1; A.cell_meta = w.cell_meta;
     A.accpot = w.accpot; A.nbr_count = w.nbr_count; A.group_stats = w.group_stats; A.pairs = w.pairs; A.pair_cap = (u64)ctx->nbr_capacity;
     A.counters = w.counters;
-    if (ctx->ngroup == 64) walk_kernel<2><<<grid, WALK_WARPS * 32, smem, s>>>(A, w.group_start, ctx->prm, w.walk_stack);
-    else walk_kernel<1><<<grid, WALK_WARPS * 32, smem, s>>>(A, w.group_start, ctx->prm, w.walk_stack);
+    // one CTA per group when there are too few groups to keep every warp busy to the end of the launch
+    // (the group count lives on the device; n / ngroup is its lower bound up to the fill of the groups)
+    bool coop = ctx->walk_mode == 2 || (ctx->walk_mode == 0 && 2 * (ctx->n / (size_t)ctx->ngroup) < (size_t)WALK_COOP_BELOW_X2 * grid * WALK_WARPS);
+    const dim3 block(WALK_WARPS * 32);
+    if (ctx->ngroup == 64) {
+        if (coop) walk_kernel<2, true><<<grid, block, smem, s>>>(A, w.group_start, ctx->prm, w.walk_stack);
+        else walk_kernel<2, false><<<grid, block, smem, s>>>(A, w.group_start, ctx->prm, w.walk_stack);
+    } else {
+        if (coop) walk_kernel<1, true><<<grid, block, smem, s>>>(A, w.group_start, ctx->prm, w.walk_stack);
+        else walk_kernel<1, false><<<grid, block, smem, s>>>(A, w.group_start, ctx->prm, w.walk_stack);
+    }
     P3T_CUDA(ctx, cudaGetLastError());
     return P3T_OK;
 }

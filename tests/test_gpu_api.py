@@ -128,6 +128,7 @@ def test_device_pointers_in_and_out(oracle):
     b = _binding()
     cfg = workloads.config(1, n=3000)
     with b.P3T(3000, key_bits=63) as ctx:
+        ctx.set_walk_mode(1)      # bitwise comparison of two evaluations: one warp per group
         ctx.set_params(cfg["eps"], cfg["theta"], cfg["r_in"], cfg["r_out"], cfg["r_search"])
         ctx.soft_force(cfg["mass"], cfg["pos"])
         acc_h, pot_h = ctx.get_acc_pot()
@@ -141,6 +142,7 @@ def test_results_are_deterministic_and_context_reusable():
     b = _binding()
     c1, c2 = workloads.config(1, n=4096), workloads.config(3, n=3000)
     with b.P3T(4096, key_bits=63) as ctx:
+        ctx.set_walk_mode(1)      # one warp per group: bitwise reproducible (include/p3t.h)
         outs = []
         for cfg in (c1, c2, c1):
             ctx.set_params(cfg["eps"], cfg["theta"], cfg["r_in"], 10 * cfg["r_out"], 12 * cfg["r_out"])
@@ -149,6 +151,30 @@ def test_results_are_deterministic_and_context_reusable():
         (a0, p0), (o0, n0) = outs[0]
         (a2, p2), (o2, n2) = outs[2]
         assert np.array_equal(a0, a2) and np.array_equal(p0, p2) and np.array_equal(o0, o2) and np.array_equal(n0, n2)
+
+
+@pytest.mark.parametrize("n", [777, 20011])
+def test_cooperative_walk_matches_one_warp_per_group(n):
+    """p3t_set_walk_mode: the CTA-per-group walk evaluates the same interactions (counts, neighbour lists
+    identical); sums differ only by the fp32 rounding of differently composed batches."""
+    b = _binding()
+    cfg = workloads.config(1, n=n)
+    with b.P3T(n, key_bits=63, nbr_capacity=256 * n) as ctx:
+        ctx.set_params(cfg["eps"], cfg["theta"], cfg["r_in"], 10 * cfg["r_out"], 12 * cfg["r_out"])
+        out = {}
+        for mode in (1, 2, 0):
+            ctx.set_walk_mode(mode)
+            ctx.soft_force(cfg["mass"], cfg["pos"])
+            st = ctx.get_stats()
+            out[mode] = (ctx.get_acc_pot(), ctx.get_neighbours(), (st["n_pp"], st["n_pc"], st["n_near"], st["n_neighbours"]))
+        (a1, p1), (o1, l1), c1 = out[1]
+        for mode in (2, 0):
+            (a2, p2), (o2, l2), c2 = out[mode]
+            assert c1 == c2 and np.array_equal(o1, o2) and np.array_equal(l1, l2)
+            rel = np.linalg.norm(a1 - a2, axis=1) / np.linalg.norm(a1, axis=1)
+            assert rel.max() <= 5e-6 and np.abs(p2 / p1 - 1).max() <= 2e-6
+        with pytest.raises(b.P3TError):
+            ctx.set_walk_mode(3)
 
 
 def test_all_bodies_at_one_point_and_massless_bodies(oracle):
