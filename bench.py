@@ -49,10 +49,10 @@ def algorithmic_bytes_tree(n, key_bits, n_cells, n_groups):
     """a1-a6 bytes the method must move (every array once per pass that reads or writes it)."""
     passes = 8 if key_bits == 63 else 4
     pack = 16 * n + 16 * n                        # a1: read mass+pos, write float4 bodies
-    keys = 16 * n + 12 * n                        # a2: read bodies, write u64 key + u32 idx
-    sort = passes * 2 * 12 * n                    # a3: each pass reads and writes (key, idx)
-    gather = 4 * n + 16 * n + 16 * n + 8 * n      # a4: idx, body in, body out, keys (common-prefix levels)
-    build = 4 * n + 32 * n_cells + 4 * n_groups   # a5: level/flag bytes per body, cell topology, group starts
+    keys = 16 * n + 8 * n                         # a2: read bodies, write u64 key (the first pass makes idx = iota itself)
+    sort = passes * 2 * 12 * n - 4 * n            # a3: each pass reads and writes (key, idx); pass 0 reads no idx
+    gather = 4 * n + 16 * n + 16 * n + 8 * n + n  # a4: idx, body in, body out, keys -> common-prefix levels (1 B)
+    build = 2 * n + 2 * n + 32 * n_cells + 4 * n_groups   # a5: c read twice, leaf level + cut flag written and read, topology, group starts
     moments = 16 * n + 88 * n_cells + 88 * n_cells  # a6: read bodies; write cells; parents re-read their children
     return dict(sort=pack + keys + sort + gather, build=build, moments=moments)
 
@@ -146,6 +146,7 @@ def main():
     ap.add_argument("--nleaf", type=int, default=None)
     ap.add_argument("--ngroup", type=int, default=None)
     ap.add_argument("--merge", type=int, default=None)
+    ap.add_argument("--walk-mode", type=int, default=None, help="p3t_set_walk_mode: 0 auto, 1 warp per group, 2 CTA per group")
     ap.add_argument("--n", type=int, default=None, help="override the particle count (not a bench value)")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -166,11 +167,9 @@ def main():
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
 
-    cfg = workloads.config(args.config, n=args.n)
-    if world > 1 and rank > 0:      # independent cluster per rank: same recipe, another seed
-        from paper_1506_04553_b200.workloads import plummer, salpeter_masses
-        pos, _ = plummer(cfg["n"], workloads.SEED_BASE + args.config + 100 * rank)
-        cfg["pos"] = np.ascontiguousarray((pos - pos.mean(axis=0)).astype(np.float32))
+    from paper_1506_04553_b200 import multi
+
+    cfg = multi.rank_config(args.config, rank, n=args.n)      # independent cluster per rank: same recipe, another seed
     n = cfg["n"]
     nleaf, ngroup = args.nleaf or cfg["nleaf"], args.ngroup or cfg["ngroup"]
     dev = f"cuda:{local}"
@@ -183,6 +182,8 @@ def main():
     ctx.set_tree_params(nleaf, ngroup)
     if args.merge is not None:
         ctx.set_group_merge_levels(args.merge)
+    if args.walk_mode is not None:
+        ctx.set_walk_mode(args.walk_mode)
 
     def step():
         ctx.load_particles(mass_d, pos_d)
@@ -211,11 +212,7 @@ def main():
     if dist:
         dist.barrier()
     clocks = sampler.stop() if sampler else None
-    ms = float(np.mean([a.elapsed_time(b) for a, b in ev]))
-    if dist:
-        t = torch.tensor([ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    total_n, ms = multi.aggregate(dist, n, float(np.mean([a.elapsed_time(b) for a, b in ev])), device=dev)
     st = ctx.get_stats()
     ph = {k: float(np.mean(v)) for k, v in phases.items()}
     ffma_scalar = ffma_packed = None
@@ -243,12 +240,9 @@ def main():
             d2h = acc_h.nbytes + pot_h.nbytes + off.nbytes + nbr.nbytes
             if it >= 2:
                 ts.append(dt)
-        te = float(np.mean(ts))
-        if dist:
-            t = torch.tensor([te], device=dev, dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            te = float(t.item())
-        e2e = {"value": world * n / te, "unit": "particles/s", "h2d_bytes_per_step": int(mass_h.nbytes + pos_h.nbytes),
+        _, te_ms = multi.aggregate(dist, n, 1e3 * float(np.mean(ts)), device=dev)
+        te = 1e-3 * te_ms
+        e2e = {"value": total_n / te, "unit": "particles/s", "h2d_bytes_per_step": int(mass_h.nbytes + pos_h.nbytes),
                "d2h_bytes_per_step": int(d2h), "ms_per_step": 1e3 * te}
 
     if rank != 0:
@@ -257,6 +251,14 @@ def main():
         return
 
     peaks = measured_peaks()
+    # DRAM traffic of the dominant kernel per launch: from the committed ncu --set full capture of this workload
+    traffic, traffic_src = None, None
+    tp = os.path.join(ROOT, "profiles", "walk_kernel_dram_r1.json")
+    if os.path.exists(tp):
+        tj = json.load(open(tp))
+        if tj.get("workload") == cfg["name"]:
+            traffic = tj["dram_bytes_read"] + tj["dram_bytes_write"]
+            traffic_src = "profiles/walk_kernel_dram_r1.json (ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum)"
     n_sm = torch.cuda.get_device_properties(local).multi_processor_count
     fp32_peak = 2 * FP32_LANES * n_sm * peaks["sm_max_mhz"] * 1e6 / 1e12          # TFLOP/s at the max SM clock
     flops = FLOP_PP * st["n_pp"] + FLOP_PC * st["n_pc"]
@@ -264,10 +266,11 @@ def main():
     ab = algorithmic_bytes_tree(n, cfg["key_bits"], st["n_cells"], st["n_groups"])
     hbm = {k: ab[k] / (ph["ms_" + k] * 1e-3) / 1e9 for k in ab}
     tree_ms = ph["ms_sort"] + ph["ms_build"] + ph["ms_moments"]
-    launches = 1 + (2 + st["sort_passes"] + 1) + 4 + 1 + 1 + 5
+    # pack | keys+hist, onesweep passes, gather | levels, emit | moments (leaves, internal) | walk | neighbour CSR (5)
+    launches = 1 + (1 + st["sort_passes"] + 1) + 2 + 2 + 1 + 5
 
     out = {
-        "metric": METRIC, "value": world * n / (ms * 1e-3), "unit": "particles/s", "n_gpus": world, "steps": args.steps,
+        "metric": METRIC, "value": multi.throughput(total_n, ms), "unit": "particles/s", "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": cfg["name"], "n": n, "theta": cfg["theta"], "eps": cfg["eps"], "r_out": cfg["r_out"],
@@ -280,7 +283,7 @@ def main():
         "tree": {"n_cells": st["n_cells"], "n_leaves": st["n_leaves"], "n_groups": st["n_groups"], "depth": st["depth"]},
         "phases_ms": ph,
         "roofline": {"bound": "alu", "kernel": "walk_kernel (a7+a8)", "achieved": walk_tflops, "peak": fp32_peak, "unit": "TFLOP/s",
-                     "frac": walk_tflops / fp32_peak, "traffic": None,
+                     "frac": walk_tflops / fp32_peak, "traffic": traffic, "traffic_source": traffic_src,
                      "peak_source": f"2 flop x {FP32_LANES} lanes x {n_sm} SMs x {peaks['sm_max_mhz']:.0f} MHz ({peaks['source']} sm_max_mhz; DESIGN.md section 8)",
                      "convention": f"{FLOP_PP} flop per p-p, {FLOP_PC} flop per p-c",
                      "ffma_microbench_tflops": {"scalar": ffma_scalar, "packed": ffma_packed},

@@ -161,7 +161,7 @@ __global__ void __launch_bounds__(256) keys_hist_kernel(const float4 *__restrict
 #define OS_FLAG_AGG 0x40000000u
 #define OS_FLAG_INC 0x80000000u
 #define OS_VAL_MASK 0x3fffffffu
-#define SORT_LOOKBACK 8
+#define SORT_LOOKBACK 16   // sentinel rows in front of row 0 (the widest look-back window)
 
 __device__ __forceinline__ u32 ld_status(const u32 *p)
 {
@@ -176,6 +176,21 @@ __device__ __forceinline__ void st_status(u32 *p, u32 v)
 
 __global__ void fill_u32_kernel(u32 *p, u32 v) { p[blockIdx.x * blockDim.x + threadIdx.x] = v; }
 
+// lanes of the warp that hold the same 8-bit digit: eight ballots.  (MATCH.ANY gives the same mask in one
+// instruction but sustains only about one warp instruction per 35 cycles per SM on B200 -- it was a third of the
+// pass; VOTE runs at ALU rate.)
+__device__ __forceinline__ u32 digit_peers(u32 d)
+{
+    u32 m = 0xffffffffu;
+#pragma unroll
+    for (int b = 0; b < 8; ++b) {
+        const bool bit = (d >> b) & 1u;
+        const u32 bal = __ballot_sync(0xffffffffu, bit);
+        m &= bit ? bal : ~bal;
+    }
+    return m;
+}
+
 struct OnesweepSmem {
     union {
         u32 whist[SORT_THREADS / 32][256];                      // ranking: per-warp digit counts
@@ -189,6 +204,7 @@ struct OnesweepSmem {
 
 // status rows -SORT_LOOKBACK..-1 (in front of row 0) permanently hold INC | 0, so the look-back
 // window never needs a bounds check
+template <int LB>   // look-back window: 16 when the whole grid is resident (all tiles publish at once), 8 otherwise
 __global__ void __launch_bounds__(SORT_THREADS, 2) onesweep_kernel(const u64 *__restrict__ kin, const u32 *__restrict__ vin,
                                                                    u64 *__restrict__ kout, u32 *__restrict__ vout, u32 n,
                                                                    int shift, const u32 *__restrict__ ghist, u32 *status,
@@ -197,7 +213,9 @@ __global__ void __launch_bounds__(SORT_THREADS, 2) onesweep_kernel(const u64 *__
     extern __shared__ __align__(16) unsigned char os_raw[];
     OnesweepSmem &sm = *reinterpret_cast<OnesweepSmem *>(os_raw);
     const u32 tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    if (tid == 0) sm.tile = (u32)atomicAdd(ticket, 1ull);
+    // tiles must start in index order for the look-back to make progress: guaranteed by a ticket, or by the
+    // grid being resident as a whole (ticket == nullptr)
+    if (tid == 0) sm.tile = ticket ? (u32)atomicAdd(ticket, 1ull) : blockIdx.x;
 #pragma unroll
     for (u32 t = 0; t < 8; ++t) sm.whist[warp][t * 32 + lane] = 0;
     __syncthreads();
@@ -234,7 +252,7 @@ __global__ void __launch_bounds__(SORT_THREADS, 2) onesweep_kernel(const u64 *__
     // forming a chain of match -> load -> store -> shuffle latencies.
     u32 peers[SORT_ITEMS];
 #pragma unroll
-    for (int k = 0; k < SORT_ITEMS; ++k) peers[k] = __match_any_sync(0xffffffffu, (u32)(key[k] >> shift) & 255u);
+    for (int k = 0; k < SORT_ITEMS; ++k) peers[k] = digit_peers((u32)(key[k] >> shift) & 255u);
 #pragma unroll
     for (int k = 0; k < SORT_ITEMS; ++k) {
         u32 d = (u32)(key[k] >> shift) & 255u;
@@ -281,13 +299,13 @@ __global__ void __launch_bounds__(SORT_THREADS, 2) onesweep_kernel(const u64 *__
             const u32 *p = status + (size_t)(tile - 1) * 256 + tid;
             bool done = false;
             while (!done) {
-                u32 v[SORT_LOOKBACK];
+                u32 v[LB];
 #pragma unroll
-                for (int k = 0; k < SORT_LOOKBACK; ++k) v[k] = ld_status(p - k * 256);
+                for (int k = 0; k < LB; ++k) v[k] = ld_status(p - k * 256);
                 bool go = true;
                 u32 used = 0;
 #pragma unroll
-                for (int k = 0; k < SORT_LOOKBACK; ++k) {
+                for (int k = 0; k < LB; ++k) {
                     const bool ready = v[k] >= OS_FLAG_AGG, isinc = v[k] >= OS_FLAG_INC;
                     if (go && ready) { excl += v[k] & OS_VAL_MASK; ++used; }
                     done = done || (go && isinc);
@@ -362,10 +380,15 @@ p3t_status p3t_stage_sort(p3t_ctx *ctx)
     u32 ntiles = div_up(n, SORT_TILE);
     static bool attr_set = false;
     if (!attr_set) {
-        P3T_CUDA(ctx, cudaFuncSetAttribute(onesweep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(OnesweepSmem)));
+        P3T_CUDA(ctx, cudaFuncSetAttribute(onesweep_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(OnesweepSmem)));
+        P3T_CUDA(ctx, cudaFuncSetAttribute(onesweep_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(OnesweepSmem)));
         attr_set = true;
     }
     const size_t status_rows = w.n_tiles_max + SORT_LOOKBACK;   // SORT_LOOKBACK sentinel rows in front of row 0
+    static int ctas_per_sm = 0;
+    if (!ctas_per_sm)
+        P3T_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas_per_sm, onesweep_kernel<16>, SORT_THREADS, sizeof(OnesweepSmem)));
+    const int resident = ctas_per_sm * ctx->sm_count;   // a grid up to this size is co-resident: no ticket needed
     if (!ctx->status_clean) {   // first build of this context: buffers zeroed, sentinel rows = INC | 0 
         P3T_CUDA(ctx, cudaMemsetAsync(w.tile_status, 0, 2 * status_rows * 256 * sizeof(u32), s));
         for (int b = 0; b < 2; ++b)
@@ -386,9 +409,14 @@ p3t_status p3t_stage_sort(p3t_ctx *ctx)
     for (int p = 0; p < passes; ++p) {
         u32 *st_cur = w.tile_status + ((size_t)(p & 1) * status_rows + SORT_LOOKBACK) * 256;
         u32 *st_next = w.tile_status + ((size_t)((p + 1) & 1) * status_rows + SORT_LOOKBACK) * 256;
-        onesweep_kernel<<<ntiles, SORT_THREADS, sizeof(OnesweepSmem), s>>>(w.keys[cur], p == 0 ? nullptr : w.idx[cur], w.keys[cur ^ 1],
-                                                                           w.idx[cur ^ 1], n, 8 * p, w.hist + p * 256, st_cur, st_next,
-                                                                           w.counters + CNT_SORT_TICKET + p);
+        const u32 *vin = p == 0 ? nullptr : w.idx[cur];
+        if (ntiles <= (u32)resident)
+            onesweep_kernel<16><<<ntiles, SORT_THREADS, sizeof(OnesweepSmem), s>>>(w.keys[cur], vin, w.keys[cur ^ 1], w.idx[cur ^ 1], n, 8 * p,
+                                                                                   w.hist + p * 256, st_cur, st_next, nullptr);
+        else
+            onesweep_kernel<8><<<ntiles, SORT_THREADS, sizeof(OnesweepSmem), s>>>(w.keys[cur], vin, w.keys[cur ^ 1], w.idx[cur ^ 1], n, 8 * p,
+                                                                                  w.hist + p * 256, st_cur, st_next,
+                                                                                  w.counters + CNT_SORT_TICKET + p);
         cur ^= 1;
     }
     ctx->cur = cur;

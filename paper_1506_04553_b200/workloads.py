@@ -153,16 +153,17 @@ def dr_buff(dt_soft):
     return 3.0 * SIGMA_3D * dt_soft
 
 
-def config(k, n=None):
+def config(k, n=None, seed_offset=0):
     """Workload k = 1..5 of BASELINE.json.  n overrides the particle count
     (used by tests to run a config's recipe at a size the oracle can afford).
 
     Returns a dict: mass, pos, vel as fp32 arrays (the GPU input; the oracle gets
     the same values widened to fp64) and eps, theta, r_in, r_out, r_search,
     nleaf, ngroup, key_bits, plus name / dt_soft where the config has one.
-    Missing values follow DESIGN.md section 3 (readings A17).
+    Missing values follow DESIGN.md section 3 (readings A17).  seed_offset draws another
+    realisation of the same recipe (multi.py: one independent cluster per rank).
     """
-    seed = SEED_BASE + k
+    seed = SEED_BASE + k + seed_offset
     if k == 1:
         n = n or 4096
         pos, vel = plummer(n, seed)

@@ -1,0 +1,64 @@
+"""N > 1 launch logic on CPU: two processes over gloo (rendezvous on 127.0.0.1).
+
+The soft-force path does not shard (one cluster per GPU, no data-path collective);
+what ranks exchange is only the timing reduction of bench.py, which lives in paper_1506_04553_b200/multi.py.
+"""
+import os
+import socket
+
+import numpy as np
+import pytest
+
+from paper_1506_04553_b200 import multi, workloads
+
+
+def _free_port():
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    p = s.getsockname()[1]
+    s.close()
+    return p
+
+
+def _worker(rank, world, port, q):
+    import torch.distributed as dist
+
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        cfg = multi.rank_config(1, rank, n=512)
+        fake_ms = [3.0, 5.0][rank]           # rank 1 is the slow one
+        units, ms = multi.aggregate(dist, cfg["n"], fake_ms)
+        dist.barrier()
+        q.put((rank, units, ms, float(cfg["pos"][0, 0]), cfg["n"], cfg["theta"]))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_two_ranks_over_gloo_aggregate_units_and_take_the_slowest_time():
+    import torch.multiprocessing as mp
+
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    out = sorted(q.get(timeout=120) for _ in range(2))
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    (r0, u0, ms0, x0, n0, th0), (r1, u1, ms1, x1, n1, th1) = out
+    assert (u0, u1) == (1024, 1024) and ms0 == ms1 == 5.0          # sum of units, max of times, same on every rank
+    assert n0 == n1 == 512 and th0 == th1                          # weak scaling: same problem size and parameters
+    assert x0 != x1                                                # but an independent cluster per rank
+    assert multi.throughput(u0, ms0) == pytest.approx(1024 / 5e-3)
+
+
+def test_rank_zero_is_the_single_gpu_workload_and_single_process_needs_no_backend():
+    a, b = multi.rank_config(1, 0, n=256), workloads.config(1, n=256)
+    assert np.array_equal(a["pos"], b["pos"]) and np.array_equal(a["mass"], b["mass"])
+    assert multi.aggregate(None, 256, 2.5) == (256, 2.5)
+    c = multi.rank_config(4, 1, n=256)                             # King model keeps its own generator
+    assert c["pos"].shape == (256, 3) and not np.array_equal(c["pos"], multi.rank_config(4, 0, n=256)["pos"])
