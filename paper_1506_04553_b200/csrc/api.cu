@@ -52,6 +52,8 @@ size_t p3t_layout(Workspace &ws, char *base, size_t max_n, int key_bits, size_t 
     ws.prev_ncells = b.take<u32>(4);
     ws.group_start = b.take<u32>(n + 1);
     ws.group_stats = b.take<uint4>(n);
+    ws.group_order = b.take<u32>(n);
+    ws.order_meta = b.take<u32>(4);
     ws.cell_mac = b.take<float4>(ws.cell_cap);
     ws.cell_mom0 = b.take<float4>(ws.cell_cap);
     ws.cell_mom1 = b.take<float4>(ws.cell_cap);
@@ -129,6 +131,7 @@ extern "C" p3t_status p3t_create(p3t_ctx **out, int device, size_t max_n, int ke
         return P3T_ENOMEM;
     }
     ctx->base = static_cast<char *>(workspace);
+    if (cudaMemsetAsync(ctx->ws.order_meta, 0, 4 * sizeof(u32), ctx->stream) != cudaSuccess) { delete ctx; return P3T_ECUDA; }
     for (int i = 0; i < 8; ++i) {
         if (cudaEventCreate(&ctx->ev[i]) != cudaSuccess) { delete ctx; return P3T_ECUDA; }
     }

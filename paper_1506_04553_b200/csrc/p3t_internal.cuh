@@ -87,6 +87,8 @@ struct Workspace {
     u32 *prev_ncells;              // [1] cells of the previous build: their child counters are zeroed by the next one
     u32 *group_start;              // [n+1]
     uint4 *group_stats;            // [n] per-group diagnostics of the last walk (P3T_ARR_GROUP_STATS)
+    u32 *group_order;              // [n] groups by decreasing cost of the previous walk (ticket -> group)
+    u32 *order_meta;               // [4] [0]: number of groups group_order is a permutation of (0: none)
     // cells
     float4 *cell_mac, *cell_mom0, *cell_mom1, *cell_bmin, *cell_bmax;
     uint2 *cell_meta;

@@ -397,7 +397,7 @@ p3t_status p3t_stage_sort(p3t_ctx *ctx)
     }
     P3T_CUDA(ctx, cudaMemsetAsync(w.counters + CNT_NCELLS, 0, 16 * sizeof(u64), s));   // build counters + sort tickets
     P3T_CUDA(ctx, cudaMemsetAsync(w.hist, 0, 8 * 256 * sizeof(u32), s));
-    u32 grid = min(div_up(n, 256 * 4), (u32)ctx->sm_count * 8);
+    u32 grid = min(div_up(n, 256 * 8), (u32)ctx->sm_count * 8);   // every CTA flushes 8 x 256 histogram bins with global atomics: few, fat CTAs
     if (ctx->cells_dirty) {   // first build, or the last one ended in an error: all child counters and prev_ncells -> 0
         P3T_CUDA(ctx, cudaMemsetAsync(w.cell_nchild, 0, (size_t)((char *)(w.cell_ready + w.cell_cap) - (char *)w.cell_nchild), s));
         P3T_CUDA(ctx, cudaMemsetAsync(w.prev_ncells, 0, sizeof(u32), s));

@@ -300,6 +300,8 @@ struct WalkArgs {
     float4 *__restrict__ accpot;
     u32 *__restrict__ nbr_count;
     uint4 *__restrict__ group_stats;
+    const u32 *__restrict__ group_order;   // ticket -> group, valid if order_meta[0] == number of groups
+    const u32 *__restrict__ order_meta;
     uint2 *pairs;
     u64 pair_cap;
     u64 *counters;
@@ -649,6 +651,7 @@ walk_kernel(WalkArgs A, const u32 *__restrict__ group_start, P3TParams prm, u32 
         st.limit = WALK_STACK_SMEM + WALK_STACK_GMEM;
     }
     const u32 ngroups = (u32)A.counters[CNT_NGROUPS];
+    const bool ordered = A.order_meta[0] == ngroups;   // heaviest groups of the previous call first
     u64 tot_pp = 0, tot_pc = 0, tot_near = 0;
 
     while (true) {
@@ -666,6 +669,7 @@ walk_kernel(WalkArgs A, const u32 *__restrict__ group_start, P3TParams prm, u32 
             g = __shfl_sync(0xffffffffu, g, 0);
         }
         if (g >= ngroups) break;
+        if (ordered) g = A.group_order[g];
         const u32 gs = group_start[g], ge = group_start[g + 1];
         const u64 pp0 = tot_pp, pc0 = tot_pc;
         const u32 t0 = (u32)globaltimer_ns();
@@ -686,6 +690,58 @@ walk_kernel(WalkArgs A, const u32 *__restrict__ group_start, P3TParams prm, u32 
         atomicAdd(&A.counters[CNT_NPC], tot_pc);
         atomicAdd(&A.counters[CNT_NNEAR], tot_near);
     }
+}
+
+// Groups by decreasing cost of the walk that just ran (list lengths x 13 / 33 packed operations, halved for
+// the one-body-per-lane path): the next call hands them out in this order, so the long ones start first
+// and the tail of the persistent launch is made of short ones.  Counting sort on 1024 cost classes, one CTA.
+// The order is only a schedule: results do not depend on it.
+__global__ void __launch_bounds__(1024) group_order_kernel(const uint4 *__restrict__ stats, const u32 *__restrict__ group_start,
+                                                           const u64 *__restrict__ counters, u32 *__restrict__ order, u32 *order_meta)
+{
+    __shared__ u32 s_bin[1024];
+    __shared__ u32 s_warp[32];
+    __shared__ u32 s_max;
+    const u32 ng = (u32)counters[CNT_NGROUPS], tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    auto cost = [&](u32 g) {
+        const uint4 st = stats[g];
+        const u32 c = 13u * st.x + 33u * st.y;
+        return (group_start[g + 1] - group_start[g] > 32u) ? 2u * c : c;
+    };
+    u32 mx = 1;
+    for (u32 g = tid; g < ng; g += 1024) mx = max(mx, cost(g));
+    mx = __reduce_max_sync(0xffffffffu, mx);
+    if (tid == 0) s_max = 0;
+    s_bin[tid] = 0;
+    __syncthreads();
+    if (lane == 0) atomicMax(&s_max, mx);
+    __syncthreads();
+    const float scale = 1023.f / (float)s_max;
+    for (u32 g = tid; g < ng; g += 1024) atomicAdd(&s_bin[1023u - min(1023u, (u32)((float)cost(g) * scale))], 1u);
+    __syncthreads();
+    // exclusive scan of the 1024 bins (bin 0 = most expensive)
+    u32 v = s_bin[tid], inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        u32 t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t;
+    }
+    if (lane == 31) s_warp[warp] = inc;
+    __syncthreads();
+    if (warp == 0) {
+        u32 w = s_warp[lane], wi = w;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            u32 t = __shfl_up_sync(0xffffffffu, wi, o);
+            if (lane >= o) wi += t;
+        }
+        s_warp[lane] = wi - w;
+    }
+    __syncthreads();
+    s_bin[tid] = s_warp[warp] + inc - v;
+    __syncthreads();
+    for (u32 g = tid; g < ng; g += 1024) order[atomicAdd(&s_bin[1023u - min(1023u, (u32)((float)cost(g) * scale))], 1u)] = g;
+    if (tid == 0) order_meta[0] = ng;
 }
 
 #ifdef P3T_WALK_PROFILE
@@ -719,6 +775,8 @@ p3t_status p3t_stage_walk(p3t_ctx *ctx)
     A.cell_mac = w.cell_mac; A.cell_mom0 = w.cell_mom0; A.cell_mom1 = w.cell_mom1; A.cell_meta = w.cell_meta;
     A.accpot = w.accpot; A.nbr_count = w.nbr_count; A.group_stats = w.group_stats; A.pairs = w.pairs; A.pair_cap = (u64)ctx->nbr_capacity;
     A.counters = w.counters;
+    A.group_order = w.group_order;
+    A.order_meta = w.order_meta;
     // one CTA per group when there are too few groups to keep every warp busy to the end of the launch
     // (the group count lives on the device; n / ngroup is its lower bound up to the fill of the groups)
     bool coop = ctx->walk_mode == 2 || (ctx->walk_mode == 0 && 2 * (ctx->n / (size_t)ctx->ngroup) < (size_t)WALK_COOP_BELOW_X2 * grid * WALK_WARPS);
@@ -730,6 +788,7 @@ p3t_status p3t_stage_walk(p3t_ctx *ctx)
         if (coop) walk_kernel<1, true><<<grid, block, smem, s>>>(A, w.group_start, ctx->prm, w.walk_stack);
         else walk_kernel<1, false><<<grid, block, smem, s>>>(A, w.group_start, ctx->prm, w.walk_stack);
     }
+    group_order_kernel<<<1, 1024, 0, s>>>(w.group_stats, w.group_start, w.counters, w.group_order, w.order_meta);
     P3T_CUDA(ctx, cudaGetLastError());
     return P3T_OK;
 }
