@@ -224,6 +224,13 @@ class P3T:
         self._check(_lib.p3t_get_neighbours(self._h, offset.ctypes.data, nbr.ctypes.data, cap, 0))
         return offset, nbr[: int(offset[-1])]
 
+    def get_neighbours_into(self, offset, nbr):
+        """Same, into caller-provided host buffers (e.g. pinned): offset uint64[n+1], nbr uint32[capacity].
+        Returns the total number of entries."""
+        assert offset.dtype == np.uint64 and offset.size >= self.n + 1 and nbr.dtype == np.uint32
+        self._check(_lib.p3t_get_neighbours(self._h, offset.ctypes.data, nbr.ctypes.data, nbr.size, 0))
+        return int(offset[self.n])
+
     def get_stats(self):
         s = Stats()
         self._check(_lib.p3t_get_stats(self._h, C.byref(s)))

@@ -3,6 +3,8 @@
 #include <math.h>
 #include <new>
 #include <stdlib.h>
+#include <thread>
+#include <vector>
 
 #include "p3t_internal.cuh"
 
@@ -231,6 +233,32 @@ extern "C" p3t_status p3t_set_walk_mode(p3t_ctx *ctx, int mode)
 // ------------------------------------------------------------------------------------------------
 // load / build / eval
 // ------------------------------------------------------------------------------------------------
+// Host-side finiteness check of the input (an exponent of all ones marks inf/nan): a branch-free OR over the
+// words, which the host compiler vectorises, split over a few threads for large inputs -- a scalar isfinite()
+// loop cost 2.5 ms per 1M particles, a quarter of the GPU time of the whole evaluation.
+static bool host_all_finite(const float *p, size_t count)
+{
+    auto scan = [](const float *q, size_t m) {
+        const uint32_t *w = reinterpret_cast<const uint32_t *>(q);
+        uint32_t bad = 0;
+        for (size_t i = 0; i < m; ++i) bad |= ((w[i] & 0x7f800000u) == 0x7f800000u) ? 1u : 0u;
+        return bad == 0;
+    };
+    const size_t nthr = count >= (size_t(1) << 18) ? 8 : 1;
+    if (nthr == 1) return scan(p, count);
+    std::vector<char> ok(nthr, 1);
+    std::vector<std::thread> th;
+    const size_t per = (count + nthr - 1) / nthr;
+    for (size_t t = 0; t < nthr; ++t) {
+        const size_t b = t * per, e = b + per < count ? b + per : count;
+        if (b >= e) break;
+        th.emplace_back([&, t, b, e] { ok[t] = scan(p + b, e - b) ? 1 : 0; });
+    }
+    for (auto &x : th) x.join();
+    for (char c : ok) if (!c) return false;
+    return true;
+}
+
 extern "C" p3t_status p3t_load_particles(p3t_ctx *ctx, size_t n, const float *mass, const float *pos, int on_device)
 {
     if (!ctx) return P3T_EINVAL;
@@ -239,10 +267,8 @@ extern "C" p3t_status p3t_load_particles(p3t_ctx *ctx, size_t n, const float *ma
     P3T_CUDA(ctx, cudaSetDevice(ctx->device));
     const float *d_mass = mass, *d_pos = pos;
     if (!on_device) {
-        for (size_t i = 0; i < n; ++i)
-            if (!isfinite(mass[i])) return p3t_fail(ctx, P3T_EINVAL, "non-finite mass");
-        for (size_t i = 0; i < 3 * n; ++i)
-            if (!isfinite(pos[i])) return p3t_fail(ctx, P3T_EINVAL, "non-finite position");
+        if (!host_all_finite(mass, n)) return p3t_fail(ctx, P3T_EINVAL, "non-finite mass");
+        if (!host_all_finite(pos, 3 * n)) return p3t_fail(ctx, P3T_EINVAL, "non-finite position");
         P3T_CUDA(ctx, cudaMemcpyAsync(ctx->ws.in_mass, mass, n * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
         P3T_CUDA(ctx, cudaMemcpyAsync(ctx->ws.in_pos, pos, 3 * n * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
         d_mass = ctx->ws.in_mass;
