@@ -179,9 +179,12 @@ typedef enum {
     P3T_ARR_GROUP_START = 11, /* uint32[n_groups + 1] */
     P3T_ARR_CELL_BMIN   = 12, /* float4[n_cells]: tight AABB min of the cell's bodies */
     P3T_ARR_CELL_BMAX   = 13, /* float4[n_cells] */
-    P3T_ARR_GROUP_STATS = 14  /* uint32[4][n_groups], valid after p3t_eval_soft: p-p list length,
+    P3T_ARR_GROUP_STATS = 14, /* uint32[4][n_groups], valid after p3t_eval_soft: p-p list length,
                                  p-c list length, start and end of the group's walk in ns
                                  (low 32 bits of %globaltimer) -- load-balance diagnostics */
+    P3T_ARR_GROUP_ORDER = 15  /* uint32[n_groups], valid after p3t_eval_soft: the groups by decreasing cost of that
+                                 walk (13 x p-p + 33 x p-c list length, doubled for groups of more than 32 bodies);
+                                 the next p3t_eval_soft hands the groups to the warps in this order */
 } p3t_array;
 p3t_status p3t_array_info(p3t_ctx *ctx, p3t_array which, size_t *count, size_t *elem_bytes);
 p3t_status p3t_copy_array(p3t_ctx *ctx, p3t_array which, void *dst, size_t dst_bytes, int on_device);

@@ -36,7 +36,7 @@ SYMBOLS = [
 ARRAYS = dict(root_cube=(0, np.float32, 1), keys=(1, np.uint64, 1), sorted_idx=(2, np.uint32, 1),
               bodies=(3, np.float32, 4), cell_mac=(4, np.float32, 4), cell_mom0=(5, np.float32, 4),
               cell_mom1=(6, np.float32, 4), cell_meta=(7, np.uint32, 2), cell_level=(8, np.uint8, 1),
-              cell_start=(9, np.uint32, 1), cell_parent=(10, np.uint32, 1), group_start=(11, np.uint32, 1), group_stats=(14, np.uint32, 4),
+              cell_start=(9, np.uint32, 1), cell_parent=(10, np.uint32, 1), group_start=(11, np.uint32, 1), group_stats=(14, np.uint32, 4), group_order=(15, np.uint32, 1),
               cell_bmin=(12, np.float32, 4), cell_bmax=(13, np.float32, 4))
 
 

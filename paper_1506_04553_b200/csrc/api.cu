@@ -472,6 +472,7 @@ static p3t_status array_desc(p3t_ctx *ctx, p3t_array which, const void **ptr, si
     case P3T_ARR_CELL_BMIN:   *ptr = w.cell_bmin; *count = nc; *elem = 16; break;
     case P3T_ARR_CELL_BMAX:   *ptr = w.cell_bmax; *count = nc; *elem = 16; break;
     case P3T_ARR_GROUP_STATS: *ptr = w.group_stats; *count = ng; *elem = 16; break;
+    case P3T_ARR_GROUP_ORDER: *ptr = w.group_order; *count = ng; *elem = 4; break;
     default: return p3t_fail(ctx, P3T_EINVAL, "unknown array id");
     }
     return P3T_OK;

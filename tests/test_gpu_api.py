@@ -177,6 +177,29 @@ def test_cooperative_walk_matches_one_warp_per_group(n):
             ctx.set_walk_mode(3)
 
 
+def test_group_order_is_a_permutation_by_decreasing_cost_and_changes_nothing():
+    """The schedule of the next walk (groups by decreasing measured cost) is a permutation of the groups,
+    sorted by the cost the header defines up to the 1024 cost classes, and leaves the results bitwise alike."""
+    b = _binding()
+    cfg = workloads.config(3, n=60000)
+    with b.P3T(cfg["n"], key_bits=63) as ctx:
+        ctx.set_walk_mode(1)
+        ctx.set_params(cfg["eps"], cfg["theta"], cfg["r_in"], cfg["r_out"], cfg["r_search"])
+        ctx.soft_force(cfg["mass"], cfg["pos"])          # Morton order (no history)
+        a0, p0 = ctx.get_acc_pot()
+        order = ctx.array("group_order").astype(np.int64)
+        stats = ctx.array("group_stats").astype(np.int64)
+        gs = ctx.array("group_start").astype(np.int64)
+        ng = len(gs) - 1
+        assert np.array_equal(np.sort(order), np.arange(ng))
+        cost = (13 * stats[:, 0] + 33 * stats[:, 1]) * np.where(np.diff(gs) > 32, 2, 1)
+        cls = np.minimum(1023, (cost[order].astype(np.float32) * (np.float32(1023.0) / np.float32(cost.max()))).astype(np.int64))
+        assert np.all(np.diff(cls) <= 0)
+        ctx.soft_force(cfg["mass"], cfg["pos"])          # same tree: groups handed out in that order
+        a1, p1 = ctx.get_acc_pot()
+        assert np.array_equal(a0, a1) and np.array_equal(p0, p1)
+
+
 def test_all_bodies_at_one_point_and_massless_bodies(oracle):
     b = _binding()
     n = 100

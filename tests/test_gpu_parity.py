@@ -173,14 +173,15 @@ def test_config2_leapfrog_calls(oracle):
             pos = np.ascontiguousarray(pos + dt * vel, dtype=np.float32)
 
 
-@pytest.mark.parametrize("k,n", [(3, 1 << 20), (4, 1 << 18)])
+@pytest.mark.parametrize("k,n", [(3, 1 << 20), (4, 1 << 18), (5, 1 << 22)])
 def test_full_size_sampled_parity(oracle, k, n):
-    """BASELINE configs 3 and 4 at full size, in bench.py's launch configuration; accuracy on a seeded
-    4096-subset against the direct sum and against O4; neighbour sets on the same subset; symmetry on all."""
+    """BASELINE configs 3, 4 and 5 at full size, in bench.py's launch configuration; accuracy on a seeded
+    4096-subset (2048 at N = 4M) against the direct sum and against O4; neighbour sets on the same subset;
+    symmetry on all."""
     cfg = workloads.config(k)
     assert cfg["n"] == n
     m, q = widen(cfg)
-    sub = np.sort(np.random.default_rng(cfg["config"]).choice(n, 4096, replace=False)).astype(np.int64)
+    sub = np.sort(np.random.default_rng(cfg["config"]).choice(n, 2048 if k == 5 else 4096, replace=False)).astype(np.int64)
     a, p = oracle.direct(m, q, cfg["eps"], cfg["r_in"], cfg["r_out"], subset=sub)
     tree = oracle.Tree(m, q, nleaf=cfg["nleaf"], max_depth=21)
     o4 = tree.walk(cfg["eps"], cfg["theta"], cfg["r_in"], cfg["r_out"], cfg["r_search"], subset=sub)
