@@ -19,7 +19,9 @@ typedef unsigned char u8;
 #define P3T_NO_PARENT 0xffffffffu
 
 // ---- tuning constants -------------------------------------------------
+#ifndef SORT_THREADS
 #define SORT_THREADS 512
+#endif
 #define SORT_ITEMS 8
 #define SORT_TILE (SORT_THREADS * SORT_ITEMS)
 #define BUILD_THREADS 256

@@ -205,7 +205,7 @@ struct OnesweepSmem {
 // status rows -SORT_LOOKBACK..-1 (in front of row 0) permanently hold INC | 0, so the look-back
 // window never needs a bounds check
 template <int LB>   // look-back window: 16 when the whole grid is resident (all tiles publish at once), 8 otherwise
-__global__ void __launch_bounds__(SORT_THREADS, 2) onesweep_kernel(const u64 *__restrict__ kin, const u32 *__restrict__ vin,
+__global__ void __launch_bounds__(SORT_THREADS, 1024 / SORT_THREADS) onesweep_kernel(const u64 *__restrict__ kin, const u32 *__restrict__ vin,
                                                                    u64 *__restrict__ kout, u32 *__restrict__ vout, u32 n,
                                                                    int shift, const u32 *__restrict__ ghist, u32 *status,
                                                                    u32 *status_next, u64 *ticket)
