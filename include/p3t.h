@@ -183,7 +183,8 @@ typedef enum {
                                  p-c list length, start and end of the group's walk in ns
                                  (low 32 bits of %globaltimer) -- load-balance diagnostics */
     P3T_ARR_GROUP_ORDER = 15  /* uint32[n_groups], valid after p3t_eval_soft: the groups by decreasing cost of that
-                                 walk (13 x p-p + 33 x p-c list length, doubled for groups of more than 32 bodies);
+                                 walk (13 x p-p + 33 x p-c list length, doubled for groups of more than 32 bodies; sorted by
+                                 cost class, eight classes per octave, any order inside a class);
                                  the next p3t_eval_soft hands the groups to the warps in this order */
 } p3t_array;
 p3t_status p3t_array_info(p3t_ctx *ctx, p3t_array which, size_t *count, size_t *elem_bytes);

@@ -56,6 +56,8 @@ size_t p3t_layout(Workspace &ws, char *base, size_t max_n, int key_bits, size_t 
     ws.group_stats = b.take<uint4>(n);
     ws.group_order = b.take<u32>(n);
     ws.order_meta = b.take<u32>(4);
+    ws.group_class = b.take<u32>(n);
+    ws.order_hist = b.take<u32>(2048);
     ws.cell_mac = b.take<float4>(ws.cell_cap);
     ws.cell_mom0 = b.take<float4>(ws.cell_cap);
     ws.cell_mom1 = b.take<float4>(ws.cell_cap);

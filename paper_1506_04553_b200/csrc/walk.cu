@@ -291,6 +291,16 @@ __device__ __forceinline__ u64 globaltimer_ns()
     return t;
 }
 
+// cost class of a finished group (see group_order_kernel)
+#define ORDER_CLASSES 1024
+__device__ __forceinline__ u32 cost_class(u32 pp_len, u32 pc_len, bool packed)
+{
+    const u32 c = (13u * pp_len + 33u * pc_len) * (packed ? 2u : 1u);
+    const u32 bits = __float_as_uint((float)max(c, 1u)) >> 20;        // exponent and three mantissa bits
+    const u32 lo = 127u << 3;                                         // cost 1
+    return ORDER_CLASSES - 1u - min(bits - lo, (u32)ORDER_CLASSES - 1u);   // class 0 = most expensive
+}
+
 // Arguments of the walk that do not change between groups.
 struct WalkArgs {
     const float4 *__restrict__ body;
@@ -302,6 +312,8 @@ struct WalkArgs {
     uint4 *__restrict__ group_stats;
     const u32 *__restrict__ group_order;   // ticket -> group, valid if order_meta[0] == number of groups
     const u32 *__restrict__ order_meta;
+    u32 *__restrict__ group_class;   // cost class of every group of this walk
+    u32 *order_hist;                 // [ORDER_CLASSES] groups per class
     uint2 *pairs;
     u64 pair_cap;
     u64 *counters;
@@ -678,11 +690,19 @@ walk_kernel(WalkArgs A, const u32 *__restrict__ group_start, P3TParams prm, u32 
         __syncwarp();
         // diagnostics: list lengths of this group (+1: the self term removed from tot_pp) and its time window
         if (COOP) {
-            if (threadIdx.x == 0) A.group_stats[g] = make_uint4(ctl->stat[0], ctl->stat[1], t0, (u32)globaltimer_ns());
+            if (threadIdx.x == 0) {
+                A.group_stats[g] = make_uint4(ctl->stat[0], ctl->stat[1], t0, (u32)globaltimer_ns());
+                const u32 c = cost_class(ctl->stat[0], ctl->stat[1], ge - gs > 32);
+                A.group_class[g] = c;
+                atomicAdd(&A.order_hist[c], 1u);
+            }
             __syncthreads();   // ctl is rewritten for the next group
         } else if (lane == 0) {
-            A.group_stats[g] = make_uint4((u32)((tot_pp - pp0) / (ge - gs)) + 1u, (u32)((tot_pc - pc0) / (ge - gs)), t0,
-                                          (u32)globaltimer_ns());
+            const u32 lpp = (u32)((tot_pp - pp0) / (ge - gs)) + 1u, lpc = (u32)((tot_pc - pc0) / (ge - gs));
+            A.group_stats[g] = make_uint4(lpp, lpc, t0, (u32)globaltimer_ns());
+            const u32 c = cost_class(lpp, lpc, ge - gs > 32);
+            A.group_class[g] = c;
+            atomicAdd(&A.order_hist[c], 1u);
         }
     }
     if (lane == 0) {
@@ -694,33 +714,21 @@ walk_kernel(WalkArgs A, const u32 *__restrict__ group_start, P3TParams prm, u32 
 
 // Groups by decreasing cost of the walk that just ran (list lengths x 13 / 33 packed operations, halved for
 // the one-body-per-lane path): the next call hands them out in this order, so the long ones start first
-// and the tail of the persistent launch is made of short ones.  Counting sort on 1024 cost classes, one CTA.
-// The order is only a schedule: results do not depend on it.
-__global__ void __launch_bounds__(1024) group_order_kernel(const uint4 *__restrict__ stats, const u32 *__restrict__ group_start,
-                                                           const u64 *__restrict__ counters, u32 *__restrict__ order, u32 *order_meta)
+// and the tail of the persistent launch is made of short ones.  The walk kernel files every finished group
+// under a cost class (top bits of the cost as a float: 8 classes per octave) and counts the classes; this
+// kernel turns the counts into offsets (every CTA scans the 1024 counters itself) and scatters the group
+// ids.  The order is only a schedule: results do not depend on it.
+__global__ void __launch_bounds__(256) group_order_kernel(const u32 *__restrict__ gclass, const u32 *__restrict__ hist, u32 *cursor,
+                                                          const u64 *__restrict__ counters, u32 *__restrict__ order, u32 *order_meta)
 {
-    __shared__ u32 s_bin[1024];
-    __shared__ u32 s_warp[32];
-    __shared__ u32 s_max;
+    __shared__ u32 s_base[ORDER_CLASSES];
+    __shared__ u32 s_warp[8];
     const u32 ng = (u32)counters[CNT_NGROUPS], tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    auto cost = [&](u32 g) {
-        const uint4 st = stats[g];
-        const u32 c = 13u * st.x + 33u * st.y;
-        return (group_start[g + 1] - group_start[g] > 32u) ? 2u * c : c;
-    };
-    u32 mx = 1;
-    for (u32 g = tid; g < ng; g += 1024) mx = max(mx, cost(g));
-    mx = __reduce_max_sync(0xffffffffu, mx);
-    if (tid == 0) s_max = 0;
-    s_bin[tid] = 0;
-    __syncthreads();
-    if (lane == 0) atomicMax(&s_max, mx);
-    __syncthreads();
-    const float scale = 1023.f / (float)s_max;
-    for (u32 g = tid; g < ng; g += 1024) atomicAdd(&s_bin[1023u - min(1023u, (u32)((float)cost(g) * scale))], 1u);
-    __syncthreads();
-    // exclusive scan of the 1024 bins (bin 0 = most expensive)
-    u32 v = s_bin[tid], inc = v;
+    // exclusive scan of the class counts: four consecutive classes per thread
+    u32 v[4], sum = 0;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) { v[k] = hist[4 * tid + k]; sum += v[k]; }
+    u32 inc = sum;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
         u32 t = __shfl_up_sync(0xffffffffu, inc, o);
@@ -728,20 +736,17 @@ __global__ void __launch_bounds__(1024) group_order_kernel(const uint4 *__restri
     }
     if (lane == 31) s_warp[warp] = inc;
     __syncthreads();
-    if (warp == 0) {
-        u32 w = s_warp[lane], wi = w;
+    u32 base = inc - sum;
+    for (u32 w = 0; w < warp; ++w) base += s_warp[w];
 #pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            u32 t = __shfl_up_sync(0xffffffffu, wi, o);
-            if (lane >= o) wi += t;
-        }
-        s_warp[lane] = wi - w;
+    for (int k = 0; k < 4; ++k) { s_base[4 * tid + k] = base; base += v[k]; }
+    __syncthreads();
+    const u32 g = blockIdx.x * blockDim.x + tid;
+    if (g < ng) {
+        const u32 c = gclass[g];
+        order[s_base[c] + atomicAdd(&cursor[c], 1u)] = g;
     }
-    __syncthreads();
-    s_bin[tid] = s_warp[warp] + inc - v;
-    __syncthreads();
-    for (u32 g = tid; g < ng; g += 1024) order[atomicAdd(&s_bin[1023u - min(1023u, (u32)((float)cost(g) * scale))], 1u)] = g;
-    if (tid == 0) order_meta[0] = ng;
+    if (g == 0) order_meta[0] = ng;
 }
 
 #ifdef P3T_WALK_PROFILE
@@ -777,6 +782,9 @@ p3t_status p3t_stage_walk(p3t_ctx *ctx)
     A.counters = w.counters;
     A.group_order = w.group_order;
     A.order_meta = w.order_meta;
+    A.group_class = w.group_class;
+    A.order_hist = w.order_hist;
+    P3T_CUDA(ctx, cudaMemsetAsync(w.order_hist, 0, 2 * ORDER_CLASSES * sizeof(u32), s));   // class counts + scatter cursors
     // one CTA per group when there are too few groups to keep every warp busy to the end of the launch
     // (the group count lives on the device; n / ngroup is its lower bound up to the fill of the groups)
     bool coop = ctx->walk_mode == 2 || (ctx->walk_mode == 0 && 2 * (ctx->n / (size_t)ctx->ngroup) < (size_t)WALK_COOP_BELOW_X2 * grid * WALK_WARPS);
@@ -788,7 +796,9 @@ p3t_status p3t_stage_walk(p3t_ctx *ctx)
         if (coop) walk_kernel<1, true><<<grid, block, smem, s>>>(A, w.group_start, ctx->prm, w.walk_stack);
         else walk_kernel<1, false><<<grid, block, smem, s>>>(A, w.group_start, ctx->prm, w.walk_stack);
     }
-    group_order_kernel<<<1, 1024, 0, s>>>(w.group_stats, w.group_start, w.counters, w.group_order, w.order_meta);
+    // (the group count lives on the device: launch for its upper bound n)
+    group_order_kernel<<<div_up(ctx->n, 256), 256, 0, s>>>(w.group_class, w.order_hist, w.order_hist + ORDER_CLASSES, w.counters,
+                                                          w.group_order, w.order_meta);
     P3T_CUDA(ctx, cudaGetLastError());
     return P3T_OK;
 }

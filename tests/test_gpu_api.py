@@ -179,7 +179,7 @@ def test_cooperative_walk_matches_one_warp_per_group(n):
 
 def test_group_order_is_a_permutation_by_decreasing_cost_and_changes_nothing():
     """The schedule of the next walk (groups by decreasing measured cost) is a permutation of the groups,
-    sorted by the cost the header defines up to the 1024 cost classes, and leaves the results bitwise alike."""
+    sorted by the cost the header defines up to the cost classes (eight per octave), and leaves the results bitwise alike."""
     b = _binding()
     cfg = workloads.config(3, n=60000)
     with b.P3T(cfg["n"], key_bits=63) as ctx:
@@ -193,8 +193,8 @@ def test_group_order_is_a_permutation_by_decreasing_cost_and_changes_nothing():
         ng = len(gs) - 1
         assert np.array_equal(np.sort(order), np.arange(ng))
         cost = (13 * stats[:, 0] + 33 * stats[:, 1]) * np.where(np.diff(gs) > 32, 2, 1)
-        cls = np.minimum(1023, (cost[order].astype(np.float32) * (np.float32(1023.0) / np.float32(cost.max()))).astype(np.int64))
-        assert np.all(np.diff(cls) <= 0)
+        bits = np.maximum(cost, 1).astype(np.float32).view(np.uint32).astype(np.int64) >> 20    # 8 classes per octave
+        assert np.all(np.diff(bits[order]) <= 0)
         ctx.soft_force(cfg["mass"], cfg["pos"])          # same tree: groups handed out in that order
         a1, p1 = ctx.get_acc_pot()
         assert np.array_equal(a0, a1) and np.array_equal(p0, p1)
