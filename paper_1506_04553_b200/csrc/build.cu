@@ -308,17 +308,22 @@ __global__ void __launch_bounds__(BUILD_THREADS) emit_kernel(
             }
         }
     }
-    lo = __reduce_min_sync(0xffffffffu, lo);
+    lo = __reduce_min_sync(0xffffffffu, lo);   // levels with nodes starting in this warp's 128 bodies
     hi = __reduce_max_sync(0xffffffffu, hi);
+    const int wlo = lo, whi = hi;
     if (lane == 0 && hi >= 0) { atomicMin(&s_lo, lo); atomicMax(&s_hi, hi); }
     __syncthreads();
     const int Llo = s_lo, Lhi = s_hi;   // levels with nodes starting in this tile
     // per-warp node counts per level
+    u32 wmask = 0;                      // levels at which this warp has nodes
     for (int L = Llo; L <= Lhi; ++L) {
         u32 cnt = 0;
+        if (L >= wlo && L <= whi) {
 #pragma unroll
-        for (int s = 0; s < BUILD_PER_THREAD; ++s) cnt += (c[s] < L && L <= D[s]) ? 1u : 0u;
-        cnt = __reduce_add_sync(0xffffffffu, cnt);
+            for (int s = 0; s < BUILD_PER_THREAD; ++s) cnt += (c[s] < L && L <= D[s]) ? 1u : 0u;
+            cnt = __reduce_add_sync(0xffffffffu, cnt);
+        }
+        if (cnt) wmask |= 1u << L;
         if (lane == 0) s_wcnt[warp][L] = cnt;
     }
     __syncthreads();
@@ -334,8 +339,14 @@ __global__ void __launch_bounds__(BUILD_THREADS) emit_kernel(
     bool prev_flag[BUILD_PER_THREAD];
 #pragma unroll
     for (int s = 0; s < BUILD_PER_THREAD; ++s) { prev_rank[s] = 0; prev_flag[s] = false; }
-    for (int L = max(Llo - 1, 0); L <= Lhi; ++L) {
+    for (int L = max(wlo - 1, 0); L <= whi; ++L) {
         const bool counted = L >= Llo;   // level Llo-1: ranks only (parents of the topmost nodes)
+        if (!((wmask >> L) & 1u)) {      // no node of this warp at this level: every body has the warp's base rank
+            const u32 r = counted ? s_wcnt[warp][L] : s_lvloff[L];
+#pragma unroll
+            for (int s = 0; s < BUILD_PER_THREAD; ++s) { prev_rank[s] = r; prev_flag[s] = false; }
+            continue;
+        }
         u32 f[BUILD_PER_THREAD], mine = 0;
 #pragma unroll
         for (int s = 0; s < BUILD_PER_THREAD; ++s) { f[s] = (counted && c[s] < L && L <= D[s]) ? 1u : 0u; mine += f[s]; }
