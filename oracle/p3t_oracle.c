@@ -15,6 +15,9 @@
  *   O3  exact neighbour sets, brute force and sort-and-sweep (L138-140)
  *   O4  pointer-based Barnes-Hut octree, monopole + quadrupole (L138),
  *       opening parameter theta (L171), rule R-MAC / R-QUAD of DESIGN.md
+ *   O6  hard acceleration (Eq. 7), its time derivative and the hard
+ *       potential (Eq. 5) -- the NEXT row of SURVEY.md 8(f), pinned by
+ *       tests/test_oracle_hard.py
  *
  * Readings of the paper used here (each listed in DESIGN.md section 3):
  *   A1  Eq. 17's denominator is (gamma-1)^7 (as extracted it is (1-gamma)^7,
@@ -154,6 +157,62 @@ void p3t_oracle_direct(int64_t n, const double *m, const double *q,
         if (pot_soft) pot_soft[k] = nval(&ps);
         if (acc_hard) for (int d = 0; d < 3; ++d) acc_hard[3 * k + d] = nval(&ah[d]);
         if (pot_hard) pot_hard[k] = nval(&ph);
+    }
+}
+
+/* ------------------------------------------------------------------ O6 -- */
+
+/* dK/dx of Eq. 12 (L85) on 0 <= x < 1, 0 elsewhere: the derivative of the printed polynomial,
+ * -140x^6 + 420x^5 - 420x^4 + 140x^3 = 140 x^3 (1-x)^3 (factored: no cancellation near x = 1). */
+double p3t_oracle_dKdx(double x)
+{
+    if (x < 0.0 || x >= 1.0) return 0.0;
+    double u = x * (1.0 - x);
+    return 140.0 * u * u * u;
+}
+
+/*
+ * Hard acceleration and its time derivative (jerk), the quantities the Hermite part integrates (Eq. 7;
+ * procedure step 3 L147), per unit mass of i, over ALL j != i:
+ *   a_i = - sum_j m_j (1 - K(s)) q_ij / s^3
+ *   j_i = d a_i / dt with q_ij -> q_ij + v_ij t:  ds/dt = (q_ij . v_ij) / s,
+ *       = - sum_j m_j [ (1 - K) ( v_ij / s^3 - 3 (q.v) q_ij / s^5 ) - (dK/ds) ((q.v)/s) q_ij / s^3 ],
+ *   dK/ds = dK/dx / (r_out (1 - gamma))   (x of Eq. 13).
+ * (The paper gives Eq. 7 only; the jerk is its time derivative written out.)
+ */
+void p3t_oracle_hard(int64_t n, const double *m, const double *q, const double *v,
+                     double eps, double r_in, double r_out,
+                     int64_t ns, const int64_t *subset, double *acc, double *jerk, double *pot)
+{
+    const double eps2 = eps * eps, g = r_in / r_out;
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t k = 0; k < ns; ++k) {
+        int64_t i = subset ? subset[k] : k;
+        nsum a[3] = {{0, 0}, {0, 0}, {0, 0}}, jk[3] = {{0, 0}, {0, 0}, {0, 0}}, ph = {0, 0};
+        for (int64_t j = 0; j < n; ++j) {
+            if (j == i) continue;
+            double d[3], w[3];
+            for (int c = 0; c < 3; ++c) { d[c] = q[3 * i + c] - q[3 * j + c]; w[c] = v[3 * i + c] - v[3 * j + c]; }
+            double s2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2] + eps2;
+            double s = sqrt(s2);
+            if (s >= r_out) continue;                       /* 1 - K = 1 - W = 0 (Eq. 12/16 third branches) */
+            double K, W;
+            pair_weights(s, r_in, r_out, &K, &W);
+            double x = (s / r_out - g) / (1.0 - g);
+            double dKds = p3t_oracle_dKdx(x) / (r_out * (1.0 - g));
+            double qv = d[0] * w[0] + d[1] * w[1] + d[2] * w[2];
+            double mr3 = m[j] / (s2 * s);
+            for (int c = 0; c < 3; ++c) {
+                nadd(&a[c], -mr3 * (1.0 - K) * d[c]);
+                nadd(&jk[c], -mr3 * ((1.0 - K) * (w[c] - 3.0 * qv * d[c] / s2) - dKds * (qv / s) * d[c]));
+            }
+            nadd(&ph, -(m[j] / s) * (1.0 - W));
+        }
+        for (int c = 0; c < 3; ++c) {
+            if (acc) acc[3 * k + c] = nval(&a[c]);
+            if (jerk) jerk[3 * k + c] = nval(&jk[c]);
+        }
+        if (pot) pot[k] = nval(&ph);
     }
 }
 

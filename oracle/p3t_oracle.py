@@ -62,6 +62,9 @@ def lib():
         L.p3t_oracle_tree_walk.restype = None
         L.p3t_oracle_tree_walk.argtypes = [vp, d, d, d, d, d, i32, i64, pi64, pd, pd, pd, pi64, pi32, i64, pi64]
         L.p3t_oracle_num_threads.restype = i32
+        L.p3t_oracle_dKdx.restype = d; L.p3t_oracle_dKdx.argtypes = [d]
+        L.p3t_oracle_hard.restype = None
+        L.p3t_oracle_hard.argtypes = [i64, pd, pd, pd, d, d, d, i64, pi64, pd, pd, pd]
         _lib = L
     return _lib
 
@@ -126,6 +129,26 @@ def direct(mass, pos, eps, r_in, r_out, subset=None, hard=False):
     lib().p3t_oracle_direct(n, _p(m, d), _p(q, d), float(eps), float(r_in), float(r_out), ns,
                             _p(sub, C.c_int64), _p(a_s, d), _p(p_s, d), _p(a_h, d), _p(p_h, d))
     return (a_s, p_s, a_h, p_h) if hard else (a_s, p_s)
+
+
+# ---------------------------------------------------------------- O6 -------
+def dKdx(x):
+    """dK/dx of Eq. 12: 140 x^3 (1-x)^3 on [0, 1)."""
+    return lib().p3t_oracle_dKdx(float(x))
+
+
+def hard(mass, pos, vel, eps, r_in, r_out, subset=None):
+    """Hard acceleration, its time derivative (jerk) and hard potential per unit mass over all j != i
+    (Eq. 7 / Eq. 5; the Hermite part's inputs, L147).  Returns (acc[ns,3], jerk[ns,3], pot[ns])."""
+    m, q, v = _f64(mass), _f64(pos).reshape(-1, 3), _f64(vel).reshape(-1, 3)
+    n = m.shape[0]
+    sub = _subset(subset)
+    ns = n if sub is None else sub.shape[0]
+    a, j, p = np.empty((ns, 3)), np.empty((ns, 3)), np.empty(ns)
+    d = C.c_double
+    lib().p3t_oracle_hard(n, _p(m, d), _p(q, d), _p(v, d), float(eps), float(r_in), float(r_out), ns,
+                          _p(sub, C.c_int64), _p(a, d), _p(j, d), _p(p, d))
+    return a, j, p
 
 
 # ---------------------------------------------------------------- O3 -------
