@@ -219,6 +219,22 @@ def main():
     if rank == 0:      # pure-FFMA calibration kernel, outside the timed region
         ffma_scalar, ffma_packed = ctx.measure_fp32_peak(False)[0], ctx.measure_fp32_peak(True)[0]
 
+    # ---- NEXT row, outside the timed region: hard force over the neighbour lists of the last step
+    hard = None
+    if rank == 0:
+        vel_d = torch.from_numpy(cfg["vel"]).to(dev)
+        ah = torch.empty((n, 3), dtype=torch.float64, device=dev); jh = torch.empty_like(ah)
+        ph_ = torch.empty(n, dtype=torch.float64, device=dev)
+        th = []
+        for _ in range(5):
+            flush.zero_()
+            ctx.eval_hard(vel_d, ah, jh, ph_)
+            th.append(ctx.get_stats()["ms_hard"])
+        ms_h = float(np.median(th[1:]))
+        hb = n * (16 + 12 + 8 + 56) + st["n_neighbours"] * (4 + 16 + 12)      # own body, velocity, offsets, outputs; per pair idx, body, velocity
+        hard = {"kernel": "hard_kernel (p3t_eval_hard: acceleration, jerk, potential over the neighbour lists, fp64)", "ms": ms_h,
+                "pairs": st["n_neighbours"], "bound": "hbm", "algorithmic_bytes": hb, "achieved": hb / (ms_h * 1e-3) / 1e9, "unit": "GB/s"}
+
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
     e2e = None
     if not args.no_e2e:
@@ -296,6 +312,9 @@ def main():
                          "per_pass_gbs": hbm, "algorithmic_bytes": ab, "peak_source": peaks["source"]},
         "clocks": clocks, "gpu_launches": launches * args.steps, "gpu_launches_per_step": launches,
     }
+    if hard:
+        hard["peak"] = peaks["hbm_gbs"]; hard["frac"] = hard["achieved"] / peaks["hbm_gbs"]
+        out["next_rows"] = {"hard_force": hard}
     if e2e:
         out["e2e"] = e2e
     if not args.no_cpu_baseline and world == 1:

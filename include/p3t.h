@@ -71,6 +71,7 @@ typedef struct {
     float ms_moments;        /* a6 */
     float ms_walk;           /* a7-a8 */
     float ms_nbr;            /* a9 */
+    float ms_hard;           /* last p3t_eval_hard */
 } p3t_stats;
 
 /* Bytes of device workspace p3t_create needs for up to max_n particles,
@@ -146,6 +147,19 @@ p3t_status p3t_get_neighbours(p3t_ctx *ctx, uint64_t *offset, uint32_t *nbr, siz
 
 /* Synchronises the stream, then reports counts and per-phase times (CUDA events). */
 p3t_status p3t_get_stats(p3t_ctx *ctx, p3t_stats *out);
+
+/* Hard part over the neighbour lists (the NEXT row of SURVEY.md 8(f); the paper evaluates it on the host,
+ * PAPER.md L138, procedure step 3 L147).  For every particle i, from the lists L_i of the last p3t_eval_soft
+ * (or p3t_eval_direct) and the positions and masses loaded then:
+ *   acc[3n]   a_i   = - sum_{j in L_i} m_j (1 - K(s_ij)) q_ij / s_ij^3        (Eq. 7, per unit mass)
+ *   jerk[3n]  d a_i / dt for relative velocities v_ij = vel_i - vel_j           (input of the Hermite scheme)
+ *   pot[n]    phi_i = - sum_{j in L_i} m_j (1 - W(s_ij)) / s_ij                 (Eq. 5)
+ * Since 1 - K = 1 - W = 0 beyond r_out <= r_search these equal the sums over all j.  vel[3n] is in user order,
+ * interleaved like pos; outputs are double precision (every pair is evaluated in fp64), user order; any output
+ * may be NULL.  vel and the outputs are all host or all device (on_device); the host form synchronises.
+ * P3T_ESTATE before an eval call; P3T_ECAPACITY if the lists did not fit nbr_capacity (outputs untouched;
+ * in the device form the error surfaces at the next synchronising call); P3T_EINVAL for null or non-finite vel. */
+p3t_status p3t_eval_hard(p3t_ctx *ctx, const float *vel, double *acc, double *jerk, double *pot, int on_device);
 
 /* Wait for all enqueued work; returns deferred device-side errors. */
 p3t_status p3t_synchronize(p3t_ctx *ctx);

@@ -28,7 +28,7 @@ _STATUS = {0: "P3T_OK", -1: "P3T_EINVAL", -2: "P3T_ESTATE", -3: "P3T_ENOMEM", -4
 # names of include/p3t.h's exported entry points (tests check that each resolves)
 SYMBOLS = [
     "p3t_workspace_bytes", "p3t_create", "p3t_destroy", "p3t_set_params", "p3t_set_tree_params",
-    "p3t_set_group_merge_levels", "p3t_set_walk_mode", "p3t_load_particles", "p3t_build_tree", "p3t_eval_soft", "p3t_eval_direct",
+    "p3t_set_group_merge_levels", "p3t_set_walk_mode", "p3t_load_particles", "p3t_build_tree", "p3t_eval_soft", "p3t_eval_direct", "p3t_eval_hard",
     "p3t_get_acc_pot", "p3t_get_neighbour_counts", "p3t_get_neighbours", "p3t_get_stats", "p3t_synchronize",
     "p3t_last_error", "p3t_array_info", "p3t_copy_array", "p3t_measure_fp32_peak",
 ]
@@ -45,7 +45,7 @@ class Stats(C.Structure):
                 ("n_neighbours", C.c_uint64), ("n_cells", C.c_uint32), ("n_leaves", C.c_uint32),
                 ("n_groups", C.c_uint32), ("depth", C.c_uint32), ("max_list", C.c_uint32),
                 ("sort_passes", C.c_uint32), ("ms_sort", C.c_float), ("ms_build", C.c_float),
-                ("ms_moments", C.c_float), ("ms_walk", C.c_float), ("ms_nbr", C.c_float)]
+                ("ms_moments", C.c_float), ("ms_walk", C.c_float), ("ms_nbr", C.c_float), ("ms_hard", C.c_float)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
@@ -65,6 +65,7 @@ def _sig():
     L.p3t_build_tree.restype = i; L.p3t_build_tree.argtypes = [vp]
     L.p3t_eval_soft.restype = i; L.p3t_eval_soft.argtypes = [vp]
     L.p3t_eval_direct.restype = i; L.p3t_eval_direct.argtypes = [vp, vp, sz, i]
+    L.p3t_eval_hard.restype = i; L.p3t_eval_hard.argtypes = [vp, vp, vp, vp, vp, i]
     L.p3t_get_acc_pot.restype = i; L.p3t_get_acc_pot.argtypes = [vp, vp, vp, i]
     L.p3t_get_neighbour_counts.restype = i; L.p3t_get_neighbour_counts.argtypes = [vp, vp, C.POINTER(C.c_uint64), i]
     L.p3t_get_neighbours.restype = i; L.p3t_get_neighbours.argtypes = [vp, vp, vp, sz, i]
@@ -209,6 +210,19 @@ class P3T:
         pa, da = _ptr(acc)
         pp, dp = _ptr(pot)
         self._check(_lib.p3t_get_acc_pot(self._h, pa, pp, da if acc is not None else dp))
+
+    def eval_hard(self, vel, acc=None, jerk=None, pot=None):
+        """Hard acceleration, jerk and potential from the neighbour lists of the last eval (p3t_eval_hard).
+        vel: float32 [n,3] numpy (host) or CUDA tensor.  Host form: returns float64 numpy (acc, jerk, pot).
+        Device form: writes the given float64 CUDA tensors (any may be None) and returns them."""
+        pv, dv = _ptr(vel)
+        if dv:
+            pa, _ = _ptr(acc); pj, _ = _ptr(jerk); pp, _ = _ptr(pot)
+            self._check(_lib.p3t_eval_hard(self._h, pv, pa, pj, pp, 1))
+            return acc, jerk, pot
+        a, j, p = np.empty((self.n, 3)), np.empty((self.n, 3)), np.empty(self.n)
+        self._check(_lib.p3t_eval_hard(self._h, pv, a.ctypes.data, j.ctypes.data, p.ctypes.data, 0))
+        return a, j, p
 
     def get_neighbour_counts(self):
         count = np.empty(self.n, dtype=np.uint32)

@@ -77,6 +77,7 @@ size_t p3t_layout(Workspace &ws, char *base, size_t max_n, int key_bits, size_t 
     ws.nbr = b.take<u32>(nbr_capacity ? nbr_capacity : 1);
     ws.nbr_cursor = b.take<u32>(n);
     ws.subset = b.take<u32>(n);
+    ws.hard_out = b.take<double>(7 * n);
     ws.counters = b.take<u64>(CNT_WORDS);
     ws.walk_stack = b.take<u32>(ws.walk_warps_max * WALK_STACK_GMEM);
     ws.scan_tmp = b.take<u64>((n + 1023) / 1024 + 2);
@@ -136,7 +137,7 @@ extern "C" p3t_status p3t_create(p3t_ctx **out, int device, size_t max_n, int ke
     }
     ctx->base = static_cast<char *>(workspace);
     if (cudaMemsetAsync(ctx->ws.order_meta, 0, 4 * sizeof(u32), ctx->stream) != cudaSuccess) { delete ctx; return P3T_ECUDA; }
-    for (int i = 0; i < 8; ++i) {
+    for (int i = 0; i < 10; ++i) {
         if (cudaEventCreate(&ctx->ev[i]) != cudaSuccess) { delete ctx; return P3T_ECUDA; }
     }
     *out = ctx;
@@ -147,7 +148,7 @@ extern "C" p3t_status p3t_destroy(p3t_ctx *ctx)
 {
     if (!ctx) return P3T_EINVAL;
     cudaStreamSynchronize(ctx->stream);
-    for (int i = 0; i < 8; ++i)
+    for (int i = 0; i < 10; ++i)
         if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
     delete ctx;
     return P3T_OK;
@@ -167,6 +168,7 @@ extern "C" p3t_status p3t_set_params(p3t_ctx *ctx, float eps, float theta, float
     ctx->eps = eps; ctx->theta = theta; ctx->r_in = r_in; ctx->r_out = r_out; ctx->r_search = r_search;
     P3TParams &p = ctx->prm;
     p.eps2 = eps * eps;
+    p.eps2_d = (double)eps * (double)eps;
     p.theta = theta;
     p.r_in = r_in; p.r_out = r_out; p.h = r_search;
     p.rout2 = r_out * r_out;
@@ -350,6 +352,42 @@ extern "C" p3t_status p3t_eval_direct(p3t_ctx *ctx, const uint32_t *i_subset, si
     return P3T_OK;
 }
 
+static p3t_status sync_and_check(p3t_ctx *ctx);
+
+// NEXT row: hard acceleration, jerk and potential from the neighbour lists
+extern "C" p3t_status p3t_eval_hard(p3t_ctx *ctx, const float *vel, double *acc, double *jerk, double *pot, int on_device)
+{
+    if (!ctx) return P3T_EINVAL;
+    if (!vel) return p3t_fail(ctx, P3T_EINVAL, "null vel");
+    if (!ctx->evaluated) return p3t_fail(ctx, P3T_ESTATE, "p3t_eval_hard needs the neighbour lists of an eval call");
+    P3T_CUDA(ctx, cudaSetDevice(ctx->device));
+    const size_t n = ctx->n;
+    const float *d_vel = vel;
+    double *d_acc = acc, *d_jerk = jerk, *d_pot = pot;
+    if (!on_device) {
+        if (!host_all_finite(vel, 3 * n)) return p3t_fail(ctx, P3T_EINVAL, "non-finite velocity");
+        P3T_CUDA(ctx, cudaMemcpyAsync(ctx->ws.in_pos, vel, 3 * n * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
+        d_vel = ctx->ws.in_pos;
+        d_acc = acc ? ctx->ws.hard_out : nullptr;
+        d_jerk = jerk ? ctx->ws.hard_out + 3 * n : nullptr;
+        d_pot = pot ? ctx->ws.hard_out + 6 * n : nullptr;
+    }
+    P3T_CUDA(ctx, cudaEventRecord(ctx->ev[7], ctx->stream));
+    p3t_status st = p3t_stage_hard(ctx, d_vel, d_acc, d_jerk, d_pot);
+    if (st != P3T_OK) return st;
+    P3T_CUDA(ctx, cudaEventRecord(ctx->ev[8], ctx->stream));
+    ctx->ev_hard = true;
+    if (on_device) return P3T_OK;
+    if (acc) P3T_CUDA(ctx, cudaMemcpyAsync(acc, d_acc, 3 * n * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    if (jerk) P3T_CUDA(ctx, cudaMemcpyAsync(jerk, d_jerk, 3 * n * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    if (pot) P3T_CUDA(ctx, cudaMemcpyAsync(pot, d_pot, n * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    st = sync_and_check(ctx);
+    if (st != P3T_OK) return st;
+    if (ctx->h_counters[CNT_PAIRS] > ctx->nbr_capacity)
+        return p3t_fail(ctx, P3T_ECAPACITY, "neighbour lists exceed the context's nbr_capacity: no hard force was computed");
+    return P3T_OK;
+}
+
 // ------------------------------------------------------------------------------------------------
 // synchronisation and deferred errors
 // ------------------------------------------------------------------------------------------------
@@ -448,6 +486,7 @@ extern "C" p3t_status p3t_get_stats(p3t_ctx *ctx, p3t_stats *out)
         cudaEventElapsedTime(&out->ms_walk, ctx->ev[4], ctx->ev[5]);
         cudaEventElapsedTime(&out->ms_nbr, ctx->ev[5], ctx->ev[6]);
     }
+    if (ctx->ev_hard) cudaEventElapsedTime(&out->ms_hard, ctx->ev[7], ctx->ev[8]);
     return st;
 }
 

@@ -47,6 +47,7 @@ struct P3TParams {
     float rout2;       // r_out^2
     float h2;          // h^2                 (neighbour test  s^2 < h^2, reading A4)
     float hnear2;      // (h (1+1e-5))^2 + slack: bodies whose box distance is below this take the slow path
+    double eps2_d;     // eps^2 in double (hard.cu evaluates pairs in fp64)
     double inv_rout;   // 1 / r_out
     double gamma;      // r_in / r_out
     double inv_1mg;    // 1 / (1 - gamma)
@@ -106,6 +107,7 @@ struct Workspace {
     u32 *nbr;                      // [cap]
     u32 *nbr_cursor;               // [n]
     u32 *subset;                   // [n] staging for eval_direct
+    double *hard_out;              // [7n] staging of p3t_eval_hard's host outputs (acc 3n, jerk 3n, pot n)
     u64 *counters;                 // [CNT_WORDS]
     u32 *walk_stack;               // [nwarps][WALK_STACK_GMEM]
     u64 *scan_tmp;                 // [nblk_scan + 1]
@@ -129,8 +131,8 @@ struct p3t_ctx {
     float eps, theta, r_in, r_out, r_search;
     Workspace ws;
     char *base;
-    cudaEvent_t ev[8];             // phase boundaries: 0 build start,1 sort end,2 build end,3 moments end,4 eval start,5 walk end,6 nbr end
-    bool ev_build, ev_eval;
+    cudaEvent_t ev[10];            // phase boundaries: 0 build start,1 sort end,2 build end,3 moments end,4 eval start,5 walk end,6 nbr end,7/8 hard
+    bool ev_build, ev_eval, ev_hard;
     char err[512];
     // host mirrors (valid after sync)
     u64 h_counters[CNT_WORDS];
@@ -166,6 +168,7 @@ p3t_status p3t_stage_walk(p3t_ctx *ctx);
 p3t_status p3t_stage_direct(p3t_ctx *ctx, const u32 *d_subset, size_t n_subset);
 p3t_status p3t_stage_neighbours(p3t_ctx *ctx);
 p3t_status p3t_stage_unpack(p3t_ctx *ctx, float *d_acc, float *d_pot);
+p3t_status p3t_stage_hard(p3t_ctx *ctx, const float *d_vel, double *d_acc, double *d_jerk, double *d_pot);
 
 #ifdef __CUDACC__
 // ---- device helpers ----------------------------------------------------------------------------
