@@ -65,7 +65,7 @@ typedef struct {
     uint32_t n_groups;       /* i-groups walked (one warp each) */
     uint32_t depth;          /* deepest level in use (root = 0) */
     uint32_t max_list;       /* longest neighbour list */
-    uint32_t sort_passes;    /* radix passes actually run (uniform digits are skipped) */
+    uint32_t sort_passes;    /* radix passes of the build (8-bit digits: 8 for 63-bit keys, 4 for 30-bit keys) */
     float ms_sort;           /* a1-a4: bounding cube, keys, radix sort, gather */
     float ms_build;          /* a5: octree + groups */
     float ms_moments;        /* a6 */

@@ -13,6 +13,15 @@
 // Pair terms:  Eq. 8 (L65) and Eq. 6 (L55) of PAPER.md; cell terms: rule R-QUAD of DESIGN.md.
 #include "p3t_internal.cuh"
 
+// unroll factors of the interaction loops (list entries in flight per warp)
+#ifndef WALK_PP_UNROLL
+#define WALK_PP_UNROLL 8
+#endif
+#ifndef WALK_PC_UNROLL
+#define WALK_PC_UNROLL 4
+#endif
+constexpr int kPpUnroll = WALK_PP_UNROLL, kPcUnroll = WALK_PC_UNROLL;
+
 #ifdef P3T_WALK_PROFILE
 // sequential attribution of a warp's cycles to phases (diagnostic builds only)
 #define WP_SLOTS 12
@@ -178,7 +187,7 @@ __device__ __forceinline__ void eval_far(const WarpShared &ws, u32 head, u32 cnt
     typedef typename VecOf<NI>::type V;
     const V eps2 = vdup<V>(eps2s);
     if (cnt == 32) {
-#pragma unroll 8
+#pragma unroll kPpUnroll
         for (u32 j = 0; j < 32; ++j) pp_body<NI>(ws.far[head + j], t, eps2, acc);
     } else {
         for (u32 j = 0; j < cnt; ++j) pp_body<NI>(ws.far[head + j], t, eps2, acc);
@@ -210,7 +219,7 @@ __device__ __forceinline__ void eval_pc(const WarpShared &ws, u32 head, u32 cnt,
 {
     typedef typename VecOf<NI>::type V;
     const V eps2 = vdup<V>(eps2s), c02 = vdup<V>(0.2f), cm04 = vdup<V>(-0.4f);
-#pragma unroll 4
+#pragma unroll kPcUnroll
     for (u32 j = 0; j < cnt; ++j) {
         const u32 e = head + j;
         const float4 P0 = ws.pc[0][e], P1 = ws.pc[1][e], P2 = ws.pc[2][e];
