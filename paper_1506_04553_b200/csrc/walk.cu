@@ -18,7 +18,7 @@
 #define WALK_PP_UNROLL 8
 #endif
 #ifndef WALK_PC_UNROLL
-#define WALK_PC_UNROLL 4
+#define WALK_PC_UNROLL 8
 #endif
 constexpr int kPpUnroll = WALK_PP_UNROLL, kPcUnroll = WALK_PC_UNROLL;
 
