@@ -46,12 +46,16 @@ __device__ __forceinline__ void st_tile_status(u32 *p, u32 v)
 {
     asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
-// Decoupled look-back of one column: publishes `own` for `tile`, returns the sum over all tiles before it.
+// Decoupled look-back of one column.  tile_publish makes `own` of `tile` visible (as early as it is known);
+// tile_resolve returns the sum over all tiles before it and publishes the inclusive prefix.
 // p0 points at status word `col` of record `tile`; records are sizeof(TileRec) apart.
-__device__ __forceinline__ u32 tile_lookback(u32 *p0, u32 tile, u32 own)
+__device__ __forceinline__ void tile_publish(u32 *p0, u32 tile, u32 own)
+{
+    st_tile_status(p0, own | (tile == 0 ? TL_FLAG_INC : TL_FLAG_AGG));
+}
+__device__ __forceinline__ u32 tile_resolve(u32 *p0, u32 tile, u32 own)
 {
     const int stride = (int)(sizeof(TileRec) / sizeof(u32));
-    st_tile_status(p0, own | (tile == 0 ? TL_FLAG_INC : TL_FLAG_AGG));
     u32 excl = 0;
     if (tile > 0) {
         const u32 *p = p0 - stride;
@@ -74,6 +78,11 @@ __device__ __forceinline__ u32 tile_lookback(u32 *p0, u32 tile, u32 own)
         st_tile_status(p0, (excl + own) | TL_FLAG_INC);
     }
     return excl;
+}
+__device__ __forceinline__ u32 tile_lookback(u32 *p0, u32 tile, u32 own)
+{
+    tile_publish(p0, tile, own);
+    return tile_resolve(p0, tile, own);
 }
 
 #define BUILD_PAD 40   // zero words behind every window: shifted reads never leave the array
@@ -332,6 +341,49 @@ __global__ void __launch_bounds__(BUILD_THREADS) emit_kernel(
         for (int w = 0; w < BUILD_THREADS / 32; ++w) { u32 t = s_wcnt[w][tid]; s_wcnt[w][tid] = sum; sum += t; }
     }
     __syncthreads();
+    // ---- group heads: every ngroup-th body of a segment (segments start at cut flags).  Counted first, so that
+    //      the tile's count is visible to its successors while the nodes are emitted; resolved at the end.
+    u32 head_mask = 0, head_inc = 0, head_mine = 0, head_total = 0;
+    {
+        u32 cf = 0;
+        if (i0 + BUILD_PER_THREAD <= n) cf = *reinterpret_cast<const u32 *>(cutflag + i0);
+        else for (int s = 0; s < BUILD_PER_THREAD; ++s) if (i0 + s < n) cf |= (u32)cutflag[i0 + s] << (8 * s);
+        int last = -1;
+#pragma unroll
+        for (int s = 0; s < BUILD_PER_THREAD; ++s) if ((cf >> (8 * s)) & 1u) last = (int)(i0 + s);
+        int run = last;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            int t = __shfl_up_sync(0xffffffffu, run, o);
+            if (lane >= o) run = max(run, t);
+        }
+        if (lane == 31) s_wmax[warp] = run;
+        __syncthreads();
+        int seg = __shfl_up_sync(0xffffffffu, run, 1);
+        if (lane == 0) seg = -1;
+        seg = max(seg, s_carry);   // cut carried in from the tiles before
+        for (int w = 0; w < warp; ++w) seg = max(seg, s_wmax[w]);
+        u32 mine = 0;
+#pragma unroll
+        for (int s = 0; s < BUILD_PER_THREAD; ++s) {
+            const u32 i = i0 + s;
+            if ((cf >> (8 * s)) & 1u) seg = (int)i;
+            const bool hd = i < n && ((i - (u32)seg) % (u32)ngroup) == 0;
+            head_mask |= hd ? 1u << s : 0u;
+            mine += hd ? 1u : 0u;
+        }
+        u32 inc = mine;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            u32 t = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= o) inc += t;
+        }
+        if (lane == 31) s_whead[warp] = inc;
+        head_inc = inc; head_mine = mine;
+        __syncthreads();
+        for (int w = 0; w < BUILD_THREADS / 32; ++w) head_total += s_whead[w];
+        if (tid == 0) tile_publish(&tiles[tile].status[24], tile, head_total);
+    }
     // ---- nodes.  rank_L(i) = number of level-L nodes starting before body i; a node's parent is the
     //      level-(L-1) node starting at the same body if there is one, else the last one before it.
     u32 nleaf_here = 0;
@@ -397,59 +449,22 @@ __global__ void __launch_bounds__(BUILD_THREADS) emit_kernel(
     }
     u32 nl = __reduce_add_sync(0xffffffffu, nleaf_here);
     if (lane == 0 && nl) atomicAdd(&counters[CNT_NLEAVES], (u64)nl);
-    // ---- group heads: every ngroup-th body of a segment (segments start at cut flags)
+    // ---- heads of the tiles before this one: look-back (most predecessors are done by now), then the compaction
     {
-        u32 cf = 0;
-        if (i0 + BUILD_PER_THREAD <= n) cf = *reinterpret_cast<const u32 *>(cutflag + i0);
-        else for (int s = 0; s < BUILD_PER_THREAD; ++s) if (i0 + s < n) cf |= (u32)cutflag[i0 + s] << (8 * s);
-        int last = -1;
-#pragma unroll
-        for (int s = 0; s < BUILD_PER_THREAD; ++s) if ((cf >> (8 * s)) & 1u) last = (int)(i0 + s);
-        int run = last;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            int t = __shfl_up_sync(0xffffffffu, run, o);
-            if (lane >= o) run = max(run, t);
-        }
-        if (lane == 31) s_wmax[warp] = run;
-        __syncthreads();
-        int seg = __shfl_up_sync(0xffffffffu, run, 1);
-        if (lane == 0) seg = -1;
-        seg = max(seg, s_carry);   // cut carried in from the tiles before
-        for (int w = 0; w < warp; ++w) seg = max(seg, s_wmax[w]);
-        bool head[BUILD_PER_THREAD];
-        u32 mine = 0;
-#pragma unroll
-        for (int s = 0; s < BUILD_PER_THREAD; ++s) {
-            const u32 i = i0 + s;
-            if ((cf >> (8 * s)) & 1u) seg = (int)i;
-            head[s] = i < n && ((i - (u32)seg) % (u32)ngroup) == 0;
-            mine += head[s] ? 1u : 0u;
-        }
-        u32 inc = mine;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            u32 t = __shfl_up_sync(0xffffffffu, inc, o);
-            if (lane >= o) inc += t;
-        }
-        if (lane == 31) s_whead[warp] = inc;
-        __syncthreads();
-        if (tid == 0) {   // heads of the tiles before: look-back (most predecessors are done by now)
-            u32 total = 0;
-            for (int w = 0; w < BUILD_THREADS / 32; ++w) total += s_whead[w];
-            const u32 excl = tile_lookback(&tiles[tile].status[24], tile, total);
+        if (tid == 0) {
+            const u32 excl = tile_resolve(&tiles[tile].status[24], tile, head_total);
             s_headbase = excl;
             if (tile == ntiles - 1) {
-                counters[CNT_NGROUPS] = (u64)(excl + total);
-                group_start[excl + total] = n;
+                counters[CNT_NGROUPS] = (u64)(excl + head_total);
+                group_start[excl + head_total] = n;
             }
         }
         __syncthreads();
-        u32 pos = s_headbase + inc - mine;
+        u32 pos = s_headbase + head_inc - head_mine;
         for (int w = 0; w < warp; ++w) pos += s_whead[w];
 #pragma unroll
         for (int s = 0; s < BUILD_PER_THREAD; ++s)
-            if (head[s]) group_start[pos++] = i0 + s;
+            if ((head_mask >> s) & 1u) group_start[pos++] = i0 + s;
     }
 }
 
