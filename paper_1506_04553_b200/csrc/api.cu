@@ -270,18 +270,20 @@ extern "C" p3t_status p3t_load_particles(p3t_ctx *ctx, size_t n, const float *ma
     if (n == 0 || n > ctx->max_n) return p3t_fail(ctx, P3T_EINVAL, "n must be in 1..max_n");
     P3T_CUDA(ctx, cudaSetDevice(ctx->device));
     const float *d_mass = mass, *d_pos = pos;
+    ctx->loaded = false;
+    ctx->built = false;
+    ctx->evaluated = false;
     if (!on_device) {
-        if (!host_all_finite(mass, n)) return p3t_fail(ctx, P3T_EINVAL, "non-finite mass");
-        if (!host_all_finite(pos, 3 * n)) return p3t_fail(ctx, P3T_EINVAL, "non-finite position");
+        // the copies are enqueued first and the host-side check runs while they are in flight (pinned memory);
+        // on failure the staging arrays hold unusable data and the context stays "not loaded"
         P3T_CUDA(ctx, cudaMemcpyAsync(ctx->ws.in_mass, mass, n * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
         P3T_CUDA(ctx, cudaMemcpyAsync(ctx->ws.in_pos, pos, 3 * n * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
+        if (!host_all_finite(mass, n)) return p3t_fail(ctx, P3T_EINVAL, "non-finite mass");
+        if (!host_all_finite(pos, 3 * n)) return p3t_fail(ctx, P3T_EINVAL, "non-finite position");
         d_mass = ctx->ws.in_mass;
         d_pos = ctx->ws.in_pos;
     }
     ctx->n = n;
-    ctx->loaded = false;
-    ctx->built = false;
-    ctx->evaluated = false;
     p3t_status st = p3t_stage_pack(ctx, d_mass, d_pos);
     if (st != P3T_OK) return st;
     ctx->loaded = true;
