@@ -146,6 +146,9 @@ def main():
     ap.add_argument("--nleaf", type=int, default=None)
     ap.add_argument("--ngroup", type=int, default=None)
     ap.add_argument("--merge", type=int, default=None)
+    ap.add_argument("--shard", action="store_true",
+                    help="strong scaling: ONE cluster, every rank walks every world-th i-group (p3t_set_shard) and the "
+                         "accelerations and potentials are summed over the ranks (NCCL all-reduce inside the timed step)")
     ap.add_argument("--walk-mode", type=int, default=None, help="p3t_set_walk_mode: 0 auto, 1 warp per group, 2 CTA per group")
     ap.add_argument("--n", type=int, default=None, help="override the particle count (not a bench value)")
     args = ap.parse_args()
@@ -169,7 +172,9 @@ def main():
 
     from paper_1506_04553_b200 import multi
 
-    cfg = multi.rank_config(args.config, rank, n=args.n)      # independent cluster per rank: same recipe, another seed
+    shard = args.shard and world > 1
+    # default: an independent cluster per rank (same recipe, another seed); --shard: the same cluster on every rank
+    cfg = multi.rank_config(args.config, 0 if shard else rank, n=args.n)
     n = cfg["n"]
     nleaf, ngroup = args.nleaf or cfg["nleaf"], args.ngroup or cfg["ngroup"]
     dev = f"cuda:{local}"
@@ -185,10 +190,18 @@ def main():
     if args.walk_mode is not None:
         ctx.set_walk_mode(args.walk_mode)
 
+    if shard:
+        ctx.set_shard(rank, world)
+        acc_d = torch.empty((n, 3), dtype=torch.float32, device=dev)
+        pot_d = torch.empty(n, dtype=torch.float32, device=dev)
+
     def step():
         ctx.load_particles(mass_d, pos_d)
         ctx.build_tree()
         ctx.eval_soft()
+        if shard:      # every rank ends the step with the accelerations and potentials of all particles
+            ctx.get_acc_pot_into(acc_d, pot_d)
+            multi.allreduce_forces(dist, acc_d, pot_d)
 
     for _ in range(args.warmup):
         flush.zero_()
@@ -213,6 +226,8 @@ def main():
         dist.barrier()
     clocks = sampler.stop() if sampler else None
     total_n, ms = multi.aggregate(dist, n, float(np.mean([a.elapsed_time(b) for a, b in ev])), device=dev)
+    if shard:
+        total_n = n      # one cluster, not one per rank
     st = ctx.get_stats()
     ph = {k: float(np.mean(v)) for k, v in phases.items()}
     ffma_scalar = ffma_packed = None
@@ -290,11 +305,12 @@ def main():
 
     out = {
         "metric": METRIC, "value": multi.throughput(total_n, ms), "unit": "particles/s", "n_gpus": world, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "strong" if shard else "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": cfg["name"], "n": n, "theta": cfg["theta"], "eps": cfg["eps"], "r_out": cfg["r_out"],
                    "r_search": cfg["r_search"], "key_bits": cfg["key_bits"], "nleaf": nleaf, "ngroup": ngroup,
-                   "l2": "flushed between steps (512 MiB write)", "parallelism": f"{world} independent cluster(s), one per GPU"},
+                   "l2": "flushed between steps (512 MiB write)", "parallelism": (f"one cluster sharded over {world} GPUs by i-groups, all-reduce of the results" if shard
+                                   else f"{world} independent cluster(s), one per GPU")},
         "interactions_per_s": (st["n_pp"] + st["n_pc"]) / (ph["ms_walk"] * 1e-3),
         "walk_particles_per_s": n / (ph["ms_walk"] * 1e-3),
         "interactions": {"n_pp": st["n_pp"], "n_pc": st["n_pc"], "n_near": st["n_near"], "n_neighbours": st["n_neighbours"],

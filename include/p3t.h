@@ -113,6 +113,14 @@ p3t_status p3t_set_group_merge_levels(p3t_ctx *ctx, int levels);
  * chosen from n.  P3T_EINVAL for another value. */
 p3t_status p3t_set_walk_mode(p3t_ctx *ctx, int mode);
 
+/* Sharding of one evaluation over `world` GPUs: every rank loads ALL particles and builds the
+ * same tree; p3t_eval_soft of the context with shard (rank, world) walks only the i-groups at positions rank,
+ * rank + world, rank + 2 world, ... of the hand-out order.  Accelerations, potentials and neighbour lists of the
+ * particles of the other groups come out as zero / empty, so the results of all ranks combine by addition of
+ * acc and pot and concatenation of the lists (paper_1506_04553_b200/multi.py does it with torch.distributed).
+ * Default (0, 1): everything.  P3T_EINVAL unless 0 <= rank < world. */
+p3t_status p3t_set_shard(p3t_ctx *ctx, int rank, int world);
+
 /* Load n particles: mass[n], pos[3n] (x,y,z interleaved), both host or both
  * device (on_device).  Host data is checked for non-finite values here
  * (P3T_EINVAL); device data is checked on the GPU and the error surfaces at

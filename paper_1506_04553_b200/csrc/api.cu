@@ -121,6 +121,8 @@ extern "C" p3t_status p3t_create(p3t_ctx **out, int device, size_t max_n, int ke
     ctx->ngroup = 64;
     ctx->merge_levels = 1;
     ctx->cells_dirty = true;
+    ctx->shard_rank = 0;
+    ctx->shard_world = 1;
     cudaError_t e = cudaSetDevice(device);
     cudaDeviceProp prop;
     if (e == cudaSuccess) e = cudaGetDeviceProperties(&prop, device);
@@ -222,6 +224,15 @@ extern "C" p3t_status p3t_set_group_merge_levels(p3t_ctx *ctx, int levels)
     if (!ctx || levels < 0 || levels > 4) return P3T_EINVAL;
     ctx->merge_levels = levels;
     ctx->built = false;
+    ctx->evaluated = false;
+    return P3T_OK;
+}
+
+extern "C" p3t_status p3t_set_shard(p3t_ctx *ctx, int rank, int world)
+{
+    if (!ctx || world < 1 || rank < 0 || rank >= world) return P3T_EINVAL;
+    ctx->shard_rank = rank;
+    ctx->shard_world = world;
     ctx->evaluated = false;
     return P3T_OK;
 }

@@ -121,6 +121,7 @@ struct p3t_ctx {
     size_t max_n, n, nbr_capacity;
     int key_bits, max_level, nleaf, ngroup, merge_levels;
     int walk_mode;                 // 0 auto, 1 one warp per group, 2 one CTA per group (cooperative)
+    int shard_rank, shard_world;   // this context walks the groups at positions rank, rank + world, ... of the hand-out order
     int sm_count;
     bool have_params, loaded, built, evaluated;
     bool cells_dirty;              // child counters need a memset before the next build

@@ -326,6 +326,7 @@ struct WalkArgs {
     const u32 *__restrict__ order_meta;
     u32 *__restrict__ group_class;   // cost class of every group of this walk
     u32 *order_hist;                 // [ORDER_CLASSES] groups per class
+    u32 shard_rank, shard_world;     // this launch walks positions rank, rank + world, ... of the hand-out order
     uint2 *pairs;
     u64 pair_cap;
     u64 *counters;
@@ -692,6 +693,7 @@ walk_kernel(WalkArgs A, const u32 *__restrict__ group_start, P3TParams prm, u32 
             if (lane == 0) g = (u32)atomicAdd(&A.counters[CNT_GROUP_TICKET], 1ull);
             g = __shfl_sync(0xffffffffu, g, 0);
         }
+        g = g * A.shard_world + A.shard_rank;   // (overflow-free: tickets stop at ngroups / world)
         if (g >= ngroups) break;
         if (ordered) g = A.group_order[g];
         const u32 gs = group_start[g], ge = group_start[g + 1];
@@ -796,6 +798,12 @@ p3t_status p3t_stage_walk(p3t_ctx *ctx)
     A.order_meta = w.order_meta;
     A.group_class = w.group_class;
     A.order_hist = w.order_hist;
+    A.shard_rank = (u32)ctx->shard_rank;
+    A.shard_world = (u32)ctx->shard_world;
+    if (ctx->shard_world > 1) {   // particles of the groups other ranks walk: zero acceleration, potential, neighbour count
+        P3T_CUDA(ctx, cudaMemsetAsync(w.accpot, 0, ctx->n * sizeof(float4), s));
+        P3T_CUDA(ctx, cudaMemsetAsync(w.nbr_count, 0, ctx->n * sizeof(u32), s));
+    }
     P3T_CUDA(ctx, cudaMemsetAsync(w.order_hist, 0, 2 * ORDER_CLASSES * sizeof(u32), s));   // class counts + scatter cursors
     // one CTA per group when there are too few groups to keep every warp busy to the end of the launch
     // (the group count lives on the device; n / ngroup is its lower bound up to the fill of the groups)
@@ -808,7 +816,9 @@ p3t_status p3t_stage_walk(p3t_ctx *ctx)
         if (coop) walk_kernel<1, true><<<grid, block, smem, s>>>(A, w.group_start, ctx->prm, w.walk_stack);
         else walk_kernel<1, false><<<grid, block, smem, s>>>(A, w.group_start, ctx->prm, w.walk_stack);
     }
-    // (the group count lives on the device: launch for its upper bound n)
+    // (the group count lives on the device: launch for its upper bound n; a sharded walk has seen only its own groups
+    //  and leaves the order as it is)
+    if (ctx->shard_world == 1)
     group_order_kernel<<<div_up(ctx->n, 256), 256, 0, s>>>(w.group_class, w.order_hist, w.order_hist + ORDER_CLASSES, w.counters,
                                                           w.group_order, w.order_meta);
     P3T_CUDA(ctx, cudaGetLastError());

@@ -220,3 +220,41 @@ def test_all_bodies_at_one_point_and_massless_bodies(oracle):
         acc, pot = ctx.get_acc_pot()
         a, p = oracle.direct(mass.astype(np.float64), cfg["pos"].astype(np.float64), cfg["eps"], cfg["r_in"], cfg["r_out"])
         assert np.median(rel_err(acc.astype(np.float64), a)) < 1e-3
+
+
+@pytest.mark.parametrize("world,mode", [(2, 1), (3, 1), (4, 2)])
+def test_sharded_evaluations_add_up_to_the_whole(world, mode):
+    """p3t_set_shard: the ranks' results (run one after the other on this GPU) combine to the unsharded evaluation:
+    every particle is produced by exactly one rank, bitwise the same with one warp per group."""
+    from paper_1506_04553_b200 import multi
+
+    b = _binding()
+    cfg = workloads.config(3, n=50000)
+    n = cfg["n"]
+    with b.P3T(n, key_bits=63, nbr_capacity=64 * n) as ctx:
+        ctx.set_walk_mode(mode)
+        ctx.set_params(cfg["eps"], cfg["theta"], cfg["r_in"], 10 * cfg["r_out"], 12 * cfg["r_out"])
+        ctx.soft_force(cfg["mass"], cfg["pos"])
+        a_full, p_full = ctx.get_acc_pot()
+        o_full, l_full = ctx.get_neighbours()
+        full = ctx.get_stats()
+        accs, pots, csrs, npp = [], [], [], 0
+        for r in range(world):
+            ctx.set_shard(r, world)
+            ctx.soft_force(cfg["mass"], cfg["pos"])
+            a, p = ctx.get_acc_pot()
+            accs.append(a); pots.append(p); csrs.append(ctx.get_neighbours())
+            st = ctx.get_stats()
+            npp += st["n_pp"] + st["n_pc"]
+        owners = sum((np.abs(p) > 0).astype(np.int64) for p in pots)
+        assert np.all(owners == 1)                                   # phi < 0 for every particle of a cluster
+        assert npp == full["n_pp"] + full["n_pc"]
+        a, p = multi.merge_forces(accs), multi.merge_forces(pots)
+        off, nbr = multi.merge_csr(csrs, n)
+        assert np.array_equal(off, o_full) and np.array_equal(nbr, l_full)
+        if mode == 1:
+            assert np.array_equal(a, a_full) and np.array_equal(p, p_full)
+        else:
+            assert np.abs(p / p_full - 1).max() <= 2e-6
+        with pytest.raises(b.P3TError):
+            ctx.set_shard(2, 2)

@@ -62,3 +62,59 @@ def test_rank_zero_is_the_single_gpu_workload_and_single_process_needs_no_backen
     assert multi.aggregate(None, 256, 2.5) == (256, 2.5)
     c = multi.rank_config(4, 1, n=256)                             # King model keeps its own generator
     assert c["pos"].shape == (256, 3) and not np.array_equal(c["pos"], multi.rank_config(4, 0, n=256)["pos"])
+
+
+def _shard_worker(rank, world, port, q):
+    import torch
+    import torch.distributed as dist
+
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        n = 10
+        owner = np.arange(n) % world                      # particle i is produced by rank i % world
+        acc = np.where((owner == rank)[:, None], np.arange(3 * n, dtype=np.float32).reshape(n, 3) + 1, 0).astype(np.float32)
+        pot = np.where(owner == rank, -np.arange(n, dtype=np.float32) - 1, 0).astype(np.float32)
+        cnt = np.where(owner == rank, np.arange(n) % 3, 0)
+        off = np.zeros(n + 1, dtype=np.uint64); off[1:] = np.cumsum(cnt)
+        nbr = np.concatenate([np.full(c, 100 * i, dtype=np.uint32) + np.arange(c, dtype=np.uint32) for i, c in enumerate(cnt)] + [np.zeros(0, np.uint32)])
+        ta, tp = torch.from_numpy(acc.copy()), torch.from_numpy(pot.copy())
+        multi.allreduce_forces(dist, ta, tp)
+        goff, gnbr = multi.allgather_csr(dist, off, nbr, n)
+        q.put((rank, ta.numpy(), tp.numpy(), goff, gnbr))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_sharded_results_combine_over_gloo():
+    import torch.multiprocessing as mp
+
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_shard_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    out = sorted((q.get(timeout=120) for _ in range(2)), key=lambda t: t[0])
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    n = 10
+    exp_acc = np.arange(3 * n, dtype=np.float32).reshape(n, 3) + 1
+    exp_pot = -np.arange(n, dtype=np.float32) - 1
+    cnt = np.arange(n) % 3
+    exp_off = np.zeros(n + 1, dtype=np.uint64); exp_off[1:] = np.cumsum(cnt)
+    exp_nbr = np.concatenate([np.full(c, 100 * i, dtype=np.uint32) + np.arange(c, dtype=np.uint32) for i, c in enumerate(cnt)])
+    for rank, acc, pot, off, nbr in out:                  # every rank ends with the full result
+        assert np.array_equal(acc, exp_acc) and np.array_equal(pot, exp_pot)
+        assert np.array_equal(off, exp_off) and np.array_equal(nbr, exp_nbr)
+
+
+def test_merge_csr_handles_empty_ranks():
+    n = 4
+    a = (np.array([0, 2, 2, 2, 3], dtype=np.uint64), np.array([7, 8, 9], dtype=np.uint32))
+    b = (np.zeros(n + 1, dtype=np.uint64), np.zeros(0, dtype=np.uint32))
+    c = (np.array([0, 0, 1, 1, 1], dtype=np.uint64), np.array([5], dtype=np.uint32))
+    off, nbr = multi.merge_csr([a, b, c], n)
+    assert off.tolist() == [0, 2, 3, 3, 4] and nbr.tolist() == [7, 8, 5, 9]
