@@ -231,6 +231,11 @@ def main():
     st = ctx.get_stats()
     ph = {k: float(np.mean(v)) for k, v in phases.items()}
     ffma_scalar = ffma_packed = None
+    nbr_hist = None
+    if rank == 0:      # neighbour-list length histogram of the last step (BASELINE.json config 4 asks for it)
+        cnt, _ = ctx.get_neighbour_counts()
+        hh = np.bincount(np.minimum(cnt, 16), minlength=17)
+        nbr_hist = {"length_0..15_and_16+": [int(x) for x in hh], "max": int(cnt.max()), "mean": float(cnt.mean())}
     if rank == 0:      # pure-FFMA calibration kernel, outside the timed region
         ffma_scalar, ffma_packed = ctx.measure_fp32_peak(False)[0], ctx.measure_fp32_peak(True)[0]
 
@@ -316,6 +321,7 @@ def main():
         "interactions": {"n_pp": st["n_pp"], "n_pc": st["n_pc"], "n_near": st["n_near"], "n_neighbours": st["n_neighbours"],
                          "pp_per_particle": st["n_pp"] / n, "pc_per_particle": st["n_pc"] / n},
         "tree": {"n_cells": st["n_cells"], "n_leaves": st["n_leaves"], "n_groups": st["n_groups"], "depth": st["depth"]},
+        "neighbour_lists": nbr_hist, "workspace_bytes": int(ctx.workspace.numel()),
         "phases_ms": ph,
         "roofline": {"bound": "alu", "kernel": "walk_kernel (a7+a8)", "achieved": walk_tflops, "peak": fp32_peak, "unit": "TFLOP/s",
                      "frac": walk_tflops / fp32_peak, "traffic": traffic, "traffic_source": traffic_src,

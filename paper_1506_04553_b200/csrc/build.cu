@@ -18,6 +18,7 @@
 // Checked against a recursive construction (oracle/keytree.py) in tests/test_gpu_tree.py.
 #include "p3t_internal.cuh"
 
+#define GROUP_MERGE_MIN_LEVEL 4                        // see the cut rule in levels_kernel
 #define BUILD_HALO 64                                  // >= max(NLEAF, NGROUP)
 #define BUILD_WIN (BUILD_TILE + 2 * BUILD_HALO + 16)   // window of c values held per tile (16-bit lanes)
 #define BUILD_WORDS (BUILD_WIN / 2)
@@ -216,7 +217,12 @@ __global__ void __launch_bounds__(BUILD_THREADS) levels_kernel(const signed char
                 const int c = win_get(s_c, t) - 1;
                 const int D = min(max_level, win_get(s_d, t));
                 const int g = min(max_level, win_get(s_g, t)), gp = i > 0 ? min(max_level, win_get(s_g, t - 1)) : 0;
-                const bool cut = (i == 0) || c < max(g, gp) - merge_levels;
+                // a group may straddle cells up to merge_levels above the natural group level, but only where that
+                // level is at least GROUP_MERGE_MIN_LEVEL: in the sparse outskirts the parent cell is so large that a
+                // group of consecutive bodies spans an octant, its box reaches the core and it opens the whole tree
+                // (one such group took 4.9 ms at N = 256K, 2.2x the rest of the launch)
+                const int gm = max(g, gp);
+                const bool cut = (i == 0) || c < max(gm - merge_levels, min(gm, GROUP_MERGE_MIN_LEVEL));
                 dl |= (u32)D << (8 * s);
                 cf |= (cut ? 1u : 0u) << (8 * s);
                 if (D > c) { atomicAdd(&s_cnt[c + 1], 1); atomicAdd(&s_cnt[D + 1], -1); }
