@@ -203,6 +203,9 @@ def main():
             ctx.get_acc_pot_into(acc_d, pot_d)
             multi.allreduce_forces(dist, acc_d, pot_d)
 
+    # the clock sampler starts with the warm-up steps (nvidia-smi needs a few hundred ms to deliver its first sample;
+    # the warm-up steps are the same load as the timed ones) and runs to the end of the timed region
+    sampler = ClockSampler(local) if rank == 0 else None
     for _ in range(args.warmup):
         flush.zero_()
         step()
@@ -210,7 +213,6 @@ def main():
     if dist:
         dist.barrier()
     torch.cuda.synchronize()
-    sampler = ClockSampler(local) if rank == 0 else None
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     phases = {k: [] for k in ("ms_sort", "ms_build", "ms_moments", "ms_walk", "ms_nbr")}
     for a, b in ev:
