@@ -101,16 +101,17 @@ p3t_status p3t_set_tree_params(p3t_ctx *ctx, int nleaf, int ngroup);
 
 /* Tuning: how many octree levels above its natural level (the level whose cell holds <= ngroup
  * bodies) an i-group's bodies may straddle.  0 = every group is one octree cell (partly filled
- * warps); 1 (default) = consecutive sibling cells are merged up to ngroup bodies.  Results do
- * not depend on it beyond rounding and the R-MAC box B. levels in 0..4. */
+ * warps); 1 (default) = consecutive sibling cells are merged up to ngroup bodies.  Where the natural
+ * level is above tree level 4 (sparse outskirts) groups never straddle, whatever this value.  Results
+ * do not depend on it beyond rounding and the R-MAC box B. levels in 0..4. */
 p3t_status p3t_set_group_merge_levels(p3t_ctx *ctx, int levels);
 
 /* How i-groups are mapped to warps in the tree walk.  1: one warp per group -- results are bitwise
  * reproducible.  2: the four warps of a CTA share one group through a common stack -- keeps the GPU busy
  * when there are few groups (small n) and shortens the tail of the launch; which warp evaluates which
  * cell depends on timing, so accelerations and potentials are reproducible to fp32 rounding of the
- * batch sums (about 1e-7 relative) rather than bitwise; neighbour lists are identical.  0 (default):
- * chosen from n.  P3T_EINVAL for another value. */
+ * batch sums (a few 1e-6 relative at most) rather than bitwise; neighbour lists are identical.  0 (default):
+ * chosen from n (mode 2 below about 1.5 groups per resident warp).  P3T_EINVAL for another value. */
 p3t_status p3t_set_walk_mode(p3t_ctx *ctx, int mode);
 
 /* Sharding of one evaluation over `world` GPUs: every rank loads ALL particles and builds the
