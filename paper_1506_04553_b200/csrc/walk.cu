@@ -20,6 +20,10 @@
 #ifndef WALK_PC_UNROLL
 #define WALK_PC_UNROLL 8
 #endif
+// full batches of 32 list entries summed in fp32 before the sums go to the fp64 accumulators
+#ifndef WALK_FLUSH_EVERY
+#define WALK_FLUSH_EVERY 2
+#endif
 constexpr int kPpUnroll = WALK_PP_UNROLL, kPcUnroll = WALK_PC_UNROLL;
 
 #ifdef P3T_WALK_PROFILE
@@ -102,8 +106,14 @@ template <int NI> struct Acc {
 #pragma unroll
         for (int b = 0; b < NI; ++b) dax[b] = day[b] = daz[b] = dph[b] = 0.0;
     }
+    int pending = 0;                           // batches added to the fp32 sums since the last flush
+    __device__ __forceinline__ void flush_lazy()
+    {
+        if (++pending >= WALK_FLUSH_EVERY) flush();
+    }
     __device__ __forceinline__ void flush()
     {
+        pending = 0;
 #pragma unroll
         for (int b = 0; b < NI; ++b) {
             dax[b] += (double)vget(ax, b); day[b] += (double)vget(ay, b);
@@ -195,7 +205,7 @@ __device__ __forceinline__ void eval_far(const WarpShared &ws, u32 head, u32 cnt
     } else {
         for (u32 j = 0; j < cnt; ++j) pp_body<NI>(ws.far[head + j], t, eps2, acc);
     }
-    acc.flush();
+    acc.flush_lazy();
 }
 
 // ---- p-c, softened monopole + quadrupole about the centre of mass (rule R-QUAD), K = W = 1 ----------
@@ -248,7 +258,7 @@ __device__ __forceinline__ void eval_pc(const WarpShared &ws, u32 head, u32 cnt,
         acc.ay = vfma(coef, dy, vfma(n5, qdy, acc.ay));
         acc.az = vfma(coef, dz, vfma(n5, qdz, acc.az));
     }
-    acc.flush();
+    acc.flush_lazy();
 }
 
 // ---- p-p slow path: K (Eq. 12) on the force, W (Eq. 16-17) on the potential, j != i by index,
@@ -293,7 +303,7 @@ __device__ __forceinline__ void eval_near(const WarpShared &ws, u32 head, u32 cn
             }
         }
     }
-    acc.flush();
+    acc.flush_lazy();
 }
 
 __device__ __forceinline__ u64 globaltimer_ns()
@@ -601,6 +611,7 @@ __device__ __forceinline__ void walk_group(WarpShared *wsall, const StackRef &st
         eval_near<NI>(ws, near_head, near_cnt, tg, isorted, iuser, prm, A.sorted_idx, A.pairs, A.pair_cap, A.counters, nnb, acc, lane);
         n_near += near_cnt;
     }
+    acc.flush();
     __syncwarp();
     if (COOP) {
         // partial sums of warps 1-3 -> their own (now dead) p-c ring, neighbour counts -> far ring; warp 0 adds
