@@ -332,7 +332,7 @@ struct WalkArgs {
     float4 *__restrict__ accpot;
     u32 *__restrict__ nbr_count;
     uint4 *__restrict__ group_stats;
-    const u32 *__restrict__ group_order;   // ticket -> group, valid if order_meta[0] == number of groups
+    const u32 *__restrict__ group_order;   // position -> group of the previous call, a permutation of 0..order_meta[0]-1
     const u32 *__restrict__ order_meta;
     u32 *__restrict__ group_class;   // cost class of every group of this walk
     u32 *order_hist;                 // [ORDER_CLASSES] groups per class
@@ -687,7 +687,13 @@ walk_kernel(WalkArgs A, const u32 *__restrict__ group_start, P3TParams prm, u32 
         st.limit = WALK_STACK_SMEM + WALK_STACK_GMEM;
     }
     const u32 ngroups = (u32)A.counters[CNT_NGROUPS];
-    const bool ordered = A.order_meta[0] == ngroups;   // heaviest groups of the previous call first
+    // Hand-out order: the groups of the previous call by decreasing cost (group_order, a permutation of 0..ng_prev-1).
+    // Between two calls of a simulation the number of groups changes by a few and group g still covers about the
+    // same region, so the old order is used as it is: positions below ng_prev go through it (entries that no longer
+    // exist are skipped), positions from ng_prev on are the new groups themselves.
+    // A sharded walk hands out positions in Morton order: every rank must map positions to groups alike.
+    const u32 ng_prev = A.shard_world > 1 ? 0u : A.order_meta[0];
+    const u32 npos = max(ngroups, ng_prev);
     u64 tot_pp = 0, tot_pc = 0, tot_near = 0;
 
     while (true) {
@@ -704,9 +710,13 @@ walk_kernel(WalkArgs A, const u32 *__restrict__ group_start, P3TParams prm, u32 
             if (lane == 0) g = (u32)atomicAdd(&A.counters[CNT_GROUP_TICKET], 1ull);
             g = __shfl_sync(0xffffffffu, g, 0);
         }
-        g = g * A.shard_world + A.shard_rank;   // (overflow-free: tickets stop at ngroups / world)
-        if (g >= ngroups) break;
-        if (ordered) g = A.group_order[g];
+        g = g * A.shard_world + A.shard_rank;   // (overflow-free: tickets stop at npos / world)
+        if (g >= npos) break;
+        if (g < ng_prev) g = A.group_order[g];
+        if (g >= ngroups) {                      // a group of the previous call that is gone
+            if (COOP) __syncthreads();           // ctl is rewritten for the next ticket
+            continue;
+        }
         const u32 gs = group_start[g], ge = group_start[g + 1];
         const u64 pp0 = tot_pp, pc0 = tot_pc;
         const u32 t0 = (u32)globaltimer_ns();
