@@ -215,6 +215,14 @@ def main():
     torch.cuda.synchronize()
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     phases = {k: [] for k in ("ms_sort", "ms_build", "ms_moments", "ms_walk", "ms_nbr")}
+    # BASELINE.json configs[1]: consecutive calls "while positions are drifted by a leapfrog step dt_soft using the
+    # returned forces" -- the kick and drift run between the timed steps (torch ops on the device, not timed)
+    drift = cfg.get("dt_soft") is not None and not shard
+    if drift:
+        vel_l = torch.from_numpy(cfg["vel"]).to(dev)
+        acc_l = torch.empty((n, 3), dtype=torch.float32, device=dev)
+        pot_l = torch.empty(n, dtype=torch.float32, device=dev)
+        pos_d = pos_d.clone()
     for a, b in ev:
         flush.zero_()
         a.record()
@@ -223,6 +231,10 @@ def main():
         st = ctx.get_stats()           # synchronises; per-phase times come from the library's own CUDA events
         for k in phases:
             phases[k].append(st[k])
+        if drift:
+            ctx.get_acc_pot_into(acc_l, pot_l)
+            vel_l += cfg["dt_soft"] * acc_l
+            pos_d += cfg["dt_soft"] * vel_l
     torch.cuda.synchronize()
     if dist:
         dist.barrier()
@@ -316,7 +328,7 @@ def main():
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": cfg["name"], "n": n, "theta": cfg["theta"], "eps": cfg["eps"], "r_out": cfg["r_out"],
                    "r_search": cfg["r_search"], "key_bits": cfg["key_bits"], "nleaf": nleaf, "ngroup": ngroup,
-                   "l2": "flushed between steps (512 MiB write)", "parallelism": (f"one cluster sharded over {world} GPUs by i-groups, all-reduce of the results" if shard
+                   "l2": "flushed between steps (512 MiB write)", "positions": "drifted between steps (leapfrog, dt_soft)" if drift else "same every step", "parallelism": (f"one cluster sharded over {world} GPUs by i-groups, all-reduce of the results" if shard
                                    else f"{world} independent cluster(s), one per GPU")},
         "interactions_per_s": (st["n_pp"] + st["n_pc"]) / (ph["ms_walk"] * 1e-3),
         "walk_particles_per_s": n / (ph["ms_walk"] * 1e-3),
