@@ -124,6 +124,8 @@ struct p3t_ctx {
     int shard_rank, shard_world;   // this context walks the groups at positions rank, rank + world, ... of the hand-out order
     int sm_count;
     bool have_params, loaded, built, evaluated;
+    bool sort_attr_set, walk_attr_set;   // cudaFuncSetAttribute done on this context's device
+    int sort_ctas_per_sm;
     bool cells_dirty;              // child counters need a memset before the next build
     bool tiles_ready;              // sentinel records of the build look-back written
     bool status_clean;             // the look-back buffers have been zeroed once (they clean themselves afterwards)

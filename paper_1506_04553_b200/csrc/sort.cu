@@ -378,17 +378,14 @@ p3t_status p3t_stage_sort(p3t_ctx *ctx)
     cudaStream_t s = ctx->stream;
     int passes = (3 * ctx->max_level + 7) / 8;   // 8 for 63-bit keys, 4 for 30-bit keys
     u32 ntiles = div_up(n, SORT_TILE);
-    static bool attr_set = false;
-    if (!attr_set) {
+    if (!ctx->sort_attr_set) {   // function attributes are per device: kept per context
         P3T_CUDA(ctx, cudaFuncSetAttribute(onesweep_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(OnesweepSmem)));
         P3T_CUDA(ctx, cudaFuncSetAttribute(onesweep_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(OnesweepSmem)));
-        attr_set = true;
+        P3T_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->sort_ctas_per_sm, onesweep_kernel<16>, SORT_THREADS, sizeof(OnesweepSmem)));
+        ctx->sort_attr_set = true;
     }
     const size_t status_rows = w.n_tiles_max + SORT_LOOKBACK;   // SORT_LOOKBACK sentinel rows in front of row 0
-    static int ctas_per_sm = 0;
-    if (!ctas_per_sm)
-        P3T_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas_per_sm, onesweep_kernel<16>, SORT_THREADS, sizeof(OnesweepSmem)));
-    const int resident = ctas_per_sm * ctx->sm_count;   // a grid up to this size is co-resident: no ticket needed
+    const int resident = ctx->sort_ctas_per_sm * ctx->sm_count;   // a grid up to this size is co-resident: no ticket needed
     if (!ctx->status_clean) {   // first build of this context: buffers zeroed, sentinel rows = INC | 0 
         P3T_CUDA(ctx, cudaMemsetAsync(w.tile_status, 0, 2 * status_rows * 256 * sizeof(u32), s));
         for (int b = 0; b < 2; ++b)

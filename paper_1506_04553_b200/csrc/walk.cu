@@ -802,13 +802,12 @@ p3t_status p3t_stage_walk(p3t_ctx *ctx)
     u32 grid = (u32)ctx->sm_count * WALK_CTAS;
     if ((size_t)grid * WALK_WARPS > w.walk_warps_max) grid = (u32)(w.walk_warps_max / WALK_WARPS);
     const size_t smem = (sizeof(WarpShared) + WALK_STACK_SMEM * sizeof(u32)) * WALK_WARPS + sizeof(CtaCtl);
-    static bool attr_set = false;
-    if (!attr_set) {
+    if (!ctx->walk_attr_set) {   // function attributes are per device: kept per context
         P3T_CUDA(ctx, cudaFuncSetAttribute(walk_kernel<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         P3T_CUDA(ctx, cudaFuncSetAttribute(walk_kernel<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         P3T_CUDA(ctx, cudaFuncSetAttribute(walk_kernel<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         P3T_CUDA(ctx, cudaFuncSetAttribute(walk_kernel<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_set = true;
+        ctx->walk_attr_set = true;
     }
     WalkArgs A;
     A.body = w.body; A.sorted_idx = w.idx[ctx->cur];
