@@ -54,7 +54,7 @@ def algorithmic_bytes_tree(n, key_bits, n_cells, n_groups):
     gather = 4 * n + 16 * n + 16 * n + 8 * n + n  # a4: idx, body in, body out, keys -> common-prefix levels (1 B)
     build = 2 * n + 2 * n + 32 * n_cells + 4 * n_groups   # a5: c read twice, leaf level + cut flag written and read, topology, group starts
     moments = 16 * n + 88 * n_cells + 88 * n_cells  # a6: read bodies; write cells; parents re-read their children
-    return dict(sort=pack + keys + sort + gather, build=build, moments=moments)
+    return dict(pack=pack, sort=keys + sort + gather, build=build, moments=moments)
 
 
 class ClockSampler:
@@ -214,7 +214,7 @@ def main():
         dist.barrier()
     torch.cuda.synchronize()
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    phases = {k: [] for k in ("ms_sort", "ms_build", "ms_moments", "ms_walk", "ms_nbr")}
+    phases = {k: [] for k in ("ms_pack", "ms_sort", "ms_build", "ms_moments", "ms_walk", "ms_nbr")}
     # BASELINE.json configs[1]: consecutive calls "while positions are drifted by a leapfrog step dt_soft using the
     # returned forces" -- the kick and drift run between the timed steps (torch ops on the device, not timed)
     drift = cfg.get("dt_soft") is not None and not shard
@@ -318,7 +318,7 @@ def main():
     walk_tflops = flops / (ph["ms_walk"] * 1e-3) / 1e12
     ab = algorithmic_bytes_tree(n, cfg["key_bits"], st["n_cells"], st["n_groups"])
     hbm = {k: ab[k] / (ph["ms_" + k] * 1e-3) / 1e9 for k in ab}
-    tree_ms = ph["ms_sort"] + ph["ms_build"] + ph["ms_moments"]
+    tree_ms = ph["ms_pack"] + ph["ms_sort"] + ph["ms_build"] + ph["ms_moments"]
     # pack | keys+hist, onesweep passes, gather | levels, emit | moments (leaves, internal) | walk, group order | neighbour CSR (5)
     launches = 1 + (1 + st["sort_passes"] + 1) + 2 + 2 + 2 + 5
 

@@ -72,6 +72,7 @@ typedef struct {
     float ms_walk;           /* a7-a8 */
     float ms_nbr;            /* a9 */
     float ms_hard;           /* last p3t_eval_hard */
+    float ms_pack;           /* a1: pack + bounding cube of the last p3t_load_particles (after any host-to-device copy) */
 } p3t_stats;
 
 /* Bytes of device workspace p3t_create needs for up to max_n particles,

@@ -45,7 +45,7 @@ class Stats(C.Structure):
                 ("n_neighbours", C.c_uint64), ("n_cells", C.c_uint32), ("n_leaves", C.c_uint32),
                 ("n_groups", C.c_uint32), ("depth", C.c_uint32), ("max_list", C.c_uint32),
                 ("sort_passes", C.c_uint32), ("ms_sort", C.c_float), ("ms_build", C.c_float),
-                ("ms_moments", C.c_float), ("ms_walk", C.c_float), ("ms_nbr", C.c_float), ("ms_hard", C.c_float)]
+                ("ms_moments", C.c_float), ("ms_walk", C.c_float), ("ms_nbr", C.c_float), ("ms_hard", C.c_float), ("ms_pack", C.c_float)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}

@@ -38,12 +38,10 @@ size_t p3t_layout(Workspace &ws, char *base, size_t max_n, int key_bits, size_t 
     ws.in_pos = b.take<float>(3 * n);
     ws.body_user = b.take<float4>(n);
     ws.cube = b.take<float>(8);
-    ws.bbox_bits = b.take<u32>(8);
     ws.keys[0] = b.take<u64>(n);
     ws.keys[1] = b.take<u64>(n);
     ws.idx[0] = b.take<u32>(n);
     ws.idx[1] = b.take<u32>(n);
-    ws.hist = b.take<u32>(8 * 256);
     ws.tile_status = b.take<u32>(2 * (ws.n_tiles_max + 64) * 256);   // + sentinel rows (sort.cu)
     ws.body = b.take<float4>(n);
     ws.clev = b.take<signed char>(n + 8);
@@ -57,7 +55,6 @@ size_t p3t_layout(Workspace &ws, char *base, size_t max_n, int key_bits, size_t 
     ws.group_order = b.take<u32>(n);
     ws.order_meta = b.take<u32>(4);
     ws.group_class = b.take<u32>(n);
-    ws.order_hist = b.take<u32>(2048);
     ws.cell_mac = b.take<float4>(ws.cell_cap);
     ws.cell_mom0 = b.take<float4>(ws.cell_cap);
     ws.cell_mom1 = b.take<float4>(ws.cell_cap);
@@ -78,7 +75,10 @@ size_t p3t_layout(Workspace &ws, char *base, size_t max_n, int key_bits, size_t 
     ws.nbr_cursor = b.take<u32>(n);
     ws.subset = b.take<u32>(n);
     ws.hard_out = b.take<double>(7 * n);
+    ws.hist = b.take<u32>(8 * 256);            // hist | counters | order_hist are contiguous (p3t_internal.cuh)
     ws.counters = b.take<u64>(CNT_WORDS);
+    ws.order_hist = b.take<u32>(2048);
+    ws.bbox_bits = reinterpret_cast<u32 *>(ws.counters + CNT_BBOX);   // zeroed with the counters at load
     ws.walk_stack = b.take<u32>(ws.walk_warps_max * WALK_STACK_GMEM);
     ws.scan_tmp = b.take<u64>((n + 1023) / 1024 + 2);
     b.off = (b.off + 255) & ~size_t(255);
@@ -139,7 +139,7 @@ extern "C" p3t_status p3t_create(p3t_ctx **out, int device, size_t max_n, int ke
     }
     ctx->base = static_cast<char *>(workspace);
     if (cudaMemsetAsync(ctx->ws.order_meta, 0, 4 * sizeof(u32), ctx->stream) != cudaSuccess) { delete ctx; return P3T_ECUDA; }
-    for (int i = 0; i < 10; ++i) {
+    for (int i = 0; i < 12; ++i) {
         if (cudaEventCreate(&ctx->ev[i]) != cudaSuccess) { delete ctx; return P3T_ECUDA; }
     }
     *out = ctx;
@@ -150,7 +150,7 @@ extern "C" p3t_status p3t_destroy(p3t_ctx *ctx)
 {
     if (!ctx) return P3T_EINVAL;
     cudaStreamSynchronize(ctx->stream);
-    for (int i = 0; i < 10; ++i)
+    for (int i = 0; i < 12; ++i)
         if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
     delete ctx;
     return P3T_OK;
@@ -295,8 +295,11 @@ extern "C" p3t_status p3t_load_particles(p3t_ctx *ctx, size_t n, const float *ma
         d_pos = ctx->ws.in_pos;
     }
     ctx->n = n;
+    P3T_CUDA(ctx, cudaEventRecord(ctx->ev[9], ctx->stream));
     p3t_status st = p3t_stage_pack(ctx, d_mass, d_pos);
     if (st != P3T_OK) return st;
+    P3T_CUDA(ctx, cudaEventRecord(ctx->ev[10], ctx->stream));
+    ctx->ev_pack = true;
     ctx->loaded = true;
     return P3T_OK;
 }
@@ -500,6 +503,7 @@ extern "C" p3t_status p3t_get_stats(p3t_ctx *ctx, p3t_stats *out)
         cudaEventElapsedTime(&out->ms_nbr, ctx->ev[5], ctx->ev[6]);
     }
     if (ctx->ev_hard) cudaEventElapsedTime(&out->ms_hard, ctx->ev[7], ctx->ev[8]);
+    if (ctx->ev_pack) cudaEventElapsedTime(&out->ms_pack, ctx->ev[9], ctx->ev[10]);
     return st;
 }
 

@@ -63,7 +63,7 @@ p3t_status p3t_stage_direct(p3t_ctx *ctx, const u32 *d_subset, size_t n_subset)
     Workspace &w = ctx->ws;
     cudaStream_t s = ctx->stream;
     u32 n = (u32)ctx->n;
-    P3T_CUDA(ctx, cudaMemsetAsync(w.counters, 0, 8 * sizeof(u64), s));
+    P3T_CUDA(ctx, cudaMemsetAsync(w.counters + CNT_NPP, 0, 8 * sizeof(u64), s));
     P3T_CUDA(ctx, cudaMemsetAsync(w.accpot, 0, (size_t)n * sizeof(float4), s));
     P3T_CUDA(ctx, cudaMemsetAsync(w.nbr_count, 0, (size_t)n * sizeof(u32), s));
     direct_kernel<<<div_up(n_subset, DIRECT_THREADS), DIRECT_THREADS, 0, s>>>(w.body_user, n, d_subset, (u32)n_subset, ctx->prm,

@@ -56,15 +56,19 @@ struct P3TParams {
     double wl;
 };
 
-// Device-side counters (one block of 64-bit words in the workspace, zeroed per eval/build).
+// Device-side counters (one block of 64-bit words in the workspace).  Layout in memory:
+//   hist [8][256] u32 | counters: build words, load words, eval words | order_hist [2][1024] u32
+// so that each stage zeroes what it needs with ONE memset: the build hist + build words, load the whole
+// counter block, an evaluation the eval words + order_hist.
 enum {
-    // zeroed at every eval
-    CNT_NPP = 0, CNT_NPC, CNT_NNEAR, CNT_PAIRS, CNT_GROUP_TICKET, CNT_MAXLIST, CNT_ERR_EVAL, CNT_EVAL_SPARE,
-    // zeroed at every build
-    CNT_NCELLS = 8, CNT_NLEAVES, CNT_NGROUPS, CNT_DEPTH, CNT_ERR_BUILD, CNT_HEAD_TICKET, CNT_HEAD_SPARE0, CNT_HEAD_SPARE1,
-    CNT_SORT_TICKET = 16 /* one per pass, 8 */,
-    // zeroed at load
-    CNT_NONFINITE = 24,
+    // zeroed at every build (together with the digit histograms in front of the block)
+    CNT_NCELLS = 0, CNT_NLEAVES, CNT_NGROUPS, CNT_DEPTH, CNT_ERR_BUILD, CNT_HEAD_TICKET, CNT_HEAD_SPARE0, CNT_HEAD_SPARE1,
+    CNT_SORT_TICKET = 8 /* one per pass, 8 */,
+    // zeroed at load only
+    CNT_NONFINITE = 16,
+    CNT_BBOX = 18 /* three words: six 32-bit min/max accumulators of the bounding cube */,
+    // zeroed at every eval (together with order_hist behind the block)
+    CNT_NPP = 24, CNT_NPC, CNT_NNEAR, CNT_PAIRS, CNT_GROUP_TICKET, CNT_MAXLIST, CNT_ERR_EVAL, CNT_EVAL_SPARE,
     CNT_WORDS = 32
 };
 enum { ERR_STACK_OVERFLOW = 1, ERR_CELL_CAPACITY = 2 };
@@ -75,7 +79,7 @@ struct Workspace {
     float4 *body_user;             // (x,y,z,m) user order
     // a1-a4
     float *cube;                   // [8]: min xyz, side, max xyz, pad   (cube[0..3] = P3T_ARR_ROOT_CUBE)
-    u32 *bbox_bits;                // [6] ordered-int min/max accumulators
+    u32 *bbox_bits;                // [6] ordered-int accumulators (inverted min, max), inside the counter block
     u64 *keys[2];
     u32 *idx[2];
     u32 *hist;                     // [8][256] digit histograms -> exclusive offsets
@@ -134,8 +138,8 @@ struct p3t_ctx {
     float eps, theta, r_in, r_out, r_search;
     Workspace ws;
     char *base;
-    cudaEvent_t ev[10];            // phase boundaries: 0 build start,1 sort end,2 build end,3 moments end,4 eval start,5 walk end,6 nbr end,7/8 hard
-    bool ev_build, ev_eval, ev_hard;
+    cudaEvent_t ev[12];            // phase boundaries: 0 build start,1 sort end,2 build end,3 moments end,4 eval start,5 walk end,6 nbr end,7/8 hard,9/10 pack
+    bool ev_build, ev_eval, ev_hard, ev_pack;
     char err[512];
     // host mirrors (valid after sync)
     u64 h_counters[CNT_WORDS];

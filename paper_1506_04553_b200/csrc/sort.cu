@@ -42,7 +42,7 @@ __global__ void __launch_bounds__(256) pack_bbox_kernel(const float *__restrict_
         int d = threadIdx.x;
         float l = s_lo[0][d], h = s_hi[0][d];
         for (int w = 1; w < 8; ++w) { l = fminf(l, s_lo[w][d]); h = fmaxf(h, s_hi[w][d]); }
-        atomicMin(&bbox_bits[d], float_to_ordered(l));
+        atomicMax(&bbox_bits[d], ~float_to_ordered(l));   // minimum kept inverted: zero is the neutral start of both halves
         atomicMax(&bbox_bits[3 + d], float_to_ordered(h));
     }
     if (threadIdx.x == 0 && s_bad) atomicAdd(&counters[CNT_NONFINITE], 1ull);
@@ -53,8 +53,6 @@ p3t_status p3t_stage_pack(p3t_ctx *ctx, const float *d_mass, const float *d_pos)
     Workspace &w = ctx->ws;
     u32 n = (u32)ctx->n;
     P3T_CUDA(ctx, cudaMemsetAsync(w.counters, 0, CNT_WORDS * sizeof(u64), ctx->stream));
-    P3T_CUDA(ctx, cudaMemsetAsync(w.bbox_bits, 0xff, 3 * sizeof(u32), ctx->stream));
-    P3T_CUDA(ctx, cudaMemsetAsync(w.bbox_bits + 3, 0x00, 3 * sizeof(u32), ctx->stream));
     u32 grid = min(div_up(n, 256 * 4), (u32)ctx->sm_count * 8);
     pack_bbox_kernel<<<grid, 256, 0, ctx->stream>>>(d_mass, d_pos, w.body_user, w.bbox_bits, w.counters, n);
     P3T_CUDA(ctx, cudaGetLastError());
@@ -103,7 +101,7 @@ __device__ __forceinline__ void root_cube(const u32 *bbox_bits, float &minx, flo
 {
     float lo[3], hi[3];
 #pragma unroll
-    for (int d = 0; d < 3; ++d) { lo[d] = ordered_to_float(bbox_bits[d]); hi[d] = ordered_to_float(bbox_bits[3 + d]); }
+    for (int d = 0; d < 3; ++d) { lo[d] = ordered_to_float(~bbox_bits[d]); hi[d] = ordered_to_float(bbox_bits[3 + d]); }
     float ext = fmaxf(hi[0] - lo[0], fmaxf(hi[1] - lo[1], hi[2] - lo[2]));
     side = ext * (1.f + 4e-6f);
     if (!(side > 0.f) || !isfinite(side)) side = 1.f;
@@ -392,8 +390,8 @@ p3t_status p3t_stage_sort(p3t_ctx *ctx)
             fill_u32_kernel<<<SORT_LOOKBACK, 256, 0, s>>>(w.tile_status + b * status_rows * 256, OS_FLAG_INC);
         ctx->status_clean = true;
     }
-    P3T_CUDA(ctx, cudaMemsetAsync(w.counters + CNT_NCELLS, 0, 16 * sizeof(u64), s));   // build counters + sort tickets
-    P3T_CUDA(ctx, cudaMemsetAsync(w.hist, 0, 8 * 256 * sizeof(u32), s));
+    // digit histograms + build counters + sort tickets: contiguous, one memset
+    P3T_CUDA(ctx, cudaMemsetAsync(w.hist, 0, (size_t)((char *)(w.counters + CNT_NONFINITE) - (char *)w.hist), s));
     u32 grid = min(div_up(n, 256 * 8), (u32)ctx->sm_count * 8);   // every CTA flushes 8 x 256 histogram bins with global atomics: few, fat CTAs
     if (ctx->cells_dirty) {   // first build, or the last one ended in an error: all child counters and prev_ncells -> 0
         P3T_CUDA(ctx, cudaMemsetAsync(w.cell_nchild, 0, (size_t)((char *)(w.cell_ready + w.cell_cap) - (char *)w.cell_nchild), s));

@@ -798,7 +798,8 @@ p3t_status p3t_stage_walk(p3t_ctx *ctx)
 {
     Workspace &w = ctx->ws;
     cudaStream_t s = ctx->stream;
-    P3T_CUDA(ctx, cudaMemsetAsync(w.counters, 0, 8 * sizeof(u64), s));   // eval counters
+    // eval counters + cost-class counts and scatter cursors of the group order: contiguous, one memset
+    P3T_CUDA(ctx, cudaMemsetAsync(w.counters + CNT_NPP, 0, 8 * sizeof(u64) + 2 * ORDER_CLASSES * sizeof(u32), s));
     u32 grid = (u32)ctx->sm_count * WALK_CTAS;
     if ((size_t)grid * WALK_WARPS > w.walk_warps_max) grid = (u32)(w.walk_warps_max / WALK_WARPS);
     const size_t smem = (sizeof(WarpShared) + WALK_STACK_SMEM * sizeof(u32)) * WALK_WARPS + sizeof(CtaCtl);
@@ -824,7 +825,6 @@ p3t_status p3t_stage_walk(p3t_ctx *ctx)
         P3T_CUDA(ctx, cudaMemsetAsync(w.accpot, 0, ctx->n * sizeof(float4), s));
         P3T_CUDA(ctx, cudaMemsetAsync(w.nbr_count, 0, ctx->n * sizeof(u32), s));
     }
-    P3T_CUDA(ctx, cudaMemsetAsync(w.order_hist, 0, 2 * ORDER_CLASSES * sizeof(u32), s));   // class counts + scatter cursors
     // one CTA per group when there are too few groups to keep every warp busy to the end of the launch
     // (the group count lives on the device; n / ngroup is its lower bound up to the fill of the groups)
     bool coop = ctx->walk_mode == 2 || (ctx->walk_mode == 0 && 2 * (ctx->n / (size_t)ctx->ngroup) < (size_t)WALK_COOP_BELOW_X2 * grid * WALK_WARPS);
