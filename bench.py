@@ -102,10 +102,18 @@ def time_oracle(cfg, budget_particles):
     r = tree.walk(cfg["eps"], cfg["theta"], cfg["r_in"], cfg["r_out"], cfg["r_search"], subset=sub)
     t_walk = time.perf_counter() - t0
     t_full = t_build + t_walk * n / ns
+    # O2 (direct sum, the definition the tree approximates) on a small target subset, extrapolated to all N targets
+    nd = min(n, max(16, int(2.5e8 // n)))
+    subd = np.sort(np.random.default_rng(11).choice(n, nd, replace=False)).astype(np.int64)
+    t0 = time.perf_counter()
+    O.direct(m, q, cfg["eps"], cfg["r_in"], cfg["r_out"], subset=subd)
+    t_direct = time.perf_counter() - t0
+    direct = dict(pairs_per_s=nd * (n - 1) / t_direct, extrapolated_s_per_evaluation=t_direct * n / nd,
+                  sample=f"O2 fp64 direct sum on {nd} seeded targets ({t_direct:.2f} s), scaled by N/{nd}: extrapolated")
     return dict(value=n / t_full, unit="particles/s", cores=O.num_threads(), kind="oracle",
                 sample=f"O4 fp64 CPU Barnes-Hut (gcc -O2 -fopenmp): tree build over all {n} bodies ({t_build:.2f} s) + walk of "
                        f"{ns} seeded random targets ({t_walk:.2f} s), walk time scaled by N/{ns}",
-                interactions_per_s=float((r["n_pp"].sum() + r["n_pc"].sum()) / t_walk)), t_build + t_walk
+                interactions_per_s=float((r["n_pp"].sum() + r["n_pc"].sum()) / t_walk), direct_sum=direct), t_build + t_walk
 
 
 def run_reference(args):
