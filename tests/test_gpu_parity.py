@@ -151,13 +151,15 @@ def test_p10_plummer_potential_energy():
         assert ctx.get_neighbour_counts()[1] == 0
 
 
-def test_config2_leapfrog_calls(oracle):
-    """Config 2's recipe at reduced N: 10 calls with rebuild while positions drift by leapfrog steps."""
-    cfg = workloads.config(2, n=16384)
+@pytest.mark.parametrize("n,key_bits", [(16384, 30), (65536, 63)])
+def test_config2_leapfrog_calls(oracle, n, key_bits):
+    """Config 2 (at its full N = 65536 with 63-bit keys, and at reduced N with 30-bit keys): 10 calls with rebuild while
+    positions drift by leapfrog steps; the first and the last call checked against the direct sum on all targets."""
+    cfg = workloads.config(2, n=n)
     m, q = widen(cfg)
     pos, vel = cfg["pos"].copy(), cfg["vel"].copy()
     dt = np.float32(cfg["dt_soft"])
-    with _ctx(cfg) as ctx:
+    with _ctx(cfg, key_bits=key_bits) as ctx:
         ctx.set_params(cfg["eps"], cfg["theta"], cfg["r_in"], cfg["r_out"], cfg["r_search"])
         for step in range(10):
             ctx.soft_force(cfg["mass"], pos)
