@@ -207,3 +207,28 @@ def test_full_size_sampled_parity(oracle, k, n):
         ctx.eval_direct(sub.astype(np.uint32))
         accd, potd = ctx.get_acc_pot()
         assert rel_err(accd[sub].astype(np.float64), a).max() <= TOL_THETA0
+
+
+def test_king_core_with_long_lists(oracle):
+    """Config 4's variant of SURVEY.md 8(d): r_out = 0.01 makes the lists of the King core long (about a hundred
+    entries): the K/W path, the pair buffer and the CSR build under load, against O2 / O3 on a seeded subset that is
+    half core particles."""
+    cfg = workloads.config(4)
+    n = cfg["n"]
+    r_in, r_out, h = (float(np.float32(x)) for x in (0.001, 0.01, 0.013))
+    m, q = widen(cfg)
+    rng = np.random.default_rng(44)
+    core = np.argsort(np.linalg.norm(q, axis=1))[:20000]
+    sub = np.unique(np.concatenate([rng.choice(core, 1024, replace=False), rng.choice(n, 1024, replace=False)])).astype(np.int64)
+    a, p = oracle.direct(m, q, cfg["eps"], r_in, r_out, subset=sub)
+    with _ctx(cfg, nbr_capacity=64 * n) as ctx:
+        acc, pot, off, nbr = _run_tree(ctx, cfg, radii=(r_in, r_out, h))
+        cnt = np.diff(off.astype(np.int64))
+        print(f"King r_out=0.01: mean list {cnt.mean():.2f}, max {cnt.max()}, entries {cnt.sum()}")
+        assert cnt.max() >= 50
+        e = rel_err(acc[sub], a)
+        assert np.median(e) <= TOL_MEDIAN and np.percentile(e, 99) <= TOL_P99
+        ep = np.abs(pot[sub] / p - 1)
+        assert np.median(ep) <= TOL_MEDIAN and np.percentile(ep, 99) <= TOL_P99
+        c2 = dict(cfg)
+        _check_lists(oracle, c2, off, nbr, h, subset=sub)
