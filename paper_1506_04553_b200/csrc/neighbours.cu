@@ -111,20 +111,51 @@ __global__ void __launch_bounds__(256) fill_lists_kernel(const uint2 *__restrict
     }
 }
 
+#define SORT_LIST_SERIAL 16   // lists up to this length are sorted by their own thread
+
+// ascending order inside every list: one thread per list, insertion sort for the short ones (the usual case: a
+// fraction of an entry per particle); the long ones (dense cores, large h) are queued for sort_long_lists_kernel
 __global__ void __launch_bounds__(256) sort_lists_kernel(const u32 *__restrict__ count, const u64 *__restrict__ offset, u32 n,
-                                                         u32 *nbr, u64 pair_cap, const u64 *__restrict__ counters)
+                                                         u32 *nbr, u64 pair_cap, u64 *counters, u32 *worklist)
 {
     if (counters[CNT_PAIRS] > pair_cap) return;
     u32 i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     u32 c = count[i];
     if (c < 2) return;
+    if (c > SORT_LIST_SERIAL) {
+        worklist[atomicAdd(&counters[CNT_EVAL_SPARE], 1ull)] = i;
+        return;
+    }
     u32 *l = nbr + offset[i];
-    for (u32 a = 1; a < c; ++a) {   // insertion sort: lists are short
+    for (u32 a = 1; a < c; ++a) {
         u32 v = l[a];
         u32 b = a;
         while (b > 0 && l[b - 1] > v) { l[b] = l[b - 1]; --b; }
         l[b] = v;
+    }
+}
+
+// one warp per long list: rank sort (entries of a list are distinct) through a scratch copy
+__global__ void __launch_bounds__(256) sort_long_lists_kernel(const u32 *__restrict__ count, const u64 *__restrict__ offset,
+                                                              u32 *nbr, u32 *scratch, const u64 *__restrict__ counters,
+                                                              const u32 *__restrict__ worklist)
+{
+    const u32 nlong = (u32)counters[CNT_EVAL_SPARE];
+    const u32 lane = threadIdx.x & 31, nwarps = gridDim.x * (blockDim.x >> 5);
+    for (u32 wk = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); wk < nlong; wk += nwarps) {
+        const u32 i = worklist[wk], c = count[i];
+        u32 *l = nbr + offset[i];
+        u32 *t = scratch + offset[i];
+        for (u32 e = lane; e < c; e += 32) t[e] = l[e];
+        __syncwarp();
+        for (u32 e = lane; e < c; e += 32) {
+            const u32 v = t[e];
+            u32 rank = 0;
+            for (u32 k = 0; k < c; ++k) rank += t[k] < v ? 1u : 0u;
+            l[rank] = v;
+        }
+        __syncwarp();
     }
 }
 
@@ -141,7 +172,11 @@ p3t_status p3t_stage_neighbours(p3t_ctx *ctx)
         P3T_CUDA(ctx, cudaMemsetAsync(w.nbr_cursor, 0, (size_t)n * sizeof(u32), s));
         u32 grid = (u32)ctx->sm_count * 4;
         fill_lists_kernel<<<grid, 256, 0, s>>>(w.pairs, (u64)ctx->nbr_capacity, w.nbr_offset, w.nbr_cursor, w.nbr, w.counters);
-        sort_lists_kernel<<<div_up(n, 256), 256, 0, s>>>(w.nbr_count, w.nbr_offset, n, w.nbr, (u64)ctx->nbr_capacity, w.counters);
+        // the scatter cursors are dead after the fill: they hold the queue of long lists; the pair buffer is the scratch copy
+        sort_lists_kernel<<<div_up(n, 256), 256, 0, s>>>(w.nbr_count, w.nbr_offset, n, w.nbr, (u64)ctx->nbr_capacity, w.counters,
+                                                         w.nbr_cursor);
+        sort_long_lists_kernel<<<(u32)ctx->sm_count * 2, 256, 0, s>>>(w.nbr_count, w.nbr_offset, w.nbr, reinterpret_cast<u32 *>(w.pairs),
+                                                                       w.counters, w.nbr_cursor);
     }
     P3T_CUDA(ctx, cudaGetLastError());
     return P3T_OK;
