@@ -18,6 +18,9 @@
  *   O6  hard acceleration (Eq. 7), its time derivative and the hard
  *       potential (Eq. 5) -- the NEXT row of SURVEY.md 8(f), pinned by
  *       tests/test_oracle_hard.py
+ *   O7  one soft step under H_hard: drift of the isolated particles, fourth-order
+ *       Hermite with block timesteps over the neighbour lists (L147, Eq. 18-20
+ *       L152-163) -- rank 2 of SURVEY.md 8(f), pinned by tests/test_oracle_hermite.py
  *
  * Readings of the paper used here (each listed in DESIGN.md section 3):
  *   A1  Eq. 17's denominator is (gamma-1)^7 (as extracted it is (1-gamma)^7,
@@ -214,6 +217,156 @@ void p3t_oracle_hard(int64_t n, const double *m, const double *q, const double *
         }
         if (pot) pot[k] = nval(&ph);
     }
+}
+
+/* ------------------------------------------------------------------ O7 -- */
+
+/*
+ * Integration of all particles over one soft step T under H_hard (procedure step 3, L147; GPU procedure steps 5-6,
+ * section 2.2): particles with an empty neighbour list drift, x += T v; the others are integrated with the
+ * fourth-order Hermite scheme with block timesteps, the force being Eq. 7 (L63) summed over the particle's neighbour
+ * list (offset/list, fixed during the step; 1 - K = 0 beyond r_out <= h so the list sum is the full hard force as long
+ * as nobody outside the list comes within r_out).  Readings (A21-A24):
+ *  - time is counted in ticks of T / 2^40; a particle's step is a power of two of ticks, at most T / 2^log2_div
+ *    (Delta t_max, L150), the largest one not above the criterion that divides the particle's current time
+ *    (block steps); never below one tick (returned in floor_hits);
+ *  - first step: Eq. 20 (L163), dt = eta_s sqrt((|a|^2 + a0^2) / |a1|^2); later steps: Eq. 18 (L152) read as
+ *    Aarseth's criterion with |a| replaced by sqrt(|a|^2 + a0^2),
+ *        dt = eta sqrt( (sqrt(|a|^2 + a0^2) |a2| + |a1|^2) / (|a1| |a3| + |a2|^2) )
+ *    (the printed denominator |a||a3| is not a time squared); a2, a3 from the Hermite interpolation, a2 taken at
+ *    the end of the step (a2 + dt a3); a vanishing denominator gives Delta t_max;
+ *  - predictor x_p = x + v dt + a dt^2/2 + a1 dt^3/6, v_p = v + a dt + a1 dt^2/2 for the active particle and for
+ *    each of its neighbours from that neighbour's own last time; corrector
+ *        a2 = (-6 (a - a_n) - dt (4 a1 + 2 a1_n)) / dt^2,  a3 = (12 (a - a_n) + 6 dt (a1 + a1_n)) / dt^3,
+ *        x = x_p + a2 dt^4/24 + a3 dt^5/120,  v = v_p + a2 dt^3/6 + a3 dt^4/24   (Makino & Aarseth 1992);
+ *  - all active particles of a block are evaluated from the state before the block, then corrected together.
+ * Sums run in list order, plain fp64.  q, v are updated in place.  nstep[i] (may be NULL) receives the number of
+ * Hermite steps of particle i.  Returns the number of blocks, or -1 when more than max_blocks would be needed (a0 = 0
+ * lets Eq. 18 collapse at the edge of the cutoff sphere, L152; q, v are then left mid-step).
+ */
+#define O7_TICK_BITS 40
+
+static void o7_force(int64_t i, const double *m, const double *xp, const double *vp,
+                     const int64_t *offset, const int32_t *list,
+                     double eps2, double r_in, double r_out, double *a, double *a1)
+{
+    const double g = r_in / r_out;
+    for (int c = 0; c < 3; ++c) a[c] = a1[c] = 0.0;
+    for (int64_t e = offset[i]; e < offset[i + 1]; ++e) {
+        int64_t j = list[e];
+        const double *xj = xp + 3 * (e - offset[i] + 1), *vj = vp + 3 * (e - offset[i] + 1);
+        double d[3], w[3];
+        for (int c = 0; c < 3; ++c) { d[c] = xp[c] - xj[c]; w[c] = vp[c] - vj[c]; }
+        double s2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2] + eps2;
+        double s = sqrt(s2);
+        if (s >= r_out) continue;
+        double K, W;
+        pair_weights(s, r_in, r_out, &K, &W);
+        double x = (s / r_out - g) / (1.0 - g);
+        double dKds = p3t_oracle_dKdx(x) / (r_out * (1.0 - g));
+        double qv = d[0] * w[0] + d[1] * w[1] + d[2] * w[2];
+        double mr3 = m[j] / (s2 * s);
+        for (int c = 0; c < 3; ++c) {
+            a[c] += -mr3 * (1.0 - K) * d[c];
+            a1[c] += -mr3 * ((1.0 - K) * (w[c] - 3.0 * qv * d[c] / s2) - dKds * (qv / s) * d[c]);
+        }
+    }
+}
+
+static double o7_norm(const double *u) { return sqrt(u[0] * u[0] + u[1] * u[1] + u[2] * u[2]); }
+
+/* largest power of two of ticks <= crit (a time), <= max_ticks, dividing t; at least one tick */
+static int64_t o7_quantise(double crit, double tick, int64_t max_ticks, int64_t t, int64_t *floor_hits)
+{
+    int64_t dt;
+    double ct = crit / tick;
+    if (!(ct < (double)max_ticks)) dt = max_ticks;          /* also NaN, inf */
+    else if (ct < 1.0) { dt = 1; if (floor_hits) ++*floor_hits; }
+    else { int e; frexp(ct, &e); dt = (int64_t)1 << (e - 1); }
+    while (t % dt) dt >>= 1;
+    return dt;
+}
+
+int64_t p3t_oracle_hermite(int64_t n, const double *m, double *q, double *v,
+                           double eps, double r_in, double r_out,
+                           const int64_t *offset, const int32_t *list,
+                           double T, int log2_div, double eta, double eta_s, double a0, int64_t max_blocks,
+                           int64_t *nstep, int64_t *floor_hits)
+{
+    const double eps2 = eps * eps;
+    const int64_t total = (int64_t)1 << O7_TICK_BITS, max_ticks = total >> log2_div;
+    const double tick = T / (double)total;
+    int64_t *t = calloc((size_t)n, sizeof *t), *dt = calloc((size_t)n, sizeof *dt);
+    double *a = calloc((size_t)3 * n, sizeof *a), *a1 = calloc((size_t)3 * n, sizeof *a1);
+    double *an = calloc((size_t)3 * n, sizeof *an), *a1n = calloc((size_t)3 * n, sizeof *a1n);
+    int64_t maxl = 0, nblocks = 0;
+    if (floor_hits) *floor_hits = 0;
+    for (int64_t i = 0; i < n; ++i) if (offset[i + 1] - offset[i] > maxl) maxl = offset[i + 1] - offset[i];
+    double *xp = malloc((size_t)3 * (maxl + 1) * sizeof *xp), *vp = malloc((size_t)3 * (maxl + 1) * sizeof *vp);
+
+    /* t = 0: forces from the current state, first steps from Eq. 20 */
+    for (int64_t i = 0; i < n; ++i) {
+        if (nstep) nstep[i] = 0;
+        if (offset[i + 1] == offset[i]) continue;
+        for (int c = 0; c < 3; ++c) { xp[c] = q[3 * i + c]; vp[c] = v[3 * i + c]; }
+        for (int64_t e = offset[i]; e < offset[i + 1]; ++e)
+            for (int c = 0; c < 3; ++c) {
+                xp[3 * (e - offset[i] + 1) + c] = q[3 * (int64_t)list[e] + c];
+                vp[3 * (e - offset[i] + 1) + c] = v[3 * (int64_t)list[e] + c];
+            }
+        o7_force(i, m, xp, vp, offset, list, eps2, r_in, r_out, a + 3 * i, a1 + 3 * i);
+        double na = o7_norm(a + 3 * i), n1 = o7_norm(a1 + 3 * i);
+        double crit = n1 > 0.0 ? eta_s * sqrt((na * na + a0 * a0) / (n1 * n1)) : INFINITY;
+        dt[i] = o7_quantise(crit, tick, max_ticks, 0, floor_hits);
+    }
+    for (;;) {
+        int64_t tn = INT64_MAX;
+        for (int64_t i = 0; i < n; ++i)
+            if (offset[i + 1] > offset[i] && t[i] < total && t[i] + dt[i] < tn) tn = t[i] + dt[i];
+        if (tn == INT64_MAX) break;
+        if (++nblocks > max_blocks) { nblocks = -1; break; }
+        /* evaluate every active particle from the state before the block */
+        for (int64_t i = 0; i < n; ++i) {
+            if (offset[i + 1] == offset[i] || t[i] + dt[i] != tn) continue;
+            for (int64_t k = 0; k <= offset[i + 1] - offset[i]; ++k) {
+                int64_t j = k ? (int64_t)list[offset[i] + k - 1] : i;
+                double h = (double)(tn - t[j]) * tick;
+                for (int c = 0; c < 3; ++c) {
+                    double A = a[3 * j + c], J = a1[3 * j + c];
+                    xp[3 * k + c] = q[3 * j + c] + h * (v[3 * j + c] + h * (A / 2.0 + h * (J / 6.0)));
+                    vp[3 * k + c] = v[3 * j + c] + h * (A + h * (J / 2.0));
+                }
+            }
+            o7_force(i, m, xp, vp, offset, list, eps2, r_in, r_out, an + 3 * i, a1n + 3 * i);
+        }
+        /* correct them together */
+        for (int64_t i = 0; i < n; ++i) {
+            if (offset[i + 1] == offset[i] || t[i] + dt[i] != tn) continue;
+            double h = (double)dt[i] * tick, a2[3], a3[3], a2e[3];
+            for (int c = 0; c < 3; ++c) {
+                double A = a[3 * i + c], J = a1[3 * i + c], An = an[3 * i + c], Jn = a1n[3 * i + c];
+                a2[c] = (-6.0 * (A - An) - h * (4.0 * J + 2.0 * Jn)) / (h * h);
+                a3[c] = (12.0 * (A - An) + 6.0 * h * (J + Jn)) / (h * h * h);
+                double x_p = q[3 * i + c] + h * (v[3 * i + c] + h * (A / 2.0 + h * (J / 6.0)));
+                double v_p = v[3 * i + c] + h * (A + h * (J / 2.0));
+                q[3 * i + c] = x_p + h * h * h * h * (a2[c] / 24.0 + h * a3[c] / 120.0);
+                v[3 * i + c] = v_p + h * h * h * (a2[c] / 6.0 + h * a3[c] / 24.0);
+                a2e[c] = a2[c] + h * a3[c];
+                a[3 * i + c] = An; a1[3 * i + c] = Jn;
+            }
+            t[i] = tn;
+            if (nstep) ++nstep[i];
+            double na = o7_norm(a + 3 * i), n1 = o7_norm(a1 + 3 * i), n2 = o7_norm(a2e), n3 = o7_norm(a3);
+            double den = n1 * n3 + n2 * n2;
+            double crit = den > 0.0 ? eta * sqrt((sqrt(na * na + a0 * a0) * n2 + n1 * n1) / den) : INFINITY;
+            dt[i] = o7_quantise(crit, tick, max_ticks, tn, floor_hits);
+        }
+    }
+    for (int64_t i = 0; i < n && nblocks >= 0; ++i)
+        if (offset[i + 1] == offset[i])
+            for (int c = 0; c < 3; ++c) q[3 * i + c] += T * v[3 * i + c];
+    free(t); free(dt); free(a); free(a1); free(an); free(a1n); free(xp); free(vp);
+    return nblocks;
 }
 
 /* ------------------------------------------------------------------ O3 -- */

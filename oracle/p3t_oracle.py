@@ -65,6 +65,8 @@ def lib():
         L.p3t_oracle_dKdx.restype = d; L.p3t_oracle_dKdx.argtypes = [d]
         L.p3t_oracle_hard.restype = None
         L.p3t_oracle_hard.argtypes = [i64, pd, pd, pd, d, d, d, i64, pi64, pd, pd, pd]
+        L.p3t_oracle_hermite.restype = i64
+        L.p3t_oracle_hermite.argtypes = [i64, pd, pd, pd, d, d, d, pi64, pi32, d, i32, d, d, d, i64, pi64, pi64]
         _lib = L
     return _lib
 
@@ -149,6 +151,42 @@ def hard(mass, pos, vel, eps, r_in, r_out, subset=None):
     lib().p3t_oracle_hard(n, _p(m, d), _p(q, d), _p(v, d), float(eps), float(r_in), float(r_out), ns,
                           _p(sub, C.c_int64), _p(a, d), _p(j, d), _p(p, d))
     return a, j, p
+
+
+# ---------------------------------------------------------------- O7 -------
+def hermite(mass, pos, vel, eps, r_in, r_out, offset, nbr, T, log2_div=2, eta=0.1, eta_s=0.01, a0=0.0,
+            max_blocks=1 << 22):
+    """One soft step T under H_hard (procedure step 3, L147): drift of the particles with empty lists, fourth-order
+    Hermite with block timesteps (Eq. 18-20) over the given neighbour lists for the others.
+    Returns (pos, vel, info) with info = dict(blocks, nstep[n], floor_hits); raises when max_blocks is exceeded."""
+    m = _f64(mass)
+    q, v = _f64(pos).reshape(-1, 3).copy(), _f64(vel).reshape(-1, 3).copy()
+    n = m.shape[0]
+    off = np.ascontiguousarray(offset, dtype=np.int64)
+    lst = np.ascontiguousarray(nbr, dtype=np.int32)
+    if lst.size == 0:
+        lst = np.zeros(1, dtype=np.int32)
+    nstep = np.zeros(n, dtype=np.int64)
+    fh = np.zeros(1, dtype=np.int64)
+    d, i64 = C.c_double, C.c_int64
+    nb = lib().p3t_oracle_hermite(n, _p(m, d), _p(q, d), _p(v, d), float(eps), float(r_in), float(r_out),
+                                  _p(off, i64), _p(lst, C.c_int32), float(T), int(log2_div), float(eta),
+                                  float(eta_s), float(a0), int(max_blocks), _p(nstep, i64), _p(fh, i64))
+    if nb < 0:
+        raise RuntimeError(f"hermite: more than {max_blocks} blocks (a0 = {a0})")
+    return q, v, dict(blocks=int(nb), nstep=nstep, floor_hits=int(fh[0]))
+
+
+def p3t_step(mass, pos, vel, acc_soft, offset, nbr, eps, r_in, r_out, h, T, log2_div=2, eta=0.1, eta_s=0.01, a0=0.0):
+    """One step of the scheme (L142-153) with the soft force by direct sum (O2) and exact lists (O3):
+    kick T/2 with acc_soft(t), hard integration over T with the lists made at t, soft force and lists at t + T,
+    kick T/2.  Returns (pos, vel, acc_soft, offset, nbr, info)."""
+    v = _f64(vel).reshape(-1, 3) + 0.5 * T * _f64(acc_soft).reshape(-1, 3)
+    q, v, info = hermite(mass, pos, v, eps, r_in, r_out, offset, nbr, T, log2_div, eta, eta_s, a0)
+    a, _ = direct(mass, q, eps, r_in, r_out)
+    off, lst, _ = neighbours(q, eps, h)
+    v = v + 0.5 * T * a
+    return q, v, a, off, lst, info
 
 
 # ---------------------------------------------------------------- O3 -------
