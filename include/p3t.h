@@ -48,7 +48,8 @@ typedef enum {
     P3T_ENOMEM    = -3,  /* workspace too small, or host allocation failed */
     P3T_ECAPACITY = -4,  /* neighbour buffer (nbr_capacity) or a caller's output buffer too small;
                             the true total is still reported by p3t_get_neighbour_counts */
-    P3T_ECUDA     = -5   /* a CUDA runtime call failed; see p3t_last_error */
+    P3T_ECUDA     = -5,  /* a CUDA runtime call failed; see p3t_last_error */
+    P3T_ELIMIT    = -6   /* the Hermite part needed more than max_blocks block steps */
 } p3t_status;
 
 /* Per-call statistics.  Interaction counts are pair evaluations for real
@@ -170,6 +171,42 @@ p3t_status p3t_get_stats(p3t_ctx *ctx, p3t_stats *out);
  * P3T_ESTATE before an eval call; P3T_ECAPACITY if the lists did not fit nbr_capacity (outputs untouched;
  * in the device form the error surfaces at the next synchronising call); P3T_EINVAL for null or non-finite vel. */
 p3t_status p3t_eval_hard(p3t_ctx *ctx, const float *vel, double *acc, double *jerk, double *pot, int on_device);
+
+/* Statistics of the Hermite part of one soft step. */
+typedef struct {
+    uint64_t n_nonisolated;  /* particles with a non-empty neighbour list (integrated by the Hermite scheme) */
+    uint64_t n_blocks;       /* block steps (distinct times at which some particle was advanced) */
+    uint64_t n_steps;        /* Hermite steps summed over particles (N_step of Eq. 21) */
+    uint64_t floor_hits;     /* times the criterion asked for less than one tick (dt_soft / 2^40) */
+    float ms;                /* device time of the Hermite part incl. the drift of the isolated particles */
+} p3t_hermite_info;
+
+/* One soft step under H_hard (the NEXT row of SURVEY.md 8(f), rank 2; procedure step 3; steps 5-6 of the
+ * GPU procedure in section 2.2, which the paper runs on the host).  pos[3n], vel[3n] (double, user order, interleaved)
+ * are advanced in place over dt_soft: particles whose list of the last evaluation is empty ("isolated") drift,
+ * pos += dt_soft vel; the others are integrated with the fourth-order Hermite scheme with block timesteps, their force
+ * being Eq. 7 (L63) over their list with the masses loaded for that evaluation, every pair in fp64.
+ *   - time runs in ticks of dt_soft / 2^40; a step is a power of two of ticks, at most dt_soft / 2^log2_div
+ *     (Delta t_max, L158), the largest not above the criterion that divides the particle's current time;
+ *   - first step: Eq. 20 (L163) with eta_s; afterwards Eq. 18 (L152) with eta, read as Aarseth's criterion with
+ *     |a| -> sqrt(|a|^2 + a0^2) (A22); a2, a3 from the Hermite interpolation;
+ *   - a0 = alpha m / r_cut^2 (Eq. 19) is the caller's to compute; with a0 = 0 the criterion collapses when a
+ *     neighbour sits at the cutoff radius and the call ends with P3T_ELIMIT after max_blocks blocks (pos, vel are
+ *     then mid-step and must be discarded).
+ * The lists must be symmetric (j in L_i <=> i in L_j), which holds for the lists this library makes.  pos and vel are
+ * both host or both device (on_device); the call synchronises either way (info is filled; may be NULL).
+ * P3T_ESTATE before an eval call; P3T_ECAPACITY if the lists did not fit nbr_capacity; P3T_EINVAL for bad arguments. */
+p3t_status p3t_hermite_step(p3t_ctx *ctx, double *pos, double *vel, double dt_soft, int log2_div, double eta, double eta_s,
+                            double a0, long long max_blocks, int on_device, p3t_hermite_info *info);
+
+/* One step of the scheme (L142-153) on a state the caller keeps in double precision: velocity kick by dt_soft / 2 with
+ * the soft acceleration of the last evaluation (step 2), p3t_hermite_step (step 3), then positions rounded to float,
+ * p3t_load_particles + p3t_build_tree + p3t_eval_soft at the new time and the second kick (step 4).  Before the first
+ * step the caller loads the float-rounded positions and calls p3t_eval_soft once; afterwards the context always holds
+ * the soft force and the lists of the current positions.  mass[n] float as in p3t_load_particles; mass, pos, vel are
+ * all host or all device.  Errors as for the calls it is made of. */
+p3t_status p3t_step(p3t_ctx *ctx, const float *mass, double *pos, double *vel, double dt_soft, int log2_div, double eta,
+                    double eta_s, double a0, long long max_blocks, int on_device, p3t_hermite_info *info);
 
 /* Wait for all enqueued work; returns deferred device-side errors. */
 p3t_status p3t_synchronize(p3t_ctx *ctx);

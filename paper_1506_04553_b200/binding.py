@@ -22,13 +22,14 @@ if not os.path.exists(_LIBPATH):
 
 _lib = C.CDLL(_LIBPATH)
 
-OK, EINVAL, ESTATE, ENOMEM, ECAPACITY, ECUDA = 0, -1, -2, -3, -4, -5
-_STATUS = {0: "P3T_OK", -1: "P3T_EINVAL", -2: "P3T_ESTATE", -3: "P3T_ENOMEM", -4: "P3T_ECAPACITY", -5: "P3T_ECUDA"}
+OK, EINVAL, ESTATE, ENOMEM, ECAPACITY, ECUDA, ELIMIT = 0, -1, -2, -3, -4, -5, -6
+_STATUS = {0: "P3T_OK", -1: "P3T_EINVAL", -2: "P3T_ESTATE", -3: "P3T_ENOMEM", -4: "P3T_ECAPACITY", -5: "P3T_ECUDA", -6: "P3T_ELIMIT"}
 
 # names of include/p3t.h's exported entry points (tests check that each resolves)
 SYMBOLS = [
     "p3t_workspace_bytes", "p3t_create", "p3t_destroy", "p3t_set_params", "p3t_set_tree_params",
     "p3t_set_group_merge_levels", "p3t_set_walk_mode", "p3t_set_shard", "p3t_load_particles", "p3t_build_tree", "p3t_eval_soft", "p3t_eval_direct", "p3t_eval_hard",
+    "p3t_hermite_step", "p3t_step",
     "p3t_get_acc_pot", "p3t_get_neighbour_counts", "p3t_get_neighbours", "p3t_get_stats", "p3t_synchronize",
     "p3t_last_error", "p3t_array_info", "p3t_copy_array", "p3t_measure_fp32_peak",
 ]
@@ -51,6 +52,14 @@ class Stats(C.Structure):
         return {k: getattr(self, k) for k, _ in self._fields_}
 
 
+class HermiteInfo(C.Structure):
+    _fields_ = [("n_nonisolated", C.c_uint64), ("n_blocks", C.c_uint64), ("n_steps", C.c_uint64),
+                ("floor_hits", C.c_uint64), ("ms", C.c_float)]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_}
+
+
 def _sig():
     vp, sz, i, f = C.c_void_p, C.c_size_t, C.c_int, C.c_float
     L = _lib
@@ -67,6 +76,9 @@ def _sig():
     L.p3t_eval_soft.restype = i; L.p3t_eval_soft.argtypes = [vp]
     L.p3t_eval_direct.restype = i; L.p3t_eval_direct.argtypes = [vp, vp, sz, i]
     L.p3t_eval_hard.restype = i; L.p3t_eval_hard.argtypes = [vp, vp, vp, vp, vp, i]
+    d, ll = C.c_double, C.c_longlong
+    L.p3t_hermite_step.restype = i; L.p3t_hermite_step.argtypes = [vp, vp, vp, d, i, d, d, d, ll, i, C.POINTER(HermiteInfo)]
+    L.p3t_step.restype = i; L.p3t_step.argtypes = [vp, vp, vp, vp, d, i, d, d, d, ll, i, C.POINTER(HermiteInfo)]
     L.p3t_get_acc_pot.restype = i; L.p3t_get_acc_pot.argtypes = [vp, vp, vp, i]
     L.p3t_get_neighbour_counts.restype = i; L.p3t_get_neighbour_counts.argtypes = [vp, vp, C.POINTER(C.c_uint64), i]
     L.p3t_get_neighbours.restype = i; L.p3t_get_neighbours.argtypes = [vp, vp, vp, sz, i]
@@ -227,6 +239,30 @@ class P3T:
         a, j, p = np.empty((self.n, 3)), np.empty((self.n, 3)), np.empty(self.n)
         self._check(_lib.p3t_eval_hard(self._h, pv, a.ctypes.data, j.ctypes.data, p.ctypes.data, 0))
         return a, j, p
+
+    def hermite_step(self, pos, vel, dt_soft, log2_div=2, eta=0.1, eta_s=0.01, a0=0.0, max_blocks=1 << 22):
+        """One soft step under H_hard over the lists of the last eval (p3t_hermite_step): pos, vel float64 [n,3], both
+        numpy (host) or both CUDA tensors, advanced IN PLACE.  Returns the statistics as a dict."""
+        pp, dp = _ptr(pos)
+        pv, dv = _ptr(vel)
+        assert dp == dv and pos.dtype == vel.dtype and str(pos.dtype).endswith("float64")
+        info = HermiteInfo()
+        self._check(_lib.p3t_hermite_step(self._h, pp, pv, float(dt_soft), int(log2_div), float(eta), float(eta_s),
+                                          float(a0), int(max_blocks), dp, C.byref(info)))
+        return info.as_dict()
+
+    def step(self, mass, pos, vel, dt_soft, log2_div=2, eta=0.1, eta_s=0.01, a0=0.0, max_blocks=1 << 22):
+        """One step of the scheme (p3t_step): kick, hard part, soft force at the new time, kick.  mass float32 [n],
+        pos, vel float64 [n,3], all numpy or all CUDA tensors; pos and vel are advanced IN PLACE."""
+        pm, dm = _ptr(mass)
+        pp, dp = _ptr(pos)
+        pv, dv = _ptr(vel)
+        assert dm == dp == dv and str(pos.dtype).endswith("float64") and str(vel.dtype).endswith("float64")
+        assert str(mass.dtype).endswith("float32")
+        info = HermiteInfo()
+        self._check(_lib.p3t_step(self._h, pm, pp, pv, float(dt_soft), int(log2_div), float(eta), float(eta_s),
+                                  float(a0), int(max_blocks), dp, C.byref(info)))
+        return info.as_dict()
 
     def get_neighbour_counts(self):
         count = np.empty(self.n, dtype=np.uint32)

@@ -1,6 +1,7 @@
 // api.cu -- the C ABI of include/p3t.h: argument checks, workspace layout, stage sequencing.
 // Every numerical step is a CUDA kernel in the other files of this directory; no CPU fallback.
 #include <math.h>
+#include <cmath>
 #include <new>
 #include <stdlib.h>
 #include <thread>
@@ -75,6 +76,10 @@ size_t p3t_layout(Workspace &ws, char *base, size_t max_n, int key_bits, size_t 
     ws.nbr_cursor = b.take<u32>(n);
     ws.subset = b.take<u32>(n);
     ws.hard_out = b.take<double>(7 * n);
+    ws.herm_ids = b.take<u32>(n);
+    ws.herm_tdt = b.take<u64>(n);
+    ws.herm_state = b.take<double>(12 * n);
+    ws.herm_ctl = b.take<u64>(8);
     ws.hist = b.take<u32>(8 * 256);            // hist | counters | order_hist are contiguous (p3t_internal.cuh)
     ws.counters = b.take<u64>(CNT_WORDS);
     ws.order_hist = b.take<u32>(2048);
@@ -139,7 +144,7 @@ extern "C" p3t_status p3t_create(p3t_ctx **out, int device, size_t max_n, int ke
     }
     ctx->base = static_cast<char *>(workspace);
     if (cudaMemsetAsync(ctx->ws.order_meta, 0, 4 * sizeof(u32), ctx->stream) != cudaSuccess) { delete ctx; return P3T_ECUDA; }
-    for (int i = 0; i < 12; ++i) {
+    for (int i = 0; i < 14; ++i) {
         if (cudaEventCreate(&ctx->ev[i]) != cudaSuccess) { delete ctx; return P3T_ECUDA; }
     }
     *out = ctx;
@@ -150,7 +155,7 @@ extern "C" p3t_status p3t_destroy(p3t_ctx *ctx)
 {
     if (!ctx) return P3T_EINVAL;
     cudaStreamSynchronize(ctx->stream);
-    for (int i = 0; i < 12; ++i)
+    for (int i = 0; i < 14; ++i)
         if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
     delete ctx;
     return P3T_OK;
@@ -401,6 +406,107 @@ extern "C" p3t_status p3t_eval_hard(p3t_ctx *ctx, const float *vel, double *acc,
     if (st != P3T_OK) return st;
     if (ctx->h_counters[CNT_PAIRS] > ctx->nbr_capacity)
         return p3t_fail(ctx, P3T_ECAPACITY, "neighbour lists exceed the context's nbr_capacity: no hard force was computed");
+    return P3T_OK;
+}
+
+// NEXT row: one soft step under H_hard, and the whole step of the scheme
+static p3t_status hermite_args_ok(p3t_ctx *ctx, double dt_soft, int log2_div, double eta, double eta_s, double a0, long long max_blocks)
+{
+    if (!(dt_soft > 0.0) || !std::isfinite(dt_soft)) return p3t_fail(ctx, P3T_EINVAL, "dt_soft must be positive and finite");
+    if (log2_div < 0 || log2_div > 30) return p3t_fail(ctx, P3T_EINVAL, "log2_div must be in 0..30");
+    if (!(eta > 0.0) || !(eta_s > 0.0) || !std::isfinite(eta) || !std::isfinite(eta_s)) return p3t_fail(ctx, P3T_EINVAL, "eta, eta_s must be positive");
+    if (!(a0 >= 0.0) || !std::isfinite(a0)) return p3t_fail(ctx, P3T_EINVAL, "a0 must be >= 0");
+    if (max_blocks < 1) return p3t_fail(ctx, P3T_EINVAL, "max_blocks must be >= 1");
+    return P3T_OK;
+}
+
+// device part shared by p3t_hermite_step and p3t_step; fills info after a synchronisation
+static p3t_status hermite_on_device(p3t_ctx *ctx, double *d_pos, double *d_vel, double dt_soft, int log2_div, double eta,
+                                    double eta_s, double a0, long long max_blocks, p3t_hermite_info *info)
+{
+    p3t_status st = sync_and_check(ctx);                  // the lists must be complete and must have fitted
+    if (st != P3T_OK) return st;
+    if (ctx->h_counters[CNT_PAIRS] > ctx->nbr_capacity)
+        return p3t_fail(ctx, P3T_ECAPACITY, "neighbour lists exceed the context's nbr_capacity: nothing was integrated");
+    u64 h_ctl[8] = {0};
+    P3T_CUDA(ctx, cudaEventRecord(ctx->ev[11], ctx->stream));
+    st = p3t_stage_hermite(ctx, d_pos, d_vel, dt_soft, log2_div, eta, eta_s, a0, max_blocks, h_ctl);
+    if (st != P3T_OK) return st;
+    P3T_CUDA(ctx, cudaEventRecord(ctx->ev[12], ctx->stream));
+    P3T_CUDA(ctx, cudaMemcpyAsync(h_ctl, ctx->ws.herm_ctl, sizeof(h_ctl), cudaMemcpyDeviceToHost, ctx->stream));
+    P3T_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    if (info) {
+        info->n_nonisolated = h_ctl[0];
+        info->n_blocks = h_ctl[4];
+        info->n_steps = h_ctl[5];
+        info->floor_hits = h_ctl[6];
+        info->ms = 0.f;
+        cudaEventElapsedTime(&info->ms, ctx->ev[11], ctx->ev[12]);
+    }
+    if (h_ctl[7]) return p3t_fail(ctx, P3T_ELIMIT, "Hermite part: more than max_blocks block steps (a0 = 0 lets Eq. 18 collapse at the cutoff radius); pos, vel are mid-step");
+    return P3T_OK;
+}
+
+extern "C" p3t_status p3t_hermite_step(p3t_ctx *ctx, double *pos, double *vel, double dt_soft, int log2_div, double eta,
+                                       double eta_s, double a0, long long max_blocks, int on_device, p3t_hermite_info *info)
+{
+    if (!ctx) return P3T_EINVAL;
+    if (!pos || !vel) return p3t_fail(ctx, P3T_EINVAL, "null pos/vel");
+    if (!ctx->evaluated) return p3t_fail(ctx, P3T_ESTATE, "p3t_hermite_step needs the neighbour lists of an eval call");
+    p3t_status st = hermite_args_ok(ctx, dt_soft, log2_div, eta, eta_s, a0, max_blocks);
+    if (st != P3T_OK) return st;
+    P3T_CUDA(ctx, cudaSetDevice(ctx->device));
+    const size_t n = ctx->n;
+    double *d_pos = pos, *d_vel = vel;
+    if (!on_device) {
+        d_pos = ctx->ws.hard_out;
+        d_vel = ctx->ws.hard_out + 3 * n;
+        P3T_CUDA(ctx, cudaMemcpyAsync(d_pos, pos, 3 * n * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
+        P3T_CUDA(ctx, cudaMemcpyAsync(d_vel, vel, 3 * n * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
+    }
+    st = hermite_on_device(ctx, d_pos, d_vel, dt_soft, log2_div, eta, eta_s, a0, max_blocks, info);
+    if (st != P3T_OK) return st;
+    if (!on_device) {
+        P3T_CUDA(ctx, cudaMemcpyAsync(pos, d_pos, 3 * n * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+        P3T_CUDA(ctx, cudaMemcpyAsync(vel, d_vel, 3 * n * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+        P3T_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    }
+    return P3T_OK;
+}
+
+extern "C" p3t_status p3t_step(p3t_ctx *ctx, const float *mass, double *pos, double *vel, double dt_soft, int log2_div,
+                               double eta, double eta_s, double a0, long long max_blocks, int on_device, p3t_hermite_info *info)
+{
+    if (!ctx) return P3T_EINVAL;
+    if (!mass || !pos || !vel) return p3t_fail(ctx, P3T_EINVAL, "null mass/pos/vel");
+    if (!ctx->evaluated) return p3t_fail(ctx, P3T_ESTATE, "p3t_step needs the soft force and lists of an eval call at the current positions");
+    p3t_status st = hermite_args_ok(ctx, dt_soft, log2_div, eta, eta_s, a0, max_blocks);
+    if (st != P3T_OK) return st;
+    P3T_CUDA(ctx, cudaSetDevice(ctx->device));
+    const size_t n = ctx->n;
+    double *d_pos = pos, *d_vel = vel;
+    const float *d_mass = mass;
+    if (!on_device) {
+        d_pos = ctx->ws.hard_out;
+        d_vel = ctx->ws.hard_out + 3 * n;
+        d_mass = ctx->ws.in_mass;
+        P3T_CUDA(ctx, cudaMemcpyAsync(d_pos, pos, 3 * n * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
+        P3T_CUDA(ctx, cudaMemcpyAsync(d_vel, vel, 3 * n * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
+        P3T_CUDA(ctx, cudaMemcpyAsync(ctx->ws.in_mass, mass, n * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
+    }
+    if ((st = p3t_stage_kick(ctx, d_vel, 0.5 * dt_soft)) != P3T_OK) return st;                 // step 2
+    st = hermite_on_device(ctx, d_pos, d_vel, dt_soft, log2_div, eta, eta_s, a0, max_blocks, info);   // step 3
+    if (st != P3T_OK) return st;
+    if ((st = p3t_stage_narrow(ctx, d_pos, ctx->ws.in_pos)) != P3T_OK) return st;              // step 4: soft force at t + dt
+    if ((st = p3t_load_particles(ctx, n, d_mass, ctx->ws.in_pos, 1)) != P3T_OK) return st;
+    if ((st = p3t_build_tree(ctx)) != P3T_OK) return st;
+    if ((st = p3t_eval_soft(ctx)) != P3T_OK) return st;
+    if ((st = p3t_stage_kick(ctx, d_vel, 0.5 * dt_soft)) != P3T_OK) return st;
+    if (!on_device) {
+        P3T_CUDA(ctx, cudaMemcpyAsync(pos, d_pos, 3 * n * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+        P3T_CUDA(ctx, cudaMemcpyAsync(vel, d_vel, 3 * n * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+        return sync_and_check(ctx);
+    }
     return P3T_OK;
 }
 

@@ -111,7 +111,11 @@ struct Workspace {
     u32 *nbr;                      // [cap]
     u32 *nbr_cursor;               // [n]
     u32 *subset;                   // [n] staging for eval_direct
-    double *hard_out;              // [7n] staging of p3t_eval_hard's host outputs (acc 3n, jerk 3n, pot n)
+    double *hard_out;              // [7n] staging of p3t_eval_hard's host outputs (acc 3n, jerk 3n, pot n); of p3t_hermite_step's pos, vel
+    u32 *herm_ids;                 // [n] slot list of the non-isolated particles (hermite.cu)
+    u64 *herm_tdt;                 // [n] t << 8 | log2 dt, in ticks
+    double *herm_state;            // [4][3 max_n] a, a1 and the block's new a, a1
+    u64 *herm_ctl;                 // [8] slot count, rotating block times, statistics
     u64 *counters;                 // [CNT_WORDS]
     u32 *walk_stack;               // [nwarps][WALK_STACK_GMEM]
     u64 *scan_tmp;                 // [nblk_scan + 1]
@@ -138,7 +142,7 @@ struct p3t_ctx {
     float eps, theta, r_in, r_out, r_search;
     Workspace ws;
     char *base;
-    cudaEvent_t ev[12];            // phase boundaries: 0 build start,1 sort end,2 build end,3 moments end,4 eval start,5 walk end,6 nbr end,7/8 hard,9/10 pack
+    cudaEvent_t ev[14];            // phase boundaries: 0 build start,1 sort end,2 build end,3 moments end,4 eval start,5 walk end,6 nbr end,7/8 hard,9/10 pack,11/12 hermite
     bool ev_build, ev_eval, ev_hard, ev_pack;
     char err[512];
     // host mirrors (valid after sync)
@@ -176,6 +180,10 @@ p3t_status p3t_stage_direct(p3t_ctx *ctx, const u32 *d_subset, size_t n_subset);
 p3t_status p3t_stage_neighbours(p3t_ctx *ctx);
 p3t_status p3t_stage_unpack(p3t_ctx *ctx, float *d_acc, float *d_pot);
 p3t_status p3t_stage_hard(p3t_ctx *ctx, const float *d_vel, double *d_acc, double *d_jerk, double *d_pot);
+p3t_status p3t_stage_hermite(p3t_ctx *ctx, double *d_pos, double *d_vel, double T, int log2_div, double eta, double eta_s,
+                             double a0, long long max_blocks, u64 *h_ctl);
+p3t_status p3t_stage_kick(p3t_ctx *ctx, double *d_vel, double dt);
+p3t_status p3t_stage_narrow(p3t_ctx *ctx, const double *d_pos, float *d_pos32);
 
 #ifdef __CUDACC__
 // ---- device helpers ----------------------------------------------------------------------------

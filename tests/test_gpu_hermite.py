@@ -1,0 +1,203 @@
+"""GPU parity of the Hermite row (include/p3t.h p3t_hermite_step, p3t_step) against oracle O7.
+
+Both sides integrate in fp64 from the same fp32-rounded inputs over the same lists (the test first checks that the
+GPU's lists ARE the oracle's), count time in the same ticks and take every step-size decision in fp64, so they walk
+through the same blocks; what separates them is the rounding of the force sums (fused multiply-adds on the GPU),
+amplified by the dynamics over one soft step.  Tolerance: 1e-9 of the particle's displacement scale for positions,
+1e-9 of the velocity scale for velocities (observed ~1e-13), block and step counts equal.  Isolated particles:
+bit-exact drift.
+"""
+import numpy as np
+import pytest
+
+from paper_1506_04553_b200 import workloads
+
+pytestmark = pytest.mark.gpu
+
+
+def _binding():
+    from paper_1506_04553_b200 import binding
+    return binding
+
+
+def _lists_equal(off, nbr, ooff, olst):
+    return np.array_equal(np.asarray(off, dtype=np.int64), ooff) and np.array_equal(np.asarray(nbr, dtype=np.int64), olst.astype(np.int64))
+
+
+def _run_pair(oracle, mass, pos, vel, eps, r_in, r_out, h, T, theta=0.4, on_device=False, **kw):
+    """GPU hermite_step and oracle.hermite on the same inputs; returns (gpu pos, vel, info, oracle pos, vel, info)."""
+    b = _binding()
+    eps, r_in, r_out, h = (float(np.float32(x)) for x in (eps, r_in, r_out, h))
+    n = len(mass)
+    m64, q64, v64 = mass.astype(np.float64), pos.astype(np.float64), vel.astype(np.float64)
+    ooff, olst, band = oracle.neighbours(q64, eps, h)
+    assert len(band) == 0, "pick another seed: a pair sits in the 1e-6 band around h"
+    with b.P3T(n, key_bits=63, nbr_capacity=max(int(ooff[-1]) + 1024, 1 << 16)) as ctx:
+        ctx.set_params(eps, theta, r_in, r_out, h)
+        ctx.soft_force(mass, pos)
+        off, nbr = ctx.get_neighbours()
+        assert _lists_equal(off, nbr, ooff, olst)
+        if on_device:
+            import torch
+            qd, vd = torch.from_numpy(q64).cuda(), torch.from_numpy(v64).cuda()
+            info = ctx.hermite_step(qd, vd, T, **kw)
+            q, v = qd.cpu().numpy(), vd.cpu().numpy()
+        else:
+            q, v = q64.copy(), v64.copy()
+            info = ctx.hermite_step(q, v, T, **kw)
+    oq, ov, oinfo = oracle.hermite(m64, q64, v64, eps, r_in, r_out, ooff, olst, T, **kw)
+    return q, v, info, oq, ov, oinfo, ooff
+
+
+def _assert_parity(q, v, info, oq, ov, oinfo, ooff, q0, v0, T):
+    iso = np.diff(ooff) == 0
+    assert info["n_nonisolated"] == int((~iso).sum())
+    assert info["n_blocks"] == oinfo["blocks"] and info["n_steps"] == int(oinfo["nstep"].sum())
+    assert info["floor_hits"] == oinfo["floor_hits"]
+    assert np.array_equal(q[iso], oq[iso]) and np.array_equal(v[iso], v0[iso])          # drift: same bits
+    scale_q = np.abs(T * v0).max()
+    scale_v = np.abs(v0).max()
+    assert np.abs(q - oq).max() <= 1e-9 * scale_q, np.abs(q - oq).max() / scale_q
+    assert np.abs(v - ov).max() <= 1e-9 * scale_v, np.abs(v - ov).max() / scale_v
+
+
+def test_two_body_orbit_inside_r_in_is_the_oracles(oracle):
+    r = 0.01
+    m = np.array([0.6, 0.4], dtype=np.float32)
+    M = 1.0
+    vrel = np.sqrt(M / r)
+    pos = np.array([[r * 0.4, 0, 0], [-r * 0.6, 0, 0]], dtype=np.float32)
+    vel = np.array([[0, vrel * 0.4, 0], [0, -vrel * 0.6, 0]], dtype=np.float32)
+    period = 2 * np.pi * np.sqrt(r ** 3 / M)
+    out = _run_pair(oracle, m, pos, vel, 0.0, 0.5, 1.0, 1.5, 0.7 * period, log2_div=2, eta=0.05, eta_s=0.005)
+    _assert_parity(*out, pos.astype(np.float64), vel.astype(np.float64), 0.7 * period)
+    q, v, info = out[:3]
+    assert info["n_steps"] > 100
+    d = np.linalg.norm(q[0] - q[1])
+    assert d == pytest.approx(np.linalg.norm(pos[0].astype(np.float64) - pos[1]), rel=1e-5)       # still on the circle
+
+
+@pytest.mark.parametrize("seed,n,on_device", [(1, 2000, False), (2, 5000, True), (3, 257, False)])
+def test_clumpy_cluster_matches_the_oracle(oracle, seed, n, on_device):
+    """Dense clumps: long lists, separations on both sides of r_in and r_out, many block levels."""
+    rng = np.random.default_rng(1000 + seed)
+    k = 8
+    centres = rng.uniform(-1, 1, (k, 3))
+    which = rng.integers(0, k, n)
+    pos = (centres[which] + 0.02 * rng.normal(size=(n, 3))).astype(np.float32)
+    vel = (0.5 * rng.normal(size=(n, 3))).astype(np.float32)
+    mass = (rng.uniform(0.5, 1.5, n) / n).astype(np.float32)
+    r_out, T = 0.01, 1.0 / 256
+    out = _run_pair(oracle, mass, pos, vel, 1e-4, 0.1 * r_out, r_out, r_out + 3 * 0.5 * T, T, on_device=on_device,
+                    log2_div=2, eta=0.1, eta_s=0.01, a0=0.1 * float(mass.mean()) / r_out ** 2)
+    _assert_parity(*out, pos.astype(np.float64), vel.astype(np.float64), T)
+    assert out[2]["n_nonisolated"] > n // 4 and out[2]["n_blocks"] >= 4
+
+
+def test_config2_full_size(oracle):
+    """BASELINE.json config 2 (64K Plummer model, dt_soft = 1/256, h = r_out + 3 sigma dt_soft) at full size."""
+    cfg = workloads.config(2)
+    T = cfg["dt_soft"]
+    out = _run_pair(oracle, cfg["mass"], cfg["pos"], cfg["vel"], cfg["eps"], cfg["r_in"], cfg["r_out"], cfg["r_search"], T,
+                    theta=cfg["theta"], log2_div=2, eta=0.1, eta_s=0.01, a0=0.1 * float(cfg["mass"][0]) / cfg["r_out"] ** 2)
+    _assert_parity(*out, cfg["pos"].astype(np.float64), cfg["vel"].astype(np.float64), T)
+    assert out[2]["n_nonisolated"] > 1000
+
+
+def test_block_limit_is_reported_and_the_context_stays_usable(oracle):
+    """a0 = 0 and a neighbour leaving the cutoff sphere: Eq. 18 collapses (L152); the call must end, not hang."""
+    b = _binding()
+    m = np.array([0.5, 0.5], dtype=np.float32)
+    pos = np.array([[0, 0, 0], [0.0099, 0, 0]], dtype=np.float32)
+    q = pos.astype(np.float64)
+    v = np.array([[0, 0, 0], [1.0, 0, 0]], dtype=np.float64)
+    with b.P3T(2, nbr_capacity=1 << 16) as ctx:
+        ctx.set_params(0.0, 0.4, 0.001, 0.01, 0.02)
+        ctx.soft_force(m, pos)
+        with pytest.raises(b.P3TError) as e:
+            ctx.hermite_step(q.copy(), v.copy(), 0.01, a0=0.0, max_blocks=2000)
+        assert e.value.status == b.ELIMIT
+        with pytest.raises(RuntimeError):
+            oracle.hermite(m.astype(np.float64), q, v, 0.0, 0.001, 0.01, np.array([0, 1, 2]), np.array([1, 0], dtype=np.int32),
+                           0.01, a0=0.0, max_blocks=2000)
+        q2, v2 = q.copy(), v.copy()
+        info = ctx.hermite_step(q2, v2, 0.01, a0=0.1 * 0.5 / 0.01 ** 2)                          # with a0 it goes through
+        assert info["n_blocks"] < 2000 and q2[1, 0] > 0.0199
+        for bad in (dict(dt_soft=0.0), dict(dt_soft=0.01, log2_div=31), dict(dt_soft=0.01, eta=0.0), dict(dt_soft=0.01, a0=-1.0),
+                    dict(dt_soft=0.01, max_blocks=0)):
+            with pytest.raises(b.P3TError) as e:
+                ctx.hermite_step(q2, v2, **bad)
+            assert e.value.status == b.EINVAL
+
+
+def test_needs_an_evaluation_first():
+    b = _binding()
+    with b.P3T(4) as ctx:
+        ctx.set_params(0.0, 0.4, 0.001, 0.01, 0.02)
+        with pytest.raises(b.P3TError) as e:
+            ctx.hermite_step(np.zeros((4, 3)), np.zeros((4, 3)), 0.01)
+        assert e.value.status == b.ESTATE
+
+
+def test_whole_step_follows_the_oracles_scheme_at_theta_zero(oracle):
+    """p3t_step against oracle.p3t_step (soft force by direct sum O2, lists O3, Hermite O7) over four steps.  The GPU's
+    soft force is fp32 (1e-5 per particle at theta = 0, north_star) and its tree sees float-rounded positions, so the
+    kicks differ at that level: tolerance 2e-5 of the velocity change per step, positions 2e-5 of the displacement."""
+    b = _binding()
+    rng = np.random.default_rng(77)
+    n = 700
+    pos = (rng.normal(size=(n, 3)) * 0.3).astype(np.float32)
+    vel = (rng.normal(size=(n, 3)) * 0.5).astype(np.float32)
+    mass = np.full(n, 1.0 / n, dtype=np.float32)
+    eps, r_out, T = (float(np.float32(x)) for x in (1e-3, 0.05, 1.0 / 128))
+    r_in, h = float(np.float32(0.1 * r_out)), float(np.float32(r_out + 3 * 0.5 * T))
+    a0 = 0.1 / n / r_out ** 2
+    m64 = mass.astype(np.float64)
+    oq, ov = pos.astype(np.float64), vel.astype(np.float64)
+    oa, _ = oracle.direct(m64, oq, eps, r_in, r_out)
+    ooff, olst, _ = oracle.neighbours(oq, eps, h)
+    q, v = oq.copy(), ov.copy()
+    with b.P3T(n, nbr_capacity=1 << 20) as ctx:
+        ctx.set_params(eps, 0.0, r_in, r_out, h)
+        ctx.soft_force(mass, pos)
+        steps = 0
+        for _ in range(4):
+            info = ctx.step(mass, q, v, T, a0=a0)
+            steps += info["n_steps"]
+            oq, ov, oa, ooff, olst, oinfo = oracle.p3t_step(m64, oq, ov, oa, ooff, olst, eps, r_in, r_out, h, T, a0=a0)
+        acc, _ = ctx.get_acc_pot()
+    assert steps > 0
+    dv = np.abs(ov - vel).max()
+    dq = np.abs(oq - pos).max()
+    assert np.abs(v - ov).max() <= 2e-5 * dv and np.abs(q - oq).max() <= 2e-5 * dq
+    an = np.linalg.norm(oa, axis=1)
+    assert (np.linalg.norm(acc - oa, axis=1) / np.maximum(an, np.median(an))).max() <= 2e-5    # force of the final state
+
+
+def test_whole_step_conserves_energy_with_the_tree(oracle):
+    """Property at the workload's theta: total energy (kinetic + plain softened Newtonian potential by direct sum, as
+    the paper measures it, L183) over 16 device-resident steps of a 4096-body Plummer model."""
+    import torch
+    b = _binding()
+    cfg = workloads.config(2, n=4096)
+    n, T = cfg["n"], cfg["dt_soft"]
+    m64 = cfg["mass"].astype(np.float64)
+
+    def energy(q, v):
+        _, p = oracle.direct(m64, q, cfg["eps"], 0.0, 0.0)         # r_out = 0: K = W = 1, the whole potential
+        return 0.5 * np.sum(m64 * (v ** 2).sum(1)) + 0.5 * np.sum(m64 * p)
+
+    q0, v0 = cfg["pos"].astype(np.float64), cfg["vel"].astype(np.float64)
+    e0 = energy(q0, v0)
+    md = torch.from_numpy(cfg["mass"]).cuda()
+    qd, vd = torch.from_numpy(q0).cuda(), torch.from_numpy(v0).cuda()
+    with b.P3T(n, nbr_capacity=1 << 20) as ctx:
+        ctx.set_params(cfg["eps"], cfg["theta"], cfg["r_in"], cfg["r_out"], cfg["r_search"])
+        ctx.soft_force(cfg["mass"], cfg["pos"])
+        total = 0
+        for _ in range(16):
+            total += ctx.step(md, qd, vd, T, a0=0.1 * float(m64[0]) / cfg["r_out"] ** 2)["n_steps"]
+        ctx.synchronize()
+    e1 = energy(qd.cpu().numpy(), vd.cpu().numpy())
+    assert total > 0
+    assert abs(e1 / e0 - 1.0) < 2e-4, e1 / e0 - 1.0
