@@ -175,9 +175,11 @@ p3t_status p3t_eval_hard(p3t_ctx *ctx, const float *vel, double *acc, double *je
 /* Statistics of the Hermite part of one soft step. */
 typedef struct {
     uint64_t n_nonisolated;  /* particles with a non-empty neighbour list (integrated by the Hermite scheme) */
-    uint64_t n_blocks;       /* block steps (distinct times at which some particle was advanced) */
+    uint64_t n_blocks;       /* block steps of the neighbour cluster that needed most (clusters keep their own block times) */
     uint64_t n_steps;        /* Hermite steps summed over particles (N_step of Eq. 21) */
     uint64_t floor_hits;     /* times the criterion asked for less than one tick (dt_soft / 2^40) */
+    uint64_t n_components;   /* neighbour clusters: connected components of the neighbour graph */
+    uint64_t max_component;  /* particles in the largest one */
     float ms;                /* device time of the Hermite part incl. the drift of the isolated particles */
 } p3t_hermite_info;
 

@@ -54,7 +54,7 @@ class Stats(C.Structure):
 
 class HermiteInfo(C.Structure):
     _fields_ = [("n_nonisolated", C.c_uint64), ("n_blocks", C.c_uint64), ("n_steps", C.c_uint64),
-                ("floor_hits", C.c_uint64), ("ms", C.c_float)]
+                ("floor_hits", C.c_uint64), ("n_components", C.c_uint64), ("max_component", C.c_uint64), ("ms", C.c_float)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}

@@ -79,7 +79,11 @@ size_t p3t_layout(Workspace &ws, char *base, size_t max_n, int key_bits, size_t 
     ws.herm_ids = b.take<u32>(n);
     ws.herm_tdt = b.take<u64>(n);
     ws.herm_state = b.take<double>(12 * n);
-    ws.herm_ctl = b.take<u64>(8);
+    ws.herm_parent = b.take<u32>(n);
+    ws.herm_csize = b.take<u32>(n);
+    ws.herm_cstart = b.take<u32>(n);
+    ws.herm_comps = b.take<uint2>(n / 2 + 1);
+    ws.herm_ctl = b.take<u64>(16);
     ws.hist = b.take<u32>(8 * 256);            // hist | counters | order_hist are contiguous (p3t_internal.cuh)
     ws.counters = b.take<u64>(CNT_WORDS);
     ws.order_hist = b.take<u32>(2048);
@@ -428,7 +432,7 @@ static p3t_status hermite_on_device(p3t_ctx *ctx, double *d_pos, double *d_vel, 
     if (st != P3T_OK) return st;
     if (ctx->h_counters[CNT_PAIRS] > ctx->nbr_capacity)
         return p3t_fail(ctx, P3T_ECAPACITY, "neighbour lists exceed the context's nbr_capacity: nothing was integrated");
-    u64 h_ctl[8] = {0};
+    u64 h_ctl[16] = {0};
     P3T_CUDA(ctx, cudaEventRecord(ctx->ev[11], ctx->stream));
     st = p3t_stage_hermite(ctx, d_pos, d_vel, dt_soft, log2_div, eta, eta_s, a0, max_blocks, h_ctl);
     if (st != P3T_OK) return st;
@@ -440,6 +444,8 @@ static p3t_status hermite_on_device(p3t_ctx *ctx, double *d_pos, double *d_vel, 
         info->n_blocks = h_ctl[4];
         info->n_steps = h_ctl[5];
         info->floor_hits = h_ctl[6];
+        info->n_components = h_ctl[11];
+        info->max_component = h_ctl[12];
         info->ms = 0.f;
         cudaEventElapsedTime(&info->ms, ctx->ev[11], ctx->ev[12]);
     }

@@ -8,13 +8,15 @@
 // with |a| -> sqrt(|a|^2 + a0^2); all active particles of a block are evaluated from the state before the block and
 // corrected together.
 //
-// Design.  The whole block loop runs inside ONE cooperative kernel: the non-isolated particles are compacted into a slot
-// list; every block each thread looks at its slots, evaluates the active ones (predicting the particle and each of
-// its neighbours from that neighbour's own time, fp64), grid barrier, corrects them and chooses the next step, grid
-// barrier.  The next block time is a 64-bit atomicMin over (t + dt) into one of three rotating words, so no host
-// round trip and no launch per block: a block costs two grid barriers.  The grid is only as large as the slot count
-// needs (a handful of particles: one CTA, the barrier is then a __syncthreads).  State is indexed by particle:
-// (t << 8 | log2 dt), a, a1, and the new a, a1 of the block.
+// Design.  During a soft step the lists are fixed, so a particle's arithmetic only involves its connected component of
+// the neighbour graph ("neighbour cluster"): block times need to be agreed on inside a component only, and the result
+// is the same as with global blocks (the oracle's locality pin P6).  The components are found on the device (lock-free
+// union-find: hook by compare-and-swap, flatten, count, lay the members out contiguously).  A component of up to 64
+// particles -- nearly all of them: pairs and triples -- is integrated by ONE WARP, its block loop synchronised by
+// __syncwarp and a shuffle minimum: no grid barrier, no launch per block, thousands of components in flight.  The
+// members of all larger components (dense cores, where the spheres percolate) go through one cooperative kernel whose
+// block loop uses two grid barriers per block and a 64-bit atomicMin over (t + dt) into rotating words.  State is
+// indexed by particle: (t << 8 | log2 dt), a, a1, and the new a, a1 of the block; everything fp64.
 #include "p3t_internal.cuh"
 #include <cooperative_groups.h>
 #include <math_constants.h>
@@ -22,7 +24,9 @@ namespace cg = cooperative_groups;
 
 #define HERM_THREADS 256
 #define HERM_TICK_BITS 40
-enum { HC_COUNT = 0, HC_TMIN0, HC_TMIN1, HC_TMIN2, HC_BLOCKS, HC_STEPS, HC_FLOOR, HC_ERR, HC_WORDS = 8 };
+#define HERM_WARP_MAX 64        // largest component one warp integrates
+enum { HC_COUNT = 0, HC_TMIN0, HC_TMIN1, HC_TMIN2, HC_BLOCKS, HC_STEPS, HC_FLOOR, HC_ERR,
+       HC_NSMALL, HC_SMALL_CURSOR, HC_BIG_CURSOR, HC_NCOMP, HC_MAXCOMP, HC_WORDS = 16 };
 
 __device__ __forceinline__ void herm_weights(const P3TParams &p, double s, double &omK, double &dKds)
 {
@@ -36,18 +40,87 @@ __device__ __forceinline__ void herm_weights(const P3TParams &p, double s, doubl
     dKds = 140.0 * u * u * u * p.inv_1mg * p.inv_rout;
 }
 
-// slot list of the particles whose list is not empty (order is irrelevant: a particle's arithmetic only involves its list)
-__global__ void herm_collect_kernel(const u64 *__restrict__ offset, u32 n, u32 *__restrict__ ids, u64 *__restrict__ ctl)
+// ---- connected components of the neighbour graph ---------------------------------------------------------------
+
+__device__ __forceinline__ u32 cc_find(volatile u32 *parent, u32 i)
+{
+    u32 p = parent[i];
+    while (p != i) {                       // path halving; pointers only ever move towards the root
+        const u32 gp = parent[p];
+        if (gp != p) parent[i] = gp;
+        i = p;
+        p = gp;
+    }
+    return i;
+}
+
+__global__ void cc_init_kernel(const u64 *__restrict__ offset, u32 n, u32 *__restrict__ parent, u32 *__restrict__ csize)
+{
+    const u32 i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n || offset[i + 1] == offset[i]) return;
+    parent[i] = i;
+    csize[i] = 0;
+}
+
+__global__ void cc_hook_kernel(const u64 *__restrict__ offset, const u32 *__restrict__ nbr, u32 n, u32 *parent)
+{
+    const u32 i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    for (u64 k = offset[i], e = offset[i + 1]; k < e; ++k) {
+        const u32 j = nbr[k];
+        if (j >= i) break;                 // lists ascend; every edge is hooked once, from its larger end
+        u32 ri = i, rj = j;
+        for (;;) {
+            ri = cc_find(parent, ri);
+            rj = cc_find(parent, rj);
+            if (ri == rj) break;
+            if (ri < rj) { const u32 t = ri; ri = rj; rj = t; }
+            if (atomicCAS(&parent[ri], ri, rj) == ri) break;       // the larger root goes under the smaller
+        }
+    }
+}
+
+__global__ void cc_count_kernel(const u64 *__restrict__ offset, u32 n, u32 *parent, u32 *csize, u64 *ctl)
 {
     const u32 i = blockIdx.x * blockDim.x + threadIdx.x;
     const bool has = i < n && offset[i + 1] > offset[i];
+    if (has) {
+        const u32 r = cc_find(parent, i);
+        parent[i] = r;
+        atomicAdd(&csize[r], 1u);
+    }
     const u32 m = __ballot_sync(0xffffffffu, has);
-    if (!m) return;
-    const u32 lane = threadIdx.x & 31;
-    u32 base = 0;
-    if (lane == 0) base = (u32)atomicAdd((unsigned long long *)&ctl[HC_COUNT], (unsigned long long)__popc(m));
-    base = __shfl_sync(0xffffffffu, base, 0);
-    if (has) ids[base + __popc(m & ((1u << lane) - 1))] = i;
+    if (m && (threadIdx.x & 31) == 0) atomicAdd((unsigned long long *)&ctl[HC_COUNT], (unsigned long long)__popc(m));
+}
+
+// member ranges: small components from the front of members[], the others from the back (HC_COUNT is final here)
+__global__ void cc_assign_kernel(const u64 *__restrict__ offset, u32 n, const u32 *__restrict__ parent, u32 *csize,
+                                 u32 *__restrict__ cstart, uint2 *__restrict__ comps, u64 *ctl)
+{
+    const u32 i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n || offset[i + 1] == offset[i] || parent[i] != i) return;
+    const u32 sz = csize[i];
+    u32 st;
+    if (sz <= HERM_WARP_MAX) {
+        st = (u32)atomicAdd((unsigned long long *)&ctl[HC_SMALL_CURSOR], (unsigned long long)sz);
+        const u32 c = (u32)atomicAdd((unsigned long long *)&ctl[HC_NSMALL], 1ull);
+        comps[c] = make_uint2(st, sz);
+    } else {
+        st = (u32)ctl[HC_COUNT] - ((u32)atomicAdd((unsigned long long *)&ctl[HC_BIG_CURSOR], (unsigned long long)sz) + sz);
+    }
+    cstart[i] = st;
+    csize[i] = 0;                          // becomes the fill cursor of the scatter
+    atomicAdd((unsigned long long *)&ctl[HC_NCOMP], 1ull);
+    atomicMax((unsigned long long *)&ctl[HC_MAXCOMP], (unsigned long long)sz);
+}
+
+__global__ void cc_scatter_kernel(const u64 *__restrict__ offset, u32 n, const u32 *__restrict__ parent, u32 *csize,
+                                  const u32 *__restrict__ cstart, u32 *__restrict__ members)
+{
+    const u32 i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n || offset[i + 1] == offset[i]) return;
+    const u32 r = parent[i];
+    members[cstart[r] + atomicAdd(&csize[r], 1u)] = i;     // order inside a component is irrelevant
 }
 
 __global__ void herm_drift_kernel(const u64 *__restrict__ offset, u32 n, double T, double *__restrict__ pos,
@@ -60,11 +133,14 @@ __global__ void herm_drift_kernel(const u64 *__restrict__ offset, u32 n, double 
         pos[3 * (size_t)i + c] = __dadd_rn(pos[3 * (size_t)i + c], __dmul_rn(T, vel[3 * (size_t)i + c]));
 }
 
+// ---- the Hermite scheme -----------------------------------------------------------------------------------------
+
 struct HermArgs {
     const float4 *body_user;       // mass in .w (the masses of the evaluation that made the lists)
     const u64 *offset;
     const u32 *nbr;
-    const u32 *ids;
+    const u32 *members;            // particles by component
+    const uint2 *comps;            // (start, size) of the components of up to HERM_WARP_MAX members
     double *pos, *vel;             // [n][3] in/out
     u64 *tdt;                      // [n] t << 8 | log2(dt)
     double *a, *a1, *an, *a1n;     // [n][3]
@@ -72,6 +148,7 @@ struct HermArgs {
     P3TParams prm;
     double tick, eta, eta_s, a0;
     u64 max_ticks, max_blocks;
+    u32 big_begin, big_count;      // members[big_begin .. big_begin + big_count): the larger components
 };
 
 // Eq. 7 and its time derivative over the list of i at time tn (ticks); the particle and its neighbours are predicted
@@ -135,110 +212,184 @@ __device__ __forceinline__ u32 herm_quantise(const HermArgs &A, double crit, u64
     return k;
 }
 
-__global__ void __launch_bounds__(HERM_THREADS) hermite_kernel(HermArgs A)
+// t = 0: force from the current state, first step from Eq. 20.  Returns the particle's first block time.
+__device__ __forceinline__ u64 herm_start(const HermArgs &A, u32 i, u32 &floor_hits)
+{
+    double a[3], a1[3];
+    herm_force(A, i, 0, true, a, a1);
+    const double na = norm3(a), n1 = norm3(a1);
+    const double crit = n1 > 0.0 ? A.eta_s * sqrt((na * na + A.a0 * A.a0) / (n1 * n1)) : CUDART_INF;
+    const u32 k = herm_quantise(A, crit, 0, floor_hits);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) { A.a[3 * (size_t)i + c] = a[c]; A.a1[3 * (size_t)i + c] = a1[c]; }   // nobody reads a, a1, tdt at t = 0
+    A.tdt[i] = k;
+    return 1ull << k;
+}
+
+// first half of a block: the new force of an active particle from the state before the block.  Returns true if active;
+// otherwise te is the particle's own next time (~0 when it has arrived at the end of the soft step).
+__device__ __forceinline__ bool herm_evaluate(const HermArgs &A, u32 i, u64 tn, u64 &te)
+{
+    const u64 total = 1ull << HERM_TICK_BITS;
+    const u64 w = A.tdt[i];
+    const u64 t = w >> 8;
+    te = t >= total ? ~0ull : t + (1ull << (w & 63));
+    if (te != tn) return false;
+    double a[3], a1[3];
+    herm_force(A, i, tn, false, a, a1);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) { A.an[3 * (size_t)i + c] = a[c]; A.a1n[3 * (size_t)i + c] = a1[c]; }
+    return true;
+}
+
+// second half: corrector and the next step (Eq. 18) of a particle that herm_evaluate found active.  Returns its next time.
+__device__ __forceinline__ u64 herm_correct(const HermArgs &A, u32 i, u64 tn, u32 &floor_hits)
+{
+    const u64 total = 1ull << HERM_TICK_BITS;
+    const u64 w = A.tdt[i];
+    const double h = (double)(1ull << (w & 63)) * A.tick;
+    double an[3], jn[3], a2e[3], a3[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const size_t o = 3 * (size_t)i + c;
+        const double Ac = A.a[o], Jc = A.a1[o], An = A.an[o], Jn = A.a1n[o];
+        const double a2 = (-6.0 * (Ac - An) - h * (4.0 * Jc + 2.0 * Jn)) / (h * h);
+        a3[c] = (12.0 * (Ac - An) + 6.0 * h * (Jc + Jn)) / (h * h * h);
+        const double X = A.pos[o], V = A.vel[o];
+        const double xp = X + h * (V + h * (Ac / 2.0 + h * (Jc / 6.0)));
+        const double vp = V + h * (Ac + h * (Jc / 2.0));
+        A.pos[o] = xp + h * h * h * h * (a2 / 24.0 + h * a3[c] / 120.0);
+        A.vel[o] = vp + h * h * h * (a2 / 6.0 + h * a3[c] / 24.0);
+        a2e[c] = a2 + h * a3[c];
+        A.a[o] = An; A.a1[o] = Jn;
+        an[c] = An; jn[c] = Jn;
+    }
+    const double na = norm3(an), n1 = norm3(jn), n2 = norm3(a2e), n3 = norm3(a3);
+    const double den = n1 * n3 + n2 * n2;
+    const double crit = den > 0.0 ? A.eta * sqrt((sqrt(na * na + A.a0 * A.a0) * n2 + n1 * n1) / den) : CUDART_INF;
+    const u32 k = herm_quantise(A, crit, tn, floor_hits);
+    A.tdt[i] = tn << 8 | k;
+    return tn < total ? tn + (1ull << k) : ~0ull;
+}
+
+__device__ __forceinline__ u64 warp_min_u64(u64 v)
+{
+#pragma unroll
+    for (int o = 16; o; o >>= 1) {
+        const u64 x = __shfl_xor_sync(0xffffffffu, v, o);
+        v = x < v ? x : v;
+    }
+    return v;
+}
+
+// one warp per component of up to HERM_WARP_MAX particles (two per lane)
+__global__ void __launch_bounds__(HERM_THREADS) hermite_warp_kernel(HermArgs A)
+{
+    const u32 wid = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    if (wid >= (u32)A.ctl[HC_NSMALL]) return;
+    const uint2 comp = A.comps[wid];
+    constexpr int PER = HERM_WARP_MAX / 32;
+    u32 mine[PER];
+    bool have[PER];
+#pragma unroll
+    for (int q = 0; q < PER; ++q) {
+        have[q] = lane + 32 * q < comp.y;
+        mine[q] = have[q] ? A.members[comp.x + lane + 32 * q] : 0u;
+    }
+    u32 floor_hits = 0, steps = 0;
+    u64 next = ~0ull;
+#pragma unroll
+    for (int q = 0; q < PER; ++q)
+        if (have[q]) next = min(next, herm_start(A, mine[q], floor_hits));
+    __syncwarp();
+    u64 tn = warp_min_u64(next);
+    u64 b = 0;
+    while (tn != ~0ull) {
+        if (b >= A.max_blocks) { if (lane == 0) A.ctl[HC_ERR] = 1; break; }
+        ++b;
+        bool act[PER];
+        u64 te[PER];
+#pragma unroll
+        for (int q = 0; q < PER; ++q) act[q] = have[q] && herm_evaluate(A, mine[q], tn, te[q]);
+        __syncwarp();
+        next = ~0ull;
+#pragma unroll
+        for (int q = 0; q < PER; ++q) {
+            if (!have[q]) continue;
+            if (act[q]) { next = min(next, herm_correct(A, mine[q], tn, floor_hits)); ++steps; }
+            else next = min(next, te[q]);
+        }
+        __syncwarp();
+        tn = warp_min_u64(next);
+    }
+    if (steps) atomicAdd((unsigned long long *)&A.ctl[HC_STEPS], (unsigned long long)steps);
+    if (floor_hits) atomicAdd((unsigned long long *)&A.ctl[HC_FLOOR], (unsigned long long)floor_hits);
+    if (lane == 0) atomicMax((unsigned long long *)&A.ctl[HC_BLOCKS], (unsigned long long)b);
+}
+
+// all larger components together: global blocks, two grid barriers per block
+__global__ void __launch_bounds__(HERM_THREADS) hermite_grid_kernel(HermArgs A)
 {
     cg::grid_group grid = cg::this_grid();
-    const u32 M = (u32)A.ctl[HC_COUNT];
+    const u32 M = A.big_count;
+    const u32 *ids = A.members + A.big_begin;
     const u32 tid = blockIdx.x * blockDim.x + threadIdx.x, stride = gridDim.x * blockDim.x;
-    const u64 total = 1ull << HERM_TICK_BITS;
     u32 floor_hits = 0, steps = 0;
-
-    // t = 0: forces from the current state, first steps from Eq. 20
     {
         u64 local_min = ~0ull;
-        for (u32 s = tid; s < M; s += stride) {
-            const u32 i = A.ids[s];
-            double a[3], a1[3];
-            herm_force(A, i, 0, true, a, a1);
-            const double na = norm3(a), n1 = norm3(a1);
-            const double crit = n1 > 0.0 ? A.eta_s * sqrt((na * na + A.a0 * A.a0) / (n1 * n1)) : CUDART_INF;
-            const u32 k = herm_quantise(A, crit, 0, floor_hits);
-#pragma unroll
-            for (int c = 0; c < 3; ++c) { A.a[3 * (size_t)i + c] = a[c]; A.a1[3 * (size_t)i + c] = a1[c]; }   // nobody reads a, a1, tdt at t = 0
-            A.tdt[i] = k;                                   // t = 0
-            local_min = min(local_min, 1ull << k);
-        }
+        for (u32 s = tid; s < M; s += stride) local_min = min(local_min, herm_start(A, ids[s], floor_hits));
         if (local_min != ~0ull) atomicMin((unsigned long long *)&A.ctl[HC_TMIN0], (unsigned long long)local_min);
     }
     grid.sync();
-
     u64 b = 0;
     for (;; ++b) {
         const u64 tn = *(volatile u64 *)&A.ctl[HC_TMIN0 + b % 3];
         if (tn == ~0ull) break;
         if (b >= A.max_blocks) { if (tid == 0) A.ctl[HC_ERR] = 1; break; }
-        u64 *next = &A.ctl[HC_TMIN0 + (b + 1) % 3];
         u64 local_min = ~0ull;
-        // evaluate the active particles from the state before the block
-        for (u32 s = tid; s < M; s += stride) {
-            const u32 i = A.ids[s];
-            const u64 w = A.tdt[i];
-            const u64 t = w >> 8, te = t + (1ull << (w & 63));
-            if (t >= total) continue;
-            if (te != tn) { local_min = min(local_min, te); continue; }
-            double a[3], a1[3];
-            herm_force(A, i, tn, false, a, a1);
-#pragma unroll
-            for (int c = 0; c < 3; ++c) { A.an[3 * (size_t)i + c] = a[c]; A.a1n[3 * (size_t)i + c] = a1[c]; }
+        for (u32 s = tid; s < M; s += stride) {            // evaluate the active particles from the state before the block
+            u64 te;
+            if (!herm_evaluate(A, ids[s], tn, te)) local_min = min(local_min, te);
         }
         grid.sync();
-        // correct them together, choose the next steps (Eq. 18)
-        for (u32 s = tid; s < M; s += stride) {
-            const u32 i = A.ids[s];
+        for (u32 s = tid; s < M; s += stride) {            // correct them together
+            const u32 i = ids[s];
             const u64 w = A.tdt[i];
-            const u64 t = w >> 8;
-            if (t >= total || t + (1ull << (w & 63)) != tn) continue;
-            const double h = (double)(1ull << (w & 63)) * A.tick;
-            double an[3], jn[3], a2e[3], a3[3];
-#pragma unroll
-            for (int c = 0; c < 3; ++c) {
-                const size_t o = 3 * (size_t)i + c;
-                const double Ac = A.a[o], Jc = A.a1[o], An = A.an[o], Jn = A.a1n[o];
-                const double a2 = (-6.0 * (Ac - An) - h * (4.0 * Jc + 2.0 * Jn)) / (h * h);
-                a3[c] = (12.0 * (Ac - An) + 6.0 * h * (Jc + Jn)) / (h * h * h);
-                const double X = A.pos[o], V = A.vel[o];
-                const double xp = X + h * (V + h * (Ac / 2.0 + h * (Jc / 6.0)));
-                const double vp = V + h * (Ac + h * (Jc / 2.0));
-                A.pos[o] = xp + h * h * h * h * (a2 / 24.0 + h * a3[c] / 120.0);
-                A.vel[o] = vp + h * h * h * (a2 / 6.0 + h * a3[c] / 24.0);
-                a2e[c] = a2 + h * a3[c];
-                A.a[o] = An; A.a1[o] = Jn;
-                an[c] = An; jn[c] = Jn;
-            }
+            if ((w >> 8) + (1ull << (w & 63)) != tn || (w >> 8) >= (1ull << HERM_TICK_BITS)) continue;
+            local_min = min(local_min, herm_correct(A, i, tn, floor_hits));
             ++steps;
-            const double na = norm3(an), n1 = norm3(jn), n2 = norm3(a2e), n3 = norm3(a3);
-            const double den = n1 * n3 + n2 * n2;
-            const double crit = den > 0.0 ? A.eta * sqrt((sqrt(na * na + A.a0 * A.a0) * n2 + n1 * n1) / den) : CUDART_INF;
-            const u32 k = herm_quantise(A, crit, tn, floor_hits);
-            A.tdt[i] = tn << 8 | k;
-            if (tn < total) local_min = min(local_min, tn + (1ull << k));
         }
-        if (local_min != ~0ull) atomicMin((unsigned long long *)next, (unsigned long long)local_min);
+        if (local_min != ~0ull) atomicMin((unsigned long long *)&A.ctl[HC_TMIN0 + (b + 1) % 3], (unsigned long long)local_min);
         if (tid == 0) A.ctl[HC_TMIN0 + (b + 2) % 3] = ~0ull;
         grid.sync();
     }
     if (steps) atomicAdd((unsigned long long *)&A.ctl[HC_STEPS], (unsigned long long)steps);
     if (floor_hits) atomicAdd((unsigned long long *)&A.ctl[HC_FLOOR], (unsigned long long)floor_hits);
-    if (tid == 0) A.ctl[HC_BLOCKS] = b;
+    if (tid == 0) atomicMax((unsigned long long *)&A.ctl[HC_BLOCKS], (unsigned long long)b);
 }
 
-// Enqueues the collection, reads the slot count back (one synchronisation: the grid is sized by it), then the block
-// loop and the drift.  d_pos, d_vel: device [n][3] doubles, updated in place.
+// Enqueues the component search, reads the counts back (one synchronisation: the grids are sized by them), then the two
+// integration kernels and the drift.  d_pos, d_vel: device [n][3] doubles, updated in place.  h_ctl[HC_WORDS].
 p3t_status p3t_stage_hermite(p3t_ctx *ctx, double *d_pos, double *d_vel, double T, int log2_div, double eta, double eta_s,
                              double a0, long long max_blocks, u64 *h_ctl)
 {
     Workspace &w = ctx->ws;
     const u32 n = (u32)ctx->n;
+    const u32 g = div_up(n, 256);
     P3T_CUDA(ctx, cudaMemsetAsync(w.herm_ctl, 0, HC_WORDS * sizeof(u64), ctx->stream));
     P3T_CUDA(ctx, cudaMemsetAsync(w.herm_ctl + HC_TMIN0, 0xff, 3 * sizeof(u64), ctx->stream));
-    herm_collect_kernel<<<div_up(n, 256), 256, 0, ctx->stream>>>(w.nbr_offset, n, w.herm_ids, w.herm_ctl);
+    cc_init_kernel<<<g, 256, 0, ctx->stream>>>(w.nbr_offset, n, w.herm_parent, w.herm_csize);
+    cc_hook_kernel<<<g, 256, 0, ctx->stream>>>(w.nbr_offset, w.nbr, n, w.herm_parent);
+    cc_count_kernel<<<g, 256, 0, ctx->stream>>>(w.nbr_offset, n, w.herm_parent, w.herm_csize, w.herm_ctl);
+    cc_assign_kernel<<<g, 256, 0, ctx->stream>>>(w.nbr_offset, n, w.herm_parent, w.herm_csize, w.herm_cstart, w.herm_comps, w.herm_ctl);
+    cc_scatter_kernel<<<g, 256, 0, ctx->stream>>>(w.nbr_offset, n, w.herm_parent, w.herm_csize, w.herm_cstart, w.herm_ids);
     P3T_CUDA(ctx, cudaGetLastError());
-    P3T_CUDA(ctx, cudaMemcpyAsync(h_ctl, w.herm_ctl, sizeof(u64), cudaMemcpyDeviceToHost, ctx->stream));
+    P3T_CUDA(ctx, cudaMemcpyAsync(h_ctl, w.herm_ctl, HC_WORDS * sizeof(u64), cudaMemcpyDeviceToHost, ctx->stream));
     P3T_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
-    const u64 M = h_ctl[HC_COUNT];
+    const u64 M = h_ctl[HC_COUNT], nsmall = h_ctl[HC_NSMALL], nbig = h_ctl[HC_BIG_CURSOR];
     if (M) {
         HermArgs A;
-        A.body_user = w.body_user; A.offset = w.nbr_offset; A.nbr = w.nbr; A.ids = w.herm_ids;
+        A.body_user = w.body_user; A.offset = w.nbr_offset; A.nbr = w.nbr; A.members = w.herm_ids; A.comps = w.herm_comps;
         A.pos = d_pos; A.vel = d_vel;
         A.tdt = w.herm_tdt; A.a = w.herm_state; A.a1 = w.herm_state + 3 * (size_t)ctx->max_n;
         A.an = w.herm_state + 6 * (size_t)ctx->max_n; A.a1n = w.herm_state + 9 * (size_t)ctx->max_n;
@@ -248,15 +399,22 @@ p3t_status p3t_stage_hermite(p3t_ctx *ctx, double *d_pos, double *d_vel, double 
         A.eta = eta; A.eta_s = eta_s; A.a0 = a0;
         A.max_ticks = (1ull << HERM_TICK_BITS) >> log2_div;
         A.max_blocks = (u64)max_blocks;
-        int per_sm = 0;
-        P3T_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, hermite_kernel, HERM_THREADS, 0));
-        if (per_sm < 1) return p3t_fail(ctx, P3T_ECUDA, "hermite_kernel does not fit an SM");
-        u32 grid = (u32)((M + HERM_THREADS - 1) / HERM_THREADS);
-        if (grid > (u32)ctx->sm_count) grid = (u32)ctx->sm_count;       // one CTA per SM: the barrier is the cost of a block
-        void *args[] = {&A};
-        P3T_CUDA(ctx, cudaLaunchCooperativeKernel((void *)hermite_kernel, dim3(grid), dim3(HERM_THREADS), args, 0, ctx->stream));
+        A.big_begin = (u32)(M - nbig); A.big_count = (u32)nbig;
+        if (nsmall) {
+            hermite_warp_kernel<<<div_up(nsmall * 32, HERM_THREADS), HERM_THREADS, 0, ctx->stream>>>(A);
+            P3T_CUDA(ctx, cudaGetLastError());
+        }
+        if (nbig) {
+            int per_sm = 0;
+            P3T_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, hermite_grid_kernel, HERM_THREADS, 0));
+            if (per_sm < 1) return p3t_fail(ctx, P3T_ECUDA, "hermite_grid_kernel does not fit an SM");
+            u32 grid = (u32)((nbig + HERM_THREADS - 1) / HERM_THREADS);
+            if (grid > (u32)ctx->sm_count) grid = (u32)ctx->sm_count;   // one CTA per SM: the barrier is the cost of a block
+            void *args[] = {&A};
+            P3T_CUDA(ctx, cudaLaunchCooperativeKernel((void *)hermite_grid_kernel, dim3(grid), dim3(HERM_THREADS), args, 0, ctx->stream));
+        }
     }
-    herm_drift_kernel<<<div_up(n, 256), 256, 0, ctx->stream>>>(w.nbr_offset, n, T, d_pos, d_vel);
+    herm_drift_kernel<<<g, 256, 0, ctx->stream>>>(w.nbr_offset, n, T, d_pos, d_vel);
     P3T_CUDA(ctx, cudaGetLastError());
     return P3T_OK;
 }
