@@ -277,6 +277,31 @@ def main():
         hard = {"kernel": "hard_kernel (p3t_eval_hard: acceleration, jerk, potential over the neighbour lists, fp64)", "ms": ms_h,
                 "pairs": st["n_neighbours"], "bound": "hbm", "algorithmic_bytes": hb, "achieved": hb / (ms_h * 1e-3) / 1e9, "unit": "GB/s"}
 
+    # ---- NEXT row (rank 2), outside the timed region: whole steps of the scheme on a device-resident fp64 state
+    # (kick, Hermite part by neighbour cluster / drift, soft force at the new time, kick; p3t_step)
+    whole = None
+    if rank == 0 and not shard:
+        dt_soft = cfg.get("dt_soft") or 1.0 / 1024.0
+        a0 = 0.1 * float(cfg["mass"].mean()) / cfg["r_out"] ** 2           # Eq. 19, alpha = 0.1 (L160)
+        q64 = torch.from_numpy(cfg["pos"].astype(np.float64)).to(dev)
+        v64 = torch.from_numpy(cfg["vel"].astype(np.float64)).to(dev)
+        ctx.load_particles(mass_d, torch.from_numpy(cfg["pos"]).to(dev)); ctx.build_tree(); ctx.eval_soft()
+        tw, infos = [], []
+        for _ in range(6):
+            flush.zero_()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            infos.append(ctx.step(mass_d, q64, v64, dt_soft, log2_div=2, eta=0.1, eta_s=0.01, a0=a0))
+            e1.record()
+            torch.cuda.synchronize()
+            tw.append(e0.elapsed_time(e1))
+        ms_w = float(np.median(tw[1:]))
+        last = infos[-1]
+        whole = {"call": "p3t_step (device-resident fp64 state)", "dt_soft": dt_soft, "ms_per_step": ms_w,
+                 "particles_per_s": n / (ms_w * 1e-3), "ms_hermite": float(np.median([i["ms"] for i in infos[1:]])),
+                 "nonisolated": last["n_nonisolated"], "hermite_steps": last["n_steps"], "clusters": last["n_components"],
+                 "largest_cluster": last["max_component"], "blocks_of_busiest_cluster": last["n_blocks"]}
+
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
     e2e = None
     if not args.no_e2e:
@@ -359,6 +384,8 @@ def main():
     if hard:
         hard["peak"] = peaks["hbm_gbs"]; hard["frac"] = hard["achieved"] / peaks["hbm_gbs"]
         out["next_rows"] = {"hard_force": hard}
+        if whole:
+            out["next_rows"]["p3t_step"] = whole
     if e2e:
         out["e2e"] = e2e
     if not args.no_cpu_baseline and world == 1:

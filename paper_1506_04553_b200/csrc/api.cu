@@ -449,6 +449,7 @@ static p3t_status hermite_on_device(p3t_ctx *ctx, double *d_pos, double *d_vel, 
         info->ms = 0.f;
         cudaEventElapsedTime(&info->ms, ctx->ev[11], ctx->ev[12]);
     }
+    if (h_ctl[7] == 2) return p3t_fail(ctx, P3T_ESTATE, "Hermite part: the neighbour lists are not symmetric; pos, vel are unusable");
     if (h_ctl[7]) return p3t_fail(ctx, P3T_ELIMIT, "Hermite part: more than max_blocks block steps (a0 = 0 lets Eq. 18 collapse at the cutoff radius); pos, vel are mid-step");
     return P3T_OK;
 }

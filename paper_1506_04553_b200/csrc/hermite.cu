@@ -15,8 +15,9 @@
 // particles -- nearly all of them: pairs and triples -- is integrated by ONE WARP, its block loop synchronised by
 // __syncwarp and a shuffle minimum: no grid barrier, no launch per block, thousands of components in flight.  The
 // members of all larger components (dense cores, where the spheres percolate) go through one cooperative kernel whose
-// block loop uses two grid barriers per block and a 64-bit atomicMin over (t + dt) into rotating words.  State is
-// indexed by particle: (t << 8 | log2 dt), a, a1, and the new a, a1 of the block; everything fp64.
+// block loop uses two grid barriers per block and a 64-bit atomicMin over (t + dt) into rotating words.  A warp keeps
+// its component's state ((t << 8 | log2 dt), x, v, a, a1 and the block's new a, a1) in shared memory, the grid kernel in
+// global arrays indexed by particle; everything fp64.
 #include "p3t_internal.cuh"
 #include <cooperative_groups.h>
 #include <math_constants.h>
@@ -135,58 +136,79 @@ __global__ void herm_drift_kernel(const u64 *__restrict__ offset, u32 n, double 
 
 // ---- the Hermite scheme -----------------------------------------------------------------------------------------
 
+// (constant divisors are multiplied by their rounded reciprocals: the block loop of a cluster is one dependent chain of
+// fp64 operations, a division costs ~30 of them; the oracle divides, the difference is an ulp per operation)
+constexpr double kSixth = 1.0 / 6.0;
+
+struct HermConst {
+    P3TParams prm;
+    double tick, rtick, eta, eta_s, a0;
+    u64 max_ticks, max_blocks;
+};
+
+// Where a set of particles keeps its state.  Global view: arrays indexed by particle id, lists hold particle ids, masses
+// come from body_user.  Local view (one warp's component): arrays in shared memory indexed by the member's slot, lists
+// hold slots, masses in `mass`.
+struct HermView {
+    double *pos, *vel;             // [.][3]
+    double *a, *a1, *an, *a1n;     // [.][3]
+    u64 *tdt;                      // t << 8 | log2(dt)
+    const u32 *nbr;                // list entries
+    const float4 *body_user;       // global view: mass in .w (the masses of the evaluation that made the lists)
+    const double *mass;            // local view
+};
+
 struct HermArgs {
-    const float4 *body_user;       // mass in .w (the masses of the evaluation that made the lists)
+    HermConst C;
+    HermView G;                    // the global view
     const u64 *offset;
-    const u32 *nbr;
     const u32 *members;            // particles by component
     const uint2 *comps;            // (start, size) of the components of up to HERM_WARP_MAX members
-    double *pos, *vel;             // [n][3] in/out
-    u64 *tdt;                      // [n] t << 8 | log2(dt)
-    double *a, *a1, *an, *a1n;     // [n][3]
+    u32 *lnbr;                     // [capacity] list entries as slots of the particle's component (warp kernel)
     u64 *ctl;
-    P3TParams prm;
-    double tick, eta, eta_s, a0;
-    u64 max_ticks, max_blocks;
     u32 big_begin, big_count;      // members[big_begin .. big_begin + big_count): the larger components
 };
 
-// Eq. 7 and its time derivative over the list of i at time tn (ticks); the particle and its neighbours are predicted
-// from their own last times.  first: t = 0, nothing to predict.
-__device__ __forceinline__ void herm_force(const HermArgs &A, u32 i, u64 tn, bool first, double *a, double *a1)
+// Eq. 7 and its time derivative over the list [k0, k1) of i at time tn (ticks); the particle and its neighbours are
+// predicted from their own last times.  first: t = 0, nothing to predict.
+template <bool LOCAL>
+__device__ __forceinline__ void herm_force(const HermConst &C, const HermView &V, u32 i, u64 k0, u64 k1, u64 tn, bool first,
+                                           double *a, double *a1)
 {
     double xi[3], vi[3];
     {
-        const double h = first ? 0.0 : (double)(tn - (A.tdt[i] >> 8)) * A.tick;
+        const double h = first ? 0.0 : (double)(tn - (V.tdt[i] >> 8)) * C.tick;
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
-            const double X = A.pos[3 * (size_t)i + c], V = A.vel[3 * (size_t)i + c];
-            const double Ac = first ? 0.0 : A.a[3 * (size_t)i + c], Jc = first ? 0.0 : A.a1[3 * (size_t)i + c];
-            xi[c] = X + h * (V + h * (Ac / 2.0 + h * (Jc / 6.0)));
-            vi[c] = V + h * (Ac + h * (Jc / 2.0));
+            const double X = V.pos[3 * (size_t)i + c], Vc = V.vel[3 * (size_t)i + c];
+            const double Ac = first ? 0.0 : V.a[3 * (size_t)i + c], Jc = first ? 0.0 : V.a1[3 * (size_t)i + c];
+            xi[c] = X + h * (Vc + h * (Ac * 0.5 + h * (Jc * kSixth)));
+            vi[c] = Vc + h * (Ac + h * (Jc * 0.5));
         }
     }
-    const double eps2 = A.prm.eps2_d;
+    const double eps2 = C.prm.eps2_d;
     double ax = 0, ay = 0, az = 0, jx = 0, jy = 0, jz = 0;
-    for (u64 k = A.offset[i], e = A.offset[i + 1]; k < e; ++k) {
-        const u32 j = A.nbr[k];
-        const double h = first ? 0.0 : (double)(tn - (A.tdt[j] >> 8)) * A.tick;
+    for (u64 k = k0; k < k1; ++k) {
+        const u32 j = V.nbr[k];
+        const double h = first ? 0.0 : (double)(tn - (V.tdt[j] >> 8)) * C.tick;
         double d[3], w[3];
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
-            const double X = A.pos[3 * (size_t)j + c], V = A.vel[3 * (size_t)j + c];
-            const double Ac = first ? 0.0 : A.a[3 * (size_t)j + c], Jc = first ? 0.0 : A.a1[3 * (size_t)j + c];
-            d[c] = xi[c] - (X + h * (V + h * (Ac / 2.0 + h * (Jc / 6.0))));
-            w[c] = vi[c] - (V + h * (Ac + h * (Jc / 2.0)));
+            const double X = V.pos[3 * (size_t)j + c], Vc = V.vel[3 * (size_t)j + c];
+            const double Ac = first ? 0.0 : V.a[3 * (size_t)j + c], Jc = first ? 0.0 : V.a1[3 * (size_t)j + c];
+            d[c] = xi[c] - (X + h * (Vc + h * (Ac * 0.5 + h * (Jc * kSixth))));
+            w[c] = vi[c] - (Vc + h * (Ac + h * (Jc * 0.5)));
         }
         const double s2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2] + eps2;
         const double s = sqrt(s2);
         double omK, dKds;
-        herm_weights(A.prm, s, omK, dKds);
+        herm_weights(C.prm, s, omK, dKds);
         if (omK == 0.0 && dKds == 0.0) continue;
         const double qv = d[0] * w[0] + d[1] * w[1] + d[2] * w[2];
-        const double mr3 = (double)A.body_user[j].w / (s2 * s);
-        const double c1 = mr3 * omK, c2 = mr3 * (3.0 * omK * qv / s2 + dKds * qv / s);
+        const double mj = LOCAL ? V.mass[j] : (double)V.body_user[j].w;
+        const double rs2 = 1.0 / s2, rs = s * rs2;          // one division per pair; the block loop is a latency chain
+        const double mr3 = mj * rs2 * rs;
+        const double c1 = mr3 * omK, c2 = mr3 * qv * (3.0 * omK * rs2 + dKds * rs);
         ax -= c1 * d[0]; ay -= c1 * d[1]; az -= c1 * d[2];
         jx -= c1 * w[0] - c2 * d[0]; jy -= c1 * w[1] - c2 * d[1]; jz -= c1 * w[2] - c2 * d[2];
     }
@@ -197,12 +219,12 @@ __device__ __forceinline__ void herm_force(const HermArgs &A, u32 i, u64 tn, boo
 __device__ __forceinline__ double norm3(const double *u) { return sqrt(u[0] * u[0] + u[1] * u[1] + u[2] * u[2]); }
 
 // log2 of the largest power of two of ticks <= crit (a time), <= max_ticks, dividing t; at least one tick
-__device__ __forceinline__ u32 herm_quantise(const HermArgs &A, double crit, u64 t, u32 &floor_hits)
+__device__ __forceinline__ u32 herm_quantise(const HermConst &C, double crit, u64 t, u32 &floor_hits)
 {
-    const double ct = crit / A.tick;
+    const double ct = crit * C.rtick;
     u32 k;
-    const u32 kmax = 63 - __clzll((long long)A.max_ticks);
-    if (!(ct < (double)A.max_ticks)) k = kmax;
+    const u32 kmax = 63 - __clzll((long long)C.max_ticks);
+    if (!(ct < (double)C.max_ticks)) k = kmax;
     else if (ct < 1.0) { k = 0; ++floor_hits; }
     else k = (u32)((__double2hiint(ct) >> 20) & 0x7ff) - 1023u;
     if (t) {
@@ -213,62 +235,65 @@ __device__ __forceinline__ u32 herm_quantise(const HermArgs &A, double crit, u64
 }
 
 // t = 0: force from the current state, first step from Eq. 20.  Returns the particle's first block time.
-__device__ __forceinline__ u64 herm_start(const HermArgs &A, u32 i, u32 &floor_hits)
+template <bool LOCAL>
+__device__ __forceinline__ u64 herm_start(const HermConst &C, const HermView &V, u32 i, u64 k0, u64 k1, u32 &floor_hits)
 {
     double a[3], a1[3];
-    herm_force(A, i, 0, true, a, a1);
+    herm_force<LOCAL>(C, V, i, k0, k1, 0, true, a, a1);
     const double na = norm3(a), n1 = norm3(a1);
-    const double crit = n1 > 0.0 ? A.eta_s * sqrt((na * na + A.a0 * A.a0) / (n1 * n1)) : CUDART_INF;
-    const u32 k = herm_quantise(A, crit, 0, floor_hits);
+    const double crit = n1 > 0.0 ? C.eta_s * sqrt((na * na + C.a0 * C.a0) / (n1 * n1)) : CUDART_INF;
+    const u32 k = herm_quantise(C, crit, 0, floor_hits);
 #pragma unroll
-    for (int c = 0; c < 3; ++c) { A.a[3 * (size_t)i + c] = a[c]; A.a1[3 * (size_t)i + c] = a1[c]; }   // nobody reads a, a1, tdt at t = 0
-    A.tdt[i] = k;
+    for (int c = 0; c < 3; ++c) { V.a[3 * (size_t)i + c] = a[c]; V.a1[3 * (size_t)i + c] = a1[c]; }   // nobody reads a, a1, tdt at t = 0
+    V.tdt[i] = k;
     return 1ull << k;
 }
 
 // first half of a block: the new force of an active particle from the state before the block.  Returns true if active;
 // otherwise te is the particle's own next time (~0 when it has arrived at the end of the soft step).
-__device__ __forceinline__ bool herm_evaluate(const HermArgs &A, u32 i, u64 tn, u64 &te)
+template <bool LOCAL>
+__device__ __forceinline__ bool herm_evaluate(const HermConst &C, const HermView &V, u32 i, u64 k0, u64 k1, u64 tn, u64 &te)
 {
     const u64 total = 1ull << HERM_TICK_BITS;
-    const u64 w = A.tdt[i];
+    const u64 w = V.tdt[i];
     const u64 t = w >> 8;
     te = t >= total ? ~0ull : t + (1ull << (w & 63));
     if (te != tn) return false;
     double a[3], a1[3];
-    herm_force(A, i, tn, false, a, a1);
+    herm_force<LOCAL>(C, V, i, k0, k1, tn, false, a, a1);
 #pragma unroll
-    for (int c = 0; c < 3; ++c) { A.an[3 * (size_t)i + c] = a[c]; A.a1n[3 * (size_t)i + c] = a1[c]; }
+    for (int c = 0; c < 3; ++c) { V.an[3 * (size_t)i + c] = a[c]; V.a1n[3 * (size_t)i + c] = a1[c]; }
     return true;
 }
 
 // second half: corrector and the next step (Eq. 18) of a particle that herm_evaluate found active.  Returns its next time.
-__device__ __forceinline__ u64 herm_correct(const HermArgs &A, u32 i, u64 tn, u32 &floor_hits)
+__device__ __forceinline__ u64 herm_correct(const HermConst &C, const HermView &V, u32 i, u64 tn, u32 &floor_hits)
 {
     const u64 total = 1ull << HERM_TICK_BITS;
-    const u64 w = A.tdt[i];
-    const double h = (double)(1ull << (w & 63)) * A.tick;
+    const u64 w = V.tdt[i];
+    const double h = (double)(1ull << (w & 63)) * C.tick;
+    const double rh = 1.0 / h, rh2 = rh * rh, rh3 = rh2 * rh;
     double an[3], jn[3], a2e[3], a3[3];
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
         const size_t o = 3 * (size_t)i + c;
-        const double Ac = A.a[o], Jc = A.a1[o], An = A.an[o], Jn = A.a1n[o];
-        const double a2 = (-6.0 * (Ac - An) - h * (4.0 * Jc + 2.0 * Jn)) / (h * h);
-        a3[c] = (12.0 * (Ac - An) + 6.0 * h * (Jc + Jn)) / (h * h * h);
-        const double X = A.pos[o], V = A.vel[o];
-        const double xp = X + h * (V + h * (Ac / 2.0 + h * (Jc / 6.0)));
-        const double vp = V + h * (Ac + h * (Jc / 2.0));
-        A.pos[o] = xp + h * h * h * h * (a2 / 24.0 + h * a3[c] / 120.0);
-        A.vel[o] = vp + h * h * h * (a2 / 6.0 + h * a3[c] / 24.0);
+        const double Ac = V.a[o], Jc = V.a1[o], An = V.an[o], Jn = V.a1n[o];
+        const double a2 = (-6.0 * (Ac - An) - h * (4.0 * Jc + 2.0 * Jn)) * rh2;
+        a3[c] = (12.0 * (Ac - An) + 6.0 * h * (Jc + Jn)) * rh3;
+        const double X = V.pos[o], Vc = V.vel[o];
+        const double xp = X + h * (Vc + h * (Ac * 0.5 + h * (Jc * kSixth)));
+        const double vp = Vc + h * (Ac + h * (Jc * 0.5));
+        V.pos[o] = xp + h * h * h * h * (a2 * (1.0 / 24.0) + h * a3[c] * (1.0 / 120.0));
+        V.vel[o] = vp + h * h * h * (a2 * kSixth + h * a3[c] * (1.0 / 24.0));
         a2e[c] = a2 + h * a3[c];
-        A.a[o] = An; A.a1[o] = Jn;
+        V.a[o] = An; V.a1[o] = Jn;
         an[c] = An; jn[c] = Jn;
     }
     const double na = norm3(an), n1 = norm3(jn), n2 = norm3(a2e), n3 = norm3(a3);
     const double den = n1 * n3 + n2 * n2;
-    const double crit = den > 0.0 ? A.eta * sqrt((sqrt(na * na + A.a0 * A.a0) * n2 + n1 * n1) / den) : CUDART_INF;
-    const u32 k = herm_quantise(A, crit, tn, floor_hits);
-    A.tdt[i] = tn << 8 | k;
+    const double crit = den > 0.0 ? C.eta * sqrt((sqrt(na * na + C.a0 * C.a0) * n2 + n1 * n1) / den) : CUDART_INF;
+    const u32 k = herm_quantise(C, crit, tn, floor_hits);
+    V.tdt[i] = tn << 8 | k;
     return tn < total ? tn + (1ull << k) : ~0ull;
 }
 
@@ -282,46 +307,97 @@ __device__ __forceinline__ u64 warp_min_u64(u64 v)
     return v;
 }
 
-// one warp per component of up to HERM_WARP_MAX particles (two per lane)
-__global__ void __launch_bounds__(HERM_THREADS) hermite_warp_kernel(HermArgs A)
+// One warp per component of up to HERM_WARP_MAX particles (two per lane).  The component's whole state lives in shared
+// memory for the duration of the soft step (a block then costs shared-memory latencies, not L2 round trips); the lists
+// are rewritten once as slots of the component.
+#define HERM_WARPS 4
+struct WarpState {
+    double pos[3 * HERM_WARP_MAX], vel[3 * HERM_WARP_MAX];
+    double a[3 * HERM_WARP_MAX], a1[3 * HERM_WARP_MAX], an[3 * HERM_WARP_MAX], a1n[3 * HERM_WARP_MAX];
+    u64 tdt[HERM_WARP_MAX];
+    double mass[HERM_WARP_MAX];
+    u32 gid[HERM_WARP_MAX];
+};
+
+__global__ void __launch_bounds__(32 * HERM_WARPS) hermite_warp_kernel(HermArgs A)
 {
+    __shared__ WarpState sm_all[HERM_WARPS];
     const u32 wid = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (wid >= (u32)A.ctl[HC_NSMALL]) return;
+    WarpState &S = sm_all[threadIdx.x >> 5];
     const uint2 comp = A.comps[wid];
     constexpr int PER = HERM_WARP_MAX / 32;
-    u32 mine[PER];
+    u32 slot[PER];
+    u64 k0[PER], k1[PER];
     bool have[PER];
 #pragma unroll
     for (int q = 0; q < PER; ++q) {
-        have[q] = lane + 32 * q < comp.y;
-        mine[q] = have[q] ? A.members[comp.x + lane + 32 * q] : 0u;
+        slot[q] = lane + 32 * q;
+        have[q] = slot[q] < comp.y;
+        k0[q] = k1[q] = 0;
+        if (have[q]) {
+            const u32 g = A.members[comp.x + slot[q]];
+            S.gid[slot[q]] = g;
+            k0[q] = A.offset[g]; k1[q] = A.offset[g + 1];
+            S.mass[slot[q]] = (double)A.G.body_user[g].w;
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                S.pos[3 * slot[q] + c] = A.G.pos[3 * (size_t)g + c];
+                S.vel[3 * slot[q] + c] = A.G.vel[3 * (size_t)g + c];
+            }
+        }
     }
+    __syncwarp();
+#pragma unroll
+    for (int q = 0; q < PER; ++q)
+        for (u64 k = k0[q]; k < k1[q]; ++k) {             // list entries -> slots (every neighbour is a member)
+            const u32 g = A.G.nbr[k];
+            u32 sidx = 0;
+            while (sidx < comp.y && S.gid[sidx] != g) ++sidx;
+            if (sidx == comp.y) { A.ctl[HC_ERR] = 2; sidx = slot[q]; }   // a list that is not symmetric: reported, result unusable
+            A.lnbr[k] = sidx;
+        }
+    HermView V;
+    V.pos = S.pos; V.vel = S.vel; V.a = S.a; V.a1 = S.a1; V.an = S.an; V.a1n = S.a1n; V.tdt = S.tdt;
+    V.nbr = A.lnbr; V.body_user = nullptr; V.mass = S.mass;
+    const HermConst &C = A.C;
+
     u32 floor_hits = 0, steps = 0;
     u64 next = ~0ull;
 #pragma unroll
     for (int q = 0; q < PER; ++q)
-        if (have[q]) next = min(next, herm_start(A, mine[q], floor_hits));
+        if (have[q]) next = min(next, herm_start<true>(C, V, slot[q], k0[q], k1[q], floor_hits));
     __syncwarp();
     u64 tn = warp_min_u64(next);
     u64 b = 0;
     while (tn != ~0ull) {
-        if (b >= A.max_blocks) { if (lane == 0) A.ctl[HC_ERR] = 1; break; }
+        if (b >= C.max_blocks) { if (lane == 0) A.ctl[HC_ERR] = 1; break; }
         ++b;
         bool act[PER];
         u64 te[PER];
 #pragma unroll
-        for (int q = 0; q < PER; ++q) act[q] = have[q] && herm_evaluate(A, mine[q], tn, te[q]);
+        for (int q = 0; q < PER; ++q) act[q] = have[q] && herm_evaluate<true>(C, V, slot[q], k0[q], k1[q], tn, te[q]);
         __syncwarp();
         next = ~0ull;
 #pragma unroll
         for (int q = 0; q < PER; ++q) {
             if (!have[q]) continue;
-            if (act[q]) { next = min(next, herm_correct(A, mine[q], tn, floor_hits)); ++steps; }
+            if (act[q]) { next = min(next, herm_correct(C, V, slot[q], tn, floor_hits)); ++steps; }
             else next = min(next, te[q]);
         }
         __syncwarp();
         tn = warp_min_u64(next);
     }
+#pragma unroll
+    for (int q = 0; q < PER; ++q)
+        if (have[q]) {
+            const u32 g = S.gid[slot[q]];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                A.G.pos[3 * (size_t)g + c] = S.pos[3 * slot[q] + c];
+                A.G.vel[3 * (size_t)g + c] = S.vel[3 * slot[q] + c];
+            }
+        }
     if (steps) atomicAdd((unsigned long long *)&A.ctl[HC_STEPS], (unsigned long long)steps);
     if (floor_hits) atomicAdd((unsigned long long *)&A.ctl[HC_FLOOR], (unsigned long long)floor_hits);
     if (lane == 0) atomicMax((unsigned long long *)&A.ctl[HC_BLOCKS], (unsigned long long)b);
@@ -333,11 +409,16 @@ __global__ void __launch_bounds__(HERM_THREADS) hermite_grid_kernel(HermArgs A)
     cg::grid_group grid = cg::this_grid();
     const u32 M = A.big_count;
     const u32 *ids = A.members + A.big_begin;
+    const HermConst &C = A.C;
+    const HermView &V = A.G;
     const u32 tid = blockIdx.x * blockDim.x + threadIdx.x, stride = gridDim.x * blockDim.x;
     u32 floor_hits = 0, steps = 0;
     {
         u64 local_min = ~0ull;
-        for (u32 s = tid; s < M; s += stride) local_min = min(local_min, herm_start(A, ids[s], floor_hits));
+        for (u32 s = tid; s < M; s += stride) {
+            const u32 i = ids[s];
+            local_min = min(local_min, herm_start<false>(C, V, i, A.offset[i], A.offset[i + 1], floor_hits));
+        }
         if (local_min != ~0ull) atomicMin((unsigned long long *)&A.ctl[HC_TMIN0], (unsigned long long)local_min);
     }
     grid.sync();
@@ -345,18 +426,19 @@ __global__ void __launch_bounds__(HERM_THREADS) hermite_grid_kernel(HermArgs A)
     for (;; ++b) {
         const u64 tn = *(volatile u64 *)&A.ctl[HC_TMIN0 + b % 3];
         if (tn == ~0ull) break;
-        if (b >= A.max_blocks) { if (tid == 0) A.ctl[HC_ERR] = 1; break; }
+        if (b >= C.max_blocks) { if (tid == 0) A.ctl[HC_ERR] = 1; break; }
         u64 local_min = ~0ull;
         for (u32 s = tid; s < M; s += stride) {            // evaluate the active particles from the state before the block
+            const u32 i = ids[s];
             u64 te;
-            if (!herm_evaluate(A, ids[s], tn, te)) local_min = min(local_min, te);
+            if (!herm_evaluate<false>(C, V, i, A.offset[i], A.offset[i + 1], tn, te)) local_min = min(local_min, te);
         }
         grid.sync();
         for (u32 s = tid; s < M; s += stride) {            // correct them together
             const u32 i = ids[s];
-            const u64 w = A.tdt[i];
+            const u64 w = V.tdt[i];
             if ((w >> 8) + (1ull << (w & 63)) != tn || (w >> 8) >= (1ull << HERM_TICK_BITS)) continue;
-            local_min = min(local_min, herm_correct(A, i, tn, floor_hits));
+            local_min = min(local_min, herm_correct(C, V, i, tn, floor_hits));
             ++steps;
         }
         if (local_min != ~0ull) atomicMin((unsigned long long *)&A.ctl[HC_TMIN0 + (b + 1) % 3], (unsigned long long)local_min);
@@ -389,19 +471,22 @@ p3t_status p3t_stage_hermite(p3t_ctx *ctx, double *d_pos, double *d_vel, double 
     const u64 M = h_ctl[HC_COUNT], nsmall = h_ctl[HC_NSMALL], nbig = h_ctl[HC_BIG_CURSOR];
     if (M) {
         HermArgs A;
-        A.body_user = w.body_user; A.offset = w.nbr_offset; A.nbr = w.nbr; A.members = w.herm_ids; A.comps = w.herm_comps;
-        A.pos = d_pos; A.vel = d_vel;
-        A.tdt = w.herm_tdt; A.a = w.herm_state; A.a1 = w.herm_state + 3 * (size_t)ctx->max_n;
-        A.an = w.herm_state + 6 * (size_t)ctx->max_n; A.a1n = w.herm_state + 9 * (size_t)ctx->max_n;
+        A.G.body_user = w.body_user; A.G.nbr = w.nbr; A.G.mass = nullptr;
+        A.G.pos = d_pos; A.G.vel = d_vel;
+        A.G.tdt = w.herm_tdt; A.G.a = w.herm_state; A.G.a1 = w.herm_state + 3 * (size_t)ctx->max_n;
+        A.G.an = w.herm_state + 6 * (size_t)ctx->max_n; A.G.a1n = w.herm_state + 9 * (size_t)ctx->max_n;
+        A.offset = w.nbr_offset; A.members = w.herm_ids; A.comps = w.herm_comps;
+        A.lnbr = reinterpret_cast<u32 *>(w.pairs);          // the walk's pair buffer is free once the lists are built
         A.ctl = w.herm_ctl;
-        A.prm = ctx->prm;
-        A.tick = T / (double)(1ull << HERM_TICK_BITS);
-        A.eta = eta; A.eta_s = eta_s; A.a0 = a0;
-        A.max_ticks = (1ull << HERM_TICK_BITS) >> log2_div;
-        A.max_blocks = (u64)max_blocks;
+        A.C.prm = ctx->prm;
+        A.C.tick = T / (double)(1ull << HERM_TICK_BITS);
+        A.C.rtick = (double)(1ull << HERM_TICK_BITS) / T;
+        A.C.eta = eta; A.C.eta_s = eta_s; A.C.a0 = a0;
+        A.C.max_ticks = (1ull << HERM_TICK_BITS) >> log2_div;
+        A.C.max_blocks = (u64)max_blocks;
         A.big_begin = (u32)(M - nbig); A.big_count = (u32)nbig;
         if (nsmall) {
-            hermite_warp_kernel<<<div_up(nsmall * 32, HERM_THREADS), HERM_THREADS, 0, ctx->stream>>>(A);
+            hermite_warp_kernel<<<div_up(nsmall, HERM_WARPS), 32 * HERM_WARPS, 0, ctx->stream>>>(A);
             P3T_CUDA(ctx, cudaGetLastError());
         }
         if (nbig) {
