@@ -80,6 +80,7 @@ size_t p3t_layout(Workspace &ws, char *base, size_t max_n, int key_bits, size_t 
     ws.herm_tdt = b.take<u64>(n);
     ws.herm_state = b.take<double>(12 * n);
     ws.herm_parent = b.take<u32>(n);
+    ws.herm_root = b.take<u32>(n);
     ws.herm_csize = b.take<u32>(n);
     ws.herm_cstart = b.take<u32>(n);
     ws.herm_comps = b.take<uint2>(n / 2 + 1);

@@ -81,13 +81,15 @@ __global__ void cc_hook_kernel(const u64 *__restrict__ offset, const u32 *__rest
     }
 }
 
-__global__ void cc_count_kernel(const u64 *__restrict__ offset, u32 n, u32 *parent, u32 *csize, u64 *ctl)
+// (the roots go to their own array: writing them into parent[] here would race with the path halving of the finds that
+// other threads still run through this particle, which may put a non-root ancestor back)
+__global__ void cc_count_kernel(const u64 *__restrict__ offset, u32 n, u32 *parent, u32 *__restrict__ root, u32 *csize, u64 *ctl)
 {
     const u32 i = blockIdx.x * blockDim.x + threadIdx.x;
     const bool has = i < n && offset[i + 1] > offset[i];
     if (has) {
         const u32 r = cc_find(parent, i);
-        parent[i] = r;
+        root[i] = r;
         atomicAdd(&csize[r], 1u);
     }
     const u32 m = __ballot_sync(0xffffffffu, has);
@@ -95,11 +97,11 @@ __global__ void cc_count_kernel(const u64 *__restrict__ offset, u32 n, u32 *pare
 }
 
 // member ranges: small components from the front of members[], the others from the back (HC_COUNT is final here)
-__global__ void cc_assign_kernel(const u64 *__restrict__ offset, u32 n, const u32 *__restrict__ parent, u32 *csize,
+__global__ void cc_assign_kernel(const u64 *__restrict__ offset, u32 n, const u32 *__restrict__ root, u32 *csize,
                                  u32 *__restrict__ cstart, uint2 *__restrict__ comps, u64 *ctl)
 {
     const u32 i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n || offset[i + 1] == offset[i] || parent[i] != i) return;
+    if (i >= n || offset[i + 1] == offset[i] || root[i] != i) return;
     const u32 sz = csize[i];
     u32 st;
     if (sz <= HERM_WARP_MAX) {
@@ -115,12 +117,12 @@ __global__ void cc_assign_kernel(const u64 *__restrict__ offset, u32 n, const u3
     atomicMax((unsigned long long *)&ctl[HC_MAXCOMP], (unsigned long long)sz);
 }
 
-__global__ void cc_scatter_kernel(const u64 *__restrict__ offset, u32 n, const u32 *__restrict__ parent, u32 *csize,
+__global__ void cc_scatter_kernel(const u64 *__restrict__ offset, u32 n, const u32 *__restrict__ root, u32 *csize,
                                   const u32 *__restrict__ cstart, u32 *__restrict__ members)
 {
     const u32 i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n || offset[i + 1] == offset[i]) return;
-    const u32 r = parent[i];
+    const u32 r = root[i];
     members[cstart[r] + atomicAdd(&csize[r], 1u)] = i;     // order inside a component is irrelevant
 }
 
@@ -462,9 +464,9 @@ p3t_status p3t_stage_hermite(p3t_ctx *ctx, double *d_pos, double *d_vel, double 
     P3T_CUDA(ctx, cudaMemsetAsync(w.herm_ctl + HC_TMIN0, 0xff, 3 * sizeof(u64), ctx->stream));
     cc_init_kernel<<<g, 256, 0, ctx->stream>>>(w.nbr_offset, n, w.herm_parent, w.herm_csize);
     cc_hook_kernel<<<g, 256, 0, ctx->stream>>>(w.nbr_offset, w.nbr, n, w.herm_parent);
-    cc_count_kernel<<<g, 256, 0, ctx->stream>>>(w.nbr_offset, n, w.herm_parent, w.herm_csize, w.herm_ctl);
-    cc_assign_kernel<<<g, 256, 0, ctx->stream>>>(w.nbr_offset, n, w.herm_parent, w.herm_csize, w.herm_cstart, w.herm_comps, w.herm_ctl);
-    cc_scatter_kernel<<<g, 256, 0, ctx->stream>>>(w.nbr_offset, n, w.herm_parent, w.herm_csize, w.herm_cstart, w.herm_ids);
+    cc_count_kernel<<<g, 256, 0, ctx->stream>>>(w.nbr_offset, n, w.herm_parent, w.herm_root, w.herm_csize, w.herm_ctl);
+    cc_assign_kernel<<<g, 256, 0, ctx->stream>>>(w.nbr_offset, n, w.herm_root, w.herm_csize, w.herm_cstart, w.herm_comps, w.herm_ctl);
+    cc_scatter_kernel<<<g, 256, 0, ctx->stream>>>(w.nbr_offset, n, w.herm_root, w.herm_csize, w.herm_cstart, w.herm_ids);
     P3T_CUDA(ctx, cudaGetLastError());
     P3T_CUDA(ctx, cudaMemcpyAsync(h_ctl, w.herm_ctl, HC_WORDS * sizeof(u64), cudaMemcpyDeviceToHost, ctx->stream));
     P3T_CUDA(ctx, cudaStreamSynchronize(ctx->stream));

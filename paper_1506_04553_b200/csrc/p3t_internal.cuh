@@ -113,7 +113,7 @@ struct Workspace {
     u32 *subset;                   // [n] staging for eval_direct
     double *hard_out;              // [7n] staging of p3t_eval_hard's host outputs (acc 3n, jerk 3n, pot n); of p3t_hermite_step's pos, vel
     u32 *herm_ids;                 // [n] non-isolated particles by connected component of the neighbour graph (hermite.cu)
-    u32 *herm_parent, *herm_csize, *herm_cstart;   // [n] union-find parent, component size / fill cursor, first member slot
+    u32 *herm_parent, *herm_root, *herm_csize, *herm_cstart;   // [n] union-find parent, root, component size / fill cursor, first member slot
     uint2 *herm_comps;             // [n/2] (start, size) of the components one warp integrates
     u64 *herm_tdt;                 // [n] t << 8 | log2 dt, in ticks
     double *herm_state;            // [4][3 max_n] a, a1 and the block's new a, a1

@@ -239,3 +239,33 @@ def test_whole_step_conserves_energy_with_the_tree(oracle):
     e1 = energy(qd.cpu().numpy(), vd.cpu().numpy())
     assert total > 0
     assert abs(e1 / e0 - 1.0) < 2e-4, e1 / e0 - 1.0
+
+
+def test_king_core_with_long_lists_goes_through_the_grid_kernel(oracle):
+    """A percolating core (config 4's recipe, r_out widened until the core's lists hold ~100 entries): one large
+    component, global blocks with grid barriers, many block levels."""
+    cfg = workloads.config(4, n=32768)
+    T = 1.0 / 1024
+    out = _run_pair(oracle, cfg["mass"], cfg["pos"], cfg["vel"], cfg["eps"], 0.002, 0.02, 0.026, T, theta=cfg["theta"],
+                    log2_div=2, eta=0.1, eta_s=0.01, a0=0.1 * float(cfg["mass"][0]) / 0.02 ** 2)
+    _assert_parity(*out, cfg["pos"].astype(np.float64), cfg["vel"].astype(np.float64), T)
+    info, ooff = out[2], out[6]
+    print(f"King core: longest list {np.diff(ooff).max()}, largest cluster {info['max_component']}, blocks {info['n_blocks']}, "
+          f"steps {info['n_steps']}, {info['ms']:.2f} ms")
+    assert np.diff(ooff).max() >= 50 and info["max_component"] > 1000
+
+
+def test_everybody_isolated_is_a_plain_drift():
+    b = _binding()
+    rng = np.random.default_rng(5)
+    n = 1000
+    pos = rng.uniform(-1, 1, (n, 3)).astype(np.float32)
+    q, v = pos.astype(np.float64), rng.normal(size=(n, 3))
+    with b.P3T(n) as ctx:
+        ctx.set_params(1e-6, 0.4, 1e-6, 1e-5, 2e-5)
+        ctx.soft_force(np.full(n, 1.0 / n, dtype=np.float32), pos)
+        assert ctx.get_stats()["n_neighbours"] == 0
+        q2, v2 = q.copy(), v.copy()
+        info = ctx.hermite_step(q2, v2, 0.125)
+    assert info["n_nonisolated"] == 0 and info["n_steps"] == 0 and info["n_components"] == 0
+    assert np.array_equal(q2, q + 0.125 * v) and np.array_equal(v2, v)
