@@ -96,25 +96,47 @@ __global__ void cc_count_kernel(const u64 *__restrict__ offset, u32 n, u32 *pare
     if (m && (threadIdx.x & 31) == 0) atomicAdd((unsigned long long *)&ctl[HC_COUNT], (unsigned long long)__popc(m));
 }
 
-// member ranges: small components from the front of members[], the others from the back (HC_COUNT is final here)
+// member ranges: small components from the front of members[], the others from the back (HC_COUNT is final here).
+// One atomic per warp and counter: the roots of a warp take consecutive ranges (warp scans of the sizes).
 __global__ void cc_assign_kernel(const u64 *__restrict__ offset, u32 n, const u32 *__restrict__ root, u32 *csize,
                                  u32 *__restrict__ cstart, uint2 *__restrict__ comps, u64 *ctl)
 {
-    const u32 i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n || offset[i + 1] == offset[i] || root[i] != i) return;
-    const u32 sz = csize[i];
+    const u32 i = blockIdx.x * blockDim.x + threadIdx.x, lane = threadIdx.x & 31;
+    const bool is_root = i < n && offset[i + 1] > offset[i] && root[i] == i;
+    const u32 sz = is_root ? csize[i] : 0u;
+    const bool small = is_root && sz <= HERM_WARP_MAX, big = is_root && !small;
+    const u32 m_root = __ballot_sync(0xffffffffu, is_root);
+    if (!m_root) return;
+    const u32 m_small = __ballot_sync(0xffffffffu, small);
+    u32 ss = small ? sz : 0u, sb = big ? sz : 0u;          // inclusive warp scans of the sizes
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const u32 a = __shfl_up_sync(0xffffffffu, ss, o), c = __shfl_up_sync(0xffffffffu, sb, o);
+        if (lane >= (u32)o) { ss += a; sb += c; }
+    }
+    const u32 tot_s = __shfl_sync(0xffffffffu, ss, 31), tot_b = __shfl_sync(0xffffffffu, sb, 31);
+    const u32 mx = __reduce_max_sync(0xffffffffu, sz);
+    u32 base_s = 0, base_b = 0, base_c = 0;
+    if (lane == 0) {
+        if (tot_s) base_s = (u32)atomicAdd((unsigned long long *)&ctl[HC_SMALL_CURSOR], (unsigned long long)tot_s);
+        if (tot_b) base_b = (u32)atomicAdd((unsigned long long *)&ctl[HC_BIG_CURSOR], (unsigned long long)tot_b);
+        if (m_small) base_c = (u32)atomicAdd((unsigned long long *)&ctl[HC_NSMALL], (unsigned long long)__popc(m_small));
+        atomicAdd((unsigned long long *)&ctl[HC_NCOMP], (unsigned long long)__popc(m_root));
+        atomicMax((unsigned long long *)&ctl[HC_MAXCOMP], (unsigned long long)mx);
+    }
+    base_s = __shfl_sync(0xffffffffu, base_s, 0);
+    base_b = __shfl_sync(0xffffffffu, base_b, 0);
+    base_c = __shfl_sync(0xffffffffu, base_c, 0);
+    if (!is_root) return;
     u32 st;
-    if (sz <= HERM_WARP_MAX) {
-        st = (u32)atomicAdd((unsigned long long *)&ctl[HC_SMALL_CURSOR], (unsigned long long)sz);
-        const u32 c = (u32)atomicAdd((unsigned long long *)&ctl[HC_NSMALL], 1ull);
-        comps[c] = make_uint2(st, sz);
+    if (small) {
+        st = base_s + ss - sz;
+        comps[base_c + __popc(m_small & ((1u << lane) - 1))] = make_uint2(st, sz);
     } else {
-        st = (u32)ctl[HC_COUNT] - ((u32)atomicAdd((unsigned long long *)&ctl[HC_BIG_CURSOR], (unsigned long long)sz) + sz);
+        st = (u32)ctl[HC_COUNT] - (base_b + sb);
     }
     cstart[i] = st;
     csize[i] = 0;                          // becomes the fill cursor of the scatter
-    atomicAdd((unsigned long long *)&ctl[HC_NCOMP], 1ull);
-    atomicMax((unsigned long long *)&ctl[HC_MAXCOMP], (unsigned long long)sz);
 }
 
 __global__ void cc_scatter_kernel(const u64 *__restrict__ offset, u32 n, const u32 *__restrict__ root, u32 *csize,
