@@ -352,8 +352,8 @@ def main():
     ab = algorithmic_bytes_tree(n, cfg["key_bits"], st["n_cells"], st["n_groups"])
     hbm = {k: ab[k] / (ph["ms_" + k] * 1e-3) / 1e9 for k in ab}
     tree_ms = ph["ms_pack"] + ph["ms_sort"] + ph["ms_build"] + ph["ms_moments"]
-    # pack | keys+hist, onesweep passes, gather | levels, emit | moments (leaves, internal) | walk, group order | neighbour CSR (6)
-    launches = 1 + (1 + st["sort_passes"] + 1) + 2 + 2 + 2 + 6
+    # pack | keys+hist, onesweep passes, gather | levels, emit | moments (leaves, internal) | group prediction + order, walk | neighbour CSR (6)
+    launches = 1 + (1 + st["sort_passes"] + 1) + 2 + 2 + (3 if not shard else 1) + 6
 
     out = {
         "metric": METRIC, "value": multi.throughput(total_n, ms), "unit": "particles/s", "n_gpus": world, "steps": args.steps,

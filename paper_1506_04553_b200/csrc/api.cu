@@ -56,6 +56,7 @@ size_t p3t_layout(Workspace &ws, char *base, size_t max_n, int key_bits, size_t 
     ws.group_order = b.take<u32>(n);
     ws.order_meta = b.take<u32>(4);
     ws.group_class = b.take<u32>(n);
+    ws.body_class = b.take<u32>(n);
     ws.cell_mac = b.take<float4>(ws.cell_cap);
     ws.cell_mom0 = b.take<float4>(ws.cell_cap);
     ws.cell_mom1 = b.take<float4>(ws.cell_cap);
@@ -149,6 +150,7 @@ extern "C" p3t_status p3t_create(p3t_ctx **out, int device, size_t max_n, int ke
     }
     ctx->base = static_cast<char *>(workspace);
     if (cudaMemsetAsync(ctx->ws.order_meta, 0, 4 * sizeof(u32), ctx->stream) != cudaSuccess) { delete ctx; return P3T_ECUDA; }
+    if (cudaMemsetAsync(ctx->ws.body_class, 0, max_n * sizeof(u32), ctx->stream) != cudaSuccess) { delete ctx; return P3T_ECUDA; }   // no history: one class, Morton order
     for (int i = 0; i < 14; ++i) {
         if (cudaEventCreate(&ctx->ev[i]) != cudaSuccess) { delete ctx; return P3T_ECUDA; }
     }

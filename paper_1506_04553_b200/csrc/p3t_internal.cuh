@@ -96,7 +96,8 @@ struct Workspace {
     uint4 *group_stats;            // [n] per-group diagnostics of the last walk (P3T_ARR_GROUP_STATS)
     u32 *group_order;              // [n] groups by decreasing cost of the previous walk (ticket -> group)
     u32 *order_meta;               // [4] [0]: number of groups group_order is a permutation of (0: none)
-    u32 *group_class;              // [n] cost class of every group of the last walk
+    u32 *group_class;              // [n] predicted cost class of every group of this walk
+    u32 *body_class;               // [n] user order: cost class of the group each body was in at the last walk
     u32 *order_hist;               // [2][1024] groups per cost class, scatter cursors
     // cells
     float4 *cell_mac, *cell_mom0, *cell_mom1, *cell_bmin, *cell_bmax;

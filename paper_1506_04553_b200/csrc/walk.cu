@@ -161,7 +161,7 @@ struct CtaCtl {
     u32 group;     // ticket of the group in flight
     u32 err;
     u32 stat[2];   // list lengths (p-p, p-c entries) summed over the warps, for P3T_ARR_GROUP_STATS
-    u32 pad;
+    u32 cls;       // cost class of the group just finished (read by all threads after the barrier)
 };
 __device__ __forceinline__ u32 vload(const u32 *p) { return *reinterpret_cast<const volatile u32 *>(p); }
 __device__ __forceinline__ void vstore(u32 *p, u32 v) { *reinterpret_cast<volatile u32 *>(p) = v; }
@@ -334,7 +334,7 @@ struct WalkArgs {
     uint4 *__restrict__ group_stats;
     const u32 *__restrict__ group_order;   // position -> group of the previous call, a permutation of 0..order_meta[0]-1
     const u32 *__restrict__ order_meta;
-    u32 *__restrict__ group_class;   // cost class of every group of this walk
+    u32 *__restrict__ body_class;    // [n] user order: cost class of the group each body was in (this walk's record for the next call)
     u32 *order_hist;                 // [ORDER_CLASSES] groups per class
     u32 shard_rank, shard_world;     // this launch walks positions rank, rank + world, ... of the hand-out order
     uint2 *pairs;
@@ -687,10 +687,9 @@ walk_kernel(WalkArgs A, const u32 *__restrict__ group_start, P3TParams prm, u32 
         st.limit = WALK_STACK_SMEM + WALK_STACK_GMEM;
     }
     const u32 ngroups = (u32)A.counters[CNT_NGROUPS];
-    // Hand-out order: the groups of the previous call by decreasing cost (group_order, a permutation of 0..ng_prev-1).
-    // Between two calls of a simulation the number of groups changes by a few and group g still covers about the
-    // same region, so the old order is used as it is: positions below ng_prev go through it (entries that no longer
-    // exist are skipped), positions from ng_prev on are the new groups themselves.
+    // Hand-out order: this call's groups by decreasing PREDICTED cost (group_order, a permutation of 0..ngroups-1 made
+    // by group_predict_kernel + group_order_kernel just before this launch: a group is expected to cost what the group
+    // that held its first body cost in the previous call).
     // A sharded walk hands out positions in Morton order: every rank must map positions to groups alike.
     const u32 ng_prev = A.shard_world > 1 ? 0u : A.order_meta[0];
     const u32 npos = max(ngroups, ng_prev);
@@ -727,17 +726,19 @@ walk_kernel(WalkArgs A, const u32 *__restrict__ group_start, P3TParams prm, u32 
         if (COOP) {
             if (threadIdx.x == 0) {
                 A.group_stats[g] = make_uint4(ctl->stat[0], ctl->stat[1], t0, (u32)globaltimer_ns());
-                const u32 c = cost_class(ctl->stat[0], ctl->stat[1], ge - gs > 32);
-                A.group_class[g] = c;
-                atomicAdd(&A.order_hist[c], 1u);
+                ctl->cls = cost_class(ctl->stat[0], ctl->stat[1], ge - gs > 32);
             }
-            __syncthreads();   // ctl is rewritten for the next group
-        } else if (lane == 0) {
-            const u32 lpp = (u32)((tot_pp - pp0) / (ge - gs)) + 1u, lpc = (u32)((tot_pc - pc0) / (ge - gs));
-            A.group_stats[g] = make_uint4(lpp, lpc, t0, (u32)globaltimer_ns());
-            const u32 c = cost_class(lpp, lpc, ge - gs > 32);
-            A.group_class[g] = c;
-            atomicAdd(&A.order_hist[c], 1u);
+            __syncthreads();   // ctl is rewritten for the next group (cls only at the end of that group)
+            for (u32 bb = gs + threadIdx.x; bb < ge; bb += blockDim.x) A.body_class[A.sorted_idx[bb]] = ctl->cls;
+        } else {
+            u32 c = 0;
+            if (lane == 0) {
+                const u32 lpp = (u32)((tot_pp - pp0) / (ge - gs)) + 1u, lpc = (u32)((tot_pc - pc0) / (ge - gs));
+                A.group_stats[g] = make_uint4(lpp, lpc, t0, (u32)globaltimer_ns());
+                c = cost_class(lpp, lpc, ge - gs > 32);
+            }
+            c = __shfl_sync(0xffffffffu, c, 0);
+            for (u32 bb = gs + lane; bb < ge; bb += 32) A.body_class[A.sorted_idx[bb]] = c;
         }
     }
     if (lane == 0) {
@@ -747,12 +748,25 @@ walk_kernel(WalkArgs A, const u32 *__restrict__ group_start, P3TParams prm, u32 
     }
 }
 
-// Groups by decreasing cost of the walk that just ran (list lengths x 13 / 33 packed operations, halved for
-// the one-body-per-lane path): the next call hands them out in this order, so the long ones start first
-// and the tail of the persistent launch is made of short ones.  The walk kernel files every finished group
-// under a cost class (top bits of the cost as a float: 8 classes per octave) and counts the classes; this
-// kernel turns the counts into offsets (every CTA scans the 1024 counters itself) and scatters the group
-// ids.  The order is only a schedule: results do not depend on it.
+// Groups by decreasing predicted cost, so that the long ones start first and the tail of the persistent launch is made
+// of short ones.  The walk files every body under the cost class of its group (list lengths x 13 / 33 packed
+// operations, halved for the one-body-per-lane path; top bits of the cost as a float: 8 classes per octave).  The next
+// call, whose tree is a little different (bodies have moved, group boundaries and numbers have shifted), predicts for
+// each of ITS groups the class its first body had (group_predict_kernel) and counts the classes; group_order_kernel
+// turns the counts into offsets (every CTA scans the 1024 counters itself) and scatters the group ids.  (Keyed by group
+// number instead, the order of the previous call was worth 0.32 ms of 9 at N = 1M when the positions did not change and
+// almost nothing when they did.)  The order is only a schedule: results do not depend on it.
+__global__ void __launch_bounds__(256) group_predict_kernel(const u32 *__restrict__ group_start, const u32 *__restrict__ sorted_idx,
+                                                            const u32 *__restrict__ body_class, const u64 *__restrict__ counters,
+                                                            u32 *__restrict__ gclass, u32 *hist)
+{
+    const u32 g = blockIdx.x * blockDim.x + threadIdx.x;
+    if (g >= (u32)counters[CNT_NGROUPS]) return;
+    const u32 c = min(body_class[sorted_idx[group_start[g]]], (u32)ORDER_CLASSES - 1u);
+    gclass[g] = c;
+    atomicAdd(&hist[c], 1u);
+}
+
 __global__ void __launch_bounds__(256) group_order_kernel(const u32 *__restrict__ gclass, const u32 *__restrict__ hist, u32 *cursor,
                                                           const u64 *__restrict__ counters, u32 *__restrict__ order, u32 *order_meta)
 {
@@ -817,13 +831,20 @@ p3t_status p3t_stage_walk(p3t_ctx *ctx)
     A.counters = w.counters;
     A.group_order = w.group_order;
     A.order_meta = w.order_meta;
-    A.group_class = w.group_class;
+    A.body_class = w.body_class;
     A.order_hist = w.order_hist;
     A.shard_rank = (u32)ctx->shard_rank;
     A.shard_world = (u32)ctx->shard_world;
     if (ctx->shard_world > 1) {   // particles of the groups other ranks walk: zero acceleration, potential, neighbour count
         P3T_CUDA(ctx, cudaMemsetAsync(w.accpot, 0, ctx->n * sizeof(float4), s));
         P3T_CUDA(ctx, cudaMemsetAsync(w.nbr_count, 0, ctx->n * sizeof(u32), s));
+    }
+    // hand-out order of this call's groups from the classes the previous call left per body (the group count lives on
+    // the device: launch for its upper bound n / 1 .. n groups; a sharded walk keeps Morton order)
+    if (ctx->shard_world == 1) {
+        group_predict_kernel<<<div_up(ctx->n, 256), 256, 0, s>>>(w.group_start, w.idx[ctx->cur], w.body_class, w.counters, w.group_class, w.order_hist);
+        group_order_kernel<<<div_up(ctx->n, 256), 256, 0, s>>>(w.group_class, w.order_hist, w.order_hist + ORDER_CLASSES, w.counters,
+                                                              w.group_order, w.order_meta);
     }
     // one CTA per group when there are too few groups to keep every warp busy to the end of the launch
     // (the group count lives on the device; n / ngroup is its lower bound up to the fill of the groups)
@@ -836,11 +857,6 @@ p3t_status p3t_stage_walk(p3t_ctx *ctx)
         if (coop) walk_kernel<1, true><<<grid, block, smem, s>>>(A, w.group_start, ctx->prm, w.walk_stack);
         else walk_kernel<1, false><<<grid, block, smem, s>>>(A, w.group_start, ctx->prm, w.walk_stack);
     }
-    // (the group count lives on the device: launch for its upper bound n; a sharded walk has seen only its own groups
-    //  and leaves the order as it is)
-    if (ctx->shard_world == 1)
-    group_order_kernel<<<div_up(ctx->n, 256), 256, 0, s>>>(w.group_class, w.order_hist, w.order_hist + ORDER_CLASSES, w.counters,
-                                                          w.group_order, w.order_meta);
     P3T_CUDA(ctx, cudaGetLastError());
     return P3T_OK;
 }

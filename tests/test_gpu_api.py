@@ -178,26 +178,41 @@ def test_cooperative_walk_matches_one_warp_per_group(n):
 
 
 def test_group_order_is_a_permutation_by_decreasing_cost_and_changes_nothing():
-    """The schedule of the next walk (groups by decreasing measured cost) is a permutation of the groups,
-    sorted by the cost the header defines up to the cost classes (eight per octave), and leaves the results bitwise alike."""
+    """The schedule of a walk (its groups by decreasing predicted cost: the cost class the group of each group's first
+    body had in the previous call) is a permutation of the groups; with unchanged positions it is sorted by the cost the
+    header defines up to the cost classes (eight per octave); and it leaves the results bitwise alike."""
     b = _binding()
     cfg = workloads.config(3, n=60000)
     with b.P3T(cfg["n"], key_bits=63) as ctx:
         ctx.set_walk_mode(1)
         ctx.set_params(cfg["eps"], cfg["theta"], cfg["r_in"], cfg["r_out"], cfg["r_search"])
-        ctx.soft_force(cfg["mass"], cfg["pos"])          # Morton order (no history)
+        ctx.soft_force(cfg["mass"], cfg["pos"])          # no history: one class, any order
         a0, p0 = ctx.get_acc_pot()
+        gs = ctx.array("group_start").astype(np.int64)
+        ng = len(gs) - 1
+        assert np.array_equal(np.sort(ctx.array("group_order").astype(np.int64)), np.arange(ng))
+        ctx.soft_force(cfg["mass"], cfg["pos"])          # same tree: groups handed out by the costs of the first call
+        a1, p1 = ctx.get_acc_pot()
+        assert np.array_equal(a0, a1) and np.array_equal(p0, p1)
+        order = ctx.array("group_order").astype(np.int64)
+        stats = ctx.array("group_stats").astype(np.int64)
+        assert np.array_equal(np.sort(order), np.arange(ng))
+        cost = (13 * stats[:, 0] + 33 * stats[:, 1]) * np.where(np.diff(gs) > 32, 2, 1)
+        bits = np.maximum(cost, 1).astype(np.float32).view(np.uint32).astype(np.int64) >> 20    # 8 classes per octave
+        assert np.all(np.diff(bits[order]) <= 0) and bits[order][0] > bits[order][-1]
+        # moved positions: another tree, other group numbers -- still a permutation, still close to cost order
+        rng = np.random.default_rng(3)
+        pos2 = (cfg["pos"] + 1e-3 * rng.normal(size=cfg["pos"].shape)).astype(np.float32)
+        ctx.soft_force(cfg["mass"], pos2)
         order = ctx.array("group_order").astype(np.int64)
         stats = ctx.array("group_stats").astype(np.int64)
         gs = ctx.array("group_start").astype(np.int64)
         ng = len(gs) - 1
         assert np.array_equal(np.sort(order), np.arange(ng))
         cost = (13 * stats[:, 0] + 33 * stats[:, 1]) * np.where(np.diff(gs) > 32, 2, 1)
-        bits = np.maximum(cost, 1).astype(np.float32).view(np.uint32).astype(np.int64) >> 20    # 8 classes per octave
-        assert np.all(np.diff(bits[order]) <= 0)
-        ctx.soft_force(cfg["mass"], cfg["pos"])          # same tree: groups handed out in that order
-        a1, p1 = ctx.get_acc_pot()
-        assert np.array_equal(a0, a1) and np.array_equal(p0, p1)
+        rank = np.empty(ng); rank[order] = np.arange(ng)
+        from scipy.stats import spearmanr
+        assert spearmanr(rank, -cost).correlation > 0.8       # predicted order follows the measured cost
 
 
 def test_all_bodies_at_one_point_and_massless_bodies(oracle):
