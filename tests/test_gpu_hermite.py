@@ -269,3 +269,39 @@ def test_everybody_isolated_is_a_plain_drift():
         info = ctx.hermite_step(q2, v2, 0.125)
     assert info["n_nonisolated"] == 0 and info["n_steps"] == 0 and info["n_components"] == 0
     assert np.array_equal(q2, q + 0.125 * v) and np.array_equal(v2, v)
+
+
+def test_energy_error_falls_with_theta_down_to_the_integrator_floor_as_in_figure_3(oracle):
+    """Fig. 3 (L189), qualitatively: the energy error falls with theta until the integration error takes over ("the
+    energy error does not drop below ... because the error of the leapfrog integrator is larger than the tree force
+    error").  4096-body Plummer model, 64 whole steps of dt_soft = 1/1024, maximum error over the run: observed
+    9e-7, 5e-7 at theta = 1.0, 0.8 and a floor of 3.3e-7 for theta <= 0.6."""
+    import torch
+    b = _binding()
+    cfg = workloads.config(2, n=4096)
+    n, T = cfg["n"], cfg["dt_soft"] / 4
+    m64 = cfg["mass"].astype(np.float64)
+
+    def energy(q, v):
+        _, p = oracle.direct(m64, q, cfg["eps"], 0.0, 0.0)
+        return 0.5 * np.sum(m64 * (v ** 2).sum(1)) + 0.5 * np.sum(m64 * p)
+
+    q0, v0 = cfg["pos"].astype(np.float64), cfg["vel"].astype(np.float64)
+    e0 = energy(q0, v0)
+    md = torch.from_numpy(cfg["mass"]).cuda()
+    worst = {}
+    for theta in (1.0, 0.8, 0.6, 0.4, 0.2):
+        qd, vd = torch.from_numpy(q0).cuda(), torch.from_numpy(v0).cuda()
+        with b.P3T(n, nbr_capacity=1 << 20) as ctx:
+            ctx.set_params(cfg["eps"], theta, cfg["r_in"], cfg["r_out"], cfg["r_search"])
+            ctx.soft_force(cfg["mass"], cfg["pos"])
+            w = 0.0
+            for k in range(64):
+                ctx.step(md, qd, vd, T, a0=0.1 * float(m64[0]) / cfg["r_out"] ** 2)
+                if k % 8 == 7:
+                    w = max(w, abs(energy(qd.cpu().numpy(), vd.cpu().numpy()) / e0 - 1.0))
+        worst[theta] = w
+    plateau = [worst[t] for t in (0.2, 0.4, 0.6)]
+    assert worst[1.0] > 1.5 * min(plateau) and worst[1.0] > worst[0.8] > min(plateau), worst     # tree error shows at large theta
+    assert max(plateau) < 1.5 * min(plateau), worst                                                # integrator floor below
+    assert max(worst.values()) < 1e-5, worst
