@@ -113,7 +113,7 @@ p3t_status p3t_set_group_merge_levels(p3t_ctx *ctx, int levels);
  * when there are few groups (small n) and shortens the tail of the launch; which warp evaluates which
  * cell depends on timing, so accelerations and potentials are reproducible to fp32 rounding of the
  * batch sums (a few 1e-6 relative at most) rather than bitwise; neighbour lists are identical.  0 (default):
- * chosen from n (mode 2 below about 1.5 groups per resident warp).  P3T_EINVAL for another value. */
+ * chosen from n (mode 2 below about 0.65 groups per resident warp).  P3T_EINVAL for another value. */
 p3t_status p3t_set_walk_mode(p3t_ctx *ctx, int mode);
 
 /* Sharding of one evaluation over `world` GPUs: every rank loads ALL particles and builds the

@@ -32,8 +32,9 @@ typedef unsigned char u8;
 #endif
 #define WALK_STACK_SMEM 512          // stack entries per warp held in shared memory
 #define WALK_STACK_GMEM 7168         // overflow entries per warp in global memory
-#ifndef WALK_COOP_BELOW_X2
-#define WALK_COOP_BELOW_X2 3           // auto mode: one CTA per group below WALK_COOP_BELOW_X2 / 2 groups per resident warp
+#ifndef WALK_COOP_BELOW_X20
+#define WALK_COOP_BELOW_X20 13         // auto mode: one CTA per group below 13 / 20 groups per resident warp (measured crossover:
+                                      // n = 100K for groups of 64, 45K for groups of 32, on 2368 resident warps)
 #endif
 
 // Parameters handed to kernels by value.  The coefficients of W are prepared on the host in

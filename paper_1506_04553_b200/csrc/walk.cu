@@ -848,7 +848,7 @@ p3t_status p3t_stage_walk(p3t_ctx *ctx)
     }
     // one CTA per group when there are too few groups to keep every warp busy to the end of the launch
     // (the group count lives on the device; n / ngroup is its lower bound up to the fill of the groups)
-    bool coop = ctx->walk_mode == 2 || (ctx->walk_mode == 0 && 2 * (ctx->n / (size_t)ctx->ngroup) < (size_t)WALK_COOP_BELOW_X2 * grid * WALK_WARPS);
+    bool coop = ctx->walk_mode == 2 || (ctx->walk_mode == 0 && 20 * (ctx->n / (size_t)ctx->ngroup) < (size_t)WALK_COOP_BELOW_X20 * grid * WALK_WARPS);
     const dim3 block(WALK_WARPS * 32);
     if (ctx->ngroup == 64) {
         if (coop) walk_kernel<2, true><<<grid, block, smem, s>>>(A, w.group_start, ctx->prm, w.walk_stack);
