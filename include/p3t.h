@@ -201,6 +201,12 @@ typedef struct {
 p3t_status p3t_hermite_step(p3t_ctx *ctx, double *pos, double *vel, double dt_soft, int log2_div, double eta, double eta_s,
                             double a0, long long max_blocks, int on_device, p3t_hermite_info *info);
 
+/* Tuning knob of p3t_hermite_step: the largest neighbour cluster (connected component of the lists) that one thread-block
+ * cluster of 8 CTAs integrates with its own block times; still larger ones go together through a cooperative kernel
+ * with grid barriers.  Components of up to 64 particles always take one warp each.  Default 4096; 64..1048576.
+ * Results do not depend on it beyond rounding of nothing: the arithmetic per particle is the same. */
+p3t_status p3t_set_hermite_cluster_max(p3t_ctx *ctx, int max_members);
+
 /* One step of the scheme (L142-153) on a state the caller keeps in double precision: velocity kick by dt_soft / 2 with
  * the soft acceleration of the last evaluation (step 2), p3t_hermite_step (step 3), then positions rounded to float,
  * p3t_load_particles + p3t_build_tree + p3t_eval_soft at the new time and the second kick (step 4).  Before the first

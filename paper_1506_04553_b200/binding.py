@@ -29,7 +29,7 @@ _STATUS = {0: "P3T_OK", -1: "P3T_EINVAL", -2: "P3T_ESTATE", -3: "P3T_ENOMEM", -4
 SYMBOLS = [
     "p3t_workspace_bytes", "p3t_create", "p3t_destroy", "p3t_set_params", "p3t_set_tree_params",
     "p3t_set_group_merge_levels", "p3t_set_walk_mode", "p3t_set_shard", "p3t_load_particles", "p3t_build_tree", "p3t_eval_soft", "p3t_eval_direct", "p3t_eval_hard",
-    "p3t_hermite_step", "p3t_step",
+    "p3t_hermite_step", "p3t_step", "p3t_set_hermite_cluster_max",
     "p3t_get_acc_pot", "p3t_get_neighbour_counts", "p3t_get_neighbours", "p3t_get_stats", "p3t_synchronize",
     "p3t_last_error", "p3t_array_info", "p3t_copy_array", "p3t_measure_fp32_peak",
 ]
@@ -70,6 +70,7 @@ def _sig():
     L.p3t_set_tree_params.restype = i; L.p3t_set_tree_params.argtypes = [vp, i, i]
     L.p3t_set_group_merge_levels.restype = i; L.p3t_set_group_merge_levels.argtypes = [vp, i]
     L.p3t_set_walk_mode.restype = i; L.p3t_set_walk_mode.argtypes = [vp, i]
+    L.p3t_set_hermite_cluster_max.restype = i; L.p3t_set_hermite_cluster_max.argtypes = [vp, i]
     L.p3t_set_shard.restype = i; L.p3t_set_shard.argtypes = [vp, i, i]
     L.p3t_load_particles.restype = i; L.p3t_load_particles.argtypes = [vp, sz, vp, vp, i]
     L.p3t_build_tree.restype = i; L.p3t_build_tree.argtypes = [vp]
@@ -239,6 +240,9 @@ class P3T:
         a, j, p = np.empty((self.n, 3)), np.empty((self.n, 3)), np.empty(self.n)
         self._check(_lib.p3t_eval_hard(self._h, pv, a.ctypes.data, j.ctypes.data, p.ctypes.data, 0))
         return a, j, p
+
+    def set_hermite_cluster_max(self, max_members):
+        self._check(_lib.p3t_set_hermite_cluster_max(self._h, int(max_members)))
 
     def hermite_step(self, pos, vel, dt_soft, log2_div=2, eta=0.1, eta_s=0.01, a0=0.0, max_blocks=1 << 22):
         """One soft step under H_hard over the lists of the last eval (p3t_hermite_step): pos, vel float64 [n,3], both

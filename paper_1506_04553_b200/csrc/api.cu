@@ -86,6 +86,7 @@ size_t p3t_layout(Workspace &ws, char *base, size_t max_n, int key_bits, size_t 
     ws.herm_cstart = b.take<u32>(n);
     ws.herm_comps = b.take<uint2>(n / 2 + 1);
     ws.herm_ctl = b.take<u64>(16);
+    ws.herm_bigctl = b.take<u64>(8 * (n / 65 + 1));
     ws.hist = b.take<u32>(8 * 256);            // hist | counters | order_hist are contiguous (p3t_internal.cuh)
     ws.counters = b.take<u64>(CNT_WORDS);
     ws.order_hist = b.take<u32>(2048);
@@ -132,6 +133,7 @@ extern "C" p3t_status p3t_create(p3t_ctx **out, int device, size_t max_n, int ke
     ctx->ngroup = 64;
     ctx->merge_levels = 1;
     ctx->cells_dirty = true;
+    ctx->herm_cluster_max = 4096;
     ctx->shard_rank = 0;
     ctx->shard_world = 1;
     cudaError_t e = cudaSetDevice(device);
@@ -154,6 +156,10 @@ extern "C" p3t_status p3t_create(p3t_ctx **out, int device, size_t max_n, int ke
     for (int i = 0; i < 14; ++i) {
         if (cudaEventCreate(&ctx->ev[i]) != cudaSuccess) { delete ctx; return P3T_ECUDA; }
     }
+    // side stream of the Hermite part (small and mid-size clusters run beside the grid kernel of the large ones)
+    if (cudaStreamCreateWithFlags(&ctx->side_stream, cudaStreamNonBlocking) != cudaSuccess ||
+        cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&ctx->ev_join, cudaEventDisableTiming) != cudaSuccess) { delete ctx; return P3T_ECUDA; }
     *out = ctx;
     return P3T_OK;
 }
@@ -164,6 +170,9 @@ extern "C" p3t_status p3t_destroy(p3t_ctx *ctx)
     cudaStreamSynchronize(ctx->stream);
     for (int i = 0; i < 14; ++i)
         if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
+    if (ctx->side_stream) { cudaStreamSynchronize(ctx->side_stream); cudaStreamDestroy(ctx->side_stream); }
+    if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
+    if (ctx->ev_join) cudaEventDestroy(ctx->ev_join);
     delete ctx;
     return P3T_OK;
 }
@@ -246,6 +255,14 @@ extern "C" p3t_status p3t_set_shard(p3t_ctx *ctx, int rank, int world)
     ctx->shard_rank = rank;
     ctx->shard_world = world;
     ctx->evaluated = false;
+    return P3T_OK;
+}
+
+extern "C" p3t_status p3t_set_hermite_cluster_max(p3t_ctx *ctx, int max_members)
+{
+    if (!ctx) return P3T_EINVAL;
+    if (max_members < 64 || max_members > (1 << 20)) return p3t_fail(ctx, P3T_EINVAL, "max_members must be in 64..1048576");
+    ctx->herm_cluster_max = max_members;
     return P3T_OK;
 }
 

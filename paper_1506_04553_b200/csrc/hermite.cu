@@ -10,14 +10,16 @@
 //
 // Design.  During a soft step the lists are fixed, so a particle's arithmetic only involves its connected component of
 // the neighbour graph ("neighbour cluster"): block times need to be agreed on inside a component only, and the result
-// is the same as with global blocks (the oracle's locality pin P6).  The components are found on the device (lock-free
-// union-find: hook by compare-and-swap, flatten, count, lay the members out contiguously).  A component of up to 64
-// particles -- nearly all of them: pairs and triples -- is integrated by ONE WARP, its block loop synchronised by
-// __syncwarp and a shuffle minimum: no grid barrier, no launch per block, thousands of components in flight.  The
-// members of all larger components (dense cores, where the spheres percolate) go through one cooperative kernel whose
-// block loop uses two grid barriers per block and a 64-bit atomicMin over (t + dt) into rotating words.  A warp keeps
-// its component's state ((t << 8 | log2 dt), x, v, a, a1 and the block's new a, a1) in shared memory, the grid kernel in
-// global arrays indexed by particle; everything fp64.
+// is the same as with global blocks (the oracle's locality pin S6).  The components are found on the device (lock-free
+// union-find: hook by compare-and-swap, flatten, count, lay the members out contiguously).  Three tiers:
+//  1. a component of up to 64 particles -- nearly all of them: pairs and triples -- is integrated by ONE WARP, its state
+//     in shared memory, its block loop synchronised by __syncwarp and a shuffle minimum;
+//  2. a component of up to cluster_max (4096) particles by ONE THREAD-BLOCK CLUSTER of 8 CTAs: cluster barriers, active
+//     particles compacted per block, several lanes per list;
+//  3. the members of all larger components (percolating cores) together in one cooperative kernel on all SMs: two grid
+//     barriers per block, a 64-bit atomicMin per CTA over (t + dt) into rotating words.
+// Tiers 1 and 2 run on a side stream beside tier 3.  No launch and no host round trip per block.  Everything fp64; the
+// state of tiers 2 and 3 lives in global arrays indexed by particle ((t << 8 | log2 dt), a, a1, the block's new a, a1).
 #include "p3t_internal.cuh"
 #include <cooperative_groups.h>
 #include <math_constants.h>
@@ -26,8 +28,11 @@ namespace cg = cooperative_groups;
 #define HERM_THREADS 256
 #define HERM_TICK_BITS 40
 #define HERM_WARP_MAX 64        // largest component one warp integrates
+#define HERM_CLUSTER 8           // CTAs of the thread-block cluster that integrates one mid-size component
+#define HERM_CLUSTER_THREADS 512
 enum { HC_COUNT = 0, HC_TMIN0, HC_TMIN1, HC_TMIN2, HC_BLOCKS, HC_STEPS, HC_FLOOR, HC_ERR,
-       HC_NSMALL, HC_SMALL_CURSOR, HC_BIG_CURSOR, HC_NCOMP, HC_MAXCOMP, HC_WORDS = 16 };
+       HC_NSMALL, HC_SMALL_CURSOR, HC_BIG_CURSOR, HC_NCOMP, HC_MAXCOMP, HC_NBIGC, HC_GRID_CURSOR, HC_WORDS = 16 };
+#define HERM_GRID_FLAG 0x80000000u   // cstart: the component's members go to the grid tier's own array
 
 __device__ __forceinline__ void herm_weights(const P3TParams &p, double s, double &omK, double &dKds)
 {
@@ -96,56 +101,64 @@ __global__ void cc_count_kernel(const u64 *__restrict__ offset, u32 n, u32 *pare
     if (m && (threadIdx.x & 31) == 0) atomicAdd((unsigned long long *)&ctl[HC_COUNT], (unsigned long long)__popc(m));
 }
 
-// member ranges: small components from the front of members[], the others from the back (HC_COUNT is final here).
-// One atomic per warp and counter: the roots of a warp take consecutive ranges (warp scans of the sizes).
+// member ranges: small components (one warp each) from the front of members[], mid-size ones (one thread-block cluster
+// each, up to cluster_max members) from the back, the members of still larger ones (all together in the cooperative grid
+// kernel) in an array of their own.  HC_COUNT is final here.  One atomic per warp and counter for the many small
+// components: the roots of a warp take consecutive ranges (warp scan of the sizes); the few large ones take theirs singly.
 __global__ void cc_assign_kernel(const u64 *__restrict__ offset, u32 n, const u32 *__restrict__ root, u32 *csize,
-                                 u32 *__restrict__ cstart, uint2 *__restrict__ comps, u64 *ctl)
+                                 u32 *__restrict__ cstart, uint2 *__restrict__ comps, u32 comps_last, u64 *__restrict__ bigctl,
+                                 u32 cluster_max, u64 *ctl)
 {
     const u32 i = blockIdx.x * blockDim.x + threadIdx.x, lane = threadIdx.x & 31;
     const bool is_root = i < n && offset[i + 1] > offset[i] && root[i] == i;
     const u32 sz = is_root ? csize[i] : 0u;
-    const bool small = is_root && sz <= HERM_WARP_MAX, big = is_root && !small;
+    const bool small = is_root && sz <= HERM_WARP_MAX;
     const u32 m_root = __ballot_sync(0xffffffffu, is_root);
     if (!m_root) return;
     const u32 m_small = __ballot_sync(0xffffffffu, small);
-    u32 ss = small ? sz : 0u, sb = big ? sz : 0u;          // inclusive warp scans of the sizes
+    u32 ss = small ? sz : 0u;                              // inclusive warp scan of the small sizes
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
-        const u32 a = __shfl_up_sync(0xffffffffu, ss, o), c = __shfl_up_sync(0xffffffffu, sb, o);
-        if (lane >= (u32)o) { ss += a; sb += c; }
+        const u32 a = __shfl_up_sync(0xffffffffu, ss, o);
+        if (lane >= (u32)o) ss += a;
     }
-    const u32 tot_s = __shfl_sync(0xffffffffu, ss, 31), tot_b = __shfl_sync(0xffffffffu, sb, 31);
+    const u32 tot_s = __shfl_sync(0xffffffffu, ss, 31);
     const u32 mx = __reduce_max_sync(0xffffffffu, sz);
-    u32 base_s = 0, base_b = 0, base_c = 0;
+    u32 base_s = 0, base_c = 0;
     if (lane == 0) {
         if (tot_s) base_s = (u32)atomicAdd((unsigned long long *)&ctl[HC_SMALL_CURSOR], (unsigned long long)tot_s);
-        if (tot_b) base_b = (u32)atomicAdd((unsigned long long *)&ctl[HC_BIG_CURSOR], (unsigned long long)tot_b);
         if (m_small) base_c = (u32)atomicAdd((unsigned long long *)&ctl[HC_NSMALL], (unsigned long long)__popc(m_small));
         atomicAdd((unsigned long long *)&ctl[HC_NCOMP], (unsigned long long)__popc(m_root));
         atomicMax((unsigned long long *)&ctl[HC_MAXCOMP], (unsigned long long)mx);
     }
     base_s = __shfl_sync(0xffffffffu, base_s, 0);
-    base_b = __shfl_sync(0xffffffffu, base_b, 0);
     base_c = __shfl_sync(0xffffffffu, base_c, 0);
     if (!is_root) return;
     u32 st;
     if (small) {
         st = base_s + ss - sz;
         comps[base_c + __popc(m_small & ((1u << lane) - 1))] = make_uint2(st, sz);
+    } else if (sz <= cluster_max) {
+        st = (u32)ctl[HC_COUNT] - ((u32)atomicAdd((unsigned long long *)&ctl[HC_BIG_CURSOR], (unsigned long long)sz) + sz);
+        const u32 c = (u32)atomicAdd((unsigned long long *)&ctl[HC_NBIGC], 1ull);
+        comps[comps_last - c] = make_uint2(st, sz);
+        bigctl[8 * c + 0] = ~0ull; bigctl[8 * c + 1] = ~0ull; bigctl[8 * c + 2] = ~0ull; bigctl[8 * c + 3] = 0ull;
     } else {
-        st = (u32)ctl[HC_COUNT] - (base_b + sb);
+        st = (u32)atomicAdd((unsigned long long *)&ctl[HC_GRID_CURSOR], (unsigned long long)sz) | HERM_GRID_FLAG;
     }
     cstart[i] = st;
     csize[i] = 0;                          // becomes the fill cursor of the scatter
 }
 
 __global__ void cc_scatter_kernel(const u64 *__restrict__ offset, u32 n, const u32 *__restrict__ root, u32 *csize,
-                                  const u32 *__restrict__ cstart, u32 *__restrict__ members)
+                                  const u32 *__restrict__ cstart, u32 *__restrict__ members, u32 *__restrict__ grid_members)
 {
     const u32 i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n || offset[i + 1] == offset[i]) return;
     const u32 r = root[i];
-    members[cstart[r] + atomicAdd(&csize[r], 1u)] = i;     // order inside a component is irrelevant
+    const u32 st = cstart[r], p = atomicAdd(&csize[r], 1u);            // order inside a component is irrelevant
+    if (st & HERM_GRID_FLAG) grid_members[(st & ~HERM_GRID_FLAG) + p] = i;
+    else members[st + p] = i;
 }
 
 __global__ void herm_drift_kernel(const u64 *__restrict__ offset, u32 n, double T, double *__restrict__ pos,
@@ -187,15 +200,21 @@ struct HermArgs {
     HermView G;                    // the global view
     const u64 *offset;
     const u32 *members;            // particles by component
-    const uint2 *comps;            // (start, size) of the components of up to HERM_WARP_MAX members
+    const uint2 *comps;            // (start, size): warp-tier components from the front, cluster-tier ones from comps_last down
+    u32 comps_last;
+    u32 *active;                   // [n] cluster tier: active particles of the block, same ranges as members
+    u64 *bigctl;                   // [8 per cluster-tier component] rotating block times, active count
     u32 *lnbr;                     // [capacity] list entries as slots of the particle's component (warp kernel)
     u64 *ctl;
-    u32 big_begin, big_count;      // members[big_begin .. big_begin + big_count): the larger components
+    const u32 *grid_members;       // grid tier: the members of all components above cluster_max
+    u32 grid_count;
 };
 
 // Eq. 7 and its time derivative over the list [k0, k1) of i at time tn (ticks); the particle and its neighbours are
 // predicted from their own last times.  first: t = 0, nothing to predict.
-template <bool LOCAL>
+// SPLIT > 1: SPLIT consecutive lanes share the list of one particle (entry k0 + sub, k0 + sub + SPLIT, ...) and add their
+// partial sums with shuffles; every lane of the warp must make the call (lanes without a particle pass k0 = k1).
+template <bool LOCAL, int SPLIT = 1>
 __device__ __forceinline__ void herm_force(const HermConst &C, const HermView &V, u32 i, u64 k0, u64 k1, u64 tn, bool first,
                                            double *a, double *a1)
 {
@@ -212,7 +231,7 @@ __device__ __forceinline__ void herm_force(const HermConst &C, const HermView &V
     }
     const double eps2 = C.prm.eps2_d;
     double ax = 0, ay = 0, az = 0, jx = 0, jy = 0, jz = 0;
-    for (u64 k = k0; k < k1; ++k) {
+    for (u64 k = k0 + (SPLIT > 1 ? (threadIdx.x & (SPLIT - 1)) : 0); k < k1; k += SPLIT) {
         const u32 j = V.nbr[k];
         const double h = first ? 0.0 : (double)(tn - (V.tdt[j] >> 8)) * C.tick;
         double d[3], w[3];
@@ -235,6 +254,14 @@ __device__ __forceinline__ void herm_force(const HermConst &C, const HermView &V
         const double c1 = mr3 * omK, c2 = mr3 * qv * (3.0 * omK * rs2 + dKds * rs);
         ax -= c1 * d[0]; ay -= c1 * d[1]; az -= c1 * d[2];
         jx -= c1 * w[0] - c2 * d[0]; jy -= c1 * w[1] - c2 * d[1]; jz -= c1 * w[2] - c2 * d[2];
+    }
+    if (SPLIT > 1) {
+        __syncwarp();
+#pragma unroll
+        for (int o = SPLIT / 2; o; o >>= 1) {
+            ax += __shfl_xor_sync(0xffffffffu, ax, o); ay += __shfl_xor_sync(0xffffffffu, ay, o); az += __shfl_xor_sync(0xffffffffu, az, o);
+            jx += __shfl_xor_sync(0xffffffffu, jx, o); jy += __shfl_xor_sync(0xffffffffu, jy, o); jz += __shfl_xor_sync(0xffffffffu, jz, o);
+        }
     }
     a[0] = ax; a[1] = ay; a[2] = az;
     a1[0] = jx; a1[1] = jy; a1[2] = jz;
@@ -427,23 +454,154 @@ __global__ void __launch_bounds__(32 * HERM_WARPS) hermite_warp_kernel(HermArgs 
     if (lane == 0) atomicMax((unsigned long long *)&A.ctl[HC_BLOCKS], (unsigned long long)b);
 }
 
-// all larger components together: global blocks, two grid barriers per block
-__global__ void __launch_bounds__(HERM_THREADS) hermite_grid_kernel(HermArgs A)
+#ifdef P3T_HERM_PROFILE
+__device__ unsigned long long g_hprof[8];
+#define HPROF(k) do { if (tid == 0 && M > 10000) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); if (k) atomicAdd(&g_hprof[k], t_ - hp_last); hp_last = t_; } } while (0)
+extern "C" void p3t_debug_hprof(unsigned long long *out) { cudaDeviceSynchronize(); cudaMemcpyFromSymbol(out, g_hprof, sizeof(g_hprof)); unsigned long long z[8] = {0}; cudaMemcpyToSymbol(g_hprof, z, sizeof(z)); }
+#else
+#define HPROF(k)
+#endif
+template <int SPLIT>
+__device__ __forceinline__ void cluster_evaluate(const HermArgs &A, const u32 *active, const u32 *ids, u32 na, u32 tid, u32 stride, u64 tn)
 {
-    cg::grid_group grid = cg::this_grid();
-    const u32 M = A.big_count;
-    const u32 *ids = A.members + A.big_begin;
+    const HermView &V = A.G;
+    const u32 lane = threadIdx.x & 31;
+    constexpr u32 PER_WARP = 32 / SPLIT;
+    for (u32 e0 = (tid >> 5) * PER_WARP; e0 < na; e0 += (stride >> 5) * PER_WARP) {
+        const u32 e = e0 + lane / SPLIT;
+        const bool ok = e < na;
+        const u32 i = ok ? active[e] : 0u;
+        const u64 k0 = ok ? A.offset[i] : 0ull, k1 = ok ? A.offset[i + 1] : 0ull;
+        double a[3], a1[3];
+        herm_force<false, SPLIT>(A.C, V, ok ? i : ids[0], k0, k1, tn, false, a, a1);
+        if (ok && (lane & (SPLIT - 1)) == 0) {
+#pragma unroll
+            for (int k = 0; k < 3; ++k) { V.an[3 * (size_t)i + k] = a[k]; V.a1n[3 * (size_t)i + k] = a1[k]; }
+        }
+    }
+}
+
+// One thread-block cluster (8 CTAs x 512 threads) per mid-size component: the block loop is synchronised by the
+// hardware cluster barrier (a fraction of a microsecond, against several for a grid barrier), components run side by
+// side.  Per block: scan the members (next block time of the inactive ones, active ones appended to a list), barrier,
+// evaluate the active list one particle per thread, barrier, correct, barrier.  State in global memory (L2).
+__global__ void __cluster_dims__(HERM_CLUSTER, 1, 1) __launch_bounds__(HERM_CLUSTER_THREADS) hermite_cluster_kernel(HermArgs A)
+{
+    cg::cluster_group cl = cg::this_cluster();
+    const u32 c = blockIdx.x / HERM_CLUSTER;
+    const uint2 comp = A.comps[A.comps_last - c];
+    const u32 M = comp.y;
+    const u32 *ids = A.members + comp.x;
+    u32 *active = A.active + comp.x;
+    u64 *ctl = A.bigctl + 8 * (size_t)c;
     const HermConst &C = A.C;
     const HermView &V = A.G;
-    const u32 tid = blockIdx.x * blockDim.x + threadIdx.x, stride = gridDim.x * blockDim.x;
+    const u32 tid = cl.block_rank() * blockDim.x + threadIdx.x, stride = HERM_CLUSTER * blockDim.x, lane = threadIdx.x & 31;
     u32 floor_hits = 0, steps = 0;
+    unsigned long long hp_last = 0; (void)hp_last;
     {
         u64 local_min = ~0ull;
         for (u32 s = tid; s < M; s += stride) {
             const u32 i = ids[s];
             local_min = min(local_min, herm_start<false>(C, V, i, A.offset[i], A.offset[i + 1], floor_hits));
         }
-        if (local_min != ~0ull) atomicMin((unsigned long long *)&A.ctl[HC_TMIN0], (unsigned long long)local_min);
+        local_min = warp_min_u64(local_min);
+        if (lane == 0 && local_min != ~0ull) atomicMin((unsigned long long *)&ctl[0], (unsigned long long)local_min);
+    }
+    cl.sync();
+    u64 b = 0;
+    for (;; ++b) {
+        const u64 tn = *(volatile u64 *)&ctl[b % 3];
+        if (tn == ~0ull) break;
+        if (b >= C.max_blocks) { if (tid == 0) A.ctl[HC_ERR] = 1; break; }
+        u64 local_min = ~0ull;
+        HPROF(0);
+        // scan: four members per thread and round, their time words requested together
+        for (u32 s0 = tid; s0 - lane < M; s0 += 4 * stride) {   // (warp-uniform trip count: the ballots below need every lane)
+            u32 id[4];
+            u64 w[4];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) id[q] = s0 + q * stride < M ? ids[s0 + q * stride] : 0xffffffffu;
+#pragma unroll
+            for (int q = 0; q < 4; ++q) w[q] = id[q] != 0xffffffffu ? V.tdt[id[q]] : ~0ull;
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const u64 t = w[q] >> 8;
+                const bool live = id[q] != 0xffffffffu && t < (1ull << HERM_TICK_BITS);
+                const u64 te = live ? t + (1ull << (w[q] & 63)) : ~0ull;
+                const bool act = live && te == tn;
+                if (!act) local_min = min(local_min, te);
+                const u32 m = __ballot_sync(0xffffffffu, act);
+                if (m) {
+                    u32 base = 0;
+                    if (lane == 0) base = (u32)atomicAdd((unsigned long long *)&ctl[3], (unsigned long long)__popc(m));
+                    base = __shfl_sync(0xffffffffu, base, 0);
+                    if (act) active[base + __popc(m & ((1u << lane) - 1))] = id[q];
+                }
+            }
+        }
+        HPROF(1);
+        cl.sync();
+        HPROF(2);
+        const u32 na = (u32)*(volatile u64 *)&ctl[3];
+        // evaluate the active particles from the state before the block; as many lanes share a particle's list as the
+        // cluster has to spare (the longest list of the block is the critical path: every entry is an L2 round trip plus
+        // an fp64 chain)
+        if (na * 8 <= stride) cluster_evaluate<8>(A, active, ids, na, tid, stride, tn);
+        else if (na * 4 <= stride) cluster_evaluate<4>(A, active, ids, na, tid, stride, tn);
+        else if (na * 2 <= stride) cluster_evaluate<2>(A, active, ids, na, tid, stride, tn);
+        else cluster_evaluate<1>(A, active, ids, na, tid, stride, tn);
+        HPROF(3);
+        cl.sync();
+        HPROF(4);
+        for (u32 e = tid; e < na; e += stride) {           // correct them together
+            local_min = min(local_min, herm_correct(C, V, active[e], tn, floor_hits));
+            ++steps;
+        }
+        local_min = warp_min_u64(local_min);
+        if (lane == 0 && local_min != ~0ull) atomicMin((unsigned long long *)&ctl[(b + 1) % 3], (unsigned long long)local_min);
+        if (tid == 0) { ctl[(b + 2) % 3] = ~0ull; ctl[3] = 0ull; }
+        HPROF(5);
+        cl.sync();
+        HPROF(6);
+    }
+    if (steps) atomicAdd((unsigned long long *)&A.ctl[HC_STEPS], (unsigned long long)steps);
+    if (floor_hits) atomicAdd((unsigned long long *)&A.ctl[HC_FLOOR], (unsigned long long)floor_hits);
+    if (tid == 0) atomicMax((unsigned long long *)&A.ctl[HC_BLOCKS], (unsigned long long)b);
+}
+
+// the components above cluster_max, all together: global blocks, two grid barriers per block
+// minimum over the CTA, then one atomicMin
+__device__ __forceinline__ void cta_min_to(u64 *dst, u64 v, u64 *s_min)
+{
+    v = warp_min_u64(v);
+    if ((threadIdx.x & 31) == 0) s_min[threadIdx.x >> 5] = v;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (u32 w = 1; w < blockDim.x / 32; ++w) v = min(v, s_min[w]);
+        if (v != ~0ull) atomicMin((unsigned long long *)dst, (unsigned long long)v);
+    }
+    __syncthreads();
+}
+
+__global__ void __launch_bounds__(HERM_THREADS) hermite_grid_kernel(HermArgs A)
+{
+    __shared__ u64 s_min[HERM_THREADS / 32];
+    cg::grid_group grid = cg::this_grid();
+    const u32 M = A.grid_count;
+    const u32 *ids = A.grid_members;
+    const HermConst &C = A.C;
+    const HermView &V = A.G;
+    const u32 tid = blockIdx.x * blockDim.x + threadIdx.x, stride = gridDim.x * blockDim.x, lane = threadIdx.x & 31;
+    u32 floor_hits = 0, steps = 0;
+    unsigned long long hp_last = 0; (void)hp_last;
+    {
+        u64 local_min = ~0ull;
+        for (u32 s = tid; s < M; s += stride) {
+            const u32 i = ids[s];
+            local_min = min(local_min, herm_start<false>(C, V, i, A.offset[i], A.offset[i + 1], floor_hits));
+        }
+        cta_min_to(&A.ctl[HC_TMIN0], local_min, s_min);
     }
     grid.sync();
     u64 b = 0;
@@ -452,12 +610,37 @@ __global__ void __launch_bounds__(HERM_THREADS) hermite_grid_kernel(HermArgs A)
         if (tn == ~0ull) break;
         if (b >= C.max_blocks) { if (tid == 0) A.ctl[HC_ERR] = 1; break; }
         u64 local_min = ~0ull;
-        for (u32 s = tid; s < M; s += stride) {            // evaluate the active particles from the state before the block
-            const u32 i = ids[s];
-            u64 te;
-            if (!herm_evaluate<false>(C, V, i, A.offset[i], A.offset[i + 1], tn, te)) local_min = min(local_min, te);
+        HPROF(0);
+        // evaluate the active particles from the state before the block: a warp looks at 32 members, then takes its
+        // active ones four at a time, eight lanes sharing a particle's list
+        for (u32 s0 = tid; s0 - lane < M; s0 += stride) {
+            const bool in = s0 < M;
+            const u32 i = in ? ids[s0] : 0u;
+            const u64 w = in ? V.tdt[i] : ~0ull;
+            const u64 t = w >> 8;
+            const bool live = in && t < (1ull << HERM_TICK_BITS);
+            const u64 te = live ? t + (1ull << (w & 63)) : ~0ull;
+            const bool act = live && te == tn;
+            if (!act) local_min = min(local_min, te);
+            u32 mask = __ballot_sync(0xffffffffu, act);
+            while (mask) {
+                const u32 src = __fns(mask, 0, (lane >> 3) + 1);       // the (lane / 8 + 1)-th active lane, or none
+                const bool ok = src != 0xffffffffu;
+                const u32 ii = __shfl_sync(0xffffffffu, i, ok ? src : 0);
+                const u64 k0 = ok ? A.offset[ii] : 0ull, k1 = ok ? A.offset[ii + 1] : 0ull;
+                double a[3], a1[3];
+                herm_force<false, 8>(C, V, ok ? ii : ids[0], k0, k1, tn, false, a, a1);
+                if (ok && (lane & 7) == 0) {
+#pragma unroll
+                    for (int k = 0; k < 3; ++k) { V.an[3 * (size_t)ii + k] = a[k]; V.a1n[3 * (size_t)ii + k] = a1[k]; }
+                }
+#pragma unroll
+                for (int q = 0; q < 4; ++q) mask &= mask - 1;           // the four lowest set bits are done
+            }
         }
+        HPROF(3);
         grid.sync();
+        HPROF(4);
         for (u32 s = tid; s < M; s += stride) {            // correct them together
             const u32 i = ids[s];
             const u64 w = V.tdt[i];
@@ -465,9 +648,12 @@ __global__ void __launch_bounds__(HERM_THREADS) hermite_grid_kernel(HermArgs A)
             local_min = min(local_min, herm_correct(C, V, i, tn, floor_hits));
             ++steps;
         }
-        if (local_min != ~0ull) atomicMin((unsigned long long *)&A.ctl[HC_TMIN0 + (b + 1) % 3], (unsigned long long)local_min);
+        cta_min_to(&A.ctl[HC_TMIN0 + (b + 1) % 3], local_min, s_min);     // (one atomic per CTA: one per thread on the same
+                                                                          //  word cost 20 us per block)
         if (tid == 0) A.ctl[HC_TMIN0 + (b + 2) % 3] = ~0ull;
+        HPROF(5);
         grid.sync();
+        HPROF(6);
     }
     if (steps) atomicAdd((unsigned long long *)&A.ctl[HC_STEPS], (unsigned long long)steps);
     if (floor_hits) atomicAdd((unsigned long long *)&A.ctl[HC_FLOOR], (unsigned long long)floor_hits);
@@ -487,19 +673,24 @@ p3t_status p3t_stage_hermite(p3t_ctx *ctx, double *d_pos, double *d_vel, double 
     cc_init_kernel<<<g, 256, 0, ctx->stream>>>(w.nbr_offset, n, w.herm_parent, w.herm_csize);
     cc_hook_kernel<<<g, 256, 0, ctx->stream>>>(w.nbr_offset, w.nbr, n, w.herm_parent);
     cc_count_kernel<<<g, 256, 0, ctx->stream>>>(w.nbr_offset, n, w.herm_parent, w.herm_root, w.herm_csize, w.herm_ctl);
-    cc_assign_kernel<<<g, 256, 0, ctx->stream>>>(w.nbr_offset, n, w.herm_root, w.herm_csize, w.herm_cstart, w.herm_comps, w.herm_ctl);
-    cc_scatter_kernel<<<g, 256, 0, ctx->stream>>>(w.nbr_offset, n, w.herm_root, w.herm_csize, w.herm_cstart, w.herm_ids);
+    const u32 comps_last = (u32)(ctx->max_n / 2);
+    cc_assign_kernel<<<g, 256, 0, ctx->stream>>>(w.nbr_offset, n, w.herm_root, w.herm_csize, w.herm_cstart, w.herm_comps, comps_last,
+                                                 w.herm_bigctl, (u32)ctx->herm_cluster_max, w.herm_ctl);
+    cc_scatter_kernel<<<g, 256, 0, ctx->stream>>>(w.nbr_offset, n, w.herm_root, w.herm_csize, w.herm_cstart, w.herm_ids, w.herm_parent);
     P3T_CUDA(ctx, cudaGetLastError());
     P3T_CUDA(ctx, cudaMemcpyAsync(h_ctl, w.herm_ctl, HC_WORDS * sizeof(u64), cudaMemcpyDeviceToHost, ctx->stream));
     P3T_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
-    const u64 M = h_ctl[HC_COUNT], nsmall = h_ctl[HC_NSMALL], nbig = h_ctl[HC_BIG_CURSOR];
+    const u64 M = h_ctl[HC_COUNT], nsmall = h_ctl[HC_NSMALL], nbigc = h_ctl[HC_NBIGC], ngrid = h_ctl[HC_GRID_CURSOR];
     if (M) {
         HermArgs A;
         A.G.body_user = w.body_user; A.G.nbr = w.nbr; A.G.mass = nullptr;
         A.G.pos = d_pos; A.G.vel = d_vel;
         A.G.tdt = w.herm_tdt; A.G.a = w.herm_state; A.G.a1 = w.herm_state + 3 * (size_t)ctx->max_n;
         A.G.an = w.herm_state + 6 * (size_t)ctx->max_n; A.G.a1n = w.herm_state + 9 * (size_t)ctx->max_n;
-        A.offset = w.nbr_offset; A.members = w.herm_ids; A.comps = w.herm_comps;
+        A.offset = w.nbr_offset; A.members = w.herm_ids; A.comps = w.herm_comps; A.comps_last = comps_last;
+        A.active = w.herm_cstart;                           // free once the members are laid out
+        A.bigctl = w.herm_bigctl;
+        A.grid_members = w.herm_parent; A.grid_count = (u32)ngrid;   // parent[] is free once the roots are known
         A.lnbr = reinterpret_cast<u32 *>(w.pairs);          // the walk's pair buffer is free once the lists are built
         A.ctl = w.herm_ctl;
         A.C.prm = ctx->prm;
@@ -508,21 +699,37 @@ p3t_status p3t_stage_hermite(p3t_ctx *ctx, double *d_pos, double *d_vel, double 
         A.C.eta = eta; A.C.eta_s = eta_s; A.C.a0 = a0;
         A.C.max_ticks = (1ull << HERM_TICK_BITS) >> log2_div;
         A.C.max_blocks = (u64)max_blocks;
-        A.big_begin = (u32)(M - nbig); A.big_count = (u32)nbig;
-        if (nsmall) {
-            hermite_warp_kernel<<<div_up(nsmall, HERM_WARPS), 32 * HERM_WARPS, 0, ctx->stream>>>(A);
-            P3T_CUDA(ctx, cudaGetLastError());
-        }
-        if (nbig) {
+        // The grid tier (if any) goes first on the caller's stream: one CTA per SM, mostly waiting at its barriers; the
+        // warp and cluster tiers run beside it on the side stream (disjoint particles), joined before the drift.
+        cudaStream_t rest = ctx->stream;
+        if (ngrid) {
             int per_sm = 0;
             P3T_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, hermite_grid_kernel, HERM_THREADS, 0));
             if (per_sm < 1) return p3t_fail(ctx, P3T_ECUDA, "hermite_grid_kernel does not fit an SM");
-            u32 grid = (u32)((nbig + HERM_THREADS - 1) / HERM_THREADS);
+            u32 grid = (u32)((ngrid + HERM_THREADS - 1) / HERM_THREADS);
             if (grid > (u32)ctx->sm_count) grid = (u32)ctx->sm_count;   // one CTA per SM: the barrier is the cost of a block
+            if (nsmall || nbigc) {
+                P3T_CUDA(ctx, cudaEventRecord(ctx->ev_fork, ctx->stream));
+                P3T_CUDA(ctx, cudaStreamWaitEvent(ctx->side_stream, ctx->ev_fork, 0));
+                rest = ctx->side_stream;
+            }
             void *args[] = {&A};
             P3T_CUDA(ctx, cudaLaunchCooperativeKernel((void *)hermite_grid_kernel, dim3(grid), dim3(HERM_THREADS), args, 0, ctx->stream));
         }
+        if (nsmall) {
+            hermite_warp_kernel<<<div_up(nsmall, HERM_WARPS), 32 * HERM_WARPS, 0, rest>>>(A);
+            P3T_CUDA(ctx, cudaGetLastError());
+        }
+        if (nbigc) {
+            hermite_cluster_kernel<<<(u32)nbigc * HERM_CLUSTER, HERM_CLUSTER_THREADS, 0, rest>>>(A);
+            P3T_CUDA(ctx, cudaGetLastError());
+        }
+        if (rest != ctx->stream) {
+            P3T_CUDA(ctx, cudaEventRecord(ctx->ev_join, rest));
+            P3T_CUDA(ctx, cudaStreamWaitEvent(ctx->stream, ctx->ev_join, 0));
+        }
     }
+    (void)M;
     herm_drift_kernel<<<g, 256, 0, ctx->stream>>>(w.nbr_offset, n, T, d_pos, d_vel);
     P3T_CUDA(ctx, cudaGetLastError());
     return P3T_OK;

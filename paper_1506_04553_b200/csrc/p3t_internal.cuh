@@ -120,6 +120,7 @@ struct Workspace {
     u64 *herm_tdt;                 // [n] t << 8 | log2 dt, in ticks
     double *herm_state;            // [4][3 max_n] a, a1 and the block's new a, a1
     u64 *herm_ctl;                 // [16] counts, cursors, rotating block times, statistics
+    u64 *herm_bigctl;              // [8 per cluster-tier component] rotating block times, active count
     u64 *counters;                 // [CNT_WORDS]
     u32 *walk_stack;               // [nwarps][WALK_STACK_GMEM]
     u64 *scan_tmp;                 // [nblk_scan + 1]
@@ -130,8 +131,11 @@ struct Workspace {
 struct p3t_ctx {
     int device;
     cudaStream_t stream;
+    cudaStream_t side_stream;      // Hermite part: warp and cluster tiers beside the grid tier
+    cudaEvent_t ev_fork, ev_join;
     size_t max_n, n, nbr_capacity;
     int key_bits, max_level, nleaf, ngroup, merge_levels;
+    int herm_cluster_max;          // largest component a thread-block cluster integrates (larger ones: grid kernel)
     int walk_mode;                 // 0 auto, 1 one warp per group, 2 one CTA per group (cooperative)
     int shard_rank, shard_world;   // this context walks the groups at positions rank, rank + world, ... of the hand-out order
     int sm_count;

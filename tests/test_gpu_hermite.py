@@ -24,7 +24,7 @@ def _lists_equal(off, nbr, ooff, olst):
     return np.array_equal(np.asarray(off, dtype=np.int64), ooff) and np.array_equal(np.asarray(nbr, dtype=np.int64), olst.astype(np.int64))
 
 
-def _run_pair(oracle, mass, pos, vel, eps, r_in, r_out, h, T, theta=0.4, on_device=False, **kw):
+def _run_pair(oracle, mass, pos, vel, eps, r_in, r_out, h, T, theta=0.4, on_device=False, cluster_max=None, **kw):
     """GPU hermite_step and oracle.hermite on the same inputs; returns (gpu pos, vel, info, oracle pos, vel, info)."""
     b = _binding()
     eps, r_in, r_out, h = (float(np.float32(x)) for x in (eps, r_in, r_out, h))
@@ -37,6 +37,8 @@ def _run_pair(oracle, mass, pos, vel, eps, r_in, r_out, h, T, theta=0.4, on_devi
         ctx.soft_force(mass, pos)
         off, nbr = ctx.get_neighbours()
         assert _lists_equal(off, nbr, ooff, olst)
+        if cluster_max:
+            ctx.set_hermite_cluster_max(cluster_max)
         if on_device:
             import torch
             qd, vd = torch.from_numpy(q64).cuda(), torch.from_numpy(v64).cuda()
@@ -81,19 +83,25 @@ def test_two_body_orbit_inside_r_in_is_the_oracles(oracle):
     assert d == pytest.approx(np.linalg.norm(pos[0].astype(np.float64) - pos[1]), rel=1e-5)       # still on the circle
 
 
-@pytest.mark.parametrize("seed,n,on_device", [(1, 2000, False), (2, 5000, True), (3, 257, False)])
-def test_clumpy_cluster_matches_the_oracle(oracle, seed, n, on_device):
-    """Dense clumps: long lists, separations on both sides of r_in and r_out, many block levels."""
-    rng = np.random.default_rng(1000 + seed)
-    k = 8
-    centres = rng.uniform(-1, 1, (k, 3))
-    which = rng.integers(0, k, n)
-    pos = (centres[which] + 0.02 * rng.normal(size=(n, 3))).astype(np.float32)
-    vel = (0.5 * rng.normal(size=(n, 3))).astype(np.float32)
-    mass = (rng.uniform(0.5, 1.5, n) / n).astype(np.float32)
+@pytest.mark.parametrize("seed,n,on_device,cluster_max", [(1, 2000, False, None), (2, 5000, True, None), (3, 257, False, None),
+                                                          (1, 2000, True, 100), (4, 9000, False, 400)])
+def test_clumpy_cluster_matches_the_oracle(oracle, seed, n, on_device, cluster_max):
+    """Dense clumps: long lists, separations on both sides of r_in and r_out, many block levels.  All three tiers:
+    a warp per small component, a thread-block cluster per mid-size one, the grid kernel above cluster_max."""
+    r_out, T = 0.01, 1.0 / 256
+    for attempt in range(8):                       # a realisation without a pair in the 1e-6 band around h
+        rng = np.random.default_rng(1000 + seed + 100 * attempt)
+        k = 8
+        centres = rng.uniform(-1, 1, (k, 3))
+        which = rng.integers(0, k, n)
+        pos = (centres[which] + 0.02 * rng.normal(size=(n, 3))).astype(np.float32)
+        vel = (0.5 * rng.normal(size=(n, 3))).astype(np.float32)
+        mass = (rng.uniform(0.5, 1.5, n) / n).astype(np.float32)
+        if len(oracle.neighbours(pos.astype(np.float64), float(np.float32(1e-4)), float(np.float32(r_out + 3 * 0.5 * T)))[2]) == 0:
+            break
     r_out, T = 0.01, 1.0 / 256
     out = _run_pair(oracle, mass, pos, vel, 1e-4, 0.1 * r_out, r_out, r_out + 3 * 0.5 * T, T, on_device=on_device,
-                    log2_div=2, eta=0.1, eta_s=0.01, a0=0.1 * float(mass.mean()) / r_out ** 2)
+                    cluster_max=cluster_max, log2_div=2, eta=0.1, eta_s=0.01, a0=0.1 * float(mass.mean()) / r_out ** 2)
     _assert_parity(*out, pos.astype(np.float64), vel.astype(np.float64), T)
     assert out[2]["n_nonisolated"] > n // 4 and out[2]["n_blocks"] >= 4
     if n >= 2000:
@@ -241,13 +249,14 @@ def test_whole_step_conserves_energy_with_the_tree(oracle):
     assert abs(e1 / e0 - 1.0) < 2e-4, e1 / e0 - 1.0
 
 
-def test_king_core_with_long_lists_goes_through_the_grid_kernel(oracle):
+@pytest.mark.parametrize("cluster_max", [None, 1000])
+def test_king_core_with_long_lists(oracle, cluster_max):
     """A percolating core (config 4's recipe, r_out widened until the core's lists hold ~100 entries): one large
-    component, global blocks with grid barriers, many block levels."""
+    component, integrated by a thread-block cluster (default) or by the grid kernel (cluster_max below its size)."""
     cfg = workloads.config(4, n=32768)
     T = 1.0 / 1024
     out = _run_pair(oracle, cfg["mass"], cfg["pos"], cfg["vel"], cfg["eps"], 0.002, 0.02, 0.026, T, theta=cfg["theta"],
-                    log2_div=2, eta=0.1, eta_s=0.01, a0=0.1 * float(cfg["mass"][0]) / 0.02 ** 2)
+                    cluster_max=cluster_max, log2_div=2, eta=0.1, eta_s=0.01, a0=0.1 * float(cfg["mass"][0]) / 0.02 ** 2)
     _assert_parity(*out, cfg["pos"].astype(np.float64), cfg["vel"].astype(np.float64), T)
     info, ooff = out[2], out[6]
     print(f"King core: longest list {np.diff(ooff).max()}, largest cluster {info['max_component']}, blocks {info['n_blocks']}, "
