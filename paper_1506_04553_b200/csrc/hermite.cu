@@ -97,8 +97,14 @@ __global__ void cc_count_kernel(const u64 *__restrict__ offset, u32 n, u32 *pare
         root[i] = r;
         atomicAdd(&csize[r], 1u);
     }
+    // one atomic per CTA on the shared counter (non-isolated particles are sparse: one per warp would be one per particle)
+    __shared__ u32 s_cnt;
+    if (threadIdx.x == 0) s_cnt = 0;
+    __syncthreads();
     const u32 m = __ballot_sync(0xffffffffu, has);
-    if (m && (threadIdx.x & 31) == 0) atomicAdd((unsigned long long *)&ctl[HC_COUNT], (unsigned long long)__popc(m));
+    if (m && (threadIdx.x & 31) == 0) atomicAdd(&s_cnt, (u32)__popc(m));
+    __syncthreads();
+    if (threadIdx.x == 0 && s_cnt) atomicAdd((unsigned long long *)&ctl[HC_COUNT], (unsigned long long)s_cnt);
 }
 
 // member ranges: small components (one warp each) from the front of members[], mid-size ones (one thread-block cluster
@@ -114,7 +120,6 @@ __global__ void cc_assign_kernel(const u64 *__restrict__ offset, u32 n, const u3
     const u32 sz = is_root ? csize[i] : 0u;
     const bool small = is_root && sz <= HERM_WARP_MAX;
     const u32 m_root = __ballot_sync(0xffffffffu, is_root);
-    if (!m_root) return;
     const u32 m_small = __ballot_sync(0xffffffffu, small);
     u32 ss = small ? sz : 0u;                              // inclusive warp scan of the small sizes
 #pragma unroll
@@ -124,15 +129,28 @@ __global__ void cc_assign_kernel(const u64 *__restrict__ offset, u32 n, const u3
     }
     const u32 tot_s = __shfl_sync(0xffffffffu, ss, 31);
     const u32 mx = __reduce_max_sync(0xffffffffu, sz);
-    u32 base_s = 0, base_c = 0;
-    if (lane == 0) {
-        if (tot_s) base_s = (u32)atomicAdd((unsigned long long *)&ctl[HC_SMALL_CURSOR], (unsigned long long)tot_s);
-        if (m_small) base_c = (u32)atomicAdd((unsigned long long *)&ctl[HC_NSMALL], (unsigned long long)__popc(m_small));
-        atomicAdd((unsigned long long *)&ctl[HC_NCOMP], (unsigned long long)__popc(m_root));
-        atomicMax((unsigned long long *)&ctl[HC_MAXCOMP], (unsigned long long)mx);
+    // CTA level: the warps take ranges of the CTA's totals (shared-memory atomics), one thread takes the CTA's ranges
+    // of the global cursors (roots are sparse: per-warp global atomics would be one per root on the same words)
+    __shared__ u32 s_tot[4], s_base[2];                    // [0] member slots, [1] small components, [2] roots, [3] max size
+    if (threadIdx.x < 4) s_tot[threadIdx.x] = 0;
+    __syncthreads();
+    u32 off_s = 0, off_c = 0;
+    if (lane == 0 && m_root) {
+        if (tot_s) off_s = atomicAdd(&s_tot[0], tot_s);
+        if (m_small) off_c = atomicAdd(&s_tot[1], (u32)__popc(m_small));
+        atomicAdd(&s_tot[2], (u32)__popc(m_root));
+        atomicMax(&s_tot[3], mx);
     }
-    base_s = __shfl_sync(0xffffffffu, base_s, 0);
-    base_c = __shfl_sync(0xffffffffu, base_c, 0);
+    __syncthreads();
+    if (threadIdx.x == 0 && s_tot[2]) {
+        s_base[0] = s_tot[0] ? (u32)atomicAdd((unsigned long long *)&ctl[HC_SMALL_CURSOR], (unsigned long long)s_tot[0]) : 0u;
+        s_base[1] = s_tot[1] ? (u32)atomicAdd((unsigned long long *)&ctl[HC_NSMALL], (unsigned long long)s_tot[1]) : 0u;
+        atomicAdd((unsigned long long *)&ctl[HC_NCOMP], (unsigned long long)s_tot[2]);
+        atomicMax((unsigned long long *)&ctl[HC_MAXCOMP], (unsigned long long)s_tot[3]);
+    }
+    __syncthreads();
+    const u32 base_s = s_base[0] + __shfl_sync(0xffffffffu, off_s, 0);
+    const u32 base_c = s_base[1] + __shfl_sync(0xffffffffu, off_c, 0);
     if (!is_root) return;
     u32 st;
     if (small) {
@@ -672,9 +690,9 @@ p3t_status p3t_stage_hermite(p3t_ctx *ctx, double *d_pos, double *d_vel, double 
     P3T_CUDA(ctx, cudaMemsetAsync(w.herm_ctl + HC_TMIN0, 0xff, 3 * sizeof(u64), ctx->stream));
     cc_init_kernel<<<g, 256, 0, ctx->stream>>>(w.nbr_offset, n, w.herm_parent, w.herm_csize);
     cc_hook_kernel<<<g, 256, 0, ctx->stream>>>(w.nbr_offset, w.nbr, n, w.herm_parent);
-    cc_count_kernel<<<g, 256, 0, ctx->stream>>>(w.nbr_offset, n, w.herm_parent, w.herm_root, w.herm_csize, w.herm_ctl);
+    cc_count_kernel<<<div_up(n, 1024), 1024, 0, ctx->stream>>>(w.nbr_offset, n, w.herm_parent, w.herm_root, w.herm_csize, w.herm_ctl);
     const u32 comps_last = (u32)(ctx->max_n / 2);
-    cc_assign_kernel<<<g, 256, 0, ctx->stream>>>(w.nbr_offset, n, w.herm_root, w.herm_csize, w.herm_cstart, w.herm_comps, comps_last,
+    cc_assign_kernel<<<div_up(n, 1024), 1024, 0, ctx->stream>>>(w.nbr_offset, n, w.herm_root, w.herm_csize, w.herm_cstart, w.herm_comps, comps_last,
                                                  w.herm_bigctl, (u32)ctx->herm_cluster_max, w.herm_ctl);
     cc_scatter_kernel<<<g, 256, 0, ctx->stream>>>(w.nbr_offset, n, w.herm_root, w.herm_csize, w.herm_cstart, w.herm_ids, w.herm_parent);
     P3T_CUDA(ctx, cudaGetLastError());
