@@ -198,6 +198,7 @@ constexpr double kSixth = 1.0 / 6.0;
 struct HermConst {
     P3TParams prm;
     double tick, rtick, eta, eta_s, a0;
+    double c2, c2_s;               // (eta / tick)^2, (eta_s / tick)^2
     u64 max_ticks, max_blocks;
 };
 
@@ -287,15 +288,25 @@ __device__ __forceinline__ void herm_force(const HermConst &C, const HermView &V
 
 __device__ __forceinline__ double norm3(const double *u) { return sqrt(u[0] * u[0] + u[1] * u[1] + u[2] * u[2]); }
 
-// log2 of the largest power of two of ticks <= crit (a time), <= max_ticks, dividing t; at least one tick
-__device__ __forceinline__ u32 herm_quantise(const HermConst &C, double crit, u64 t, u32 &floor_hits)
+// log2 of the largest power of two of ticks <= crit (a time), <= max_ticks, dividing t; at least one tick.  The
+// criterion comes as ct^2 = P / Q (ct = crit / tick, P >= 0, Q > 0): floor(log2 ct) = floor(floor(log2(P / Q)) / 2) is
+// read off the exponents and mantissas of P and Q, which saves the division and the square root at the end of the
+// dependent chain of every step (the oracle takes the root and divides; the two differ only when ct is within
+// rounding of a power of two).
+__device__ __forceinline__ u32 herm_quantise(const HermConst &C, double P, double Q, u64 t, u32 &floor_hits)
 {
-    const double ct = crit * C.rtick;
-    u32 k;
     const u32 kmax = 63 - __clzll((long long)C.max_ticks);
-    if (!(ct < (double)C.max_ticks)) k = kmax;
-    else if (ct < 1.0) { k = 0; ++floor_hits; }
-    else k = (u32)((__double2hiint(ct) >> 20) & 0x7ff) - 1023u;
+    u32 k;
+    if (!(Q > 0.0) || !(P == P)) k = kmax;                 // vanishing denominator (or NaN): the maximum step
+    else {
+        const long long bp = __double_as_longlong(P), bq = __double_as_longlong(Q);
+        const int ep = (int)((bp >> 52) & 0x7ff), eq = (int)((bq >> 52) & 0x7ff);
+        const unsigned long long mp = (unsigned long long)bp & 0xfffffffffffffull, mq = (unsigned long long)bq & 0xfffffffffffffull;
+        const int L = ep - eq - (mp < mq ? 1 : 0);         // floor(log2(P / Q)) for normal numbers; P = 0 gives a large negative
+        if (L >= 2 * (int)kmax) k = kmax;
+        else if (L < 0) { k = 0; ++floor_hits; }
+        else k = (u32)L >> 1;
+    }
     if (t) {
         const u32 tz = __ffsll((long long)t) - 1;          // t % 2^k == 0  <=>  k <= trailing zeros of t
         if (k > tz) k = tz;
@@ -309,9 +320,8 @@ __device__ __forceinline__ u64 herm_start(const HermConst &C, const HermView &V,
 {
     double a[3], a1[3];
     herm_force<LOCAL>(C, V, i, k0, k1, 0, true, a, a1);
-    const double na = norm3(a), n1 = norm3(a1);
-    const double crit = n1 > 0.0 ? C.eta_s * sqrt((na * na + C.a0 * C.a0) / (n1 * n1)) : CUDART_INF;
-    const u32 k = herm_quantise(C, crit, 0, floor_hits);
+    const double d0 = a[0] * a[0] + a[1] * a[1] + a[2] * a[2], d1 = a1[0] * a1[0] + a1[1] * a1[1] + a1[2] * a1[2];
+    const u32 k = herm_quantise(C, C.c2_s * (d0 + C.a0 * C.a0), d1, 0, floor_hits);          // Eq. 20, squared
 #pragma unroll
     for (int c = 0; c < 3; ++c) { V.a[3 * (size_t)i + c] = a[c]; V.a1[3 * (size_t)i + c] = a1[c]; }   // nobody reads a, a1, tdt at t = 0
     V.tdt[i] = k;
@@ -341,7 +351,8 @@ __device__ __forceinline__ u64 herm_correct(const HermConst &C, const HermView &
     const u64 total = 1ull << HERM_TICK_BITS;
     const u64 w = V.tdt[i];
     const double h = (double)(1ull << (w & 63)) * C.tick;
-    const double rh = 1.0 / h, rh2 = rh * rh, rh3 = rh2 * rh;
+    const double rh = __longlong_as_double((long long)(1023 - (int)(w & 63)) << 52) * C.rtick;   // 2^-k / tick, no division
+    const double rh2 = rh * rh, rh3 = rh2 * rh;
     double an[3], jn[3], a2e[3], a3[3];
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
@@ -358,10 +369,11 @@ __device__ __forceinline__ u64 herm_correct(const HermConst &C, const HermView &
         V.a[o] = An; V.a1[o] = Jn;
         an[c] = An; jn[c] = Jn;
     }
-    const double na = norm3(an), n1 = norm3(jn), n2 = norm3(a2e), n3 = norm3(a3);
-    const double den = n1 * n3 + n2 * n2;
-    const double crit = den > 0.0 ? C.eta * sqrt((sqrt(na * na + C.a0 * C.a0) * n2 + n1 * n1) / den) : CUDART_INF;
-    const u32 k = herm_quantise(C, crit, tn, floor_hits);
+    // Eq. 18 squared: ct^2 = (eta / tick)^2 (sqrt(|a|^2 + a0^2) |a2| + |a1|^2) / (|a1| |a3| + |a2|^2), |a1| |a3| as one root
+    const double d0 = an[0] * an[0] + an[1] * an[1] + an[2] * an[2], d1 = jn[0] * jn[0] + jn[1] * jn[1] + jn[2] * jn[2];
+    const double d2 = a2e[0] * a2e[0] + a2e[1] * a2e[1] + a2e[2] * a2e[2], d3 = a3[0] * a3[0] + a3[1] * a3[1] + a3[2] * a3[2];
+    const double den = sqrt(d1 * d3) + d2;
+    const u32 k = herm_quantise(C, C.c2 * (sqrt((d0 + C.a0 * C.a0) * d2) + d1), den, tn, floor_hits);
     V.tdt[i] = tn << 8 | k;
     return tn < total ? tn + (1ull << k) : ~0ull;
 }
@@ -715,6 +727,7 @@ p3t_status p3t_stage_hermite(p3t_ctx *ctx, double *d_pos, double *d_vel, double 
         A.C.tick = T / (double)(1ull << HERM_TICK_BITS);
         A.C.rtick = (double)(1ull << HERM_TICK_BITS) / T;
         A.C.eta = eta; A.C.eta_s = eta_s; A.C.a0 = a0;
+        A.C.c2 = (eta * A.C.rtick) * (eta * A.C.rtick); A.C.c2_s = (eta_s * A.C.rtick) * (eta_s * A.C.rtick);
         A.C.max_ticks = (1ull << HERM_TICK_BITS) >> log2_div;
         A.C.max_blocks = (u64)max_blocks;
         // The grid tier (if any) goes first on the caller's stream: one CTA per SM, mostly waiting at its barriers; the
