@@ -762,7 +762,11 @@ __global__ void __launch_bounds__(256) group_predict_kernel(const u32 *__restric
 {
     const u32 g = blockIdx.x * blockDim.x + threadIdx.x;
     if (g >= (u32)counters[CNT_NGROUPS]) return;
-    const u32 c = min(body_class[sorted_idx[group_start[g]]], (u32)ORDER_CLASSES - 1u);
+    // (class 0 = most expensive: the minimum over the first, middle and last body guards against a group that inherited
+    //  its first body from a cheaper neighbour)
+    const u32 gs = group_start[g], ge = group_start[g + 1];
+    const u32 c = min(min(body_class[sorted_idx[gs]], body_class[sorted_idx[gs + (ge - gs) / 2]]),
+                      min(body_class[sorted_idx[ge - 1]], (u32)ORDER_CLASSES - 1u));
     gclass[g] = c;
     atomicAdd(&hist[c], 1u);
 }
