@@ -51,20 +51,22 @@ def _run_pair(oracle, mass, pos, vel, eps, r_in, r_out, h, T, theta=0.4, on_devi
     return q, v, info, oq, ov, oinfo, ooff
 
 
-def _assert_parity(q, v, info, oq, ov, oinfo, ooff, q0, v0, T):
+def _assert_parity(q, v, info, oq, ov, oinfo, ooff, q0, v0, T, tol=1e-9):
     iso = np.diff(ooff) == 0
     assert info["n_nonisolated"] == int((~iso).sum())
     # the GPU keeps block times per neighbour cluster (connected component of the lists), the oracle globally: the
     # particles' steps are the same (locality, pin P6), the block count is the busiest cluster's
     assert info["n_steps"] == int(oinfo["nstep"].sum())
-    assert info["n_blocks"] == oinfo["blocks"] if info["n_components"] == 1 else 0 < info["n_blocks"] <= oinfo["blocks"]
-    assert info["n_blocks"] >= int(oinfo["nstep"].max())
+    if info["n_components"] <= 1:
+        assert info["n_blocks"] == oinfo["blocks"]
+    else:
+        assert int(oinfo["nstep"].max()) <= info["n_blocks"] <= oinfo["blocks"]
     assert info["floor_hits"] == oinfo["floor_hits"]
     assert np.array_equal(q[iso], oq[iso]) and np.array_equal(v[iso], v0[iso])          # drift: same bits
     scale_q = np.abs(T * v0).max()
     scale_v = np.abs(v0).max()
-    assert np.abs(q - oq).max() <= 1e-9 * scale_q, np.abs(q - oq).max() / scale_q
-    assert np.abs(v - ov).max() <= 1e-9 * scale_v, np.abs(v - ov).max() / scale_v
+    assert np.abs(q - oq).max() <= tol * scale_q, np.abs(q - oq).max() / scale_q
+    assert np.abs(v - ov).max() <= tol * scale_v, np.abs(v - ov).max() / scale_v
 
 
 def test_two_body_orbit_inside_r_in_is_the_oracles(oracle):
@@ -314,3 +316,37 @@ def test_energy_error_falls_with_theta_down_to_the_integrator_floor_as_in_figure
     assert worst[1.0] > 1.5 * min(plateau) and worst[1.0] > worst[0.8] > min(plateau), worst     # tree error shows at large theta
     assert max(plateau) < 1.5 * min(plateau), worst                                                # integrator floor below
     assert max(worst.values()) < 1e-5, worst
+
+
+@pytest.mark.parametrize("case", range(10))
+def test_random_hermite_cases_match_the_oracle(oracle, case):
+    """Seeded random geometries, sizes, radii, step parameters and tier limits: every particle takes the oracle's steps.
+    (Softening of a few per cent of r_out, soft steps of a few per cent of the clumps' dynamical time: with near-collisions -- eps of
+    1e-4 r_out, hundreds of steps per particle -- rounding differences of 1e-16 grow to order one within the soft step
+    and no two implementations agree; all three tiers still agree with each other bitwise there.  Tolerance 1e-6: dense
+    clumps with hundreds of steps per particle amplify the rounding differences to ~1e-8; a wrong term shows at 1e-3.)"""
+    rng = np.random.default_rng(4242 + case)
+    n = int(rng.choice([2, 3, 65, 300, 1500, 4000, 12000]))
+    k = int(rng.integers(1, 6))
+    spread = 10.0 ** rng.uniform(-2.5, -1.0)
+    r_out = float(spread * 10.0 ** rng.uniform(-1.0, -0.3))
+    eps = r_out * 10.0 ** rng.uniform(-2.0, -1.0)
+    T = float(0.05 * np.sqrt(spread ** 3 * k) * rng.uniform(0.3, 1.0))      # a fraction of the clumps' dynamical time
+    h = r_out * float(rng.choice([1.0, 1.3, 1.6]))
+    for attempt in range(8):
+        centres = rng.uniform(-1, 1, (k, 3))
+        which = rng.integers(0, k, n)
+        pos = (centres[which] + spread * rng.normal(size=(n, 3))).astype(np.float32)
+        if len(oracle.neighbours(pos.astype(np.float64), float(np.float32(eps)), float(np.float32(h)))[2]) == 0:
+            break
+    vel = (rng.uniform(0.3, 1.0) * np.sqrt(1.0 / (k * spread)) * rng.normal(size=(n, 3))).astype(np.float32)   # about virial
+    mass = (rng.uniform(0.2, 1.8, n) / n).astype(np.float32)
+    if case % 3 == 0:
+        mass[rng.integers(0, n, max(1, n // 8))] = 0.0
+    kw = dict(log2_div=int(rng.integers(0, 5)), eta=float(rng.choice([0.05, 0.1, 0.2])), a0=0.1 * float(mass.mean()) / r_out ** 2)
+    kw["eta_s"] = kw["eta"] / 10
+    out = _run_pair(oracle, mass, pos, vel, eps, float(rng.choice([0.0, 0.1, 0.5])) * r_out, r_out, h, T,
+                    on_device=bool(case % 2), cluster_max=int(rng.choice([64, 128, 1000, 4096])), **kw)
+    _assert_parity(*out, pos.astype(np.float64), vel.astype(np.float64), T, tol=1e-6)
+    print(f"case {case}: n={n} non-isolated {out[2]['n_nonisolated']} clusters {out[2]['n_components']} largest {out[2]['max_component']} "
+          f"steps {out[2]['n_steps']} blocks {out[2]['n_blocks']}")
