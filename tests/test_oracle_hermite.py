@@ -194,3 +194,88 @@ def test_p8_whole_scheme_conserves_the_total_energy_at_second_order_in_the_soft_
         errs.append(worst)
     assert errs[2] < 1e-4
     assert errs[0] / errs[1] > 2.5 and errs[1] / errs[2] > 2.5         # second order: factor 4 per halving
+
+
+def _ode_reference(oracle, m, q, v, T, accel):
+    """Plain ODE solution x'' = accel(x) with scipy's DOP853 at rtol 1e-12 (an integrator that shares nothing with O7)."""
+    from scipy.integrate import solve_ivp
+    n = len(m)
+
+    def rhs(t, y):
+        x = y[: 3 * n].reshape(n, 3)
+        return np.concatenate([y[3 * n:], accel(x).ravel()])
+
+    sol = solve_ivp(rhs, (0.0, T), np.concatenate([q.ravel(), v.ravel()]), method="DOP853", rtol=1e-12, atol=1e-15)
+    return sol.y[: 3 * n, -1].reshape(n, 3), sol.y[3 * n:, -1].reshape(n, 3)
+
+
+def test_p9_hard_part_is_the_solution_of_the_hard_equations_of_motion(oracle):
+    """Four bodies whose separations cross r_in and r_out, forces of Eq. 7 written out here with K from O1 (pinned in
+    test_oracle_cutoff), integrated by DOP853: O7 converges to that solution at fourth order in eta."""
+    eps, r_in, r_out = 1e-3, 0.01, 0.1
+    m = np.array([0.4, 0.3, 0.2, 0.1])
+    q = np.array([[0.0, 0, 0], [0.06, 0.01, 0], [-0.03, 0.07, 0.02], [0.02, -0.09, 0.05]])
+    v = np.array([[0.0, 0.5, 0], [0.3, -1.0, 0.2], [0.8, 0.1, -0.3], [-0.9, 0.6, 0.1]])
+    n = 4
+
+    def accel(x):
+        a = np.zeros_like(x)
+        for i in range(n):
+            for j in range(n):
+                if i == j:
+                    continue
+                d = x[i] - x[j]
+                s = np.sqrt(d @ d + eps * eps)
+                xx = (s / r_out - r_in / r_out) / (1.0 - r_in / r_out)
+                a[i] -= m[j] * (1.0 - oracle.K(xx)) * d / s ** 3
+        return a
+
+    T = 0.05
+    qr, vr = _ode_reference(oracle, m, q, v, T, accel)
+    off = np.arange(n + 1, dtype=np.int64) * (n - 1)
+    lst = np.concatenate([[j for j in range(n) if j != i] for i in range(n)]).astype(np.int32)
+    errs = []
+    for eta in (0.2, 0.1, 0.05):
+        q2, v2, info = oracle.hermite(m, q, v, eps, r_in, r_out, off, lst, T, log2_div=4, eta=eta, eta_s=eta / 10,
+                                      a0=0.1 * m.mean() / r_out ** 2)
+        errs.append(max(np.abs(q2 - qr).max() / np.abs(qr - q).max(), np.abs(v2 - vr).max() / np.abs(vr).max()))
+    d0 = np.linalg.norm(q[:, None] - q[None], axis=-1)[np.triu_indices(n, 1)]
+    d1 = np.linalg.norm(qr[:, None] - qr[None], axis=-1)[np.triu_indices(n, 1)]
+    assert ((d0 < r_out) != (d1 < r_out)).any() or d1.min() < 0.5 * d0.min()       # the geometry did change
+    assert errs[2] < 5e-6 and errs[0] > 5 * errs[1] > 25 * errs[2], errs          # observed 3.4e-4, 2.2e-5, 1.5e-6: factor 15 per halving
+
+
+def test_p10_whole_scheme_converges_to_newtonian_motion_at_second_order(oracle):
+    """Steps 1-5 (L142-153) against the DOP853 solution of the unsplit softened Newtonian equations: the splitting error
+    is O(dt_soft^2) -- a wrong kick factor (a whole instead of half a kick, a missing second kick) breaks the order."""
+    rng = np.random.default_rng(12)
+    n = 12
+    m = rng.uniform(0.5, 1.5, n) / n
+    q = rng.normal(size=(n, 3)) * 0.15
+    v = rng.normal(size=(n, 3)) * 0.8
+    eps, r_out = 5e-3, 0.12
+    r_in = 0.1 * r_out
+
+    def accel(x):
+        d = x[:, None, :] - x[None, :, :]
+        s2 = (d ** 2).sum(-1) + eps ** 2
+        np.fill_diagonal(s2, 1.0)
+        w = m[None, :] / s2 ** 1.5
+        np.fill_diagonal(w, 0.0)
+        return -(w[:, :, None] * d).sum(1)
+
+    Ttot = 0.1
+    qr, vr = _ode_reference(oracle, m, q, v, Ttot, accel)
+    errs = []
+    for nsteps in (32, 64, 128):
+        T = Ttot / nsteps
+        h = r_out + 3.0 * T
+        qq, vv = q.copy(), v.copy()
+        a, _ = oracle.direct(m, qq, eps, r_in, r_out)
+        off, lst, _ = oracle.neighbours(qq, eps, h)
+        for _ in range(nsteps):
+            qq, vv, a, off, lst, _info = oracle.p3t_step(m, qq, vv, a, off, lst, eps, r_in, r_out, h, T, log2_div=3, eta=0.02,
+                                                         eta_s=0.002, a0=0.1 * m.mean() / r_out ** 2)
+        errs.append(np.abs(qq - qr).max() / np.abs(qr - q).max())
+    assert errs[2] < 5e-5, errs                                                   # observed 4.0e-4, 7.8e-5, 2.0e-5
+    assert 2.5 < errs[0] / errs[1] < 7.0 and 2.5 < errs[1] / errs[2] < 7.0, errs
