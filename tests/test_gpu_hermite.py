@@ -55,7 +55,7 @@ def _assert_parity(q, v, info, oq, ov, oinfo, ooff, q0, v0, T, tol=1e-9):
     iso = np.diff(ooff) == 0
     assert info["n_nonisolated"] == int((~iso).sum())
     # the GPU keeps block times per neighbour cluster (connected component of the lists), the oracle globally: the
-    # particles' steps are the same (locality, pin P6), the block count is the busiest cluster's
+    # particles' steps are the same (locality, pin S6), the block count is the busiest cluster's
     assert info["n_steps"] == int(oinfo["nstep"].sum())
     if info["n_components"] <= 1:
         assert info["n_blocks"] == oinfo["blocks"]

@@ -18,7 +18,7 @@ def _two_body(r, ecc=0.0, m1=0.6, m2=0.4):
 PAIR = (np.array([0, 1, 2]), np.array([1, 0], dtype=np.int32))
 
 
-def test_p1_circular_orbit_follows_the_closed_form_at_fourth_order(oracle):
+def test_s1_circular_orbit_follows_the_closed_form_at_fourth_order(oracle):
     """Inside r_in the hard force is plain Newton (K = 0, Eq. 12 first branch): x(t) = R (cos wt, sin wt)."""
     r = 0.01
     m, q, v, period = _two_body(r)
@@ -35,7 +35,7 @@ def test_p1_circular_orbit_follows_the_closed_form_at_fourth_order(oracle):
     assert errs[0] / errs[1] > 6.0 and errs[1] / errs[2] > 8.0         # step halves -> error / 16 (block quantisation blurs it)
 
 
-def test_p2_eccentric_orbit_conserves_energy_and_angular_momentum(oracle):
+def test_s2_eccentric_orbit_conserves_energy_and_angular_momentum(oracle):
     r, ecc = 0.01, 0.7
     m, q, v, period = _two_body(r, ecc)
 
@@ -62,7 +62,7 @@ def test_p2_eccentric_orbit_conserves_energy_and_angular_momentum(oracle):
     assert info["nstep"][0] > 1.5 * ic["nstep"][0]
 
 
-def test_p3_particles_with_empty_lists_drift(oracle):
+def test_s3_particles_with_empty_lists_drift(oracle):
     rng = np.random.default_rng(3)
     n = 20
     q, v, m = rng.normal(size=(n, 3)), rng.normal(size=(n, 3)), rng.uniform(1, 2, n)
@@ -72,7 +72,7 @@ def test_p3_particles_with_empty_lists_drift(oracle):
     assert info["blocks"] == 0 and not info["nstep"].any()
 
 
-def test_p4_buffer_shell_pair_takes_the_maximum_step_and_moves_on_straight_lines(oracle):
+def test_s4_buffer_shell_pair_takes_the_maximum_step_and_moves_on_straight_lines(oracle):
     """Neighbours outside r_out but inside h feel no hard force (1 - K = 0): a = a1 = 0, Eq. 20 gives infinity,
     so each takes exactly 2^log2_div steps of Delta t_max and the Hermite result is the drift."""
     m = np.array([1.0, 1.0])
@@ -96,7 +96,7 @@ def _hard_energy(oracle, m, q, v, eps, r_in, r_out):
     return 0.5 * np.sum(m * (v ** 2).sum(1)) + 0.5 * np.sum(m * oracle.hard(m, q, v, eps, r_in, r_out)[2])
 
 
-def test_p5_hard_hamiltonian_is_conserved_across_the_cutoff(oracle):
+def test_s5_hard_hamiltonian_is_conserved_across_the_cutoff(oracle):
     """A small cluster whose separations span the changeover and r > r_out, several pairs crossing r_out during the
     step; all-to-all lists.  Delta t_max = T/32: a body outside every cutoff sphere has a = 0 and takes the maximum
     step, which must stay small against r_out / v (L152: a_0, Delta t_max)."""
@@ -121,7 +121,7 @@ def test_p5_hard_hamiltonian_is_conserved_across_the_cutoff(oracle):
     assert errs[0] < 1e-5 and errs[2] < errs[0] / 20.0
 
 
-def test_p6_clusters_that_share_no_list_entry_do_not_see_each_other(oracle):
+def test_s6_clusters_that_share_no_list_entry_do_not_see_each_other(oracle):
     """Locality: integrating two clusters together equals integrating each alone (block times are global, the
     arithmetic of a particle only involves its list)."""
     eps, r_in, r_out = 1e-4, 0.004, 0.04
@@ -146,7 +146,7 @@ def test_p6_clusters_that_share_no_list_entry_do_not_see_each_other(oracle):
     assert np.array_equal(q2[4:], qb2) and np.array_equal(v2[4:], vb2)
 
 
-def test_p7_relabelling_the_particles_changes_nothing_but_rounding(oracle):
+def test_s7_relabelling_the_particles_changes_nothing_but_rounding(oracle):
     eps, r_in, r_out = 1e-4, 0.004, 0.04
     m, q, v = _cluster(31, n=7)
     n = 7
@@ -159,7 +159,7 @@ def test_p7_relabelling_the_particles_changes_nothing_but_rounding(oracle):
     assert np.allclose(q3, q2[perm], rtol=0, atol=1e-12) and np.allclose(v3, v2[perm], rtol=1e-9, atol=1e-9)
 
 
-def test_p8_whole_scheme_conserves_the_total_energy_at_second_order_in_the_soft_step(oracle):
+def test_s8_whole_scheme_conserves_the_total_energy_at_second_order_in_the_soft_step(oracle):
     """Steps 1-5 of L142-153 on a small Plummer-like cluster with the soft force by direct sum: the energy error is
     that of the leapfrog splitting, O(dt_soft^2) (L187: 'the error is dominated by the truncation error of the
     leapfrog integrator')."""
@@ -209,7 +209,7 @@ def _ode_reference(oracle, m, q, v, T, accel):
     return sol.y[: 3 * n, -1].reshape(n, 3), sol.y[3 * n:, -1].reshape(n, 3)
 
 
-def test_p9_hard_part_is_the_solution_of_the_hard_equations_of_motion(oracle):
+def test_s9_hard_part_is_the_solution_of_the_hard_equations_of_motion(oracle):
     """Four bodies whose separations cross r_in and r_out, forces of Eq. 7 written out here with K from O1 (pinned in
     test_oracle_cutoff), integrated by DOP853: O7 converges to that solution at fourth order in eta."""
     eps, r_in, r_out = 1e-3, 0.01, 0.1
@@ -245,7 +245,7 @@ def test_p9_hard_part_is_the_solution_of_the_hard_equations_of_motion(oracle):
     assert errs[2] < 5e-6 and errs[0] > 5 * errs[1] > 25 * errs[2], errs          # observed 3.4e-4, 2.2e-5, 1.5e-6: factor 15 per halving
 
 
-def test_p10_whole_scheme_converges_to_newtonian_motion_at_second_order(oracle):
+def test_s10_whole_scheme_converges_to_newtonian_motion_at_second_order(oracle):
     """Steps 1-5 (L142-153) against the DOP853 solution of the unsplit softened Newtonian equations: the splitting error
     is O(dt_soft^2) -- a wrong kick factor (a whole instead of half a kick, a missing second kick) breaks the order."""
     rng = np.random.default_rng(12)
