@@ -32,8 +32,11 @@
  * Pins (tests/test_oracle_*.py, -m "not gpu"): see DESIGN.md section 4.
  * Parity unpinned: the absolute tree-error level at a given theta (the paper
  * prints only whole-integration energy errors, Fig. 2-3); O4 is pinned by
- * theta=0 == O2, neighbour sets == O3, the (l/d)^3 error slope and moment
- * identities instead.
+ * theta=0 == O2, neighbour sets == O3, the (l/d)^3 error slope of the
+ * acceleration AND of the potential, a = -grad phi of the accepted cells and
+ * moment identities instead.  Also unpinned by nature: the exact form of the
+ * step criterion Eq. 18 (reading A22; pins S1-S10 hold for any criterion of
+ * the right dimension).
  */
 #include <math.h>
 #include <stdint.h>

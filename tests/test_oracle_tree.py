@@ -93,6 +93,78 @@ def test_p13_quadrupole_error_slope(oracle):
     assert np.all(eq < em)
 
 
+def _clump(seed=3, n=64):
+    rng = np.random.default_rng(seed)
+    clump = rng.uniform(-0.5, 0.5, (n, 3))
+    m = rng.uniform(0.5, 1.5, n + 1) / n
+    m[-1] = 1e-30  # the probe
+    return n, clump, m
+
+
+def test_p13_quadrupole_potential_error_slope(oracle):
+    """R-QUAD's potential term (L138 "up to the quadrupole moment"): the relative error of phi against the
+    exact sum falls as (l/d)^3 with Q and as (l/d)^2 without -- a wrong sign or factor in either half of
+    -1/2 [3 RQR/s^5 - trQ/s^3] leaves a second-order error and fails the slope."""
+    n, clump, m = _clump()
+    # rms over five directions: along a single one the octupole can nearly vanish and spoil the fit
+    us = np.array([[0.48, -0.6, 0.64], [0.6, 0.64, -0.48], [-0.64, 0.48, 0.6], [1.0, 0.0, 0.0], [0.0, 0.6, 0.8]])
+    ds = (8.0, 16.0, 32.0, 64.0)
+
+    def errors(use_quad, eps):
+        out = []
+        for d in ds:
+            e2 = 0.0
+            for u in us:
+                pos = np.vstack([clump, d * u])
+                t = oracle.Tree(m, pos, nleaf=n, max_depth=1)
+                sub = np.array([n])
+                r = t.walk(eps, 100.0, 1e-6, 1e-5, 2e-5, subset=sub, use_quad=use_quad)
+                _, p = oracle.direct(m, pos, eps, 1e-6, 1e-5, subset=sub)
+                assert r["n_pp"][0] == 0 and r["n_pc"][0] >= 1
+                e2 += ((r["pot"][0] - p[0]) / p[0]) ** 2
+            out.append(math.sqrt(e2 / len(us)))
+        return np.array(out)
+
+    for eps in (0.0, 0.7):      # softened cell terms carry the same eps (reading A8)
+        eq, em = errors(True, eps), errors(False, eps)
+        slope_q = np.polyfit(np.log(ds), np.log(eq), 1)[0]
+        slope_m = np.polyfit(np.log(ds), np.log(em), 1)[0]
+        assert -3.4 < slope_q < -2.7, (eps, slope_q)
+        assert -2.4 < slope_m < -1.7, (eps, slope_m)
+        assert np.all(eq < 0.2 * em)
+
+
+def test_p13_cell_acceleration_is_minus_gradient_of_cell_potential(oracle):
+    """a = -grad phi term by term for accepted cells: central differences of the walk's potential for a
+    probe moved by +-delta, the accepted set frozen (theta huge, one split: every octant of the clump is
+    accepted whole, the probe sits alone in its own), equal the walk's acceleration."""
+    n, clump, m = _clump(seed=5)
+    probe = np.array([2.9, -3.7, 4.3])
+    for eps in (0.0, 0.9):
+        def walk(p):
+            pos = np.vstack([clump, p])
+            t = oracle.Tree(m, pos, nleaf=n, max_depth=1)
+            r = t.walk(eps, 100.0, 1e-6, 1e-5, 2e-5, subset=np.array([n]))
+            assert r["n_pp"][0] == 0
+            # signature of the decomposition: which bodies sit in which cell
+            return r, (int(r["n_pc"][0]), t.nodes()["count"].tolist(), t.perm().tolist())
+        r0, npc0 = walk(probe)
+        delta = 1e-4
+        grad = np.zeros(3)
+        for ax in range(3):
+            e = np.zeros(3); e[ax] = delta
+            rp, npc_p = walk(probe + e)
+            rm, npc_m = walk(probe - e)
+            assert npc_p == npc_m == npc0          # same cells, same members: the accepted set is frozen
+            grad[ax] = (rp["pot"][0] - rm["pot"][0]) / (2 * delta)
+        np.testing.assert_allclose(r0["acc"][0], -grad, rtol=1e-6, atol=1e-6 * np.linalg.norm(grad))
+        # and the quadrupole part is not negligible here: dropping Q moves the result far beyond that tolerance
+        pos = np.vstack([clump, probe])
+        t = oracle.Tree(m, pos, nleaf=n, max_depth=1)
+        rq = t.walk(eps, 100.0, 1e-6, 1e-5, 2e-5, subset=np.array([n]), use_quad=False)
+        assert abs(rq["pot"][0] - r0["pot"][0]) > 1e-4 * abs(r0["pot"][0])
+
+
 def test_p14_moments_and_topology(oracle, cfg):
     m, q = cfg["m64"], cfg["q64"]
     t = oracle.Tree(m, q, nleaf=16)
