@@ -195,9 +195,13 @@ typedef struct {
  *   - a0 = alpha m / r_cut^2 (Eq. 19) is the caller's to compute; with a0 = 0 the criterion collapses when a
  *     neighbour sits at the cutoff radius and the call ends with P3T_ELIMIT after max_blocks blocks (pos, vel are
  *     then mid-step and must be discarded).
- * The lists must be symmetric (j in L_i <=> i in L_j), which holds for the lists this library makes.  pos and vel are
- * both host or both device (on_device); the call synchronises either way (info is filled; may be NULL).
- * P3T_ESTATE before an eval call; P3T_ECAPACITY if the lists did not fit nbr_capacity; P3T_EINVAL for bad arguments. */
+ * The lists must be symmetric (j in L_i <=> i in L_j) and complete: that holds for p3t_eval_soft on an unsharded
+ * context and for p3t_eval_direct over all particles; after a sharded evaluation (p3t_set_shard with world > 1) or a
+ * subset p3t_eval_direct the call returns P3T_ESTATE, and the symmetry is checked on the device besides (P3T_ESTATE,
+ * whatever the size of the cluster).  pos and vel are both host or both device (on_device); the call synchronises either
+ * way (info is filled; may be NULL).
+ * P3T_ESTATE before an eval call; P3T_ECAPACITY if the lists did not fit nbr_capacity; P3T_EINVAL for bad arguments
+ * and when a force came out non-finite (coincident particles with eps = 0): pos, vel are then unusable. */
 p3t_status p3t_hermite_step(p3t_ctx *ctx, double *pos, double *vel, double dt_soft, int log2_div, double eta, double eta_s,
                             double a0, long long max_blocks, int on_device, p3t_hermite_info *info);
 
@@ -212,7 +216,8 @@ p3t_status p3t_set_hermite_cluster_max(p3t_ctx *ctx, int max_members);
  * p3t_load_particles + p3t_build_tree + p3t_eval_soft at the new time and the second kick (step 4).  Before the first
  * step the caller loads the float-rounded positions and calls p3t_eval_soft once; afterwards the context always holds
  * the soft force and the lists of the current positions.  mass[n] float as in p3t_load_particles; mass, pos, vel are
- * all host or all device.  Errors as for the calls it is made of. */
+ * all host or all device.  Errors as for the calls it is made of; P3T_ESTATE on a sharded context (the kick needs the
+ * soft force of all particles, the Hermite part their lists). */
 p3t_status p3t_step(p3t_ctx *ctx, const float *mass, double *pos, double *vel, double dt_soft, int log2_div, double eta,
                     double eta_s, double a0, long long max_blocks, int on_device, p3t_hermite_info *info);
 

@@ -368,6 +368,7 @@ extern "C" p3t_status p3t_eval_soft(p3t_ctx *ctx)
     P3T_CUDA(ctx, cudaEventRecord(ctx->ev[6], ctx->stream));
     ctx->ev_eval = true;
     ctx->evaluated = true;
+    ctx->lists_complete = ctx->shard_world == 1;   // a shard holds the lists of its own groups only: not symmetric
     return P3T_OK;
 }
 
@@ -394,6 +395,7 @@ extern "C" p3t_status p3t_eval_direct(p3t_ctx *ctx, const uint32_t *i_subset, si
     P3T_CUDA(ctx, cudaEventRecord(ctx->ev[6], ctx->stream));
     ctx->ev_eval = true;
     ctx->evaluated = true;
+    ctx->lists_complete = i_subset == nullptr;     // a subset leaves the other particles' lists empty
     return P3T_OK;
 }
 
@@ -422,7 +424,10 @@ extern "C" p3t_status p3t_eval_hard(p3t_ctx *ctx, const float *vel, double *acc,
     if (st != P3T_OK) return st;
     P3T_CUDA(ctx, cudaEventRecord(ctx->ev[8], ctx->stream));
     ctx->ev_hard = true;
-    if (on_device) return P3T_OK;
+    if (on_device) {
+        ctx->hard_unchecked = true;   // a capacity overflow (nothing computed) surfaces at the next synchronising call
+        return P3T_OK;
+    }
     if (acc) P3T_CUDA(ctx, cudaMemcpyAsync(acc, d_acc, 3 * n * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     if (jerk) P3T_CUDA(ctx, cudaMemcpyAsync(jerk, d_jerk, 3 * n * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     if (pot) P3T_CUDA(ctx, cudaMemcpyAsync(pot, d_pot, n * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
@@ -469,6 +474,7 @@ static p3t_status hermite_on_device(p3t_ctx *ctx, double *d_pos, double *d_vel, 
         info->ms = 0.f;
         cudaEventElapsedTime(&info->ms, ctx->ev[11], ctx->ev[12]);
     }
+    if (h_ctl[7] == 3) return p3t_fail(ctx, P3T_EINVAL, "Hermite part: non-finite force (coincident particles with eps = 0?); pos, vel are unusable");
     if (h_ctl[7] == 2) return p3t_fail(ctx, P3T_ESTATE, "Hermite part: the neighbour lists are not symmetric; pos, vel are unusable");
     if (h_ctl[7]) return p3t_fail(ctx, P3T_ELIMIT, "Hermite part: more than max_blocks block steps (a0 = 0 lets Eq. 18 collapse at the cutoff radius); pos, vel are mid-step");
     return P3T_OK;
@@ -480,6 +486,8 @@ extern "C" p3t_status p3t_hermite_step(p3t_ctx *ctx, double *pos, double *vel, d
     if (!ctx) return P3T_EINVAL;
     if (!pos || !vel) return p3t_fail(ctx, P3T_EINVAL, "null pos/vel");
     if (!ctx->evaluated) return p3t_fail(ctx, P3T_ESTATE, "p3t_hermite_step needs the neighbour lists of an eval call");
+    if (!ctx->lists_complete)
+        return p3t_fail(ctx, P3T_ESTATE, "p3t_hermite_step needs the lists of ALL particles: the last evaluation was sharded or a subset");
     p3t_status st = hermite_args_ok(ctx, dt_soft, log2_div, eta, eta_s, a0, max_blocks);
     if (st != P3T_OK) return st;
     P3T_CUDA(ctx, cudaSetDevice(ctx->device));
@@ -507,6 +515,8 @@ extern "C" p3t_status p3t_step(p3t_ctx *ctx, const float *mass, double *pos, dou
     if (!ctx) return P3T_EINVAL;
     if (!mass || !pos || !vel) return p3t_fail(ctx, P3T_EINVAL, "null mass/pos/vel");
     if (!ctx->evaluated) return p3t_fail(ctx, P3T_ESTATE, "p3t_step needs the soft force and lists of an eval call at the current positions");
+    if (!ctx->lists_complete || ctx->shard_world > 1)
+        return p3t_fail(ctx, P3T_ESTATE, "p3t_step needs the soft force and lists of ALL particles: not available on a sharded context or after a subset evaluation");
     p3t_status st = hermite_args_ok(ctx, dt_soft, log2_div, eta, eta_s, a0, max_blocks);
     if (st != P3T_OK) return st;
     P3T_CUDA(ctx, cudaSetDevice(ctx->device));
@@ -550,6 +560,11 @@ static p3t_status sync_and_check(p3t_ctx *ctx)
     if (ctx->h_counters[CNT_ERR_BUILD]) ctx->cells_dirty = true;
     if (f & ERR_CELL_CAPACITY) return p3t_fail(ctx, P3T_ENOMEM, "octree cell capacity (3 n + 1024) exceeded");
     if (f & ERR_STACK_OVERFLOW) return p3t_fail(ctx, P3T_ENOMEM, "tree-walk stack overflow");
+    if (ctx->hard_unchecked) {
+        ctx->hard_unchecked = false;
+        if (ctx->h_counters[CNT_PAIRS] > ctx->nbr_capacity)
+            return p3t_fail(ctx, P3T_ECAPACITY, "neighbour lists exceed the context's nbr_capacity: the last p3t_eval_hard computed nothing");
+    }
     return P3T_OK;
 }
 

@@ -33,6 +33,7 @@ namespace cg = cooperative_groups;
 enum { HC_COUNT = 0, HC_TMIN0, HC_TMIN1, HC_TMIN2, HC_BLOCKS, HC_STEPS, HC_FLOOR, HC_ERR,
        HC_NSMALL, HC_SMALL_CURSOR, HC_BIG_CURSOR, HC_NCOMP, HC_MAXCOMP, HC_NBIGC, HC_GRID_CURSOR, HC_WORDS = 16 };
 #define HERM_GRID_FLAG 0x80000000u   // cstart: the component's members go to the grid tier's own array
+#define HERM_NONFINITE 0x80000000u   // high bit of a thread's floor_hits counter: it met a non-finite force (herm_quantise)
 
 __device__ __forceinline__ void herm_weights(const P3TParams &p, double s, double &omK, double &dKds)
 {
@@ -48,6 +49,11 @@ __device__ __forceinline__ void herm_weights(const P3TParams &p, double s, doubl
 
 // ---- connected components of the neighbour graph ---------------------------------------------------------------
 
+__device__ __forceinline__ void herm_set_err(u64 *ctl, u32 code)
+{
+    atomicMax((unsigned long long *)&ctl[7 /* HC_ERR */], (unsigned long long)code);
+}
+
 __device__ __forceinline__ u32 cc_find(volatile u32 *parent, u32 i)
 {
     u32 p = parent[i];
@@ -62,16 +68,35 @@ __device__ __forceinline__ u32 cc_find(volatile u32 *parent, u32 i)
 
 __global__ void cc_init_kernel(const u64 *__restrict__ offset, u32 n, u32 *__restrict__ parent, u32 *__restrict__ csize)
 {
+    // every particle is its own root, isolated ones too: a list entry may then name ANY particle without the finds
+    // below leaving initialised memory (lists that are not symmetric are reported by cc_hook_kernel, not trusted)
     const u32 i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n || offset[i + 1] == offset[i]) return;
+    if (i >= n) return;
     parent[i] = i;
     csize[i] = 0;
 }
 
-__global__ void cc_hook_kernel(const u64 *__restrict__ offset, const u32 *__restrict__ nbr, u32 n, u32 *parent)
+// HC_ERR values, the largest wins (atomicMax): 1 = more than max_blocks block steps, 2 = the lists are not symmetric,
+// 3 = a non-finite force (coincident particles with eps = 0)
+__global__ void cc_hook_kernel(const u64 *__restrict__ offset, const u32 *__restrict__ nbr, u32 n, u32 *parent, u64 *ctl)
 {
     const u32 i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
+    // symmetry of the lists (j in L_i <=> i in L_j), which every tier relies on: binary search of i in the ascending L_j
+    for (u64 k = offset[i], e = offset[i + 1]; k < e; ++k) {
+        const u32 j = nbr[k];
+        bool found = false;
+        if (j < n) {
+            u64 lo = offset[j], hi = offset[j + 1];
+            while (lo < hi) {
+                const u64 mid = (lo + hi) >> 1;
+                const u32 v = nbr[mid];
+                if (v == i) { found = true; break; }
+                if (v < i) lo = mid + 1; else hi = mid;
+            }
+        }
+        if (!found) { herm_set_err(ctl, 2u); return; }
+    }
     for (u64 k = offset[i], e = offset[i + 1]; k < e; ++k) {
         const u32 j = nbr[k];
         if (j >= i) break;                 // lists ascend; every edge is hooked once, from its larger end
@@ -297,7 +322,10 @@ __device__ __forceinline__ u32 herm_quantise(const HermConst &C, double P, doubl
 {
     const u32 kmax = 63 - __clzll((long long)C.max_ticks);
     u32 k;
-    if (!(Q > 0.0) || !(P == P)) k = kmax;                 // vanishing denominator (or NaN): the maximum step
+    if (!(P - P == 0.0) || !(Q - Q == 0.0)) {              // a non-finite force or jerk: reported (HERM_NONFINITE), the step is void
+        floor_hits |= HERM_NONFINITE;
+        k = kmax;
+    } else if (!(Q > 0.0)) k = kmax;                       // vanishing denominator: the maximum step
     else {
         const long long bp = __double_as_longlong(P), bq = __double_as_longlong(Q);
         const int ep = (int)((bp >> 52) & 0x7ff), eq = (int)((bq >> 52) & 0x7ff);
@@ -435,7 +463,7 @@ __global__ void __launch_bounds__(32 * HERM_WARPS) hermite_warp_kernel(HermArgs 
             const u32 g = A.G.nbr[k];
             u32 sidx = 0;
             while (sidx < comp.y && S.gid[sidx] != g) ++sidx;
-            if (sidx == comp.y) { A.ctl[HC_ERR] = 2; sidx = slot[q]; }   // a list that is not symmetric: reported, result unusable
+            if (sidx == comp.y) { herm_set_err(A.ctl, 2u); sidx = slot[q]; }   // a list that is not symmetric: reported, result unusable
             A.lnbr[k] = sidx;
         }
     HermView V;
@@ -452,7 +480,7 @@ __global__ void __launch_bounds__(32 * HERM_WARPS) hermite_warp_kernel(HermArgs 
     u64 tn = warp_min_u64(next);
     u64 b = 0;
     while (tn != ~0ull) {
-        if (b >= C.max_blocks) { if (lane == 0) A.ctl[HC_ERR] = 1; break; }
+        if (b >= C.max_blocks) { if (lane == 0) herm_set_err(A.ctl, 1u); break; }
         ++b;
         bool act[PER];
         u64 te[PER];
@@ -480,7 +508,8 @@ __global__ void __launch_bounds__(32 * HERM_WARPS) hermite_warp_kernel(HermArgs 
             }
         }
     if (steps) atomicAdd((unsigned long long *)&A.ctl[HC_STEPS], (unsigned long long)steps);
-    if (floor_hits) atomicAdd((unsigned long long *)&A.ctl[HC_FLOOR], (unsigned long long)floor_hits);
+    if (floor_hits & HERM_NONFINITE) herm_set_err(A.ctl, 3u);
+    if (floor_hits & ~HERM_NONFINITE) atomicAdd((unsigned long long *)&A.ctl[HC_FLOOR], (unsigned long long)(floor_hits & ~HERM_NONFINITE));
     if (lane == 0) atomicMax((unsigned long long *)&A.ctl[HC_BLOCKS], (unsigned long long)b);
 }
 
@@ -543,7 +572,7 @@ __global__ void __cluster_dims__(HERM_CLUSTER, 1, 1) __launch_bounds__(HERM_CLUS
     for (;; ++b) {
         const u64 tn = *(volatile u64 *)&ctl[b % 3];
         if (tn == ~0ull) break;
-        if (b >= C.max_blocks) { if (tid == 0) A.ctl[HC_ERR] = 1; break; }
+        if (b >= C.max_blocks) { if (tid == 0) herm_set_err(A.ctl, 1u); break; }
         u64 local_min = ~0ull;
         HPROF(0);
         // scan: four members per thread and round, their time words requested together
@@ -596,7 +625,8 @@ __global__ void __cluster_dims__(HERM_CLUSTER, 1, 1) __launch_bounds__(HERM_CLUS
         HPROF(6);
     }
     if (steps) atomicAdd((unsigned long long *)&A.ctl[HC_STEPS], (unsigned long long)steps);
-    if (floor_hits) atomicAdd((unsigned long long *)&A.ctl[HC_FLOOR], (unsigned long long)floor_hits);
+    if (floor_hits & HERM_NONFINITE) herm_set_err(A.ctl, 3u);
+    if (floor_hits & ~HERM_NONFINITE) atomicAdd((unsigned long long *)&A.ctl[HC_FLOOR], (unsigned long long)(floor_hits & ~HERM_NONFINITE));
     if (tid == 0) atomicMax((unsigned long long *)&A.ctl[HC_BLOCKS], (unsigned long long)b);
 }
 
@@ -638,7 +668,7 @@ __global__ void __launch_bounds__(HERM_THREADS) hermite_grid_kernel(HermArgs A)
     for (;; ++b) {
         const u64 tn = *(volatile u64 *)&A.ctl[HC_TMIN0 + b % 3];
         if (tn == ~0ull) break;
-        if (b >= C.max_blocks) { if (tid == 0) A.ctl[HC_ERR] = 1; break; }
+        if (b >= C.max_blocks) { if (tid == 0) herm_set_err(A.ctl, 1u); break; }
         u64 local_min = ~0ull;
         HPROF(0);
         // evaluate the active particles from the state before the block: a warp looks at 32 members, then takes its
@@ -686,7 +716,8 @@ __global__ void __launch_bounds__(HERM_THREADS) hermite_grid_kernel(HermArgs A)
         HPROF(6);
     }
     if (steps) atomicAdd((unsigned long long *)&A.ctl[HC_STEPS], (unsigned long long)steps);
-    if (floor_hits) atomicAdd((unsigned long long *)&A.ctl[HC_FLOOR], (unsigned long long)floor_hits);
+    if (floor_hits & HERM_NONFINITE) herm_set_err(A.ctl, 3u);
+    if (floor_hits & ~HERM_NONFINITE) atomicAdd((unsigned long long *)&A.ctl[HC_FLOOR], (unsigned long long)(floor_hits & ~HERM_NONFINITE));
     if (tid == 0) atomicMax((unsigned long long *)&A.ctl[HC_BLOCKS], (unsigned long long)b);
 }
 
@@ -701,7 +732,7 @@ p3t_status p3t_stage_hermite(p3t_ctx *ctx, double *d_pos, double *d_vel, double 
     P3T_CUDA(ctx, cudaMemsetAsync(w.herm_ctl, 0, HC_WORDS * sizeof(u64), ctx->stream));
     P3T_CUDA(ctx, cudaMemsetAsync(w.herm_ctl + HC_TMIN0, 0xff, 3 * sizeof(u64), ctx->stream));
     cc_init_kernel<<<g, 256, 0, ctx->stream>>>(w.nbr_offset, n, w.herm_parent, w.herm_csize);
-    cc_hook_kernel<<<g, 256, 0, ctx->stream>>>(w.nbr_offset, w.nbr, n, w.herm_parent);
+    cc_hook_kernel<<<g, 256, 0, ctx->stream>>>(w.nbr_offset, w.nbr, n, w.herm_parent, w.herm_ctl);
     cc_count_kernel<<<div_up(n, 1024), 1024, 0, ctx->stream>>>(w.nbr_offset, n, w.herm_parent, w.herm_root, w.herm_csize, w.herm_ctl);
     const u32 comps_last = (u32)(ctx->max_n / 2);
     cc_assign_kernel<<<div_up(n, 1024), 1024, 0, ctx->stream>>>(w.nbr_offset, n, w.herm_root, w.herm_csize, w.herm_cstart, w.herm_comps, comps_last,

@@ -140,6 +140,8 @@ struct p3t_ctx {
     int shard_rank, shard_world;   // this context walks the groups at positions rank, rank + world, ... of the hand-out order
     int sm_count;
     bool have_params, loaded, built, evaluated;
+    bool lists_complete;           // the last evaluation made the lists of ALL particles (not a shard, not a subset): they are symmetric
+    bool hard_unchecked;           // a device-form p3t_eval_hard whose capacity check is still due (sync_and_check)
     bool sort_attr_set, walk_attr_set;   // cudaFuncSetAttribute done on this context's device
     int sort_ctas_per_sm;
     bool cells_dirty;              // child counters need a memset before the next build

@@ -95,3 +95,13 @@ def test_hard_force_call_order_and_capacity():
         with pytest.raises(b.P3TError) as e:
             ctx.eval_hard(bad)
         assert e.value.status == b.EINVAL
+        # device form: the call only enqueues; the overflow (nothing was computed) surfaces at the next synchronising call
+        import torch
+        vd = torch.from_numpy(cfg["vel"]).cuda()
+        ad = torch.full((2048, 3), 7.0, dtype=torch.float64, device="cuda")
+        ctx.eval_hard(vd, ad, None, None)
+        with pytest.raises(b.P3TError) as e:
+            ctx.synchronize()
+        assert e.value.status == b.ECAPACITY
+        assert float(ad.min()) == 7.0                       # untouched
+        ctx.synchronize()                                   # reported once; the context stays usable

@@ -187,6 +187,53 @@ def test_needs_an_evaluation_first():
         assert e.value.status == b.ESTATE
 
 
+def test_incomplete_lists_are_refused():
+    """The Hermite part needs symmetric lists of ALL particles: a sharded evaluation or a subset direct evaluation
+    leaves one-sided lists and the calls say so instead of integrating one-sided forces."""
+    b = _binding()
+    cfg = workloads.config(1, n=2048)
+    q, v = cfg["pos"].astype(np.float64), cfg["vel"].astype(np.float64)
+    with b.P3T(2048, key_bits=63) as ctx:
+        ctx.set_params(cfg["eps"], cfg["theta"], 0.01, 0.1, 0.12)
+        ctx.set_shard(0, 2)
+        ctx.soft_force(cfg["mass"], cfg["pos"])
+        with pytest.raises(b.P3TError) as e:
+            ctx.hermite_step(q.copy(), v.copy(), 1 / 256, a0=1.0)
+        assert e.value.status == b.ESTATE
+        with pytest.raises(b.P3TError) as e:
+            ctx.step(cfg["mass"], q.copy(), v.copy(), 1 / 256, a0=1.0)
+        assert e.value.status == b.ESTATE
+        ctx.set_shard(0, 1)
+        ctx.load_particles(cfg["mass"], cfg["pos"])
+        ctx.eval_direct(np.arange(0, 2048, 2))
+        with pytest.raises(b.P3TError) as e:
+            ctx.hermite_step(q.copy(), v.copy(), 1 / 256, a0=1.0)
+        assert e.value.status == b.ESTATE
+        ctx.eval_direct()                                   # all particles: complete, symmetric lists
+        info = ctx.hermite_step(q.copy(), v.copy(), 1 / 256, a0=1.0)
+        assert info["n_nonisolated"] > 0
+        ctx.soft_force(cfg["mass"], cfg["pos"])
+        assert ctx.hermite_step(q.copy(), v.copy(), 1 / 256, a0=1.0)["n_steps"] == info["n_steps"]
+
+
+def test_nonfinite_force_is_reported():
+    """Two bodies at one point with eps = 0: the hard force is 0/0.  Reported (P3T_EINVAL), not integrated."""
+    b = _binding()
+    rng = np.random.default_rng(5)
+    pos = rng.uniform(-1, 1, (64, 3)).astype(np.float32)
+    pos[1] = pos[0]
+    mass = np.full(64, 1 / 64, dtype=np.float32)
+    q, v = pos.astype(np.float64), np.zeros((64, 3))
+    with b.P3T(64, key_bits=63) as ctx:
+        ctx.set_params(0.0, 0.4, 0.001, 0.01, 0.02)
+        ctx.soft_force(mass, pos)
+        cnt, total = ctx.get_neighbour_counts()
+        assert cnt[0] >= 1 and cnt[1] >= 1
+        with pytest.raises(b.P3TError) as e:
+            ctx.hermite_step(q, v, 1 / 256, a0=1.0)
+        assert e.value.status == b.EINVAL
+
+
 def test_whole_step_follows_the_oracles_scheme_at_theta_zero(oracle):
     """p3t_step against oracle.p3t_step (soft force by direct sum O2, lists O3, Hermite O7) over four steps.  The GPU's
     soft force is fp32 (1e-5 per particle at theta = 0, north_star) and its tree sees float-rounded positions, so the
