@@ -22,10 +22,19 @@ _lib = None
 
 
 def build(force: bool = False) -> str:
-    """Compile the oracle with gcc (-O2, OpenMP, strict IEEE: no -ffast-math)."""
+    """Compile the oracle with gcc (-O2, OpenMP, strict IEEE: no -ffast-math).
+
+    P3T_ORACLE_SANITIZE=1 in the environment builds libp3t_oracle_san.so with AddressSanitizer and
+    UndefinedBehaviorSanitizer instead (run python with LD_PRELOAD=$(gcc -print-file-name=libasan.so);
+    profiles/sanitizer_r2.md has the command and its result)."""
+    global _LIB
+    san = os.environ.get("P3T_ORACLE_SANITIZE") == "1"
+    if san:
+        _LIB = os.path.join(_HERE, "libp3t_oracle_san.so")
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-        cmd = ["gcc", "-O2", "-fopenmp", "-fPIC", "-shared", "-std=c99", "-Wall",
-               "-o", _LIB, _SRC, "-lm"]
+        flags = ["-O1", "-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined",
+                 "-fno-omit-frame-pointer"] if san else ["-O2"]
+        cmd = ["gcc"] + flags + ["-fopenmp", "-fPIC", "-shared", "-std=c99", "-Wall", "-o", _LIB, _SRC, "-lm"]
         subprocess.run(cmd, check=True)
     return _LIB
 

@@ -125,3 +125,29 @@ def test_coincident_points_make_a_deep_leaf():
     big = [(int(meta[i, 1]) & 0x7fffffff, int(level[i])) for i in range(len(cells)) if int(meta[i, 1]) & LEAF and (int(meta[i, 1]) & 0x7fffffff) > 16]
     assert big == [(60, 21)]
     ctx.close()
+
+
+def test_rebuilding_one_tree_300_times_gives_the_same_bits():
+    """Repeat-stress of the inter-CTA protocols racecheck cannot see (global memory): the radix sort's relaxed look-back
+    words, the build's look-back columns and the moments climb (release fence + relaxed arrival counter, children read
+    back from L2).  One 200K-body tree is rebuilt 300 times; sorted order, cell topology, groups AND moments must be
+    bitwise identical every time (PAPER.md L142-153 is the GPU procedure these kernels implement)."""
+    cfg = workloads.config(3, n=200003)
+    ctx, _ = _build(cfg, 63)
+    names = ["root_cube", "keys", "sorted_idx", "bodies", "cell_meta", "cell_level", "cell_start", "cell_parent", "group_start",
+             "cell_mac", "cell_mom0", "cell_mom1", "cell_bmin", "cell_bmax"]
+    first = {k: ctx.array(k).copy() for k in names}
+    st0 = ctx.get_stats()
+    assert st0["n_cells"] > 20000 and st0["depth"] >= 8
+    for it in range(300):
+        if it % 3 == 0:
+            ctx.load_particles(cfg["mass"], cfg["pos"])         # also re-runs pack + bounding cube
+        else:
+            ctx.set_params(cfg["eps"], cfg["theta"], cfg["r_in"], cfg["r_out"], cfg["r_search"])   # invalidates the tree
+        ctx.build_tree()
+        st = ctx.get_stats()
+        assert (st["n_cells"], st["n_leaves"], st["n_groups"], st["depth"]) == (st0["n_cells"], st0["n_leaves"], st0["n_groups"], st0["depth"])
+        for k in names:
+            got = ctx.array(k)
+            assert got.tobytes() == first[k].tobytes(), f"rebuild {it}: {k} differs"
+    ctx.close()
