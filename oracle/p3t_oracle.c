@@ -21,6 +21,9 @@
  *   O7  one soft step under H_hard: drift of the isolated particles, fourth-order
  *       Hermite with block timesteps over the neighbour lists (L147, Eq. 18-20
  *       L152-163) -- rank 2 of SURVEY.md 8(f), pinned by tests/test_oracle_hermite.py
+ *   O8  per-pair-class cutoffs (section 3.2.2.1): O2, O3, O6 and O4 with a class
+ *       per body and (eps, r_in, r_cut, h) per kind of pair, unsplit BH-BH pairs --
+ *       rank 3 of SURVEY.md 8(f), pinned by tests/test_oracle_classes.py
  *
  * Readings of the paper used here (each listed in DESIGN.md section 3):
  *   A1  Eq. 17's denominator is (gamma-1)^7 (as extracted it is (1-gamma)^7,
@@ -768,6 +771,253 @@ void p3t_oracle_tree_walk(const void *tree, double eps, double theta, double r_i
         if (w.nbr && w.nbr_n > 1)
             qsort(w.nbr, (size_t)(w.nbr_n < w.nbr_cap ? w.nbr_n : w.nbr_cap), sizeof(int32_t), cmp_i32);
     }
+}
+
+/* ------------------------------------------------------------------ O8 -- */
+
+/*
+ * Per-pair-class cutoffs (section 3.2.2.1: "three values for the cut off radius with respect to three different
+ * kinds of interactions"): every body carries a class, 0 = field star (FS) or 1 = black hole (BH); the kind of a pair is
+ * k = cls_i + cls_j (0: FS-FS, 1: BH-FS, 2: BH-BH) and each kind has its own softening, cutoff radii and neighbour
+ * radius, tab[4 k .. 4 k + 3] = (eps, r_in, r_cut, h).  A kind whose r_cut is +infinity is NOT SPLIT (L287: "the force
+ * is not split and F_soft = 0 ... integrated with the pure Hermite scheme"): K = W = 0 in the soft sums, 1 - K = 1 - W
+ * = 1 in the hard sums at every separation, and the two bodies are always in each other's neighbour list.  Everything
+ * else is O2 / O3 / O6 / O4 with the pair's own numbers.  With all classes 0 these functions reduce to the ones above.
+ */
+typedef struct { double eps2, r_in, r_out, h; int unsplit; } pairprm;
+
+static inline pairprm pair_of(const double *tab, const uint8_t *cls, int64_t i, int64_t j)
+{
+    const double *t = tab + 4 * ((int)cls[i] + (int)cls[j]);
+    pairprm p = { t[0] * t[0], t[1], t[2], t[3], isinf(t[2]) ? 1 : 0 };
+    return p;
+}
+
+/* K, W of a pair at softened separation s */
+static inline void pair_weights_cls(const pairprm *p, double s, double *K, double *W)
+{
+    if (p->unsplit) { *K = 0.0; *W = 0.0; }
+    else if (s >= p->r_out) { *K = 1.0; *W = 1.0; }
+    else pair_weights(s, p->r_in, p->r_out, K, W);
+}
+
+/* O2 with classes: soft and complementary hard acceleration and potential by direct sum (Eq. 5-8 with L287) */
+void p3t_oracle_direct_classes(int64_t n, const double *m, const double *q, const uint8_t *cls, const double *tab,
+                               int64_t ns, const int64_t *subset,
+                               double *acc_soft, double *pot_soft, double *acc_hard, double *pot_hard)
+{
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t k = 0; k < ns; ++k) {
+        int64_t i = subset ? subset[k] : k;
+        nsum as[3] = {{0, 0}, {0, 0}, {0, 0}}, ah[3] = {{0, 0}, {0, 0}, {0, 0}};
+        nsum ps = {0, 0}, ph = {0, 0};
+        for (int64_t j = 0; j < n; ++j) {
+            if (j == i) continue;
+            pairprm p = pair_of(tab, cls, i, j);
+            double d[3] = { q[3 * i] - q[3 * j], q[3 * i + 1] - q[3 * j + 1], q[3 * i + 2] - q[3 * j + 2] };
+            double s2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2] + p.eps2;
+            double s = sqrt(s2), K, W;
+            pair_weights_cls(&p, s, &K, &W);
+            double mr1 = m[j] / s, mr3 = mr1 / s2;
+            for (int c = 0; c < 3; ++c) { nadd(&as[c], -mr3 * K * d[c]); nadd(&ah[c], -mr3 * (1.0 - K) * d[c]); }
+            nadd(&ps, -mr1 * W);
+            nadd(&ph, -mr1 * (1.0 - W));
+        }
+        if (acc_soft) for (int c = 0; c < 3; ++c) acc_soft[3 * k + c] = nval(&as[c]);
+        if (pot_soft) pot_soft[k] = nval(&ps);
+        if (acc_hard) for (int c = 0; c < 3; ++c) acc_hard[3 * k + c] = nval(&ah[c]);
+        if (pot_hard) pot_hard[k] = nval(&ph);
+    }
+}
+
+/* O3 with classes: L_i = { j != i : s_ij < h_kind(i,j) }, every pair of an unsplit kind included.  Same two-pass
+ * convention and band bookkeeping as p3t_oracle_neighbours (the band is around the pair's own h). */
+int64_t p3t_oracle_neighbours_classes(int64_t n, const double *q, const uint8_t *cls, const double *tab,
+                                      int64_t ns, const int64_t *subset,
+                                      int64_t *count, const int64_t *offset, int32_t *list,
+                                      double band, int64_t *band_pairs, int64_t band_cap)
+{
+    int64_t nband = 0;
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t k = 0; k < ns; ++k) {
+        int64_t i = subset ? subset[k] : k;
+        int64_t c = 0;
+        for (int64_t j = 0; j < n; ++j) {
+            if (j == i) continue;
+            pairprm p = pair_of(tab, cls, i, j);
+            double dx = q[3 * i] - q[3 * j], dy = q[3 * i + 1] - q[3 * j + 1], dz = q[3 * i + 2] - q[3 * j + 2];
+            double s = sqrt(dx * dx + dy * dy + dz * dz + p.eps2);
+            if (p.unsplit || s < p.h) {
+                if (list) list[offset[k] + c] = (int32_t)j;
+                ++c;
+            }
+            if (!p.unsplit && band > 0.0 && fabs(s / p.h - 1.0) < band) {
+                int64_t slot;
+#pragma omp atomic capture
+                slot = nband++;
+                if (band_pairs && slot < band_cap) { band_pairs[2 * slot] = k; band_pairs[2 * slot + 1] = j; }
+            }
+        }
+        if (count) count[k] = c;
+    }
+    return nband;
+}
+
+/* O6 with classes: hard acceleration, jerk and potential over ALL j != i with the pair's own numbers; an unsplit
+ * pair contributes the whole (eps_kind-softened) Newtonian term at every separation (1 - K = 1, dK/ds = 0). */
+void p3t_oracle_hard_classes(int64_t n, const double *m, const double *q, const double *v, const uint8_t *cls,
+                             const double *tab, int64_t ns, const int64_t *subset,
+                             double *acc, double *jerk, double *pot)
+{
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t k = 0; k < ns; ++k) {
+        int64_t i = subset ? subset[k] : k;
+        nsum a[3] = {{0, 0}, {0, 0}, {0, 0}}, jk[3] = {{0, 0}, {0, 0}, {0, 0}}, ph = {0, 0};
+        for (int64_t j = 0; j < n; ++j) {
+            if (j == i) continue;
+            pairprm p = pair_of(tab, cls, i, j);
+            double d[3], w[3];
+            for (int c = 0; c < 3; ++c) { d[c] = q[3 * i + c] - q[3 * j + c]; w[c] = v[3 * i + c] - v[3 * j + c]; }
+            double s2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2] + p.eps2;
+            double s = sqrt(s2);
+            if (!p.unsplit && s >= p.r_out) continue;
+            double K, W, dKds = 0.0;
+            pair_weights_cls(&p, s, &K, &W);
+            if (!p.unsplit) {
+                double g = p.r_in / p.r_out;
+                dKds = p3t_oracle_dKdx((s / p.r_out - g) / (1.0 - g)) / (p.r_out * (1.0 - g));
+            }
+            double qv = d[0] * w[0] + d[1] * w[1] + d[2] * w[2];
+            double mr3 = m[j] / (s2 * s);
+            for (int c = 0; c < 3; ++c) {
+                nadd(&a[c], -mr3 * (1.0 - K) * d[c]);
+                nadd(&jk[c], -mr3 * ((1.0 - K) * (w[c] - 3.0 * qv * d[c] / s2) - dKds * (qv / s) * d[c]));
+            }
+            nadd(&ph, -(m[j] / s) * (1.0 - W));
+        }
+        for (int c = 0; c < 3; ++c) {
+            if (acc) acc[3 * k + c] = nval(&a[c]);
+            if (jerk) jerk[3 * k + c] = nval(&jk[c]);
+        }
+        if (pot) pot[k] = nval(&ph);
+    }
+}
+
+/*
+ * O4 with classes.  A cell may stand for its bodies only if every one of them is a plain Newtonian partner (K = W = 1)
+ * of every body of the target box, so clause 3 of R-MAC becomes: for every class ci in the box and every class cj in
+ * the cell, kind (ci, cj) is split and D(B, AABB_C) >= h_kind.  The cell term (R-QUAD) uses ONE softening for all the
+ * bodies of the cell: the split kinds must share their eps (the paper's runs do, L287: "eps = 1e-4 for the
+ * interactions between FS-FS and FS-SMBH"); tab[0] is used.  Leaves: O8 direct terms and list test.
+ */
+typedef struct {
+    walk_state w;
+    const uint8_t *cls; const double *tab; const uint8_t *node_mask;
+    int box_mask;
+} walk_state_cls;
+
+static void walk_rec_cls(walk_state_cls *wc, int32_t id)
+{
+    walk_state *w = &wc->w;
+    const onode *nd = &w->t->node[id];
+    if (nd->count == 0) return;
+    int accept = 0;
+    if (w->theta > 0.0) {
+        double delta = sqrt((nd->c[0] - nd->g[0]) * (nd->c[0] - nd->g[0]) +
+                            (nd->c[1] - nd->g[1]) * (nd->c[1] - nd->g[1]) +
+                            (nd->c[2] - nd->g[2]) * (nd->c[2] - nd->g[2]));
+        double rc = nd->side / w->theta + delta;
+        double d2 = box_point_dist2(w->bmin, w->bmax, nd->c);
+        double D2 = box_box_dist2(w->bmin, w->bmax, nd->bmin, nd->bmax);
+        accept = d2 > rc * rc;
+        for (int ci = 0; ci < 2 && accept; ++ci)
+            for (int cj = 0; cj < 2 && accept; ++cj) {
+                if (!((wc->box_mask >> ci) & 1) || !((wc->node_mask[id] >> cj) & 1)) continue;
+                const double *t = wc->tab + 4 * (ci + cj);
+                if (isinf(t[2]) || !(D2 >= t[3] * t[3])) accept = 0;
+            }
+    }
+    if (accept) {
+        double R[3] = { w->x[0] - nd->c[0], w->x[1] - nd->c[1], w->x[2] - nd->c[2] };
+        double s2 = R[0] * R[0] + R[1] * R[1] + R[2] * R[2] + wc->tab[0] * wc->tab[0];
+        double s = sqrt(s2), s3 = s * s2, s5 = s3 * s2, s7 = s5 * s2;
+        const double *Q = nd->Q;
+        double phi = -nd->M / s;
+        double a[3] = { -nd->M * R[0] / s3, -nd->M * R[1] / s3, -nd->M * R[2] / s3 };
+        if (w->use_quad) {
+            double QR[3] = { Q[0] * R[0] + Q[3] * R[1] + Q[4] * R[2],
+                             Q[3] * R[0] + Q[1] * R[1] + Q[5] * R[2],
+                             Q[4] * R[0] + Q[5] * R[1] + Q[2] * R[2] };
+            double RQR = R[0] * QR[0] + R[1] * QR[1] + R[2] * QR[2];
+            double trQ = Q[0] + Q[1] + Q[2];
+            phi += -0.5 * (3.0 * RQR / s5 - trQ / s3);
+            for (int d = 0; d < 3; ++d)
+                a[d] += 3.0 * QR[d] / s5 - 7.5 * RQR * R[d] / s7 + 1.5 * trQ * R[d] / s5;
+        }
+        for (int d = 0; d < 3; ++d) nadd(&w->a[d], a[d]);
+        nadd(&w->phi, phi);
+        w->n_pc++;
+        return;
+    }
+    if (nd->leaf) {
+        for (int32_t k = 0; k < nd->count; ++k) {
+            int64_t j = w->t->perm[nd->first + k];
+            if (j == w->i) continue;
+            pairprm p = pair_of(wc->tab, wc->cls, w->i, j);
+            double d[3] = { w->x[0] - w->t->q[3 * j], w->x[1] - w->t->q[3 * j + 1], w->x[2] - w->t->q[3 * j + 2] };
+            double s2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2] + p.eps2;
+            double s = sqrt(s2), K, W;
+            pair_weights_cls(&p, s, &K, &W);
+            double mr1 = w->t->m[j] / s, mr3 = mr1 / s2;
+            for (int c = 0; c < 3; ++c) nadd(&w->a[c], -mr3 * K * d[c]);
+            nadd(&w->phi, -mr1 * W);
+            w->n_pp++;
+            if (p.unsplit || s < p.h) {
+                if (w->nbr && w->nbr_n < w->nbr_cap) w->nbr[w->nbr_n] = (int32_t)j;
+                w->nbr_n++;
+            }
+        }
+        return;
+    }
+    for (int o = 0; o < 8; ++o)
+        if (nd->child[o] >= 0) walk_rec_cls(wc, nd->child[o]);
+}
+
+/* Same calling convention as p3t_oracle_tree_walk; box_mask[k] (NULL: the target's own class) is the set of classes,
+ * bit 0 = FS, bit 1 = BH, present in the box of target k. */
+void p3t_oracle_tree_walk_classes(const void *tree, const uint8_t *cls, const double *tab, double theta,
+                                  int use_quad, int64_t ns, const int64_t *subset, const double *box, const uint8_t *box_mask,
+                                  double *acc, double *pot, int64_t *counts,
+                                  int32_t *nbr, int64_t nbr_stride, int64_t *nbr_count)
+{
+    const otree *t = (const otree *)tree;
+    uint8_t *mask = (uint8_t *)calloc((size_t)t->nnode, 1);
+    for (int64_t id = 0; id < t->nnode; ++id)
+        for (int32_t k = 0; k < t->node[id].count; ++k) mask[id] |= (uint8_t)(1u << cls[t->perm[t->node[id].first + k]]);
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t k = 0; k < ns; ++k) {
+        walk_state_cls wc;
+        memset(&wc, 0, sizeof wc);
+        walk_state *w = &wc.w;
+        w->t = t; w->i = subset ? subset[k] : k;
+        for (int d = 0; d < 3; ++d) {
+            w->x[d] = t->q[3 * w->i + d];
+            w->bmin[d] = box ? box[6 * k + d] : w->x[d];
+            w->bmax[d] = box ? box[6 * k + 3 + d] : w->x[d];
+        }
+        w->theta = theta; w->use_quad = use_quad;
+        w->nbr = nbr ? nbr + k * nbr_stride : NULL; w->nbr_cap = nbr_stride;
+        wc.cls = cls; wc.tab = tab; wc.node_mask = mask;
+        wc.box_mask = box_mask ? box_mask[k] : (1 << cls[w->i]);
+        walk_rec_cls(&wc, 0);
+        if (acc) for (int d = 0; d < 3; ++d) acc[3 * k + d] = nval(&w->a[d]);
+        if (pot) pot[k] = nval(&w->phi);
+        if (counts) { counts[2 * k] = w->n_pp; counts[2 * k + 1] = w->n_pc; }
+        if (nbr_count) nbr_count[k] = w->nbr_n;
+        if (w->nbr && w->nbr_n > 1)
+            qsort(w->nbr, (size_t)(w->nbr_n < w->nbr_cap ? w->nbr_n : w->nbr_cap), sizeof(int32_t), cmp_i32);
+    }
+    free(mask);
 }
 
 int p3t_oracle_num_threads(void)

@@ -76,6 +76,15 @@ def lib():
         L.p3t_oracle_hard.argtypes = [i64, pd, pd, pd, d, d, d, i64, pi64, pd, pd, pd]
         L.p3t_oracle_hermite.restype = i64
         L.p3t_oracle_hermite.argtypes = [i64, pd, pd, pd, d, d, d, pi64, pi32, d, i32, d, d, d, i64, pi64, pi64]
+        pu8 = C.POINTER(C.c_uint8)
+        L.p3t_oracle_direct_classes.restype = None
+        L.p3t_oracle_direct_classes.argtypes = [i64, pd, pd, pu8, pd, i64, pi64, pd, pd, pd, pd]
+        L.p3t_oracle_neighbours_classes.restype = i64
+        L.p3t_oracle_neighbours_classes.argtypes = [i64, pd, pu8, pd, i64, pi64, pi64, pi64, pi32, d, pi64, i64]
+        L.p3t_oracle_hard_classes.restype = None
+        L.p3t_oracle_hard_classes.argtypes = [i64, pd, pd, pd, pu8, pd, i64, pi64, pd, pd, pd]
+        L.p3t_oracle_tree_walk_classes.restype = None
+        L.p3t_oracle_tree_walk_classes.argtypes = [vp, pu8, pd, d, i32, i64, pi64, pd, pu8, pd, pd, pi64, pi32, i64, pi64]
         _lib = L
     return _lib
 
@@ -241,6 +250,67 @@ def neighbours_sweep(pos, eps, h, plain=False):
     return offset, lst[: int(offset[-1])]
 
 
+# ---------------------------------------------------------------- O8 -------
+def pair_table(eps, r_in, r_out, h, r_in_bf, r_out_bf, h_bf, eps_bb=0.0, eps_bf=None):
+    """tab[3][4] = (eps, r_in, r_cut, h) for the kinds FS-FS, BH-FS, BH-BH of section 3.2.2.1 (L287); BH-BH is not
+    split (r_cut = inf).  eps_bf defaults to eps (the paper uses one softening for FS-FS and FS-SMBH)."""
+    return np.array([[eps, r_in, r_out, h],
+                     [eps if eps_bf is None else eps_bf, r_in_bf, r_out_bf, h_bf],
+                     [eps_bb, np.inf, np.inf, np.inf]], dtype=np.float64)
+
+
+def _cls(classes):
+    return np.ascontiguousarray(np.asarray(classes), dtype=np.uint8)
+
+
+def direct_classes(mass, pos, classes, tab, subset=None, hard=False):
+    """O2 with a class per body and cutoffs per kind of pair (L287)."""
+    m, q, c, t = _f64(mass), _f64(pos).reshape(-1, 3), _cls(classes), _f64(tab)
+    n = m.shape[0]
+    sub = _subset(subset)
+    ns = n if sub is None else sub.shape[0]
+    a_s, p_s = np.empty((ns, 3)), np.empty(ns)
+    a_h = np.empty((ns, 3)) if hard else None
+    p_h = np.empty(ns) if hard else None
+    d = C.c_double
+    lib().p3t_oracle_direct_classes(n, _p(m, d), _p(q, d), _p(c, C.c_uint8), _p(t, d), ns, _p(sub, C.c_int64),
+                                    _p(a_s, d), _p(p_s, d), _p(a_h, d), _p(p_h, d))
+    return (a_s, p_s, a_h, p_h) if hard else (a_s, p_s)
+
+
+def neighbours_classes(pos, classes, tab, subset=None, band=1e-6):
+    """O3 with the pair's own h; pairs of an unsplit kind are always neighbours."""
+    q, c, t = _f64(pos).reshape(-1, 3), _cls(classes), _f64(tab)
+    n = q.shape[0]
+    sub = _subset(subset)
+    ns = n if sub is None else sub.shape[0]
+    count = np.zeros(ns, dtype=np.int64)
+    d, i64 = C.c_double, C.c_int64
+    L = lib()
+    nb = L.p3t_oracle_neighbours_classes(n, _p(q, d), _p(c, C.c_uint8), _p(t, d), ns, _p(sub, i64),
+                                         _p(count, i64), None, None, float(band), None, 0)
+    offset = np.zeros(ns + 1, dtype=np.int64)
+    np.cumsum(count, out=offset[1:])
+    lst = np.empty(max(int(offset[-1]), 1), dtype=np.int32)
+    bp = np.empty((max(int(nb), 1), 2), dtype=np.int64)
+    L.p3t_oracle_neighbours_classes(n, _p(q, d), _p(c, C.c_uint8), _p(t, d), ns, _p(sub, i64),
+                                    None, _p(offset, i64), _p(lst, C.c_int32), float(band), _p(bp, i64), int(nb))
+    return offset, lst[: int(offset[-1])], bp[: int(nb)]
+
+
+def hard_classes(mass, pos, vel, classes, tab, subset=None):
+    """O6 with classes: (acc, jerk, pot) of the hard part over all j != i."""
+    m, q, v, c, t = _f64(mass), _f64(pos).reshape(-1, 3), _f64(vel).reshape(-1, 3), _cls(classes), _f64(tab)
+    n = m.shape[0]
+    sub = _subset(subset)
+    ns = n if sub is None else sub.shape[0]
+    a, j, p = np.empty((ns, 3)), np.empty((ns, 3)), np.empty(ns)
+    d = C.c_double
+    lib().p3t_oracle_hard_classes(n, _p(m, d), _p(q, d), _p(v, d), _p(c, C.c_uint8), _p(t, d), ns,
+                                  _p(sub, C.c_int64), _p(a, d), _p(j, d), _p(p, d))
+    return a, j, p
+
+
 # ---------------------------------------------------------------- O4 -------
 class Tree:
     """Pointer-based Barnes-Hut octree with monopole + quadrupole moments (L138)."""
@@ -292,4 +362,21 @@ class Tree:
         lib().p3t_oracle_tree_walk(self._h, float(eps), float(theta), float(r_in), float(r_out), float(h),
                                    int(use_quad), ns, _p(sub, i64), _p(bx, d), _p(acc, d), _p(pot, d),
                                    _p(counts, i64), _p(nbr, C.c_int32), int(nbr_stride), _p(nbr_count, i64))
+        return dict(acc=acc, pot=pot, n_pp=counts[:, 0], n_pc=counts[:, 1], nbr_count=nbr_count, nbr=nbr)
+
+    def walk_classes(self, classes, tab, theta, subset=None, box=None, box_mask=None, use_quad=True, nbr_stride=0):
+        """O4 with classes (L287): same outputs as walk()."""
+        sub = _subset(subset)
+        ns = self.n if sub is None else sub.shape[0]
+        acc, pot = np.empty((ns, 3)), np.empty(ns)
+        counts = np.zeros((ns, 2), dtype=np.int64)
+        nbr_count = np.zeros(ns, dtype=np.int64)
+        nbr = np.full((ns, nbr_stride), -1, dtype=np.int32) if nbr_stride else None
+        bx = None if box is None else _f64(box).reshape(ns, 6)
+        bm = None if box_mask is None else _cls(box_mask)
+        c, t = _cls(classes), _f64(tab)
+        d, i64 = C.c_double, C.c_int64
+        lib().p3t_oracle_tree_walk_classes(self._h, _p(c, C.c_uint8), _p(t, d), float(theta), int(use_quad), ns,
+                                           _p(sub, i64), _p(bx, d), _p(bm, C.c_uint8), _p(acc, d), _p(pot, d),
+                                           _p(counts, i64), _p(nbr, C.c_int32), int(nbr_stride), _p(nbr_count, i64))
         return dict(acc=acc, pot=pot, n_pp=counts[:, 0], n_pc=counts[:, 1], nbr_count=nbr_count, nbr=nbr)

@@ -154,7 +154,8 @@ def dr_buff(dt_soft):
 
 
 def config(k, n=None, seed_offset=0):
-    """Workload k = 1..5 of BASELINE.json.  n overrides the particle count
+    """Workload k = 1..5 of BASELINE.json (6: the SMBH-binary workload of PAPER.md L287, for the pair-class row).
+    n overrides the particle count
     (used by tests to run a config's recipe at a size the oracle can afford).
 
     Returns a dict: mass, pos, vel as fp32 arrays (the GPU input; the oracle gets
@@ -192,15 +193,35 @@ def config(k, n=None, seed_offset=0):
         pos, vel = plummer(n, seed)
         mass = np.full(n, 1.0 / n)
         prm = dict(eps=1e-7, theta=0.5, r_out=0.0015, r_search=0.00195, key_bits=63, name="plummer-4m")
+    elif k == 6:
+        # the SMBH-binary workload of section 3.2.2.1, not one of BASELINE.json's five: a Plummer model
+        # of n field stars (mass 1 in all) plus two black holes of mass 0.01 at (+-0.5, 0, 0) with velocities
+        # (0, +-0.5, 0); r_cut = 1/256 between field stars, 1/32 between a black hole and a field star, black hole
+        # pairs not split; eps = 1e-4 (0 between the black holes); dt_soft = 1/1024, dr_buff = 3 sigma dt_soft
+        nfs = n or 16384
+        pos, vel = plummer(nfs, seed)
+        mass = np.full(nfs, 1.0 / nfs)
+        pos, vel = _recentre(mass, pos, vel)
+        pos = np.concatenate([pos, [[0.5, 0.0, 0.0], [-0.5, 0.0, 0.0]]])
+        vel = np.concatenate([vel, [[0.0, 0.5, 0.0], [0.0, -0.5, 0.0]]])
+        mass = np.concatenate([mass, [0.01, 0.01]])
+        n = nfs + 2
+        dt = 1.0 / 1024.0
+        prm = dict(eps=1e-4, theta=0.4, r_out=1.0 / 256.0, r_search=1.0 / 256.0 + dr_buff(dt), dt_soft=dt, key_bits=63,
+                   name="plummer-16k-smbh-binary", classes=np.concatenate([np.zeros(nfs, np.uint8), np.ones(2, np.uint8)]),
+                   class_params=dict(r_in_bf=0.1 / 32.0, r_out_bf=1.0 / 32.0, r_search_bf=1.0 / 32.0 + dr_buff(dt), eps_bb=0.0))
     else:
-        raise ValueError("config must be 1..5")
-    pos, vel = _recentre(mass, pos, vel)
+        raise ValueError("config must be 1..6")
+    if k != 6:
+        pos, vel = _recentre(mass, pos, vel)
     prm["r_in"] = 0.1 * prm["r_out"]      # gamma = 0.1 in all runs (Table 1)
     # i-groups of 32 below ~100K particles (more, lighter groups fill the GPU better and their boxes are smaller), 64 above
     prm.update(nleaf=16, ngroup=32 if n < 100000 else 64, n=n, config=k)
     # fp32 parameters: what the C ABI receives; the oracle gets these same values
     for key in ("eps", "theta", "r_in", "r_out", "r_search"):
         prm[key] = float(np.float32(prm[key]))
+    if "class_params" in prm:
+        prm["class_params"] = {key: float(np.float32(v)) for key, v in prm["class_params"].items()}
     prm["mass"] = mass.astype(np.float32)
     prm["pos"] = np.ascontiguousarray(pos.astype(np.float32))
     prm["vel"] = np.ascontiguousarray(vel.astype(np.float32))
