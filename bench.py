@@ -8,11 +8,14 @@ synthetic input: load -> bounding cube, Morton keys, radix sort, gather -> octre
 moments -> group walk + interactions -> neighbour CSR.  The default workload is BASELINE.json
 configs[2] (the N = 1,048,576 Salpeter-mass Plummer sphere the metric is quoted on).
 
-Timing: every step is bracketed by CUDA events on the stream the library launches on; between
-steps the L2 is flushed by writing a 512 MiB buffer (the 16 MB input is far smaller than the 126 MB
-L2); ms_per_step is the mean over the K timed steps; with N > 1 ranks each rank evaluates its own
-independent cluster (weak scaling, no data-path collective) and the slowest rank's time is used.
-Prints ONE JSON line on rank 0.
+Timing: every step is bracketed by CUDA events on the stream the library launches on and ends with the
+accelerations and potentials in the caller's device arrays (p3t_get_acc_pot, the "output in user order" half
+of row a9); between steps the L2 is flushed by writing a 512 MiB buffer (the 16 MB input is far smaller
+than the 126 MB L2) and the bodies are moved by one leapfrog step dt_soft with the returned forces (torch
+ops, outside the event window), so that the walk's cost-ordered hand-out of the groups works from a
+PREDICTION, as it does inside an integration; ms_per_step is the mean over the K timed steps; with N > 1
+ranks each rank evaluates its own independent cluster (weak scaling, no data-path collective) and the
+slowest rank's time is used.  Prints ONE JSON line on rank 0.
 """
 from __future__ import annotations
 
@@ -62,7 +65,7 @@ class ClockSampler:
         self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
         try:
             self.p = subprocess.Popen(["nvidia-smi", f"--query-gpu={CLOCK_QUERY}", "--format=csv,noheader,nounits",
-                                       "-lms", "20", "-i", str(index)], stdout=self.f, stderr=subprocess.DEVNULL)
+                                       "-lms", "10", "-i", str(index)], stdout=self.f, stderr=subprocess.DEVNULL)
         except OSError:
             self.p = None
 
@@ -159,6 +162,9 @@ def main():
                          "accelerations and potentials are summed over the ranks (NCCL all-reduce inside the timed step)")
     ap.add_argument("--walk-mode", type=int, default=None, help="p3t_set_walk_mode: 0 auto, 1 warp per group, 2 CTA per group")
     ap.add_argument("--n", type=int, default=None, help="override the particle count (not a bench value)")
+    ap.add_argument("--same-positions", action="store_true", help="do not move the bodies between steps (not the headline case)")
+    ap.add_argument("--settle", type=float, default=1.2, help="seconds of untimed steps before the warm-up (clock sampler)")
+    ap.add_argument("--refit", type=int, default=0, help="tree reuse: p3t_refit_tree with a rebuild every REFIT calls (not the headline case)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -200,37 +206,54 @@ def main():
 
     if shard:
         ctx.set_shard(rank, world)
-        acc_d = torch.empty((n, 3), dtype=torch.float32, device=dev)
-        pot_d = torch.empty(n, dtype=torch.float32, device=dev)
+    acc_d = torch.empty((n, 3), dtype=torch.float32, device=dev)
+    pot_d = torch.empty(n, dtype=torch.float32, device=dev)
+    if args.refit:
+        ctx.set_tree_reuse(args.refit)
 
     def step():
         ctx.load_particles(mass_d, pos_d)
-        ctx.build_tree()
+        if args.refit:
+            ctx.refit_tree()           # rebuilds by itself every args.refit calls or when too many bodies have strayed
+        else:
+            ctx.build_tree()
         ctx.eval_soft()
+        ctx.get_acc_pot_into(acc_d, pot_d)   # a9: accelerations and potentials in user order, in the caller's arrays
         if shard:      # every rank ends the step with the accelerations and potentials of all particles
-            ctx.get_acc_pot_into(acc_d, pot_d)
             multi.allreduce_forces(dist, acc_d, pot_d)
 
-    # the clock sampler starts with the warm-up steps (nvidia-smi needs a few hundred ms to deliver its first sample;
-    # the warm-up steps are the same load as the timed ones) and runs to the end of the timed region
+    # Between steps the bodies move by one leapfrog step with the returned forces (BASELINE.json configs[1] asks for it
+    # in so many words: "positions are drifted by a leapfrog step dt_soft using the returned forces"; for the other
+    # configs it makes the timed case the one an integration sees).  Torch ops on the device, outside the event window.
+    dt_soft = cfg.get("dt_soft") or 1.0 / 1024.0
+    drift = not shard and not args.same_positions
+    vel_l = torch.from_numpy(cfg["vel"]).to(dev)
+    pos_d = pos_d.clone()
+
+    def move():
+        if drift:
+            vel_l.add_(acc_d, alpha=dt_soft)
+            pos_d.add_(vel_l, alpha=dt_soft)
+
+    # The clock sampler (nvidia-smi every 10 ms; its first sample takes a few hundred ms) runs from here to the end of
+    # the timed region.  Small configs finish W + K steps before it delivers ten samples, so the same step first runs
+    # untimed until 1.2 s have passed (same load as the timed steps), then the W warm-up steps, then the K timed ones.
     sampler = ClockSampler(local) if rank == 0 else None
+    settle_steps, t_settle = 0, time.perf_counter()
+    while time.perf_counter() - t_settle < args.settle:
+        step()
+        ctx.synchronize()
+        settle_steps += 1
     for _ in range(args.warmup):
         flush.zero_()
         step()
+        move()
     ctx.synchronize()
     if dist:
         dist.barrier()
     torch.cuda.synchronize()
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     phases = {k: [] for k in ("ms_pack", "ms_sort", "ms_build", "ms_moments", "ms_walk", "ms_nbr")}
-    # BASELINE.json configs[1]: consecutive calls "while positions are drifted by a leapfrog step dt_soft using the
-    # returned forces" -- the kick and drift run between the timed steps (torch ops on the device, not timed)
-    drift = cfg.get("dt_soft") is not None and not shard
-    if drift:
-        vel_l = torch.from_numpy(cfg["vel"]).to(dev)
-        acc_l = torch.empty((n, 3), dtype=torch.float32, device=dev)
-        pot_l = torch.empty(n, dtype=torch.float32, device=dev)
-        pos_d = pos_d.clone()
     for a, b in ev:
         flush.zero_()
         a.record()
@@ -239,10 +262,7 @@ def main():
         st = ctx.get_stats()           # synchronises; per-phase times come from the library's own CUDA events
         for k in phases:
             phases[k].append(st[k])
-        if drift:
-            ctx.get_acc_pot_into(acc_l, pot_l)
-            vel_l += cfg["dt_soft"] * acc_l
-            pos_d += cfg["dt_soft"] * vel_l
+        move()
     torch.cuda.synchronize()
     if dist:
         dist.barrier()
@@ -252,12 +272,34 @@ def main():
         total_n = n      # one cluster, not one per rank
     st = ctx.get_stats()
     ph = {k: float(np.mean(v)) for k, v in phases.items()}
+    # secondary key: the same step with the positions of the last timed step repeated (the group order is then a
+    # perfect prediction: the favourable case round 1 quoted)
+    same_ms = None
+    if drift and rank == 0:
+        ts = []
+        for _ in range(1 + min(args.steps, 5)):
+            flush.zero_()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); step(); e1.record()
+            torch.cuda.synchronize()
+            ts.append((e0.elapsed_time(e1), ctx.get_stats()["ms_walk"]))
+        same_ms = {"ms_per_step": float(np.mean([t[0] for t in ts[1:]])), "ms_walk": float(np.mean([t[1] for t in ts[1:]]))}
     ffma_scalar = ffma_packed = None
     nbr_hist = None
     if rank == 0:      # neighbour-list length histogram of the last step (BASELINE.json config 4 asks for it)
         cnt, _ = ctx.get_neighbour_counts()
         hh = np.bincount(np.minimum(cnt, 16), minlength=17)
         nbr_hist = {"length_0..15_and_16+": [int(x) for x in hh], "max": int(cnt.max()), "mean": float(cnt.mean())}
+    tree_hist = None
+    if rank == 0:      # depth / leaf-occupancy histograms of the last tree
+        meta, lev = ctx.array("cell_meta"), ctx.array("cell_level")
+        leaf = (meta[:, 1] & 0x80000000) != 0
+        occ = (meta[leaf, 1] & 0x7fffffff).astype(np.int64)
+        tree_hist = {"leaves_per_level": [int(x) for x in np.bincount(lev[leaf], minlength=st["depth"] + 1)],
+                     "cells_per_level": [int(x) for x in np.bincount(lev, minlength=st["depth"] + 1)],
+                     "leaf_occupancy_1..nleaf_and_above": [int(x) for x in np.bincount(np.minimum(occ, nleaf + 1), minlength=nleaf + 2)[1:]],
+                     "bodies_per_leaf_level": [int(x) for x in np.bincount(lev[leaf], weights=occ, minlength=st["depth"] + 1)],
+                     "mean_leaf_occupancy": float(occ.mean()), "max_leaf_occupancy": int(occ.max())}
     if rank == 0:      # pure-FFMA calibration kernel, outside the timed region
         ffma_scalar, ffma_packed = ctx.measure_fp32_peak(False)[0], ctx.measure_fp32_peak(True)[0]
 
@@ -353,7 +395,7 @@ def main():
     hbm = {k: ab[k] / (ph["ms_" + k] * 1e-3) / 1e9 for k in ab}
     tree_ms = ph["ms_pack"] + ph["ms_sort"] + ph["ms_build"] + ph["ms_moments"]
     # pack | keys+hist, onesweep passes, gather | levels, emit | moments (leaves, internal) | group prediction + order, walk | neighbour CSR (6)
-    launches = 1 + (1 + st["sort_passes"] + 1) + 2 + 2 + (3 if not shard else 1) + 6
+    launches = 1 + (1 + st["sort_passes"] + 1) + 2 + 2 + (3 if not shard else 1) + 6 + 1      # ... + unpack (get_acc_pot)
 
     out = {
         "metric": METRIC, "value": multi.throughput(total_n, ms), "unit": "particles/s", "n_gpus": world, "steps": args.steps,
@@ -361,17 +403,19 @@ def main():
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": cfg["name"], "n": n, "theta": cfg["theta"], "eps": cfg["eps"], "r_out": cfg["r_out"],
                    "r_search": cfg["r_search"], "key_bits": cfg["key_bits"], "nleaf": nleaf, "ngroup": ngroup,
-                   "l2": "flushed between steps (512 MiB write)", "positions": "drifted between steps (leapfrog, dt_soft)" if drift else "same every step", "parallelism": (f"one cluster sharded over {world} GPUs by i-groups, all-reduce of the results" if shard
+                   "l2": "flushed between steps (512 MiB write)", "positions": f"drifted between steps (leapfrog with the returned forces, dt_soft = 1/{round(1 / dt_soft)})" if drift else "same every step",
+                   "timed_region": "load_particles + build_tree + eval_soft + get_acc_pot (device arrays)", "clock_settle_steps": settle_steps, "parallelism": (f"one cluster sharded over {world} GPUs by i-groups, all-reduce of the results" if shard
                                    else f"{world} independent cluster(s), one per GPU")},
         "interactions_per_s": (st["n_pp"] + st["n_pc"]) / (ph["ms_walk"] * 1e-3),
         "walk_particles_per_s": n / (ph["ms_walk"] * 1e-3),
         "interactions": {"n_pp": st["n_pp"], "n_pc": st["n_pc"], "n_near": st["n_near"], "n_neighbours": st["n_neighbours"],
                          "pp_per_particle": st["n_pp"] / n, "pc_per_particle": st["n_pc"] / n},
-        "tree": {"n_cells": st["n_cells"], "n_leaves": st["n_leaves"], "n_groups": st["n_groups"], "depth": st["depth"]},
+        "tree": {"n_cells": st["n_cells"], "n_leaves": st["n_leaves"], "n_groups": st["n_groups"], "depth": st["depth"], "histograms": tree_hist},
+        "same_positions": same_ms,
         "neighbour_lists": nbr_hist, "workspace_bytes": int(ctx.workspace.numel()),
         "phases_ms": ph,
         "roofline": {"bound": "alu", "kernel": "walk_kernel (a7+a8)", "achieved": walk_tflops, "peak": fp32_peak, "unit": "TFLOP/s",
-                     "frac": walk_tflops / fp32_peak, "traffic": traffic, "traffic_source": traffic_src,
+                     "frac": walk_tflops / fp32_peak, "traffic": None, "traffic_committed_capture": traffic, "traffic_source": traffic_src,
                      "peak_source": f"2 flop x {FP32_LANES} lanes x {n_sm} SMs x {peaks['sm_max_mhz']:.0f} MHz ({peaks['source']} sm_max_mhz; DESIGN.md section 8)",
                      "convention": f"{FLOP_PP} flop per p-p, {FLOP_PC} flop per p-c",
                      "ffma_microbench_tflops": {"scalar": ffma_scalar, "packed": ffma_packed},

@@ -74,6 +74,8 @@ typedef struct {
     float ms_nbr;            /* a9 */
     float ms_hard;           /* last p3t_eval_hard */
     float ms_pack;           /* a1: pack + bounding cube of the last p3t_load_particles (after any host-to-device copy) */
+    uint32_t tree_refits;    /* p3t_refit_tree: refits since the last full build (0: the current tree is a fresh build) */
+    uint32_t n_stray;        /* of the current refit: bodies outside the cube of their leaf by more than stray_dist leaf sides */
 } p3t_stats;
 
 /* Bytes of device workspace p3t_create needs for up to max_n particles,
@@ -133,6 +135,23 @@ p3t_status p3t_load_particles(p3t_ctx *ctx, size_t n, const float *mass, const f
 /* a1-a6: bounding cube, Morton keys, radix sort, body gather, octree + groups,
  * moments (mass, centre of mass, quadrupole, acceptance radius). */
 p3t_status p3t_build_tree(p3t_ctx *ctx);
+
+/* Tree reuse between soft steps (PAPER.md L27-29 (section 1): "the cost of the usual complete
+ * reconstruction of the tree is O(N log N) and not negligible"; the cost model counts one tree per soft step, L193 and
+ * Eq. 28).  p3t_refit_tree replaces p3t_build_tree after a p3t_load_particles of the SAME particles (same n, same
+ * order) at moved positions: sorted order, cells and i-groups of the last full build are kept; bodies are gathered again
+ * and moments, tight boxes and acceptance radii are made from the new positions on the old topology (no keys, no sort,
+ * no build).  Results keep the guarantees of a fresh tree -- accepted cells hold no body within r_search of the group
+ * (lists exact), and the opening test uses, for a cell whose bodies have left its cube, the side of the smallest cube
+ * about the cell's geometric centre that holds them -- what degrades is only how tight cells and groups are, i.e. the
+ * number of interactions.  The call counts on the device the bodies that sit outside the cube of their leaf by more than
+ * stray_dist leaf sides; if they are more than max_stray_fraction * n, or max_refits refits have been made since the
+ * last build, or there is no tree to reuse (first call, n or tree parameters changed), the call does a full
+ * p3t_build_tree instead.  It synchronises the stream once (to read the count).  p3t_set_params may change between refits.
+ * Defaults: max_refits = 0 (p3t_refit_tree always rebuilds; p3t_step uses this call, so it rebuilds every step unless
+ * reuse is switched on), stray_dist = 0.5, max_stray_fraction = 0.02.  P3T_EINVAL for negative or non-finite values. */
+p3t_status p3t_set_tree_reuse(p3t_ctx *ctx, int max_refits, float stray_dist, float max_stray_fraction);
+p3t_status p3t_refit_tree(p3t_ctx *ctx);
 
 /* a7-a9: group walk, interactions, neighbour lists.  Needs a tree built for the
  * loaded positions and current parameters. */

@@ -28,7 +28,7 @@ _STATUS = {0: "P3T_OK", -1: "P3T_EINVAL", -2: "P3T_ESTATE", -3: "P3T_ENOMEM", -4
 # names of include/p3t.h's exported entry points (tests check that each resolves)
 SYMBOLS = [
     "p3t_workspace_bytes", "p3t_create", "p3t_destroy", "p3t_set_params", "p3t_set_tree_params",
-    "p3t_set_group_merge_levels", "p3t_set_walk_mode", "p3t_set_shard", "p3t_load_particles", "p3t_build_tree", "p3t_eval_soft", "p3t_eval_direct", "p3t_eval_hard",
+    "p3t_set_group_merge_levels", "p3t_set_walk_mode", "p3t_set_shard", "p3t_load_particles", "p3t_build_tree", "p3t_set_tree_reuse", "p3t_refit_tree", "p3t_eval_soft", "p3t_eval_direct", "p3t_eval_hard",
     "p3t_hermite_step", "p3t_step", "p3t_set_hermite_cluster_max",
     "p3t_get_acc_pot", "p3t_get_neighbour_counts", "p3t_get_neighbours", "p3t_get_stats", "p3t_synchronize",
     "p3t_last_error", "p3t_array_info", "p3t_copy_array", "p3t_measure_fp32_peak",
@@ -46,7 +46,8 @@ class Stats(C.Structure):
                 ("n_neighbours", C.c_uint64), ("n_cells", C.c_uint32), ("n_leaves", C.c_uint32),
                 ("n_groups", C.c_uint32), ("depth", C.c_uint32), ("max_list", C.c_uint32),
                 ("sort_passes", C.c_uint32), ("ms_sort", C.c_float), ("ms_build", C.c_float),
-                ("ms_moments", C.c_float), ("ms_walk", C.c_float), ("ms_nbr", C.c_float), ("ms_hard", C.c_float), ("ms_pack", C.c_float)]
+                ("ms_moments", C.c_float), ("ms_walk", C.c_float), ("ms_nbr", C.c_float), ("ms_hard", C.c_float), ("ms_pack", C.c_float),
+                ("tree_refits", C.c_uint32), ("n_stray", C.c_uint32)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
@@ -75,6 +76,8 @@ def _sig():
     L.p3t_load_particles.restype = i; L.p3t_load_particles.argtypes = [vp, sz, vp, vp, i]
     L.p3t_build_tree.restype = i; L.p3t_build_tree.argtypes = [vp]
     L.p3t_eval_soft.restype = i; L.p3t_eval_soft.argtypes = [vp]
+    L.p3t_refit_tree.restype = i; L.p3t_refit_tree.argtypes = [vp]
+    L.p3t_set_tree_reuse.restype = i; L.p3t_set_tree_reuse.argtypes = [vp, i, f, f]
     L.p3t_eval_direct.restype = i; L.p3t_eval_direct.argtypes = [vp, vp, sz, i]
     L.p3t_eval_hard.restype = i; L.p3t_eval_hard.argtypes = [vp, vp, vp, vp, vp, i]
     d, ll = C.c_double, C.c_longlong
@@ -202,6 +205,12 @@ class P3T:
 
     def eval_soft(self):
         self._check(_lib.p3t_eval_soft(self._h))
+
+    def set_tree_reuse(self, max_refits, stray_dist=0.5, max_stray_fraction=0.02):
+        self._check(_lib.p3t_set_tree_reuse(self._h, int(max_refits), stray_dist, max_stray_fraction))
+
+    def refit_tree(self):
+        self._check(_lib.p3t_refit_tree(self._h))
 
     def eval_direct(self, subset=None):
         if subset is None:

@@ -136,6 +136,9 @@ extern "C" p3t_status p3t_create(p3t_ctx **out, int device, size_t max_n, int ke
     ctx->herm_cluster_max = 4096;
     ctx->shard_rank = 0;
     ctx->shard_world = 1;
+    ctx->max_refits = 0;
+    ctx->stray_dist = 0.5f;
+    ctx->max_stray_fraction = 0.02f;
     cudaError_t e = cudaSetDevice(device);
     cudaDeviceProp prop;
     if (e == cudaSuccess) e = cudaGetDeviceProperties(&prop, device);
@@ -152,6 +155,7 @@ extern "C" p3t_status p3t_create(p3t_ctx **out, int device, size_t max_n, int ke
     }
     ctx->base = static_cast<char *>(workspace);
     if (cudaMemsetAsync(ctx->ws.order_meta, 0, 4 * sizeof(u32), ctx->stream) != cudaSuccess) { delete ctx; return P3T_ECUDA; }
+    if (cudaMemsetAsync(ctx->ws.counters, 0, CNT_WORDS * sizeof(u64), ctx->stream) != cudaSuccess) { delete ctx; return P3T_ECUDA; }
     if (cudaMemsetAsync(ctx->ws.body_class, 0, max_n * sizeof(u32), ctx->stream) != cudaSuccess) { delete ctx; return P3T_ECUDA; }   // no history: one class, Morton order
     for (int i = 0; i < 14; ++i) {
         if (cudaEventCreate(&ctx->ev[i]) != cudaSuccess) { delete ctx; return P3T_ECUDA; }
@@ -235,6 +239,7 @@ extern "C" p3t_status p3t_set_tree_params(p3t_ctx *ctx, int nleaf, int ngroup)
     ctx->ngroup = ngroup;
     ctx->built = false;
     ctx->evaluated = false;
+    ctx->topo_valid = false;
     return P3T_OK;
 }
 
@@ -246,6 +251,7 @@ extern "C" p3t_status p3t_set_group_merge_levels(p3t_ctx *ctx, int levels)
     ctx->merge_levels = levels;
     ctx->built = false;
     ctx->evaluated = false;
+    ctx->topo_valid = false;
     return P3T_OK;
 }
 
@@ -341,6 +347,7 @@ extern "C" p3t_status p3t_build_tree(p3t_ctx *ctx)
     P3T_CUDA(ctx, cudaSetDevice(ctx->device));
     ctx->built = false;
     ctx->evaluated = false;
+    ctx->topo_valid = false;
     p3t_status st;
     P3T_CUDA(ctx, cudaEventRecord(ctx->ev[0], ctx->stream));
     if ((st = p3t_stage_sort(ctx)) != P3T_OK) return st;
@@ -351,6 +358,54 @@ extern "C" p3t_status p3t_build_tree(p3t_ctx *ctx)
     P3T_CUDA(ctx, cudaEventRecord(ctx->ev[3], ctx->stream));
     ctx->ev_build = true;
     ctx->built = true;
+    ctx->topo_valid = true;
+    ctx->topo_n = ctx->n;
+    ctx->refits = 0;
+    ctx->last_rebuilt = true;
+    ctx->last_stray = 0;
+    return P3T_OK;
+}
+
+static p3t_status sync_and_check(p3t_ctx *ctx);
+
+// Tree reuse between soft steps (first half, cost per soft step L193, Eq. 28)
+extern "C" p3t_status p3t_set_tree_reuse(p3t_ctx *ctx, int max_refits, float stray_dist, float max_stray_fraction)
+{
+    if (!ctx) return P3T_EINVAL;
+    if (max_refits < 0 || !(stray_dist >= 0.f) || !(max_stray_fraction >= 0.f) || !isfinite(stray_dist) || !isfinite(max_stray_fraction))
+        return p3t_fail(ctx, P3T_EINVAL, "need max_refits >= 0, stray_dist >= 0, max_stray_fraction >= 0");
+    ctx->max_refits = max_refits;
+    ctx->stray_dist = stray_dist;
+    ctx->max_stray_fraction = max_stray_fraction;
+    return P3T_OK;
+}
+
+extern "C" p3t_status p3t_refit_tree(p3t_ctx *ctx)
+{
+    if (!ctx) return P3T_EINVAL;
+    if (!ctx->loaded) return p3t_fail(ctx, P3T_ESTATE, "p3t_refit_tree before p3t_load_particles");
+    if (!ctx->have_params) return p3t_fail(ctx, P3T_ESTATE, "p3t_refit_tree before p3t_set_params");
+    // no tree of these particles to reuse, or enough refits in a row: a full build
+    if (!ctx->topo_valid || ctx->topo_n != ctx->n || ctx->refits >= ctx->max_refits) return p3t_build_tree(ctx);
+    P3T_CUDA(ctx, cudaSetDevice(ctx->device));
+    ctx->built = false;
+    ctx->evaluated = false;
+    p3t_status st;
+    P3T_CUDA(ctx, cudaEventRecord(ctx->ev[0], ctx->stream));
+    if ((st = p3t_stage_refit_begin(ctx)) != P3T_OK) return st;
+    // the stray count decides between finishing the refit and rebuilding: one small copy and a stream synchronisation
+    // (the leaf moments are already enqueued behind the gather, so the device does not idle while the host decides)
+    if ((st = sync_and_check(ctx)) != P3T_OK) return st;
+    ctx->last_stray = ctx->h_counters[CNT_STRAY];
+    if ((double)ctx->last_stray > (double)ctx->max_stray_fraction * (double)ctx->n) return p3t_build_tree(ctx);
+    P3T_CUDA(ctx, cudaEventRecord(ctx->ev[1], ctx->stream));
+    P3T_CUDA(ctx, cudaEventRecord(ctx->ev[2], ctx->stream));
+    if ((st = p3t_stage_refit_finish(ctx)) != P3T_OK) return st;
+    P3T_CUDA(ctx, cudaEventRecord(ctx->ev[3], ctx->stream));
+    ctx->ev_build = true;
+    ctx->built = true;
+    ctx->refits += 1;
+    ctx->last_rebuilt = false;
     return P3T_OK;
 }
 
@@ -398,8 +453,6 @@ extern "C" p3t_status p3t_eval_direct(p3t_ctx *ctx, const uint32_t *i_subset, si
     ctx->lists_complete = i_subset == nullptr;     // a subset leaves the other particles' lists empty
     return P3T_OK;
 }
-
-static p3t_status sync_and_check(p3t_ctx *ctx);
 
 // NEXT row: hard acceleration, jerk and potential from the neighbour lists
 extern "C" p3t_status p3t_eval_hard(p3t_ctx *ctx, const float *vel, double *acc, double *jerk, double *pot, int on_device)
@@ -536,7 +589,7 @@ extern "C" p3t_status p3t_step(p3t_ctx *ctx, const float *mass, double *pos, dou
     if (st != P3T_OK) return st;
     if ((st = p3t_stage_narrow(ctx, d_pos, ctx->ws.in_pos)) != P3T_OK) return st;              // step 4: soft force at t + dt
     if ((st = p3t_load_particles(ctx, n, d_mass, ctx->ws.in_pos, 1)) != P3T_OK) return st;
-    if ((st = p3t_build_tree(ctx)) != P3T_OK) return st;
+    if ((st = p3t_refit_tree(ctx)) != P3T_OK) return st;      // a full build unless p3t_set_tree_reuse allows refits
     if ((st = p3t_eval_soft(ctx)) != P3T_OK) return st;
     if ((st = p3t_stage_kick(ctx, d_vel, 0.5 * dt_soft)) != P3T_OK) return st;
     if (!on_device) {
@@ -557,7 +610,7 @@ static p3t_status sync_and_check(p3t_ctx *ctx)
     P3T_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     if (ctx->h_counters[CNT_NONFINITE]) return p3t_fail(ctx, P3T_EINVAL, "non-finite mass or position in the device input");
     u64 f = ctx->h_counters[CNT_ERR_BUILD] | ctx->h_counters[CNT_ERR_EVAL];
-    if (ctx->h_counters[CNT_ERR_BUILD]) ctx->cells_dirty = true;
+    if (ctx->h_counters[CNT_ERR_BUILD]) { ctx->cells_dirty = true; ctx->topo_valid = false; }
     if (f & ERR_CELL_CAPACITY) return p3t_fail(ctx, P3T_ENOMEM, "octree cell capacity (3 n + 1024) exceeded");
     if (f & ERR_STACK_OVERFLOW) return p3t_fail(ctx, P3T_ENOMEM, "tree-walk stack overflow");
     if (ctx->hard_unchecked) {
@@ -652,6 +705,8 @@ extern "C" p3t_status p3t_get_stats(p3t_ctx *ctx, p3t_stats *out)
     }
     if (ctx->ev_hard) cudaEventElapsedTime(&out->ms_hard, ctx->ev[7], ctx->ev[8]);
     if (ctx->ev_pack) cudaEventElapsedTime(&out->ms_pack, ctx->ev[9], ctx->ev[10]);
+    out->tree_refits = (u32)ctx->refits;
+    out->n_stray = (u32)(ctx->last_rebuilt ? 0 : ctx->last_stray);
     return st;
 }
 

@@ -29,6 +29,7 @@ struct Mom {
     float lox, loy, loz, hix, hiy, hiz;
 };
 
+template <bool REFIT>
 __device__ __forceinline__ void store_cell(u32 k, const Mom &m, int level, u64 key, const float *__restrict__ cube,
                                            int max_level, float theta, float h, float4 *cell_mac, float4 *cell_mom0,
                                            float4 *cell_mom1, float4 *cell_bmin, float4 *cell_bmax)
@@ -47,7 +48,15 @@ __device__ __forceinline__ void store_cell(u32 k, const Mom &m, int level, u64 k
     float rmax = sqrtf(fx * fx + fy * fy + fz * fz) * (1.f + 1e-6f);
     float slack = 8.f * 1.1920929e-7f * (fabsf(cube[0]) + fabsf(cube[1]) + fabsf(cube[2]) + 2.f * side);
     float rc3 = (h + rmax) * (1.f + 1e-5f) + slack;
-    float rc1 = theta > 0.f ? l / theta + delta : INFINITY;
+    // Refit (p3t_refit_tree): the bodies have moved since the keys were made and may sit outside the cell's cube; the
+    // opening test then takes the side of the smallest cube about the geometric centre that holds them all, which
+    // keeps the geometric meaning of l / theta (for bodies inside the cube nothing changes).
+    float lm = l;
+    if (REFIT) {
+        const float ox = fmaxf(gx - m.lox, m.hix - gx), oy = fmaxf(gy - m.loy, m.hiy - gy), oz = fmaxf(gz - m.loz, m.hiz - gz);
+        lm = fmaxf(l, 2.f * fmaxf(ox, fmaxf(oy, oz)) * (1.f + 1e-6f));
+    }
+    float rc1 = theta > 0.f ? lm / theta + delta : INFINITY;
     float rc = fmaxf(rc1, rc3);
     cell_mac[k] = make_float4(m.cx, m.cy, m.cz, rc * rc);
     cell_mom0[k] = make_float4(m.M, m.qxx, m.qyy, m.qzz);
@@ -101,7 +110,7 @@ __device__ __forceinline__ void merge_children(u32 first, u32 nch, const float4 
 //   merge go to L2, so no acquire (L1 invalidation) is needed.  Children are merged in index order:
 //   the result is deterministic.  The counters are read-only here (a late thread must still see whether
 //   its cell waits for children); keys_hist_kernel of the next build zeroes them.
-template <int PHASE>
+template <int PHASE, bool REFIT>
 __global__ void __launch_bounds__(128, 4) moments_kernel(
     const float4 *__restrict__ body, const u64 *__restrict__ keys, const float *__restrict__ cube,
     const u8 *__restrict__ cell_level, const u32 *__restrict__ cell_start, const u32 *__restrict__ cell_parent,
@@ -155,7 +164,7 @@ __global__ void __launch_bounds__(128, 4) moments_kernel(
                 m.cx = 0.5f * (m.lox + m.hix); m.cy = 0.5f * (m.loy + m.hiy); m.cz = 0.5f * (m.loz + m.hiz);
                 m.qxx = m.qyy = m.qzz = m.qxy = m.qxz = m.qyz = 0.f;
             }
-            store_cell(k, m, level, keys[start], cube, max_level, theta, h, cell_mac, cell_mom0, cell_mom1, cell_bmin, cell_bmax);
+            store_cell<REFIT>(k, m, level, keys[start], cube, max_level, theta, h, cell_mac, cell_mom0, cell_mom1, cell_bmin, cell_bmax);
             continue;
         }
         // ---- internal cell
@@ -175,7 +184,7 @@ __global__ void __launch_bounds__(128, 4) moments_kernel(
             }
             merge_children(first, nch, cell_mac, cell_mom0, cell_mom1, cell_bmin, cell_bmax, m);
             const u64 pkey = parent != P3T_NO_PARENT ? keys[pstart] : 0ull;
-            store_cell(k, m, level, key, cube, max_level, theta, h, cell_mac, cell_mom0, cell_mom1, cell_bmin, cell_bmax);
+            store_cell<REFIT>(k, m, level, key, cube, max_level, theta, h, cell_mac, cell_mom0, cell_mom1, cell_bmin, cell_bmax);
             cell_meta[k] = make_uint2(first, nch);
             if (parent == P3T_NO_PARENT) break;
             __threadfence();             // my record is visible before my arrival is
@@ -193,14 +202,86 @@ p3t_status p3t_stage_moments(p3t_ctx *ctx)
     size_t bound = ctx->n * (size_t)(ctx->max_level + 1);
     if (bound > w.cell_cap) bound = w.cell_cap;
     const u32 grid = (u32)min((size_t)div_up(bound, 128), (size_t)ctx->sm_count * 16);
-    moments_kernel<0><<<grid, 128, 0, s>>>(w.body, w.keys[ctx->cur], w.cube, w.cell_level, w.cell_start, w.cell_parent, w.cell_first,
+    moments_kernel<0, false><<<grid, 128, 0, s>>>(w.body, w.keys[ctx->cur], w.cube, w.cell_level, w.cell_start, w.cell_parent, w.cell_first,
                                            w.cell_nchild, w.cell_ready, w.cell_meta, w.cell_mac, w.cell_mom0, w.cell_mom1,
                                            w.cell_bmin, w.cell_bmax, w.counters, (u32)w.cell_cap, ctx->max_level, ctx->prm.theta,
                                            ctx->prm.h);
-    moments_kernel<1><<<grid, 128, 0, s>>>(w.body, w.keys[ctx->cur], w.cube, w.cell_level, w.cell_start, w.cell_parent, w.cell_first,
+    moments_kernel<1, false><<<grid, 128, 0, s>>>(w.body, w.keys[ctx->cur], w.cube, w.cell_level, w.cell_start, w.cell_parent, w.cell_first,
                                            w.cell_nchild, w.cell_ready, w.cell_meta, w.cell_mac, w.cell_mom0, w.cell_mom1,
                                            w.cell_bmin, w.cell_bmax, w.counters, (u32)w.cell_cap, ctx->max_level, ctx->prm.theta,
                                            ctx->prm.h);
+    P3T_CUDA(ctx, cudaGetLastError());
+    return P3T_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Tree reuse between soft steps ("the cost of the usual complete
+// reconstruction of the tree is O(N log N) and not negligible"): the bodies have moved a little, the sorted order, the
+// cells and the groups of the last build are kept, and only what depends on the positions is made again -- the
+// gathered bodies, then moments, tight boxes and acceptance radii on the old topology.  Lists and forces stay exact in
+// the sense of R-MAC (boxes and radii come from the new positions); what degrades is the tightness of cells and
+// groups, so the refit also counts the bodies that left the cube of their leaf by more than stray_dist leaf sides.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) refit_gather_kernel(const float4 *__restrict__ body_user, const u32 *__restrict__ idx,
+                                                           const u64 *__restrict__ keys, const u8 *__restrict__ dlev,
+                                                           const float *__restrict__ cube, float4 *__restrict__ body, u32 n,
+                                                           int max_level, float stray_dist, u32 *cell_ready,
+                                                           const u32 *__restrict__ prev_ncells, u32 cell_cap, u64 *counters)
+{
+    // arrival counters of the climb -> 0 (a build has keys_hist_kernel do this)
+    for (u32 k = blockIdx.x * blockDim.x + threadIdx.x, nc = min(*prev_ncells, cell_cap); k < nc; k += gridDim.x * blockDim.x)
+        cell_ready[k] = 0;
+    const float side = cube[3];
+    u32 stray = 0;
+    for (u32 i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        const float4 b = body_user[idx[i]];
+        body[i] = b;
+        const int D = dlev[i];
+        const u64 pre = D ? (keys[i] >> (3 * (max_level - D))) : 0ull;
+        const float l = ldexpf(side, -D);
+        const float lx = cube[0] + (float)compact3(pre >> 2) * l, ly = cube[1] + (float)compact3(pre >> 1) * l,
+                    lz = cube[2] + (float)compact3(pre) * l;
+        const float ex = fmaxf(fmaxf(lx - b.x, b.x - (lx + l)), 0.f), ey = fmaxf(fmaxf(ly - b.y, b.y - (ly + l)), 0.f),
+                    ez = fmaxf(fmaxf(lz - b.z, b.z - (lz + l)), 0.f);
+        stray += fmaxf(ex, fmaxf(ey, ez)) > stray_dist * l ? 1u : 0u;
+    }
+    stray = __reduce_add_sync(0xffffffffu, stray);
+    if ((threadIdx.x & 31) == 0 && stray) atomicAdd(&counters[CNT_STRAY], (u64)stray);
+}
+
+// first half: gather + stray count + leaf moments (the caller reads the stray count, then either finishes the refit
+// with p3t_stage_refit_finish or rebuilds)
+p3t_status p3t_stage_refit_begin(p3t_ctx *ctx)
+{
+    Workspace &w = ctx->ws;
+    cudaStream_t s = ctx->stream;
+    const u32 n = (u32)ctx->n;
+    P3T_CUDA(ctx, cudaMemsetAsync(w.counters + CNT_STRAY, 0, sizeof(u64), s));
+    refit_gather_kernel<<<min(div_up(n, 256), (u32)ctx->sm_count * 8), 256, 0, s>>>(
+        w.body_user, w.idx[ctx->cur], w.keys[ctx->cur], w.dlev, w.cube, w.body, n, ctx->max_level, ctx->stray_dist, w.cell_ready,
+        w.prev_ncells, (u32)w.cell_cap, w.counters);
+    size_t bound = ctx->n * (size_t)(ctx->max_level + 1);
+    if (bound > w.cell_cap) bound = w.cell_cap;
+    const u32 grid = (u32)min((size_t)div_up(bound, 128), (size_t)ctx->sm_count * 16);
+    moments_kernel<0, true><<<grid, 128, 0, s>>>(w.body, w.keys[ctx->cur], w.cube, w.cell_level, w.cell_start, w.cell_parent, w.cell_first,
+                                                 w.cell_nchild, w.cell_ready, w.cell_meta, w.cell_mac, w.cell_mom0, w.cell_mom1,
+                                                 w.cell_bmin, w.cell_bmax, w.counters, (u32)w.cell_cap, ctx->max_level, ctx->prm.theta,
+                                                 ctx->prm.h);
+    P3T_CUDA(ctx, cudaGetLastError());
+    return P3T_OK;
+}
+
+p3t_status p3t_stage_refit_finish(p3t_ctx *ctx)
+{
+    Workspace &w = ctx->ws;
+    cudaStream_t s = ctx->stream;
+    size_t bound = ctx->n * (size_t)(ctx->max_level + 1);
+    if (bound > w.cell_cap) bound = w.cell_cap;
+    const u32 grid = (u32)min((size_t)div_up(bound, 128), (size_t)ctx->sm_count * 16);
+    moments_kernel<1, true><<<grid, 128, 0, s>>>(w.body, w.keys[ctx->cur], w.cube, w.cell_level, w.cell_start, w.cell_parent, w.cell_first,
+                                                 w.cell_nchild, w.cell_ready, w.cell_meta, w.cell_mac, w.cell_mom0, w.cell_mom1,
+                                                 w.cell_bmin, w.cell_bmax, w.counters, (u32)w.cell_cap, ctx->max_level, ctx->prm.theta,
+                                                 ctx->prm.h);
     P3T_CUDA(ctx, cudaGetLastError());
     return P3T_OK;
 }

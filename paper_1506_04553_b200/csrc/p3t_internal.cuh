@@ -65,8 +65,9 @@ enum {
     // zeroed at every build (together with the digit histograms in front of the block)
     CNT_NCELLS = 0, CNT_NLEAVES, CNT_NGROUPS, CNT_DEPTH, CNT_ERR_BUILD, CNT_HEAD_TICKET, CNT_HEAD_SPARE0, CNT_HEAD_SPARE1,
     CNT_SORT_TICKET = 8 /* one per pass, 8 */,
-    // zeroed at load only
+    // words from CNT_ERR_BUILD on are zeroed at load (the tree counts in front survive: a refit needs them)
     CNT_NONFINITE = 16,
+    CNT_STRAY = 17 /* refit: bodies that left the cube of their leaf by more than stray_dist leaf sides */,
     CNT_BBOX = 18 /* three words: six 32-bit min/max accumulators of the bounding cube */,
     // zeroed at every eval (together with order_hist behind the block)
     CNT_NPP = 24, CNT_NPC, CNT_NNEAR, CNT_PAIRS, CNT_GROUP_TICKET, CNT_MAXLIST, CNT_ERR_EVAL, CNT_EVAL_SPARE,
@@ -144,6 +145,12 @@ struct p3t_ctx {
     bool hard_unchecked;           // a device-form p3t_eval_hard whose capacity check is still due (sync_and_check)
     bool sort_attr_set, walk_attr_set;   // cudaFuncSetAttribute done on this context's device
     int sort_ctas_per_sm;
+    bool topo_valid;               // sorted order, cells and groups of the last p3t_build_tree are intact (n, tree parameters unchanged)
+    size_t topo_n;                 // particles of that build
+    int refits, max_refits;        // refits since that build; p3t_refit_tree rebuilds after max_refits of them
+    float stray_dist, max_stray_fraction;
+    u64 last_stray;                // stray count of the last refit
+    bool last_rebuilt;             // the last p3t_refit_tree ended in a rebuild
     bool cells_dirty;              // child counters need a memset before the next build
     bool tiles_ready;              // sentinel records of the build look-back written
     bool status_clean;             // the look-back buffers have been zeroed once (they clean themselves afterwards)
@@ -185,6 +192,8 @@ p3t_status p3t_stage_pack(p3t_ctx *ctx, const float *d_mass, const float *d_pos)
 p3t_status p3t_stage_sort(p3t_ctx *ctx);
 p3t_status p3t_stage_build(p3t_ctx *ctx);
 p3t_status p3t_stage_moments(p3t_ctx *ctx);
+p3t_status p3t_stage_refit_begin(p3t_ctx *ctx);
+p3t_status p3t_stage_refit_finish(p3t_ctx *ctx);
 p3t_status p3t_stage_walk(p3t_ctx *ctx);
 p3t_status p3t_stage_direct(p3t_ctx *ctx, const u32 *d_subset, size_t n_subset);
 p3t_status p3t_stage_neighbours(p3t_ctx *ctx);

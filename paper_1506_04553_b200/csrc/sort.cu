@@ -52,7 +52,9 @@ p3t_status p3t_stage_pack(p3t_ctx *ctx, const float *d_mass, const float *d_pos)
 {
     Workspace &w = ctx->ws;
     u32 n = (u32)ctx->n;
-    P3T_CUDA(ctx, cudaMemsetAsync(w.counters, 0, CNT_WORDS * sizeof(u64), ctx->stream));
+    // load words (non-finite flag, bounding-cube accumulators), the build's error word and tickets, the eval words; the
+    // tree counts in front (cells, leaves, groups, depth) survive a load: p3t_refit_tree works on the old tree
+    P3T_CUDA(ctx, cudaMemsetAsync(w.counters + CNT_ERR_BUILD, 0, (CNT_WORDS - CNT_ERR_BUILD) * sizeof(u64), ctx->stream));
     u32 grid = min(div_up(n, 256 * 4), (u32)ctx->sm_count * 8);
     pack_bbox_kernel<<<grid, 256, 0, ctx->stream>>>(d_mass, d_pos, w.body_user, w.bbox_bits, w.counters, n);
     P3T_CUDA(ctx, cudaGetLastError());
