@@ -99,6 +99,27 @@ p3t_status p3t_destroy(p3t_ctx *ctx);
  * (theta and r_search enter the per-cell acceptance radius). */
 p3t_status p3t_set_params(p3t_ctx *ctx, float eps, float theta, float r_in, float r_out, float r_search);
 
+/* Per-pair-class cutoffs (section 3.2.2.1: "We use three values for the cut off
+ * radius with respect to three different kinds of interactions").  cls[n] gives every particle (user order) a class,
+ * 0 = field star (FS), 1 = black hole (BH); the kind of a pair is class_i + class_j:
+ *   0  FS-FS  r_in, r_out, r_search, eps of p3t_set_params                       (paper: r_cut,FS-FS = 1/256)
+ *   1  BH-FS  r_in_bf, r_out_bf, r_search_bf, the same eps                        (paper: r_cut,BH-FS = 1/32)
+ *   2  BH-BH  not split: "the force is not split and F_soft = 0 ... integrated with the pure Hermite scheme": K = W = 0
+ *             in a_i and phi_i at every separation, the two are ALWAYS in each other's list, and the hard part
+ *             (p3t_eval_hard) gives them the whole Newtonian term with the softening eps_bb (paper: none)
+ * in every formula of this header (Eq. 6-8, the list rule).  A cell is used as a multipole only if every body in it is a
+ * plain Newtonian partner of every body of the group: a cell or a group that holds a black hole keeps clear of
+ * max(r_search, r_search_bf), and a group with a black hole opens every cell that holds one.  The split kinds share
+ * one softening, as in the paper's runs, because a cell term has only one.
+ * cls is host or device memory (on_device); it is copied, the classes stay with the particle ids over later
+ * p3t_load_particles calls of the same n.  cls = NULL switches classes off.  A built tree becomes invalid.
+ * P3T_EINVAL: n = 0 or > max_n, a class above 1 (host input; device input is reduced to its lowest bit), not
+ * (0 <= r_in_bf < r_out_bf <= r_search_bf), eps_bb < 0, non-finite values.  P3T_ESTATE from p3t_build_tree and
+ * p3t_eval_direct when n differs from the loaded particle count, and from p3t_hermite_step / p3t_step while classes
+ * are set (the Hermite part on the device knows one kind of pair; eta_BH of L287 is the caller's integrator's). */
+p3t_status p3t_set_pair_classes(p3t_ctx *ctx, size_t n, const uint8_t *cls, int on_device, float r_in_bf, float r_out_bf,
+                                float r_search_bf, float eps_bb);
+
 /* nleaf in 1..32: a cell with more than nleaf bodies is split (unless at the
  * key depth limit); ngroup in {32, 64}: bodies per i-group (one warp). */
 p3t_status p3t_set_tree_params(p3t_ctx *ctx, int nleaf, int ngroup);
@@ -263,7 +284,8 @@ typedef enum {
     P3T_ARR_BODIES      = 3,  /* float4[n]: sorted (x,y,z,m) */
     P3T_ARR_CELL_MAC    = 4,  /* float4[n_cells]: centre of mass, squared acceptance radius */
     P3T_ARR_CELL_MOM0   = 5,  /* float4[n_cells]: M, Qxx, Qyy, Qzz (traceful, about the COM) */
-    P3T_ARR_CELL_MOM1   = 6,  /* float4[n_cells]: Qxy, Qxz, Qyz, bounding radius about the COM */
+    P3T_ARR_CELL_MOM1   = 6,  /* float4[n_cells]: Qxy, Qxz, Qyz, bounding radius about the COM (with pair classes its
+                                 sign bit marks the cells that hold a black hole) */
     P3T_ARR_CELL_META   = 7,  /* uint32[2][n_cells]: leaf: body start, count | 0x80000000;
                                                      internal: first child, child count */
     P3T_ARR_CELL_LEVEL  = 8,  /* uint8[n_cells] */

@@ -76,6 +76,8 @@ size_t p3t_layout(Workspace &ws, char *base, size_t max_n, int key_bits, size_t 
     ws.nbr = b.take<u32>(nbr_capacity ? nbr_capacity : 1);
     ws.nbr_cursor = b.take<u32>(n);
     ws.subset = b.take<u32>(n);
+    ws.cls_user = b.take<u8>(n + 4);
+    ws.cls_sorted = b.take<u8>(n + 4);
     ws.hard_out = b.take<double>(7 * n);
     ws.herm_ids = b.take<u32>(n);
     ws.herm_tdt = b.take<u64>(n);
@@ -186,6 +188,46 @@ extern "C" const char *p3t_last_error(const p3t_ctx *ctx) { return ctx ? ctx->er
 // ------------------------------------------------------------------------------------------------
 // parameters
 // ------------------------------------------------------------------------------------------------
+// W(y; gamma) of Eq. 16-17 as coefficients of y^k and y ln y; the denominator of Eq. 17 is taken
+// as (gamma-1)^7 (reading A1).
+static void p3t_fill_cutoff(CutoffSet &c, float r_in, float r_out)
+{
+    double g = (double)r_in / (double)r_out;
+    double g2 = g * g, g3 = g2 * g, g4 = g2 * g2, g5 = g4 * g, g6 = g3 * g3, g7 = g6 * g;
+    double D = pow(g - 1.0, 7);
+    c.gamma = g;
+    c.inv_rout = 1.0 / (double)r_out;
+    c.inv_1mg = 1.0 / (1.0 - g);
+    c.wc[7] = (-10.0 / 3.0) / D;
+    c.wc[6] = 14.0 * (g + 1.0) / D;
+    c.wc[5] = -21.0 * (g2 + 3.0 * g + 1.0) / D;
+    c.wc[4] = (35.0 / 3.0) * (g3 + 9.0 * g2 + 9.0 * g + 1.0) / D;
+    c.wc[3] = -70.0 * (g3 + 3.0 * g2 + g) / D;
+    c.wc[2] = 210.0 * (g3 + g2) / D;
+    c.wc[0] = (g7 - 7.0 * g6 + 21.0 * g5 - 35.0 * g4) / D;
+    c.wl = -140.0 * g3 / D;
+    double G1 = c.wc[7] + c.wc[6] + c.wc[5] + c.wc[4] + c.wc[3] + c.wc[2] + c.wc[0];   // ln 1 = 0
+    c.wc[1] = 1.0 - G1;
+    double glog = g > 0.0 ? 60.0 * g3 * log(g) : 0.0;
+    c.cin = 7.0 * (g6 - 9.0 * g5 + 45.0 * g4 - glog - 45.0 * g2 + 9.0 * g - 1.0) / (3.0 * D);
+}
+
+// the per-kind numbers of P3TParams from the context's two parameter sets (kind 1 = kind 0 while no classes are set)
+static void p3t_refresh_class_params(p3t_ctx *ctx)
+{
+    P3TParams &p = ctx->prm;
+    p.classes = ctx->cls_n ? 1 : 0;
+    const float r_in1 = p.classes ? ctx->r_in_bf : ctx->r_in, r_out1 = p.classes ? ctx->r_out_bf : ctx->r_out,
+                h1 = p.classes ? ctx->r_search_bf : ctx->r_search;
+    p.rout2_k[0] = p.rout2; p.h2_k[0] = p.h2;
+    p.rout2_k[1] = r_out1 * r_out1; p.h2_k[1] = h1 * h1;
+    p.h_bf = fmaxf(ctx->r_search, h1);
+    const float hn = p.h_bf * (1.f + 1e-5f);
+    p.hnear2_bf = hn * hn;
+    p.eps2_bb_d = (double)ctx->eps_bb * (double)ctx->eps_bb;
+    if (r_out1 > 0.f) p3t_fill_cutoff(p.cs[1], r_in1, r_out1);
+}
+
 extern "C" p3t_status p3t_set_params(p3t_ctx *ctx, float eps, float theta, float r_in, float r_out, float r_search)
 {
     if (!ctx) return P3T_EINVAL;
@@ -204,29 +246,40 @@ extern "C" p3t_status p3t_set_params(p3t_ctx *ctx, float eps, float theta, float
         float hn = r_search * (1.f + 1e-5f);
         p.hnear2 = hn * hn;
     }
-    // W(y; gamma) of Eq. 16-17 as coefficients of y^k and y ln y; the
-    // denominator of Eq. 17 is taken as (gamma-1)^7 (reading A1).
-    double g = (double)r_in / (double)r_out;
-    double g2 = g * g, g3 = g2 * g, g4 = g2 * g2, g5 = g4 * g, g6 = g3 * g3, g7 = g6 * g;
-    double D = pow(g - 1.0, 7);
-    p.gamma = g;
-    p.inv_rout = 1.0 / (double)r_out;
-    p.inv_1mg = 1.0 / (1.0 - g);
-    p.wc[7] = (-10.0 / 3.0) / D;
-    p.wc[6] = 14.0 * (g + 1.0) / D;
-    p.wc[5] = -21.0 * (g2 + 3.0 * g + 1.0) / D;
-    p.wc[4] = (35.0 / 3.0) * (g3 + 9.0 * g2 + 9.0 * g + 1.0) / D;
-    p.wc[3] = -70.0 * (g3 + 3.0 * g2 + g) / D;
-    p.wc[2] = 210.0 * (g3 + g2) / D;
-    p.wc[0] = (g7 - 7.0 * g6 + 21.0 * g5 - 35.0 * g4) / D;
-    p.wl = -140.0 * g3 / D;
-    double G1 = p.wc[7] + p.wc[6] + p.wc[5] + p.wc[4] + p.wc[3] + p.wc[2] + p.wc[0];   // ln 1 = 0
-    p.wc[1] = 1.0 - G1;
-    double glog = g > 0.0 ? 60.0 * g3 * log(g) : 0.0;
-    p.cin = 7.0 * (g6 - 9.0 * g5 + 45.0 * g4 - glog - 45.0 * g2 + 9.0 * g - 1.0) / (3.0 * D);
+    p3t_fill_cutoff(p.cs[0], r_in, r_out);
+    p3t_refresh_class_params(ctx);
     ctx->have_params = true;
     ctx->built = false;        // theta and h enter the per-cell acceptance radius
     ctx->evaluated = false;
+    return P3T_OK;
+}
+
+// Per-pair-class cutoffs (section 3.2.2.1)
+extern "C" p3t_status p3t_set_pair_classes(p3t_ctx *ctx, size_t n, const uint8_t *cls, int on_device, float r_in_bf, float r_out_bf,
+                                           float r_search_bf, float eps_bb)
+{
+    if (!ctx) return P3T_EINVAL;
+    ctx->built = false;
+    ctx->evaluated = false;
+    ctx->topo_valid = false;          // the classes are gathered into Morton order by a build
+    if (!cls) {                       // back to one kind of pair
+        ctx->cls_n = 0;
+        p3t_refresh_class_params(ctx);
+        return P3T_OK;
+    }
+    if (n == 0 || n > ctx->max_n) return p3t_fail(ctx, P3T_EINVAL, "n must be in 1..max_n");
+    if (!(r_in_bf >= 0.f) || !(r_in_bf < r_out_bf) || !(r_out_bf <= r_search_bf) || !isfinite(r_search_bf) || !(eps_bb >= 0.f) || !isfinite(eps_bb))
+        return p3t_fail(ctx, P3T_EINVAL, "need 0 <= r_in_bf < r_out_bf <= r_search_bf and eps_bb >= 0, all finite");
+    P3T_CUDA(ctx, cudaSetDevice(ctx->device));
+    if (!on_device)
+        for (size_t i = 0; i < n; ++i)
+            if (cls[i] > 1) return p3t_fail(ctx, P3T_EINVAL, "classes must be 0 (field star) or 1 (black hole)");
+    // (device input: values are reduced to their lowest bit when they are gathered)
+    P3T_CUDA(ctx, cudaMemcpyAsync(ctx->ws.cls_user, cls, n, on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, ctx->stream));
+    if (!on_device) P3T_CUDA(ctx, cudaStreamSynchronize(ctx->stream));    // the caller's array may be pageable and short-lived
+    ctx->cls_n = n;
+    ctx->r_in_bf = r_in_bf; ctx->r_out_bf = r_out_bf; ctx->r_search_bf = r_search_bf; ctx->eps_bb = eps_bb;
+    p3t_refresh_class_params(ctx);
     return P3T_OK;
 }
 
@@ -344,6 +397,7 @@ extern "C" p3t_status p3t_build_tree(p3t_ctx *ctx)
     if (!ctx) return P3T_EINVAL;
     if (!ctx->loaded) return p3t_fail(ctx, P3T_ESTATE, "p3t_build_tree before p3t_load_particles");
     if (!ctx->have_params) return p3t_fail(ctx, P3T_ESTATE, "p3t_build_tree before p3t_set_params");
+    if (ctx->cls_n && ctx->cls_n != ctx->n) return p3t_fail(ctx, P3T_ESTATE, "the classes of p3t_set_pair_classes were given for another particle count");
     P3T_CUDA(ctx, cudaSetDevice(ctx->device));
     ctx->built = false;
     ctx->evaluated = false;
@@ -387,6 +441,7 @@ extern "C" p3t_status p3t_refit_tree(p3t_ctx *ctx)
     if (!ctx->have_params) return p3t_fail(ctx, P3T_ESTATE, "p3t_refit_tree before p3t_set_params");
     // no tree of these particles to reuse, or enough refits in a row: a full build
     if (!ctx->topo_valid || ctx->topo_n != ctx->n || ctx->refits >= ctx->max_refits) return p3t_build_tree(ctx);
+    if (ctx->cls_n && ctx->cls_n != ctx->n) return p3t_fail(ctx, P3T_ESTATE, "the classes of p3t_set_pair_classes were given for another particle count");
     P3T_CUDA(ctx, cudaSetDevice(ctx->device));
     ctx->built = false;
     ctx->evaluated = false;
@@ -432,6 +487,7 @@ extern "C" p3t_status p3t_eval_direct(p3t_ctx *ctx, const uint32_t *i_subset, si
     if (!ctx) return P3T_EINVAL;
     if (!ctx->loaded) return p3t_fail(ctx, P3T_ESTATE, "p3t_eval_direct before p3t_load_particles");
     if (!ctx->have_params) return p3t_fail(ctx, P3T_ESTATE, "p3t_eval_direct before p3t_set_params");
+    if (ctx->cls_n && ctx->cls_n != ctx->n) return p3t_fail(ctx, P3T_ESTATE, "the classes of p3t_set_pair_classes were given for another particle count");
     if (i_subset && (n_subset == 0 || n_subset > ctx->n)) return p3t_fail(ctx, P3T_EINVAL, "bad subset size");
     P3T_CUDA(ctx, cudaSetDevice(ctx->device));
     const u32 *d_subset = i_subset;
@@ -541,6 +597,7 @@ extern "C" p3t_status p3t_hermite_step(p3t_ctx *ctx, double *pos, double *vel, d
     if (!ctx->evaluated) return p3t_fail(ctx, P3T_ESTATE, "p3t_hermite_step needs the neighbour lists of an eval call");
     if (!ctx->lists_complete)
         return p3t_fail(ctx, P3T_ESTATE, "p3t_hermite_step needs the lists of ALL particles: the last evaluation was sharded or a subset");
+    if (ctx->cls_n) return p3t_fail(ctx, P3T_ESTATE, "the Hermite part does not know pair classes (p3t_set_pair_classes): use p3t_eval_hard");
     p3t_status st = hermite_args_ok(ctx, dt_soft, log2_div, eta, eta_s, a0, max_blocks);
     if (st != P3T_OK) return st;
     P3T_CUDA(ctx, cudaSetDevice(ctx->device));
@@ -568,6 +625,7 @@ extern "C" p3t_status p3t_step(p3t_ctx *ctx, const float *mass, double *pos, dou
     if (!ctx) return P3T_EINVAL;
     if (!mass || !pos || !vel) return p3t_fail(ctx, P3T_EINVAL, "null mass/pos/vel");
     if (!ctx->evaluated) return p3t_fail(ctx, P3T_ESTATE, "p3t_step needs the soft force and lists of an eval call at the current positions");
+    if (ctx->cls_n) return p3t_fail(ctx, P3T_ESTATE, "p3t_step does not know pair classes (p3t_set_pair_classes)");
     if (!ctx->lists_complete || ctx->shard_world > 1)
         return p3t_fail(ctx, P3T_ESTATE, "p3t_step needs the soft force and lists of ALL particles: not available on a sharded context or after a subset evaluation");
     p3t_status st = hermite_args_ok(ctx, dt_soft, log2_div, eta, eta_s, a0, max_blocks);

@@ -9,19 +9,23 @@
 __global__ void __launch_bounds__(DIRECT_THREADS) direct_kernel(const float4 *__restrict__ body_user, u32 n,
                                                                 const u32 *__restrict__ subset, u32 ns, P3TParams prm,
                                                                 float4 *__restrict__ accpot, u32 *__restrict__ nbr_count,
-                                                                uint2 *pairs, u64 pair_cap, u64 *counters)
+                                                                uint2 *pairs, u64 pair_cap, u64 *counters,
+                                                                const u8 *__restrict__ cls_user)
 {
     __shared__ float4 s_b[DIRECT_THREADS];
+    __shared__ u8 s_c[DIRECT_THREADS];
     const u32 k = blockIdx.x * DIRECT_THREADS + threadIdx.x;
     const bool active = k < ns;
     const u32 i = active ? (subset ? subset[k] : k) : 0u;
     const float4 bi = body_user[i];
+    const u32 ci = cls_user ? (cls_user[i] & 1u) : 0u;    // pair classes: kind of a pair = ci + cj
     double ax = 0.0, ay = 0.0, az = 0.0, ph = 0.0;
     u32 cnt = 0;
     u64 npairs = 0;
     for (u32 j0 = 0; j0 < n; j0 += DIRECT_THREADS) {
         u32 jl = j0 + threadIdx.x;
         s_b[threadIdx.x] = jl < n ? body_user[jl] : make_float4(0.f, 0.f, 0.f, 0.f);
+        s_c[threadIdx.x] = (cls_user && jl < n) ? (cls_user[jl] & 1u) : 0u;
         __syncthreads();
         u32 lim = min((u32)DIRECT_THREADS, n - j0);
         float fx = 0.f, fy = 0.f, fz = 0.f, fp = 0.f;
@@ -36,8 +40,10 @@ __global__ void __launch_bounds__(DIRECT_THREADS) direct_kernel(const float4 *__
                 float mrinv = bj.w * rinv;
                 float mr3 = mrinv * (rinv * rinv);
                 float K = 1.f, W = 1.f;
-                if (s2 < prm.h2) {
-                    if (s2 < prm.rout2) p3t_pair_weights(prm, s2, K, W);
+                const u32 kind = ci + s_c[jj];
+                if (kind == 2u) { K = 0.f; W = 0.f; }                   // two black holes: not split, all of it hard
+                if (kind == 2u || s2 < prm.h2_k[kind & 1u]) {
+                    if (kind < 2u && s2 < prm.rout2_k[kind]) p3t_pair_weights(prm.cs[kind], s2, K, W);
                     u64 pos = atomicAdd(&counters[CNT_PAIRS], 1ull);
                     if (pos < pair_cap) pairs[pos] = make_uint2(i, j);
                     ++cnt;
@@ -68,7 +74,8 @@ p3t_status p3t_stage_direct(p3t_ctx *ctx, const u32 *d_subset, size_t n_subset)
     P3T_CUDA(ctx, cudaMemsetAsync(w.nbr_count, 0, (size_t)n * sizeof(u32), s));
     direct_kernel<<<div_up(n_subset, DIRECT_THREADS), DIRECT_THREADS, 0, s>>>(w.body_user, n, d_subset, (u32)n_subset, ctx->prm,
                                                                               w.accpot, w.nbr_count, w.pairs,
-                                                                              (u64)ctx->nbr_capacity, w.counters);
+                                                                              (u64)ctx->nbr_capacity, w.counters,
+                                                                              ctx->cls_n ? w.cls_user : nullptr);
     P3T_CUDA(ctx, cudaGetLastError());
     return P3T_OK;
 }

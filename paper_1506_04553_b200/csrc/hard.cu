@@ -12,7 +12,7 @@
 #include "p3t_internal.cuh"
 
 // K, dK/ds and W in double for gamma <= y < 1 (Eq. 12, 16-17 with reading A1); coefficients from set_params
-__device__ __forceinline__ void hard_weights(const P3TParams &p, double s, double &omK, double &dKds, double &omW)
+__device__ __forceinline__ void hard_weights(const CutoffSet &p, double s, double &omK, double &dKds, double &omW)
 {
     const double y = s * p.inv_rout;
     if (y >= 1.0) { omK = 0.0; dKds = 0.0; omW = 0.0; return; }
@@ -36,14 +36,14 @@ __global__ void __launch_bounds__(HARD_THREADS) hard_kernel(const float4 *__rest
                                                             const u64 *__restrict__ offset, const u32 *__restrict__ nbr,
                                                             const u64 *__restrict__ counters, u64 capacity, P3TParams prm, u32 n,
                                                             double *__restrict__ acc, double *__restrict__ jerk,
-                                                            double *__restrict__ pot)
+                                                            double *__restrict__ pot, const u8 *__restrict__ cls_user)
 {
     const u32 i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     if (counters[CNT_PAIRS] > capacity) return;     // the lists did not fit: the caller gets P3T_ECAPACITY
     const float4 bi = body_user[i];
     const double vix = vel[3 * (size_t)i], viy = vel[3 * (size_t)i + 1], viz = vel[3 * (size_t)i + 2];
-    const double eps2 = prm.eps2_d;
+    const u32 ci = cls_user ? (cls_user[i] & 1u) : 0u;     // pair classes: kind of a pair = ci + cj
     double ax = 0, ay = 0, az = 0, jx = 0, jy = 0, jz = 0, ph = 0;
     for (u64 k = offset[i], e = offset[i + 1]; k < e; ++k) {
         const u32 j = nbr[k];
@@ -51,10 +51,11 @@ __global__ void __launch_bounds__(HARD_THREADS) hard_kernel(const float4 *__rest
         const double dx = (double)bi.x - (double)bj.x, dy = (double)bi.y - (double)bj.y, dz = (double)bi.z - (double)bj.z;
         const double wx = vix - (double)vel[3 * (size_t)j], wy = viy - (double)vel[3 * (size_t)j + 1],
                      wz = viz - (double)vel[3 * (size_t)j + 2];
-        const double s2 = dx * dx + dy * dy + dz * dz + eps2;
+        const u32 kind = ci + (cls_user ? (cls_user[j] & 1u) : 0u);
+        const double s2 = dx * dx + dy * dy + dz * dz + (kind == 2u ? prm.eps2_bb_d : prm.eps2_d);
         const double s = sqrt(s2);
-        double omK, dKds, omW;
-        hard_weights(prm, s, omK, dKds, omW);
+        double omK = 1.0, dKds = 0.0, omW = 1.0;         // kind 2 (two black holes): not split, the whole Newtonian term
+        if (kind < 2u) hard_weights(prm.cs[kind], s, omK, dKds, omW);
         const double qv = dx * wx + dy * wy + dz * wz;
         const double mr3 = (double)bj.w / (s2 * s);
         const double c1 = mr3 * omK, c2 = mr3 * (3.0 * omK * qv / s2 + dKds * qv / s);
@@ -72,7 +73,7 @@ p3t_status p3t_stage_hard(p3t_ctx *ctx, const float *d_vel, double *d_acc, doubl
     Workspace &w = ctx->ws;
     const u32 n = (u32)ctx->n;
     hard_kernel<<<div_up(n, HARD_THREADS), HARD_THREADS, 0, ctx->stream>>>(w.body_user, d_vel, w.nbr_offset, w.nbr, w.counters, (u64)ctx->nbr_capacity,
-                                                        ctx->prm, n, d_acc, d_jerk, d_pot);
+                                                        ctx->prm, n, d_acc, d_jerk, d_pot, ctx->cls_n ? w.cls_user : nullptr);
     P3T_CUDA(ctx, cudaGetLastError());
     return P3T_OK;
 }

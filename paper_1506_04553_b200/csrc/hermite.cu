@@ -35,7 +35,7 @@ enum { HC_COUNT = 0, HC_TMIN0, HC_TMIN1, HC_TMIN2, HC_BLOCKS, HC_STEPS, HC_FLOOR
 #define HERM_GRID_FLAG 0x80000000u   // cstart: the component's members go to the grid tier's own array
 #define HERM_NONFINITE 0x80000000u   // high bit of a thread's floor_hits counter: it met a non-finite force (herm_quantise)
 
-__device__ __forceinline__ void herm_weights(const P3TParams &p, double s, double &omK, double &dKds)
+__device__ __forceinline__ void herm_weights(const CutoffSet &p, double s, double &omK, double &dKds)
 {
     const double y = s * p.inv_rout;
     if (y >= 1.0) { omK = 0.0; dKds = 0.0; return; }
@@ -289,7 +289,7 @@ __device__ __forceinline__ void herm_force(const HermConst &C, const HermView &V
         const double s2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2] + eps2;
         const double s = sqrt(s2);
         double omK, dKds;
-        herm_weights(C.prm, s, omK, dKds);
+        herm_weights(C.prm.cs[0], s, omK, dKds);
         if (omK == 0.0 && dKds == 0.0) continue;
         const double qv = d[0] * w[0] + d[1] * w[1] + d[2] * w[2];
         const double mj = LOCAL ? V.mass[j] : (double)V.body_user[j].w;

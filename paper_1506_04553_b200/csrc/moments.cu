@@ -27,6 +27,7 @@ struct Mom {
     float cx, cy, cz, M;
     float qxx, qyy, qzz, qxy, qxz, qyz;
     float lox, loy, loz, hix, hiy, hiz;
+    bool heavy;        // pair classes: the cell holds a black hole (kept in the sign bit of the stored rmax)
 };
 
 template <bool REFIT>
@@ -47,7 +48,7 @@ __device__ __forceinline__ void store_cell(u32 k, const Mom &m, int level, u64 k
           fz = fmaxf(m.cz - m.loz, m.hiz - m.cz);
     float rmax = sqrtf(fx * fx + fy * fy + fz * fz) * (1.f + 1e-6f);
     float slack = 8.f * 1.1920929e-7f * (fabsf(cube[0]) + fabsf(cube[1]) + fabsf(cube[2]) + 2.f * side);
-    float rc3 = (h + rmax) * (1.f + 1e-5f) + slack;
+    float rc3 = (h + rmax) * (1.f + 1e-5f) + slack;          // h: the caller passes h_bf for a cell that holds a black hole
     // Refit (p3t_refit_tree): the bodies have moved since the keys were made and may sit outside the cell's cube; the
     // opening test then takes the side of the smallest cube about the geometric centre that holds them all, which
     // keeps the geometric meaning of l / theta (for bodies inside the cube nothing changes).
@@ -60,7 +61,7 @@ __device__ __forceinline__ void store_cell(u32 k, const Mom &m, int level, u64 k
     float rc = fmaxf(rc1, rc3);
     cell_mac[k] = make_float4(m.cx, m.cy, m.cz, rc * rc);
     cell_mom0[k] = make_float4(m.M, m.qxx, m.qyy, m.qzz);
-    cell_mom1[k] = make_float4(m.qxy, m.qxz, m.qyz, rmax);
+    cell_mom1[k] = make_float4(m.qxy, m.qxz, m.qyz, m.heavy ? -rmax : rmax);
     cell_bmin[k] = make_float4(m.lox, m.loy, m.loz, l);
     cell_bmax[k] = make_float4(m.hix, m.hiy, m.hiz, delta);
 }
@@ -75,6 +76,7 @@ __device__ __forceinline__ void merge_children(u32 first, u32 nch, const float4 
     float M = 0.f, sx = 0.f, sy = 0.f, sz = 0.f;
     float qxx = 0.f, qyy = 0.f, qzz = 0.f, qxy = 0.f, qxz = 0.f, qyz = 0.f;
     m.lox = m.loy = m.loz = INFINITY; m.hix = m.hiy = m.hiz = -INFINITY;
+    m.heavy = false;
 #pragma unroll
     for (int c = 0; c < 8; ++c) {
         if ((u32)c < nch) {
@@ -82,6 +84,7 @@ __device__ __forceinline__ void merge_children(u32 first, u32 nch, const float4 
             const float4 a = __ldcg(&cell_mac[ci]), q0 = __ldcg(&cell_mom0[ci]), q1 = __ldcg(&cell_mom1[ci]);
             const float4 lo = __ldcg(&cell_bmin[ci]), hi = __ldcg(&cell_bmax[ci]);
             const float mc = q0.x, rx = a.x - a0.x, ry = a.y - a0.y, rz = a.z - a0.z;
+            m.heavy = m.heavy || (__float_as_uint(q1.w) >> 31);
             M += mc;
             sx += mc * rx; sy += mc * ry; sz += mc * rz;
             qxx += q0.y + mc * rx * rx; qyy += q0.z + mc * ry * ry; qzz += q0.w + mc * rz * rz;
@@ -116,7 +119,8 @@ __global__ void __launch_bounds__(128, 4) moments_kernel(
     const u8 *__restrict__ cell_level, const u32 *__restrict__ cell_start, const u32 *__restrict__ cell_parent,
     const u32 *__restrict__ cell_first, u32 *cell_nchild, u32 *cell_ready, uint2 *cell_meta,
     float4 *cell_mac, float4 *cell_mom0, float4 *cell_mom1, float4 *cell_bmin,
-    float4 *cell_bmax, const u64 *__restrict__ counters, u32 cell_cap, int max_level, float theta, float h)
+    float4 *cell_bmax, const u64 *__restrict__ counters, u32 cell_cap, int max_level, float theta, float h,
+    const u8 *__restrict__ cls_sorted, float h_bf)
 {
     const u32 ncell = (u32)min((u64)cell_cap, counters[CNT_NCELLS]);
     for (u32 k0 = blockIdx.x * blockDim.x + threadIdx.x; k0 < ncell; k0 += gridDim.x * blockDim.x) {
@@ -135,6 +139,9 @@ __global__ void __launch_bounds__(128, 4) moments_kernel(
             float sx = 0.f, sy = 0.f, sz = 0.f, M = 0.f;
             float qxx = 0.f, qyy = 0.f, qzz = 0.f, qxy = 0.f, qxz = 0.f, qyz = 0.f;
             m.lox = m.hix = b0.x; m.loy = m.hiy = b0.y; m.loz = m.hiz = b0.z;
+            m.heavy = false;
+            if (cls_sorted)
+                for (u32 j = 0; j < cnt; ++j) m.heavy = m.heavy || cls_sorted[start + j] != 0;
             for (u32 j0 = 0; j0 < cnt; j0 += 4) {
                 float4 bb[4];
 #pragma unroll
@@ -164,7 +171,7 @@ __global__ void __launch_bounds__(128, 4) moments_kernel(
                 m.cx = 0.5f * (m.lox + m.hix); m.cy = 0.5f * (m.loy + m.hiy); m.cz = 0.5f * (m.loz + m.hiz);
                 m.qxx = m.qyy = m.qzz = m.qxy = m.qxz = m.qyz = 0.f;
             }
-            store_cell<REFIT>(k, m, level, keys[start], cube, max_level, theta, h, cell_mac, cell_mom0, cell_mom1, cell_bmin, cell_bmax);
+            store_cell<REFIT>(k, m, level, keys[start], cube, max_level, theta, m.heavy ? h_bf : h, cell_mac, cell_mom0, cell_mom1, cell_bmin, cell_bmax);
             continue;
         }
         // ---- internal cell
@@ -184,7 +191,7 @@ __global__ void __launch_bounds__(128, 4) moments_kernel(
             }
             merge_children(first, nch, cell_mac, cell_mom0, cell_mom1, cell_bmin, cell_bmax, m);
             const u64 pkey = parent != P3T_NO_PARENT ? keys[pstart] : 0ull;
-            store_cell<REFIT>(k, m, level, key, cube, max_level, theta, h, cell_mac, cell_mom0, cell_mom1, cell_bmin, cell_bmax);
+            store_cell<REFIT>(k, m, level, key, cube, max_level, theta, m.heavy ? h_bf : h, cell_mac, cell_mom0, cell_mom1, cell_bmin, cell_bmax);
             cell_meta[k] = make_uint2(first, nch);
             if (parent == P3T_NO_PARENT) break;
             __threadfence();             // my record is visible before my arrival is
@@ -205,11 +212,11 @@ p3t_status p3t_stage_moments(p3t_ctx *ctx)
     moments_kernel<0, false><<<grid, 128, 0, s>>>(w.body, w.keys[ctx->cur], w.cube, w.cell_level, w.cell_start, w.cell_parent, w.cell_first,
                                            w.cell_nchild, w.cell_ready, w.cell_meta, w.cell_mac, w.cell_mom0, w.cell_mom1,
                                            w.cell_bmin, w.cell_bmax, w.counters, (u32)w.cell_cap, ctx->max_level, ctx->prm.theta,
-                                           ctx->prm.h);
+                                           ctx->prm.h, ctx->cls_n ? w.cls_sorted : nullptr, ctx->prm.h_bf);
     moments_kernel<1, false><<<grid, 128, 0, s>>>(w.body, w.keys[ctx->cur], w.cube, w.cell_level, w.cell_start, w.cell_parent, w.cell_first,
                                            w.cell_nchild, w.cell_ready, w.cell_meta, w.cell_mac, w.cell_mom0, w.cell_mom1,
                                            w.cell_bmin, w.cell_bmax, w.counters, (u32)w.cell_cap, ctx->max_level, ctx->prm.theta,
-                                           ctx->prm.h);
+                                           ctx->prm.h, ctx->cls_n ? w.cls_sorted : nullptr, ctx->prm.h_bf);
     P3T_CUDA(ctx, cudaGetLastError());
     return P3T_OK;
 }
@@ -266,7 +273,7 @@ p3t_status p3t_stage_refit_begin(p3t_ctx *ctx)
     moments_kernel<0, true><<<grid, 128, 0, s>>>(w.body, w.keys[ctx->cur], w.cube, w.cell_level, w.cell_start, w.cell_parent, w.cell_first,
                                                  w.cell_nchild, w.cell_ready, w.cell_meta, w.cell_mac, w.cell_mom0, w.cell_mom1,
                                                  w.cell_bmin, w.cell_bmax, w.counters, (u32)w.cell_cap, ctx->max_level, ctx->prm.theta,
-                                                 ctx->prm.h);
+                                                 ctx->prm.h, ctx->cls_n ? w.cls_sorted : nullptr, ctx->prm.h_bf);
     P3T_CUDA(ctx, cudaGetLastError());
     return P3T_OK;
 }
@@ -281,7 +288,7 @@ p3t_status p3t_stage_refit_finish(p3t_ctx *ctx)
     moments_kernel<1, true><<<grid, 128, 0, s>>>(w.body, w.keys[ctx->cur], w.cube, w.cell_level, w.cell_start, w.cell_parent, w.cell_first,
                                                  w.cell_nchild, w.cell_ready, w.cell_meta, w.cell_mac, w.cell_mom0, w.cell_mom1,
                                                  w.cell_bmin, w.cell_bmax, w.counters, (u32)w.cell_cap, ctx->max_level, ctx->prm.theta,
-                                                 ctx->prm.h);
+                                                 ctx->prm.h, ctx->cls_n ? w.cls_sorted : nullptr, ctx->prm.h_bf);
     P3T_CUDA(ctx, cudaGetLastError());
     return P3T_OK;
 }

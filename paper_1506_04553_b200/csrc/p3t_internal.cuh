@@ -41,6 +41,18 @@ typedef unsigned char u8;
 // double precision (set_params): for gamma <= y < 1
 //   W(y) = sum_{k=0..7} wc[k] y^k + wl * y ln y          (Eq. 16-17 with reading A1)
 // and W(y) = cin * y below gamma.  K(x) = x^4 (35 - 84 x + 70 x^2 - 20 x^3)  (Eq. 12).
+struct CutoffSet {
+    double inv_rout;   // 1 / r_out
+    double gamma;      // r_in / r_out
+    double inv_1mg;    // 1 / (1 - gamma)
+    double cin;        // slope of W below gamma
+    double wc[8];
+    double wl;
+};
+// Kinds of pairs when the bodies carry classes (section 3.2.2.1; 0 = field star, 1 = black hole):
+// kind = class_i + class_j: 0 FS-FS, 1 BH-FS (its own cutoff radii and neighbour radius, the same softening), 2 BH-BH
+// (not split: K = W = 0 in the soft sums, always neighbours, softening eps_bb in the hard part).  Without classes every
+// pair is of kind 0.
 struct P3TParams {
     float eps2;        // eps^2
     float theta;
@@ -48,13 +60,13 @@ struct P3TParams {
     float rout2;       // r_out^2
     float h2;          // h^2                 (neighbour test  s^2 < h^2, reading A4)
     float hnear2;      // (h (1+1e-5))^2 + slack: bodies whose box distance is below this take the slow path
+    int classes;       // bodies carry classes
+    float h_bf;        // max(h, h of BH-FS pairs): what a cell with a black hole, or a group with one, keeps clear
+    float hnear2_bf;   // hnear2 with h_bf
+    float rout2_k[2], h2_k[2];   // per kind of split pair
     double eps2_d;     // eps^2 in double (hard.cu evaluates pairs in fp64)
-    double inv_rout;   // 1 / r_out
-    double gamma;      // r_in / r_out
-    double inv_1mg;    // 1 / (1 - gamma)
-    double cin;        // slope of W below gamma
-    double wc[8];
-    double wl;
+    double eps2_bb_d;  // softening^2 of the unsplit BH-BH pairs (hard part only)
+    CutoffSet cs[2];   // K, W coefficients of kind 0 and kind 1
 };
 
 // Device-side counters (one block of 64-bit words in the workspace).  Layout in memory:
@@ -114,6 +126,7 @@ struct Workspace {
     u32 *nbr;                      // [cap]
     u32 *nbr_cursor;               // [n]
     u32 *subset;                   // [n] staging for eval_direct
+    u8 *cls_user, *cls_sorted;     // [n] class of every body (0 field star, 1 black hole), user order and Morton order
     double *hard_out;              // [7n] staging of p3t_eval_hard's host outputs (acc 3n, jerk 3n, pot n); of p3t_hermite_step's pos, vel
     u32 *herm_ids;                 // [n] non-isolated particles by connected component of the neighbour graph (hermite.cu)
     u32 *herm_parent, *herm_root, *herm_csize, *herm_cstart;   // [n] union-find parent, root, component size / fill cursor, first member slot
@@ -138,6 +151,8 @@ struct p3t_ctx {
     int key_bits, max_level, nleaf, ngroup, merge_levels;
     int herm_cluster_max;          // largest component a thread-block cluster integrates (larger ones: grid kernel)
     int walk_mode;                 // 0 auto, 1 one warp per group, 2 one CTA per group (cooperative)
+    size_t cls_n;                  // 0: no classes; else the particle count the classes were given for
+    float r_in_bf, r_out_bf, r_search_bf, eps_bb;
     int shard_rank, shard_world;   // this context walks the groups at positions rank, rank + world, ... of the hand-out order
     int sm_count;
     bool have_params, loaded, built, evaluated;
@@ -209,7 +224,7 @@ p3t_status p3t_stage_narrow(p3t_ctx *ctx, const double *d_pos, float *d_pos32);
 
 // Cutoff weights on the slow path (pairs with s < r_out), double precision because the closed
 // form of W cancels from terms of size ~57 at gamma = 0.1 (hard part 8).
-__device__ __forceinline__ void p3t_pair_weights(const P3TParams &p, float s2, float &K, float &W)
+__device__ __forceinline__ void p3t_pair_weights(const CutoffSet &p, float s2, float &K, float &W)
 {
     double s = sqrt((double)s2);
     double y = s * p.inv_rout;

@@ -353,12 +353,15 @@ __global__ void __launch_bounds__(SORT_THREADS, 1024 / SORT_THREADS) onesweep_ke
 // clev[0] = clev[n] = -1.
 __global__ void __launch_bounds__(256) gather_kernel(const float4 *__restrict__ body_user, const u32 *__restrict__ idx,
                                                      const u64 *__restrict__ keys, float4 *__restrict__ body,
-                                                     signed char *__restrict__ clev, u32 n, int max_level)
+                                                     signed char *__restrict__ clev, u32 n, int max_level,
+                                                     const u8 *__restrict__ cls_user, u8 *__restrict__ cls_sorted)
 {
     u32 i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i > n) return;
     if (i == n) { clev[n] = -1; return; }
-    body[i] = body_user[idx[i]];
+    const u32 src = idx[i];
+    body[i] = body_user[src];
+    if (cls_user) cls_sorted[i] = cls_user[src] & 1u;   // pair classes (p3t_set_pair_classes): 0 field star, 1 black hole
     int c = -1;
     if (i > 0) {
         u64 x = keys[i] ^ keys[i - 1];
@@ -417,7 +420,8 @@ p3t_status p3t_stage_sort(p3t_ctx *ctx)
         cur ^= 1;
     }
     ctx->cur = cur;
-    gather_kernel<<<div_up(n + 1, 256), 256, 0, s>>>(w.body_user, w.idx[cur], w.keys[cur], w.body, w.clev, n, ctx->max_level);
+    gather_kernel<<<div_up(n + 1, 256), 256, 0, s>>>(w.body_user, w.idx[cur], w.keys[cur], w.body, w.clev, n, ctx->max_level,
+                                                     ctx->cls_n ? w.cls_user : nullptr, w.cls_sorted);
     P3T_CUDA(ctx, cudaGetLastError());
     return P3T_OK;
 }

@@ -263,27 +263,33 @@ __device__ __forceinline__ void eval_pc(const WarpShared &ws, u32 head, u32 cnt,
 
 // ---- p-p slow path: K (Eq. 12) on the force, W (Eq. 16-17) on the potential, j != i by index,
 //      neighbour emission for s_ij < h (reading A4) -------------------------------------------------
-template <int NI>
+//      With pair classes (CLS): the kind of the pair, class_i + class_j, selects the cutoff radii and the
+//      neighbour radius; a pair of kind 2 (two black holes) is not split: nothing in the soft sums, always neighbours.
+template <int NI, bool CLS>
 __device__ __forceinline__ void eval_near(const WarpShared &ws, u32 head, u32 cnt, const Targets<NI> &t,
-                                          const u32 (&isorted)[NI], const u32 (&iuser)[NI],
+                                          const u32 (&isorted)[NI], const u32 (&iuser)[NI], const u32 (&icls)[NI],
                                           const P3TParams &prm, const u32 *__restrict__ sorted_idx, uint2 *pairs, u64 pair_cap,
                                           u64 *counters, u32 (&nnb)[NI], Acc<NI> &acc, u32 lane)
 {
     for (u32 j = 0; j < cnt; ++j) {
         float4 bj = ws.near_buf[head + j];
         u32 js = ws.near_idx[head + j];
+        u32 cj = 0;
+        if (CLS) { cj = js >> 31; js &= 0x7fffffffu; }
 #pragma unroll
         for (int b = 0; b < NI; ++b) {
+            const u32 kind = CLS ? icls[b] + cj : 0u;
             float dx = bj.x + vget(t.nx, b), dy = bj.y + vget(t.ny, b), dz = bj.z + vget(t.nz, b);
             float s2 = fmaf(dx, dx, fmaf(dy, dy, fmaf(dz, dz, prm.eps2)));
             bool live = isorted[b] != 0xffffffffu && isorted[b] != js;
-            bool hit = live && s2 < prm.h2;
-            if (live) {
+            bool hit = live && (CLS ? (kind == 2u || s2 < prm.h2_k[kind & 1u]) : s2 < prm.h2);
+            if (live && !(CLS && kind == 2u)) {
                 float rinv = rsq(s2);
                 float mrinv = bj.w * rinv;
                 float mr3 = mrinv * (rinv * rinv);
                 float K = 1.f, W = 1.f;
-                if (s2 < prm.rout2) p3t_pair_weights(prm, s2, K, W);
+                if (CLS) { if (s2 < prm.rout2_k[kind]) p3t_pair_weights(prm.cs[kind], s2, K, W); }
+                else if (s2 < prm.rout2) p3t_pair_weights(prm.cs[0], s2, K, W);
                 mr3 *= K;
                 vref(acc.ax, b) = fmaf(mr3, dx, vget(acc.ax, b));
                 vref(acc.ay, b) = fmaf(mr3, dy, vget(acc.ay, b));
@@ -340,6 +346,8 @@ struct WalkArgs {
     uint2 *pairs;
     u64 pair_cap;
     u64 *counters;
+    const u8 *__restrict__ cls_sorted;   // pair classes (walk_kernel<.., .., true> only)
+    const float *__restrict__ cube;
 };
 
 // starts the asynchronous copy of the records of the popped cells into the landing area
@@ -400,7 +408,11 @@ __device__ __forceinline__ u32 coop_acquire(WarpShared &ws, const StackRef &st, 
 // cells from the shared stack (under a lock, lane 0), builds and evaluates its own lists; the partial
 // sums of warps 1-3 are added to warp 0's at the end.  Which warp meets which cell depends on timing,
 // so results are reproducible to fp32 rounding of the batch sums, not bitwise.
-template <int NI, bool COOP>
+// CLS (pair classes): a group that holds a black hole keeps every cell with a body within h_bf of its box
+// open (cells were given their radius for field-star groups: h, or h_bf if the cell itself holds a black hole) and never
+// accepts a cell that holds a black hole (BH-BH pairs are not split); bodies go to the K/W path when they are within
+// the neighbour radius of the kinds of pairs they can form with the group, black holes met by such a group always.
+template <int NI, bool COOP, bool CLS>
 __device__ __forceinline__ void walk_group(WarpShared *wsall, const StackRef &st, CtaCtl *ctl, const WalkArgs &A,
                                            const P3TParams &prm, u32 gs, u32 ge, u32 lane, u32 warp, u64 &tot_pp, u64 &tot_pc,
                                            u64 &tot_near)
@@ -410,7 +422,7 @@ __device__ __forceinline__ void walk_group(WarpShared *wsall, const StackRef &st
     WPROF_DECL;
     // ---- my bodies; empty slots replicate the group's first body and are flagged dead
     Targets<NI> tg;
-    u32 isorted[NI], iuser[NI], nnb[NI];
+    u32 isorted[NI], iuser[NI], nnb[NI], icls[NI];
     float lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY};
 #pragma unroll
     for (int b = 0; b < NI; ++b) {
@@ -420,6 +432,7 @@ __device__ __forceinline__ void walk_group(WarpShared *wsall, const StackRef &st
         vref(tg.nx, b) = -p.x; vref(tg.ny, b) = -p.y; vref(tg.nz, b) = -p.z;
         isorted[b] = ok ? k : 0xffffffffu;
         iuser[b] = ok ? A.sorted_idx[k] : 0u;
+        icls[b] = (CLS && ok) ? (u32)A.cls_sorted[k] : 0u;
         nnb[b] = 0;
         lo[0] = fminf(lo[0], p.x); hi[0] = fmaxf(hi[0], p.x);
         lo[1] = fminf(lo[1], p.y); hi[1] = fmaxf(hi[1], p.y);
@@ -437,6 +450,15 @@ __device__ __forceinline__ void walk_group(WarpShared *wsall, const StackRef &st
     acc.zero();
     tg.seal();
     WP(9);
+    bool heavy_group = false;
+    float slack = 0.f;
+    if (CLS) {
+        u32 any = 0;
+#pragma unroll
+        for (int b = 0; b < NI; ++b) any |= icls[b];
+        heavy_group = __any_sync(0xffffffffu, any != 0);
+        slack = 8.f * 1.1920929e-7f * (fabsf(A.cube[0]) + fabsf(A.cube[1]) + fabsf(A.cube[2]) + 2.f * A.cube[3]);   // as moments.cu
+    }
 
     u32 top = 1;
     if (!COOP && lane == 0) st.smem[0] = 0;   // root (cooperative mode: placed by the kernel)
@@ -461,6 +483,11 @@ __device__ __forceinline__ void walk_group(WarpShared *wsall, const StackRef &st
             float ez = fmaxf(0.f, fmaxf(lo[2] - a.z, a.z - hi[2]));
             float d2 = fmaf(ex, ex, fmaf(ey, ey, ez * ez));
             accept = d2 > a.w;
+            if (CLS && heavy_group && accept) {
+                const float rm = ws.l_mom1[lane].w;                       // bounding radius; sign bit: the cell holds a black hole
+                const float rc = (prm.h_bf + fabsf(rm)) * (1.f + 1e-5f) + slack;
+                accept = !(__float_as_uint(rm) >> 31) && d2 > rc * rc;
+            }
             if (!accept) {
                 uint2 meta = ws.l_meta[lane];
                 if (meta.y & P3T_LEAF_FLAG) { lstart = meta.x; lcount = meta.y & ~P3T_LEAF_FLAG; }
@@ -529,7 +556,7 @@ __device__ __forceinline__ void walk_group(WarpShared *wsall, const StackRef &st
             }
             const u32 total = __shfl_sync(0xffffffffu, inc, 31);
             const u32 excl = inc - lcount;
-            auto fetch = [&](u32 v0, float4 &bj, u32 &bidx, bool &hv) {
+            auto fetch = [&](u32 v0, float4 &bj, u32 &bidx, bool &hv, u32 &cj) {
                 u32 v = v0 + lane;
                 u32 s = 0;   // owner lane: largest s with excl[s] <= v
 #pragma unroll
@@ -543,20 +570,26 @@ __device__ __forceinline__ void walk_group(WarpShared *wsall, const StackRef &st
                 hv = v < total;
                 bidx = s_start + (v - s_excl);
                 bj = A.body[hv ? bidx : gs];
+                if (CLS) cj = A.cls_sorted[hv ? bidx : gs];
             };
             float4 bj = make_float4(0.f, 0.f, 0.f, 0.f), bn = bj;
-            u32 bidx = 0, bidxn = 0;
+            u32 bidx = 0, bidxn = 0, cj = 0, cjn = 0;
             bool hv = false, hvn = false;
-            if (total) fetch(0, bj, bidx, hv);
+            if (total) fetch(0, bj, bidx, hv, cj);
             for (u32 v0 = 0; v0 < total; v0 += 32) {
                 WPC(11);
                 hvn = false;
-                if (v0 + 32 < total) fetch(v0 + 32, bn, bidxn, hvn);
+                if (v0 + 32 < total) fetch(v0 + 32, bn, bidxn, hvn, cjn);
                 float ex = fmaxf(0.f, fmaxf(lo[0] - bj.x, bj.x - hi[0]));
                 float ey = fmaxf(0.f, fmaxf(lo[1] - bj.y, bj.y - hi[1]));
                 float ez = fmaxf(0.f, fmaxf(lo[2] - bj.z, bj.z - hi[2]));
                 float d2 = fmaf(ex, ex, fmaf(ey, ey, ez * ez));
-                bool isnear = hv && d2 < prm.hnear2;
+                float thr = prm.hnear2;
+                if (CLS) {
+                    if (cj != 0 || heavy_group) thr = prm.hnear2_bf;
+                    if (cj != 0 && heavy_group) thr = INFINITY;          // two black holes: always the slow path
+                }
+                bool isnear = hv && d2 < thr;
                 bool isfar = hv && !isnear;
                 u32 fb = __ballot_sync(0xffffffffu, isfar), nb = __ballot_sync(0xffffffffu, isnear);
                 if (isfar) {
@@ -566,7 +599,7 @@ __device__ __forceinline__ void walk_group(WarpShared *wsall, const StackRef &st
                 if (isnear) {
                     u32 slot = (near_head + near_cnt + __popc(nb & lanemask_lt())) & 63u;
                     ws.near_buf[slot] = bj;
-                    ws.near_idx[slot] = bidx;
+                    ws.near_idx[slot] = CLS ? (bidx | (cj << 31)) : bidx;
                 }
                 far_cnt += __popc(fb);
                 near_cnt += __popc(nb);
@@ -579,13 +612,13 @@ __device__ __forceinline__ void walk_group(WarpShared *wsall, const StackRef &st
                 }
                 if (near_cnt >= 32) {
                     WP(5);
-                    eval_near<NI>(ws, near_head, 32, tg, isorted, iuser, prm, A.sorted_idx, A.pairs, A.pair_cap, A.counters, nnb,
+                    eval_near<NI, CLS>(ws, near_head, 32, tg, isorted, iuser, icls, prm, A.sorted_idx, A.pairs, A.pair_cap, A.counters, nnb,
                                   acc, lane);
                     WP(6);
                     near_head = (near_head + 32) & 63u; near_cnt -= 32; n_near += 32;
                 }
                 __syncwarp();
-                bj = bn; bidx = bidxn; hv = hvn;
+                bj = bn; bidx = bidxn; hv = hvn; cj = cjn;
             }
         }
         // ---- a full batch of accepted cells
@@ -608,7 +641,7 @@ __device__ __forceinline__ void walk_group(WarpShared *wsall, const StackRef &st
     if (pc_cnt) { eval_pc<NI>(ws, pc_head, pc_cnt, tg, prm.eps2, acc); n_pc += pc_cnt; }
     if (far_cnt) { eval_far<NI>(ws, far_head, far_cnt, tg, prm.eps2, acc); n_far += far_cnt; }
     if (near_cnt) {
-        eval_near<NI>(ws, near_head, near_cnt, tg, isorted, iuser, prm, A.sorted_idx, A.pairs, A.pair_cap, A.counters, nnb, acc, lane);
+        eval_near<NI, CLS>(ws, near_head, near_cnt, tg, isorted, iuser, icls, prm, A.sorted_idx, A.pairs, A.pair_cap, A.counters, nnb, acc, lane);
         n_near += near_cnt;
     }
     acc.flush();
@@ -667,7 +700,7 @@ __device__ __forceinline__ void walk_group(WarpShared *wsall, const StackRef &st
 // (COOP = false) or one per CTA (COOP = true).  A group of at most 32 bodies takes the one-body-per-lane
 // path (half the FP32 work of the packed path).
 // Shared memory: WALK_WARPS x WarpShared | WALK_WARPS x WALK_STACK_SMEM stack words | CtaCtl
-template <int NIMAX, bool COOP>
+template <int NIMAX, bool COOP, bool CLS>
 __global__ void __launch_bounds__(WALK_WARPS * 32, WALK_CTAS)
 walk_kernel(WalkArgs A, const u32 *__restrict__ group_start, P3TParams prm, u32 *walk_stack)
 {
@@ -719,8 +752,8 @@ walk_kernel(WalkArgs A, const u32 *__restrict__ group_start, P3TParams prm, u32 
         const u32 gs = group_start[g], ge = group_start[g + 1];
         const u64 pp0 = tot_pp, pc0 = tot_pc;
         const u32 t0 = (u32)globaltimer_ns();
-        if (NIMAX == 2 && ge - gs > 32) walk_group<2, COOP>(wsall, st, ctl, A, prm, gs, ge, lane, warp, tot_pp, tot_pc, tot_near);
-        else walk_group<1, COOP>(wsall, st, ctl, A, prm, gs, ge, lane, warp, tot_pp, tot_pc, tot_near);
+        if (NIMAX == 2 && ge - gs > 32) walk_group<2, COOP, CLS>(wsall, st, ctl, A, prm, gs, ge, lane, warp, tot_pp, tot_pc, tot_near);
+        else walk_group<1, COOP, CLS>(wsall, st, ctl, A, prm, gs, ge, lane, warp, tot_pp, tot_pc, tot_near);
         __syncwarp();
         // diagnostics: list lengths of this group (+1: the self term removed from tot_pp) and its time window
         if (COOP) {
@@ -821,11 +854,11 @@ p3t_status p3t_stage_walk(p3t_ctx *ctx)
     u32 grid = (u32)ctx->sm_count * WALK_CTAS;
     if ((size_t)grid * WALK_WARPS > w.walk_warps_max) grid = (u32)(w.walk_warps_max / WALK_WARPS);
     const size_t smem = (sizeof(WarpShared) + WALK_STACK_SMEM * sizeof(u32)) * WALK_WARPS + sizeof(CtaCtl);
+    typedef void (*walk_fn)(WalkArgs, const u32 *, P3TParams, u32 *);
+    static const walk_fn fns[8] = {walk_kernel<1, false, false>, walk_kernel<2, false, false>, walk_kernel<1, true, false>, walk_kernel<2, true, false>,
+                                   walk_kernel<1, false, true>,  walk_kernel<2, false, true>,  walk_kernel<1, true, true>,  walk_kernel<2, true, true>};
     if (!ctx->walk_attr_set) {   // function attributes are per device: kept per context
-        P3T_CUDA(ctx, cudaFuncSetAttribute(walk_kernel<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        P3T_CUDA(ctx, cudaFuncSetAttribute(walk_kernel<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        P3T_CUDA(ctx, cudaFuncSetAttribute(walk_kernel<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        P3T_CUDA(ctx, cudaFuncSetAttribute(walk_kernel<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        for (int k = 0; k < 8; ++k) P3T_CUDA(ctx, cudaFuncSetAttribute(fns[k], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         ctx->walk_attr_set = true;
     }
     WalkArgs A;
@@ -839,6 +872,8 @@ p3t_status p3t_stage_walk(p3t_ctx *ctx)
     A.order_hist = w.order_hist;
     A.shard_rank = (u32)ctx->shard_rank;
     A.shard_world = (u32)ctx->shard_world;
+    A.cls_sorted = w.cls_sorted;
+    A.cube = w.cube;
     if (ctx->shard_world > 1) {   // particles of the groups other ranks walk: zero acceleration, potential, neighbour count
         P3T_CUDA(ctx, cudaMemsetAsync(w.accpot, 0, ctx->n * sizeof(float4), s));
         P3T_CUDA(ctx, cudaMemsetAsync(w.nbr_count, 0, ctx->n * sizeof(u32), s));
@@ -854,13 +889,7 @@ p3t_status p3t_stage_walk(p3t_ctx *ctx)
     // (the group count lives on the device; n / ngroup is its lower bound up to the fill of the groups)
     bool coop = ctx->walk_mode == 2 || (ctx->walk_mode == 0 && 20 * (ctx->n / (size_t)ctx->ngroup) < (size_t)WALK_COOP_BELOW_X20 * grid * WALK_WARPS);
     const dim3 block(WALK_WARPS * 32);
-    if (ctx->ngroup == 64) {
-        if (coop) walk_kernel<2, true><<<grid, block, smem, s>>>(A, w.group_start, ctx->prm, w.walk_stack);
-        else walk_kernel<2, false><<<grid, block, smem, s>>>(A, w.group_start, ctx->prm, w.walk_stack);
-    } else {
-        if (coop) walk_kernel<1, true><<<grid, block, smem, s>>>(A, w.group_start, ctx->prm, w.walk_stack);
-        else walk_kernel<1, false><<<grid, block, smem, s>>>(A, w.group_start, ctx->prm, w.walk_stack);
-    }
+    fns[(ctx->ngroup == 64 ? 1 : 0) + (coop ? 2 : 0) + (ctx->cls_n ? 4 : 0)]<<<grid, block, smem, s>>>(A, w.group_start, ctx->prm, w.walk_stack);
     P3T_CUDA(ctx, cudaGetLastError());
     return P3T_OK;
 }
