@@ -429,6 +429,7 @@ __global__ void __launch_bounds__(BUILD_THREADS) emit_kernel(
                     u32 parent = P3T_NO_PARENT;
                     if (L > 0) {
                         parent = prev_flag[s] ? prev_rank[s] : prev_rank[s] - 1;
+                        P3T_DEV_ASSERT(parent < rank);
                         atomicAdd(&cell_nchild[parent], L == D[s] ? 1u : 0x10001u);   // children | internal children << 16
                     }
                     cell_parent[rank] = parent;
@@ -439,6 +440,7 @@ __global__ void __launch_bounds__(BUILD_THREADS) emit_kernel(
                         while (tl + cnt <= BUILD_TILE + BUILD_HALO && s_c[tl + cnt] >= L) ++cnt;
                         if (tl + cnt > BUILD_TILE + BUILD_HALO)
                             while (i + cnt < n && clev[i + cnt] >= L) ++cnt;   // a deep leaf longer than the window
+                        P3T_DEV_ASSERT(i + cnt <= n);
                         cell_meta[rank] = make_uint2(i, cnt | P3T_LEAF_FLAG);
                         ++nleaf_here;
                     } else {
@@ -470,7 +472,7 @@ __global__ void __launch_bounds__(BUILD_THREADS) emit_kernel(
         for (int w = 0; w < warp; ++w) pos += s_whead[w];
 #pragma unroll
         for (int s = 0; s < BUILD_PER_THREAD; ++s)
-            if ((head_mask >> s) & 1u) group_start[pos++] = i0 + s;
+            if ((head_mask >> s) & 1u) { P3T_DEV_ASSERT(pos < n); group_start[pos++] = i0 + s; }
     }
 }
 

@@ -47,6 +47,7 @@ __global__ void __launch_bounds__(HARD_THREADS) hard_kernel(const float4 *__rest
     double ax = 0, ay = 0, az = 0, jx = 0, jy = 0, jz = 0, ph = 0;
     for (u64 k = offset[i], e = offset[i + 1]; k < e; ++k) {
         const u32 j = nbr[k];
+        P3T_DEV_ASSERT(j < n && j != i);
         const float4 bj = body_user[j];
         const double dx = (double)bi.x - (double)bj.x, dy = (double)bi.y - (double)bj.y, dz = (double)bi.z - (double)bj.z;
         const double wx = vix - (double)vel[3 * (size_t)j], wy = viy - (double)vel[3 * (size_t)j + 1],

@@ -200,6 +200,7 @@ __global__ void cc_scatter_kernel(const u64 *__restrict__ offset, u32 n, const u
     if (i >= n || offset[i + 1] == offset[i]) return;
     const u32 r = root[i];
     const u32 st = cstart[r], p = atomicAdd(&csize[r], 1u);            // order inside a component is irrelevant
+    P3T_DEV_ASSERT(r < n && (st & ~HERM_GRID_FLAG) + p < n);
     if (st & HERM_GRID_FLAG) grid_members[(st & ~HERM_GRID_FLAG) + p] = i;
     else members[st + p] = i;
 }

@@ -135,6 +135,7 @@ __global__ void __launch_bounds__(128, 4) moments_kernel(
         if (PHASE == 0) {
             // ---- leaf: one pass over its bodies, sums about the first body, then shifted to the centre of mass
             const u32 cnt = meta.y & ~P3T_LEAF_FLAG;
+            P3T_DEV_ASSERT(cnt >= 1 && meta.x == start);
             const float4 b0 = body[start];
             float sx = 0.f, sy = 0.f, sz = 0.f, M = 0.f;
             float qxx = 0.f, qyy = 0.f, qzz = 0.f, qxy = 0.f, qxz = 0.f, qyz = 0.f;
@@ -181,6 +182,7 @@ __global__ void __launch_bounds__(128, 4) moments_kernel(
         u64 key = keys[start];
         while (true) {
             const u32 nch = cw & 0xffffu;
+            P3T_DEV_ASSERT(nch >= 1 && nch <= 8 && first > k && first + nch <= ncell && (parent == P3T_NO_PARENT || parent < k));
             // what the next step needs of the parent does not depend on this merge: requested now, so that
             // one level of the climb costs the merge loads, a fence and an atomic, nothing more
             u32 pcw = 0, pfirst = 0, pparent = P3T_NO_PARENT, pstart = 0;

@@ -107,6 +107,7 @@ __global__ void __launch_bounds__(256) fill_lists_kernel(const uint2 *__restrict
     for (u64 p = (u64)blockIdx.x * blockDim.x + threadIdx.x; p < total; p += (u64)gridDim.x * blockDim.x) {
         uint2 pr = pairs[p];
         u32 slot = atomicAdd(&cursor[pr.x], 1u);
+        P3T_DEV_ASSERT(offset[pr.x] + slot < offset[pr.x + 1] && offset[pr.x + 1] <= total);
         nbr[offset[pr.x] + slot] = pr.y;
     }
 }
@@ -124,7 +125,9 @@ __global__ void __launch_bounds__(256) sort_lists_kernel(const u32 *__restrict__
     u32 c = count[i];
     if (c < 2) return;
     if (c > SORT_LIST_SERIAL) {
-        worklist[atomicAdd(&counters[CNT_EVAL_SPARE], 1ull)] = i;
+        const u64 wslot = atomicAdd(&counters[CNT_EVAL_SPARE], 1ull);
+        P3T_DEV_ASSERT(wslot < n);
+        worklist[wslot] = i;
         return;
     }
     u32 *l = nbr + offset[i];

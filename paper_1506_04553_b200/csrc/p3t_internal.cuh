@@ -220,6 +220,21 @@ p3t_status p3t_stage_kick(p3t_ctx *ctx, double *d_vel, double dt);
 p3t_status p3t_stage_narrow(p3t_ctx *ctx, const double *d_pos, float *d_pos32);
 
 #ifdef __CUDACC__
+// Checked build (P3T_CHECKED=1 python -m paper_1506_04553_b200.build --force; profiles/sanitizer_r2.md): every index a
+// kernel takes from the tree, a list or a look-back result is tested against the size of the array it goes into; a
+// violation prints the place and traps (the launch fails, the next API call returns P3T_ECUDA).  Nothing in a normal build.
+#ifdef P3T_CHECKED
+#define P3T_DEV_ASSERT(cond)                                                                                         \
+    do {                                                                                                             \
+        if (!(cond)) {                                                                                               \
+            printf("P3T_DEV_ASSERT failed: %s (%s:%d) block %u thread %u\n", #cond, __FILE__, __LINE__, blockIdx.x, threadIdx.x); \
+            __trap();                                                                                                \
+        }                                                                                                            \
+    } while (0)
+#else
+#define P3T_DEV_ASSERT(cond) do { } while (0)
+#endif
+
 // ---- device helpers ----------------------------------------------------------------------------
 
 // Cutoff weights on the slow path (pairs with s < r_out), double precision because the closed

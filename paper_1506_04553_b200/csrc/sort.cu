@@ -220,6 +220,7 @@ __global__ void __launch_bounds__(SORT_THREADS, 1024 / SORT_THREADS) onesweep_ke
     for (u32 t = 0; t < 8; ++t) sm.whist[warp][t * 32 + lane] = 0;
     __syncthreads();
     const u32 tile = sm.tile;
+    P3T_DEV_ASSERT(tile < (n + SORT_TILE - 1) / SORT_TILE);
     const u32 tile_base = tile * SORT_TILE;
     const u32 tile_valid = min((u32)SORT_TILE, n - tile_base);
     if (tid < 256) status_next[(size_t)tile * 256 + tid] = 0;   // row of the buffer the next pass uses
@@ -340,6 +341,7 @@ __global__ void __launch_bounds__(SORT_THREADS, 1024 / SORT_THREADS) onesweep_ke
             u64 kk = sm.x.key[p];
             u32 d = (u32)(kk >> shift) & 255u;
             u32 dst = sm.goff[d] + p;
+            P3T_DEV_ASSERT(dst < n);
             kout[dst] = kk;
             vout[dst] = sm.x.val[p];
         }
@@ -360,6 +362,7 @@ __global__ void __launch_bounds__(256) gather_kernel(const float4 *__restrict__ 
     if (i > n) return;
     if (i == n) { clev[n] = -1; return; }
     const u32 src = idx[i];
+    P3T_DEV_ASSERT(src < n);
     body[i] = body_user[src];
     if (cls_user) cls_sorted[i] = cls_user[src] & 1u;   // pair classes (p3t_set_pair_classes): 0 field star, 1 black hole
     int c = -1;

@@ -145,9 +145,14 @@ struct StackRef {
     u32 cap;       // shared-memory entries
     u32 limit;     // total entries
 };
-__device__ __forceinline__ u32 stack_read(const StackRef &st, u32 pos) { return pos < st.cap ? st.smem[pos] : st.gmem[pos - st.cap]; }
+__device__ __forceinline__ u32 stack_read(const StackRef &st, u32 pos)
+{
+    P3T_DEV_ASSERT(pos < st.limit);
+    return pos < st.cap ? st.smem[pos] : st.gmem[pos - st.cap];
+}
 __device__ __forceinline__ void stack_write(const StackRef &st, u32 pos, u32 v)
 {
+    P3T_DEV_ASSERT(pos < st.limit);
     if (pos < st.cap) st.smem[pos] = v;
     else st.gmem[pos - st.cap] = v;
 }
@@ -303,6 +308,7 @@ __device__ __forceinline__ void eval_near(const WarpShared &ws, u32 head, u32 cn
                 base = __shfl_sync(0xffffffffu, base, 0);
                 if (hit) {
                     u64 pos = base + __popc(hb & lanemask_lt());
+                    P3T_DEV_ASSERT(js < 0x40000000u);
                     if (pos < pair_cap) pairs[pos] = make_uint2(iuser[b], sorted_idx[js]);
                     ++nnb[b];
                 }
@@ -348,12 +354,14 @@ struct WalkArgs {
     u64 *counters;
     const u8 *__restrict__ cls_sorted;   // pair classes (walk_kernel<.., .., true> only)
     const float *__restrict__ cube;
+    u32 n;                               // bodies (checked builds test indices against it)
 };
 
 // starts the asynchronous copy of the records of the popped cells into the landing area
 __device__ __forceinline__ void request_cells(WarpShared &ws, const WalkArgs &A, u32 take, u32 lane, u32 cell)
 {
     if (lane < take) {
+        P3T_DEV_ASSERT((u64)cell < A.counters[CNT_NCELLS]);
         cp_async16(&ws.l_mac[lane], &A.cell_mac[cell]);
         cp_async8(&ws.l_meta[lane], &A.cell_meta[cell]);
         cp_async16(&ws.l_mom0[lane], &A.cell_mom0[cell]);
@@ -490,8 +498,8 @@ __device__ __forceinline__ void walk_group(WarpShared *wsall, const StackRef &st
             }
             if (!accept) {
                 uint2 meta = ws.l_meta[lane];
-                if (meta.y & P3T_LEAF_FLAG) { lstart = meta.x; lcount = meta.y & ~P3T_LEAF_FLAG; }
-                else { first = meta.x; nch = meta.y; }
+                if (meta.y & P3T_LEAF_FLAG) { lstart = meta.x; lcount = meta.y & ~P3T_LEAF_FLAG; P3T_DEV_ASSERT(lcount >= 1 && lstart + lcount <= A.n); }
+                else { first = meta.x; nch = meta.y; P3T_DEV_ASSERT(nch >= 1 && nch <= 8 && (u64)first + nch <= A.counters[CNT_NCELLS]); }
             }
         }
         // ---- accepted cells -> p-c ring (at most 31 pending + 32 new entries, capacity 64)
@@ -569,6 +577,7 @@ __device__ __forceinline__ void walk_group(WarpShared *wsall, const StackRef &st
                 u32 s_excl = __shfl_sync(0xffffffffu, excl, s);
                 hv = v < total;
                 bidx = s_start + (v - s_excl);
+                P3T_DEV_ASSERT(!hv || bidx < A.n);
                 bj = A.body[hv ? bidx : gs];
                 if (CLS) cj = A.cls_sorted[hv ? bidx : gs];
             };
@@ -750,6 +759,7 @@ walk_kernel(WalkArgs A, const u32 *__restrict__ group_start, P3TParams prm, u32 
             continue;
         }
         const u32 gs = group_start[g], ge = group_start[g + 1];
+        P3T_DEV_ASSERT(gs < ge && ge <= A.n && ge - gs <= 32u * NIMAX);
         const u64 pp0 = tot_pp, pc0 = tot_pc;
         const u32 t0 = (u32)globaltimer_ns();
         if (NIMAX == 2 && ge - gs > 32) walk_group<2, COOP, CLS>(wsall, st, ctl, A, prm, gs, ge, lane, warp, tot_pp, tot_pc, tot_near);
@@ -874,6 +884,7 @@ p3t_status p3t_stage_walk(p3t_ctx *ctx)
     A.shard_world = (u32)ctx->shard_world;
     A.cls_sorted = w.cls_sorted;
     A.cube = w.cube;
+    A.n = (u32)ctx->n;
     if (ctx->shard_world > 1) {   // particles of the groups other ranks walk: zero acceleration, potential, neighbour count
         P3T_CUDA(ctx, cudaMemsetAsync(w.accpot, 0, ctx->n * sizeof(float4), s));
         P3T_CUDA(ctx, cudaMemsetAsync(w.nbr_count, 0, ctx->n * sizeof(u32), s));
