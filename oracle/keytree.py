@@ -3,6 +3,10 @@
 Plain numpy / pure-Python restatement of
   a2  Morton keys: quantise to `max_level` bits per dimension relative to the root cube and
       interleave (x most significant)                                  -- north_star; A11
+      Peano-Hilbert keys: the same quantised cell coordinates taken through the transform of J. Skilling,
+      "Programming the Hilbert curve" (AIP Conf. Proc. 707, 2004: AxestoTranspose / TransposetoAxes), then
+      interleaved the same way.  Both curves visit the same octree cells (a level-l cell is a run of keys
+      sharing their top 3 l bits); they differ in the order of the octants inside a cell       -- DESIGN.md A25
   a5  octree from the sorted keys: a cell (a maximal run of keys sharing a 3*level-bit prefix) with
       more than NLEAF bodies is split into its non-empty octants, until <= NLEAF or level =
       max_level ("Barnes-Hut tree"; leaf capacity and depth: DESIGN.md A11)
@@ -29,6 +33,80 @@ def root_cube(pos):
     lo, hi = q.min(axis=0), q.max(axis=0)
     side = float((hi - lo).max())
     return 0.5 * (lo + hi) - 0.5 * side, side
+
+
+def _interleave(cells, max_level):
+    key = np.zeros(cells[0].shape[0], dtype=np.uint64)
+    for k in range(max_level):
+        for d, sh in ((0, 2), (1, 1), (2, 0)):
+            bit = (cells[d] >> np.uint64(k)) & np.uint64(1)
+            key |= bit << np.uint64(3 * k + sh)
+    return key
+
+
+def quantise(pos, cube_min, side, max_level, dtype=np.float32):
+    """Integer cell coordinates (three uint64 arrays) of positions at the finest level, as morton_keys takes them."""
+    ft = np.dtype(dtype).type
+    q = np.asarray(pos, dtype=dtype).reshape(-1, 3)
+    cmin = np.asarray(cube_min, dtype=dtype)
+    scale = ft(ft(1 << max_level) / ft(side))
+    qmax = (1 << max_level) - 1
+    cells = []
+    for d in range(3):
+        t = np.maximum((q[:, d] - cmin[d]) * scale, ft(0.0))
+        cells.append(np.minimum(t.astype(np.int64), qmax).astype(np.uint64))
+    return cells
+
+
+def hilbert_keys(pos, cube_min, side, max_level, dtype=np.float32):
+    """Peano-Hilbert keys: Skilling's AxestoTranspose on the quantised coordinates, written out for arrays, then
+    the bits interleaved as in morton_keys (X[0] most significant in every triple)."""
+    X = quantise(pos, cube_min, side, max_level, dtype)
+    one = np.uint64(1)
+    M = one << np.uint64(max_level - 1)
+    Q = M
+    while Q > one:                                   # "inverse undo"
+        P = Q - one
+        for i in range(3):
+            hit = (X[i] & Q) != 0
+            t = np.where(hit, np.uint64(0), (X[0] ^ X[i]) & P)
+            X[0] = np.where(hit, X[0] ^ P, X[0] ^ t)   # invert / exchange
+            X[i] = X[i] ^ t if i else X[0]
+        Q >>= one
+    for i in range(1, 3):                            # Gray encode
+        X[i] = X[i] ^ X[i - 1]
+    t = np.zeros_like(X[0])
+    Q = M
+    while Q > one:
+        t = np.where((X[2] & Q) != 0, t ^ (Q - one), t)
+        Q >>= one
+    return _interleave([x ^ t for x in X], max_level)
+
+
+def hilbert_decode(key, max_level):
+    """Integer cell coordinates (ix, iy, iz) of one key: Skilling's TransposetoAxes, python ints."""
+    key = int(key)
+    X = [0, 0, 0]
+    for k in range(max_level):
+        for d, sh in ((0, 2), (1, 1), (2, 0)):
+            X[d] |= ((key >> (3 * k + sh)) & 1) << k
+    N = 2 << (max_level - 1)
+    t = X[2] >> 1                                    # Gray decode
+    for i in (2, 1):
+        X[i] ^= X[i - 1]
+    X[0] ^= t
+    Q = 2
+    while Q != N:                                    # undo excess work
+        P = Q - 1
+        for i in (2, 1, 0):
+            if X[i] & Q:
+                X[0] ^= P
+            else:
+                t = (X[0] ^ X[i]) & P
+                X[0] ^= t
+                X[i] ^= t
+        Q <<= 1
+    return tuple(X)
 
 
 def morton_keys(pos, cube_min, side, max_level, dtype=np.float32):
@@ -84,10 +162,14 @@ def build_cells(keys_sorted, nleaf, max_level):
     return cells
 
 
-def cell_geometry(cell, key, cube_min, side, max_level):
-    """Geometric centre and side of a cell from the key prefix of any of its bodies."""
+def cell_geometry(cell, key, cube_min, side, max_level, curve="morton"):
+    """Geometric centre and side of a cell from the key of any of its bodies."""
     L = cell["level"]
     l = side / (1 << L)
+    if curve == "hilbert":
+        ix, iy, iz = (c >> (max_level - L) for c in hilbert_decode(key, max_level))
+        g = np.asarray(cube_min, dtype=np.float64) + (np.array([ix, iy, iz]) + 0.5) * l
+        return g, l
     pre = int(key) >> (3 * (max_level - L)) if L else 0
     ix = iy = iz = 0
     for k in range(L):

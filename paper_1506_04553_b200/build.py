@@ -23,6 +23,8 @@ NVCC_FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-gencode", "arch=compute_100a,c
 # P3T_CHECKED=1: the kernels' own bounds checks (P3T_DEV_ASSERT of csrc/p3t_internal.cuh) are compiled in; use with --force
 if os.environ.get("P3T_CHECKED") == "1":
     NVCC_FLAGS = NVCC_FLAGS + ["-DP3T_CHECKED"]
+# tuning experiments: extra nvcc flags (e.g. P3T_NVCC_EXTRA="-DWALK_STACK_SMEM=1024"); use with --force
+NVCC_FLAGS = NVCC_FLAGS + os.environ.get("P3T_NVCC_EXTRA", "").split()
 
 
 def _nvcc():

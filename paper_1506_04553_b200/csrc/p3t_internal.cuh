@@ -30,7 +30,9 @@ typedef unsigned char u8;
 #ifndef WALK_CTAS
 #define WALK_CTAS 4                  // resident CTAs per SM the walk kernel is compiled for (register budget)
 #endif
+#ifndef WALK_STACK_SMEM
 #define WALK_STACK_SMEM 512          // stack entries per warp held in shared memory
+#endif
 #define WALK_STACK_GMEM 7168         // overflow entries per warp in global memory
 #ifndef WALK_COOP_BELOW_X20
 #define WALK_COOP_BELOW_X20 13         // auto mode: one CTA per group below 13 / 20 groups per resident warp (measured crossover:

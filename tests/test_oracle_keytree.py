@@ -40,15 +40,55 @@ def test_key_order_is_depth_first_octant_order():
     assert paths == sorted(paths)
 
 
+@pytest.mark.parametrize("b", [1, 2, 3, 4])
+def test_hilbert_keys_visit_a_lattice_once_and_move_to_a_face_neighbour_each_step(b):
+    """What makes a curve a Hilbert curve: a bijection of the 8^b cells onto 0 .. 8^b - 1 whose consecutive cells share
+    a face.  (Morton order fails the second half at every octant boundary.)"""
+    n = 1 << b
+    ijk = np.array([[x, y, z] for x in range(n) for y in range(n) for z in range(n)])
+    pts = (ijk + 0.5) / n
+    k = keytree.hilbert_keys(pts, [0, 0, 0], 1.0, b, dtype=np.float64)
+    assert sorted(k.tolist()) == list(range(8 ** b))
+    path = ijk[np.argsort(k)]
+    assert np.all(np.abs(np.diff(path, axis=0)).sum(axis=1) == 1)
+    assert path[0].tolist() == [0, 0, 0]
+    km = keytree.morton_keys(pts, [0, 0, 0], 1.0, b, dtype=np.float64)
+    if b > 1:
+        assert np.any(np.abs(np.diff(ijk[np.argsort(km)], axis=0)).sum(axis=1) > 1)
+    for key, c in zip(k, ijk):                                   # the inverse transform gives the cell back
+        assert keytree.hilbert_decode(key, b) == tuple(c)
+
+
+def test_hilbert_and_morton_keys_have_the_same_cells_at_every_level():
+    """A level-l cell is the set of bodies with equal top 3 l key bits, for both curves: the octree built from either
+    key is the same tree (only the order of the children differs)."""
+    rng = np.random.default_rng(9)
+    p = rng.uniform(0, 1, (4000, 3)) ** 2                       # clustered towards a corner: deep levels get used
+    L = 21
+    kh = keytree.hilbert_keys(p, [0, 0, 0], 1.0, L, dtype=np.float64)
+    km = keytree.morton_keys(p, [0, 0, 0], 1.0, L, dtype=np.float64)
+    cells = keytree.quantise(p, [0, 0, 0], 1.0, L, dtype=np.float64)
+    for l in (1, 2, 5, 9, 14, 21):
+        sh = np.uint64(3 * (L - l))
+        pairs = set(zip((kh >> sh).tolist(), (km >> sh).tolist()))
+        assert len(pairs) == len({a for a, _ in pairs}) == len({b for _, b in pairs})
+    for i in range(0, 4000, 97):
+        assert keytree.hilbert_decode(kh[i], L) == tuple(int(c[i]) for c in cells)
+    # 10-bit keys are the top 30 bits' worth of the same construction on the coarser lattice
+    k10 = keytree.hilbert_keys(p, [0, 0, 0], 1.0, 10, dtype=np.float64)
+    assert np.array_equal(k10, kh >> np.uint64(33))
+
+
+@pytest.mark.parametrize("curve", ["morton", "hilbert"])
 @pytest.mark.parametrize("nleaf,max_level", [(16, 10), (4, 21), (1, 21)])
-def test_key_tree_equals_pointer_tree(oracle, nleaf, max_level):
+def test_key_tree_equals_pointer_tree(oracle, nleaf, max_level, curve):
     c = workloads.config(1, n=3000)
     m, q = c["mass"].astype(np.float64), c["pos"].astype(np.float64)
     t = oracle.Tree(m, q, nleaf=nleaf, max_depth=max_level)
     nd = t.nodes()
     side = nd["side"][0]
     cmin = nd["g"][0] - 0.5 * side
-    keys = keytree.morton_keys(q, cmin, side, max_level, dtype=np.float64)
+    keys = (keytree.hilbert_keys if curve == "hilbert" else keytree.morton_keys)(q, cmin, side, max_level, dtype=np.float64)
     order = np.argsort(keys, kind="stable")
     cells = keytree.build_cells(keys[order], nleaf, max_level)
     assert len(cells) == t.nnodes
@@ -60,7 +100,7 @@ def test_key_tree_equals_pointer_tree(oracle, nleaf, max_level):
     geo_ptr = {(int(l), tuple(np.round(g / side, 9))) for l, g in zip(nd["level"], nd["g"])}
     geo_key = set()
     for x in cells:
-        g, l = keytree.cell_geometry(x, keys[order][x["start"]], cmin, side, max_level)
+        g, l = keytree.cell_geometry(x, keys[order][x["start"]], cmin, side, max_level, curve=curve)
         geo_key.add((x["level"], tuple(np.round(g / side, 9))))
     assert geo_ptr == geo_key
 
