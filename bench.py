@@ -157,6 +157,7 @@ def main():
     ap.add_argument("--nleaf", type=int, default=None)
     ap.add_argument("--ngroup", type=int, default=None)
     ap.add_argument("--merge", type=int, default=None)
+    ap.add_argument("--curve", default=None, choices=["morton", "hilbert"], help="p3t_set_key_curve (default: the library's, hilbert)")
     ap.add_argument("--shard", action="store_true",
                     help="strong scaling: ONE cluster, every rank walks every world-th i-group (p3t_set_shard) and the "
                          "accelerations and potentials are summed over the ranks (NCCL all-reduce inside the timed step)")
@@ -199,6 +200,8 @@ def main():
     ctx = binding.P3T(n, key_bits=cfg["key_bits"], nbr_capacity=max(n, 1 << 16), device=local)
     ctx.set_params(cfg["eps"], cfg["theta"], cfg["r_in"], cfg["r_out"], cfg["r_search"])
     ctx.set_tree_params(nleaf, ngroup)
+    if args.curve is not None:
+        ctx.set_key_curve(args.curve)
     if args.merge is not None:
         ctx.set_group_merge_levels(args.merge)
     if args.walk_mode is not None:

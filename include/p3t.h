@@ -124,11 +124,21 @@ p3t_status p3t_set_pair_classes(p3t_ctx *ctx, size_t n, const uint8_t *cls, int 
  * key depth limit); ngroup in {32, 64}: bodies per i-group (one warp). */
 p3t_status p3t_set_tree_params(p3t_ctx *ctx, int nleaf, int ngroup);
 
+/* Space-filling curve of the keys (row a2).  0: Morton (bit-interleaved quantised coordinates, what north_star names);
+ * 1 (default): Peano-Hilbert -- the same quantised coordinates taken through Skilling's transform before the
+ * interleave.  Both give the same octree (a level-l cell is the run of keys sharing their top 3 l bits; only the order
+ * of the octants inside a cell differs), the same cells, moments and, up to the grouping of the targets, the same
+ * results; the Hilbert order makes consecutive bodies neighbours in space everywhere, so i-groups can be plain runs of
+ * ngroup consecutive bodies with full warps and tight boxes (A25, section 7).  Invalidates a built tree.
+ * P3T_EINVAL for another value. */
+p3t_status p3t_set_key_curve(p3t_ctx *ctx, int curve);
+
 /* Tuning: how many octree levels above its natural level (the level whose cell holds <= ngroup
  * bodies) an i-group's bodies may straddle.  0 = every group is one octree cell (partly filled
  * warps); 1 (default) = consecutive sibling cells are merged up to ngroup bodies.  Where the natural
  * level is above tree level 4 (sparse outskirts) groups never straddle, whatever this value.  Results
- * do not depend on it beyond rounding and the R-MAC box B. levels in 0..4. */
+ * do not depend on it beyond rounding and the R-MAC box B. levels in 0..4, or 32: no cuts at all, every group is a plain
+ * run of ngroup consecutive bodies (meant for the Peano-Hilbert order). */
 p3t_status p3t_set_group_merge_levels(p3t_ctx *ctx, int levels);
 
 /* How i-groups are mapped to warps in the tree walk.  1: one warp per group -- results are bitwise

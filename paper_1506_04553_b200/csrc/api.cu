@@ -133,7 +133,8 @@ extern "C" p3t_status p3t_create(p3t_ctx **out, int device, size_t max_n, int ke
     ctx->nbr_capacity = nbr_capacity;
     ctx->nleaf = 16;
     ctx->ngroup = 64;
-    ctx->merge_levels = 1;
+    ctx->merge_levels = 3;          // the Peano-Hilbert default (Morton: 1); see p3t_set_key_curve
+    ctx->key_curve = 1;
     ctx->cells_dirty = true;
     ctx->herm_cluster_max = 4096;
     ctx->shard_rank = 0;
@@ -300,8 +301,20 @@ extern "C" p3t_status p3t_set_tree_params(p3t_ctx *ctx, int nleaf, int ngroup)
 // boundaries an i-group may straddle (0 = groups are single octree cells)
 extern "C" p3t_status p3t_set_group_merge_levels(p3t_ctx *ctx, int levels)
 {
-    if (!ctx || levels < 0 || levels > 4) return P3T_EINVAL;
+    if (!ctx || levels < 0 || (levels > 4 && levels != 32)) return P3T_EINVAL;
     ctx->merge_levels = levels;
+    ctx->merge_user_set = true;
+    ctx->built = false;
+    ctx->evaluated = false;
+    ctx->topo_valid = false;
+    return P3T_OK;
+}
+
+extern "C" p3t_status p3t_set_key_curve(p3t_ctx *ctx, int curve)
+{
+    if (!ctx || curve < 0 || curve > 1) return P3T_EINVAL;
+    ctx->key_curve = curve;
+    if (!ctx->merge_user_set) ctx->merge_levels = curve ? 3 : 1;   // measured optimum of either order
     ctx->built = false;
     ctx->evaluated = false;
     ctx->topo_valid = false;

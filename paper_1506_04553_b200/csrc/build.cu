@@ -80,6 +80,26 @@ __device__ __forceinline__ u32 tile_resolve(u32 *p0, u32 tile, u32 own)
     }
     return excl;
 }
+// The same for "the last marked position before this tile": own = position + 1 of the tile's last mark, 0 if it has
+// none; going backwards the first non-zero word decides (tile 0 always has a mark: body 0 starts a segment).
+__device__ __forceinline__ u32 tile_lookback_last(u32 *p0, u32 tile, u32 own)
+{
+    const int stride = (int)(sizeof(TileRec) / sizeof(u32));
+    st_tile_status(p0, own | ((tile == 0 || own) ? TL_FLAG_INC : TL_FLAG_AGG));   // a tile with a mark needs no look-back by others
+    u32 last = 0;
+    if (tile > 0) {
+        const u32 *p = p0 - stride;
+        while (!last) {
+            const u32 v = ld_tile_status(p);
+            if (v < TL_FLAG_AGG) continue;            // not published yet
+            last = v & TL_VAL_MASK;
+            if (v >= TL_FLAG_INC) break;              // inclusive word: final even if zero (cannot be: tile 0 has a mark)
+            p -= stride;
+        }
+        if (!own) st_tile_status(p0, last | TL_FLAG_INC);
+    }
+    return last;
+}
 __device__ __forceinline__ u32 tile_lookback(u32 *p0, u32 tile, u32 own)
 {
     tile_publish(p0, tile, own);
@@ -166,9 +186,9 @@ __global__ void __launch_bounds__(BUILD_THREADS) levels_kernel(const signed char
     // windows: c, leaf level, group level, minimum over NLEAF entries, two scratch
     __shared__ Window s_c, s_d, s_g, s_m, s_a, s_b;
     __shared__ int s_cnt[32];
-    __shared__ u32 s_tile;
+    __shared__ u32 s_tile, s_lastcut;
     const int tid = threadIdx.x, lane = tid & 31;
-    if (tid == 0) s_tile = (u32)atomicAdd(&counters[CNT_HEAD_TICKET], 1ull);   // tiles in scheduling order (look-back)
+    if (tid == 0) { s_tile = (u32)atomicAdd(&counters[CNT_HEAD_TICKET], 1ull); s_lastcut = 0; }   // tiles in scheduling order (look-back)
     __syncthreads();
     const u32 tile = s_tile;
     const long long base = (long long)tile * BUILD_TILE;
@@ -222,7 +242,10 @@ __global__ void __launch_bounds__(BUILD_THREADS) levels_kernel(const signed char
                 // group of consecutive bodies spans an octant, its box reaches the core and it opens the whole tree
                 // (one such group took 4.9 ms at N = 256K, 2.2x the rest of the launch)
                 const int gm = max(g, gp);
-                const bool cut = (i == 0) || c < max(gm - merge_levels, min(gm, GROUP_MERGE_MIN_LEVEL));
+                // (merge_levels >= P3T_MAX_LEVELS: no cuts at all, groups are plain runs of ngroup consecutive bodies --
+                //  what a Peano-Hilbert order allows, whose consecutive bodies are neighbours in space everywhere)
+                const int minlev = merge_levels >= P3T_MAX_LEVELS ? 0 : GROUP_MERGE_MIN_LEVEL;
+                const bool cut = (i == 0) || c < max(gm - merge_levels, min(gm, minlev));
                 dl |= (u32)D << (8 * s);
                 cf |= (cut ? 1u : 0u) << (8 * s);
                 if (D > c) { atomicAdd(&s_cnt[c + 1], 1); atomicAdd(&s_cnt[D + 1], -1); }
@@ -232,6 +255,7 @@ __global__ void __launch_bounds__(BUILD_THREADS) levels_kernel(const signed char
             *reinterpret_cast<u32 *>(dlev + i0) = dl;
             *reinterpret_cast<u32 *>(cutflag + i0) = cf;
         }
+        if (cf) atomicMax(&s_lastcut, (u32)i0 + (31u - __clz(cf)) / 8u + 1u);   // position + 1 of my last cut
     }
     __syncthreads();
     // ---- warp 0: nodes per level -> look-back over the tiles before -> exclusive prefixes
@@ -248,6 +272,8 @@ __global__ void __launch_bounds__(BUILD_THREADS) levels_kernel(const signed char
             const u32 excl = tile_lookback(&tiles[tile].status[lane], tile, own);
             tiles[tile].excl[lane] = excl;
             tot = excl + own;
+        } else if (lane == 25) {   // the last cut before this tile: emit_kernel's segments start there
+            tiles[tile].excl[25] = tile_lookback_last(&tiles[tile].status[25], tile, s_lastcut);
         }
         if (tile == ntiles - 1) {   // the last tile holds the totals: nodes per level, cells, deepest level in use
             if (lane < 24) level_total[lane] = tot;
@@ -294,17 +320,9 @@ __global__ void __launch_bounds__(BUILD_THREADS) emit_kernel(
         for (int L = 0; L < tid; ++L) off += level_total[L];
         s_lvloff[tid] = off + tiles[tile].excl[tid];
     }
-    // warp 7: the last cut before the tile, by a backward search over the cut flags (cutflag[0] = 1)
-    if (warp == BUILD_THREADS / 32 - 1) {
-        int found = -1;
-        for (long long top = (long long)base - 1; top >= 0 && found < 0; top -= 32) {
-            const long long pos = top - lane;
-            const bool hit = pos >= 0 && cutflag[pos];
-            const u32 b = __ballot_sync(0xffffffffu, hit);
-            if (b) found = (int)(top - (__ffs(b) - 1));   // lowest lane = nearest position
-        }
-        if (lane == 0) s_carry = found;
-    }
+    // the last cut before the tile: left by levels_kernel (a look-back column of its own; a backward search over the
+    // cut flags here cost 0.2 ms at N = 1M once groups were allowed to span several cells)
+    if (tid == 0) s_carry = (int)tiles[tile].excl[25] - 1;
     __syncthreads();
     int c[BUILD_PER_THREAD], D[BUILD_PER_THREAD];
     int lo = 99, hi = -1;

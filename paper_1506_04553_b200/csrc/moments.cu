@@ -12,16 +12,6 @@
 // K = W = 1 and hold no neighbours.  theta = 0 gives rcrit = inf (nothing is accepted).
 #include "p3t_internal.cuh"
 
-__device__ __forceinline__ u32 compact3(u64 x)
-{
-    x &= 0x1249249249249249ull;
-    x = (x ^ (x >> 2)) & 0x10c30c30c30c30c3ull;
-    x = (x ^ (x >> 4)) & 0x100f00f00f00f00full;
-    x = (x ^ (x >> 8)) & 0x1f0000ff0000ffull;
-    x = (x ^ (x >> 16)) & 0x1f00000000ffffull;
-    x = (x ^ (x >> 32)) & 0x1fffffull;
-    return (u32)x;
-}
 
 struct Mom {
     float cx, cy, cz, M;
@@ -32,16 +22,18 @@ struct Mom {
 
 template <bool REFIT>
 __device__ __forceinline__ void store_cell(u32 k, const Mom &m, int level, u64 key, const float *__restrict__ cube,
-                                           int max_level, float theta, float h, float4 *cell_mac, float4 *cell_mom0,
+                                           int max_level, int hilbert, float theta, float h, float4 *cell_mac, float4 *cell_mom0,
                                            float4 *cell_mom1, float4 *cell_bmin, float4 *cell_bmax)
 {
     const float side = cube[3];
     const float l = ldexpf(side, -level);
-    // geometric centre from the key prefix
-    u64 pre = level ? (key >> (3 * (max_level - level))) : 0ull;
-    float gx = cube[0] + ((float)compact3(pre >> 2) + 0.5f) * l;
-    float gy = cube[1] + ((float)compact3(pre >> 1) + 0.5f) * l;
-    float gz = cube[2] + ((float)compact3(pre) + 0.5f) * l;
+    // geometric centre from the key of the cell's first body: its quantised coordinates, cut to `level` bits
+    u32 qx, qy, qz;
+    p3t_decode_key(key, max_level, hilbert, qx, qy, qz);
+    const int sh = max_level - level;
+    float gx = cube[0] + ((float)(qx >> sh) + 0.5f) * l;
+    float gy = cube[1] + ((float)(qy >> sh) + 0.5f) * l;
+    float gz = cube[2] + ((float)(qz >> sh) + 0.5f) * l;
     float dx = m.cx - gx, dy = m.cy - gy, dz = m.cz - gz;
     float delta = sqrtf(dx * dx + dy * dy + dz * dz);
     float fx = fmaxf(m.cx - m.lox, m.hix - m.cx), fy = fmaxf(m.cy - m.loy, m.hiy - m.cy),
@@ -119,7 +111,7 @@ __global__ void __launch_bounds__(128, 4) moments_kernel(
     const u8 *__restrict__ cell_level, const u32 *__restrict__ cell_start, const u32 *__restrict__ cell_parent,
     const u32 *__restrict__ cell_first, u32 *cell_nchild, u32 *cell_ready, uint2 *cell_meta,
     float4 *cell_mac, float4 *cell_mom0, float4 *cell_mom1, float4 *cell_bmin,
-    float4 *cell_bmax, const u64 *__restrict__ counters, u32 cell_cap, int max_level, float theta, float h,
+    float4 *cell_bmax, const u64 *__restrict__ counters, u32 cell_cap, int max_level, int hilbert, float theta, float h,
     const u8 *__restrict__ cls_sorted, float h_bf)
 {
     const u32 ncell = (u32)min((u64)cell_cap, counters[CNT_NCELLS]);
@@ -172,7 +164,7 @@ __global__ void __launch_bounds__(128, 4) moments_kernel(
                 m.cx = 0.5f * (m.lox + m.hix); m.cy = 0.5f * (m.loy + m.hiy); m.cz = 0.5f * (m.loz + m.hiz);
                 m.qxx = m.qyy = m.qzz = m.qxy = m.qxz = m.qyz = 0.f;
             }
-            store_cell<REFIT>(k, m, level, keys[start], cube, max_level, theta, m.heavy ? h_bf : h, cell_mac, cell_mom0, cell_mom1, cell_bmin, cell_bmax);
+            store_cell<REFIT>(k, m, level, keys[start], cube, max_level, hilbert, theta, m.heavy ? h_bf : h, cell_mac, cell_mom0, cell_mom1, cell_bmin, cell_bmax);
             continue;
         }
         // ---- internal cell
@@ -193,7 +185,7 @@ __global__ void __launch_bounds__(128, 4) moments_kernel(
             }
             merge_children(first, nch, cell_mac, cell_mom0, cell_mom1, cell_bmin, cell_bmax, m);
             const u64 pkey = parent != P3T_NO_PARENT ? keys[pstart] : 0ull;
-            store_cell<REFIT>(k, m, level, key, cube, max_level, theta, m.heavy ? h_bf : h, cell_mac, cell_mom0, cell_mom1, cell_bmin, cell_bmax);
+            store_cell<REFIT>(k, m, level, key, cube, max_level, hilbert, theta, m.heavy ? h_bf : h, cell_mac, cell_mom0, cell_mom1, cell_bmin, cell_bmax);
             cell_meta[k] = make_uint2(first, nch);
             if (parent == P3T_NO_PARENT) break;
             __threadfence();             // my record is visible before my arrival is
@@ -213,11 +205,11 @@ p3t_status p3t_stage_moments(p3t_ctx *ctx)
     const u32 grid = (u32)min((size_t)div_up(bound, 128), (size_t)ctx->sm_count * 16);
     moments_kernel<0, false><<<grid, 128, 0, s>>>(w.body, w.keys[ctx->cur], w.cube, w.cell_level, w.cell_start, w.cell_parent, w.cell_first,
                                            w.cell_nchild, w.cell_ready, w.cell_meta, w.cell_mac, w.cell_mom0, w.cell_mom1,
-                                           w.cell_bmin, w.cell_bmax, w.counters, (u32)w.cell_cap, ctx->max_level, ctx->prm.theta,
+                                           w.cell_bmin, w.cell_bmax, w.counters, (u32)w.cell_cap, ctx->max_level, ctx->key_curve, ctx->prm.theta,
                                            ctx->prm.h, ctx->cls_n ? w.cls_sorted : nullptr, ctx->prm.h_bf);
     moments_kernel<1, false><<<grid, 128, 0, s>>>(w.body, w.keys[ctx->cur], w.cube, w.cell_level, w.cell_start, w.cell_parent, w.cell_first,
                                            w.cell_nchild, w.cell_ready, w.cell_meta, w.cell_mac, w.cell_mom0, w.cell_mom1,
-                                           w.cell_bmin, w.cell_bmax, w.counters, (u32)w.cell_cap, ctx->max_level, ctx->prm.theta,
+                                           w.cell_bmin, w.cell_bmax, w.counters, (u32)w.cell_cap, ctx->max_level, ctx->key_curve, ctx->prm.theta,
                                            ctx->prm.h, ctx->cls_n ? w.cls_sorted : nullptr, ctx->prm.h_bf);
     P3T_CUDA(ctx, cudaGetLastError());
     return P3T_OK;
@@ -234,7 +226,7 @@ p3t_status p3t_stage_moments(p3t_ctx *ctx)
 __global__ void __launch_bounds__(256) refit_gather_kernel(const float4 *__restrict__ body_user, const u32 *__restrict__ idx,
                                                            const u64 *__restrict__ keys, const u8 *__restrict__ dlev,
                                                            const float *__restrict__ cube, float4 *__restrict__ body, u32 n,
-                                                           int max_level, float stray_dist, u32 *cell_ready,
+                                                           int max_level, int hilbert, float stray_dist, u32 *cell_ready,
                                                            const u32 *__restrict__ prev_ncells, u32 cell_cap, u64 *counters)
 {
     // arrival counters of the climb -> 0 (a build has keys_hist_kernel do this)
@@ -246,10 +238,11 @@ __global__ void __launch_bounds__(256) refit_gather_kernel(const float4 *__restr
         const float4 b = body_user[idx[i]];
         body[i] = b;
         const int D = dlev[i];
-        const u64 pre = D ? (keys[i] >> (3 * (max_level - D))) : 0ull;
+        u32 qx, qy, qz;
+        p3t_decode_key(keys[i], max_level, hilbert, qx, qy, qz);
+        const int sh = max_level - D;
         const float l = ldexpf(side, -D);
-        const float lx = cube[0] + (float)compact3(pre >> 2) * l, ly = cube[1] + (float)compact3(pre >> 1) * l,
-                    lz = cube[2] + (float)compact3(pre) * l;
+        const float lx = cube[0] + (float)(qx >> sh) * l, ly = cube[1] + (float)(qy >> sh) * l, lz = cube[2] + (float)(qz >> sh) * l;
         const float ex = fmaxf(fmaxf(lx - b.x, b.x - (lx + l)), 0.f), ey = fmaxf(fmaxf(ly - b.y, b.y - (ly + l)), 0.f),
                     ez = fmaxf(fmaxf(lz - b.z, b.z - (lz + l)), 0.f);
         stray += fmaxf(ex, fmaxf(ey, ez)) > stray_dist * l ? 1u : 0u;
@@ -267,14 +260,14 @@ p3t_status p3t_stage_refit_begin(p3t_ctx *ctx)
     const u32 n = (u32)ctx->n;
     P3T_CUDA(ctx, cudaMemsetAsync(w.counters + CNT_STRAY, 0, sizeof(u64), s));
     refit_gather_kernel<<<min(div_up(n, 256), (u32)ctx->sm_count * 8), 256, 0, s>>>(
-        w.body_user, w.idx[ctx->cur], w.keys[ctx->cur], w.dlev, w.cube, w.body, n, ctx->max_level, ctx->stray_dist, w.cell_ready,
+        w.body_user, w.idx[ctx->cur], w.keys[ctx->cur], w.dlev, w.cube, w.body, n, ctx->max_level, ctx->key_curve, ctx->stray_dist, w.cell_ready,
         w.prev_ncells, (u32)w.cell_cap, w.counters);
     size_t bound = ctx->n * (size_t)(ctx->max_level + 1);
     if (bound > w.cell_cap) bound = w.cell_cap;
     const u32 grid = (u32)min((size_t)div_up(bound, 128), (size_t)ctx->sm_count * 16);
     moments_kernel<0, true><<<grid, 128, 0, s>>>(w.body, w.keys[ctx->cur], w.cube, w.cell_level, w.cell_start, w.cell_parent, w.cell_first,
                                                  w.cell_nchild, w.cell_ready, w.cell_meta, w.cell_mac, w.cell_mom0, w.cell_mom1,
-                                                 w.cell_bmin, w.cell_bmax, w.counters, (u32)w.cell_cap, ctx->max_level, ctx->prm.theta,
+                                                 w.cell_bmin, w.cell_bmax, w.counters, (u32)w.cell_cap, ctx->max_level, ctx->key_curve, ctx->prm.theta,
                                                  ctx->prm.h, ctx->cls_n ? w.cls_sorted : nullptr, ctx->prm.h_bf);
     P3T_CUDA(ctx, cudaGetLastError());
     return P3T_OK;
@@ -289,7 +282,7 @@ p3t_status p3t_stage_refit_finish(p3t_ctx *ctx)
     const u32 grid = (u32)min((size_t)div_up(bound, 128), (size_t)ctx->sm_count * 16);
     moments_kernel<1, true><<<grid, 128, 0, s>>>(w.body, w.keys[ctx->cur], w.cube, w.cell_level, w.cell_start, w.cell_parent, w.cell_first,
                                                  w.cell_nchild, w.cell_ready, w.cell_meta, w.cell_mac, w.cell_mom0, w.cell_mom1,
-                                                 w.cell_bmin, w.cell_bmax, w.counters, (u32)w.cell_cap, ctx->max_level, ctx->prm.theta,
+                                                 w.cell_bmin, w.cell_bmax, w.counters, (u32)w.cell_cap, ctx->max_level, ctx->key_curve, ctx->prm.theta,
                                                  ctx->prm.h, ctx->cls_n ? w.cls_sorted : nullptr, ctx->prm.h_bf);
     P3T_CUDA(ctx, cudaGetLastError());
     return P3T_OK;

@@ -151,6 +151,8 @@ struct p3t_ctx {
     cudaEvent_t ev_fork, ev_join;
     size_t max_n, n, nbr_capacity;
     int key_bits, max_level, nleaf, ngroup, merge_levels;
+    int key_curve;                 // 0 Morton, 1 Peano-Hilbert (default)
+    bool merge_user_set;           // p3t_set_group_merge_levels was called: p3t_set_key_curve keeps its value
     int herm_cluster_max;          // largest component a thread-block cluster integrates (larger ones: grid kernel)
     int walk_mode;                 // 0 auto, 1 one warp per group, 2 one CTA per group (cooperative)
     size_t cls_n;                  // 0: no classes; else the particle count the classes were given for
@@ -263,6 +265,67 @@ __device__ __forceinline__ u32 lanemask_lt()
     u32 m;
     asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
     return m;
+}
+
+// ---- space-filling curve of the keys (A25) -------------------------------------------------------------
+// Both curves interleave three `bits`-bit integers (first most significant): for Morton keys these are the quantised
+// coordinates themselves, for Peano-Hilbert keys their image under Skilling's transform ("Programming the Hilbert
+// curve", AIP Conf. Proc. 707, 2004).  Either way a level-l cell is the run of keys that share their top 3 l bits.
+__device__ __forceinline__ u64 p3t_spread3(u32 v)   // bit k -> bit 3k (21 bits)
+{
+    u64 x = v & 0x1fffffu;
+    x = (x | x << 32) & 0x1f00000000ffffull;
+    x = (x | x << 16) & 0x1f0000ff0000ffull;
+    x = (x | x << 8) & 0x100f00f00f00f00full;
+    x = (x | x << 4) & 0x10c30c30c30c30c3ull;
+    x = (x | x << 2) & 0x1249249249249249ull;
+    return x;
+}
+__device__ __forceinline__ u32 p3t_compact3(u64 x)   // bit 3k -> bit k
+{
+    x &= 0x1249249249249249ull;
+    x = (x ^ (x >> 2)) & 0x10c30c30c30c30c3ull;
+    x = (x ^ (x >> 4)) & 0x100f00f00f00f00full;
+    x = (x ^ (x >> 8)) & 0x1f0000ff0000ffull;
+    x = (x ^ (x >> 16)) & 0x1f00000000ffffull;
+    x = (x ^ (x >> 32)) & 0x1fffffull;
+    return (u32)x;
+}
+// quantised coordinates -> key
+__device__ __forceinline__ u64 p3t_encode_key(u32 x, u32 y, u32 z, int bits, int hilbert)
+{
+    if (hilbert) {
+        // Skilling: AxestoTranspose, written without branches (a warp's lanes take all paths anyway):
+        //   if (X[i] & Q) X[0] ^= P; else { t = (X[0] ^ X[i]) & P; X[0] ^= t; X[i] ^= t; }    for i = 0, 1, 2
+        for (int b = bits - 1; b > 0; --b) {
+            const u32 P = (1u << b) - 1u;
+            x ^= P & (0u - ((x >> b) & 1u));                    // i = 0: invert (the exchange with itself is void)
+            u32 hit = 0u - ((y >> b) & 1u), t = (x ^ y) & P & ~hit;
+            x ^= (P & hit) | t; y ^= t;
+            hit = 0u - ((z >> b) & 1u); t = (x ^ z) & P & ~hit;
+            x ^= (P & hit) | t; z ^= t;
+        }
+        y ^= x; z ^= y;                                         // Gray encode
+        u32 t = 0;
+        for (int b = bits - 1; b > 0; --b) t ^= ((1u << b) - 1u) & (0u - ((z >> b) & 1u));
+        x ^= t; y ^= t; z ^= t;
+    }
+    return (p3t_spread3(x) << 2) | (p3t_spread3(y) << 1) | p3t_spread3(z);
+}
+// key -> quantised coordinates (all `bits` bits; a level-l cell index is the result >> (bits - l))
+__device__ __forceinline__ void p3t_decode_key(u64 key, int bits, int hilbert, u32 &x, u32 &y, u32 &z)
+{
+    x = p3t_compact3(key >> 2); y = p3t_compact3(key >> 1); z = p3t_compact3(key);
+    if (hilbert) {
+        u32 t = z >> 1;                                         // Skilling: TransposetoAxes
+        z ^= y; y ^= x; x ^= t;
+        for (u32 Q = 2u; Q != (2u << (bits - 1)); Q <<= 1) {
+            const u32 P = Q - 1u;
+            if (z & Q) x ^= P; else { t = (x ^ z) & P; x ^= t; z ^= t; }
+            if (y & Q) x ^= P; else { t = (x ^ y) & P; x ^= t; y ^= t; }
+            if (x & Q) x ^= P;
+        }
+    }
 }
 
 // order-preserving float <-> uint mapping for atomicMin/Max on floats

@@ -85,17 +85,6 @@ p3t_status p3t_stage_unpack(p3t_ctx *ctx, float *d_acc, float *d_pot)
 // ------------------------------------------------------------------------------------------------
 // a2: root cube + Morton keys + digit histograms of all passes
 // ------------------------------------------------------------------------------------------------
-// spread the low 21 bits of v so that bit k lands at bit 3k
-__device__ __forceinline__ u64 spread3(u32 v)
-{
-    u64 x = v & 0x1fffffu;
-    x = (x | x << 32) & 0x1f00000000ffffull;
-    x = (x | x << 16) & 0x1f0000ff0000ffull;
-    x = (x | x << 8) & 0x100f00f00f00f00full;
-    x = (x | x << 4) & 0x10c30c30c30c30c3ull;
-    x = (x | x << 2) & 0x1249249249249249ull;
-    return x;
-}
 
 // Root cube from the reduced min/max: centre = midpoint of the AABB, side = largest extent padded
 // so that the maximum maps inside.  Every thread recomputes it (6 loads), block 0 publishes it.
@@ -114,7 +103,7 @@ __device__ __forceinline__ void root_cube(const u32 *bbox_bits, float &minx, flo
 
 __global__ void __launch_bounds__(256) keys_hist_kernel(const float4 *__restrict__ body, const u32 *__restrict__ bbox_bits,
                                                         float *cube, u64 *__restrict__ keys, u32 *hist, u32 n,
-                                                        int max_level, int passes, const u32 *__restrict__ prev_ncells,
+                                                        int max_level, int hilbert, int passes, const u32 *__restrict__ prev_ncells,
                                                         u32 cell_cap, u32 *cell_nchild, u32 *cell_ready)
 {
     // child counters of the cells of the previous build -> 0 (emit_kernel accumulates into them)
@@ -135,7 +124,7 @@ __global__ void __launch_bounds__(256) keys_hist_kernel(const float4 *__restrict
         u32 qx = min((u32)fmaxf((b.x - minx) * scale, 0.f), qmax);
         u32 qy = min((u32)fmaxf((b.y - miny) * scale, 0.f), qmax);
         u32 qz = min((u32)fmaxf((b.z - minz) * scale, 0.f), qmax);
-        u64 key = (spread3(qx) << 2) | (spread3(qy) << 1) | spread3(qz);
+        u64 key = p3t_encode_key(qx, qy, qz, max_level, hilbert);
         keys[i] = key;
         for (int p = 0; p < passes; ++p) atomicAdd(&s_hist[p * 256 + (u32)((key >> (8 * p)) & 255u)], 1u);
     }
@@ -406,7 +395,7 @@ p3t_status p3t_stage_sort(p3t_ctx *ctx)
         P3T_CUDA(ctx, cudaMemsetAsync(w.prev_ncells, 0, sizeof(u32), s));
         ctx->cells_dirty = false;
     }
-    keys_hist_kernel<<<grid, 256, 0, s>>>(w.body_user, w.bbox_bits, w.cube, w.keys[0], w.hist, n, ctx->max_level, passes,
+    keys_hist_kernel<<<grid, 256, 0, s>>>(w.body_user, w.bbox_bits, w.cube, w.keys[0], w.hist, n, ctx->max_level, ctx->key_curve, passes,
                                           w.prev_ncells, (u32)w.cell_cap, w.cell_nchild, w.cell_ready);
     int cur = 0;
     for (int p = 0; p < passes; ++p) {

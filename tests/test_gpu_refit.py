@@ -92,7 +92,7 @@ def test_refit_keeps_the_topology_and_recomputes_moments_boxes_and_radii():
             np.testing.assert_allclose(mac[i, :3], com, atol=3e-6 * ext + 2e-7 * np.abs(com).max())
             np.testing.assert_allclose(np.concatenate([m0[i, 1:], m1[i, :3]]), Q, atol=2e-5 * M * ext * ext + 1e-30)
             assert np.array_equal(bmin[i, :3], lo.astype(np.float32)) and np.array_equal(bmax[i, :3], hi.astype(np.float32))
-            g, l = keytree.cell_geometry(c, keys[c["start"]], cube[:3], cube[3], 21)
+            g, l = keytree.cell_geometry(c, keys[c["start"]], cube[:3], cube[3], 21, curve="hilbert")
             # side of the smallest cube about the geometric centre that holds the bodies (= l while they are inside)
             lm = max(l, 2.0 * float(np.maximum(g - lo, hi - g).max()))
             grown += lm > l * (1 + 1e-6)

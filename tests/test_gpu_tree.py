@@ -13,11 +13,12 @@ pytestmark = pytest.mark.gpu
 LEAF = 0x80000000
 
 
-def _build(cfg, key_bits=None, nleaf=16, ngroup=64, theta=None):
+def _build(cfg, key_bits=None, nleaf=16, ngroup=64, theta=None, curve="hilbert"):
     from paper_1506_04553_b200 import binding
 
     kb = key_bits or cfg["key_bits"]
     ctx = binding.P3T(cfg["n"], key_bits=kb)
+    ctx.set_key_curve(curve)
     ctx.set_params(cfg["eps"], cfg["theta"] if theta is None else theta, cfg["r_in"], cfg["r_out"], cfg["r_search"])
     ctx.set_tree_params(nleaf, ngroup)
     ctx.load_particles(cfg["mass"], cfg["pos"])
@@ -32,12 +33,13 @@ CASES = [  # (config, n, key_bits, nleaf, ngroup)
 ]
 
 
+@pytest.mark.parametrize("curve", ["morton", "hilbert"])
 @pytest.mark.parametrize("k,n,kb,nleaf,ngroup", CASES)
-def test_keys_sort_octree_match_keytree_oracle(k, n, kb, nleaf, ngroup):
+def test_keys_sort_octree_match_keytree_oracle(k, n, kb, nleaf, ngroup, curve):
     from oracle import keytree
 
     cfg = workloads.config(k, n=n)
-    ctx, max_level = _build(cfg, kb, nleaf, ngroup)
+    ctx, max_level = _build(cfg, kb, nleaf, ngroup, curve=curve)
     cube = ctx.array("root_cube")
     # a1: the cube is the oracle's definition (centre = AABB midpoint, side = largest extent), padded
     cmin, side = keytree.root_cube(cfg["pos"])
@@ -47,7 +49,7 @@ def test_keys_sort_octree_match_keytree_oracle(k, n, kb, nleaf, ngroup):
     # a2-a3: keys bit-exact, sorted; a4: permutation and gathered bodies
     keys = ctx.array("keys")
     idx = ctx.array("sorted_idx")
-    ref = keytree.morton_keys(cfg["pos"], cube[:3], cube[3], max_level)
+    ref = (keytree.hilbert_keys if curve == "hilbert" else keytree.morton_keys)(cfg["pos"], cube[:3], cube[3], max_level)
     assert np.array_equal(np.sort(idx), np.arange(n, dtype=np.uint32))
     assert np.array_equal(keys, ref[idx])
     assert np.all(keys[1:] >= keys[:-1])
@@ -77,12 +79,13 @@ def test_keys_sort_octree_match_keytree_oracle(k, n, kb, nleaf, ngroup):
     ctx.close()
 
 
+@pytest.mark.parametrize("curve", ["morton", "hilbert"])
 @pytest.mark.parametrize("k,n,kb", [(1, 4096, 30), (3, 20011, 63), (4, 30000, 63)])
-def test_moments_match_fp64_recomputation(k, n, kb):
+def test_moments_match_fp64_recomputation(k, n, kb, curve):
     from oracle import keytree
 
     cfg = workloads.config(k, n=n)
-    ctx, max_level = _build(cfg, kb)
+    ctx, max_level = _build(cfg, kb, curve=curve)
     keys, bodies, cube = ctx.array("keys"), ctx.array("bodies"), ctx.array("root_cube")
     cells = keytree.build_cells(keys, 16, max_level)
     mac, m0, m1 = ctx.array("cell_mac"), ctx.array("cell_mom0"), ctx.array("cell_mom1")
@@ -100,7 +103,7 @@ def test_moments_match_fp64_recomputation(k, n, kb):
         np.testing.assert_allclose(np.concatenate([m0[i, 1:], m1[i, :3]]), Q, atol=2e-5 * qscale + 1e-30)
         assert np.array_equal(bmin[i, :3], lo.astype(np.float32)) and np.array_equal(bmax[i, :3], hi.astype(np.float32))
         # acceptance radius: never below either clause of R-MAC (A9, A10)
-        g, l = keytree.cell_geometry(c, keys[c["start"]], cube[:3], cube[3], max_level)
+        g, l = keytree.cell_geometry(c, keys[c["start"]], cube[:3], cube[3], max_level, curve=curve)
         delta = np.linalg.norm(com - g)
         rmax = np.linalg.norm(bodies[c["start"]:c["start"] + c["count"], :3].astype(np.float64) - com, axis=1).max()
         rc = np.sqrt(float(mac[i, 3]))
