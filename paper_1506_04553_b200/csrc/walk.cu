@@ -276,41 +276,72 @@ __device__ __forceinline__ void eval_near(const WarpShared &ws, u32 head, u32 cn
                                           const P3TParams &prm, const u32 *__restrict__ sorted_idx, uint2 *pairs, u64 pair_cap,
                                           u64 *counters, u32 (&nnb)[NI], Acc<NI> &acc, u32 lane)
 {
+    // Nearly all near entries are plain Newtonian partners of all the group's bodies (they are "near" the group's BOX):
+    // the packed plain term is evaluated for everybody, with the mass of a pair that is not plain (self, closer than
+    // the neighbour radius, two black holes) set to zero -- masked, not subtracted afterwards: a close pair's plain term
+    // would be many orders of magnitude above the sum -- and the K/W term and the list entry of such pairs are done by a
+    // branch that a warp takes for about one entry in fifty.
+    typedef typename VecOf<NI>::type V;
+    const V eps2v = vdup<V>(prm.eps2);
     for (u32 j = 0; j < cnt; ++j) {
         float4 bj = ws.near_buf[head + j];
         u32 js = ws.near_idx[head + j];
         u32 cj = 0;
         if (CLS) { cj = js >> 31; js &= 0x7fffffffu; }
+        V dx = vadd(vdup<V>(bj.x), t.nx), dy = vadd(vdup<V>(bj.y), t.ny), dz = vadd(vdup<V>(bj.z), t.nz);
+        V r2 = vfma(dx, dx, vfma(dy, dy, vfma(dz, dz, eps2v)));
+        V r2s = r2, meff;
+        bool slow[NI], anyslow = false;
 #pragma unroll
         for (int b = 0; b < NI; ++b) {
             const u32 kind = CLS ? icls[b] + cj : 0u;
-            float dx = bj.x + vget(t.nx, b), dy = bj.y + vget(t.ny, b), dz = bj.z + vget(t.nz, b);
-            float s2 = fmaf(dx, dx, fmaf(dy, dy, fmaf(dz, dz, prm.eps2)));
-            bool live = isorted[b] != 0xffffffffu && isorted[b] != js;
-            bool hit = live && (CLS ? (kind == 2u || s2 < prm.h2_k[kind & 1u]) : s2 < prm.h2);
-            if (live && !(CLS && kind == 2u)) {
-                float rinv = rsq(s2);
-                float mrinv = bj.w * rinv;
-                float mr3 = mrinv * (rinv * rinv);
-                float K = 1.f, W = 1.f;
-                if (CLS) { if (s2 < prm.rout2_k[kind]) p3t_pair_weights(prm.cs[kind], s2, K, W); }
-                else if (s2 < prm.rout2) p3t_pair_weights(prm.cs[0], s2, K, W);
-                mr3 *= K;
-                vref(acc.ax, b) = fmaf(mr3, dx, vget(acc.ax, b));
-                vref(acc.ay, b) = fmaf(mr3, dy, vget(acc.ay, b));
-                vref(acc.az, b) = fmaf(mr3, dz, vget(acc.az, b));
-                vref(acc.ph, b) = fmaf(W, mrinv, vget(acc.ph, b));
-            }
-            u32 hb = __ballot_sync(0xffffffffu, hit);
-            if (hb) {
-                u64 base = 0;
-                if (lane == 0) base = atomicAdd(&counters[CNT_PAIRS], (u64)__popc(hb));
-                base = __shfl_sync(0xffffffffu, base, 0);
-                if (hit) {
-                    u64 pos = base + __popc(hb & lanemask_lt());
-                    P3T_DEV_ASSERT(js < 0x40000000u);
-                    if (pos < pair_cap) pairs[pos] = make_uint2(iuser[b], sorted_idx[js]);
-                    ++nnb[b];
+            const bool live = isorted[b] != 0xffffffffu && isorted[b] != js;
+            const float thr = CLS ? (kind == 2u ? INFINITY : prm.h2_k[kind & 1u]) : prm.h2;
+            slow[b] = live && vget(r2, b) < thr;
+            const bool plain = live && !slow[b];
+            vref(meff, b) = plain ? bj.w : 0.f;
+            if (!plain) vref(r2s, b) = 1.f;           // keeps 0 * rsqrt(0) out of the sums (self pair with eps = 0)
+            anyslow = anyslow || slow[b];
+        }
+        {
+            V rinv = vrsqrt(r2s);
+            V mrinv = vmul(meff, rinv);
+            V mr3 = vmul(mrinv, vmul(rinv, rinv));
+            acc.ax = vfma(mr3, dx, acc.ax);
+            acc.ay = vfma(mr3, dy, acc.ay);
+            acc.az = vfma(mr3, dz, acc.az);
+            acc.ph = vadd(acc.ph, mrinv);
+        }
+        if (__any_sync(0xffffffffu, anyslow)) {
+#pragma unroll
+            for (int b = 0; b < NI; ++b) {
+                const u32 kind = CLS ? icls[b] + cj : 0u;
+                const bool hit = slow[b];                 // within the neighbour radius of its kind (always, for kind 2)
+                if (hit && !(CLS && kind == 2u)) {
+                    const float s2 = vget(r2, b);
+                    float rinv = rsq(s2);
+                    float mrinv = bj.w * rinv;
+                    float mr3 = mrinv * (rinv * rinv);
+                    float K = 1.f, W = 1.f;
+                    if (CLS) { if (s2 < prm.rout2_k[kind]) p3t_pair_weights(prm.cs[kind], s2, K, W); }
+                    else if (s2 < prm.rout2) p3t_pair_weights(prm.cs[0], s2, K, W);
+                    mr3 *= K;
+                    vref(acc.ax, b) = fmaf(mr3, vget(dx, b), vget(acc.ax, b));
+                    vref(acc.ay, b) = fmaf(mr3, vget(dy, b), vget(acc.ay, b));
+                    vref(acc.az, b) = fmaf(mr3, vget(dz, b), vget(acc.az, b));
+                    vref(acc.ph, b) = fmaf(W, mrinv, vget(acc.ph, b));
+                }
+                u32 hb = __ballot_sync(0xffffffffu, hit);
+                if (hb) {
+                    u64 base = 0;
+                    if (lane == 0) base = atomicAdd(&counters[CNT_PAIRS], (u64)__popc(hb));
+                    base = __shfl_sync(0xffffffffu, base, 0);
+                    if (hit) {
+                        u64 pos = base + __popc(hb & lanemask_lt());
+                        P3T_DEV_ASSERT(js < 0x40000000u);
+                        if (pos < pair_cap) pairs[pos] = make_uint2(iuser[b], sorted_idx[js]);
+                        ++nnb[b];
+                    }
                 }
             }
         }
@@ -522,7 +553,13 @@ __device__ __forceinline__ void walk_group(WarpShared *wsall, const StackRef &st
             if (!COOP) {
                 if (top + total > st.limit) { overflow = true; break; }
                 u32 pos = top + inc - nch;
-                for (u32 c = 0; c < nch; ++c) stack_write(st, pos + c, first + c);
+                if (top + total <= st.cap) {      // (warp-uniform) everything lands in shared memory: no per-entry test
+#pragma unroll
+                    for (u32 c = 0; c < 8; ++c)
+                        if (c < nch) st.smem[pos + c] = first + c;
+                } else {
+                    for (u32 c = 0; c < nch; ++c) stack_write(st, pos + c, first + c);
+                }
                 top += total;
                 __syncwarp();
                 // ---- request the records of the next step before any interaction work
