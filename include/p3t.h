@@ -133,6 +133,13 @@ p3t_status p3t_set_tree_params(p3t_ctx *ctx, int nleaf, int ngroup);
  * P3T_EINVAL for another value. */
 p3t_status p3t_set_key_curve(p3t_ctx *ctx, int curve);
 
+/* Inspection (host only, no GPU involved): the state tables the key kernel uses for Peano-Hilbert keys, derived by the
+ * library from Skilling's transform on a 32^3 lattice.  tab[state * 64 + two octants] = next state << 6 | two key digits
+ * (24 states, the root cell has state 0; an octant is 4 x-bit + 2 y-bit + z-bit), then tab[1536 + state * 8 + octant] =
+ * next state << 3 | key digit.  words >= 1728.  P3T_EINVAL for bad arguments, P3T_ECUDA if the derivation found the
+ * curve not to be a state machine (cannot happen; the same test guards p3t_create). */
+p3t_status p3t_hilbert_state_tables(uint32_t *tab, size_t words);
+
 /* Tuning: how many octree levels above its natural level (the level whose cell holds <= ngroup
  * bodies) an i-group's bodies may straddle.  0 = every group is one octree cell (partly filled
  * warps); 1 (default) = consecutive sibling cells are merged up to ngroup bodies.  Where the natural
@@ -158,9 +165,11 @@ p3t_status p3t_set_walk_mode(p3t_ctx *ctx, int mode);
 p3t_status p3t_set_shard(p3t_ctx *ctx, int rank, int world);
 
 /* Load n particles: mass[n], pos[3n] (x,y,z interleaved), both host or both
- * device (on_device).  Host data is checked for non-finite values here
- * (P3T_EINVAL); device data is checked on the GPU and the error surfaces at
- * p3t_build_tree's successor calls that synchronise. */
+ * device (on_device).  Every value is tested for being finite by the kernel that
+ * packs the bodies.  Host data: the call waits for the copies and that kernel and
+ * returns P3T_EINVAL itself (the host arrays may be reused when it returns); device
+ * data: the call only enqueues, and the error surfaces at the next call that
+ * synchronises. */
 p3t_status p3t_load_particles(p3t_ctx *ctx, size_t n, const float *mass, const float *pos, int on_device);
 
 /* a1-a6: bounding cube, Morton keys, radix sort, body gather, octree + groups,

@@ -28,7 +28,7 @@ _STATUS = {0: "P3T_OK", -1: "P3T_EINVAL", -2: "P3T_ESTATE", -3: "P3T_ENOMEM", -4
 # names of include/p3t.h's exported entry points (tests check that each resolves)
 SYMBOLS = [
     "p3t_workspace_bytes", "p3t_create", "p3t_destroy", "p3t_set_params", "p3t_set_tree_params",
-    "p3t_set_pair_classes", "p3t_set_key_curve", "p3t_set_group_merge_levels", "p3t_set_walk_mode", "p3t_set_shard", "p3t_load_particles", "p3t_build_tree", "p3t_set_tree_reuse", "p3t_refit_tree", "p3t_eval_soft", "p3t_eval_direct", "p3t_eval_hard",
+    "p3t_set_pair_classes", "p3t_set_key_curve", "p3t_hilbert_state_tables", "p3t_set_group_merge_levels", "p3t_set_walk_mode", "p3t_set_shard", "p3t_load_particles", "p3t_build_tree", "p3t_set_tree_reuse", "p3t_refit_tree", "p3t_eval_soft", "p3t_eval_direct", "p3t_eval_hard",
     "p3t_hermite_step", "p3t_step", "p3t_set_hermite_cluster_max",
     "p3t_get_acc_pot", "p3t_get_neighbour_counts", "p3t_get_neighbours", "p3t_get_stats", "p3t_synchronize",
     "p3t_last_error", "p3t_array_info", "p3t_copy_array", "p3t_measure_fp32_peak",
@@ -72,6 +72,7 @@ def _sig():
     L.p3t_set_pair_classes.restype = i; L.p3t_set_pair_classes.argtypes = [vp, sz, vp, i, f, f, f, f]
     L.p3t_set_group_merge_levels.restype = i; L.p3t_set_group_merge_levels.argtypes = [vp, i]
     L.p3t_set_key_curve.restype = i; L.p3t_set_key_curve.argtypes = [vp, i]
+    L.p3t_hilbert_state_tables.restype = i; L.p3t_hilbert_state_tables.argtypes = [vp, sz]
     L.p3t_set_walk_mode.restype = i; L.p3t_set_walk_mode.argtypes = [vp, i]
     L.p3t_set_hermite_cluster_max.restype = i; L.p3t_set_hermite_cluster_max.argtypes = [vp, i]
     L.p3t_set_shard.restype = i; L.p3t_set_shard.argtypes = [vp, i, i]
@@ -104,6 +105,15 @@ class P3TError(RuntimeError):
     def __init__(self, status, msg):
         super().__init__(f"{_STATUS.get(status, status)}: {msg}")
         self.status = status
+
+
+def hilbert_state_tables():
+    """The state tables the key kernel uses for Peano-Hilbert keys (host only, no GPU needed): uint32[24 * 64 + 24 * 8]."""
+    tab = np.zeros(24 * 64 + 24 * 8, dtype=np.uint32)
+    st = _lib.p3t_hilbert_state_tables(tab.ctypes.data, tab.size)
+    if st != OK:
+        raise P3TError(st, "the tables derived from the transform are inconsistent")
+    return tab
 
 
 def p3t_workspace_bytes(max_n, key_bits=63, nbr_capacity=0):

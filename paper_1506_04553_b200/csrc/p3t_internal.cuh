@@ -128,6 +128,7 @@ struct Workspace {
     u32 *nbr;                      // [cap]
     u32 *nbr_cursor;               // [n]
     u32 *subset;                   // [n] staging for eval_direct
+    u32 *hilbert_tab;              // [24 * 64 + 24 * 8] state tables of the Peano-Hilbert keys (sort.cu: p3t_hilbert_tables)
     u8 *cls_user, *cls_sorted;     // [n] class of every body (0 field star, 1 black hole), user order and Morton order
     double *hard_out;              // [7n] staging of p3t_eval_hard's host outputs (acc 3n, jerk 3n, pot n); of p3t_hermite_step's pos, vel
     u32 *herm_ids;                 // [n] non-isolated particles by connected component of the neighbour graph (hermite.cu)
@@ -208,6 +209,9 @@ static inline u32 div_up(size_t a, size_t b) { return (u32)((a + b - 1) / b); }
 
 // stage entry points (each enqueues kernels on ctx->stream)
 p3t_status p3t_stage_pack(p3t_ctx *ctx, const float *d_mass, const float *d_pos);
+#define P3T_HILBERT_STATES 24
+#define P3T_HILBERT_TAB_WORDS (P3T_HILBERT_STATES * 64 + P3T_HILBERT_STATES * 8)
+bool p3t_hilbert_tables(u32 *tab /* [P3T_HILBERT_TAB_WORDS], host */);
 p3t_status p3t_stage_sort(p3t_ctx *ctx);
 p3t_status p3t_stage_build(p3t_ctx *ctx);
 p3t_status p3t_stage_moments(p3t_ctx *ctx);

@@ -4,6 +4,8 @@
 // this library's own (north_star).  All kernels are HBM/L2-bandwidth bound.
 #include "p3t_internal.cuh"
 
+#include <vector>
+
 // ------------------------------------------------------------------------------------------------
 // a1: pack (mass, pos) -> float4 bodies in user order, min/max of positions, finiteness check
 // ------------------------------------------------------------------------------------------------
@@ -86,6 +88,102 @@ p3t_status p3t_stage_unpack(p3t_ctx *ctx, float *d_acc, float *d_pot)
 // a2: root cube + Morton keys + digit histograms of all passes
 // ------------------------------------------------------------------------------------------------
 
+// ---- Peano-Hilbert keys by table (A25) ------------------------------------------------------------------
+// Skilling's transform (p3t_encode_key) walks all bits of all three coordinates for every level: ~600 instructions per
+// body.  The curve it defines is self-similar: inside a cell the order of the eight octants is one of 24 "states"
+// (orientations), and the state of a child follows from the parent's state and the child's octant.  The tables are not
+// typed in: p3t_hilbert_tables derives them on the host from the plain transform on a 32^3 lattice and checks that
+// they are consistent (same state, same octant -> same child state) before any context uses them.
+//   tab[state * 64 + two octants (6 bits)] = next state << 6 | two key digits (6 bits)      two levels per step
+//   tab[24 * 64 + state * 8 + octant]      = next state << 3 | key digit                     the odd last level
+static void host_hilbert_transpose(u32 &x, u32 &y, u32 &z, int bits)   // Skilling's AxestoTranspose, plain
+{
+    u32 X[3] = {x, y, z};
+    for (u32 Q = 1u << (bits - 1); Q > 1u; Q >>= 1) {
+        const u32 P = Q - 1u;
+        for (int i = 0; i < 3; ++i) {
+            if (X[i] & Q) X[0] ^= P;
+            else { const u32 t = (X[0] ^ X[i]) & P; X[0] ^= t; X[i] ^= t; }
+        }
+    }
+    for (int i = 1; i < 3; ++i) X[i] ^= X[i - 1];
+    u32 t = 0;
+    for (u32 Q = 1u << (bits - 1); Q > 1u; Q >>= 1)
+        if (X[2] & Q) t ^= Q - 1u;
+    x = X[0] ^ t; y = X[1] ^ t; z = X[2] ^ t;
+}
+
+bool p3t_hilbert_tables(u32 *tab)
+{
+    const int B = 5, N = 1 << B;
+    // digit[l] of every lattice point, and the octant -> digit map of every cell (level, prefix path of octants)
+    std::vector<std::vector<u32>> maps(B);                 // per level: 8 digits per prefix, packed 3 bits each; ~0u = unset
+    for (int l = 0; l < B; ++l) maps[l].assign((size_t)1 << (3 * l), 0u);
+    std::vector<std::vector<u32>> seen(B);
+    for (int l = 0; l < B; ++l) seen[l].assign((size_t)1 << (3 * l), 0u);
+    for (u32 x = 0; x < (u32)N; ++x) for (u32 y = 0; y < (u32)N; ++y) for (u32 z = 0; z < (u32)N; ++z) {
+        u32 tx = x, ty = y, tz = z;
+        host_hilbert_transpose(tx, ty, tz, B);
+        u32 pre = 0;
+        for (int l = 0; l < B; ++l) {
+            const int b = B - 1 - l;
+            const u32 oct = ((x >> b) & 1u) << 2 | ((y >> b) & 1u) << 1 | ((z >> b) & 1u);
+            const u32 dig = ((tx >> b) & 1u) << 2 | ((ty >> b) & 1u) << 1 | ((tz >> b) & 1u);
+            if ((seen[l][pre] >> oct) & 1u) { if (((maps[l][pre] >> (3 * oct)) & 7u) != dig) return false; }
+            else { maps[l][pre] |= dig << (3 * oct); seen[l][pre] |= 1u << oct; }
+            pre = pre * 8 + oct;
+        }
+    }
+    // states = distinct maps, numbered in order of discovery from the root; transitions must be functions of (state, octant)
+    std::vector<u32> state_map;                            // state -> packed map
+    auto state_of = [&](u32 m) { for (size_t s = 0; s < state_map.size(); ++s) if (state_map[s] == m) return (int)s; state_map.push_back(m); return (int)state_map.size() - 1; };
+    int next[64][8];
+    for (auto &r : next) for (int &v : r) v = -1;
+    for (int l = 0; l + 1 < B; ++l)
+        for (size_t pre = 0; pre < maps[l].size(); ++pre) {
+            const int s = state_of(maps[l][pre]);
+            if (s >= 64) return false;
+            for (u32 oct = 0; oct < 8; ++oct) {
+                const int c = state_of(maps[l + 1][pre * 8 + oct]);
+                if (c >= 64) return false;
+                if (next[s][oct] >= 0 && next[s][oct] != c) return false;
+                next[s][oct] = c;
+            }
+        }
+    if (state_map.size() != P3T_HILBERT_STATES || state_of(maps[0][0]) != 0) return false;
+    for (int s = 0; s < P3T_HILBERT_STATES; ++s)
+        for (u32 oct = 0; oct < 8; ++oct) {
+            if (next[s][oct] < 0) return false;
+            tab[P3T_HILBERT_STATES * 64 + s * 8 + oct] = (u32)next[s][oct] << 3 | ((state_map[s] >> (3 * oct)) & 7u);
+        }
+    for (int s = 0; s < P3T_HILBERT_STATES; ++s)
+        for (u32 o2 = 0; o2 < 64; ++o2) {
+            const u32 e1 = tab[P3T_HILBERT_STATES * 64 + s * 8 + (o2 >> 3)], e2 = tab[P3T_HILBERT_STATES * 64 + (e1 >> 3) * 8 + (o2 & 7u)];
+            tab[s * 64 + o2] = (e2 >> 3) << 6 | (e1 & 7u) << 3 | (e2 & 7u);
+        }
+    return true;
+}
+
+// quantised coordinates -> Peano-Hilbert key with the tables in shared memory
+__device__ __forceinline__ u64 hilbert_key_tab(const u32 *s_tab, u32 x, u32 y, u32 z, int bits)
+{
+    // interleave first: the octants of all levels as 3-bit groups (x most significant), then two levels per lookup
+    const u64 m = (p3t_spread3(x) << 2) | (p3t_spread3(y) << 1) | p3t_spread3(z);
+    u64 key = 0;
+    u32 st = 0;
+    int b = bits;
+    for (; b >= 2; b -= 2) {
+        const u32 e = s_tab[st * 64 + (u32)((m >> (3 * (b - 2))) & 63u)];
+        key = key << 6 | (e & 63u);
+        st = e >> 6;
+    }
+    if (b) {
+        const u32 e = s_tab[P3T_HILBERT_STATES * 64 + st * 8 + (u32)(m & 7u)];
+        key = key << 3 | (e & 7u);
+    }
+    return key;
+}
+
 // Root cube from the reduced min/max: centre = midpoint of the AABB, side = largest extent padded
 // so that the maximum maps inside.  Every thread recomputes it (6 loads), block 0 publishes it.
 __device__ __forceinline__ void root_cube(const u32 *bbox_bits, float &minx, float &miny, float &minz, float &side)
@@ -103,7 +201,7 @@ __device__ __forceinline__ void root_cube(const u32 *bbox_bits, float &minx, flo
 
 __global__ void __launch_bounds__(256) keys_hist_kernel(const float4 *__restrict__ body, const u32 *__restrict__ bbox_bits,
                                                         float *cube, u64 *__restrict__ keys, u32 *hist, u32 n,
-                                                        int max_level, int hilbert, int passes, const u32 *__restrict__ prev_ncells,
+                                                        int max_level, const u32 *__restrict__ hilbert_tab, int passes, const u32 *__restrict__ prev_ncells,
                                                         u32 cell_cap, u32 *cell_nchild, u32 *cell_ready)
 {
     // child counters of the cells of the previous build -> 0 (emit_kernel accumulates into them)
@@ -112,7 +210,10 @@ __global__ void __launch_bounds__(256) keys_hist_kernel(const float4 *__restrict
         cell_ready[k] = 0;
     }
     __shared__ u32 s_hist[8 * 256];
+    __shared__ u32 s_tab[P3T_HILBERT_TAB_WORDS];
     for (int t = threadIdx.x; t < 8 * 256; t += blockDim.x) s_hist[t] = 0;
+    if (hilbert_tab)
+        for (int t = threadIdx.x; t < P3T_HILBERT_TAB_WORDS; t += blockDim.x) s_tab[t] = hilbert_tab[t];
     float minx, miny, minz, side;
     root_cube(bbox_bits, minx, miny, minz, side);
     if (blockIdx.x == 0 && threadIdx.x == 0) { cube[0] = minx; cube[1] = miny; cube[2] = minz; cube[3] = side; }
@@ -124,7 +225,7 @@ __global__ void __launch_bounds__(256) keys_hist_kernel(const float4 *__restrict
         u32 qx = min((u32)fmaxf((b.x - minx) * scale, 0.f), qmax);
         u32 qy = min((u32)fmaxf((b.y - miny) * scale, 0.f), qmax);
         u32 qz = min((u32)fmaxf((b.z - minz) * scale, 0.f), qmax);
-        u64 key = p3t_encode_key(qx, qy, qz, max_level, hilbert);
+        u64 key = hilbert_tab ? hilbert_key_tab(s_tab, qx, qy, qz, max_level) : p3t_encode_key(qx, qy, qz, max_level, 0);
         keys[i] = key;
         for (int p = 0; p < passes; ++p) atomicAdd(&s_hist[p * 256 + (u32)((key >> (8 * p)) & 255u)], 1u);
     }
@@ -395,7 +496,7 @@ p3t_status p3t_stage_sort(p3t_ctx *ctx)
         P3T_CUDA(ctx, cudaMemsetAsync(w.prev_ncells, 0, sizeof(u32), s));
         ctx->cells_dirty = false;
     }
-    keys_hist_kernel<<<grid, 256, 0, s>>>(w.body_user, w.bbox_bits, w.cube, w.keys[0], w.hist, n, ctx->max_level, ctx->key_curve, passes,
+    keys_hist_kernel<<<grid, 256, 0, s>>>(w.body_user, w.bbox_bits, w.cube, w.keys[0], w.hist, n, ctx->max_level, ctx->key_curve ? w.hilbert_tab : nullptr, passes,
                                           w.prev_ncells, (u32)w.cell_cap, w.cell_nchild, w.cell_ready);
     int cur = 0;
     for (int p = 0; p < passes; ++p) {
