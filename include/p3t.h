@@ -294,6 +294,13 @@ const char *p3t_last_error(const p3t_ctx *ctx);
  * [host, nullable].  P3T_EINVAL for null ctx/tflops, iters <= 0 or packed outside 0..4. */
 p3t_status p3t_measure_fp32_peak(p3t_ctx *ctx, int packed, int iters, double *tflops, float *ms);
 
+/* Latency probes behind the floor table of the a1-a6 chain (profiles/tree_latency_floor_r2.md; not part of the hot path):
+ * ns per step of `iters` dependent steps of  what = 0: loads that hit L2;  1: global atomics;  2: back-to-back launches
+ * of an empty kernel;  3: the same launched with programmatic dependent launch;  4: fence + atomic + L2 load (one level
+ * of the moments climb).  Uses the first 32 MiB of the workspace as scratch: the context must be loaded again afterwards
+ * (P3T_ENOMEM if the workspace is smaller).  Synchronises.  P3T_EINVAL for bad arguments. */
+p3t_status p3t_measure_latency(p3t_ctx *ctx, int what, int iters, double *ns);
+
 /* Inspection of intermediate arrays (for the a1-a6 parity tests).  Valid after
  * p3t_build_tree.  p3t_array_info gives element count and element size. */
 typedef enum {

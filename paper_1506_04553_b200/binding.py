@@ -31,7 +31,7 @@ SYMBOLS = [
     "p3t_set_pair_classes", "p3t_set_key_curve", "p3t_hilbert_state_tables", "p3t_set_group_merge_levels", "p3t_set_walk_mode", "p3t_set_shard", "p3t_load_particles", "p3t_build_tree", "p3t_set_tree_reuse", "p3t_refit_tree", "p3t_eval_soft", "p3t_eval_direct", "p3t_eval_hard",
     "p3t_hermite_step", "p3t_step", "p3t_set_hermite_cluster_max",
     "p3t_get_acc_pot", "p3t_get_neighbour_counts", "p3t_get_neighbours", "p3t_get_stats", "p3t_synchronize",
-    "p3t_last_error", "p3t_array_info", "p3t_copy_array", "p3t_measure_fp32_peak",
+    "p3t_last_error", "p3t_array_info", "p3t_copy_array", "p3t_measure_fp32_peak", "p3t_measure_latency",
 ]
 
 ARRAYS = dict(root_cube=(0, np.float32, 1), keys=(1, np.uint64, 1), sorted_idx=(2, np.uint32, 1),
@@ -94,6 +94,7 @@ def _sig():
     L.p3t_last_error.restype = C.c_char_p; L.p3t_last_error.argtypes = [vp]
     L.p3t_array_info.restype = i; L.p3t_array_info.argtypes = [vp, i, C.POINTER(sz), C.POINTER(sz)]
     L.p3t_copy_array.restype = i; L.p3t_copy_array.argtypes = [vp, i, vp, sz, i]
+    L.p3t_measure_latency.restype = i; L.p3t_measure_latency.argtypes = [vp, i, i, C.POINTER(C.c_double)]
     L.p3t_measure_fp32_peak.restype = i
     L.p3t_measure_fp32_peak.argtypes = [vp, i, i, C.POINTER(C.c_double), C.POINTER(C.c_float)]
 
@@ -339,6 +340,13 @@ class P3T:
         tf, ms = C.c_double(), C.c_float()
         self._check(_lib.p3t_measure_fp32_peak(self._h, int(packed), int(iters), C.byref(tf), C.byref(ms)))
         return tf.value, ms.value
+
+    def measure_latency(self, what, iters=2000):
+        """ns per dependent step (p3t_measure_latency); scribbles over the workspace: load particles again afterwards."""
+        ns = C.c_double()
+        self._check(_lib.p3t_measure_latency(self._h, int(what), int(iters), C.byref(ns)))
+        self.n = 0
+        return ns.value
 
     def array(self, name):
         """Copy of an intermediate array (a1-a6 inspection), as numpy."""

@@ -188,8 +188,10 @@ __global__ void __launch_bounds__(BUILD_THREADS) levels_kernel(const signed char
     __shared__ int s_cnt[32];
     __shared__ u32 s_tile, s_lastcut;
     const int tid = threadIdx.x, lane = tid & 31;
+    P3T_GRID_TRIGGER();
     if (tid == 0) { s_tile = (u32)atomicAdd(&counters[CNT_HEAD_TICKET], 1ull); s_lastcut = 0; }   // tiles in scheduling order (look-back)
     __syncthreads();
+    P3T_GRID_WAIT();
     const u32 tile = s_tile;
     const long long base = (long long)tile * BUILD_TILE;
     // ---- window of biased c values (c + 1 in 0..22; 0 outside the array), two per word
@@ -302,8 +304,10 @@ __global__ void __launch_bounds__(BUILD_THREADS) emit_kernel(
     __shared__ u32 s_tile, s_headbase;
     __shared__ int s_carry;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    P3T_GRID_TRIGGER();
     if (tid == 0) { s_tile = (u32)atomicAdd(&counters[CNT_HEAD_SPARE0], 1ull); s_lo = 99; s_hi = -1; }
     __syncthreads();
+    P3T_GRID_WAIT();
     const u32 tile = s_tile;
     const u32 base = tile * BUILD_TILE;
     for (int q = tid; q < (BUILD_TILE + BUILD_HALO + 4) / 4; q += BUILD_THREADS) {   // c[base ..] four at a time
@@ -511,12 +515,13 @@ p3t_status p3t_stage_build(p3t_ctx *ctx)
         ctx->tiles_ready = true;
     }
     TileRec *tiles = recs + BUILD_LOOKBACK;
-    P3T_CUDA(ctx, cudaMemsetAsync(tiles, 0, (size_t)ntiles * sizeof(TileRec), s));
-    levels_kernel<<<ntiles, BUILD_THREADS, 0, s>>>(w.clev, w.dlev, w.cutflag, tiles, w.level_total, w.prev_ncells, n, ntiles, ctx->max_level,
-                                                  ctx->nleaf, ctx->ngroup, ctx->merge_levels, w.counters);
-    emit_kernel<<<ntiles, BUILD_THREADS, 0, s>>>(w.clev, w.dlev, w.cutflag, tiles, w.level_total, n, ntiles, ctx->max_level,
-                                                ctx->ngroup, (u32)w.cell_cap, w.cell_start, w.cell_level, w.cell_parent,
-                                                w.cell_first, w.cell_nchild, w.cell_meta, w.group_start, w.counters);
+    // (the tile records were zeroed by p3t_stage_sort, at the head of the chain)
+    static_assert(sizeof(TileRec) == 256 && BUILD_LOOKBACK == 8, "p3t_stage_sort zeroes the records behind 8 sentinels of 256 bytes");
+    P3T_CUDA(ctx, p3t_launch_pdl(levels_kernel, dim3(ntiles), dim3(BUILD_THREADS), 0, s, (const signed char *)w.clev, w.dlev, w.cutflag, tiles,
+                                 w.level_total, w.prev_ncells, n, ntiles, ctx->max_level, ctx->nleaf, ctx->ngroup, ctx->merge_levels, w.counters));
+    P3T_CUDA(ctx, p3t_launch_pdl(emit_kernel, dim3(ntiles), dim3(BUILD_THREADS), 0, s, (const signed char *)w.clev, (const u8 *)w.dlev,
+                                 (const u8 *)w.cutflag, tiles, (const u32 *)w.level_total, n, ntiles, ctx->max_level, ctx->ngroup, (u32)w.cell_cap,
+                                 w.cell_start, w.cell_level, w.cell_parent, w.cell_first, w.cell_nchild, w.cell_meta, w.group_start, w.counters));
     P3T_CUDA(ctx, cudaGetLastError());
     return P3T_OK;
 }

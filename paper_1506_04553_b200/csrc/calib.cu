@@ -111,3 +111,89 @@ extern "C" p3t_status p3t_measure_fp32_peak(p3t_ctx *ctx, int packed, int iters,
     if (ms_out) *ms_out = best;
     return P3T_OK;
 }
+
+// ------------------------------------------------------------------------------------------------
+// Latency probes for the floor table of the a1-a6 chain (profiles/tree_latency_floor_r2.md): what one dependent round
+// trip of the kind the look-back, climb and launch chains are made of costs on this device.
+//   0  dependent loads that hit L2 (ld.global.cg through a strided cycle over 32 MiB of the workspace), one thread
+//   1  dependent global atomics (atomicAdd whose result addresses the next one), one thread
+//   2  back-to-back launches of an empty kernel on the stream (ns per launch)
+//   3  the same with programmatic dependent launch (the attribute the a1-a6 chain uses)
+//   4  release fence + relaxed atomic + dependent L2 load: one level of the moments climb
+// ------------------------------------------------------------------------------------------------
+#define LAT_LINES (1u << 18)          // 128-byte lines in the probe buffer (32 MiB)
+#define LAT_STRIDE 40503u             // odd: i -> i + stride (mod 2^18) is one cycle through all lines
+
+__global__ void lat_init_kernel(u32 *buf)
+{
+    const u32 i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < LAT_LINES) buf[(size_t)i * 32] = ((i + LAT_STRIDE) & (LAT_LINES - 1u)) * 32u;
+}
+template <int WHAT>
+__global__ void lat_chase_kernel(u32 *buf, u32 steps, u32 *out)
+{
+    u32 p = 0;
+    for (u32 k = 0; k < steps; ++k) {
+        if (WHAT == 0) p = __ldcg(buf + p);
+        if (WHAT == 1) p = atomicAdd(buf + p, 0u);
+        if (WHAT == 4) { __threadfence(); atomicAdd(buf + p + 1, 1u); p = __ldcg(buf + p); }
+    }
+    out[0] = p;
+}
+__global__ void lat_empty_kernel(u32 *out)
+{
+    P3T_GRID_TRIGGER();
+    P3T_GRID_WAIT();
+    if (out == nullptr) printf("never\n");
+}
+
+extern "C" p3t_status p3t_measure_latency(p3t_ctx *ctx, int what, int iters, double *ns)
+{
+    if (!ctx || !ns || iters <= 0 || what < 0 || what > 4) return p3t_fail(ctx, P3T_EINVAL, "p3t_measure_latency: bad argument");
+    if (ctx->ws.total_bytes < ((size_t)LAT_LINES * 128 + 4096)) return p3t_fail(ctx, P3T_ENOMEM, "p3t_measure_latency needs a workspace of 32 MiB (max_n >= 65536)");
+    cudaStream_t s = ctx->stream;
+    u32 *buf = reinterpret_cast<u32 *>(ctx->base);          // scratch use of the workspace: the context must be reloaded afterwards
+    u32 *out = buf + (size_t)LAT_LINES * 32;
+    ctx->loaded = ctx->built = ctx->evaluated = ctx->topo_valid = false;
+    ctx->status_clean = ctx->tiles_ready = false;
+    ctx->cells_dirty = true;
+    cudaEvent_t e0, e1;
+    P3T_CUDA(ctx, cudaEventCreate(&e0));
+    P3T_CUDA(ctx, cudaEventCreate(&e1));
+    float best = 1e30f;
+    for (int rep = 0; rep < 4; ++rep) {
+        if (what == 0 || what == 1 || what == 4) {
+            P3T_CUDA(ctx, cudaMemsetAsync(buf, 0, (size_t)LAT_LINES * 128, s));
+            lat_init_kernel<<<LAT_LINES / 256, 256, 0, s>>>(buf);
+        }
+        P3T_CUDA(ctx, cudaEventRecord(e0, s));
+        if (what == 0) lat_chase_kernel<0><<<1, 1, 0, s>>>(buf, (u32)iters, out);
+        else if (what == 1) lat_chase_kernel<1><<<1, 1, 0, s>>>(buf, (u32)iters, out);
+        else if (what == 4) lat_chase_kernel<4><<<1, 1, 0, s>>>(buf, (u32)iters, out);
+        else
+            for (int k = 0; k < iters; ++k) {
+                if (what == 2) lat_empty_kernel<<<148, 128, 0, s>>>(out);
+                else P3T_CUDA(ctx, p3t_launch_pdl(lat_empty_kernel, dim3(148), dim3(128), 0, s, out));
+            }
+        P3T_CUDA(ctx, cudaEventRecord(e1, s));
+        P3T_CUDA(ctx, cudaEventSynchronize(e1));
+        float ms = 0.f;
+        P3T_CUDA(ctx, cudaEventElapsedTime(&ms, e0, e1));
+        if (rep > 0 && ms < best) best = ms;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    P3T_CUDA(ctx, cudaGetLastError());
+    // the hilbert tables live in the workspace the probe has scribbled over
+    {
+        static u32 tab[P3T_HILBERT_TAB_WORDS];
+        if (!p3t_hilbert_tables(tab)) return p3t_fail(ctx, P3T_ECUDA, "hilbert tables");
+        P3T_CUDA(ctx, cudaMemcpyAsync(ctx->ws.hilbert_tab, tab, sizeof(tab), cudaMemcpyHostToDevice, s));
+        P3T_CUDA(ctx, cudaMemsetAsync(ctx->ws.order_meta, 0, 4 * sizeof(u32), s));
+        P3T_CUDA(ctx, cudaMemsetAsync(ctx->ws.body_class, 0, ctx->max_n * sizeof(u32), s));
+        P3T_CUDA(ctx, cudaMemsetAsync(ctx->ws.counters, 0, CNT_WORDS * sizeof(u64), s));
+        P3T_CUDA(ctx, cudaStreamSynchronize(s));
+    }
+    *ns = (double)best * 1e6 / (double)iters;
+    return P3T_OK;
+}

@@ -21,15 +21,24 @@ struct Mom {
 };
 
 template <bool REFIT>
-__device__ __forceinline__ void store_cell(u32 k, const Mom &m, int level, u64 key, const float *__restrict__ cube,
+__device__ __forceinline__ void store_cell(u32 k, const Mom &m, int level, u64 key, const float4 &b0, const float *__restrict__ cube,
                                            int max_level, int hilbert, float theta, float h, float4 *cell_mac, float4 *cell_mom0,
                                            float4 *cell_mom1, float4 *cell_bmin, float4 *cell_bmax)
 {
     const float side = cube[3];
     const float l = ldexpf(side, -level);
-    // geometric centre from the key of the cell's first body: its quantised coordinates, cut to `level` bits
+    // geometric centre from the cell's first body: its quantised coordinates, cut to `level` bits.  A build takes them
+    // from the body's position with the arithmetic of keys_hist_kernel (the same integers, no inverse transform in the
+    // latency chain of the climb); a refit, whose bodies have moved, from the body's key.
     u32 qx, qy, qz;
-    p3t_decode_key(key, max_level, hilbert, qx, qy, qz);
+    if (REFIT) p3t_decode_key(key, max_level, hilbert, qx, qy, qz);
+    else {
+        const float scale = (float)(1u << max_level) / side;
+        const u32 qmax = (1u << max_level) - 1u;
+        qx = min((u32)fmaxf((b0.x - cube[0]) * scale, 0.f), qmax);
+        qy = min((u32)fmaxf((b0.y - cube[1]) * scale, 0.f), qmax);
+        qz = min((u32)fmaxf((b0.z - cube[2]) * scale, 0.f), qmax);
+    }
     const int sh = max_level - level;
     float gx = cube[0] + ((float)(qx >> sh) + 0.5f) * l;
     float gy = cube[1] + ((float)(qy >> sh) + 0.5f) * l;
@@ -114,6 +123,8 @@ __global__ void __launch_bounds__(128, 4) moments_kernel(
     float4 *cell_bmax, const u64 *__restrict__ counters, u32 cell_cap, int max_level, int hilbert, float theta, float h,
     const u8 *__restrict__ cls_sorted, float h_bf)
 {
+    P3T_GRID_TRIGGER();
+    P3T_GRID_WAIT();
     const u32 ncell = (u32)min((u64)cell_cap, counters[CNT_NCELLS]);
     for (u32 k0 = blockIdx.x * blockDim.x + threadIdx.x; k0 < ncell; k0 += gridDim.x * blockDim.x) {
         u32 k = k0;
@@ -164,14 +175,15 @@ __global__ void __launch_bounds__(128, 4) moments_kernel(
                 m.cx = 0.5f * (m.lox + m.hix); m.cy = 0.5f * (m.loy + m.hiy); m.cz = 0.5f * (m.loz + m.hiz);
                 m.qxx = m.qyy = m.qzz = m.qxy = m.qxz = m.qyz = 0.f;
             }
-            store_cell<REFIT>(k, m, level, keys[start], cube, max_level, hilbert, theta, m.heavy ? h_bf : h, cell_mac, cell_mom0, cell_mom1, cell_bmin, cell_bmax);
+            store_cell<REFIT>(k, m, level, REFIT ? keys[start] : 0ull, b0, cube, max_level, hilbert, theta, m.heavy ? h_bf : h, cell_mac, cell_mom0, cell_mom1, cell_bmin, cell_bmax);
             continue;
         }
         // ---- internal cell
         u32 cw = cell_nchild[k];
         if (cw >> 16) continue;          // has internal children: computed by the last of them to arrive
         u32 first = cell_first[k], parent = cell_parent[k];
-        u64 key = keys[start];
+        u64 key = REFIT ? keys[start] : 0ull;
+        float4 bfirst = REFIT ? make_float4(0.f, 0.f, 0.f, 0.f) : body[start];
         while (true) {
             const u32 nch = cw & 0xffffu;
             P3T_DEV_ASSERT(nch >= 1 && nch <= 8 && first > k && first + nch <= ncell && (parent == P3T_NO_PARENT || parent < k));
@@ -184,13 +196,14 @@ __global__ void __launch_bounds__(128, 4) moments_kernel(
                 plevel = cell_level[parent]; pstart = cell_start[parent];
             }
             merge_children(first, nch, cell_mac, cell_mom0, cell_mom1, cell_bmin, cell_bmax, m);
-            const u64 pkey = parent != P3T_NO_PARENT ? keys[pstart] : 0ull;
-            store_cell<REFIT>(k, m, level, key, cube, max_level, hilbert, theta, m.heavy ? h_bf : h, cell_mac, cell_mom0, cell_mom1, cell_bmin, cell_bmax);
+            const u64 pkey = (REFIT && parent != P3T_NO_PARENT) ? keys[pstart] : 0ull;
+            const float4 pb = (!REFIT && parent != P3T_NO_PARENT) ? body[pstart] : make_float4(0.f, 0.f, 0.f, 0.f);
+            store_cell<REFIT>(k, m, level, key, bfirst, cube, max_level, hilbert, theta, m.heavy ? h_bf : h, cell_mac, cell_mom0, cell_mom1, cell_bmin, cell_bmax);
             cell_meta[k] = make_uint2(first, nch);
             if (parent == P3T_NO_PARENT) break;
             __threadfence();             // my record is visible before my arrival is
             if (atomicAdd(&cell_ready[parent], 1u) + 1 != (pcw >> 16)) break;
-            k = parent; cw = pcw; first = pfirst; parent = pparent; level = plevel; start = pstart; key = pkey;
+            k = parent; cw = pcw; first = pfirst; parent = pparent; level = plevel; start = pstart; key = pkey; bfirst = pb;
         }
     }
 }
@@ -203,14 +216,16 @@ p3t_status p3t_stage_moments(p3t_ctx *ctx)
     size_t bound = ctx->n * (size_t)(ctx->max_level + 1);
     if (bound > w.cell_cap) bound = w.cell_cap;
     const u32 grid = (u32)min((size_t)div_up(bound, 128), (size_t)ctx->sm_count * 16);
-    moments_kernel<0, false><<<grid, 128, 0, s>>>(w.body, w.keys[ctx->cur], w.cube, w.cell_level, w.cell_start, w.cell_parent, w.cell_first,
-                                           w.cell_nchild, w.cell_ready, w.cell_meta, w.cell_mac, w.cell_mom0, w.cell_mom1,
-                                           w.cell_bmin, w.cell_bmax, w.counters, (u32)w.cell_cap, ctx->max_level, ctx->key_curve, ctx->prm.theta,
-                                           ctx->prm.h, ctx->cls_n ? w.cls_sorted : nullptr, ctx->prm.h_bf);
-    moments_kernel<1, false><<<grid, 128, 0, s>>>(w.body, w.keys[ctx->cur], w.cube, w.cell_level, w.cell_start, w.cell_parent, w.cell_first,
-                                           w.cell_nchild, w.cell_ready, w.cell_meta, w.cell_mac, w.cell_mom0, w.cell_mom1,
-                                           w.cell_bmin, w.cell_bmax, w.counters, (u32)w.cell_cap, ctx->max_level, ctx->key_curve, ctx->prm.theta,
-                                           ctx->prm.h, ctx->cls_n ? w.cls_sorted : nullptr, ctx->prm.h_bf);
+    P3T_CUDA(ctx, p3t_launch_pdl(moments_kernel<0, false>, dim3(grid), dim3(128), 0, s, (const float4 *)w.body, (const u64 *)w.keys[ctx->cur],
+                                 (const float *)w.cube, (const u8 *)w.cell_level, (const u32 *)w.cell_start, (const u32 *)w.cell_parent,
+                                 (const u32 *)w.cell_first, w.cell_nchild, w.cell_ready, w.cell_meta, w.cell_mac, w.cell_mom0, w.cell_mom1,
+                                 w.cell_bmin, w.cell_bmax, (const u64 *)w.counters, (u32)w.cell_cap, ctx->max_level, ctx->key_curve,
+                                 ctx->prm.theta, ctx->prm.h, (const u8 *)(ctx->cls_n ? w.cls_sorted : nullptr), ctx->prm.h_bf));
+    P3T_CUDA(ctx, p3t_launch_pdl(moments_kernel<1, false>, dim3(grid), dim3(128), 0, s, (const float4 *)w.body, (const u64 *)w.keys[ctx->cur],
+                                 (const float *)w.cube, (const u8 *)w.cell_level, (const u32 *)w.cell_start, (const u32 *)w.cell_parent,
+                                 (const u32 *)w.cell_first, w.cell_nchild, w.cell_ready, w.cell_meta, w.cell_mac, w.cell_mom0, w.cell_mom1,
+                                 w.cell_bmin, w.cell_bmax, (const u64 *)w.counters, (u32)w.cell_cap, ctx->max_level, ctx->key_curve,
+                                 ctx->prm.theta, ctx->prm.h, (const u8 *)(ctx->cls_n ? w.cls_sorted : nullptr), ctx->prm.h_bf));
     P3T_CUDA(ctx, cudaGetLastError());
     return P3T_OK;
 }

@@ -207,6 +207,27 @@ static inline p3t_status p3t_fail(p3t_ctx *ctx, p3t_status st, const char *msg)
 
 static inline u32 div_up(size_t a, size_t b) { return (u32)((a + b - 1) / b); }
 
+#ifdef __CUDACC__
+// Programmatic dependent launch: the kernels of the a1-a6 chain are launched with the stream-serialisation attribute,
+// so a kernel's CTAs may become resident and run their prologue (ticket, shared-memory clears, parameter loads) while
+// the kernel before it drains; P3T_GRID_WAIT() (griddepcontrol.wait) stands in front of the first access to anything
+// a predecessor wrote or still reads, P3T_GRID_TRIGGER() (griddepcontrol.launch_dependents) at the top of each kernel.
+// Every kernel launched this way must execute P3T_GRID_WAIT() on all paths: completion is only transitive through it.
+#define P3T_GRID_WAIT() cudaGridDependencySynchronize()
+#define P3T_GRID_TRIGGER() cudaTriggerProgrammaticLaunchCompletion()
+template <class K, class... A>
+static inline cudaError_t p3t_launch_pdl(K kernel, dim3 grid, dim3 block, size_t smem, cudaStream_t s, A... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = s;
+    cudaLaunchAttribute attr;
+    attr.id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr.val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = &attr; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, args...);
+}
+#endif
+
 // stage entry points (each enqueues kernels on ctx->stream)
 p3t_status p3t_stage_pack(p3t_ctx *ctx, const float *d_mass, const float *d_pos);
 #define P3T_HILBERT_STATES 24

@@ -305,10 +305,12 @@ __global__ void __launch_bounds__(SORT_THREADS, 1024 / SORT_THREADS) onesweep_ke
     const u32 tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     // tiles must start in index order for the look-back to make progress: guaranteed by a ticket, or by the
     // grid being resident as a whole (ticket == nullptr)
+    P3T_GRID_TRIGGER();
     if (tid == 0) sm.tile = ticket ? (u32)atomicAdd(ticket, 1ull) : blockIdx.x;
 #pragma unroll
     for (u32 t = 0; t < 8; ++t) sm.whist[warp][t * 32 + lane] = 0;
     __syncthreads();
+    P3T_GRID_WAIT();      // the pass before: its keys and values, and its last reads of the status rows zeroed below
     const u32 tile = sm.tile;
     P3T_DEV_ASSERT(tile < (n + SORT_TILE - 1) / SORT_TILE);
     const u32 tile_base = tile * SORT_TILE;
@@ -448,6 +450,8 @@ __global__ void __launch_bounds__(256) gather_kernel(const float4 *__restrict__ 
                                                      signed char *__restrict__ clev, u32 n, int max_level,
                                                      const u8 *__restrict__ cls_user, u8 *__restrict__ cls_sorted)
 {
+    P3T_GRID_TRIGGER();
+    P3T_GRID_WAIT();
     u32 i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i > n) return;
     if (i == n) { clev[n] = -1; return; }
@@ -496,6 +500,9 @@ p3t_status p3t_stage_sort(p3t_ctx *ctx)
         P3T_CUDA(ctx, cudaMemsetAsync(w.prev_ncells, 0, sizeof(u32), s));
         ctx->cells_dirty = false;
     }
+    // (the build's tile records are zeroed here, not in front of levels_kernel: a memset between two kernels would break
+    //  the chain of programmatic launches)
+    P3T_CUDA(ctx, cudaMemsetAsync(reinterpret_cast<char *>(w.build_tiles) + 8 * 256, 0, (size_t)div_up(n, BUILD_TILE) * 256, s));
     keys_hist_kernel<<<grid, 256, 0, s>>>(w.body_user, w.bbox_bits, w.cube, w.keys[0], w.hist, n, ctx->max_level, ctx->key_curve ? w.hilbert_tab : nullptr, passes,
                                           w.prev_ncells, (u32)w.cell_cap, w.cell_nchild, w.cell_ready);
     int cur = 0;
@@ -503,18 +510,21 @@ p3t_status p3t_stage_sort(p3t_ctx *ctx)
         u32 *st_cur = w.tile_status + ((size_t)(p & 1) * status_rows + SORT_LOOKBACK) * 256;
         u32 *st_next = w.tile_status + ((size_t)((p + 1) & 1) * status_rows + SORT_LOOKBACK) * 256;
         const u32 *vin = p == 0 ? nullptr : w.idx[cur];
+        // (tiles always take their index from the ticket: the order in which resident CTAs of a look-back chain start is
+        //  not something CUDA promises, least of all next to other work on the device)
+        u64 *ticket = w.counters + CNT_SORT_TICKET + p;
         if (ntiles <= (u32)resident)
-            onesweep_kernel<16><<<ntiles, SORT_THREADS, sizeof(OnesweepSmem), s>>>(w.keys[cur], vin, w.keys[cur ^ 1], w.idx[cur ^ 1], n, 8 * p,
-                                                                                   w.hist + p * 256, st_cur, st_next, nullptr);
+            P3T_CUDA(ctx, p3t_launch_pdl(onesweep_kernel<16>, dim3(ntiles), dim3(SORT_THREADS), sizeof(OnesweepSmem), s, (const u64 *)w.keys[cur], vin,
+                                         w.keys[cur ^ 1], w.idx[cur ^ 1], n, 8 * p, (const u32 *)(w.hist + p * 256), st_cur, st_next, ticket));
         else
-            onesweep_kernel<8><<<ntiles, SORT_THREADS, sizeof(OnesweepSmem), s>>>(w.keys[cur], vin, w.keys[cur ^ 1], w.idx[cur ^ 1], n, 8 * p,
-                                                                                  w.hist + p * 256, st_cur, st_next,
-                                                                                  w.counters + CNT_SORT_TICKET + p);
+            P3T_CUDA(ctx, p3t_launch_pdl(onesweep_kernel<8>, dim3(ntiles), dim3(SORT_THREADS), sizeof(OnesweepSmem), s, (const u64 *)w.keys[cur], vin,
+                                         w.keys[cur ^ 1], w.idx[cur ^ 1], n, 8 * p, (const u32 *)(w.hist + p * 256), st_cur, st_next, ticket));
         cur ^= 1;
     }
     ctx->cur = cur;
-    gather_kernel<<<div_up(n + 1, 256), 256, 0, s>>>(w.body_user, w.idx[cur], w.keys[cur], w.body, w.clev, n, ctx->max_level,
-                                                     ctx->cls_n ? w.cls_user : nullptr, w.cls_sorted);
+    P3T_CUDA(ctx, p3t_launch_pdl(gather_kernel, dim3(div_up(n + 1, 256)), dim3(256), 0, s, (const float4 *)w.body_user, (const u32 *)w.idx[cur],
+                                 (const u64 *)w.keys[cur], w.body, w.clev, n, ctx->max_level,
+                                 (const u8 *)(ctx->cls_n ? w.cls_user : nullptr), w.cls_sorted));
     P3T_CUDA(ctx, cudaGetLastError());
     return P3T_OK;
 }

@@ -840,15 +840,17 @@ __global__ void __launch_bounds__(256) group_predict_kernel(const u32 *__restric
                                                             const u32 *__restrict__ body_class, const u64 *__restrict__ counters,
                                                             u32 *__restrict__ gclass, u32 *hist)
 {
-    const u32 g = blockIdx.x * blockDim.x + threadIdx.x;
-    if (g >= (u32)counters[CNT_NGROUPS]) return;
-    // (class 0 = most expensive: the minimum over the first, middle and last body guards against a group that inherited
-    //  its first body from a cheaper neighbour)
-    const u32 gs = group_start[g], ge = group_start[g + 1];
-    const u32 c = min(min(body_class[sorted_idx[gs]], body_class[sorted_idx[gs + (ge - gs) / 2]]),
-                      min(body_class[sorted_idx[ge - 1]], (u32)ORDER_CLASSES - 1u));
-    gclass[g] = c;
-    atomicAdd(&hist[c], 1u);
+    const u32 ng = (u32)counters[CNT_NGROUPS];
+    // (the group count lives on the device: a fixed grid strides over it)
+    for (u32 g = blockIdx.x * blockDim.x + threadIdx.x; g < ng; g += gridDim.x * blockDim.x) {
+        // (class 0 = most expensive: the minimum over the first, middle and last body guards against a group that
+        //  inherited its first body from a cheaper neighbour)
+        const u32 gs = group_start[g], ge = group_start[g + 1];
+        const u32 c = min(min(body_class[sorted_idx[gs]], body_class[sorted_idx[gs + (ge - gs) / 2]]),
+                          min(body_class[sorted_idx[ge - 1]], (u32)ORDER_CLASSES - 1u));
+        gclass[g] = c;
+        atomicAdd(&hist[c], 1u);
+    }
 }
 
 __global__ void __launch_bounds__(256) group_order_kernel(const u32 *__restrict__ gclass, const u32 *__restrict__ hist, u32 *cursor,
@@ -874,12 +876,11 @@ __global__ void __launch_bounds__(256) group_order_kernel(const u32 *__restrict_
 #pragma unroll
     for (int k = 0; k < 4; ++k) { s_base[4 * tid + k] = base; base += v[k]; }
     __syncthreads();
-    const u32 g = blockIdx.x * blockDim.x + tid;
-    if (g < ng) {
+    for (u32 g = blockIdx.x * blockDim.x + tid; g < ng; g += gridDim.x * blockDim.x) {
         const u32 c = gclass[g];
         order[s_base[c] + atomicAdd(&cursor[c], 1u)] = g;
     }
-    if (g == 0) order_meta[0] = ng;
+    if (blockIdx.x == 0 && tid == 0) order_meta[0] = ng;
 }
 
 #ifdef P3T_WALK_PROFILE
@@ -929,8 +930,9 @@ p3t_status p3t_stage_walk(p3t_ctx *ctx)
     // hand-out order of this call's groups from the classes the previous call left per body (the group count lives on
     // the device: launch for its upper bound n / 1 .. n groups; a sharded walk keeps Morton order)
     if (ctx->shard_world == 1) {
-        group_predict_kernel<<<div_up(ctx->n, 256), 256, 0, s>>>(w.group_start, w.idx[ctx->cur], w.body_class, w.counters, w.group_class, w.order_hist);
-        group_order_kernel<<<div_up(ctx->n, 256), 256, 0, s>>>(w.group_class, w.order_hist, w.order_hist + ORDER_CLASSES, w.counters,
+        const u32 ogrid = min(div_up(ctx->n, 256 * 32), (u32)ctx->sm_count * 4);     // about n / 50 groups: a few per thread
+        group_predict_kernel<<<ogrid, 256, 0, s>>>(w.group_start, w.idx[ctx->cur], w.body_class, w.counters, w.group_class, w.order_hist);
+        group_order_kernel<<<ogrid, 256, 0, s>>>(w.group_class, w.order_hist, w.order_hist + ORDER_CLASSES, w.counters,
                                                               w.group_order, w.order_meta);
     }
     // one CTA per group when there are too few groups to keep every warp busy to the end of the launch
