@@ -211,6 +211,7 @@ def main():
         ctx.set_shard(rank, world)
     acc_d = torch.empty((n, 3), dtype=torch.float32, device=dev)
     pot_d = torch.empty(n, dtype=torch.float32, device=dev)
+    rec_d = torch.empty((n, 5), dtype=torch.float32, device=dev) if shard else None
     if args.refit:
         ctx.set_tree_reuse(args.refit)
 
@@ -221,9 +222,10 @@ def main():
         else:
             ctx.build_tree()
         ctx.eval_soft()
-        ctx.get_acc_pot_into(acc_d, pot_d)   # a9: accelerations and potentials in user order, in the caller's arrays
-        if shard:      # every rank ends the step with the accelerations and potentials of all particles
-            multi.allreduce_forces(dist, acc_d, pot_d)
+        if shard:      # every rank ends the step with the accelerations and potentials of all particles: one all-reduce
+            multi.allreduce_shard(dist, ctx, rec_d)
+        else:
+            ctx.get_acc_pot_into(acc_d, pot_d)   # a9: accelerations and potentials in user order, in the caller's arrays
 
     # Between steps the bodies move by one leapfrog step with the returned forces (BASELINE.json configs[1] asks for it
     # in so many words: "positions are drifted by a leapfrog step dt_soft using the returned forces"; for the other

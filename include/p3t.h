@@ -164,6 +164,19 @@ p3t_status p3t_set_walk_mode(p3t_ctx *ctx, int mode);
  * Default (0, 1): everything.  P3T_EINVAL unless 0 <= rank < world. */
 p3t_status p3t_set_shard(p3t_ctx *ctx, int rank, int world);
 
+/* The exchange of a sharded evaluation as ONE all-reduce (sum) over the ranks.  p3t_get_shard_record writes, for every
+ * particle in user order, five floats to rec[5n] [device]: (a_x, a_y, a_z, phi, cost class + 1) -- all zero for the
+ * particles of the groups other ranks walked, so the sum over the ranks holds the acceleration, the potential and the
+ * cost class of every particle.  p3t_put_shard_classes hands the summed record back [device]: the context takes the cost
+ * classes from it, and since every rank now holds the same classes, the next p3t_eval_soft orders the groups by
+ * predicted cost on every rank alike (an order kernel without atomics) and deals the positions of that order round
+ * robin to the ranks -- each rank gets the same mix of expensive and cheap groups, longest first (SURVEY.md 8(e):
+ * "balanced by the previous call's per-group interaction counts").  Without the exchange a sharded walk deals the groups
+ * out in key order.  Both calls only enqueue.  P3T_ESTATE before an eval call; P3T_EINVAL for a null pointer.
+ * (paper_1506_04553_b200/multi.py: allreduce_shard.) */
+p3t_status p3t_get_shard_record(p3t_ctx *ctx, float *rec);
+p3t_status p3t_put_shard_classes(p3t_ctx *ctx, const float *rec);
+
 /* Load n particles: mass[n], pos[3n] (x,y,z interleaved), both host or both
  * device (on_device).  Every value is tested for being finite by the kernel that
  * packs the bodies.  Host data: the call waits for the copies and that kernel and

@@ -28,7 +28,7 @@ _STATUS = {0: "P3T_OK", -1: "P3T_EINVAL", -2: "P3T_ESTATE", -3: "P3T_ENOMEM", -4
 # names of include/p3t.h's exported entry points (tests check that each resolves)
 SYMBOLS = [
     "p3t_workspace_bytes", "p3t_create", "p3t_destroy", "p3t_set_params", "p3t_set_tree_params",
-    "p3t_set_pair_classes", "p3t_set_key_curve", "p3t_hilbert_state_tables", "p3t_set_group_merge_levels", "p3t_set_walk_mode", "p3t_set_shard", "p3t_load_particles", "p3t_build_tree", "p3t_set_tree_reuse", "p3t_refit_tree", "p3t_eval_soft", "p3t_eval_direct", "p3t_eval_hard",
+    "p3t_set_pair_classes", "p3t_set_key_curve", "p3t_hilbert_state_tables", "p3t_set_group_merge_levels", "p3t_set_walk_mode", "p3t_set_shard", "p3t_get_shard_record", "p3t_put_shard_classes", "p3t_load_particles", "p3t_build_tree", "p3t_set_tree_reuse", "p3t_refit_tree", "p3t_eval_soft", "p3t_eval_direct", "p3t_eval_hard",
     "p3t_hermite_step", "p3t_step", "p3t_set_hermite_cluster_max",
     "p3t_get_acc_pot", "p3t_get_neighbour_counts", "p3t_get_neighbours", "p3t_get_stats", "p3t_synchronize",
     "p3t_last_error", "p3t_array_info", "p3t_copy_array", "p3t_measure_fp32_peak", "p3t_measure_latency",
@@ -76,6 +76,8 @@ def _sig():
     L.p3t_set_walk_mode.restype = i; L.p3t_set_walk_mode.argtypes = [vp, i]
     L.p3t_set_hermite_cluster_max.restype = i; L.p3t_set_hermite_cluster_max.argtypes = [vp, i]
     L.p3t_set_shard.restype = i; L.p3t_set_shard.argtypes = [vp, i, i]
+    L.p3t_get_shard_record.restype = i; L.p3t_get_shard_record.argtypes = [vp, vp]
+    L.p3t_put_shard_classes.restype = i; L.p3t_put_shard_classes.argtypes = [vp, vp]
     L.p3t_load_particles.restype = i; L.p3t_load_particles.argtypes = [vp, sz, vp, vp, i]
     L.p3t_build_tree.restype = i; L.p3t_build_tree.argtypes = [vp]
     L.p3t_eval_soft.restype = i; L.p3t_eval_soft.argtypes = [vp]
@@ -212,6 +214,19 @@ class P3T:
 
     def set_shard(self, rank, world):
         self._check(_lib.p3t_set_shard(self._h, rank, world))
+
+    def get_shard_record(self, rec=None):
+        """float32 CUDA tensor [n, 5]: (a, phi, cost class + 1) of the particles this shard produced, zeros elsewhere."""
+        t = self.torch
+        if rec is None:
+            rec = t.empty((self.n, 5), dtype=t.float32, device=f"cuda:{self.device}")
+        assert rec.is_cuda and rec.is_contiguous() and rec.numel() == 5 * self.n and rec.dtype == t.float32
+        self._check(_lib.p3t_get_shard_record(self._h, rec.data_ptr()))
+        return rec
+
+    def put_shard_classes(self, rec):
+        assert rec.is_cuda and rec.is_contiguous() and rec.numel() == 5 * self.n
+        self._check(_lib.p3t_put_shard_classes(self._h, rec.data_ptr()))
 
     def load_particles(self, mass, pos):
         """mass[n], pos[n,3] (or [3n]): float32 numpy arrays (host) or CUDA tensors (device)."""

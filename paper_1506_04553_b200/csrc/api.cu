@@ -341,7 +341,28 @@ extern "C" p3t_status p3t_set_shard(p3t_ctx *ctx, int rank, int world)
     ctx->shard_rank = rank;
     ctx->shard_world = world;
     ctx->evaluated = false;
+    ctx->shard_classes_fresh = false;
     return P3T_OK;
+}
+
+extern "C" p3t_status p3t_get_shard_record(p3t_ctx *ctx, float *rec)
+{
+    if (!ctx) return P3T_EINVAL;
+    if (!rec) return p3t_fail(ctx, P3T_EINVAL, "null rec");
+    if (!ctx->evaluated) return p3t_fail(ctx, P3T_ESTATE, "p3t_get_shard_record before an eval call");
+    P3T_CUDA(ctx, cudaSetDevice(ctx->device));
+    return p3t_stage_shard_record(ctx, rec);
+}
+
+extern "C" p3t_status p3t_put_shard_classes(p3t_ctx *ctx, const float *rec)
+{
+    if (!ctx) return P3T_EINVAL;
+    if (!rec) return p3t_fail(ctx, P3T_EINVAL, "null rec");
+    if (!ctx->evaluated) return p3t_fail(ctx, P3T_ESTATE, "p3t_put_shard_classes before an eval call");
+    P3T_CUDA(ctx, cudaSetDevice(ctx->device));
+    p3t_status st = p3t_stage_shard_classes(ctx, rec);
+    if (st == P3T_OK) ctx->shard_classes_fresh = true;
+    return st;
 }
 
 extern "C" p3t_status p3t_set_hermite_cluster_max(p3t_ctx *ctx, int max_members)

@@ -158,6 +158,7 @@ struct p3t_ctx {
     int walk_mode;                 // 0 auto, 1 one warp per group, 2 one CTA per group (cooperative)
     size_t cls_n;                  // 0: no classes; else the particle count the classes were given for
     float r_in_bf, r_out_bf, r_search_bf, eps_bb;
+    bool shard_classes_fresh;      // p3t_put_shard_classes since the last sharded walk: all ranks hold the same cost classes
     int shard_rank, shard_world;   // this context walks the groups at positions rank, rank + world, ... of the hand-out order
     int sm_count;
     bool have_params, loaded, built, evaluated;
@@ -239,6 +240,8 @@ p3t_status p3t_stage_moments(p3t_ctx *ctx);
 p3t_status p3t_stage_refit_begin(p3t_ctx *ctx);
 p3t_status p3t_stage_refit_finish(p3t_ctx *ctx);
 p3t_status p3t_stage_walk(p3t_ctx *ctx);
+p3t_status p3t_stage_shard_record(p3t_ctx *ctx, float *d_rec);
+p3t_status p3t_stage_shard_classes(p3t_ctx *ctx, const float *d_rec);
 p3t_status p3t_stage_direct(p3t_ctx *ctx, const u32 *d_subset, size_t n_subset);
 p3t_status p3t_stage_neighbours(p3t_ctx *ctx);
 p3t_status p3t_stage_unpack(p3t_ctx *ctx, float *d_acc, float *d_pot);

@@ -380,6 +380,7 @@ struct WalkArgs {
     u32 *__restrict__ body_class;    // [n] user order: cost class of the group each body was in (this walk's record for the next call)
     u32 *order_hist;                 // [ORDER_CLASSES] groups per class
     u32 shard_rank, shard_world;     // this launch walks positions rank, rank + world, ... of the hand-out order
+    u32 use_order;                   // 0: positions are group numbers (a sharded walk whose ranks have not exchanged cost classes)
     uint2 *pairs;
     u64 pair_cap;
     u64 *counters;
@@ -769,8 +770,9 @@ walk_kernel(WalkArgs A, const u32 *__restrict__ group_start, P3TParams prm, u32 
     // Hand-out order: this call's groups by decreasing PREDICTED cost (group_order, a permutation of 0..ngroups-1 made
     // by group_predict_kernel + group_order_kernel just before this launch: a group is expected to cost what the group
     // that held its first body cost in the previous call).
-    // A sharded walk hands out positions in Morton order: every rank must map positions to groups alike.
-    const u32 ng_prev = A.shard_world > 1 ? 0u : A.order_meta[0];
+    // Every rank of a sharded walk must map positions to groups alike: it uses the order only if the ranks have exchanged
+    // their cost classes since the last walk (p3t_put_shard_classes), else positions are group numbers (key order).
+    const u32 ng_prev = A.use_order ? A.order_meta[0] : 0u;
     const u32 npos = max(ngroups, ng_prev);
     u64 tot_pp = 0, tot_pc = 0, tot_near = 0;
 
@@ -883,6 +885,71 @@ __global__ void __launch_bounds__(256) group_order_kernel(const u32 *__restrict_
     if (blockIdx.x == 0 && tid == 0) order_meta[0] = ng;
 }
 
+// The same order without atomics: one CTA, groups taken 1024 at a time, a group's place inside its class = the places
+// taken by earlier chunks + the number of groups of its class before it in the chunk.  Slower (about 50 us per 20 000
+// groups) but a function of the classes alone: the ranks of a sharded walk all get the SAME order, which is what lets
+// them deal its positions out among themselves (p3t_set_shard).
+__global__ void __launch_bounds__(1024) group_order_det_kernel(const u32 *__restrict__ gclass, const u32 *__restrict__ hist,
+                                                               const u64 *__restrict__ counters, u32 *__restrict__ order, u32 *order_meta)
+{
+    __shared__ u32 s_base[ORDER_CLASSES], s_cur[ORDER_CLASSES], s_cls[1024];
+    const u32 ng = (u32)counters[CNT_NGROUPS], tid = threadIdx.x;
+    if (tid == 0) {
+        u32 run = 0;
+        for (u32 c = 0; c < ORDER_CLASSES; ++c) { s_base[c] = run; run += hist[c]; }
+    }
+    s_cur[tid] = 0;
+    __syncthreads();
+    for (u32 g0 = 0; g0 < ng; g0 += 1024) {
+        const u32 g = g0 + tid;
+        const u32 c = g < ng ? gclass[g] : 0xffffffffu;
+        s_cls[tid] = c;
+        __syncthreads();
+        if (g < ng) {
+            u32 r = 0;
+            for (u32 t = 0; t < tid; ++t) r += s_cls[t] == c ? 1u : 0u;
+            order[s_base[c] + s_cur[c] + r] = g;
+        }
+        __syncthreads();
+        if (g < ng) atomicAdd(&s_cur[c], 1u);     // counts only: the order of these additions does not matter
+        __syncthreads();
+    }
+    if (tid == 0) order_meta[0] = ng;
+}
+
+// records of a sharded evaluation for ONE all-reduce (sum) over the ranks: (ax, ay, az, phi, cost class + 1) per particle
+// in user order, all zero for the particles of the groups other ranks walked
+__global__ void __launch_bounds__(256) shard_record_kernel(const float4 *__restrict__ accpot, const u32 *__restrict__ body_class,
+                                                           float *__restrict__ rec, u32 n)
+{
+    const u32 i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const float4 a = accpot[i];
+    const u32 c = body_class[i];
+    float *r = rec + 5 * (size_t)i;
+    r[0] = a.x; r[1] = a.y; r[2] = a.z; r[3] = a.w;
+    r[4] = c == 0xffffffffu ? 0.f : (float)(c + 1u);
+}
+__global__ void __launch_bounds__(256) shard_classes_kernel(const float *__restrict__ rec, u32 *__restrict__ body_class, u32 n)
+{
+    const u32 i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const float v = rec[5 * (size_t)i + 4];
+    body_class[i] = v >= 0.5f ? min((u32)(v - 0.5f), (u32)ORDER_CLASSES - 1u) : (u32)ORDER_CLASSES - 1u;
+}
+p3t_status p3t_stage_shard_record(p3t_ctx *ctx, float *d_rec)
+{
+    shard_record_kernel<<<div_up(ctx->n, 256), 256, 0, ctx->stream>>>(ctx->ws.accpot, ctx->ws.body_class, d_rec, (u32)ctx->n);
+    P3T_CUDA(ctx, cudaGetLastError());
+    return P3T_OK;
+}
+p3t_status p3t_stage_shard_classes(p3t_ctx *ctx, const float *d_rec)
+{
+    shard_classes_kernel<<<div_up(ctx->n, 256), 256, 0, ctx->stream>>>(d_rec, ctx->ws.body_class, (u32)ctx->n);
+    P3T_CUDA(ctx, cudaGetLastError());
+    return P3T_OK;
+}
+
 #ifdef P3T_WALK_PROFILE
 extern "C" void p3t_debug_wprof(unsigned long long *out)
 {
@@ -928,12 +995,22 @@ p3t_status p3t_stage_walk(p3t_ctx *ctx)
         P3T_CUDA(ctx, cudaMemsetAsync(w.nbr_count, 0, ctx->n * sizeof(u32), s));
     }
     // hand-out order of this call's groups from the classes the previous call left per body (the group count lives on
-    // the device: launch for its upper bound n / 1 .. n groups; a sharded walk keeps Morton order)
-    if (ctx->shard_world == 1) {
+    // the device).  A sharded walk orders its groups only if the ranks have exchanged their classes since the last walk
+    // (then all ranks hold the same classes, and the atomic-free order kernel gives all of them the same order); it then
+    // marks every body "not mine" so that the next exchange can tell whose class is whose.
+    A.use_order = (ctx->shard_world == 1 || ctx->shard_classes_fresh) ? 1u : 0u;
+    if (A.use_order) {
         const u32 ogrid = min(div_up(ctx->n, 256 * 32), (u32)ctx->sm_count * 4);     // about n / 50 groups: a few per thread
         group_predict_kernel<<<ogrid, 256, 0, s>>>(w.group_start, w.idx[ctx->cur], w.body_class, w.counters, w.group_class, w.order_hist);
-        group_order_kernel<<<ogrid, 256, 0, s>>>(w.group_class, w.order_hist, w.order_hist + ORDER_CLASSES, w.counters,
-                                                              w.group_order, w.order_meta);
+        if (ctx->shard_world == 1)
+            group_order_kernel<<<ogrid, 256, 0, s>>>(w.group_class, w.order_hist, w.order_hist + ORDER_CLASSES, w.counters,
+                                                                  w.group_order, w.order_meta);
+        else
+            group_order_det_kernel<<<1, 1024, 0, s>>>(w.group_class, w.order_hist, w.counters, w.group_order, w.order_meta);
+    }
+    if (ctx->shard_world > 1) {
+        P3T_CUDA(ctx, cudaMemsetAsync(w.body_class, 0xff, ctx->n * sizeof(u32), s));
+        ctx->shard_classes_fresh = false;
     }
     // one CTA per group when there are too few groups to keep every warp busy to the end of the launch
     // (the group count lives on the device; n / ngroup is its lower bound up to the fill of the groups)

@@ -65,6 +65,58 @@ def merge_csr(parts, n):
     return offset.astype(np.uint64), nbr
 
 
+def allreduce_shard(dist, ctx, rec=None):
+    """The exchange of one sharded evaluation: ONE all-reduce (sum) of the records (a, phi, cost class + 1) of all
+    particles (20 bytes per particle over NVLink with NCCL; `rec` may be a caller-owned [n, 5] float32 tensor), after
+    which every rank holds the accelerations and potentials of all particles and hands the summed cost classes back to
+    its context, so that the next sharded walk deals the groups out by predicted cost, the same way on every rank
+    (include/p3t.h p3t_get_shard_record / p3t_put_shard_classes).  `ctx` needs get_shard_record(rec) and
+    put_shard_classes(rec).  Returns (acc [n, 3], pot [n]) as views of the record."""
+    rec = ctx.get_shard_record(rec)
+    if dist is not None and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(rec, op=dist.ReduceOp.SUM)
+    ctx.put_shard_classes(rec)
+    r = rec.view(-1, 5)
+    return r[:, :3], r[:, 3]
+
+
+def allgather_csr_tensors(dist, count, nbr):
+    """Neighbour lists of all ranks on every rank, as tensors (NCCL with device tensors, gloo with CPU tensors; nothing
+    is pickled).  count [n] int64 and nbr [total_r] int64/int32: this rank's list lengths (zero for the particles other
+    ranks produced) and entries, lists in particle order.  Two collectives: an all-reduce of the lengths (every list has
+    one owner, so the sum is the global length) and an all-gather of the entries padded to the longest rank; every rank
+    then places the entries of rank r's particle i behind the global offset of i.
+    Returns (offset [n + 1] int64, nbr [total] of nbr's dtype)."""
+    import torch
+
+    n = count.shape[0]
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        off = torch.zeros(n + 1, dtype=torch.int64, device=count.device)
+        off[1:] = torch.cumsum(count, 0)
+        return off, nbr
+    world = dist.get_world_size()
+    counts = [torch.empty_like(count) for _ in range(world)]
+    dist.all_gather(counts, count.contiguous())
+    total = torch.stack(counts).sum(0)
+    off = torch.zeros(n + 1, dtype=torch.int64, device=count.device)
+    off[1:] = torch.cumsum(total, 0)
+    lens = torch.stack([c.sum() for c in counts])
+    pad = int(lens.max().item())
+    mine = torch.zeros(max(pad, 1), dtype=nbr.dtype, device=nbr.device)
+    mine[: nbr.shape[0]] = nbr
+    parts = [torch.empty_like(mine) for _ in range(world)]
+    dist.all_gather(parts, mine)
+    out = torch.empty(int(off[-1].item()), dtype=nbr.dtype, device=nbr.device)
+    for c, part in zip(counts, parts):
+        t = int(c.sum().item())
+        if t == 0:
+            continue
+        local_off = torch.cumsum(c, 0) - c
+        dst = torch.repeat_interleave(off[:-1] - local_off, c) + torch.arange(t, dtype=torch.int64, device=c.device)
+        out[dst] = part[:t]
+    return off, out
+
+
 def allreduce_forces(dist, acc, pot):
     """In-place sum over ranks of the torch tensors acc, pot (device tensors with NCCL, CPU tensors with gloo)."""
     if dist is not None and dist.is_initialized() and dist.get_world_size() > 1:

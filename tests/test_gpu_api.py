@@ -273,3 +273,53 @@ def test_sharded_evaluations_add_up_to_the_whole(world, mode):
             assert np.abs(p / p_full - 1).max() <= 2e-6
         with pytest.raises(b.P3TError):
             ctx.set_shard(2, 2)
+
+
+def test_sharded_walks_with_exchanged_cost_classes_deal_the_same_order_to_every_rank():
+    """p3t_get_shard_record / p3t_put_shard_classes: after the ranks (here: three contexts on this GPU, one after the
+    other) have summed their records, every context holds every particle's cost class, orders the groups alike
+    (atomic-free order kernel) and takes every third position of that order: each group has exactly one owner, the union
+    is bitwise the unsharded result, and each rank's groups are a fair share of the predicted cost."""
+    import torch
+    from paper_1506_04553_b200 import multi
+
+    b = _binding()
+    cfg = workloads.config(3, n=60000)
+    n, world = cfg["n"], 3
+    with b.P3T(n, key_bits=63, nbr_capacity=64 * n) as full:
+        full.set_walk_mode(1)
+        full.set_params(cfg["eps"], cfg["theta"], cfg["r_in"], 10 * cfg["r_out"], 12 * cfg["r_out"])
+        full.soft_force(cfg["mass"], cfg["pos"])
+        a_full, p_full = full.get_acc_pot()
+        o_full, l_full = full.get_neighbours()
+        gstats = full.array("group_stats")
+    ctxs = []
+    for r in range(world):
+        c = b.P3T(n, key_bits=63, nbr_capacity=64 * n)
+        c.set_walk_mode(1)
+        c.set_params(cfg["eps"], cfg["theta"], cfg["r_in"], 10 * cfg["r_out"], 12 * cfg["r_out"])
+        c.set_shard(r, world)
+        ctxs.append(c)
+    for call in range(3):
+        recs = []
+        for c in ctxs:
+            c.soft_force(cfg["mass"], cfg["pos"])
+            recs.append(c.get_shard_record())
+        total = torch.stack(recs).sum(0)
+        owners = torch.stack([(r[:, 4] > 0).to(torch.int32) for r in recs]).sum(0)
+        assert bool((owners == 1).all())                                   # every particle produced by exactly one rank
+        acc, pot = total[:, :3].cpu().numpy(), total[:, 3].cpu().numpy()
+        assert np.array_equal(acc, a_full) and np.array_equal(pot, p_full)
+        off, nbr = multi.merge_csr([c.get_neighbours() for c in ctxs], n)
+        assert np.array_equal(off, o_full) and np.array_equal(nbr, l_full)
+        if call > 0:      # the walks of this call used the order made from the exchanged classes
+            orders = [c.array("group_order") for c in ctxs]
+            assert all(np.array_equal(orders[0], o) for o in orders[1:])
+            cost = 13.0 * gstats[:, 0] + 33.0 * gstats[:, 1]
+            by_rank = [cost[orders[0][r::world]].sum() for r in range(world)]
+            assert max(by_rank) <= 1.02 * min(by_rank), by_rank              # positions of a cost-sorted order, dealt round robin
+            assert cost[orders[0][:50]].mean() > 3 * cost[orders[0][-50:]].mean()   # longest first
+        for c in ctxs:
+            c.put_shard_classes(total)
+    for c in ctxs:
+        c.close()
