@@ -165,6 +165,7 @@ def main():
     ap.add_argument("--n", type=int, default=None, help="override the particle count (not a bench value)")
     ap.add_argument("--same-positions", action="store_true", help="do not move the bodies between steps (not the headline case)")
     ap.add_argument("--settle", type=float, default=1.2, help="seconds of untimed steps before the warm-up (clock sampler)")
+    ap.add_argument("--dt-soft", type=float, default=None, help="soft step of the drift between timed steps (default: the config's, else 1/1024)")
     ap.add_argument("--refit", type=int, default=0, help="tree reuse: p3t_refit_tree with a rebuild every REFIT calls (not the headline case)")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -230,7 +231,7 @@ def main():
     # Between steps the bodies move by one leapfrog step with the returned forces (BASELINE.json configs[1] asks for it
     # in so many words: "positions are drifted by a leapfrog step dt_soft using the returned forces"; for the other
     # configs it makes the timed case the one an integration sees).  Torch ops on the device, outside the event window.
-    dt_soft = cfg.get("dt_soft") or 1.0 / 1024.0
+    dt_soft = args.dt_soft or cfg.get("dt_soft") or 1.0 / 1024.0
     drift = not shard and not args.same_positions
     vel_l = torch.from_numpy(cfg["vel"]).to(dev)
     pos_d = pos_d.clone()
@@ -428,6 +429,7 @@ def main():
         "roofline_hbm": {"bound": "hbm", "passes": "a1-a6 (sort, build, moments)", "achieved": sum(ab.values()) / (tree_ms * 1e-3) / 1e9,
                          "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": sum(ab.values()) / (tree_ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
                          "per_pass_gbs": hbm, "algorithmic_bytes": ab, "peak_source": peaks["source"]},
+        "tree_reuse": ({"max_refits": args.refit, "tree_refits_at_end": st["tree_refits"], "n_stray": st["n_stray"]} if args.refit else None),
         "clocks": clocks, "gpu_launches": launches * args.steps, "gpu_launches_per_step": launches,
     }
     if hard:
