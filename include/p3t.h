@@ -152,8 +152,12 @@ p3t_status p3t_set_group_merge_levels(p3t_ctx *ctx, int levels);
  * reproducible.  2: the four warps of a CTA share one group through a common stack -- keeps the GPU busy
  * when there are few groups (small n) and shortens the tail of the launch; which warp evaluates which
  * cell depends on timing, so accelerations and potentials are reproducible to fp32 rounding of the
- * batch sums (a few 1e-6 relative at most) rather than bitwise; neighbour lists are identical.  0 (default):
- * chosen from n (mode 2 below about 0.65 groups per resident warp).  P3T_EINVAL for another value. */
+ * batch sums (a few 1e-6 relative at most) rather than bitwise; neighbour lists are identical.  3, 4: split walk -- 2 or 4
+ * warps per group, each walking every 2nd / 4th cell of one tree level and everything below it, their sums added in a
+ * fixed order by a small kernel (bitwise reproducible; sums differ from mode 1's by the rounding of the partial sums):
+ * for mid-size n, where all groups start at once and the launch would end in a long tail of lone warps.  0 (default):
+ * chosen from n / ngroup per resident warp (mode 2 below 0.3, mode 4 below 0.65, mode 3 below 1.3, else mode 1).
+ * P3T_EINVAL for another value. */
 p3t_status p3t_set_walk_mode(p3t_ctx *ctx, int mode);
 
 /* Sharding of one evaluation over `world` GPUs: every rank loads ALL particles and builds the

@@ -375,7 +375,7 @@ extern "C" p3t_status p3t_set_hermite_cluster_max(p3t_ctx *ctx, int max_members)
 
 extern "C" p3t_status p3t_set_walk_mode(p3t_ctx *ctx, int mode)
 {
-    if (!ctx || mode < 0 || mode > 2) return P3T_EINVAL;
+    if (!ctx || mode < 0 || mode > 4) return P3T_EINVAL;
     ctx->walk_mode = mode;
     ctx->evaluated = false;
     return P3T_OK;

@@ -34,9 +34,16 @@ typedef unsigned char u8;
 #define WALK_STACK_SMEM 512          // stack entries per warp held in shared memory
 #endif
 #define WALK_STACK_GMEM 7168         // overflow entries per warp in global memory
+#ifndef WALK_SPLIT_BELOW_X20
+#define WALK_SPLIT_BELOW_X20 26        // auto mode: split walk below 26 / 20 = 1.3 groups (n / ngroup) per resident warp: 2 parts, 4 below 0.65
+#endif
+#ifndef WALK_SPLIT_CELLS
+#define WALK_SPLIT_CELLS 512           // split level: the first tree level with at least this many cells per part
+#endif
 #ifndef WALK_COOP_BELOW_X20
-#define WALK_COOP_BELOW_X20 13         // auto mode: one CTA per group below 13 / 20 groups per resident warp (measured crossover:
-                                      // n = 100K for groups of 64, 45K for groups of 32, on 2368 resident warps)
+#define WALK_COOP_BELOW_X20 6          // auto mode: one CTA per group below 6 / 20 = 0.3 groups (n / ngroup) per resident warp; between
+                                      // that and 1.3 a split walk (measured, 2368 resident warps, groups of 64: 32K coop 0.36 ms against
+                                      // 0.56 split; 64K split x 4 0.56 against coop 0.62; 96K split x 2 0.79 against coop 0.89)
 #endif
 
 // Parameters handed to kernels by value.  The coefficients of W are prepared on the host in

@@ -52,6 +52,7 @@ struct WarpShared {
     // step: their latency is hidden behind the interaction batches of the current step
     float4 l_mac[32], l_mom0[32], l_mom1[32];
     uint2 l_meta[32];
+    u32 l_cell[32];     // their indices (written and read by a split walk only)
 };
 
 __device__ __forceinline__ void cp_async16(void *smem, const void *gmem)
@@ -387,13 +388,24 @@ struct WalkArgs {
     const u8 *__restrict__ cls_sorted;   // pair classes (walk_kernel<.., .., true> only)
     const float *__restrict__ cube;
     u32 n;                               // bodies (checked builds test indices against it)
+    // split walk (mid-size n: about as many groups as warps, so that all of them start at once and the launch ends in a
+    // long tail of lone warps): every group is walked by `nparts` warps, each taking every nparts-th cell of one tree
+    // level (and everything below those); what is accepted or is a leaf above that level is dealt out likewise.  Parts 1..
+    // write their sums to split_acc / split_cnt, a small kernel adds them in fixed order.
+    u32 nparts;                          // 1, 2 or 4
+    const u32 *__restrict__ level_total; // cells per level (build.cu)
+    float4 *__restrict__ split_acc;      // [nparts - 1][n]
+    u32 *__restrict__ split_cnt;         // [nparts - 1][n]
 };
+struct SplitRule { u32 part, nparts, lo, hi; };   // this warp's part; cell indices [lo, hi) of the split level
 
 // starts the asynchronous copy of the records of the popped cells into the landing area
+template <bool SPLIT = false>
 __device__ __forceinline__ void request_cells(WarpShared &ws, const WalkArgs &A, u32 take, u32 lane, u32 cell)
 {
     if (lane < take) {
         P3T_DEV_ASSERT((u64)cell < A.counters[CNT_NCELLS]);
+        if (SPLIT) ws.l_cell[lane] = cell;
         cp_async16(&ws.l_mac[lane], &A.cell_mac[cell]);
         cp_async8(&ws.l_meta[lane], &A.cell_meta[cell]);
         cp_async16(&ws.l_mom0[lane], &A.cell_mom0[cell]);
@@ -402,12 +414,13 @@ __device__ __forceinline__ void request_cells(WarpShared &ws, const WalkArgs &A,
     cp_async_commit();
 }
 // pops up to 32 cells of a warp-private stack
+template <bool SPLIT = false>
 __device__ __forceinline__ u32 pop_cells(WarpShared &ws, const StackRef &st, const WalkArgs &A, u32 &top, u32 lane)
 {
     const u32 take = min(32u, top);
     top -= take;
     const u32 cell = lane < take ? stack_read(st, top + lane) : 0u;
-    request_cells(ws, A, take, lane, cell);
+    request_cells<SPLIT>(ws, A, take, lane, cell);
     return take;
 }
 // cooperative mode: a warp without cells takes up to 32 from the shared stack; waits while other warps may
@@ -452,10 +465,10 @@ __device__ __forceinline__ u32 coop_acquire(WarpShared &ws, const StackRef &st, 
 // open (cells were given their radius for field-star groups: h, or h_bf if the cell itself holds a black hole) and never
 // accepts a cell that holds a black hole (BH-BH pairs are not split); bodies go to the K/W path when they are within
 // the neighbour radius of the kinds of pairs they can form with the group, black holes met by such a group always.
-template <int NI, bool COOP, bool CLS>
+template <int NI, bool COOP, bool CLS, bool SPLIT>
 __device__ __forceinline__ void walk_group(WarpShared *wsall, const StackRef &st, CtaCtl *ctl, const WalkArgs &A,
                                            const P3TParams &prm, u32 gs, u32 ge, u32 lane, u32 warp, u64 &tot_pp, u64 &tot_pc,
-                                           u64 &tot_near)
+                                           u64 &tot_near, const SplitRule &sr, u32 &len_pp, u32 &len_pc)
 {
     WarpShared &ws = wsall[warp];
     const u32 gcount = ge - gs;
@@ -506,14 +519,14 @@ __device__ __forceinline__ void walk_group(WarpShared *wsall, const StackRef &st
     u32 n_far = 0, n_near = 0, n_pc = 0;
     bool overflow = false;
     __syncwarp();
-    u32 take = COOP ? coop_acquire(ws, st, ctl, A, lane) : pop_cells(ws, st, A, top, lane);
+    u32 take = COOP ? coop_acquire(ws, st, ctl, A, lane) : pop_cells<SPLIT>(ws, st, A, top, lane);
     while (take > 0) {
         const bool have = lane < take;
         WP(8);
         cp_async_wait_all();
         WP(2); WPC(10);
         // ---- consume the landed records: acceptance test (R-MAC, folded radius of moments.cu)
-        bool accept = false;
+        bool accept = false, skip = false;
         u32 nch = 0, first = 0, lcount = 0, lstart = 0;
         float4 a = make_float4(0.f, 0.f, 0.f, 0.f);
         if (have) {
@@ -523,12 +536,21 @@ __device__ __forceinline__ void walk_group(WarpShared *wsall, const StackRef &st
             float ez = fmaxf(0.f, fmaxf(lo[2] - a.z, a.z - hi[2]));
             float d2 = fmaf(ex, ex, fmaf(ey, ey, ez * ez));
             accept = d2 > a.w;
+            if (SPLIT) {      // is this cell mine?
+                const u32 c = ws.l_cell[lane];
+                if (c >= sr.lo) {
+                    if (c < sr.hi && ((c - sr.lo) & (sr.nparts - 1u)) != sr.part) { skip = true; accept = false; }
+                } else if ((c & (sr.nparts - 1u)) != sr.part) {      // above the split level all parts meet the cell: what is
+                    skip = accept || (ws.l_meta[lane].y & P3T_LEAF_FLAG) != 0;   // accepted or a leaf there goes to one of them
+                    accept = false;
+                }
+            }
             if (CLS && heavy_group && accept) {
                 const float rm = ws.l_mom1[lane].w;                       // bounding radius; sign bit: the cell holds a black hole
                 const float rc = (prm.h_bf + fabsf(rm)) * (1.f + 1e-5f) + slack;
                 accept = !(__float_as_uint(rm) >> 31) && d2 > rc * rc;
             }
-            if (!accept) {
+            if (!accept && !(SPLIT && skip)) {
                 uint2 meta = ws.l_meta[lane];
                 if (meta.y & P3T_LEAF_FLAG) { lstart = meta.x; lcount = meta.y & ~P3T_LEAF_FLAG; P3T_DEV_ASSERT(lcount >= 1 && lstart + lcount <= A.n); }
                 else { first = meta.x; nch = meta.y; P3T_DEV_ASSERT(nch >= 1 && nch <= 8 && (u64)first + nch <= A.counters[CNT_NCELLS]); }
@@ -564,7 +586,7 @@ __device__ __forceinline__ void walk_group(WarpShared *wsall, const StackRef &st
                 top += total;
                 __syncwarp();
                 // ---- request the records of the next step before any interaction work
-                take = top > 0 ? pop_cells(ws, st, A, top, lane) : 0u;
+                take = top > 0 ? pop_cells<SPLIT>(ws, st, A, top, lane) : 0u;
             } else {
                 // one critical section: push the children, take the next 32 cells (mostly my own children)
                 u32 base = 0;
@@ -721,13 +743,16 @@ __device__ __forceinline__ void walk_group(WarpShared *wsall, const StackRef &st
             }
         }
     }
-    // ---- results, user order
+    // ---- results, user order (split walk: parts 1.. to their own arrays)
     if (!COOP || warp == 0) {
+        float4 *out = A.accpot;
+        u32 *cnt = A.nbr_count;
+        if (SPLIT && sr.part) { out = A.split_acc + (size_t)(sr.part - 1u) * A.n; cnt = A.split_cnt + (size_t)(sr.part - 1u) * A.n; }
 #pragma unroll
     for (int b = 0; b < NI; ++b) {
         if (isorted[b] != 0xffffffffu) {
-            A.accpot[iuser[b]] = make_float4((float)acc.dax[b], (float)acc.day[b], (float)acc.daz[b], (float)(-acc.dph[b]));
-            A.nbr_count[iuser[b]] = nnb[b];
+            out[iuser[b]] = make_float4((float)acc.dax[b], (float)acc.day[b], (float)acc.daz[b], (float)(-acc.dph[b]));
+            cnt[iuser[b]] = nnb[b];
         }
     }
     }
@@ -736,18 +761,38 @@ __device__ __forceinline__ void walk_group(WarpShared *wsall, const StackRef &st
     WP(7);
     if (lane == 0) for (int k_ = 0; k_ < WP_SLOTS; ++k_) atomicAdd(&g_wprof[k_], (unsigned long long)wp_acc[k_]);
 #endif
-    // each live body met itself once on the near path (distance 0 to its own group's box)
-    const u64 self = (!COOP || warp == 0) ? gcount : 0;   // counted once per group (u64 arithmetic wraps harmlessly)
+    // each live body met itself once on the near path (distance 0 to its own group's box): removed once per group, by
+    // warp 0 / part 0 (the per-warp totals are u64 and wrap harmlessly; their sum is right)
+    const u64 self = (COOP ? warp == 0 : (!SPLIT || sr.part == 0)) ? gcount : 0;
     tot_pp += (u64)(n_far + n_near) * gcount - self;
     tot_near += (u64)n_near * gcount - self;
     tot_pc += (u64)n_pc * gcount;
+    len_pp = n_far + n_near; len_pc = n_pc;
+}
+
+// split walk: accpot += the sums of parts 1.., nbr_count likewise, in fixed order (deterministic)
+__global__ void __launch_bounds__(256) split_combine_kernel(float4 *__restrict__ accpot, u32 *__restrict__ nbr_count,
+                                                            const float4 *__restrict__ split_acc, const u32 *__restrict__ split_cnt,
+                                                            u32 n, u32 nparts)
+{
+    const u32 i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    float4 a = accpot[i];
+    u32 c = nbr_count[i];
+    for (u32 p = 0; p + 1 < nparts; ++p) {
+        const float4 b = split_acc[(size_t)p * n + i];
+        a.x += b.x; a.y += b.y; a.z += b.z; a.w += b.w;
+        c += split_cnt[(size_t)p * n + i];
+    }
+    accpot[i] = a;
+    nbr_count[i] = c;
 }
 
 // Persistent grid: 148 SMs x 4 CTAs x 4 warps; groups are handed out by an atomic ticket, one per warp
 // (COOP = false) or one per CTA (COOP = true).  A group of at most 32 bodies takes the one-body-per-lane
 // path (half the FP32 work of the packed path).
 // Shared memory: WALK_WARPS x WarpShared | WALK_WARPS x WALK_STACK_SMEM stack words | CtaCtl
-template <int NIMAX, bool COOP, bool CLS>
+template <int NIMAX, bool COOP, bool CLS, bool SPLIT = false>
 __global__ void __launch_bounds__(WALK_WARPS * 32, WALK_CTAS)
 walk_kernel(WalkArgs A, const u32 *__restrict__ group_start, P3TParams prm, u32 *walk_stack)
 {
@@ -775,6 +820,18 @@ walk_kernel(WalkArgs A, const u32 *__restrict__ group_start, P3TParams prm, u32 
     const u32 ng_prev = A.use_order ? A.order_meta[0] : 0u;
     const u32 npos = max(ngroups, ng_prev);
     u64 tot_pp = 0, tot_pc = 0, tot_near = 0;
+    // split walk: the level whose cells are dealt to the parts = the first one with at least WALK_SPLIT_CELLS cells per
+    // part (fine enough for the near field of a group to spread over all parts), or the deepest level
+    SplitRule sr = {0u, SPLIT ? A.nparts : 1u, 0u, 0u};
+    if (SPLIT) {
+        u32 lo = 0, cnt = 0;
+        for (int L = 0; L < 24; ++L) {
+            cnt = A.level_total[L];
+            if (cnt >= (u32)WALK_SPLIT_CELLS * sr.nparts || (L < 23 && A.level_total[L + 1] == 0)) break;
+            lo += cnt;
+        }
+        sr.lo = lo; sr.hi = lo + cnt;
+    }
 
     while (true) {
         u32 g = 0;
@@ -791,6 +848,7 @@ walk_kernel(WalkArgs A, const u32 *__restrict__ group_start, P3TParams prm, u32 
             g = __shfl_sync(0xffffffffu, g, 0);
         }
         g = g * A.shard_world + A.shard_rank;   // (overflow-free: tickets stop at npos / world)
+        if (SPLIT) { sr.part = g & (sr.nparts - 1u); g /= sr.nparts; }   // the parts of a group: consecutive tickets
         if (g >= npos) break;
         if (g < ng_prev) g = A.group_order[g];
         if (g >= ngroups) {                      // a group of the previous call that is gone
@@ -799,10 +857,10 @@ walk_kernel(WalkArgs A, const u32 *__restrict__ group_start, P3TParams prm, u32 
         }
         const u32 gs = group_start[g], ge = group_start[g + 1];
         P3T_DEV_ASSERT(gs < ge && ge <= A.n && ge - gs <= 32u * NIMAX);
-        const u64 pp0 = tot_pp, pc0 = tot_pc;
         const u32 t0 = (u32)globaltimer_ns();
-        if (NIMAX == 2 && ge - gs > 32) walk_group<2, COOP, CLS>(wsall, st, ctl, A, prm, gs, ge, lane, warp, tot_pp, tot_pc, tot_near);
-        else walk_group<1, COOP, CLS>(wsall, st, ctl, A, prm, gs, ge, lane, warp, tot_pp, tot_pc, tot_near);
+        u32 len_pp = 0, len_pc = 0;
+        if (NIMAX == 2 && ge - gs > 32) walk_group<2, COOP, CLS, SPLIT>(wsall, st, ctl, A, prm, gs, ge, lane, warp, tot_pp, tot_pc, tot_near, sr, len_pp, len_pc);
+        else walk_group<1, COOP, CLS, SPLIT>(wsall, st, ctl, A, prm, gs, ge, lane, warp, tot_pp, tot_pc, tot_near, sr, len_pp, len_pc);
         __syncwarp();
         // diagnostics: list lengths of this group (+1: the self term removed from tot_pp) and its time window
         if (COOP) {
@@ -812,10 +870,11 @@ walk_kernel(WalkArgs A, const u32 *__restrict__ group_start, P3TParams prm, u32 
             }
             __syncthreads();   // ctl is rewritten for the next group (cls only at the end of that group)
             for (u32 bb = gs + threadIdx.x; bb < ge; bb += blockDim.x) A.body_class[A.sorted_idx[bb]] = ctl->cls;
-        } else {
+        } else if (!SPLIT || sr.part == 0) {
+            // (a split walk files the group under nparts x part 0's list lengths: the parts take alike shares)
             u32 c = 0;
             if (lane == 0) {
-                const u32 lpp = (u32)((tot_pp - pp0) / (ge - gs)) + 1u, lpc = (u32)((tot_pc - pc0) / (ge - gs));
+                const u32 lpp = len_pp * sr.nparts, lpc = len_pc * sr.nparts;
                 A.group_stats[g] = make_uint4(lpp, lpc, t0, (u32)globaltimer_ns());
                 c = cost_class(lpp, lpc, ge - gs > 32);
             }
@@ -970,10 +1029,12 @@ p3t_status p3t_stage_walk(p3t_ctx *ctx)
     if ((size_t)grid * WALK_WARPS > w.walk_warps_max) grid = (u32)(w.walk_warps_max / WALK_WARPS);
     const size_t smem = (sizeof(WarpShared) + WALK_STACK_SMEM * sizeof(u32)) * WALK_WARPS + sizeof(CtaCtl);
     typedef void (*walk_fn)(WalkArgs, const u32 *, P3TParams, u32 *);
-    static const walk_fn fns[8] = {walk_kernel<1, false, false>, walk_kernel<2, false, false>, walk_kernel<1, true, false>, walk_kernel<2, true, false>,
-                                   walk_kernel<1, false, true>,  walk_kernel<2, false, true>,  walk_kernel<1, true, true>,  walk_kernel<2, true, true>};
+    static const walk_fn fns[12] = {walk_kernel<1, false, false>, walk_kernel<2, false, false>, walk_kernel<1, true, false>, walk_kernel<2, true, false>,
+                                    walk_kernel<1, false, true>,  walk_kernel<2, false, true>,  walk_kernel<1, true, true>,  walk_kernel<2, true, true>,
+                                    walk_kernel<1, false, false, true>, walk_kernel<2, false, false, true>,      // split walk
+                                    walk_kernel<1, false, true, true>,  walk_kernel<2, false, true, true>};
     if (!ctx->walk_attr_set) {   // function attributes are per device: kept per context
-        for (int k = 0; k < 8; ++k) P3T_CUDA(ctx, cudaFuncSetAttribute(fns[k], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        for (int k = 0; k < 12; ++k) P3T_CUDA(ctx, cudaFuncSetAttribute(fns[k], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         ctx->walk_attr_set = true;
     }
     WalkArgs A;
@@ -1015,8 +1076,24 @@ p3t_status p3t_stage_walk(p3t_ctx *ctx)
     // one CTA per group when there are too few groups to keep every warp busy to the end of the launch
     // (the group count lives on the device; n / ngroup is its lower bound up to the fill of the groups)
     bool coop = ctx->walk_mode == 2 || (ctx->walk_mode == 0 && 20 * (ctx->n / (size_t)ctx->ngroup) < (size_t)WALK_COOP_BELOW_X20 * grid * WALK_WARPS);
+    // split walk (modes 3, 4: 2 or 4 warps per group; auto: 2 below 1.3 groups per resident warp, 4 below 0.65), so that
+    // the hand-out has about two items per warp to balance with
+    u32 nparts = ctx->walk_mode == 3 ? 2u : ctx->walk_mode == 4 ? 4u : 1u;
+    if (ctx->walk_mode == 0 && !coop) {
+        const size_t groups = ctx->n / (size_t)ctx->ngroup, warps = (size_t)grid * WALK_WARPS;
+        nparts = 20 * groups >= WALK_SPLIT_BELOW_X20 * warps ? 1u : 40 * groups >= WALK_SPLIT_BELOW_X20 * warps ? 2u : 4u;
+    }
+    if (ctx->shard_world > 1 || coop) nparts = 1;
+    A.nparts = nparts;
+    A.level_total = w.level_total;
+    A.split_acc = reinterpret_cast<float4 *>(w.hard_out);          // 48 n bytes of the 56 n (free until p3t_eval_hard)
+    A.split_cnt = reinterpret_cast<u32 *>(w.herm_state);           // 12 n bytes of 96 n (free until p3t_hermite_step)
     const dim3 block(WALK_WARPS * 32);
-    fns[(ctx->ngroup == 64 ? 1 : 0) + (coop ? 2 : 0) + (ctx->cls_n ? 4 : 0)]<<<grid, block, smem, s>>>(A, w.group_start, ctx->prm, w.walk_stack);
+    const int fi = nparts > 1 ? 8 + (ctx->ngroup == 64 ? 1 : 0) + (ctx->cls_n ? 2 : 0)
+                              : (ctx->ngroup == 64 ? 1 : 0) + (coop ? 2 : 0) + (ctx->cls_n ? 4 : 0);
+    fns[fi]<<<grid, block, smem, s>>>(A, w.group_start, ctx->prm, w.walk_stack);
+    if (nparts > 1)
+        split_combine_kernel<<<div_up(ctx->n, 256), 256, 0, s>>>(w.accpot, w.nbr_count, A.split_acc, A.split_cnt, (u32)ctx->n, nparts);
     P3T_CUDA(ctx, cudaGetLastError());
     return P3T_OK;
 }

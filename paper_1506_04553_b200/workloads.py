@@ -215,8 +215,9 @@ def config(k, n=None, seed_offset=0):
     if k != 6:
         pos, vel = _recentre(mass, pos, vel)
     prm["r_in"] = 0.1 * prm["r_out"]      # gamma = 0.1 in all runs (Table 1)
-    # i-groups of 32 below ~100K particles (more, lighter groups fill the GPU better and their boxes are smaller), 64 above
-    prm.update(nleaf=16, ngroup=32 if n < 100000 else 64, n=n, config=k)
+    # i-groups of 32 below 40K particles (more, lighter groups fill the GPU better), 64 above (two bodies per lane: the
+    # packed path; the walk splits a group over 2 or 4 warps where there are fewer groups than warps)
+    prm.update(nleaf=16, ngroup=32 if n < 40000 else 64, n=n, config=k)
     # fp32 parameters: what the C ABI receives; the oracle gets these same values
     for key in ("eps", "theta", "r_in", "r_out", "r_search"):
         prm[key] = float(np.float32(prm[key]))

@@ -112,6 +112,8 @@ CASES = {
     "soft30_g32_coop_stress": lambda: soft(4096, 30, 32, 2, True),
     "soft63_g32_warp_stress_ragged": lambda: soft(4099, 63, 32, 1, True, nleaf=8),
     "soft63_auto_tiny": lambda: soft(37, 63, 64, 0, True),
+    "soft63_g64_split4_stress": lambda: soft(4096, 63, 64, 4, True),
+    "soft30_g32_split2": lambda: soft(4099, 30, 32, 3, False),
     "direct_and_hard": lambda: direct_and_hard(4096),
     "hermite_warp": lambda: hermite(4096, None, 0.01),
     "hermite_cluster": lambda: hermite(4096, 4096, 0.08),

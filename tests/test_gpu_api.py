@@ -153,28 +153,33 @@ def test_results_are_deterministic_and_context_reusable():
         assert np.array_equal(a0, a2) and np.array_equal(p0, p2) and np.array_equal(o0, o2) and np.array_equal(n0, n2)
 
 
-@pytest.mark.parametrize("n", [777, 20011])
-def test_cooperative_walk_matches_one_warp_per_group(n):
-    """p3t_set_walk_mode: the CTA-per-group walk evaluates the same interactions (counts, neighbour lists
-    identical); sums differ only by the fp32 rounding of differently composed batches."""
+@pytest.mark.parametrize("n", [777, 20011, 150000])
+def test_cooperative_and_split_walks_match_one_warp_per_group(n):
+    """p3t_set_walk_mode: the CTA-per-group walk and the split walks (2 or 4 warps per group, each taking every 2nd /
+    4th cell of one tree level) evaluate the same interactions (counts, neighbour lists identical); sums differ only by
+    the fp32 rounding of differently composed batches."""
     b = _binding()
     cfg = workloads.config(1, n=n)
     with b.P3T(n, key_bits=63, nbr_capacity=256 * n) as ctx:
         ctx.set_params(cfg["eps"], cfg["theta"], cfg["r_in"], 10 * cfg["r_out"], 12 * cfg["r_out"])
         out = {}
-        for mode in (1, 2, 0):
+        for mode in (1, 2, 3, 4, 0):
             ctx.set_walk_mode(mode)
             ctx.soft_force(cfg["mass"], cfg["pos"])
             st = ctx.get_stats()
             out[mode] = (ctx.get_acc_pot(), ctx.get_neighbours(), (st["n_pp"], st["n_pc"], st["n_near"], st["n_neighbours"]))
+            if mode in (3, 4):      # the split walk adds its parts in a fixed order: bitwise reproducible
+                ctx.soft_force(cfg["mass"], cfg["pos"])
+                a_again, p_again = ctx.get_acc_pot()
+                assert np.array_equal(a_again, out[mode][0][0]) and np.array_equal(p_again, out[mode][0][1])
         (a1, p1), (o1, l1), c1 = out[1]
-        for mode in (2, 0):
+        for mode in (2, 3, 4, 0):
             (a2, p2), (o2, l2), c2 = out[mode]
             assert c1 == c2 and np.array_equal(o1, o2) and np.array_equal(l1, l2)
             rel = np.linalg.norm(a1 - a2, axis=1) / np.linalg.norm(a1, axis=1)
             assert rel.max() <= 5e-6 and np.abs(p2 / p1 - 1).max() <= 2e-6
         with pytest.raises(b.P3TError):
-            ctx.set_walk_mode(3)
+            ctx.set_walk_mode(5)
 
 
 def test_group_order_is_a_permutation_by_decreasing_cost_and_changes_nothing():

@@ -60,7 +60,7 @@ def test_random_case_matches_oracle(oracle, case):
     nleaf = int(rng.choice([1, 2, 7, 16, 32]))
     ngroup = int(rng.choice([32, 64]))
     key_bits = int(rng.choice([30, 63]))
-    mode = 1 + case % 2
+    mode = 1 + case % 4
     m64, q64 = mass.astype(np.float64), pos.astype(np.float64)
     a, p = oracle.direct(m64, q64, float(eps), float(r_in), float(r_out))
     ooff, olst, band = oracle.neighbours(q64, float(eps), float(h))
