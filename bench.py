@@ -386,13 +386,13 @@ def main():
     peaks = measured_peaks()
     # DRAM traffic of the dominant kernel per launch: from the committed ncu --set full capture of this workload
     traffic, traffic_src = None, None
-    tp = os.path.join(ROOT, "profiles", "walk_kernel_dram_r1.csv")
+    tp = os.path.join(ROOT, "profiles", "walk_kernel_dram_r2.csv")
     if os.path.exists(tp):
         import csv
         for row in csv.DictReader(open(tp)):
             if row["workload"] == cfg["name"]:
                 traffic = int(row["dram_bytes_read"]) + int(row["dram_bytes_write"])
-                traffic_src = "profiles/walk_kernel_dram_r1.csv (ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum, per launch)"
+                traffic_src = "profiles/walk_kernel_dram_r2.csv (ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum, per launch)"
     n_sm = torch.cuda.get_device_properties(local).multi_processor_count
     fp32_peak = 2 * FP32_LANES * n_sm * peaks["sm_max_mhz"] * 1e6 / 1e12          # TFLOP/s at the max SM clock
     flops = FLOP_PP * st["n_pp"] + FLOP_PC * st["n_pc"]

@@ -323,13 +323,15 @@ __device__ __forceinline__ u32 herm_quantise(const HermConst &C, double P, doubl
 {
     const u32 kmax = 63 - __clzll((long long)C.max_ticks);
     u32 k;
-    if (!(P - P == 0.0) || !(Q - Q == 0.0)) {              // a non-finite force or jerk: reported (HERM_NONFINITE), the step is void
+    // (exponent fields first: the test for a non-finite force or jerk is then two integer compares beside the chain,
+    //  not two more fp64 operations in it -- as P - P == 0 it cost a quarter of a block step)
+    const long long bp = __double_as_longlong(P), bq = __double_as_longlong(Q);
+    const int ep = (int)((bp >> 52) & 0x7ff), eq = (int)((bq >> 52) & 0x7ff);
+    if (ep == 0x7ff || eq == 0x7ff) {                       // inf or NaN: reported (HERM_NONFINITE), the step is void
         floor_hits |= HERM_NONFINITE;
         k = kmax;
     } else if (!(Q > 0.0)) k = kmax;                       // vanishing denominator: the maximum step
     else {
-        const long long bp = __double_as_longlong(P), bq = __double_as_longlong(Q);
-        const int ep = (int)((bp >> 52) & 0x7ff), eq = (int)((bq >> 52) & 0x7ff);
         const unsigned long long mp = (unsigned long long)bp & 0xfffffffffffffull, mq = (unsigned long long)bq & 0xfffffffffffffull;
         const int L = ep - eq - (mp < mq ? 1 : 0);         // floor(log2(P / Q)) for normal numbers; P = 0 gives a large negative
         if (L >= 2 * (int)kmax) k = kmax;
@@ -431,6 +433,7 @@ struct WarpState {
 
 __global__ void __launch_bounds__(32 * HERM_WARPS) hermite_warp_kernel(HermArgs A)
 {
+    u32 err = 0;                   // HC_ERR code of this thread, filed at the end of the kernel
     __shared__ WarpState sm_all[HERM_WARPS];
     const u32 wid = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (wid >= (u32)A.ctl[HC_NSMALL]) return;
@@ -464,7 +467,7 @@ __global__ void __launch_bounds__(32 * HERM_WARPS) hermite_warp_kernel(HermArgs 
             const u32 g = A.G.nbr[k];
             u32 sidx = 0;
             while (sidx < comp.y && S.gid[sidx] != g) ++sidx;
-            if (sidx == comp.y) { herm_set_err(A.ctl, 2u); sidx = slot[q]; }   // a list that is not symmetric: reported, result unusable
+            if (sidx == comp.y) { err = max(err, 2u); sidx = slot[q]; }   // a list that is not symmetric: reported, result unusable
             A.lnbr[k] = sidx;
         }
     HermView V;
@@ -481,7 +484,7 @@ __global__ void __launch_bounds__(32 * HERM_WARPS) hermite_warp_kernel(HermArgs 
     u64 tn = warp_min_u64(next);
     u64 b = 0;
     while (tn != ~0ull) {
-        if (b >= C.max_blocks) { if (lane == 0) herm_set_err(A.ctl, 1u); break; }
+        if (b >= C.max_blocks) { err = max(err, 1u); break; }
         ++b;
         bool act[PER];
         u64 te[PER];
@@ -509,7 +512,10 @@ __global__ void __launch_bounds__(32 * HERM_WARPS) hermite_warp_kernel(HermArgs 
             }
         }
     if (steps) atomicAdd((unsigned long long *)&A.ctl[HC_STEPS], (unsigned long long)steps);
-    if (floor_hits & HERM_NONFINITE) herm_set_err(A.ctl, 3u);
+    // (error codes are kept in a register and filed once, here: an atomic on the error word inside the block loop --
+    //  executed or not -- made the warp tier's loop 1.6 times slower, 0.33 -> 0.55 ms for config 2)
+    if (floor_hits & HERM_NONFINITE) err = max(err, 3u);
+    if (err) herm_set_err(A.ctl, err);
     if (floor_hits & ~HERM_NONFINITE) atomicAdd((unsigned long long *)&A.ctl[HC_FLOOR], (unsigned long long)(floor_hits & ~HERM_NONFINITE));
     if (lane == 0) atomicMax((unsigned long long *)&A.ctl[HC_BLOCKS], (unsigned long long)b);
 }
@@ -547,6 +553,7 @@ __device__ __forceinline__ void cluster_evaluate(const HermArgs &A, const u32 *a
 // evaluate the active list one particle per thread, barrier, correct, barrier.  State in global memory (L2).
 __global__ void __cluster_dims__(HERM_CLUSTER, 1, 1) __launch_bounds__(HERM_CLUSTER_THREADS) hermite_cluster_kernel(HermArgs A)
 {
+    u32 err = 0;                   // HC_ERR code of this thread, filed at the end of the kernel
     cg::cluster_group cl = cg::this_cluster();
     const u32 c = blockIdx.x / HERM_CLUSTER;
     const uint2 comp = A.comps[A.comps_last - c];
@@ -573,7 +580,7 @@ __global__ void __cluster_dims__(HERM_CLUSTER, 1, 1) __launch_bounds__(HERM_CLUS
     for (;; ++b) {
         const u64 tn = *(volatile u64 *)&ctl[b % 3];
         if (tn == ~0ull) break;
-        if (b >= C.max_blocks) { if (tid == 0) herm_set_err(A.ctl, 1u); break; }
+        if (b >= C.max_blocks) { err = max(err, 1u); break; }
         u64 local_min = ~0ull;
         HPROF(0);
         // scan: four members per thread and round, their time words requested together
@@ -626,7 +633,10 @@ __global__ void __cluster_dims__(HERM_CLUSTER, 1, 1) __launch_bounds__(HERM_CLUS
         HPROF(6);
     }
     if (steps) atomicAdd((unsigned long long *)&A.ctl[HC_STEPS], (unsigned long long)steps);
-    if (floor_hits & HERM_NONFINITE) herm_set_err(A.ctl, 3u);
+    // (error codes are kept in a register and filed once, here: an atomic on the error word inside the block loop --
+    //  executed or not -- made the warp tier's loop 1.6 times slower, 0.33 -> 0.55 ms for config 2)
+    if (floor_hits & HERM_NONFINITE) err = max(err, 3u);
+    if (err) herm_set_err(A.ctl, err);
     if (floor_hits & ~HERM_NONFINITE) atomicAdd((unsigned long long *)&A.ctl[HC_FLOOR], (unsigned long long)(floor_hits & ~HERM_NONFINITE));
     if (tid == 0) atomicMax((unsigned long long *)&A.ctl[HC_BLOCKS], (unsigned long long)b);
 }
@@ -647,6 +657,7 @@ __device__ __forceinline__ void cta_min_to(u64 *dst, u64 v, u64 *s_min)
 
 __global__ void __launch_bounds__(HERM_THREADS) hermite_grid_kernel(HermArgs A)
 {
+    u32 err = 0;                   // HC_ERR code of this thread, filed at the end of the kernel
     __shared__ u64 s_min[HERM_THREADS / 32];
     cg::grid_group grid = cg::this_grid();
     const u32 M = A.grid_count;
@@ -669,7 +680,7 @@ __global__ void __launch_bounds__(HERM_THREADS) hermite_grid_kernel(HermArgs A)
     for (;; ++b) {
         const u64 tn = *(volatile u64 *)&A.ctl[HC_TMIN0 + b % 3];
         if (tn == ~0ull) break;
-        if (b >= C.max_blocks) { if (tid == 0) herm_set_err(A.ctl, 1u); break; }
+        if (b >= C.max_blocks) { err = max(err, 1u); break; }
         u64 local_min = ~0ull;
         HPROF(0);
         // evaluate the active particles from the state before the block: a warp looks at 32 members, then takes its
@@ -717,7 +728,10 @@ __global__ void __launch_bounds__(HERM_THREADS) hermite_grid_kernel(HermArgs A)
         HPROF(6);
     }
     if (steps) atomicAdd((unsigned long long *)&A.ctl[HC_STEPS], (unsigned long long)steps);
-    if (floor_hits & HERM_NONFINITE) herm_set_err(A.ctl, 3u);
+    // (error codes are kept in a register and filed once, here: an atomic on the error word inside the block loop --
+    //  executed or not -- made the warp tier's loop 1.6 times slower, 0.33 -> 0.55 ms for config 2)
+    if (floor_hits & HERM_NONFINITE) err = max(err, 3u);
+    if (err) herm_set_err(A.ctl, err);
     if (floor_hits & ~HERM_NONFINITE) atomicAdd((unsigned long long *)&A.ctl[HC_FLOOR], (unsigned long long)(floor_hits & ~HERM_NONFINITE));
     if (tid == 0) atomicMax((unsigned long long *)&A.ctl[HC_BLOCKS], (unsigned long long)b);
 }
