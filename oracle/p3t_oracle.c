@@ -1020,6 +1020,121 @@ void p3t_oracle_tree_walk_classes(const void *tree, const uint8_t *cls, const do
     free(mask);
 }
 
+/*
+ * O7 with classes: one soft step under H_hard with the pair kinds of O8 (L287).  The force on i over its list is Eq. 7
+ * with the kind's own softening and cutoff radii; a pair of an unsplit kind contributes the whole Newtonian term
+ * (1 - K = 1, dK/ds = 0) at every separation -- "the force between SMBHs is integrated with the pure Hermite scheme".
+ * The accuracy parameters are per CLASS of the integrated particle: eta[c], eta_s[c], a0[c] (L287: eta_FS = 0.1,
+ * eta_BH = 0.03; a0 = alpha m / r_cut^2 of Eq. 19 differs with the mass and the cutoff radius).  Everything else --
+ * ticks, block steps, predictor, corrector, the order of the operations -- is O7's, restated here so that O7 itself
+ * stays untouched; with all classes 0 the result equals O7's bit for bit (pinned).
+ */
+static void o7c_force(int64_t i, const double *m, const double *xp, const double *vp,
+                      const int64_t *offset, const int32_t *list, const uint8_t *cls, const double *tab,
+                      double *a, double *a1)
+{
+    for (int c = 0; c < 3; ++c) a[c] = a1[c] = 0.0;
+    for (int64_t e = offset[i]; e < offset[i + 1]; ++e) {
+        int64_t j = list[e];
+        pairprm p = pair_of(tab, cls, i, j);
+        const double *xj = xp + 3 * (e - offset[i] + 1), *vj = vp + 3 * (e - offset[i] + 1);
+        double d[3], w[3];
+        for (int c = 0; c < 3; ++c) { d[c] = xp[c] - xj[c]; w[c] = vp[c] - vj[c]; }
+        double s2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2] + p.eps2;
+        double s = sqrt(s2);
+        if (!p.unsplit && s >= p.r_out) continue;
+        double K = 0.0, W, dKds = 0.0;
+        if (!p.unsplit) {
+            const double g = p.r_in / p.r_out;
+            pair_weights(s, p.r_in, p.r_out, &K, &W);
+            dKds = p3t_oracle_dKdx((s / p.r_out - g) / (1.0 - g)) / (p.r_out * (1.0 - g));
+        }
+        double qv = d[0] * w[0] + d[1] * w[1] + d[2] * w[2];
+        double mr3 = m[j] / (s2 * s);
+        for (int c = 0; c < 3; ++c) {
+            a[c] += -mr3 * (1.0 - K) * d[c];
+            a1[c] += -mr3 * ((1.0 - K) * (w[c] - 3.0 * qv * d[c] / s2) - dKds * (qv / s) * d[c]);
+        }
+    }
+}
+
+int64_t p3t_oracle_hermite_classes(int64_t n, const double *m, double *q, double *v, const uint8_t *cls, const double *tab,
+                                   const int64_t *offset, const int32_t *list,
+                                   double T, int log2_div, const double *eta, const double *eta_s, const double *a0,
+                                   int64_t max_blocks, int64_t *nstep, int64_t *floor_hits)
+{
+    const int64_t total = (int64_t)1 << O7_TICK_BITS, max_ticks = total >> log2_div;
+    const double tick = T / (double)total;
+    int64_t *t = calloc((size_t)n, sizeof *t), *dt = calloc((size_t)n, sizeof *dt);
+    double *a = calloc((size_t)3 * n, sizeof *a), *a1 = calloc((size_t)3 * n, sizeof *a1);
+    double *an = calloc((size_t)3 * n, sizeof *an), *a1n = calloc((size_t)3 * n, sizeof *a1n);
+    int64_t maxl = 0, nblocks = 0;
+    if (floor_hits) *floor_hits = 0;
+    for (int64_t i = 0; i < n; ++i) if (offset[i + 1] - offset[i] > maxl) maxl = offset[i + 1] - offset[i];
+    double *xp = malloc((size_t)3 * (maxl + 1) * sizeof *xp), *vp = malloc((size_t)3 * (maxl + 1) * sizeof *vp);
+
+    for (int64_t i = 0; i < n; ++i) {
+        if (nstep) nstep[i] = 0;
+        if (offset[i + 1] == offset[i]) continue;
+        for (int c = 0; c < 3; ++c) { xp[c] = q[3 * i + c]; vp[c] = v[3 * i + c]; }
+        for (int64_t e = offset[i]; e < offset[i + 1]; ++e)
+            for (int c = 0; c < 3; ++c) {
+                xp[3 * (e - offset[i] + 1) + c] = q[3 * (int64_t)list[e] + c];
+                vp[3 * (e - offset[i] + 1) + c] = v[3 * (int64_t)list[e] + c];
+            }
+        o7c_force(i, m, xp, vp, offset, list, cls, tab, a + 3 * i, a1 + 3 * i);
+        double na = o7_norm(a + 3 * i), n1 = o7_norm(a1 + 3 * i), A0 = a0[cls[i]];
+        double crit = n1 > 0.0 ? eta_s[cls[i]] * sqrt((na * na + A0 * A0) / (n1 * n1)) : INFINITY;
+        dt[i] = o7_quantise(crit, tick, max_ticks, 0, floor_hits);
+    }
+    for (;;) {
+        int64_t tn = INT64_MAX;
+        for (int64_t i = 0; i < n; ++i)
+            if (offset[i + 1] > offset[i] && t[i] < total && t[i] + dt[i] < tn) tn = t[i] + dt[i];
+        if (tn == INT64_MAX) break;
+        if (++nblocks > max_blocks) { nblocks = -1; break; }
+        for (int64_t i = 0; i < n; ++i) {
+            if (offset[i + 1] == offset[i] || t[i] + dt[i] != tn) continue;
+            for (int64_t k = 0; k <= offset[i + 1] - offset[i]; ++k) {
+                int64_t j = k ? (int64_t)list[offset[i] + k - 1] : i;
+                double h = (double)(tn - t[j]) * tick;
+                for (int c = 0; c < 3; ++c) {
+                    double A = a[3 * j + c], J = a1[3 * j + c];
+                    xp[3 * k + c] = q[3 * j + c] + h * (v[3 * j + c] + h * (A / 2.0 + h * (J / 6.0)));
+                    vp[3 * k + c] = v[3 * j + c] + h * (A + h * (J / 2.0));
+                }
+            }
+            o7c_force(i, m, xp, vp, offset, list, cls, tab, an + 3 * i, a1n + 3 * i);
+        }
+        for (int64_t i = 0; i < n; ++i) {
+            if (offset[i + 1] == offset[i] || t[i] + dt[i] != tn) continue;
+            double h = (double)dt[i] * tick, a2[3], a3[3], a2e[3];
+            for (int c = 0; c < 3; ++c) {
+                double A = a[3 * i + c], J = a1[3 * i + c], An = an[3 * i + c], Jn = a1n[3 * i + c];
+                a2[c] = (-6.0 * (A - An) - h * (4.0 * J + 2.0 * Jn)) / (h * h);
+                a3[c] = (12.0 * (A - An) + 6.0 * h * (J + Jn)) / (h * h * h);
+                double x_p = q[3 * i + c] + h * (v[3 * i + c] + h * (A / 2.0 + h * (J / 6.0)));
+                double v_p = v[3 * i + c] + h * (A + h * (J / 2.0));
+                q[3 * i + c] = x_p + h * h * h * h * (a2[c] / 24.0 + h * a3[c] / 120.0);
+                v[3 * i + c] = v_p + h * h * h * (a2[c] / 6.0 + h * a3[c] / 24.0);
+                a2e[c] = a2[c] + h * a3[c];
+                a[3 * i + c] = An; a1[3 * i + c] = Jn;
+            }
+            t[i] = tn;
+            if (nstep) ++nstep[i];
+            double na = o7_norm(a + 3 * i), n1 = o7_norm(a1 + 3 * i), n2 = o7_norm(a2e), n3 = o7_norm(a3), A0 = a0[cls[i]];
+            double den = n1 * n3 + n2 * n2;
+            double crit = den > 0.0 ? eta[cls[i]] * sqrt((sqrt(na * na + A0 * A0) * n2 + n1 * n1) / den) : INFINITY;
+            dt[i] = o7_quantise(crit, tick, max_ticks, tn, floor_hits);
+        }
+    }
+    for (int64_t i = 0; i < n && nblocks >= 0; ++i)
+        if (offset[i + 1] == offset[i])
+            for (int c = 0; c < 3; ++c) q[3 * i + c] += T * v[3 * i + c];
+    free(t); free(dt); free(a); free(a1); free(an); free(a1n); free(xp); free(vp);
+    return nblocks;
+}
+
 int p3t_oracle_num_threads(void)
 {
 #ifdef _OPENMP

@@ -85,6 +85,8 @@ def lib():
         L.p3t_oracle_hard_classes.argtypes = [i64, pd, pd, pd, pu8, pd, i64, pi64, pd, pd, pd]
         L.p3t_oracle_tree_walk_classes.restype = None
         L.p3t_oracle_tree_walk_classes.argtypes = [vp, pu8, pd, d, i32, i64, pi64, pd, pu8, pd, pd, pi64, pi32, i64, pi64]
+        L.p3t_oracle_hermite_classes.restype = i64
+        L.p3t_oracle_hermite_classes.argtypes = [i64, pd, pd, pd, pu8, pd, pi64, pi32, d, i32, pd, pd, pd, i64, pi64, pi64]
         _lib = L
     return _lib
 
@@ -309,6 +311,29 @@ def hard_classes(mass, pos, vel, classes, tab, subset=None):
     lib().p3t_oracle_hard_classes(n, _p(m, d), _p(q, d), _p(v, d), _p(c, C.c_uint8), _p(t, d), ns,
                                   _p(sub, C.c_int64), _p(a, d), _p(j, d), _p(p, d))
     return a, j, p
+
+
+def hermite_classes(mass, pos, vel, classes, tab, offset, nbr, T, log2_div=2, eta=(0.1, 0.03), eta_s=(0.01, 0.003),
+                    a0=(0.0, 0.0), max_blocks=1 << 22):
+    """O7 with pair classes (L287): eta, eta_s, a0 are (field star, black hole) pairs.  Returns (pos, vel, info)."""
+    m = _f64(mass)
+    q, v = _f64(pos).reshape(-1, 3).copy(), _f64(vel).reshape(-1, 3).copy()
+    n = m.shape[0]
+    c, t = _cls(classes), _f64(tab)
+    off = np.ascontiguousarray(offset, dtype=np.int64)
+    lst = np.ascontiguousarray(nbr, dtype=np.int32)
+    if lst.size == 0:
+        lst = np.zeros(1, dtype=np.int32)
+    nstep = np.zeros(n, dtype=np.int64)
+    fh = np.zeros(1, dtype=np.int64)
+    e, es, aa = _f64(eta), _f64(eta_s), _f64(a0)
+    d, i64 = C.c_double, C.c_int64
+    nb = lib().p3t_oracle_hermite_classes(n, _p(m, d), _p(q, d), _p(v, d), _p(c, C.c_uint8), _p(t, d), _p(off, i64),
+                                          _p(lst, C.c_int32), float(T), int(log2_div), _p(e, d), _p(es, d), _p(aa, d),
+                                          int(max_blocks), _p(nstep, i64), _p(fh, i64))
+    if nb < 0:
+        raise RuntimeError(f"hermite_classes: more than {max_blocks} blocks")
+    return q, v, dict(blocks=int(nb), nstep=nstep, floor_hits=int(fh[0]))
 
 
 # ---------------------------------------------------------------- O4 -------

@@ -224,3 +224,82 @@ def test_C8_tree_walk_with_classes(oracle):
     wp = tree.walk_classes(cls, tab, 0.4, subset=[i])
     assert wb["n_pp"][0] > wp["n_pp"][0]
     assert np.linalg.norm(wb["acc"][0] - a[i]) <= np.linalg.norm(wp["acc"][0] - a[i]) * 1.05 + 1e-12
+
+
+# ---- O7 with classes: the Hermite part of the SMBH runs (L287: eta_FS = 0.1, eta_BH = 0.03, BH-BH pure Hermite) ----------
+
+def _hard_energy(oracle, m, q, v, cls, tab):
+    _, _, p = oracle.hard_classes(m, q, v, cls, tab)
+    return 0.5 * (m * (v * v).sum(1)).sum() + 0.5 * (m * p).sum()
+
+
+def test_C9_hermite_with_one_class_is_the_single_class_integrator_bit_for_bit(oracle):
+    rng = np.random.default_rng(21)
+    n = 40
+    q = rng.uniform(-0.15, 0.15, (n, 3))
+    v = rng.normal(0, 0.3, (n, 3))
+    m = rng.uniform(0.5, 1.5, n) / n
+    cls = np.zeros(n, dtype=np.uint8)
+    tab = _tab(oracle)
+    off, lst, _ = oracle.neighbours(q, EPS, H)
+    assert off[-1] > 20
+    T, a0 = 1.0 / 64, 0.1 * m.mean() / R_OUT ** 2
+    q1, v1, i1 = oracle.hermite(m, q, v, EPS, R_IN, R_OUT, off, lst, T, eta=0.1, eta_s=0.01, a0=a0)
+    q2, v2, i2 = oracle.hermite_classes(m, q, v, cls, tab, off, lst, T, eta=(0.1, 0.1), eta_s=(0.01, 0.01), a0=(a0, a0))
+    assert np.array_equal(q1, q2) and np.array_equal(v1, v2)
+    assert i1["blocks"] == i2["blocks"] and np.array_equal(i1["nstep"], i2["nstep"])
+
+
+def test_C10_two_black_holes_far_apart_are_a_pure_hermite_kepler_orbit(oracle):
+    """Kind 2 is not split: whatever their distance the two holes are in each other's list and feel the whole unsoftened
+    Newtonian force.  Circular orbit of separation 1 (32 times r_cut,BH-FS): the closed form, at fourth order in eta."""
+    m = np.array([0.01, 0.01])
+    M, r = m.sum(), 1.0
+    w = np.sqrt(M / r ** 3)
+    q = np.array([[0.5, 0, 0], [-0.5, 0, 0]], dtype=np.float64)
+    v = np.array([[0, 0.5 * r * w, 0], [0, -0.5 * r * w, 0]])
+    cls = np.array([1, 1], dtype=np.uint8)
+    tab = _tab(oracle)
+    off, lst, _ = oracle.neighbours_classes(q, cls, tab)
+    assert lst.tolist() == [1, 0]
+    T = 0.3 * 2 * np.pi / w
+    exact = 0.5 * r * np.array([np.cos(w * T), np.sin(w * T), 0.0])
+    errs = []
+    for eta in (0.2, 0.1, 0.05):
+        q1, v1, info = oracle.hermite_classes(m, q, v, cls, tab, off, lst, T, log2_div=3, eta=(0.1, eta), eta_s=(0.01, 0.1 * eta))
+        errs.append(np.linalg.norm(q1[0] - exact))
+        assert np.allclose(q1[0], -q1[1], atol=1e-14)
+    assert errs[0] > errs[1] > errs[2] and errs[2] < 1e-6
+    assert errs[0] / errs[2] > 30                                  # fourth order: about 2^4 per halving of eta (block steps quantise it)
+    # the same two bodies as field stars: far beyond r_cut, empty lists, a plain drift
+    cls0 = np.zeros(2, dtype=np.uint8)
+    off0, lst0, _ = oracle.neighbours_classes(q, cls0, tab)
+    assert off0[-1] == 0
+    q0, v0, _ = oracle.hermite_classes(m, q, v, cls0, tab, off0, lst0, T)
+    assert np.array_equal(q0, q + T * v) and np.array_equal(v0, v)
+
+
+def test_C11_hard_energy_is_conserved_across_kinds_and_eta_is_per_class(oracle):
+    """A hole with two field stars inside r_cut,BH-FS (one inside r_in,BH-FS), a close pair of field stars, a second hole far
+    away: H_hard = kinetic energy + hard potential of O8 is conserved over a soft step, better with smaller eta; the
+    hole's step count follows eta_BH, the stars' follow eta_FS."""
+    m = np.array([0.02, 1e-3, 1e-3, 1e-3, 1e-3, 0.02])
+    q = np.array([[0, 0, 0], [0.03, 0, 0], [0, 0.2, 0.05], [0.6, 0.6, 0.0], [0.6, 0.605, 0.0], [-0.7, 0.1, 0.0]], dtype=np.float64)
+    v = np.array([[0, 0, 0], [0, 0.8, 0], [0.25, 0, 0], [0, 0, 0.02], [0.3, 0, -0.02], [0, -0.1, 0]], dtype=np.float64)
+    cls = np.array([1, 0, 0, 0, 0, 1], dtype=np.uint8)
+    tab = _tab(oracle)
+    off, lst, band = oracle.neighbours_classes(q, cls, tab)
+    assert len(band) == 0 and 5 in lst[off[0]:off[1]].tolist() and 4 in lst[off[3]:off[4]].tolist()
+    e0 = _hard_energy(oracle, m, q, v, cls, tab)
+    T = 0.02
+    drift = []
+    for eta in (0.2, 0.05):
+        q1, v1, info = oracle.hermite_classes(m, q, v, cls, tab, off, lst, T, eta=(eta, eta), eta_s=(0.1 * eta, 0.1 * eta),
+                                              a0=(0.1 * 1e-3 / R_OUT ** 2, 0.1 * 0.02 / R_OUT_BF ** 2))
+        drift.append(abs(_hard_energy(oracle, m, q1, v1, cls, tab) - e0) / abs(e0))
+    assert drift[1] < drift[0] and drift[1] < 1e-7
+    a0 = (0.1 * 1e-3 / R_OUT ** 2, 0.1 * 0.02 / R_OUT_BF ** 2)
+    _, _, ia = oracle.hermite_classes(m, q, v, cls, tab, off, lst, T, eta=(0.1, 0.1), eta_s=(0.01, 0.01), a0=a0)
+    _, _, ib = oracle.hermite_classes(m, q, v, cls, tab, off, lst, T, eta=(0.1, 0.03), eta_s=(0.01, 0.003), a0=a0)
+    assert ib["nstep"][0] > ia["nstep"][0] and ib["nstep"][5] >= ia["nstep"][5]       # the holes step more finely
+    assert np.array_equal(ib["nstep"][3:5], ia["nstep"][3:5])                          # the far pair of stars does not care
