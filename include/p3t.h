@@ -115,8 +115,9 @@ p3t_status p3t_set_params(p3t_ctx *ctx, float eps, float theta, float r_in, floa
  * p3t_load_particles calls of the same n.  cls = NULL switches classes off.  A built tree becomes invalid.
  * P3T_EINVAL: n = 0 or > max_n, a class above 1 (host input; device input is reduced to its lowest bit), not
  * (0 <= r_in_bf < r_out_bf <= r_search_bf), eps_bb < 0, non-finite values.  P3T_ESTATE from p3t_build_tree and
- * p3t_eval_direct when n differs from the loaded particle count, and from p3t_hermite_step / p3t_step while classes
- * are set (the Hermite part on the device knows one kind of pair; eta_BH of L287 is the caller's integrator's). */
+ * p3t_eval_direct when n differs from the loaded particle count.  p3t_hermite_step and p3t_step integrate with the
+ * kind's own force too (two black holes: the pure Hermite scheme, unsoftened by default); the accuracy parameters of
+ * class 1 come from p3t_set_hermite_class_params (L287: eta_FS = 0.1, eta_BH = 0.03). */
 p3t_status p3t_set_pair_classes(p3t_ctx *ctx, size_t n, const uint8_t *cls, int on_device, float r_in_bf, float r_out_bf,
                                 float r_search_bf, float eps_bb);
 
@@ -280,6 +281,12 @@ typedef struct {
  * and when a force came out non-finite (coincident particles with eps = 0): pos, vel are then unusable. */
 p3t_status p3t_hermite_step(p3t_ctx *ctx, double *pos, double *vel, double dt_soft, int log2_div, double eta, double eta_s,
                             double a0, long long max_blocks, int on_device, p3t_hermite_info *info);
+
+/* Accuracy parameters of the Hermite part for particles of class 1 (black holes) when pair classes are set: eta and
+ * eta_s as in p3t_hermite_step (a value <= 0: the call's own), a0 (< 0: the call's own).  L287: "The accuracy parameter
+ * of timestep criterion for FS eta_FS is 0.1, and for SMBH eta_BH is 0.03"; a0 = alpha m / r_cut^2 (Eq. 19) differs with
+ * the mass and the cutoff radius of the class.  P3T_EINVAL for non-finite values. */
+p3t_status p3t_set_hermite_class_params(p3t_ctx *ctx, double eta_bh, double eta_s_bh, double a0_bh);
 
 /* Tuning knob of p3t_hermite_step: the largest neighbour cluster (connected component of the lists) that one thread-block
  * cluster of 8 CTAs integrates with its own block times; still larger ones go together through a cooperative kernel

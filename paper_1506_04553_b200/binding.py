@@ -29,7 +29,7 @@ _STATUS = {0: "P3T_OK", -1: "P3T_EINVAL", -2: "P3T_ESTATE", -3: "P3T_ENOMEM", -4
 SYMBOLS = [
     "p3t_workspace_bytes", "p3t_create", "p3t_destroy", "p3t_set_params", "p3t_set_tree_params",
     "p3t_set_pair_classes", "p3t_set_key_curve", "p3t_hilbert_state_tables", "p3t_set_group_merge_levels", "p3t_set_walk_mode", "p3t_set_shard", "p3t_get_shard_record", "p3t_put_shard_classes", "p3t_load_particles", "p3t_build_tree", "p3t_set_tree_reuse", "p3t_refit_tree", "p3t_eval_soft", "p3t_eval_direct", "p3t_eval_hard",
-    "p3t_hermite_step", "p3t_step", "p3t_set_hermite_cluster_max",
+    "p3t_hermite_step", "p3t_step", "p3t_set_hermite_cluster_max", "p3t_set_hermite_class_params",
     "p3t_get_acc_pot", "p3t_get_neighbour_counts", "p3t_get_neighbours", "p3t_get_stats", "p3t_synchronize",
     "p3t_last_error", "p3t_array_info", "p3t_copy_array", "p3t_measure_fp32_peak", "p3t_measure_latency",
 ]
@@ -75,6 +75,7 @@ def _sig():
     L.p3t_hilbert_state_tables.restype = i; L.p3t_hilbert_state_tables.argtypes = [vp, sz]
     L.p3t_set_walk_mode.restype = i; L.p3t_set_walk_mode.argtypes = [vp, i]
     L.p3t_set_hermite_cluster_max.restype = i; L.p3t_set_hermite_cluster_max.argtypes = [vp, i]
+    L.p3t_set_hermite_class_params.restype = i; L.p3t_set_hermite_class_params.argtypes = [vp, C.c_double, C.c_double, C.c_double]
     L.p3t_set_shard.restype = i; L.p3t_set_shard.argtypes = [vp, i, i]
     L.p3t_get_shard_record.restype = i; L.p3t_get_shard_record.argtypes = [vp, vp]
     L.p3t_put_shard_classes.restype = i; L.p3t_put_shard_classes.argtypes = [vp, vp]
@@ -292,6 +293,9 @@ class P3T:
         a, j, p = np.empty((self.n, 3)), np.empty((self.n, 3)), np.empty(self.n)
         self._check(_lib.p3t_eval_hard(self._h, pv, a.ctypes.data, j.ctypes.data, p.ctypes.data, 0))
         return a, j, p
+
+    def set_hermite_class_params(self, eta_bh=0.0, eta_s_bh=0.0, a0_bh=-1.0):
+        self._check(_lib.p3t_set_hermite_class_params(self._h, float(eta_bh), float(eta_s_bh), float(a0_bh)))
 
     def set_hermite_cluster_max(self, max_members):
         self._check(_lib.p3t_set_hermite_cluster_max(self._h, int(max_members)))

@@ -140,6 +140,7 @@ extern "C" p3t_status p3t_create(p3t_ctx **out, int device, size_t max_n, int ke
     ctx->herm_cluster_max = 4096;
     ctx->shard_rank = 0;
     ctx->shard_world = 1;
+    ctx->herm_a0_bh = -1.0;
     ctx->max_refits = 0;
     ctx->stray_dist = 0.5f;
     ctx->max_stray_fraction = 0.02f;
@@ -363,6 +364,14 @@ extern "C" p3t_status p3t_put_shard_classes(p3t_ctx *ctx, const float *rec)
     p3t_status st = p3t_stage_shard_classes(ctx, rec);
     if (st == P3T_OK) ctx->shard_classes_fresh = true;
     return st;
+}
+
+extern "C" p3t_status p3t_set_hermite_class_params(p3t_ctx *ctx, double eta_bh, double eta_s_bh, double a0_bh)
+{
+    if (!ctx) return P3T_EINVAL;
+    if (!std::isfinite(eta_bh) || !std::isfinite(eta_s_bh) || !std::isfinite(a0_bh)) return p3t_fail(ctx, P3T_EINVAL, "non-finite value");
+    ctx->herm_eta_bh = eta_bh; ctx->herm_eta_s_bh = eta_s_bh; ctx->herm_a0_bh = a0_bh;
+    return P3T_OK;
 }
 
 extern "C" p3t_status p3t_set_hermite_cluster_max(p3t_ctx *ctx, int max_members)
@@ -651,7 +660,6 @@ extern "C" p3t_status p3t_hermite_step(p3t_ctx *ctx, double *pos, double *vel, d
     if (!ctx->evaluated) return p3t_fail(ctx, P3T_ESTATE, "p3t_hermite_step needs the neighbour lists of an eval call");
     if (!ctx->lists_complete)
         return p3t_fail(ctx, P3T_ESTATE, "p3t_hermite_step needs the lists of ALL particles: the last evaluation was sharded or a subset");
-    if (ctx->cls_n) return p3t_fail(ctx, P3T_ESTATE, "the Hermite part does not know pair classes (p3t_set_pair_classes): use p3t_eval_hard");
     p3t_status st = hermite_args_ok(ctx, dt_soft, log2_div, eta, eta_s, a0, max_blocks);
     if (st != P3T_OK) return st;
     P3T_CUDA(ctx, cudaSetDevice(ctx->device));
@@ -679,7 +687,6 @@ extern "C" p3t_status p3t_step(p3t_ctx *ctx, const float *mass, double *pos, dou
     if (!ctx) return P3T_EINVAL;
     if (!mass || !pos || !vel) return p3t_fail(ctx, P3T_EINVAL, "null mass/pos/vel");
     if (!ctx->evaluated) return p3t_fail(ctx, P3T_ESTATE, "p3t_step needs the soft force and lists of an eval call at the current positions");
-    if (ctx->cls_n) return p3t_fail(ctx, P3T_ESTATE, "p3t_step does not know pair classes (p3t_set_pair_classes)");
     if (!ctx->lists_complete || ctx->shard_world > 1)
         return p3t_fail(ctx, P3T_ESTATE, "p3t_step needs the soft force and lists of ALL particles: not available on a sharded context or after a subset evaluation");
     p3t_status st = hermite_args_ok(ctx, dt_soft, log2_div, eta, eta_s, a0, max_blocks);

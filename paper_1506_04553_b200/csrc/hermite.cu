@@ -225,6 +225,7 @@ struct HermConst {
     P3TParams prm;
     double tick, rtick, eta, eta_s, a0;
     double c2, c2_s;               // (eta / tick)^2, (eta_s / tick)^2
+    double c2k[2], c2_sk[2], a0k[2];   // pair classes: the same per class of the integrated particle (eta_FS, eta_BH)
     u64 max_ticks, max_blocks;
 };
 
@@ -238,6 +239,7 @@ struct HermView {
     const u32 *nbr;                // list entries
     const float4 *body_user;       // global view: mass in .w (the masses of the evaluation that made the lists)
     const double *mass;            // local view
+    const u8 *cls;                 // pair classes only: class of every particle (global view) / member slot (local view)
 };
 
 struct HermArgs {
@@ -259,7 +261,9 @@ struct HermArgs {
 // predicted from their own last times.  first: t = 0, nothing to predict.
 // SPLIT > 1: SPLIT consecutive lanes share the list of one particle (entry k0 + sub, k0 + sub + SPLIT, ...) and add their
 // partial sums with shuffles; every lane of the warp must make the call (lanes without a particle pass k0 = k1).
-template <bool LOCAL, int SPLIT = 1>
+// CLS (pair classes, L287): the kind of a pair, class_i + class_j, selects the softening and the cutoff coefficients; a
+// pair of kind 2 (two black holes) is not split: the whole Newtonian term with eps_bb, at every separation.
+template <bool LOCAL, int SPLIT = 1, bool CLS = false>
 __device__ __forceinline__ void herm_force(const HermConst &C, const HermView &V, u32 i, u64 k0, u64 k1, u64 tn, bool first,
                                            double *a, double *a1)
 {
@@ -274,7 +278,7 @@ __device__ __forceinline__ void herm_force(const HermConst &C, const HermView &V
             vi[c] = Vc + h * (Ac + h * (Jc * 0.5));
         }
     }
-    const double eps2 = C.prm.eps2_d;
+    const u32 ci = CLS ? (u32)V.cls[i] : 0u;
     double ax = 0, ay = 0, az = 0, jx = 0, jy = 0, jz = 0;
     for (u64 k = k0 + (SPLIT > 1 ? (threadIdx.x & (SPLIT - 1)) : 0); k < k1; k += SPLIT) {
         const u32 j = V.nbr[k];
@@ -287,10 +291,11 @@ __device__ __forceinline__ void herm_force(const HermConst &C, const HermView &V
             d[c] = xi[c] - (X + h * (Vc + h * (Ac * 0.5 + h * (Jc * kSixth))));
             w[c] = vi[c] - (Vc + h * (Ac + h * (Jc * 0.5)));
         }
-        const double s2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2] + eps2;
+        const u32 kind = CLS ? ci + (u32)V.cls[j] : 0u;
+        const double s2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2] + ((CLS && kind == 2u) ? C.prm.eps2_bb_d : C.prm.eps2_d);
         const double s = sqrt(s2);
-        double omK, dKds;
-        herm_weights(C.prm.cs[0], s, omK, dKds);
+        double omK = 1.0, dKds = 0.0;
+        if (!(CLS && kind == 2u)) herm_weights(C.prm.cs[CLS ? kind : 0u], s, omK, dKds);
         if (omK == 0.0 && dKds == 0.0) continue;
         const double qv = d[0] * w[0] + d[1] * w[1] + d[2] * w[2];
         const double mj = LOCAL ? V.mass[j] : (double)V.body_user[j].w;
@@ -346,13 +351,14 @@ __device__ __forceinline__ u32 herm_quantise(const HermConst &C, double P, doubl
 }
 
 // t = 0: force from the current state, first step from Eq. 20.  Returns the particle's first block time.
-template <bool LOCAL>
+template <bool LOCAL, bool CLS = false>
 __device__ __forceinline__ u64 herm_start(const HermConst &C, const HermView &V, u32 i, u64 k0, u64 k1, u32 &floor_hits)
 {
     double a[3], a1[3];
-    herm_force<LOCAL>(C, V, i, k0, k1, 0, true, a, a1);
+    herm_force<LOCAL, 1, CLS>(C, V, i, k0, k1, 0, true, a, a1);
     const double d0 = a[0] * a[0] + a[1] * a[1] + a[2] * a[2], d1 = a1[0] * a1[0] + a1[1] * a1[1] + a1[2] * a1[2];
-    const u32 k = herm_quantise(C, C.c2_s * (d0 + C.a0 * C.a0), d1, 0, floor_hits);          // Eq. 20, squared
+    const double c2s = CLS ? C.c2_sk[V.cls[i]] : C.c2_s, a0 = CLS ? C.a0k[V.cls[i]] : C.a0;
+    const u32 k = herm_quantise(C, c2s * (d0 + a0 * a0), d1, 0, floor_hits);          // Eq. 20, squared
 #pragma unroll
     for (int c = 0; c < 3; ++c) { V.a[3 * (size_t)i + c] = a[c]; V.a1[3 * (size_t)i + c] = a1[c]; }   // nobody reads a, a1, tdt at t = 0
     V.tdt[i] = k;
@@ -361,7 +367,7 @@ __device__ __forceinline__ u64 herm_start(const HermConst &C, const HermView &V,
 
 // first half of a block: the new force of an active particle from the state before the block.  Returns true if active;
 // otherwise te is the particle's own next time (~0 when it has arrived at the end of the soft step).
-template <bool LOCAL>
+template <bool LOCAL, bool CLS = false>
 __device__ __forceinline__ bool herm_evaluate(const HermConst &C, const HermView &V, u32 i, u64 k0, u64 k1, u64 tn, u64 &te)
 {
     const u64 total = 1ull << HERM_TICK_BITS;
@@ -370,13 +376,14 @@ __device__ __forceinline__ bool herm_evaluate(const HermConst &C, const HermView
     te = t >= total ? ~0ull : t + (1ull << (w & 63));
     if (te != tn) return false;
     double a[3], a1[3];
-    herm_force<LOCAL>(C, V, i, k0, k1, tn, false, a, a1);
+    herm_force<LOCAL, 1, CLS>(C, V, i, k0, k1, tn, false, a, a1);
 #pragma unroll
     for (int c = 0; c < 3; ++c) { V.an[3 * (size_t)i + c] = a[c]; V.a1n[3 * (size_t)i + c] = a1[c]; }
     return true;
 }
 
 // second half: corrector and the next step (Eq. 18) of a particle that herm_evaluate found active.  Returns its next time.
+template <bool CLS = false>
 __device__ __forceinline__ u64 herm_correct(const HermConst &C, const HermView &V, u32 i, u64 tn, u32 &floor_hits)
 {
     const u64 total = 1ull << HERM_TICK_BITS;
@@ -404,7 +411,8 @@ __device__ __forceinline__ u64 herm_correct(const HermConst &C, const HermView &
     const double d0 = an[0] * an[0] + an[1] * an[1] + an[2] * an[2], d1 = jn[0] * jn[0] + jn[1] * jn[1] + jn[2] * jn[2];
     const double d2 = a2e[0] * a2e[0] + a2e[1] * a2e[1] + a2e[2] * a2e[2], d3 = a3[0] * a3[0] + a3[1] * a3[1] + a3[2] * a3[2];
     const double den = sqrt(d1 * d3) + d2;
-    const u32 k = herm_quantise(C, C.c2 * (sqrt((d0 + C.a0 * C.a0) * d2) + d1), den, tn, floor_hits);
+    const double c2 = CLS ? C.c2k[V.cls[i]] : C.c2, a0 = CLS ? C.a0k[V.cls[i]] : C.a0;
+    const u32 k = herm_quantise(C, c2 * (sqrt((d0 + a0 * a0) * d2) + d1), den, tn, floor_hits);
     V.tdt[i] = tn << 8 | k;
     return tn < total ? tn + (1ull << k) : ~0ull;
 }
@@ -429,8 +437,10 @@ struct WarpState {
     u64 tdt[HERM_WARP_MAX];
     double mass[HERM_WARP_MAX];
     u32 gid[HERM_WARP_MAX];
+    u8 cls[HERM_WARP_MAX];
 };
 
+template <bool CLS>
 __global__ void __launch_bounds__(32 * HERM_WARPS) hermite_warp_kernel(HermArgs A)
 {
     u32 err = 0;                   // HC_ERR code of this thread, filed at the end of the kernel
@@ -453,6 +463,7 @@ __global__ void __launch_bounds__(32 * HERM_WARPS) hermite_warp_kernel(HermArgs 
             S.gid[slot[q]] = g;
             k0[q] = A.offset[g]; k1[q] = A.offset[g + 1];
             S.mass[slot[q]] = (double)A.G.body_user[g].w;
+            if (CLS) S.cls[slot[q]] = A.G.cls[g] & 1u;
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
                 S.pos[3 * slot[q] + c] = A.G.pos[3 * (size_t)g + c];
@@ -472,14 +483,14 @@ __global__ void __launch_bounds__(32 * HERM_WARPS) hermite_warp_kernel(HermArgs 
         }
     HermView V;
     V.pos = S.pos; V.vel = S.vel; V.a = S.a; V.a1 = S.a1; V.an = S.an; V.a1n = S.a1n; V.tdt = S.tdt;
-    V.nbr = A.lnbr; V.body_user = nullptr; V.mass = S.mass;
+    V.nbr = A.lnbr; V.body_user = nullptr; V.mass = S.mass; V.cls = S.cls;
     const HermConst &C = A.C;
 
     u32 floor_hits = 0, steps = 0;
     u64 next = ~0ull;
 #pragma unroll
     for (int q = 0; q < PER; ++q)
-        if (have[q]) next = min(next, herm_start<true>(C, V, slot[q], k0[q], k1[q], floor_hits));
+        if (have[q]) next = min(next, herm_start<true, CLS>(C, V, slot[q], k0[q], k1[q], floor_hits));
     __syncwarp();
     u64 tn = warp_min_u64(next);
     u64 b = 0;
@@ -489,13 +500,13 @@ __global__ void __launch_bounds__(32 * HERM_WARPS) hermite_warp_kernel(HermArgs 
         bool act[PER];
         u64 te[PER];
 #pragma unroll
-        for (int q = 0; q < PER; ++q) act[q] = have[q] && herm_evaluate<true>(C, V, slot[q], k0[q], k1[q], tn, te[q]);
+        for (int q = 0; q < PER; ++q) act[q] = have[q] && herm_evaluate<true, CLS>(C, V, slot[q], k0[q], k1[q], tn, te[q]);
         __syncwarp();
         next = ~0ull;
 #pragma unroll
         for (int q = 0; q < PER; ++q) {
             if (!have[q]) continue;
-            if (act[q]) { next = min(next, herm_correct(C, V, slot[q], tn, floor_hits)); ++steps; }
+            if (act[q]) { next = min(next, herm_correct<CLS>(C, V, slot[q], tn, floor_hits)); ++steps; }
             else next = min(next, te[q]);
         }
         __syncwarp();
@@ -527,7 +538,7 @@ extern "C" void p3t_debug_hprof(unsigned long long *out) { cudaDeviceSynchronize
 #else
 #define HPROF(k)
 #endif
-template <int SPLIT>
+template <int SPLIT, bool CLS>
 __device__ __forceinline__ void cluster_evaluate(const HermArgs &A, const u32 *active, const u32 *ids, u32 na, u32 tid, u32 stride, u64 tn)
 {
     const HermView &V = A.G;
@@ -539,7 +550,7 @@ __device__ __forceinline__ void cluster_evaluate(const HermArgs &A, const u32 *a
         const u32 i = ok ? active[e] : 0u;
         const u64 k0 = ok ? A.offset[i] : 0ull, k1 = ok ? A.offset[i + 1] : 0ull;
         double a[3], a1[3];
-        herm_force<false, SPLIT>(A.C, V, ok ? i : ids[0], k0, k1, tn, false, a, a1);
+        herm_force<false, SPLIT, CLS>(A.C, V, ok ? i : ids[0], k0, k1, tn, false, a, a1);
         if (ok && (lane & (SPLIT - 1)) == 0) {
 #pragma unroll
             for (int k = 0; k < 3; ++k) { V.an[3 * (size_t)i + k] = a[k]; V.a1n[3 * (size_t)i + k] = a1[k]; }
@@ -551,6 +562,7 @@ __device__ __forceinline__ void cluster_evaluate(const HermArgs &A, const u32 *a
 // hardware cluster barrier (a fraction of a microsecond, against several for a grid barrier), components run side by
 // side.  Per block: scan the members (next block time of the inactive ones, active ones appended to a list), barrier,
 // evaluate the active list one particle per thread, barrier, correct, barrier.  State in global memory (L2).
+template <bool CLS>
 __global__ void __cluster_dims__(HERM_CLUSTER, 1, 1) __launch_bounds__(HERM_CLUSTER_THREADS) hermite_cluster_kernel(HermArgs A)
 {
     u32 err = 0;                   // HC_ERR code of this thread, filed at the end of the kernel
@@ -570,7 +582,7 @@ __global__ void __cluster_dims__(HERM_CLUSTER, 1, 1) __launch_bounds__(HERM_CLUS
         u64 local_min = ~0ull;
         for (u32 s = tid; s < M; s += stride) {
             const u32 i = ids[s];
-            local_min = min(local_min, herm_start<false>(C, V, i, A.offset[i], A.offset[i + 1], floor_hits));
+            local_min = min(local_min, herm_start<false, CLS>(C, V, i, A.offset[i], A.offset[i + 1], floor_hits));
         }
         local_min = warp_min_u64(local_min);
         if (lane == 0 && local_min != ~0ull) atomicMin((unsigned long long *)&ctl[0], (unsigned long long)local_min);
@@ -614,15 +626,15 @@ __global__ void __cluster_dims__(HERM_CLUSTER, 1, 1) __launch_bounds__(HERM_CLUS
         // evaluate the active particles from the state before the block; as many lanes share a particle's list as the
         // cluster has to spare (the longest list of the block is the critical path: every entry is an L2 round trip plus
         // an fp64 chain)
-        if (na * 8 <= stride) cluster_evaluate<8>(A, active, ids, na, tid, stride, tn);
-        else if (na * 4 <= stride) cluster_evaluate<4>(A, active, ids, na, tid, stride, tn);
-        else if (na * 2 <= stride) cluster_evaluate<2>(A, active, ids, na, tid, stride, tn);
-        else cluster_evaluate<1>(A, active, ids, na, tid, stride, tn);
+        if (na * 8 <= stride) cluster_evaluate<8, CLS>(A, active, ids, na, tid, stride, tn);
+        else if (na * 4 <= stride) cluster_evaluate<4, CLS>(A, active, ids, na, tid, stride, tn);
+        else if (na * 2 <= stride) cluster_evaluate<2, CLS>(A, active, ids, na, tid, stride, tn);
+        else cluster_evaluate<1, CLS>(A, active, ids, na, tid, stride, tn);
         HPROF(3);
         cl.sync();
         HPROF(4);
         for (u32 e = tid; e < na; e += stride) {           // correct them together
-            local_min = min(local_min, herm_correct(C, V, active[e], tn, floor_hits));
+            local_min = min(local_min, herm_correct<CLS>(C, V, active[e], tn, floor_hits));
             ++steps;
         }
         local_min = warp_min_u64(local_min);
@@ -655,6 +667,7 @@ __device__ __forceinline__ void cta_min_to(u64 *dst, u64 v, u64 *s_min)
     __syncthreads();
 }
 
+template <bool CLS>
 __global__ void __launch_bounds__(HERM_THREADS) hermite_grid_kernel(HermArgs A)
 {
     u32 err = 0;                   // HC_ERR code of this thread, filed at the end of the kernel
@@ -671,7 +684,7 @@ __global__ void __launch_bounds__(HERM_THREADS) hermite_grid_kernel(HermArgs A)
         u64 local_min = ~0ull;
         for (u32 s = tid; s < M; s += stride) {
             const u32 i = ids[s];
-            local_min = min(local_min, herm_start<false>(C, V, i, A.offset[i], A.offset[i + 1], floor_hits));
+            local_min = min(local_min, herm_start<false, CLS>(C, V, i, A.offset[i], A.offset[i + 1], floor_hits));
         }
         cta_min_to(&A.ctl[HC_TMIN0], local_min, s_min);
     }
@@ -701,7 +714,7 @@ __global__ void __launch_bounds__(HERM_THREADS) hermite_grid_kernel(HermArgs A)
                 const u32 ii = __shfl_sync(0xffffffffu, i, ok ? src : 0);
                 const u64 k0 = ok ? A.offset[ii] : 0ull, k1 = ok ? A.offset[ii + 1] : 0ull;
                 double a[3], a1[3];
-                herm_force<false, 8>(C, V, ok ? ii : ids[0], k0, k1, tn, false, a, a1);
+                herm_force<false, 8, CLS>(C, V, ok ? ii : ids[0], k0, k1, tn, false, a, a1);
                 if (ok && (lane & 7) == 0) {
 #pragma unroll
                     for (int k = 0; k < 3; ++k) { V.an[3 * (size_t)ii + k] = a[k]; V.a1n[3 * (size_t)ii + k] = a1[k]; }
@@ -717,7 +730,7 @@ __global__ void __launch_bounds__(HERM_THREADS) hermite_grid_kernel(HermArgs A)
             const u32 i = ids[s];
             const u64 w = V.tdt[i];
             if ((w >> 8) + (1ull << (w & 63)) != tn || (w >> 8) >= (1ull << HERM_TICK_BITS)) continue;
-            local_min = min(local_min, herm_correct(C, V, i, tn, floor_hits));
+            local_min = min(local_min, herm_correct<CLS>(C, V, i, tn, floor_hits));
             ++steps;
         }
         cta_min_to(&A.ctl[HC_TMIN0 + (b + 1) % 3], local_min, s_min);     // (one atomic per CTA: one per thread on the same
@@ -774,6 +787,14 @@ p3t_status p3t_stage_hermite(p3t_ctx *ctx, double *d_pos, double *d_vel, double 
         A.C.rtick = (double)(1ull << HERM_TICK_BITS) / T;
         A.C.eta = eta; A.C.eta_s = eta_s; A.C.a0 = a0;
         A.C.c2 = (eta * A.C.rtick) * (eta * A.C.rtick); A.C.c2_s = (eta_s * A.C.rtick) * (eta_s * A.C.rtick);
+        {   // pair classes: accuracy parameters per class of the integrated particle (class 1: p3t_set_hermite_class_params)
+            const double e1 = ctx->herm_eta_bh > 0.0 ? ctx->herm_eta_bh : eta, es1 = ctx->herm_eta_s_bh > 0.0 ? ctx->herm_eta_s_bh : eta_s;
+            A.C.c2k[0] = A.C.c2; A.C.c2_sk[0] = A.C.c2_s; A.C.a0k[0] = a0;
+            A.C.c2k[1] = (e1 * A.C.rtick) * (e1 * A.C.rtick); A.C.c2_sk[1] = (es1 * A.C.rtick) * (es1 * A.C.rtick);
+            A.C.a0k[1] = ctx->herm_a0_bh >= 0.0 ? ctx->herm_a0_bh : a0;
+        }
+        A.G.cls = w.cls_user;
+        const bool cls = ctx->cls_n != 0;
         A.C.max_ticks = (1ull << HERM_TICK_BITS) >> log2_div;
         A.C.max_blocks = (u64)max_blocks;
         // The grid tier (if any) goes first on the caller's stream: one CTA per SM, mostly waiting at its barriers; the
@@ -781,7 +802,7 @@ p3t_status p3t_stage_hermite(p3t_ctx *ctx, double *d_pos, double *d_vel, double 
         cudaStream_t rest = ctx->stream;
         if (ngrid) {
             int per_sm = 0;
-            P3T_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, hermite_grid_kernel, HERM_THREADS, 0));
+            P3T_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, hermite_grid_kernel<false>, HERM_THREADS, 0));
             if (per_sm < 1) return p3t_fail(ctx, P3T_ECUDA, "hermite_grid_kernel does not fit an SM");
             u32 grid = (u32)((ngrid + HERM_THREADS - 1) / HERM_THREADS);
             if (grid > (u32)ctx->sm_count) grid = (u32)ctx->sm_count;   // one CTA per SM: the barrier is the cost of a block
@@ -791,14 +812,17 @@ p3t_status p3t_stage_hermite(p3t_ctx *ctx, double *d_pos, double *d_vel, double 
                 rest = ctx->side_stream;
             }
             void *args[] = {&A};
-            P3T_CUDA(ctx, cudaLaunchCooperativeKernel((void *)hermite_grid_kernel, dim3(grid), dim3(HERM_THREADS), args, 0, ctx->stream));
+            P3T_CUDA(ctx, cudaLaunchCooperativeKernel(cls ? (void *)hermite_grid_kernel<true> : (void *)hermite_grid_kernel<false>, dim3(grid),
+                                                      dim3(HERM_THREADS), args, 0, ctx->stream));
         }
         if (nsmall) {
-            hermite_warp_kernel<<<div_up(nsmall, HERM_WARPS), 32 * HERM_WARPS, 0, rest>>>(A);
+            if (cls) hermite_warp_kernel<true><<<div_up(nsmall, HERM_WARPS), 32 * HERM_WARPS, 0, rest>>>(A);
+            else hermite_warp_kernel<false><<<div_up(nsmall, HERM_WARPS), 32 * HERM_WARPS, 0, rest>>>(A);
             P3T_CUDA(ctx, cudaGetLastError());
         }
         if (nbigc) {
-            hermite_cluster_kernel<<<(u32)nbigc * HERM_CLUSTER, HERM_CLUSTER_THREADS, 0, rest>>>(A);
+            if (cls) hermite_cluster_kernel<true><<<(u32)nbigc * HERM_CLUSTER, HERM_CLUSTER_THREADS, 0, rest>>>(A);
+            else hermite_cluster_kernel<false><<<(u32)nbigc * HERM_CLUSTER, HERM_CLUSTER_THREADS, 0, rest>>>(A);
             P3T_CUDA(ctx, cudaGetLastError());
         }
         if (rest != ctx->stream) {

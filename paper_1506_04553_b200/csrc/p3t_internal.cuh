@@ -165,6 +165,7 @@ struct p3t_ctx {
     int walk_mode;                 // 0 auto, 1 one warp per group, 2 one CTA per group (cooperative)
     size_t cls_n;                  // 0: no classes; else the particle count the classes were given for
     float r_in_bf, r_out_bf, r_search_bf, eps_bb;
+    double herm_eta_bh, herm_eta_s_bh, herm_a0_bh;   // Hermite part: accuracy parameters of class 1 (<= 0 / < 0: those of the call)
     bool shard_classes_fresh;      // p3t_put_shard_classes since the last sharded walk: all ranks hold the same cost classes
     int shard_rank, shard_world;   // this context walks the groups at positions rank, rank + world, ... of the hand-out order
     int sm_count;

@@ -102,6 +102,10 @@ def classes(n):
         ctx.soft_force(cfg["mass"], cfg["pos"])
         ctx.get_acc_pot()
         off, nbr = ctx.get_neighbours()
+        ctx.eval_hard(cfg["vel"])
+        ctx.set_hermite_class_params(0.03, 0.003, 0.1 * 0.01 / cfg["class_params"]["r_out_bf"] ** 2)
+        q, v = cfg["pos"].astype(np.float64), cfg["vel"].astype(np.float64)
+        ctx.step(cfg["mass"], q, v, cfg["dt_soft"], a0=0.1 * float(cfg["mass"][0]) / cfg["r_out"] ** 2)
     return int(off[-1])
 
 

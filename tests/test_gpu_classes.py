@@ -166,11 +166,73 @@ def test_class_arguments_and_state():
         off, nbr = ctx.get_neighbours()
         n = cfg["n"]
         assert n - 2 in nbr[int(off[n - 1]):int(off[n])].tolist()
-        with pytest.raises(binding.P3TError) as ei:
-            ctx.hermite_step(cfg["pos"].astype(np.float64), cfg["vel"].astype(np.float64), 1e-3)
-        assert ei.value.status == binding.ESTATE
         ctx.set_pair_classes(None)
         ctx.soft_force(cfg["mass"], cfg["pos"])
         off, nbr = ctx.get_neighbours()
         assert n - 2 not in nbr[int(off[n - 1]):int(off[n])].tolist()
         ctx.hermite_step(cfg["pos"].astype(np.float64), cfg["vel"].astype(np.float64), 1e-3)
+
+
+@pytest.mark.parametrize("n,extra,cluster_max", [(16384, 0, None), (20000, 6, None), (6000, 40, 64)])
+def test_hermite_part_with_classes_takes_the_oracles_steps(oracle, n, extra, cluster_max):
+    """p3t_hermite_step with pair classes against oracle O7-with-classes over the same lists: the two holes of the paper's
+    SMBH start (each other's neighbours at distance 1: a pure Hermite pair, unsoftened) and the field stars within
+    r_search,BH-FS of a hole; extra holes in the core make clusters with several holes (cluster_max = 64 sends the larger
+    ones to the thread-block-cluster tier)."""
+    cfg = _smbh(n, extra_holes=extra)
+    tab = _tab(oracle, cfg)
+    m, q, v = cfg["mass"].astype(np.float64), cfg["pos"].astype(np.float64), cfg["vel"].astype(np.float64)
+    cls = cfg["classes"]
+    T = cfg["dt_soft"]
+    ooff, olst, band = oracle.neighbours_classes(q, cls, tab)
+    assert len(band) == 0
+    a0 = (0.1 * float(m[0]) / cfg["r_out"] ** 2, 0.1 * 0.01 / cfg["class_params"]["r_out_bf"] ** 2)
+    eta, eta_s = (0.1, 0.03), (0.01, 0.003)
+    oq, ov, oinfo = oracle.hermite_classes(m, q, v, cls, tab, ooff, olst, T, eta=eta, eta_s=eta_s, a0=a0)
+    with _ctx(cfg, nbr_capacity=max(int(ooff[-1]) + 1024, 1 << 16)) as ctx:
+        ctx.soft_force(cfg["mass"], cfg["pos"])
+        off, nbr = ctx.get_neighbours()
+        assert np.array_equal(off.astype(np.int64), ooff) and np.array_equal(nbr.astype(np.int64), olst.astype(np.int64))
+        ctx.set_hermite_class_params(eta[1], eta_s[1], a0[1])
+        if cluster_max:
+            ctx.set_hermite_cluster_max(cluster_max)
+        gq, gv = q.copy(), v.copy()
+        info = ctx.hermite_step(gq, gv, T, eta=eta[0], eta_s=eta_s[0], a0=a0[0])
+    holes = np.flatnonzero(cls == 1)
+    assert info["n_steps"] == int(oinfo["nstep"].sum()) and oinfo["nstep"][holes].min() >= 4
+    assert info["n_nonisolated"] == int((np.diff(ooff) > 0).sum())
+    iso = np.diff(ooff) == 0
+    assert np.array_equal(gq[iso], oq[iso])
+    assert np.abs(gq - oq).max() <= 1e-9 * np.abs(T * v).max() and np.abs(gv - ov).max() <= 1e-9 * np.abs(v).max()
+    # the holes moved under each other's pull, not on straight lines
+    assert np.abs(gq[holes] - (q[holes] + T * v[holes])).max() > 1e-12
+
+
+def test_whole_steps_with_classes_conserve_energy():
+    """p3t_step on the paper's SMBH start: 16 steps; the total energy (kinetic + the kinds' own softened potentials by a
+    direct sum in numpy) stays within the soft force's tolerance."""
+    import torch
+
+    cfg = _smbh(8192)
+    m, cls = cfg["mass"].astype(np.float64), cfg["classes"]
+    T = cfg["dt_soft"]
+
+    def energy(q, v):
+        d = q[:, None, :] - q[None, :, :]
+        eps = np.where((cls[:, None] == 1) & (cls[None, :] == 1), cfg["class_params"]["eps_bb"], cfg["eps"])
+        s = np.sqrt((d * d).sum(-1) + eps ** 2)
+        np.fill_diagonal(s, np.inf)
+        return 0.5 * (m * (v * v).sum(1)).sum() - 0.5 * (m[:, None] * m[None, :] / s).sum()
+
+    q0, v0 = cfg["pos"].astype(np.float64), cfg["vel"].astype(np.float64)
+    e0 = energy(q0, v0)
+    with _ctx(cfg) as ctx:
+        ctx.set_hermite_class_params(0.03, 0.003, 0.1 * 0.01 / cfg["class_params"]["r_out_bf"] ** 2)
+        ctx.soft_force(cfg["mass"], cfg["pos"])
+        q, v = torch.from_numpy(q0).cuda(), torch.from_numpy(v0).cuda()
+        md = torch.from_numpy(cfg["mass"]).cuda()
+        for _ in range(16):
+            info = ctx.step(md, q, v, T, a0=0.1 * float(m[0]) / cfg["r_out"] ** 2)
+        assert info["n_nonisolated"] >= 2
+    e1 = energy(q.cpu().numpy(), v.cpu().numpy())
+    assert abs(e1 / e0 - 1) < 2e-4, (e0, e1)
