@@ -536,6 +536,13 @@ __device__ __forceinline__ void walk_group(WarpShared *wsall, const StackRef &st
             float ez = fmaxf(0.f, fmaxf(lo[2] - a.z, a.z - hi[2]));
             float d2 = fmaf(ex, ex, fmaf(ey, ey, ez * ez));
             accept = d2 > a.w;
+            if (CLS && heavy_group && accept) {
+                const float rm = ws.l_mom1[lane].w;                       // bounding radius; sign bit: the cell holds a black hole
+                const float rc = (prm.h_bf + fabsf(rm)) * (1.f + 1e-5f) + slack;
+                accept = !(__float_as_uint(rm) >> 31) && d2 > rc * rc;
+            }
+            // (after the acceptance is final: a part that drops a cell as "accepted, someone else's" must not find out
+            //  later that it has to be opened)
             if (SPLIT) {      // is this cell mine?
                 const u32 c = ws.l_cell[lane];
                 if (c >= sr.lo) {
@@ -544,11 +551,6 @@ __device__ __forceinline__ void walk_group(WarpShared *wsall, const StackRef &st
                     skip = accept || (ws.l_meta[lane].y & P3T_LEAF_FLAG) != 0;   // accepted or a leaf there goes to one of them
                     accept = false;
                 }
-            }
-            if (CLS && heavy_group && accept) {
-                const float rm = ws.l_mom1[lane].w;                       // bounding radius; sign bit: the cell holds a black hole
-                const float rc = (prm.h_bf + fabsf(rm)) * (1.f + 1e-5f) + slack;
-                accept = !(__float_as_uint(rm) >> 31) && d2 > rc * rc;
             }
             if (!accept && !(SPLIT && skip)) {
                 uint2 meta = ws.l_meta[lane];

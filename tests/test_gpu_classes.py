@@ -78,7 +78,8 @@ def test_theta0_with_classes_is_the_direct_sum_with_classes(oracle, ngroup, walk
         assert np.array_equal(offd, off) and np.array_equal(nbrd, nbr)
 
 
-@pytest.mark.parametrize("n,extra,ngroup,walk_mode", [(16384, 0, 32, 0), (16384, 0, 64, 1), (30000, 5, 64, 1), (30000, 5, 32, 2)])
+@pytest.mark.parametrize("n,extra,ngroup,walk_mode", [(16384, 0, 32, 0), (16384, 0, 64, 1), (30000, 5, 64, 1), (30000, 5, 32, 2),
+                                                      (30000, 5, 64, 3), (20000, 3, 32, 4)])
 def test_smbh_workload_at_theta_04(oracle, n, extra, ngroup, walk_mode):
     """16K Plummer + two m = 0.01 bodies at (+-0.5, 0, 0), r_cut,FS-FS = 1/256, r_cut,BH-FS = 1/32."""
     cfg = _smbh(n, extra_holes=extra)
@@ -109,10 +110,13 @@ def test_smbh_workload_at_theta_04(oracle, n, extra, ngroup, walk_mode):
         oa, oj, op = oracle.hard_classes(m, q, cfg["vel"].astype(np.float64), cfg["classes"], tab)
         busy = np.abs(oa).sum(1) > 0
         assert set(holes) <= set(np.flatnonzero(busy))
+        # (a pair at the very edge of its cutoff sphere has 1 - K ~ 1e-12, a difference of O(1) numbers: the comparison is
+        #  relative to the particle's own hard force, floored at 1e-4 of the typical one)
         na = np.linalg.norm(oa[busy], axis=1)
-        assert (np.linalg.norm(ah[busy] - oa[busy], axis=1) / na).max() <= 1e-7
-        assert (np.linalg.norm(jh[busy] - oj[busy], axis=1) / np.linalg.norm(oj[busy], axis=1)).max() <= 1e-6
-        assert np.abs(ph[busy] / op[busy] - 1).max() <= 1e-7
+        nj = np.linalg.norm(oj[busy], axis=1)
+        assert (np.linalg.norm(ah[busy] - oa[busy], axis=1) / np.maximum(na, 1e-4 * np.median(na))).max() <= 1e-7
+        assert (np.linalg.norm(jh[busy] - oj[busy], axis=1) / np.maximum(nj, 1e-4 * np.median(nj))).max() <= 1e-6
+        assert (np.abs(ph[busy] - op[busy]) / np.maximum(np.abs(op[busy]), 1e-4 * np.median(np.abs(op[busy])))).max() <= 1e-7
         assert not ah[~busy].any()
         # soft + hard = plain Newton for the holes (unsoftened between them, eps otherwise)
         for i in holes:
@@ -236,3 +240,28 @@ def test_whole_steps_with_classes_conserve_energy():
         assert info["n_nonisolated"] >= 2
     e1 = energy(q.cpu().numpy(), v.cpu().numpy())
     assert abs(e1 / e0 - 1) < 2e-4, (e0, e1)
+
+
+def test_refit_with_classes_keeps_lists_exact(oracle):
+    """Tree reuse with pair classes: the class bytes in key order and the black-hole flags of the cells are those of the
+    last build; boxes and radii are remade from the moved positions, so the lists (kind by kind) stay exact."""
+    cfg = _smbh(20000, extra_holes=4)
+    tab = _tab(oracle, cfg)
+    m = cfg["mass"].astype(np.float64)
+    with _ctx(cfg, walk_mode=1) as ctx:
+        ctx.set_tree_reuse(4, 0.5, 1.0)
+        pos = cfg["pos"].copy()
+        for call in range(3):
+            ctx.load_particles(cfg["mass"], pos)
+            ctx.refit_tree()
+            assert ctx.get_stats()["tree_refits"] == call
+            ctx.eval_soft()
+            acc, pot = ctx.get_acc_pot()
+            off, nbr = ctx.get_neighbours()
+            q = pos.astype(np.float64)
+            a, p = oracle.direct_classes(m, q, cfg["classes"], tab)
+            e = rel_err(acc.astype(np.float64), a)
+            assert np.median(e) <= TOL_MEDIAN and np.percentile(e, 99) <= TOL_P99
+            ooff, olst, band = oracle.neighbours_classes(q, cfg["classes"], tab)
+            assert_same_neighbour_sets(csr_sets(off, nbr), csr_sets(ooff, olst), band)
+            pos = np.ascontiguousarray(pos + np.float32(4 * cfg["dt_soft"]) * cfg["vel"], dtype=np.float32)
