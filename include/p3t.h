@@ -13,7 +13,7 @@
  *   parameter theta (L171, L193).  r_out is the paper's r_cut, r_search its h.
  *
  * All arithmetic runs in hand-written sm_100a CUDA kernels; there is no CPU
- * fallback.  Pair and cell interactions are evaluated in fp32; every 64
+ * fallback.  Pair and cell interactions are evaluated in fp32; every 128
  * interactions the fp32 partial sums are added to fp64 accumulators.
  *
  * Conventions

@@ -22,7 +22,7 @@
 #endif
 // full batches of 32 list entries summed in fp32 before the sums go to the fp64 accumulators
 #ifndef WALK_FLUSH_EVERY
-#define WALK_FLUSH_EVERY 2
+#define WALK_FLUSH_EVERY 4
 #endif
 constexpr int kPpUnroll = WALK_PP_UNROLL, kPcUnroll = WALK_PC_UNROLL;
 
@@ -568,13 +568,15 @@ __device__ __forceinline__ void walk_group(WarpShared *wsall, const StackRef &st
         WP(3);
         // ---- children of opened internal cells -> stack
         {
-            u32 inc = nch;
+            u32 inc = nch, total = 0;
+            if (__any_sync(0xffffffffu, nch != 0)) {      // (a step of accepted cells and leaves only pushes nothing)
 #pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                u32 t = __shfl_up_sync(0xffffffffu, inc, o);
-                if (lane >= o) inc += t;
+                for (int o = 1; o < 32; o <<= 1) {
+                    u32 t = __shfl_up_sync(0xffffffffu, inc, o);
+                    if (lane >= o) inc += t;
+                }
+                total = __shfl_sync(0xffffffffu, inc, 31);
             }
-            u32 total = __shfl_sync(0xffffffffu, inc, 31);
             if (!COOP) {
                 if (top + total > st.limit) { overflow = true; break; }
                 u32 pos = top + inc - nch;
@@ -617,7 +619,7 @@ __device__ __forceinline__ void walk_group(WarpShared *wsall, const StackRef &st
         WP(4);
         // ---- bodies of opened leaves -> near / far rings; the next chunk of 32 bodies is loaded
         //      while the current one is tested and (when a ring fills) evaluated
-        {
+        if (__any_sync(0xffffffffu, lcount != 0)) {      // (steps near the top of the tree open no leaf: no scan then)
             u32 inc = lcount;
 #pragma unroll
             for (int o = 1; o < 32; o <<= 1) {
