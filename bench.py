@@ -401,7 +401,8 @@ def main():
     hbm = {k: ab[k] / (ph["ms_" + k] * 1e-3) / 1e9 for k in ab}
     tree_ms = ph["ms_pack"] + ph["ms_sort"] + ph["ms_build"] + ph["ms_moments"]
     # pack | keys+hist, onesweep passes, gather | levels, emit | moments (leaves, internal) | group prediction + order, walk | neighbour CSR (6)
-    launches = 1 + (1 + st["sort_passes"] + 1) + 2 + 2 + (3 if not shard else 1) + 6 + 1      # ... + unpack (get_acc_pot)
+    launches = 1 + (1 + st["sort_passes"] + 1) + 2 + 2 + 3 + 6 + (2 if shard else 1)      # ... group prediction, order, walk; a9; unpack (sharded: record + class kernels)
+    launches += 1 if st["walk_parts"] > 1 else 0                                              # split walk: the combine kernel
 
     out = {
         "metric": METRIC, "value": multi.throughput(total_n, ms), "unit": "particles/s", "n_gpus": world, "steps": args.steps,
@@ -416,7 +417,7 @@ def main():
         "walk_particles_per_s": n / (ph["ms_walk"] * 1e-3),
         "interactions": {"n_pp": st["n_pp"], "n_pc": st["n_pc"], "n_near": st["n_near"], "n_neighbours": st["n_neighbours"],
                          "pp_per_particle": st["n_pp"] / n, "pc_per_particle": st["n_pc"] / n},
-        "tree": {"n_cells": st["n_cells"], "n_leaves": st["n_leaves"], "n_groups": st["n_groups"], "depth": st["depth"], "histograms": tree_hist},
+        "walk_parts": st["walk_parts"], "tree": {"n_cells": st["n_cells"], "n_leaves": st["n_leaves"], "n_groups": st["n_groups"], "depth": st["depth"], "histograms": tree_hist},
         "same_positions": same_ms,
         "neighbour_lists": nbr_hist, "workspace_bytes": int(ctx.workspace.numel()),
         "phases_ms": ph,

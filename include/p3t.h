@@ -76,6 +76,8 @@ typedef struct {
     float ms_pack;           /* a1: pack + bounding cube of the last p3t_load_particles (after any host-to-device copy) */
     uint32_t tree_refits;    /* p3t_refit_tree: refits since the last full build (0: the current tree is a fresh build) */
     uint32_t n_stray;        /* of the current refit: bodies outside the cube of their leaf by more than stray_dist leaf sides */
+    uint32_t walk_parts;     /* how the last walk mapped groups to warps: 1 one warp per group, 2 / 4 split walk, 0 one CTA per group */
+    uint32_t pad_;
 } p3t_stats;
 
 /* Bytes of device workspace p3t_create needs for up to max_n particles,

@@ -47,7 +47,7 @@ class Stats(C.Structure):
                 ("n_groups", C.c_uint32), ("depth", C.c_uint32), ("max_list", C.c_uint32),
                 ("sort_passes", C.c_uint32), ("ms_sort", C.c_float), ("ms_build", C.c_float),
                 ("ms_moments", C.c_float), ("ms_walk", C.c_float), ("ms_nbr", C.c_float), ("ms_hard", C.c_float), ("ms_pack", C.c_float),
-                ("tree_refits", C.c_uint32), ("n_stray", C.c_uint32)]
+                ("tree_refits", C.c_uint32), ("n_stray", C.c_uint32), ("walk_parts", C.c_uint32), ("pad_", C.c_uint32)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}

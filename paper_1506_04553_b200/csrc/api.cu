@@ -824,6 +824,7 @@ extern "C" p3t_status p3t_get_stats(p3t_ctx *ctx, p3t_stats *out)
     }
     if (ctx->ev_hard) cudaEventElapsedTime(&out->ms_hard, ctx->ev[7], ctx->ev[8]);
     if (ctx->ev_pack) cudaEventElapsedTime(&out->ms_pack, ctx->ev[9], ctx->ev[10]);
+    out->walk_parts = (u32)ctx->walk_parts_used;
     out->tree_refits = (u32)ctx->refits;
     out->n_stray = (u32)(ctx->last_rebuilt ? 0 : ctx->last_stray);
     return st;

@@ -160,6 +160,7 @@ struct p3t_ctx {
     size_t max_n, n, nbr_capacity;
     int key_bits, max_level, nleaf, ngroup, merge_levels;
     int key_curve;                 // 0 Morton, 1 Peano-Hilbert (default)
+    int walk_parts_used;           // of the last walk: 1, 2, 4 (split) or 0 (cooperative)
     bool merge_user_set;           // p3t_set_group_merge_levels was called: p3t_set_key_curve keeps its value
     int herm_cluster_max;          // largest component a thread-block cluster integrates (larger ones: grid kernel)
     int walk_mode;                 // 0 auto, 1 one warp per group, 2 one CTA per group (cooperative)

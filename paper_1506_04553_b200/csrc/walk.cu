@@ -1089,6 +1089,7 @@ p3t_status p3t_stage_walk(p3t_ctx *ctx)
     }
     if (ctx->shard_world > 1 || coop) nparts = 1;
     A.nparts = nparts;
+    ctx->walk_parts_used = coop ? 0 : (int)nparts;
     A.level_total = w.level_total;
     A.split_acc = reinterpret_cast<float4 *>(w.hard_out);          // 48 n bytes of the 56 n (free until p3t_eval_hard)
     A.split_cnt = reinterpret_cast<u32 *>(w.herm_state);           // 12 n bytes of 96 n (free until p3t_hermite_step)
