@@ -72,6 +72,7 @@ p3t_status p3t_stage_direct(p3t_ctx *ctx, const u32 *d_subset, size_t n_subset)
     P3T_CUDA(ctx, cudaMemsetAsync(w.counters + CNT_NPP, 0, 8 * sizeof(u64), s));
     P3T_CUDA(ctx, cudaMemsetAsync(w.accpot, 0, (size_t)n * sizeof(float4), s));
     P3T_CUDA(ctx, cudaMemsetAsync(w.nbr_count, 0, (size_t)n * sizeof(u32), s));
+    P3T_CUDA(ctx, cudaMemsetAsync(w.nbr_cursor, 0, (size_t)n * sizeof(u32), s));   // scatter cursors of the neighbour stage
     direct_kernel<<<div_up(n_subset, DIRECT_THREADS), DIRECT_THREADS, 0, s>>>(w.body_user, n, d_subset, (u32)n_subset, ctx->prm,
                                                                               w.accpot, w.nbr_count, w.pairs,
                                                                               (u64)ctx->nbr_capacity, w.counters,

@@ -33,6 +33,8 @@ __device__ __forceinline__ u32 block_exclusive_scan(u32 v, u32 *s_w, u32 &total)
 
 __global__ void __launch_bounds__(SCAN_THREADS) scan_tile_sums_kernel(const u32 *__restrict__ count, u32 n, u64 *tile_sum)
 {
+    P3T_GRID_TRIGGER();
+    P3T_GRID_WAIT();
     __shared__ u32 s_w[SCAN_THREADS / 32];
     u32 base = blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_ITEMS;
     u32 v = 0;
@@ -47,6 +49,8 @@ __global__ void __launch_bounds__(SCAN_THREADS) scan_tile_sums_kernel(const u32 
 // single block: exclusive scan of the tile sums in place (64-bit)
 __global__ void __launch_bounds__(1024) scan_tile_prefix_kernel(u64 *tile_sum, u32 ntiles)
 {
+    P3T_GRID_TRIGGER();
+    P3T_GRID_WAIT();
     __shared__ u64 s_w[32];
     __shared__ u64 s_carry;
     const u32 tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -76,6 +80,8 @@ __global__ void __launch_bounds__(SCAN_THREADS) scan_apply_kernel(const u32 *__r
                                                                   const u64 *__restrict__ tile_sum, u64 *__restrict__ offset,
                                                                   u64 *counters)
 {
+    P3T_GRID_TRIGGER();
+    P3T_GRID_WAIT();
     __shared__ u32 s_w[SCAN_THREADS / 32];
     u32 base = blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_ITEMS;
     u32 c[SCAN_ITEMS], v = 0, mx = 0;
@@ -102,6 +108,8 @@ __global__ void __launch_bounds__(256) fill_lists_kernel(const uint2 *__restrict
                                                          const u64 *__restrict__ offset, u32 *cursor, u32 *__restrict__ nbr,
                                                          const u64 *__restrict__ counters)
 {
+    P3T_GRID_TRIGGER();
+    P3T_GRID_WAIT();
     u64 total = counters[CNT_PAIRS];
     if (total > pair_cap) return;   // over capacity: lists are not materialised (P3T_ECAPACITY at fetch)
     for (u64 p = (u64)blockIdx.x * blockDim.x + threadIdx.x; p < total; p += (u64)gridDim.x * blockDim.x) {
@@ -119,6 +127,8 @@ __global__ void __launch_bounds__(256) fill_lists_kernel(const uint2 *__restrict
 __global__ void __launch_bounds__(256) sort_lists_kernel(const u32 *__restrict__ count, const u64 *__restrict__ offset, u32 n,
                                                          u32 *nbr, u64 pair_cap, u64 *counters, u32 *worklist)
 {
+    P3T_GRID_TRIGGER();
+    P3T_GRID_WAIT();
     if (counters[CNT_PAIRS] > pair_cap) return;
     u32 i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
@@ -144,6 +154,8 @@ __global__ void __launch_bounds__(256) sort_long_lists_kernel(const u32 *__restr
                                                               u32 *nbr, u32 *scratch, const u64 *__restrict__ counters,
                                                               const u32 *__restrict__ worklist)
 {
+    P3T_GRID_TRIGGER();
+    P3T_GRID_WAIT();
     const u32 nlong = (u32)counters[CNT_EVAL_SPARE];
     const u32 lane = threadIdx.x & 31, nwarps = gridDim.x * (blockDim.x >> 5);
     for (u32 wk = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); wk < nlong; wk += nwarps) {
@@ -168,18 +180,22 @@ p3t_status p3t_stage_neighbours(p3t_ctx *ctx)
     cudaStream_t s = ctx->stream;
     u32 n = (u32)ctx->n;
     u32 ntiles = div_up(n, SCAN_TILE);
-    scan_tile_sums_kernel<<<ntiles, SCAN_THREADS, 0, s>>>(w.nbr_count, n, w.scan_tmp);
-    scan_tile_prefix_kernel<<<1, 1024, 0, s>>>(w.scan_tmp, ntiles);
-    scan_apply_kernel<<<ntiles, SCAN_THREADS, 0, s>>>(w.nbr_count, n, w.scan_tmp, w.nbr_offset, w.counters);
+    // (programmatic dependent launch along the stage; the scatter cursors were zeroed by p3t_stage_walk / p3t_stage_direct, in
+    //  front of the evaluation, so that no memset breaks the chain)
+    P3T_CUDA(ctx, p3t_launch_pdl(scan_tile_sums_kernel, dim3(ntiles), dim3(SCAN_THREADS), 0, s, (const u32 *)w.nbr_count, n, w.scan_tmp));
+    P3T_CUDA(ctx, p3t_launch_pdl(scan_tile_prefix_kernel, dim3(1), dim3(1024), 0, s, w.scan_tmp, ntiles));
+    P3T_CUDA(ctx, p3t_launch_pdl(scan_apply_kernel, dim3(ntiles), dim3(SCAN_THREADS), 0, s, (const u32 *)w.nbr_count, n, (const u64 *)w.scan_tmp,
+                                 w.nbr_offset, w.counters));
     if (ctx->nbr_capacity) {
-        P3T_CUDA(ctx, cudaMemsetAsync(w.nbr_cursor, 0, (size_t)n * sizeof(u32), s));
         u32 grid = (u32)ctx->sm_count * 4;
-        fill_lists_kernel<<<grid, 256, 0, s>>>(w.pairs, (u64)ctx->nbr_capacity, w.nbr_offset, w.nbr_cursor, w.nbr, w.counters);
+        P3T_CUDA(ctx, p3t_launch_pdl(fill_lists_kernel, dim3(grid), dim3(256), 0, s, (const uint2 *)w.pairs, (u64)ctx->nbr_capacity,
+                                     (const u64 *)w.nbr_offset, w.nbr_cursor, w.nbr, (const u64 *)w.counters));
         // the scatter cursors are dead after the fill: they hold the queue of long lists; the pair buffer is the scratch copy
-        sort_lists_kernel<<<div_up(n, 256), 256, 0, s>>>(w.nbr_count, w.nbr_offset, n, w.nbr, (u64)ctx->nbr_capacity, w.counters,
-                                                         w.nbr_cursor);
-        sort_long_lists_kernel<<<(u32)ctx->sm_count * 2, 256, 0, s>>>(w.nbr_count, w.nbr_offset, w.nbr, reinterpret_cast<u32 *>(w.pairs),
-                                                                       w.counters, w.nbr_cursor);
+        P3T_CUDA(ctx, p3t_launch_pdl(sort_lists_kernel, dim3(div_up(n, 256)), dim3(256), 0, s, (const u32 *)w.nbr_count, (const u64 *)w.nbr_offset, n,
+                                     w.nbr, (u64)ctx->nbr_capacity, w.counters, w.nbr_cursor));
+        P3T_CUDA(ctx, p3t_launch_pdl(sort_long_lists_kernel, dim3((u32)ctx->sm_count * 2), dim3(256), 0, s, (const u32 *)w.nbr_count,
+                                     (const u64 *)w.nbr_offset, w.nbr, reinterpret_cast<u32 *>(w.pairs), (const u64 *)w.counters,
+                                     (const u32 *)w.nbr_cursor));
     }
     P3T_CUDA(ctx, cudaGetLastError());
     return P3T_OK;

@@ -68,6 +68,8 @@ p3t_status p3t_stage_pack(p3t_ctx *ctx, const float *d_mass, const float *d_pos)
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) unpack_kernel(const float4 *__restrict__ ap, float *acc, float *pot, u32 n)
 {
+    P3T_GRID_TRIGGER();
+    P3T_GRID_WAIT();
     u32 i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     float4 v = ap[i];
@@ -79,8 +81,7 @@ p3t_status p3t_stage_unpack(p3t_ctx *ctx, float *d_acc, float *d_pot)
 {
     u32 n = (u32)ctx->n;
     if (!d_acc && !d_pot) return P3T_OK;
-    unpack_kernel<<<div_up(n, 256), 256, 0, ctx->stream>>>(ctx->ws.accpot, d_acc, d_pot, n);
-    P3T_CUDA(ctx, cudaGetLastError());
+    P3T_CUDA(ctx, p3t_launch_pdl(unpack_kernel, dim3(div_up(n, 256)), dim3(256), 0, ctx->stream, (const float4 *)ctx->ws.accpot, d_acc, d_pot, n));
     return P3T_OK;
 }
 

@@ -1029,6 +1029,7 @@ p3t_status p3t_stage_walk(p3t_ctx *ctx)
     cudaStream_t s = ctx->stream;
     // eval counters + cost-class counts and scatter cursors of the group order: contiguous, one memset
     P3T_CUDA(ctx, cudaMemsetAsync(w.counters + CNT_NPP, 0, 8 * sizeof(u64) + 2 * ORDER_CLASSES * sizeof(u32), s));
+    P3T_CUDA(ctx, cudaMemsetAsync(w.nbr_cursor, 0, ctx->n * sizeof(u32), s));     // scatter cursors of the neighbour stage (no memset inside its chain)
     u32 grid = (u32)ctx->sm_count * WALK_CTAS;
     if ((size_t)grid * WALK_WARPS > w.walk_warps_max) grid = (u32)(w.walk_warps_max / WALK_WARPS);
     const size_t smem = (sizeof(WarpShared) + WALK_STACK_SMEM * sizeof(u32)) * WALK_WARPS + sizeof(CtaCtl);
