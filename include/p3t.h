@@ -317,7 +317,7 @@ const char *p3t_last_error(const p3t_ctx *ctx);
  * register-operand bandwidth test of profiles/ffma2_operand_bandwidth_r1.md) of `iters` outer
  * iterations on the context's stream, synchronises, and returns the best of four timed
  * launches as TFLOP/s (2 flop per fp32 FMA) in *tflops [host] and its duration in *ms
- * [host, nullable].  P3T_EINVAL for null ctx/tflops, iters <= 0 or packed outside 0..4. */
+ * [host, nullable].  P3T_EINVAL for null ctx/tflops, iters <= 0 or packed outside 0..7 (5, 6: the operand patterns of modes 2, 3 issued as scalar FFMAs; 7: mode 2 with one source shared by consecutive instructions). */
 p3t_status p3t_measure_fp32_peak(p3t_ctx *ctx, int packed, int iters, double *tflops, float *ms);
 
 /* Latency probes behind the floor table of the a1-a6 chain (profiles/tree_latency_floor_r2.md; not part of the hot path):

@@ -5,6 +5,9 @@
 //   2: three distinct register pairs        v = w * u + v     (measured 2/3 of the rate of mode 1)
 //   3: pair * scalar-broadcast + pair       v = w * s + v     (SASS operand Rs.F32)
 //   4: two distinct register pairs          v = w * w + v
+//   5: mode 2 as two scalar FFMAs            v.x = w.x * u.x + v.x, v.y likewise (three distinct registers each)
+//   6: mode 3 as two scalar FFMAs            v.x = w.x * s + v.x,   v.y likewise
+//   7: mode 2 with the first source shared by eight consecutive instructions (operand reuse cache: SASS .reuse)
 // which is what decides the layout of the interaction lists in walk.cu.
 // Not part of the hot path; bench.py quotes modes 0 and 1 beside the nominal peak.
 #include "p3t_internal.cuh"
@@ -16,6 +19,12 @@ __device__ __forceinline__ u64 calib_ffma2(u64 a, u64 b, u64 c)
 {
     u64 d;
     asm volatile("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+__device__ __forceinline__ float calib_ffma(float a, float b, float c)
+{
+    float d;
+    asm volatile("fma.rn.f32 %0, %1, %2, %3;" : "=f"(d) : "f"(a), "f"(b), "f"(c));
     return d;
 }
 __device__ __forceinline__ u64 calib_pack(float x, float y)
@@ -46,12 +55,41 @@ __global__ void __launch_bounds__(128, 4) ffma2_operand_kernel(float *out, int i
                 if (MODE == 2) v[k] = calib_ffma2(w[k], u[k], v[k]);
                 if (MODE == 3) v[k] = calib_ffma2(w[k], calib_pack(sc[k], sc[k]), v[k]);
                 if (MODE == 4) v[k] = calib_ffma2(w[k], w[k], v[k]);
+                if (MODE == 7) v[k] = calib_ffma2(w[r & 7], u[k], v[k]);
             }
         }
     }
     float s = 0.f;
 #pragma unroll
     for (int k = 0; k < 8; ++k) s += __uint_as_float((u32)v[k]) + __uint_as_float((u32)(v[k] >> 32));
+    if (s == 123.456f) out[0] = s;
+}
+
+// the same operand patterns issued as scalar FFMAs (two per packed operation)
+template <int MODE>
+__global__ void __launch_bounds__(128, 4) ffma_operand_kernel(float *out, int iters, float a, float b)
+{
+    float vx[8], vy[8], wx[8], wy[8], ux[8], uy[8], sc[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        vx[k] = threadIdx.x * b + k, vy[k] = 1.f + k;
+        wx[k] = a + k * b, wy[k] = a - b * threadIdx.x * (k + 1);
+        ux[k] = b * (k + 1), uy[k] = b * threadIdx.x + k;
+        sc[k] = a - b * (k + threadIdx.x);
+    }
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int r = 0; r < CALIB_INNER * 2; ++r) {
+#pragma unroll
+            for (int k = 0; k < 8; ++k) {
+                if (MODE == 5) { vx[k] = calib_ffma(wx[k], ux[k], vx[k]); vy[k] = calib_ffma(wy[k], uy[k], vy[k]); }
+                if (MODE == 6) { vx[k] = calib_ffma(wx[k], sc[k], vx[k]); vy[k] = calib_ffma(wy[k], sc[k], vy[k]); }
+            }
+        }
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) s += vx[k] + vy[k];
     if (s == 123.456f) out[0] = s;
 }
 
@@ -82,7 +120,7 @@ extern "C" p3t_status p3t_measure_fp32_peak(p3t_ctx *ctx, int packed, int iters,
 {
     if (!ctx || !tflops || iters <= 0) return p3t_fail(ctx, P3T_EINVAL, "p3t_measure_fp32_peak: bad argument");
     cudaStream_t s = ctx->stream;
-    if (packed < 0 || packed > 4) return p3t_fail(ctx, P3T_EINVAL, "p3t_measure_fp32_peak: mode must be 0..4");
+    if (packed < 0 || packed > 7) return p3t_fail(ctx, P3T_EINVAL, "p3t_measure_fp32_peak: mode must be 0..7");
     const int grid = packed >= 2 ? ctx->sm_count * 16 : ctx->sm_count * 8, block = packed >= 2 ? 128 : 256;
     cudaEvent_t e0, e1;
     P3T_CUDA(ctx, cudaEventCreate(&e0));
@@ -95,7 +133,10 @@ extern "C" p3t_status p3t_measure_fp32_peak(p3t_ctx *ctx, int packed, int iters,
         else if (packed == 0) ffma_peak_kernel<0><<<grid, block, 0, s>>>(out, iters, 0.999f, 1e-3f);
         else if (packed == 2) ffma2_operand_kernel<2><<<grid, block, 0, s>>>(out, iters, 0.999f, 1e-3f);
         else if (packed == 3) ffma2_operand_kernel<3><<<grid, block, 0, s>>>(out, iters, 0.999f, 1e-3f);
-        else ffma2_operand_kernel<4><<<grid, block, 0, s>>>(out, iters, 0.999f, 1e-3f);
+        else if (packed == 4) ffma2_operand_kernel<4><<<grid, block, 0, s>>>(out, iters, 0.999f, 1e-3f);
+        else if (packed == 5) ffma_operand_kernel<5><<<grid, block, 0, s>>>(out, iters, 0.999f, 1e-3f);
+        else if (packed == 6) ffma_operand_kernel<6><<<grid, block, 0, s>>>(out, iters, 0.999f, 1e-3f);
+        else ffma2_operand_kernel<7><<<grid, block, 0, s>>>(out, iters, 0.999f, 1e-3f);
         P3T_CUDA(ctx, cudaEventRecord(e1, s));
         P3T_CUDA(ctx, cudaEventSynchronize(e1));
         float ms = 0.f;
@@ -105,7 +146,7 @@ extern "C" p3t_status p3t_measure_fp32_peak(p3t_ctx *ctx, int packed, int iters,
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
     P3T_CUDA(ctx, cudaGetLastError());
-    // modes 0/1: 16 chains x 64 packed ops; modes 2-4: 8 chains x 128 packed ops per outer iteration
+    // modes 0/1: 16 chains x 64 packed ops; modes 2-6: 8 chains x 128 packed ops (or pairs of scalar ops) per outer iteration
     double flop = 2.0 * 2.0 * CALIB_CHAINS * CALIB_INNER * (double)iters * (double)grid * block;
     *tflops = flop / (best * 1e-3) / 1e12;
     if (ms_out) *ms_out = best;

@@ -18,7 +18,7 @@
 #define WALK_PP_UNROLL 8
 #endif
 #ifndef WALK_PC_UNROLL
-#define WALK_PC_UNROLL 8
+#define WALK_PC_UNROLL 2
 #endif
 // full batches of 32 list entries summed in fp32 before the sums go to the fp64 accumulators
 #ifndef WALK_FLUSH_EVERY
@@ -252,17 +252,18 @@ __device__ __forceinline__ void eval_pc(const WarpShared &ws, u32 head, u32 cnt,
         V r3i = vmul(r2i, rinv);
         V r4i = vmul(r2i, r2i);
         V n5 = vmul(r3i, vmul(cm04, r2i));                          // -0.4 / s^5
-        V qdx = vfma(qxx, dx, vfma(qxy, dy, vmul(qxz, dz)));
-        V qdy = vfma(qxy, dx, vfma(qyy, dy, vmul(qyz, dz)));
-        V qdz = vfma(qxz, dx, vfma(qyz, dy, vmul(qzz, dz)));
+        // (source order: the three lines of Q5 d by shared operand, then the accumulator updates by shared factor -- ptxas keeps
+        // part of it, and consecutive packed instructions that share a source register read it once: SASS .reuse)
+        V qdx = vmul(qxz, dz), qdy = vmul(qyz, dz), qdz = vmul(qzz, dz);
+        qdx = vfma(qxy, dy, qdx); qdy = vfma(qyy, dy, qdy); qdz = vfma(qyz, dy, qdz);
+        qdx = vfma(qxx, dx, qdx); qdy = vfma(qxy, dx, qdy); qdz = vfma(qxz, dx, qdz);
         V T = vfma(dx, qdx, vfma(dy, qdy, vfma(dz, qdz, vdup<V>(P2.z))));
+        acc.ax = vfma(n5, qdx, acc.ax); acc.ay = vfma(n5, qdy, acc.ay); acc.az = vfma(n5, qdz, acc.az);
         V c1 = vfma(T, r4i, M);
         V pphi = vfma(c02, c1, vdup<V>(P2.w));
         V coef = vmul(c1, r3i);
+        acc.ax = vfma(coef, dx, acc.ax); acc.ay = vfma(coef, dy, acc.ay); acc.az = vfma(coef, dz, acc.az);
         acc.ph = vfma(pphi, rinv, acc.ph);
-        acc.ax = vfma(coef, dx, vfma(n5, qdx, acc.ax));
-        acc.ay = vfma(coef, dy, vfma(n5, qdy, acc.ay));
-        acc.az = vfma(coef, dz, vfma(n5, qdz, acc.az));
     }
     acc.flush_lazy();
 }
@@ -879,7 +880,14 @@ walk_kernel(WalkArgs A, const u32 *__restrict__ group_start, P3TParams prm, u32 
             u32 c = 0;
             if (lane == 0) {
                 const u32 lpp = len_pp * sr.nparts, lpc = len_pc * sr.nparts;
+#ifdef P3T_DIAG_SLOT
+                u32 smid_, wid_;
+                asm volatile("mov.u32 %0, %%smid;" : "=r"(smid_));
+                asm volatile("mov.u32 %0, %%warpid;" : "=r"(wid_));
+                A.group_stats[g] = make_uint4((smid_ << 16) | (wid_ << 8) | ((blockIdx.x / 148u) << 4) | warp, 26 * lpp / 66 + lpc, t0, (u32)globaltimer_ns());
+#else
                 A.group_stats[g] = make_uint4(lpp, lpc, t0, (u32)globaltimer_ns());
+#endif
                 c = cost_class(lpp, lpc, ge - gs > 32);
             }
             c = __shfl_sync(0xffffffffu, c, 0);
