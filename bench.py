@@ -158,6 +158,7 @@ def main():
     ap.add_argument("--ngroup", type=int, default=None)
     ap.add_argument("--merge", type=int, default=None)
     ap.add_argument("--curve", default=None, choices=["morton", "hilbert"], help="p3t_set_key_curve (default: the library's, hilbert)")
+    ap.add_argument("--sort-passes", type=int, default=0, help="p3t_set_sort_passes (default 0: the library's plan)")
     ap.add_argument("--shard", action="store_true",
                     help="strong scaling: ONE cluster, every rank walks every world-th i-group (p3t_set_shard) and the "
                          "accelerations and potentials are summed over the ranks (NCCL all-reduce inside the timed step)")
@@ -203,6 +204,8 @@ def main():
     ctx.set_tree_params(nleaf, ngroup)
     if args.curve is not None:
         ctx.set_key_curve(args.curve)
+    if args.sort_passes:
+        ctx.set_sort_passes(args.sort_passes)
     if args.merge is not None:
         ctx.set_group_merge_levels(args.merge)
     if args.walk_mode is not None:
@@ -401,7 +404,7 @@ def main():
     hbm = {k: ab[k] / (ph["ms_" + k] * 1e-3) / 1e9 for k in ab}
     tree_ms = ph["ms_pack"] + ph["ms_sort"] + ph["ms_build"] + ph["ms_moments"]
     # pack | keys+hist, onesweep passes, gather | levels, emit | moments (leaves, internal) | group prediction + order, walk | neighbour CSR (6)
-    launches = 1 + (1 + st["sort_passes"] + 1) + 2 + 2 + 3 + 6 + (2 if shard else 1)      # ... group prediction, order, walk; a9; unpack (sharded: record + class kernels)
+    launches = 1 + (1 + st["sort_passes"] + (2 if st["sort_passes"] < (8 if cfg["key_bits"] == 63 else 4) else 0) + 1) + 2 + 2 + 3 + 6 + (2 if shard else 1)      # ... group prediction, order, walk; a9; unpack (sharded: record + class kernels)
     launches += 1 if st["walk_parts"] > 1 else 0                                              # split walk: the combine kernel
 
     out = {
@@ -417,7 +420,7 @@ def main():
         "walk_particles_per_s": n / (ph["ms_walk"] * 1e-3),
         "interactions": {"n_pp": st["n_pp"], "n_pc": st["n_pc"], "n_near": st["n_near"], "n_neighbours": st["n_neighbours"],
                          "pp_per_particle": st["n_pp"] / n, "pc_per_particle": st["n_pc"] / n},
-        "walk_parts": st["walk_parts"], "tree": {"n_cells": st["n_cells"], "n_leaves": st["n_leaves"], "n_groups": st["n_groups"], "depth": st["depth"], "histograms": tree_hist},
+        "walk_parts": st["walk_parts"], "sort_passes": st["sort_passes"], "sort_max_run": st["sort_max_run"], "tree": {"n_cells": st["n_cells"], "n_leaves": st["n_leaves"], "n_groups": st["n_groups"], "depth": st["depth"], "histograms": tree_hist},
         "same_positions": same_ms,
         "neighbour_lists": nbr_hist, "workspace_bytes": int(ctx.workspace.numel()),
         "phases_ms": ph,
@@ -429,7 +432,11 @@ def main():
                      "frac_of_ffma_microbench": walk_tflops / max(ffma_scalar, ffma_packed)},
         "roofline_hbm": {"bound": "hbm", "passes": "a1-a6 (sort, build, moments)", "achieved": sum(ab.values()) / (tree_ms * 1e-3) / 1e9,
                          "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": sum(ab.values()) / (tree_ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
-                         "per_pass_gbs": hbm, "algorithmic_bytes": ab, "peak_source": peaks["source"]},
+                         "per_pass_gbs": hbm, "algorithmic_bytes": ab, "peak_source": peaks["source"],
+                         # the byte count is SURVEY.md 8(d)'s (an LSD sort of all digits); the build sorts the upper digits by
+                         # radix passes and finishes short runs in place (p3t_set_sort_passes), so it MOVES less than it is booked for
+                         "radix_passes_booked": 8 if cfg["key_bits"] == 63 else 4, "radix_passes_run": st["sort_passes"],
+                         "moved_gbs": (sum(ab.values()) - (((8 if cfg["key_bits"] == 63 else 4) - st["sort_passes"]) * 24 * n)) / (tree_ms * 1e-3) / 1e9},
         "tree_reuse": ({"max_refits": args.refit, "tree_refits_at_end": st["tree_refits"], "n_stray": st["n_stray"]} if args.refit else None),
         "clocks": clocks, "gpu_launches": launches * args.steps, "gpu_launches_per_step": launches,
     }

@@ -66,7 +66,7 @@ typedef struct {
     uint32_t n_groups;       /* i-groups walked (one warp each) */
     uint32_t depth;          /* deepest level in use (root = 0) */
     uint32_t max_list;       /* longest neighbour list */
-    uint32_t sort_passes;    /* radix passes of the build (8-bit digits: 8 for 63-bit keys, 4 for 30-bit keys) */
+    uint32_t sort_passes;    /* radix passes of the last build (8-bit digits; at most 8 for 63-bit keys, 4 for 30-bit keys: p3t_set_sort_passes) */
     float ms_sort;           /* a1-a4: bounding cube, keys, radix sort, gather */
     float ms_build;          /* a5: octree + groups */
     float ms_moments;        /* a6 */
@@ -77,7 +77,8 @@ typedef struct {
     uint32_t tree_refits;    /* p3t_refit_tree: refits since the last full build (0: the current tree is a fresh build) */
     uint32_t n_stray;        /* of the current refit: bodies outside the cube of their leaf by more than stray_dist leaf sides */
     uint32_t walk_parts;     /* how the last walk mapped groups to warps: 1 one warp per group, 2 / 4 split walk, 0 one CTA per group */
-    uint32_t pad_;
+    uint32_t sort_max_run;   /* last build, if it sorted the upper key bits only: longest run of keys equal on them that the
+                                finishing step had to sort, 0 if none was longer than 16 */
 } p3t_stats;
 
 /* Bytes of device workspace p3t_create needs for up to max_n particles,
@@ -135,6 +136,16 @@ p3t_status p3t_set_tree_params(p3t_ctx *ctx, int nleaf, int ngroup);
  * ngroup consecutive bodies with full warps and tight boxes (A25, section 7).  Invalidates a built tree.
  * P3T_EINVAL for another value. */
 p3t_status p3t_set_key_curve(p3t_ctx *ctx, int curve);
+
+/* Radix passes of the sort (row a3).  The result of a build is always the stable order of the full keys.  passes = 0
+ * (default): the library sorts only the upper digits by radix passes -- as many bits as the tree is expected to be deep,
+ * log2 n + 14, eight more after every build whose statistics (read at the next synchronising call) show a run above 24
+ * keys -- and finishes the runs of keys that agree on those bits in place (insertion sort by one thread up to 32 keys,
+ * one CTA per longer run): the same permutation with 4 or 5 passes instead of 8 for the workloads of BASELINE.json.
+ * passes = 1..8: that many of the upper digits by radix passes (8 with 63-bit keys, 4 or more with 30-bit keys: all of
+ * them, no finishing step).  30-bit keys always take their 4 passes by default.  Invalidates a built tree.
+ * P3T_EINVAL for a value outside 0..8. */
+p3t_status p3t_set_sort_passes(p3t_ctx *ctx, int passes);
 
 /* Inspection (host only, no GPU involved): the state tables the key kernel uses for Peano-Hilbert keys, derived by the
  * library from Skilling's transform on a 32^3 lattice.  tab[state * 64 + two octants] = next state << 6 | two key digits

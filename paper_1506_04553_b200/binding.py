@@ -28,7 +28,7 @@ _STATUS = {0: "P3T_OK", -1: "P3T_EINVAL", -2: "P3T_ESTATE", -3: "P3T_ENOMEM", -4
 # names of include/p3t.h's exported entry points (tests check that each resolves)
 SYMBOLS = [
     "p3t_workspace_bytes", "p3t_create", "p3t_destroy", "p3t_set_params", "p3t_set_tree_params",
-    "p3t_set_pair_classes", "p3t_set_key_curve", "p3t_hilbert_state_tables", "p3t_set_group_merge_levels", "p3t_set_walk_mode", "p3t_set_shard", "p3t_get_shard_record", "p3t_put_shard_classes", "p3t_load_particles", "p3t_build_tree", "p3t_set_tree_reuse", "p3t_refit_tree", "p3t_eval_soft", "p3t_eval_direct", "p3t_eval_hard",
+    "p3t_set_pair_classes", "p3t_set_key_curve", "p3t_set_sort_passes", "p3t_hilbert_state_tables", "p3t_set_group_merge_levels", "p3t_set_walk_mode", "p3t_set_shard", "p3t_get_shard_record", "p3t_put_shard_classes", "p3t_load_particles", "p3t_build_tree", "p3t_set_tree_reuse", "p3t_refit_tree", "p3t_eval_soft", "p3t_eval_direct", "p3t_eval_hard",
     "p3t_hermite_step", "p3t_step", "p3t_set_hermite_cluster_max", "p3t_set_hermite_class_params",
     "p3t_get_acc_pot", "p3t_get_neighbour_counts", "p3t_get_neighbours", "p3t_get_stats", "p3t_synchronize",
     "p3t_last_error", "p3t_array_info", "p3t_copy_array", "p3t_measure_fp32_peak", "p3t_measure_latency",
@@ -47,7 +47,7 @@ class Stats(C.Structure):
                 ("n_groups", C.c_uint32), ("depth", C.c_uint32), ("max_list", C.c_uint32),
                 ("sort_passes", C.c_uint32), ("ms_sort", C.c_float), ("ms_build", C.c_float),
                 ("ms_moments", C.c_float), ("ms_walk", C.c_float), ("ms_nbr", C.c_float), ("ms_hard", C.c_float), ("ms_pack", C.c_float),
-                ("tree_refits", C.c_uint32), ("n_stray", C.c_uint32), ("walk_parts", C.c_uint32), ("pad_", C.c_uint32)]
+                ("tree_refits", C.c_uint32), ("n_stray", C.c_uint32), ("walk_parts", C.c_uint32), ("sort_max_run", C.c_uint32)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
@@ -71,6 +71,7 @@ def _sig():
     L.p3t_set_tree_params.restype = i; L.p3t_set_tree_params.argtypes = [vp, i, i]
     L.p3t_set_pair_classes.restype = i; L.p3t_set_pair_classes.argtypes = [vp, sz, vp, i, f, f, f, f]
     L.p3t_set_group_merge_levels.restype = i; L.p3t_set_group_merge_levels.argtypes = [vp, i]
+    L.p3t_set_sort_passes.restype = i; L.p3t_set_sort_passes.argtypes = [vp, i]
     L.p3t_set_key_curve.restype = i; L.p3t_set_key_curve.argtypes = [vp, i]
     L.p3t_hilbert_state_tables.restype = i; L.p3t_hilbert_state_tables.argtypes = [vp, sz]
     L.p3t_set_walk_mode.restype = i; L.p3t_set_walk_mode.argtypes = [vp, i]
@@ -206,6 +207,9 @@ class P3T:
         """'morton' / 0 or 'hilbert' / 1 (default)."""
         c = {"morton": 0, "hilbert": 1}.get(curve, curve)
         self._check(_lib.p3t_set_key_curve(self._h, int(c)))
+
+    def set_sort_passes(self, passes):
+        self._check(_lib.p3t_set_sort_passes(self._h, int(passes)))
 
     def set_group_merge_levels(self, levels):
         self._check(_lib.p3t_set_group_merge_levels(self._h, levels))

@@ -330,6 +330,16 @@ extern "C" p3t_status p3t_set_key_curve(p3t_ctx *ctx, int curve)
     return P3T_OK;
 }
 
+extern "C" p3t_status p3t_set_sort_passes(p3t_ctx *ctx, int passes)
+{
+    if (!ctx || passes < 0 || passes > 8) return P3T_EINVAL;
+    ctx->sort_passes_user = passes;
+    ctx->built = false;
+    ctx->evaluated = false;
+    ctx->topo_valid = false;
+    return P3T_OK;
+}
+
 extern "C" p3t_status p3t_hilbert_state_tables(uint32_t *tab, size_t words)
 {
     if (!tab || words < P3T_HILBERT_TAB_WORDS) return P3T_EINVAL;
@@ -730,6 +740,13 @@ static p3t_status sync_and_check(p3t_ctx *ctx)
     if (ctx->h_counters[CNT_NONFINITE]) return p3t_fail(ctx, P3T_EINVAL, "non-finite mass or position in the device input");
     u64 f = ctx->h_counters[CNT_ERR_BUILD] | ctx->h_counters[CNT_ERR_EVAL];
     if (ctx->h_counters[CNT_ERR_BUILD]) { ctx->cells_dirty = true; ctx->topo_valid = false; }
+    // radix plan of the next build (sort.cu): the last build sorted the upper key bits only and met a long run of keys
+    // equal on them (sorted all the same, by the slow path) -> eight more bits from now on
+    if (ctx->sort_adapted_build != ctx->build_count) {
+        ctx->sort_adapted_build = ctx->build_count;
+        if (ctx->sort_passes_used < (3 * ctx->max_level + 7) / 8 && ctx->h_counters[CNT_SORT_MAXRUN] > 24 && ctx->sort_extra_bits < 48)
+            ctx->sort_extra_bits += 8;
+    }
     if (f & ERR_CELL_CAPACITY) return p3t_fail(ctx, P3T_ENOMEM, "octree cell capacity (3 n + 1024) exceeded");
     if (f & ERR_STACK_OVERFLOW) return p3t_fail(ctx, P3T_ENOMEM, "tree-walk stack overflow");
     if (ctx->hard_unchecked) {
@@ -812,7 +829,8 @@ extern "C" p3t_status p3t_get_stats(p3t_ctx *ctx, p3t_stats *out)
     out->n_neighbours = c[CNT_PAIRS];
     out->n_cells = (u32)c[CNT_NCELLS]; out->n_leaves = (u32)c[CNT_NLEAVES]; out->n_groups = (u32)c[CNT_NGROUPS];
     out->depth = (u32)c[CNT_DEPTH]; out->max_list = (u32)c[CNT_MAXLIST];
-    out->sort_passes = (u32)((3 * ctx->max_level + 7) / 8);
+    out->sort_passes = (u32)ctx->sort_passes_used;
+    out->sort_max_run = ctx->sort_passes_used < (3 * ctx->max_level + 7) / 8 ? (u32)c[CNT_SORT_MAXRUN] : 0u;
     if (ctx->ev_build) {
         cudaEventElapsedTime(&out->ms_sort, ctx->ev[0], ctx->ev[1]);
         cudaEventElapsedTime(&out->ms_build, ctx->ev[1], ctx->ev[2]);

@@ -84,8 +84,10 @@ struct P3TParams {
 // counter block, an evaluation the eval words + order_hist.
 enum {
     // zeroed at every build (together with the digit histograms in front of the block)
-    CNT_NCELLS = 0, CNT_NLEAVES, CNT_NGROUPS, CNT_DEPTH, CNT_ERR_BUILD, CNT_HEAD_TICKET, CNT_HEAD_SPARE0, CNT_HEAD_SPARE1,
+    CNT_NCELLS = 0, CNT_NLEAVES, CNT_NGROUPS, CNT_DEPTH, CNT_ERR_BUILD, CNT_HEAD_TICKET, CNT_HEAD_SPARE0,
+    CNT_SORT_NRUNS /* runs of keys equal on the sorted upper bits that sort_long_runs_kernel takes */,
     CNT_SORT_TICKET = 8 /* one per pass, 8 */,
+    CNT_SORT_MAXRUN = 8 /* longest such run, if above 16: the ticket word of pass 0, which does not run when runs can exist */,
     // words from CNT_ERR_BUILD on are zeroed at load (the tree counts in front survive: a refit needs them)
     CNT_NONFINITE = 16,
     CNT_STRAY = 17 /* refit: bodies that left the cube of their leaf by more than stray_dist leaf sides */,
@@ -185,6 +187,10 @@ struct p3t_ctx {
     bool tiles_ready;              // sentinel records of the build look-back written
     bool status_clean;             // the look-back buffers have been zeroed once (they clean themselves afterwards)
     int cur;                       // which of keys[2]/idx[2] holds the sorted result
+    int sort_passes_user;          // p3t_set_sort_passes: 0 = chosen by the library
+    int sort_extra_bits;           // upper key bits added to the plan after a build met long runs (sync_and_check)
+    int sort_passes_used;          // radix passes of the last build
+    u64 build_count, sort_adapted_build;   // builds started; the build whose run statistics were last looked at
     P3TParams prm;
     float eps, theta, r_in, r_out, r_search;
     Workspace ws;

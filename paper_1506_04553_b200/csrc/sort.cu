@@ -202,7 +202,7 @@ __device__ __forceinline__ void root_cube(const u32 *bbox_bits, float &minx, flo
 
 __global__ void __launch_bounds__(256) keys_hist_kernel(const float4 *__restrict__ body, const u32 *__restrict__ bbox_bits,
                                                         float *cube, u64 *__restrict__ keys, u32 *hist, u32 n,
-                                                        int max_level, const u32 *__restrict__ hilbert_tab, int passes, const u32 *__restrict__ prev_ncells,
+                                                        int max_level, const u32 *__restrict__ hilbert_tab, int first_pass, int passes, const u32 *__restrict__ prev_ncells,
                                                         u32 cell_cap, u32 *cell_nchild, u32 *cell_ready)
 {
     // child counters of the cells of the previous build -> 0 (emit_kernel accumulates into them)
@@ -228,10 +228,10 @@ __global__ void __launch_bounds__(256) keys_hist_kernel(const float4 *__restrict
         u32 qz = min((u32)fmaxf((b.z - minz) * scale, 0.f), qmax);
         u64 key = hilbert_tab ? hilbert_key_tab(s_tab, qx, qy, qz, max_level) : p3t_encode_key(qx, qy, qz, max_level, 0);
         keys[i] = key;
-        for (int p = 0; p < passes; ++p) atomicAdd(&s_hist[p * 256 + (u32)((key >> (8 * p)) & 255u)], 1u);
+        for (int p = first_pass; p < passes; ++p) atomicAdd(&s_hist[p * 256 + (u32)((key >> (8 * p)) & 255u)], 1u);
     }
     __syncthreads();
-    for (int t = threadIdx.x; t < passes * 256; t += blockDim.x) {
+    for (int t = first_pass * 256 + threadIdx.x; t < passes * 256; t += blockDim.x) {
         u32 v = s_hist[t];
         if (v) atomicAdd(&hist[t], v);
     }
@@ -442,6 +442,107 @@ __global__ void __launch_bounds__(SORT_THREADS, 1024 / SORT_THREADS) onesweep_ke
 }
 
 // ------------------------------------------------------------------------------------------------
+// a3, last step when the radix passes covered only the UPPER key bits (p3t_stage_sort): the keys are then sorted up to
+// runs of keys that agree on those bits, each run still in index order (the passes are stable).  Sorting every run by
+// the full key, stably, gives exactly the order of the full radix sort.  Runs are short when the upper bits reach below
+// the leaf level of the tree (a few keys): the thread at the head of a run sorts it by insertion, in place.  Longer runs
+// (a plan that was too optimistic for this distribution: the next build takes more passes, sync_and_check) go to a list
+// and are sorted by one CTA each, bitonic on (key, idx) pairs -- idx breaks ties, which is the stable order.
+// Every run is touched by one thread or one CTA only; neighbours read no more than the upper bits of a foreign key,
+// which do not change while its run is permuted (8-byte loads and stores are single transactions).
+// ------------------------------------------------------------------------------------------------
+#define SORT_RUN_INLINE 32        // longest run the head thread sorts itself
+#define SORT_RUN_SMEM 2048        // longest run sort_long_runs_kernel sorts in shared memory
+
+__global__ void __launch_bounds__(256) sort_fix_kernel(u64 *keys, u32 *idx, u32 n, int tail_bits, u32 *__restrict__ runs, u64 *counters)
+{
+    P3T_GRID_TRIGGER();
+    P3T_GRID_WAIT();
+    const u32 i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const volatile u64 *vk = keys;
+    const u64 ti = vk[i] >> tail_bits;
+    if (i > 0 && (vk[i - 1] >> tail_bits) == ti) return;     // inside a run: its head takes care
+    u32 len = 1;
+    while (i + len < n && len <= SORT_RUN_INLINE && (vk[i + len] >> tail_bits) == ti) ++len;
+    if (len == 1) return;
+    if (len > 16) atomicMax(reinterpret_cast<unsigned long long *>(&counters[CNT_SORT_MAXRUN]), (unsigned long long)len);
+    if (len > SORT_RUN_INLINE) {
+        runs[atomicAdd(reinterpret_cast<unsigned long long *>(&counters[CNT_SORT_NRUNS]), 1ull)] = i;
+        return;
+    }
+    for (u32 a = 1; a < len; ++a) {                           // stable insertion sort of (key, idx)[i, i + len)
+        const u64 ka = keys[i + a];
+        const u32 va = idx[i + a];
+        u32 b = a;
+        while (b > 0 && keys[i + b - 1] > ka) {
+            keys[i + b] = keys[i + b - 1];
+            idx[i + b] = idx[i + b - 1];
+            --b;
+        }
+        if (b != a) { keys[i + b] = ka; idx[i + b] = va; }
+    }
+}
+
+// bitonic network with all comparisons ascending (first step of every merge is the flip i ^ (k - 1)): positions
+// behind the end of the run act as +infinity and never take part, so any length works
+template <class KP, class VP>
+__device__ __forceinline__ void run_bitonic(KP key, VP val, u32 len)
+{
+    u32 m = 1;
+    while (m < len) m <<= 1;
+    for (u32 k = 2; k <= m; k <<= 1) {
+        for (u32 j = k >> 1; j > 0; j >>= 1) {
+            for (u32 t = threadIdx.x; t < m; t += blockDim.x) {
+                const u32 l = (j == (k >> 1)) ? (t ^ (k - 1)) : (t ^ j);
+                if (l > t && l < len) {
+                    const u64 a = key[t], b = key[l];
+                    const u32 va = val[t], vb = val[l];
+                    if (a > b || (a == b && va > vb)) { key[t] = b; key[l] = a; val[t] = vb; val[l] = va; }
+                }
+            }
+            __syncthreads();
+        }
+    }
+}
+
+__global__ void __launch_bounds__(256) sort_long_runs_kernel(u64 *keys, u32 *idx, u32 n, int tail_bits, const u32 *__restrict__ runs,
+                                                             u64 *counters)
+{
+    P3T_GRID_TRIGGER();
+    P3T_GRID_WAIT();
+    __shared__ u64 s_key[SORT_RUN_SMEM];
+    __shared__ u32 s_val[SORT_RUN_SMEM];
+    __shared__ u32 s_len;
+    const u32 nruns = (u32)counters[CNT_SORT_NRUNS];
+    for (u32 r = blockIdx.x; r < nruns; r += gridDim.x) {
+        const u32 start = runs[r];
+        const u64 t0 = keys[start] >> tail_bits;
+        if (threadIdx.x == 0) s_len = n - start;
+        __syncthreads();
+        for (u32 base = 0; start + base < n; base += blockDim.x) {     // first position whose upper bits differ
+            const u32 pos = start + base + threadIdx.x;
+            if (pos < n && (keys[pos] >> tail_bits) != t0) atomicMin(&s_len, base + threadIdx.x);
+            __syncthreads();
+            const u32 found = s_len;
+            __syncthreads();
+            if (found <= base + blockDim.x) break;
+        }
+        const u32 len = s_len;
+        if (threadIdx.x == 0) atomicMax(reinterpret_cast<unsigned long long *>(&counters[CNT_SORT_MAXRUN]), (unsigned long long)len);
+        if (len <= SORT_RUN_SMEM) {
+            for (u32 t = threadIdx.x; t < len; t += blockDim.x) { s_key[t] = keys[start + t]; s_val[t] = idx[start + t]; }
+            __syncthreads();
+            run_bitonic(s_key, s_val, len);
+            for (u32 t = threadIdx.x; t < len; t += blockDim.x) { keys[start + t] = s_key[t]; idx[start + t] = s_val[t]; }
+        } else {
+            run_bitonic(keys + start, idx + start, len);     // in global memory: slow, and correct
+        }
+        __syncthreads();
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
 // a4: gather bodies into sorted order; common-prefix level between sorted neighbours
 // ------------------------------------------------------------------------------------------------
 // clev[i] = number of leading octree levels on which key[i-1] and key[i] agree (0..max_level);
@@ -449,11 +550,15 @@ __global__ void __launch_bounds__(SORT_THREADS, 1024 / SORT_THREADS) onesweep_ke
 __global__ void __launch_bounds__(256) gather_kernel(const float4 *__restrict__ body_user, const u32 *__restrict__ idx,
                                                      const u64 *__restrict__ keys, float4 *__restrict__ body,
                                                      signed char *__restrict__ clev, u32 n, int max_level,
-                                                     const u8 *__restrict__ cls_user, u8 *__restrict__ cls_sorted)
+                                                     const u8 *__restrict__ cls_user, u8 *__restrict__ cls_sorted,
+                                                     u32 *__restrict__ status_last, u32 status_words)
 {
     P3T_GRID_TRIGGER();
     P3T_GRID_WAIT();
     u32 i = blockIdx.x * blockDim.x + threadIdx.x;
+    // the look-back rows of the last radix pass -> 0: the first pass of the next build may be any digit, and both status
+    // buffers must be clean for it (every pass zeroes the rows of the pass behind it, nobody those of the last one)
+    if (i < status_words) status_last[i] = 0;
     if (i > n) return;
     if (i == n) { clev[n] = -1; return; }
     const u32 src = idx[i];
@@ -477,7 +582,20 @@ p3t_status p3t_stage_sort(p3t_ctx *ctx)
     Workspace &w = ctx->ws;
     u32 n = (u32)ctx->n;
     cudaStream_t s = ctx->stream;
-    int passes = (3 * ctx->max_level + 7) / 8;   // 8 for 63-bit keys, 4 for 30-bit keys
+    const int passes = (3 * ctx->max_level + 7) / 8;   // 8 for 63-bit keys, 4 for 30-bit keys
+    // Plan: radix passes over the UPPER digits only, the rest by sort_fix_kernel.  The upper bits must reach below the leaf
+    // level of the tree for the runs to be short: log2 n + 14 bits to begin with (n / 16 leaves spread over a cube with a
+    // core a few levels deeper than the mean), 8 more after every build that met a run above 24 keys.
+    int first_pass = 0;
+    if (ctx->sort_passes_user > 0) first_pass = passes - min(ctx->sort_passes_user, passes);
+    else if (ctx->max_level == 21) {
+        int lg = 0;
+        while ((1ull << lg) < (u64)n) ++lg;
+        const int need = lg + 14 + ctx->sort_extra_bits;
+        first_pass = max(0, min(passes - 1, (3 * ctx->max_level - need) / 8));
+    }
+    ctx->sort_passes_used = passes - first_pass;
+    ++ctx->build_count;
     u32 ntiles = div_up(n, SORT_TILE);
     if (!ctx->sort_attr_set) {   // function attributes are per device: kept per context
         P3T_CUDA(ctx, cudaFuncSetAttribute(onesweep_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(OnesweepSmem)));
@@ -504,13 +622,13 @@ p3t_status p3t_stage_sort(p3t_ctx *ctx)
     // (the build's tile records are zeroed here, not in front of levels_kernel: a memset between two kernels would break
     //  the chain of programmatic launches)
     P3T_CUDA(ctx, cudaMemsetAsync(reinterpret_cast<char *>(w.build_tiles) + 8 * 256, 0, (size_t)div_up(n, BUILD_TILE) * 256, s));
-    keys_hist_kernel<<<grid, 256, 0, s>>>(w.body_user, w.bbox_bits, w.cube, w.keys[0], w.hist, n, ctx->max_level, ctx->key_curve ? w.hilbert_tab : nullptr, passes,
+    keys_hist_kernel<<<grid, 256, 0, s>>>(w.body_user, w.bbox_bits, w.cube, w.keys[0], w.hist, n, ctx->max_level, ctx->key_curve ? w.hilbert_tab : nullptr, first_pass, passes,
                                           w.prev_ncells, (u32)w.cell_cap, w.cell_nchild, w.cell_ready);
     int cur = 0;
-    for (int p = 0; p < passes; ++p) {
+    for (int p = first_pass; p < passes; ++p) {
         u32 *st_cur = w.tile_status + ((size_t)(p & 1) * status_rows + SORT_LOOKBACK) * 256;
         u32 *st_next = w.tile_status + ((size_t)((p + 1) & 1) * status_rows + SORT_LOOKBACK) * 256;
-        const u32 *vin = p == 0 ? nullptr : w.idx[cur];
+        const u32 *vin = p == first_pass ? nullptr : w.idx[cur];   // the first pass makes idx = iota itself
         // (tiles always take their index from the ticket: the order in which resident CTAs of a look-back chain start is
         //  not something CUDA promises, least of all next to other work on the device)
         u64 *ticket = w.counters + CNT_SORT_TICKET + p;
@@ -523,9 +641,17 @@ p3t_status p3t_stage_sort(p3t_ctx *ctx)
         cur ^= 1;
     }
     ctx->cur = cur;
+    if (first_pass > 0) {   // runs of keys equal on the sorted bits -> full order (group_class: free until the walk stage)
+        P3T_CUDA(ctx, p3t_launch_pdl(sort_fix_kernel, dim3(div_up(n, 256)), dim3(256), 0, s, w.keys[cur], w.idx[cur], n, 8 * first_pass, w.group_class,
+                                     w.counters));
+        P3T_CUDA(ctx, p3t_launch_pdl(sort_long_runs_kernel, dim3((u32)ctx->sm_count), dim3(256), 0, s, w.keys[cur], w.idx[cur], n, 8 * first_pass,
+                                     (const u32 *)w.group_class, w.counters));
+    }
+    // (the last pass is the top digit, an odd one: its look-back rows are in buffer 1)
     P3T_CUDA(ctx, p3t_launch_pdl(gather_kernel, dim3(div_up(n + 1, 256)), dim3(256), 0, s, (const float4 *)w.body_user, (const u32 *)w.idx[cur],
                                  (const u64 *)w.keys[cur], w.body, w.clev, n, ctx->max_level,
-                                 (const u8 *)(ctx->cls_n ? w.cls_user : nullptr), w.cls_sorted));
+                                 (const u8 *)(ctx->cls_n ? w.cls_user : nullptr), w.cls_sorted,
+                                 w.tile_status + (status_rows + SORT_LOOKBACK) * 256, ntiles * 256u));
     P3T_CUDA(ctx, cudaGetLastError());
     return P3T_OK;
 }

@@ -154,3 +154,63 @@ def test_rebuilding_one_tree_300_times_gives_the_same_bits():
             got = ctx.array(k)
             assert got.tobytes() == first[k].tobytes(), f"rebuild {it}: {k} differs"
     ctx.close()
+
+
+def _sorted_order_case(kind, n, rng):
+    """Positions that make runs of keys equal on the upper bits short, long or huge."""
+    if kind == "plummer":
+        return workloads.config(3, n=n)["pos"]
+    if kind == "clump":          # most bodies in a ball of 1e-4 of the cube: they share the upper 13 levels
+        p = rng.normal(size=(n, 3)) * 1e-4
+        p[:8] = rng.uniform(-1, 1, (8, 3))
+        return p.astype(np.float32)
+    if kind == "lattice":        # repeated points: equal full keys (order by index) next to distinct ones
+        return (rng.integers(0, 12, (n, 3)) / 16.0 + rng.integers(0, 2, (n, 1)) * rng.uniform(0, 1e-6, (n, 3))).astype(np.float32)
+    raise ValueError(kind)
+
+
+@pytest.mark.parametrize("kind,n,kb,passes", [
+    ("plummer", 50000, 63, 0), ("plummer", 50000, 63, 5), ("plummer", 50000, 63, 3), ("plummer", 200003, 63, 4),
+    ("clump", 30000, 63, 0), ("clump", 30000, 63, 4), ("clump", 300000, 63, 2), ("clump", 5000, 63, 1),
+    ("lattice", 40000, 63, 0), ("lattice", 40000, 63, 2), ("lattice", 3000, 30, 2), ("plummer", 20000, 30, 3),
+    ("plummer", 1, 63, 1), ("plummer", 33, 63, 1), ("clump", 4097, 63, 1),
+])
+@pytest.mark.parametrize("curve", ["morton", "hilbert"])
+def test_radix_passes_over_the_upper_digits_give_the_full_stable_order(kind, n, kb, passes, curve):
+    """p3t_set_sort_passes: whatever the number of radix passes, the build ends with the stable order of the FULL keys
+    (runs of keys equal on the sorted bits: one thread up to 32 keys, one CTA in shared memory up to 2048, one CTA in
+    global memory beyond), and a second build on the same context -- whose plan has seen the first one's runs -- too."""
+    from oracle import keytree
+    from paper_1506_04553_b200 import binding
+
+    rng = np.random.default_rng(n + passes)
+    pos = np.ascontiguousarray(_sorted_order_case(kind, n, rng))
+    mass = np.full(n, 1.0 / n, dtype=np.float32)
+    max_level = 21 if kb == 63 else 10
+    with binding.P3T(n, key_bits=kb) as ctx:
+        ctx.set_key_curve(curve)
+        ctx.set_sort_passes(passes)
+        ctx.set_params(1e-6, 0.4, 1e-4, 1e-3, 1.2e-3)
+        used = []
+        for rebuild in range(3):
+            ctx.load_particles(mass, pos)
+            ctx.build_tree()
+            ctx.synchronize()
+            cube = ctx.array("root_cube")
+            ref = (keytree.hilbert_keys if curve == "hilbert" else keytree.morton_keys)(pos, cube[:3], cube[3], max_level)
+            idx, keys = ctx.array("sorted_idx"), ctx.array("keys")
+            assert np.array_equal(idx, np.argsort(ref, kind="stable").astype(np.uint32)), (kind, n, passes, rebuild)
+            assert np.array_equal(keys, ref[idx])
+            st = ctx.get_stats()
+            used.append((st["sort_passes"], st["sort_max_run"]))
+            bodies = ctx.array("bodies")
+            assert np.array_equal(bodies[:, :3], pos[idx])
+        total = 8 if kb == 63 else 4
+        if passes:
+            assert all(u[0] == min(passes, total) for u in used), used
+        elif kb == 30:
+            assert all(u[0] == 4 for u in used), used
+        else:
+            assert all(1 <= u[0] <= 8 for u in used) and used[0][0] <= used[1][0] <= used[2][0], used   # the plan only grows
+            if kind == "clump":
+                assert used[0][1] > 24 and used[1][0] > used[0][0], used      # long runs seen: more passes next time
