@@ -577,6 +577,13 @@ __global__ void __launch_bounds__(256) gather_kernel(const float4 *__restrict__ 
     clev[i] = (signed char)c;
 }
 
+// grid of keys_hist_kernel (instruction-bound at 1M and beyond, where 8 / 4 / 2 / 1 bodies per thread measure alike; at 64K the
+// smaller share per thread is worth 6 us)
+#ifndef KEYS_BODIES_PER_THREAD
+#define KEYS_BODIES_PER_THREAD 2
+#define KEYS_CTAS_PER_SM 8
+#endif
+
 p3t_status p3t_stage_sort(p3t_ctx *ctx)
 {
     Workspace &w = ctx->ws;
@@ -613,7 +620,7 @@ p3t_status p3t_stage_sort(p3t_ctx *ctx)
     }
     // digit histograms + build counters + sort tickets: contiguous, one memset
     P3T_CUDA(ctx, cudaMemsetAsync(w.hist, 0, (size_t)((char *)(w.counters + CNT_NONFINITE) - (char *)w.hist), s));
-    u32 grid = min(div_up(n, 256 * 8), (u32)ctx->sm_count * 8);   // every CTA flushes 8 x 256 histogram bins with global atomics: few, fat CTAs
+    u32 grid = min(div_up(n, 256 * KEYS_BODIES_PER_THREAD), (u32)ctx->sm_count * KEYS_CTAS_PER_SM);   // every CTA flushes its non-empty histogram bins with global atomics
     if (ctx->cells_dirty) {   // first build, or the last one ended in an error: all child counters and prev_ncells -> 0
         P3T_CUDA(ctx, cudaMemsetAsync(w.cell_nchild, 0, (size_t)((char *)(w.cell_ready + w.cell_cap) - (char *)w.cell_nchild), s));
         P3T_CUDA(ctx, cudaMemsetAsync(w.prev_ncells, 0, sizeof(u32), s));
