@@ -267,26 +267,17 @@ __device__ __forceinline__ void st_status(u32 *p, u32 v)
 
 __global__ void fill_u32_kernel(u32 *p, u32 v) { p[blockIdx.x * blockDim.x + threadIdx.x] = v; }
 
-// lanes of the warp that hold the same 8-bit digit: eight ballots.  (MATCH.ANY gives the same mask in one
-// instruction but sustains only about one warp instruction per 35 cycles per SM on B200 -- it was a third of the
-// pass; VOTE runs at ALU rate.)
-__device__ __forceinline__ u32 digit_peers(u32 d)
-{
-    u32 m = 0xffffffffu;
-#pragma unroll
-    for (int b = 0; b < 8; ++b) {
-        const bool bit = (d >> b) & 1u;
-        const u32 bal = __ballot_sync(0xffffffffu, bit);
-        m &= bit ? bal : ~bal;
-    }
-    return m;
-}
-
+// Lanes of the warp that hold the same 8-bit digit ("peers") come from a per-warp table of lane masks in shared memory:
+// every lane ORs its bit into the word of its digit and reads the word back.  (MATCH.ANY gives the same mask in one
+// instruction but sustains only about one warp instruction per 35 cycles per SM on B200 -- it was a third of the pass;
+// eight ballots per item were 35 % of the pass's instructions; the table costs two shared-memory operations per item:
+// a1-a4 at N = 1M 0.131 -> 0.124 ms, at 16M 1.41 -> 1.38 ms.)
 struct OnesweepSmem {
     union {
         u32 whist[SORT_THREADS / 32][256];                      // ranking: per-warp digit counts
         struct { u64 key[SORT_TILE]; u32 val[SORT_TILE]; } x;   // exchange: the tile in digit order
     };
+    u32 wmask[SORT_THREADS / 32][256];   // ranking: lanes of the warp that hold each digit in the current round
     u32 binstart[256];   // first local position of each bin
     u32 goff[256];       // global position of local position 0 of each bin, minus binstart
     u32 wsum[8];
@@ -309,7 +300,7 @@ __global__ void __launch_bounds__(SORT_THREADS, 1024 / SORT_THREADS) onesweep_ke
     P3T_GRID_TRIGGER();
     if (tid == 0) sm.tile = ticket ? (u32)atomicAdd(ticket, 1ull) : blockIdx.x;
 #pragma unroll
-    for (u32 t = 0; t < 8; ++t) sm.whist[warp][t * 32 + lane] = 0;
+    for (u32 t = 0; t < 8; ++t) { sm.whist[warp][t * 32 + lane] = 0; sm.wmask[warp][t * 32 + lane] = 0; }
     __syncthreads();
     P3T_GRID_WAIT();      // the pass before: its keys and values, and its last reads of the status rows zeroed below
     const u32 tile = sm.tile;
@@ -340,19 +331,24 @@ __global__ void __launch_bounds__(SORT_THREADS, 1024 / SORT_THREADS) onesweep_ke
         }
         if (lane == 31) sm.wsum[warp] = ginc;
     }
-    // stable rank inside the warp, items in (k, lane) order.  The peer masks of all items are found
-    // first; the per-warp counters are then advanced by the leaders in item order (shared-memory
-    // atomics of one warp execute in program order), so the eight rounds pipeline instead of
-    // forming a chain of match -> load -> store -> shuffle latencies.
+    // stable rank inside the warp, items in (k, lane) order.  Per item: the peer mask through the warp's table; the
+    // lowest peer (the leader) advances the warp's counter of that digit by the number of peers and clears the word for the
+    // next round.  Round k's updates are ordered before round k+1's by the __syncwarp()s (different lanes may lead the same
+    // digit in different rounds).
     u32 peers[SORT_ITEMS];
 #pragma unroll
-    for (int k = 0; k < SORT_ITEMS; ++k) peers[k] = digit_peers((u32)(key[k] >> shift) & 255u);
-#pragma unroll
     for (int k = 0; k < SORT_ITEMS; ++k) {
-        u32 d = (u32)(key[k] >> shift) & 255u;
+        const u32 d = (u32)(key[k] >> shift) & 255u;
+        atomicOr(&sm.wmask[warp][d], 1u << lane);
+        __syncwarp();
+        peers[k] = sm.wmask[warp][d];
+        __syncwarp();
         pos[k] = 0;
-        if ((peers[k] & lanemask_lt()) == 0) pos[k] = atomicAdd(&sm.whist[warp][d], (u32)__popc(peers[k]));
-        __syncwarp();   // round k's updates are ordered before round k+1's (different lanes may lead the same digit)
+        if ((peers[k] & lanemask_lt()) == 0) {
+            sm.wmask[warp][d] = 0;
+            pos[k] = atomicAdd(&sm.whist[warp][d], (u32)__popc(peers[k]));
+        }
+        __syncwarp();
     }
 #pragma unroll
     for (int k = 0; k < SORT_ITEMS; ++k)
