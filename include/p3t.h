@@ -234,6 +234,30 @@ p3t_status p3t_eval_soft(p3t_ctx *ctx);
  * p3t_get_* calls; for a subset, entries of other particles are zero / empty. */
 p3t_status p3t_eval_direct(p3t_ctx *ctx, const uint32_t *i_subset, size_t n_subset, int on_device);
 
+/* The same brute-force evaluation for callers that cannot allocate device memory (code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid cudaMalloc): no context, no workspace.  For all n particles,
+ *   acc[3 i ..] = - sum_{j != i} m_j K(s_ij) (q_i - q_j) / s_ij^3   (Eq. 8),   pot[i] = - sum_{j != i} m_j W(s_ij) / s_ij   (Eq. 6),
+ *   nbr_count[i] = #{ j != i : s_ij < r_search }   (the list rule; nullable),
+ * with the arithmetic of p3t_eval_direct (fp32 pair terms, one fp64 add per 128 sources).  mass [n], pos [3 n], acc
+ * [3 n], pot [n], nbr_count [n] and info [2] (nullable: info[0] = sum of the counts, info[1] = number of non-finite
+ * inputs, whose results are then meaningless) are DEVICE pointers on `device`, owned by the caller; cuda_stream is a
+ * cudaStream_t (NULL = the legacy default stream).  Asynchronous on that stream.
+ * Scratch (the bodies packed as float4 and a header of counters) is a file-scope device array of the library, sized for
+ * P3T_STATIC_MAX_N particles: 1 MiB + 256 B that every GPU which loads the library holds until the process exits.  The
+ * call makes no cudaMalloc / cudaFree and calls no allocating routine; its first call per device looks the array's
+ * device address up (cudaGetSymbolAddress, with that device current), so make that one outside a stream capture.  All
+ * calls on a device share the array: it keeps the last call's contents (the counters are cleared at the start of each
+ * call, the bodies are rewritten up to n and not read beyond), and two calls that overlap on the GPU (different streams
+ * without an ordering between them) race on it; so do calls from several host threads at once.
+ * P3T_ECAPACITY: n > P3T_STATIC_MAX_N (nothing is launched).  P3T_EINVAL: n = 0, a null mass / pos / acc / pot, device
+ * outside 0..63, eps < 0, not (0 <= r_in < r_out <= r_search), non-finite parameters.  P3T_ECUDA: a CUDA call failed.
+ * The message of the last failure: p3t_direct_static_last_error() (process-wide, not thread-safe). */
+#define P3T_STATIC_MAX_N 65536
+p3t_status p3t_direct_static(int device, void *cuda_stream, size_t n, const float *mass, const float *pos, float eps,
+                             float r_in, float r_out, float r_search, float *acc, float *pot, uint32_t *nbr_count,
+                             uint64_t *info);
+const char *p3t_direct_static_last_error(void);
+
 /* acc[3n] (x,y,z interleaved) and pot[n], user order.  Either may be NULL. */
 p3t_status p3t_get_acc_pot(p3t_ctx *ctx, float *acc, float *pot, int on_device);
 

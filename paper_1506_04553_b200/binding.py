@@ -28,7 +28,7 @@ _STATUS = {0: "P3T_OK", -1: "P3T_EINVAL", -2: "P3T_ESTATE", -3: "P3T_ENOMEM", -4
 # names of include/p3t.h's exported entry points (tests check that each resolves)
 SYMBOLS = [
     "p3t_workspace_bytes", "p3t_create", "p3t_destroy", "p3t_set_params", "p3t_set_tree_params",
-    "p3t_set_pair_classes", "p3t_set_key_curve", "p3t_set_sort_passes", "p3t_hilbert_state_tables", "p3t_set_group_merge_levels", "p3t_set_walk_mode", "p3t_set_shard", "p3t_get_shard_record", "p3t_put_shard_classes", "p3t_load_particles", "p3t_build_tree", "p3t_set_tree_reuse", "p3t_refit_tree", "p3t_eval_soft", "p3t_eval_direct", "p3t_eval_hard",
+    "p3t_set_pair_classes", "p3t_set_key_curve", "p3t_set_sort_passes", "p3t_hilbert_state_tables", "p3t_set_group_merge_levels", "p3t_set_walk_mode", "p3t_set_shard", "p3t_get_shard_record", "p3t_put_shard_classes", "p3t_load_particles", "p3t_build_tree", "p3t_set_tree_reuse", "p3t_refit_tree", "p3t_eval_soft", "p3t_eval_direct", "p3t_direct_static", "p3t_direct_static_last_error", "p3t_eval_hard",
     "p3t_hermite_step", "p3t_step", "p3t_set_hermite_cluster_max", "p3t_set_hermite_class_params",
     "p3t_get_acc_pot", "p3t_get_neighbour_counts", "p3t_get_neighbours", "p3t_get_stats", "p3t_synchronize",
     "p3t_last_error", "p3t_array_info", "p3t_copy_array", "p3t_measure_fp32_peak", "p3t_measure_latency",
@@ -72,6 +72,9 @@ def _sig():
     L.p3t_set_pair_classes.restype = i; L.p3t_set_pair_classes.argtypes = [vp, sz, vp, i, f, f, f, f]
     L.p3t_set_group_merge_levels.restype = i; L.p3t_set_group_merge_levels.argtypes = [vp, i]
     L.p3t_set_sort_passes.restype = i; L.p3t_set_sort_passes.argtypes = [vp, i]
+    L.p3t_direct_static.restype = i
+    L.p3t_direct_static.argtypes = [i, vp, C.c_size_t, vp, vp, C.c_float, C.c_float, C.c_float, C.c_float, vp, vp, vp, vp]
+    L.p3t_direct_static_last_error.restype = C.c_char_p; L.p3t_direct_static_last_error.argtypes = []
     L.p3t_set_key_curve.restype = i; L.p3t_set_key_curve.argtypes = [vp, i]
     L.p3t_hilbert_state_tables.restype = i; L.p3t_hilbert_state_tables.argtypes = [vp, sz]
     L.p3t_set_walk_mode.restype = i; L.p3t_set_walk_mode.argtypes = [vp, i]
@@ -123,6 +126,33 @@ def hilbert_state_tables():
 
 def p3t_workspace_bytes(max_n, key_bits=63, nbr_capacity=0):
     return int(_lib.p3t_workspace_bytes(max_n, key_bits, nbr_capacity))
+
+
+STATIC_MAX_N = 65536     # P3T_STATIC_MAX_N of include/p3t.h
+
+
+def direct_static(mass, pos, eps, r_in, r_out, r_search, acc, pot, nbr_count=None, info=None, stream=None):
+    """p3t_direct_static: brute-force soft force with the library's static scratch (no context, nothing allocated).
+    All arrays are contiguous CUDA tensors of the caller (mass [n], pos [n, 3], acc [n, 3], pot [n] float32; nbr_count [n]
+    int32, info [2] int64, both optional) on one device.  Asynchronous on `stream` (default: torch's current stream)."""
+    import torch
+    for t, dt in ((mass, torch.float32), (pos, torch.float32), (acc, torch.float32), (pot, torch.float32)):
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.is_contiguous() and t.dtype == dt):
+            raise TypeError("direct_static takes contiguous float32 CUDA tensors")
+    for t, dt in ((nbr_count, torch.int32), (info, torch.int64)):
+        if t is not None and not (isinstance(t, torch.Tensor) and t.is_cuda and t.is_contiguous() and t.dtype == dt):
+            raise TypeError("nbr_count must be an int32, info an int64 CUDA tensor")
+    n = mass.shape[0]
+    if pos.numel() != 3 * n or acc.numel() != 3 * n or pot.numel() != n or (nbr_count is not None and nbr_count.numel() != n) \
+            or (info is not None and info.numel() < 2):
+        raise ValueError("direct_static: array sizes do not fit n")
+    dev = mass.device.index
+    s = stream if stream is not None else torch.cuda.current_stream(dev)
+    st = _lib.p3t_direct_static(dev, s.cuda_stream, n, mass.data_ptr(), pos.data_ptr(), float(eps), float(r_in), float(r_out),
+                                float(r_search), acc.data_ptr(), pot.data_ptr(),
+                                nbr_count.data_ptr() if nbr_count is not None else None, info.data_ptr() if info is not None else None)
+    if st != OK:
+        raise P3TError(st, _lib.p3t_direct_static_last_error().decode())
 
 
 def _ptr(x):

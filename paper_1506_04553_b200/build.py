@@ -17,7 +17,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libp3t.so")
-SOURCES = ["api.cu", "sort.cu", "build.cu", "moments.cu", "walk.cu", "direct.cu", "neighbours.cu", "calib.cu", "hard.cu", "hermite.cu"]
+SOURCES = ["api.cu", "sort.cu", "build.cu", "moments.cu", "walk.cu", "direct.cu", "neighbours.cu", "calib.cu", "hard.cu", "hermite.cu", "static_direct.cu"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-gencode", "arch=compute_100a,code=sm_100a",
               "-Xcompiler", "-fPIC,-O3,-pthread", "-I", os.path.join(ROOT, "include"), "-I", CSRC]
 # P3T_CHECKED=1: the kernels' own bounds checks (P3T_DEV_ASSERT of csrc/p3t_internal.cuh) are compiled in; use with --force

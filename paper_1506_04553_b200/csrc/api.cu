@@ -200,7 +200,7 @@ extern "C" const char *p3t_last_error(const p3t_ctx *ctx) { return ctx ? ctx->er
 // ------------------------------------------------------------------------------------------------
 // W(y; gamma) of Eq. 16-17 as coefficients of y^k and y ln y; the denominator of Eq. 17 is taken
 // as (gamma-1)^7 (reading A1).
-static void p3t_fill_cutoff(CutoffSet &c, float r_in, float r_out)
+void p3t_fill_cutoff(CutoffSet &c, float r_in, float r_out)   // (also used by static_direct.cu)
 {
     double g = (double)r_in / (double)r_out;
     double g2 = g * g, g3 = g2 * g, g4 = g2 * g2, g5 = g4 * g, g6 = g3 * g3, g7 = g6 * g;

@@ -202,6 +202,9 @@ struct p3t_ctx {
     u64 h_counters[CNT_WORDS];
 };
 
+// coefficients of K and W for one pair of cutoff radii (api.cu)
+void p3t_fill_cutoff(CutoffSet &c, float r_in, float r_out);
+
 // Lays the arrays out over `base` (may be NULL to only measure).  Returns total bytes.
 size_t p3t_layout(Workspace &ws, char *base, size_t max_n, int key_bits, size_t nbr_capacity, int sm_count);
 
