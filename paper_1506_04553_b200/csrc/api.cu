@@ -773,11 +773,18 @@ extern "C" p3t_status p3t_get_acc_pot(p3t_ctx *ctx, float *acc, float *pot, int 
     P3T_CUDA(ctx, cudaSetDevice(ctx->device));
     size_t n = ctx->n;
     if (on_device) return p3t_stage_unpack(ctx, acc, pot);
-    // host destination: unpack into the (now free) input staging arrays, then copy out
-    p3t_status st = p3t_stage_unpack(ctx, acc ? ctx->ws.in_pos : nullptr, pot ? ctx->ws.in_mass : nullptr);
+    // host destination: unpack into the (now free) input staging arrays, then copy out.  Accelerations and potentials are
+    // final when the walk stage ends (event 5 of the last evaluation); the neighbour stage behind it on the context's
+    // stream touches neither them nor the staging arrays, and nothing that does can have been enqueued since (any such
+    // call clears `evaluated`).  So unpack and copies go to the side stream behind that event and run beside the
+    // neighbour stage; the call returns when both streams are done.
+    cudaStream_t side = ctx->side_stream;
+    P3T_CUDA(ctx, cudaStreamWaitEvent(side, ctx->ev[5], 0));
+    p3t_status st = p3t_stage_unpack(ctx, acc ? ctx->ws.in_pos : nullptr, pot ? ctx->ws.in_mass : nullptr, side);
     if (st != P3T_OK) return st;
-    if (acc) P3T_CUDA(ctx, cudaMemcpyAsync(acc, ctx->ws.in_pos, 3 * n * sizeof(float), cudaMemcpyDeviceToHost, ctx->stream));
-    if (pot) P3T_CUDA(ctx, cudaMemcpyAsync(pot, ctx->ws.in_mass, n * sizeof(float), cudaMemcpyDeviceToHost, ctx->stream));
+    if (acc) P3T_CUDA(ctx, cudaMemcpyAsync(acc, ctx->ws.in_pos, 3 * n * sizeof(float), cudaMemcpyDeviceToHost, side));
+    if (pot) P3T_CUDA(ctx, cudaMemcpyAsync(pot, ctx->ws.in_mass, n * sizeof(float), cudaMemcpyDeviceToHost, side));
+    P3T_CUDA(ctx, cudaStreamSynchronize(side));
     return sync_and_check(ctx);
 }
 

@@ -262,7 +262,7 @@ p3t_status p3t_stage_shard_record(p3t_ctx *ctx, float *d_rec);
 p3t_status p3t_stage_shard_classes(p3t_ctx *ctx, const float *d_rec);
 p3t_status p3t_stage_direct(p3t_ctx *ctx, const u32 *d_subset, size_t n_subset);
 p3t_status p3t_stage_neighbours(p3t_ctx *ctx);
-p3t_status p3t_stage_unpack(p3t_ctx *ctx, float *d_acc, float *d_pot);
+p3t_status p3t_stage_unpack(p3t_ctx *ctx, float *d_acc, float *d_pot, cudaStream_t stream = nullptr);   // nullptr: the context's stream
 p3t_status p3t_stage_hard(p3t_ctx *ctx, const float *d_vel, double *d_acc, double *d_jerk, double *d_pot);
 p3t_status p3t_stage_hermite(p3t_ctx *ctx, double *d_pos, double *d_vel, double T, int log2_div, double eta, double eta_s,
                              double a0, long long max_blocks, u64 *h_ctl);

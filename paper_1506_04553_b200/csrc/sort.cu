@@ -77,11 +77,11 @@ __global__ void __launch_bounds__(256) unpack_kernel(const float4 *__restrict__ 
     if (pot) pot[i] = v.w;
 }
 
-p3t_status p3t_stage_unpack(p3t_ctx *ctx, float *d_acc, float *d_pot)
+p3t_status p3t_stage_unpack(p3t_ctx *ctx, float *d_acc, float *d_pot, cudaStream_t stream)
 {
     u32 n = (u32)ctx->n;
     if (!d_acc && !d_pot) return P3T_OK;
-    P3T_CUDA(ctx, p3t_launch_pdl(unpack_kernel, dim3(div_up(n, 256)), dim3(256), 0, ctx->stream, (const float4 *)ctx->ws.accpot, d_acc, d_pot, n));
+    P3T_CUDA(ctx, p3t_launch_pdl(unpack_kernel, dim3(div_up(n, 256)), dim3(256), 0, stream ? stream : ctx->stream, (const float4 *)ctx->ws.accpot, d_acc, d_pot, n));
     return P3T_OK;
 }
 
