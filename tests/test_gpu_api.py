@@ -328,3 +328,48 @@ def test_sharded_walks_with_exchanged_cost_classes_deal_the_same_order_to_every_
             c.put_shard_classes(total)
     for c in ctxs:
         c.close()
+
+
+def test_host_fetch_of_forces_is_the_same_after_other_calls_on_the_stream():
+    """p3t_get_acc_pot to host buffers runs on the context's side stream behind the walk-end event of the last
+    evaluation; calls that queue more work on the context's stream in between (the hard force from host velocities,
+    which stages them in the arrays the unpack uses; a whole step from device state, whose last kick reads the forces)
+    must not change what it returns, in whatever order the fetches come."""
+    import torch
+
+    from paper_1506_04553_b200 import binding
+
+    cfg = workloads.config(1, n=20000)
+    n = cfg["n"]
+    vel = np.ascontiguousarray(cfg["vel"].astype(np.float32))
+    with binding.P3T(n, key_bits=63, nbr_capacity=1 << 20) as ctx:
+        ctx.set_params(cfg["eps"], cfg["theta"], 0.1 * 0.02, 0.02, 0.025)
+        ctx.set_walk_mode(1)       # one warp per group: bitwise reproducible (the cooperative walk this size would get by
+                                   # default shares its stack between warps as they come, so its rounding varies from run to run)
+        ctx.soft_force(cfg["mass"], cfg["pos"])
+        acc0, pot0 = ctx.get_acc_pot()                       # straight after the evaluation
+        a1, p1 = ctx.get_acc_pot(on_device=True)             # the device form (context's stream)
+        assert np.array_equal(a1.cpu().numpy(), acc0) and np.array_equal(p1.cpu().numpy(), pot0)
+        off0, nbr0 = ctx.get_neighbours()
+        ctx.eval_hard(vel)                                   # host velocities: staged where the unpack writes
+        acc2, pot2 = ctx.get_acc_pot()
+        assert np.array_equal(acc2, acc0) and np.array_equal(pot2, pot0)
+        off2, nbr2 = ctx.get_neighbours()
+        assert np.array_equal(off2, off0) and np.array_equal(nbr2, nbr0)
+        # a whole step from device state, then the fetch of the NEW forces to the host without a synchronisation in between
+        m = torch.from_numpy(cfg["mass"]).cuda()
+        q = torch.from_numpy(cfg["pos"].astype(np.float64)).cuda()
+        v = torch.from_numpy(cfg["vel"].astype(np.float64)).cuda()
+        ctx.step(m, q, v, 1.0 / 1024, a0=0.1 * float(cfg["mass"][0]) / 0.02 ** 2)
+        acc3, pot3 = ctx.get_acc_pot()
+        a3, p3 = ctx.get_acc_pot(on_device=True)
+        torch.cuda.synchronize()
+        assert np.array_equal(a3.cpu().numpy(), acc3) and np.array_equal(p3.cpu().numpy(), pot3)
+        # and they are the forces at the new positions: a fresh context agrees bitwise
+        qn = q.cpu().numpy().astype(np.float32)
+    with binding.P3T(n, key_bits=63, nbr_capacity=1 << 20) as ctx2:
+        ctx2.set_params(cfg["eps"], cfg["theta"], 0.1 * 0.02, 0.02, 0.025)
+        ctx2.set_walk_mode(1)
+        ctx2.soft_force(cfg["mass"], np.ascontiguousarray(qn))
+        acc4, pot4 = ctx2.get_acc_pot()
+    assert np.array_equal(acc4, acc3) and np.array_equal(pot4, pot3)
