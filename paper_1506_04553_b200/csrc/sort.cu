@@ -532,7 +532,16 @@ __global__ void __launch_bounds__(256) sort_long_runs_kernel(u64 *keys, u32 *idx
             run_bitonic(s_key, s_val, len);
             for (u32 t = threadIdx.x; t < len; t += blockDim.x) { keys[start + t] = s_key[t]; idx[start + t] = s_val[t]; }
         } else {
-            run_bitonic(keys + start, idx + start, len);     // in global memory: slow, and correct
+            // Very long runs are what coincident bodies make (equal FULL keys, at any number of passes), and those are in
+            // order already: the passes are stable, so equal keys stand in index order.  One look before sorting.
+            __shared__ u32 s_inv;
+            if (threadIdx.x == 0) s_inv = 0;
+            __syncthreads();
+            u32 inv = 0;
+            for (u32 t = threadIdx.x; t + 1 < len; t += blockDim.x) inv |= keys[start + t] > keys[start + t + 1] ? 1u : 0u;
+            if (inv) s_inv = 1;
+            __syncthreads();
+            if (s_inv) run_bitonic(keys + start, idx + start, len);     // in global memory: slow, and correct
         }
         __syncthreads();
     }

@@ -164,6 +164,10 @@ def _sorted_order_case(kind, n, rng):
         p = rng.normal(size=(n, 3)) * 1e-4
         p[:8] = rng.uniform(-1, 1, (8, 3))
         return p.astype(np.float32)
+    if kind == "coincident":     # three points hold nearly everybody: runs of equal FULL keys, a third of n long
+        p = np.repeat(rng.uniform(-1, 1, (3, 3)), (n + 2) // 3, axis=0)[:n]
+        p[:50] = rng.uniform(-1, 1, (50, 3))
+        return p[rng.permutation(n)].astype(np.float32)
     if kind == "lattice":        # repeated points: equal full keys (order by index) next to distinct ones
         return (rng.integers(0, 12, (n, 3)) / 16.0 + rng.integers(0, 2, (n, 1)) * rng.uniform(0, 1e-6, (n, 3))).astype(np.float32)
     raise ValueError(kind)
@@ -173,7 +177,7 @@ def _sorted_order_case(kind, n, rng):
     ("plummer", 50000, 63, 0), ("plummer", 50000, 63, 5), ("plummer", 50000, 63, 3), ("plummer", 200003, 63, 4),
     ("clump", 30000, 63, 0), ("clump", 30000, 63, 4), ("clump", 300000, 63, 2), ("clump", 5000, 63, 1),
     ("lattice", 40000, 63, 0), ("lattice", 40000, 63, 2), ("lattice", 3000, 30, 2), ("plummer", 20000, 30, 3),
-    ("plummer", 1, 63, 1), ("plummer", 33, 63, 1), ("clump", 4097, 63, 1),
+    ("plummer", 1, 63, 1), ("plummer", 33, 63, 1), ("clump", 4097, 63, 1), ("coincident", 400000, 63, 0), ("coincident", 9000, 63, 8),
 ])
 @pytest.mark.parametrize("curve", ["morton", "hilbert"])
 def test_radix_passes_over_the_upper_digits_give_the_full_stable_order(kind, n, kb, passes, curve):
